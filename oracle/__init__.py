@@ -1,0 +1,298 @@
+"""CPU oracle for the PM2D time step -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Thin ctypes wrapper around ``pm2d_oracle.c`` (plain C, double precision, written from the paper;
+see that file's header for citations).  Only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this package.  It imports
+nothing from ``paper_2404_14293_b200`` and the product imports nothing from here.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pm2d_oracle.c")
+_LIB = os.path.join(_HERE, "libpm2d_oracle.so")
+
+CIC, TSC, SINE = 0, 1, 2
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, no fast-math, no OpenMP)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("pad_", C.c_int32),
+                ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
+
+
+_dp = C.POINTER(C.c_double)
+
+
+class _Species(C.Structure):
+    _fields_ = [("mass", C.c_double), ("vth2", C.c_double), ("C", C.c_double), ("DD", C.c_double),
+                ("sign", C.c_int32), ("shape", C.c_int32), ("mobile", C.c_int32), ("pad_", C.c_int32),
+                ("np", C.c_int64),
+                ("X", _dp), ("Y", _dp), ("ux", _dp), ("uy", _dp), ("w", _dp),
+                ("uhx", _dp), ("uhy", _dp),
+                ("n", _dp), ("Px", _dp), ("Py", _dp), ("Fx", _dp), ("Fy", _dp)]
+
+
+class _Laser(C.Structure):
+    _fields_ = [("a0", C.c_double), ("omega", C.c_double), ("y0", C.c_double), ("w0", C.c_double),
+                ("t_rise", C.c_double), ("comp", C.c_int32), ("pad_", C.c_int32)]
+
+
+class _State(C.Structure):
+    _fields_ = [("g", _Grid), ("nsp", C.c_int32), ("nlaser", C.c_int32),
+                ("sp", C.POINTER(_Species)), ("laser", C.POINTER(_Laser)),
+                ("a_new", _dp), ("a_now", _dp), ("a_old", _dp),
+                ("rho", _dp), ("phi", _dp), ("Ex", _dp), ("Ey", _dp), ("step", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_G.restype = C.c_double
+        L.orc_G.argtypes = [C.c_int, C.c_double, C.c_double]
+        L.orc_weights_1d.restype = C.c_int
+        L.orc_weights_1d.argtypes = [C.c_int, C.c_double, C.c_double, _dp, C.POINTER(C.c_int)]
+        L.orc_deposit.restype = None
+        L.orc_deposit.argtypes = [C.POINTER(_Grid), C.c_int, C.c_double, C.c_int64] + [_dp] * 8
+        L.orc_gather.restype = None
+        L.orc_gather.argtypes = [C.POINTER(_Grid), C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
+        L.orc_a_inc.restype = C.c_double
+        L.orc_a_inc.argtypes = [C.POINTER(_Laser), C.c_double, C.c_double, C.c_double]
+        L.orc_field_step.restype = None
+        L.orc_field_step.argtypes = [C.POINTER(_State), _dp, C.c_double]
+        L.orc_fft.restype = None
+        L.orc_fft.argtypes = [_dp, _dp, C.c_int, C.c_int]
+        L.orc_dft.restype = None
+        L.orc_dft.argtypes = [_dp, _dp, _dp, _dp, C.c_int, C.c_int]
+        L.orc_poisson.restype = None
+        L.orc_poisson.argtypes = [C.POINTER(_Grid), _dp, _dp, C.c_int]
+        L.orc_efield.restype = None
+        L.orc_efield.argtypes = [C.POINTER(_Grid), _dp, _dp, _dp]
+        L.orc_force.restype = None
+        L.orc_force.argtypes = [C.POINTER(_Grid), C.POINTER(_Species), _dp, _dp, _dp, _dp, _dp]
+        L.orc_initial_deposit.restype = None
+        L.orc_initial_deposit.argtypes = [C.POINTER(_State)]
+        L.orc_step.restype = None
+        L.orc_step.argtypes = [C.POINTER(_State)]
+        L.orc_predictor.restype = None
+        L.orc_predictor.argtypes = [C.c_double] * 5 + [_dp, _dp]
+        L.orc_corrector.restype = None
+        L.orc_corrector.argtypes = [C.c_double] * 6 + [_dp, _dp]
+        L.orc_refresh_fields.restype = None
+        L.orc_refresh_fields.argtypes = [C.POINTER(_State)]
+        L.orc_energies.restype = None
+        L.orc_energies.argtypes = [C.POINTER(_State), _dp]
+        _lib = L
+    return _lib
+
+
+def _p(a: np.ndarray):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(_dp)
+
+
+def _f64(a, n=None):
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+    if n is not None:
+        assert a.size == n, (a.size, n)
+    return a
+
+
+# ---------------------------------------------------------------------------------------------
+# primitive calls (used by the pin tests)
+
+def G(shape: int, DD: float, s: float) -> float:
+    return lib().orc_G(shape, DD, s)
+
+
+def weights_1d(shape: int, DD: float, xp: float):
+    """-> (first node, np.ndarray of 4 weights)   [O1]"""
+    W = np.zeros(4)
+    cnt = C.c_int(0)
+    first = lib().orc_weights_1d(shape, DD, xp, _p(W), C.byref(cnt))
+    return first, W[: cnt.value]
+
+
+def make_grid(nx, ny, dx, dy, dt, ncomp=1):
+    return _Grid(nx, ny, ncomp, 0, dx, dy, dt)
+
+
+def deposit(g: _Grid, shape, DD, X, Y, ux, uy, w):
+    """-> n, Px, Py nodal arrays of shape (nx+1, ny)   [O2]"""
+    X, Y, ux, uy, w = map(_f64, (X, Y, ux, uy, w))
+    nn = (g.nx + 1) * g.ny
+    n, Px, Py = np.zeros(nn), np.zeros(nn), np.zeros(nn)
+    lib().orc_deposit(C.byref(g), shape, DD, X.size, _p(X), _p(Y), _p(ux), _p(uy), _p(w), _p(n), _p(Px), _p(Py))
+    sh = (g.nx + 1, g.ny)
+    return n.reshape(sh), Px.reshape(sh), Py.reshape(sh)
+
+
+def gather(g: _Grid, shape, DD, Xp, Yp, Fx, Fy):
+    Fx, Fy = _f64(Fx), _f64(Fy)
+    fx, fy = C.c_double(0), C.c_double(0)
+    lib().orc_gather(C.byref(g), shape, DD, Xp, Yp, _p(Fx), _p(Fy), C.byref(fx), C.byref(fy))
+    return fx.value, fy.value
+
+
+def fft(re, im, sign):
+    re, im = _f64(re).copy(), _f64(im).copy()
+    lib().orc_fft(_p(re), _p(im), re.size, sign)
+    return re, im
+
+
+def dft(re, im, sign):
+    re, im = _f64(re), _f64(im)
+    ore, oim = np.zeros_like(re), np.zeros_like(im)
+    lib().orc_dft(_p(re), _p(im), _p(ore), _p(oim), re.size, sign)
+    return ore, oim
+
+
+def poisson(g: _Grid, rho, use_dft=False):
+    rho = _f64(rho, (g.nx + 1) * g.ny)
+    phi = np.zeros_like(rho)
+    lib().orc_poisson(C.byref(g), _p(rho), _p(phi), int(use_dft))
+    return phi.reshape(g.nx + 1, g.ny)
+
+
+def efield(g: _Grid, phi):
+    phi = _f64(phi, (g.nx + 1) * g.ny)
+    Ex, Ey = np.zeros(g.nx * g.ny), np.zeros(g.nx * g.ny)
+    lib().orc_efield(C.byref(g), _p(phi), _p(Ex), _p(Ey))
+    return Ex.reshape(g.nx, g.ny), Ey.reshape(g.nx, g.ny)
+
+
+def predictor(dt, h, x, u, F):
+    uh, xh = C.c_double(0), C.c_double(0)
+    lib().orc_predictor(dt, h, x, u, F, C.byref(uh), C.byref(xh))
+    return uh.value, xh.value
+
+
+def corrector(dt, h, x, u, uh, Fh):
+    un, xn = C.c_double(0), C.c_double(0)
+    lib().orc_corrector(dt, h, x, u, uh, Fh, C.byref(un), C.byref(xn))
+    return un.value, xn.value
+
+
+def a_inc(laser: dict, x, y, t):
+    L = _Laser(laser["a0"], laser.get("omega", 1.0), laser.get("y0", 0.0), laser.get("w0", 0.0),
+               laser.get("t_rise", 0.0), laser.get("comp", 0), 0)
+    return lib().orc_a_inc(C.byref(L), x, y, t)
+
+
+# ---------------------------------------------------------------------------------------------
+class Oracle:
+    """The whole step (O8) over numpy-owned arrays.
+
+    species: list of dicts with keys mass, sign, T_keV, C (pressure_coeff), shape, DD, mobile and
+    particle arrays X, Y (cell units), ux, uy, w; an immobile species may instead give ``n_fixed``
+    (nodal density, shape (nx+1, ny)).  lasers: list of dicts (a0, omega, y0, w0, t_rise, comp).
+    """
+
+    def __init__(self, nx, ny, dx, dy, dt, species, lasers=(), ncomp=1):
+        self.g = make_grid(nx, ny, dx, dy, dt, ncomp)
+        self.nn = nn = (nx + 1) * ny
+        self.a = [np.zeros(ncomp * nn) for _ in range(3)]       # new, now, old
+        self.rho, self.phi = np.zeros(nn), np.zeros(nn)
+        self.Ex, self.Ey = np.zeros(nx * ny), np.zeros(nx * ny)
+        self._sp = (_Species * len(species))()
+        self.sp = []
+        for k, s in enumerate(species):
+            d = {}
+            mobile = int(s.get("mobile", 1))
+            npart = 0 if (not mobile and "X" not in s) else len(s["X"])
+            for key in ("X", "Y", "ux", "uy", "w"):
+                d[key] = _f64(s[key]).copy() if npart else np.zeros(1)
+            d["uhx"], d["uhy"] = np.zeros(max(npart, 1)), np.zeros(max(npart, 1))
+            for key in ("n", "Px", "Py", "Fx", "Fy"):
+                d[key] = np.zeros(nn)
+            mass = float(s.get("mass", 1.0))
+            shape = int(s.get("shape", SINE))
+            DD = float(s.get("DD", {CIC: 1.0, TSC: 2.0}.get(shape, 1.9)))
+            if shape == CIC:
+                assert DD == 1.0
+            if shape == TSC:
+                assert DD == 2.0
+            self._sp[k] = _Species(mass, float(s.get("T_keV", 0.0)) / 511.0 / mass, float(s.get("C", 2.0)), DD,
+                                   int(s["sign"]), shape, mobile, 0, npart,
+                                   _p(d["X"]), _p(d["Y"]), _p(d["ux"]), _p(d["uy"]), _p(d["w"]),
+                                   _p(d["uhx"]), _p(d["uhy"]),
+                                   _p(d["n"]), _p(d["Px"]), _p(d["Py"]), _p(d["Fx"]), _p(d["Fy"]))
+            d["np"] = npart
+            d["mobile"] = mobile
+            d["sign"] = int(s["sign"])
+            self.sp.append(d)
+        self._las = (_Laser * max(len(lasers), 1))()
+        for k, l in enumerate(lasers):
+            self._las[k] = _Laser(l["a0"], l.get("omega", 1.0), l.get("y0", 0.0), l.get("w0", 0.0),
+                                  l.get("t_rise", 0.0), l.get("comp", 0), 0)
+        self.st = _State(self.g, len(species), len(lasers), self._sp, self._las,
+                         _p(self.a[0]), _p(self.a[1]), _p(self.a[2]),
+                         _p(self.rho), _p(self.phi), _p(self.Ex), _p(self.Ey), 0)
+        # item (1) at step 0; immobile species: n_fixed if given, else deposited once from their
+        # particles (Q13: callers pass the electron deposit as n_fixed for exact neutrality)
+        lib().orc_initial_deposit(C.byref(self.st))
+        for k, s in enumerate(species):
+            if not self.sp[k]["mobile"]:
+                if "n_fixed" in s:
+                    self.sp[k]["n"][:] = _f64(s["n_fixed"], nn).ravel()
+                elif self.sp[k]["np"]:
+                    d = self.sp[k]
+                    n, _, _ = deposit(self.g, self._sp[k].shape, self._sp[k].DD, d["X"], d["Y"], d["ux"], d["uy"], d["w"])
+                    d["n"][:] = n.ravel()
+
+    # views ----------------------------------------------------------------------------------
+    def _abuf(self, which):
+        ptr = {"new": self.st.a_new, "now": self.st.a_now, "old": self.st.a_old}[which]
+        addr = C.addressof(ptr.contents)
+        for b in self.a:
+            if b.ctypes.data == addr:
+                return b.reshape(self.g.ncomp, self.g.nx + 1, self.g.ny)
+        raise RuntimeError("lost buffer")
+
+    @property
+    def a_now(self):
+        return self._abuf("now")
+
+    @property
+    def a_old(self):
+        return self._abuf("old")
+
+    def moment(self, s, name):
+        return self.sp[s][name].reshape(self.g.nx + 1, self.g.ny)
+
+    @property
+    def step_index(self):
+        return self.st.step
+
+    def step(self, nsteps=1):
+        for _ in range(nsteps):
+            lib().orc_step(C.byref(self.st))
+
+    def refresh_fields(self):
+        lib().orc_refresh_fields(C.byref(self.st))
+
+    def energies(self):
+        self.refresh_fields()
+        out = np.zeros(3 + 2 * len(self.sp))
+        lib().orc_energies(C.byref(self.st), _p(out))
+        d = {"W_es": out[0], "W_int": out[1], "W_em": out[2],
+             "W_kin": out[3::2].copy(), "W_th": out[4::2].copy()}
+        d["W_total"] = float(out.sum())
+        return d

@@ -1,0 +1,167 @@
+"""Physics pins of the whole oracle step (O5-O8): plasma oscillation, pressure-driven sound wave,
+Bohm-Gross shift, energy invariant.  Closed forms only; no GPU.  (P11-P13.)"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+
+
+def _period_from_zero_crossings(t, y):
+    y = np.asarray(y) - np.mean(y)
+    s = np.sign(y)
+    idx = np.where(s[:-1] * s[1:] < 0)[0]
+    tc = t[idx] - y[idx] * (t[idx + 1] - t[idx]) / (y[idx + 1] - y[idx])
+    assert len(tc) >= 6
+    return 2.0 * (tc[-1] - tc[0]) / (len(tc) - 1)
+
+
+def _lattice(nx, ny, px, py):
+    xs = (np.arange(nx * px) + 0.5) / px
+    ys = (np.arange(ny * py) + 0.5) / py
+    X, Y = [a.ravel() for a in np.meshgrid(xs, ys, indexing="ij")]
+    return X, Y
+
+
+def _run_mode(nx, ny, dx, dt, n0, px, shape, DD, sign, T_keV, C, m, nsteps, eps=0.02):
+    """Lattice-loaded species with displacement eps*sin(K x); returns t, cos-mode amplitude of n."""
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    X0, Y0 = _lattice(nx, ny, px, 1)
+    w = np.full(X0.size, n0 / px)
+    n_bg, _, _ = oracle.deposit(g, shape, DD, X0, Y0, 0 * X0, 0 * X0, w)
+    K = 2 * math.pi * m / nx                 # per cell
+    X = X0 + eps * np.sin(K * X0)
+    sp = [dict(sign=sign, mass=1.0, T_keV=T_keV, C=C, shape=shape, DD=DD, mobile=1,
+               X=X, Y=Y0, ux=0 * X, uy=0 * X, w=w)]
+    if sign != 0:
+        sp.append(dict(sign=-sign, mass=1836.0, T_keV=0.0, mobile=0, shape=shape, DD=DD, n_fixed=n_bg))
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    i = np.arange(nx + 1)[:, None]
+    basis = np.cos(K * i)
+    t, amp = [], []
+    for n in range(nsteps):
+        amp.append(((o.moment(0, "n") - n_bg) * basis).sum())
+        t.append(n * dt)
+        o.step()
+    return np.array(t), np.array(amp), o
+
+
+def test_P11_cold_plasma_oscillation_many_particles_per_cell():
+    """omega = omega_pe, i.e. W = 2 pi sqrt(n_e) per T0 (Eq. 2 + Eq. 3 linearised); 8 particles
+    per cell on a lattice, k dx = 2 pi / 64.  Also pins the sign of E (Q2): with E = +grad(phi) the
+    perturbation would grow exponentially instead of oscillating."""
+    n0, dt = 0.1, 0.035
+    t, amp, _ = _run_mode(64, 4, 0.05, dt, n0, 8, oracle.SINE, 1.9, -1, 0.0, 0.0, 1, 950)
+    period = _period_from_zero_crossings(t, amp)
+    assert period == pytest.approx(1.0 / math.sqrt(n0), rel=0.02)
+    assert np.abs(amp).max() < 1.5 * abs(amp[0])          # bounded: oscillation, not instability
+
+
+@pytest.mark.parametrize("DD", [1.9, 1.6])
+def test_P11_one_particle_per_cell_aliasing_factor(DD):
+    """The paper's own loading (1 particle per cell at the cell centre): the long-wavelength
+    frequency is W_eff = W sqrt(pi dx / (2 DD)) -- a closed form of the sine shape's Eq. 13 weights
+    (restoring force per unit displacement = n0 * dW/dx at the control-volume edge = pi/(2 DD))."""
+    n0, dt = 0.1, 0.035
+    t, amp, _ = _run_mode(64, 4, 0.05, dt, n0, 1, oracle.SINE, DD, -1, 0.0, 0.0, 1, 950, eps=0.01)
+    period = _period_from_zero_crossings(t, amp)
+    expected = 1.0 / (math.sqrt(n0) * math.sqrt(math.pi / (2 * DD)))
+    assert period == pytest.approx(expected, rel=0.01)
+
+
+def test_P12c_neutral_species_sound_wave():
+    """A neutral species feels only -C v_th^2 grad(n)/n (Eq. 2): sound wave w = sqrt(C) K v_th."""
+    T, C, m, nx, dx, dt = 10.0, 2.0, 2, 64, 0.05, 0.035
+    vth = math.sqrt(T / 511.0)
+    Kphys = 2 * math.pi * m / (nx * dx)
+    period_expected = 2 * math.pi / (math.sqrt(C) * Kphys * vth)
+    nsteps = int(4.2 * period_expected / dt)
+    t, amp, _ = _run_mode(nx, 4, dx, dt, 0.1, 8, oracle.SINE, 1.9, 0, T, C, m, nsteps, eps=0.02)
+    period = _period_from_zero_crossings(t, amp)
+    assert period == pytest.approx(period_expected, rel=0.02)
+
+
+def test_P12a_fluid_thermal_shift_cold_lattice():
+    """Cold lattice with the pressure term on: w^2 = w_pe^2 + C k^2 v_th^2 (Q8, C = 2), measured
+    as the ratio to the C = 0 run so that the shape/aliasing factor cancels."""
+    n0, dt, m, nx, dx, T = 0.02, 0.035, 4, 64, 0.05, 10.0
+    vth2 = T / 511.0
+    k = m / (nx * dx)                                     # in units of 2 pi / lambda0
+    periods = []
+    for C in (0.0, 2.0):
+        t, amp, _ = _run_mode(nx, 4, dx, dt, n0, 8, oracle.SINE, 1.9, -1, T, C, m, 1400)
+        periods.append(_period_from_zero_crossings(t, amp))
+    ratio2 = (periods[0] / periods[1]) ** 2               # w_C^2 / w_0^2
+    assert ratio2 == pytest.approx(1.0 + 2.0 * k * k * vth2 / n0, rel=0.02)
+
+
+@pytest.mark.parametrize("C,T", [(0.0, 0.0), (2.0, 10.0)])
+def test_P13_energy_invariant_coherent_oscillation(C, T):
+    """W of DESIGN.md Q11 (W_kin + W_es + W_th [+ W_int + W_em]) is constant while W_es and W_kin
+    exchange all of the wave energy: drift < 0.5 % of the exchanged energy over 200 steps."""
+    nx, ny, dx, dt, n0, px = 64, 4, 0.05, 0.035, 0.1, 8
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    X0, Y0 = _lattice(nx, ny, px, 1)
+    w = np.full(X0.size, n0 / px)
+    n_bg, _, _ = oracle.deposit(g, oracle.SINE, 1.9, X0, Y0, 0 * X0, 0 * X0, w)
+    X = X0 + 0.05 * np.sin(2 * math.pi / nx * X0)
+    sp = [dict(sign=-1, mass=1.0, T_keV=T, C=C, shape=oracle.SINE, DD=1.9, mobile=1, X=X, Y=Y0, ux=0 * X, uy=0 * X, w=w),
+          dict(sign=+1, mass=1836.0, T_keV=0.0, mobile=0, shape=oracle.SINE, DD=1.9, n_fixed=n_bg)]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    e0 = o.energies()
+    wave = e0["W_es"]
+    kin_max, dev = 0.0, 0.0
+    for _ in range(20):
+        o.step(10)
+        e = o.energies()
+        kin_max = max(kin_max, e["W_kin"][0])
+        dev = max(dev, abs(e["W_total"] - e0["W_total"]))
+    assert kin_max > 0.9 * wave              # the energy really moves between the terms
+    assert dev < 5e-3 * wave, dev / wave
+
+
+def test_P13_energy_invariant_noisy_closed_box():
+    """Same invariant with the noisy BASELINE-style load (4 random Maxwellian electrons per cell,
+    fixed ions, no laser): stated drift < 3 % of the kinetic energy over 300 steps (grid heating
+    of a 4-particle-per-cell plasma; measured 1.5 %)."""
+    nx, ny, dx, dt = 32, 16, 0.05, 0.035
+    rng = np.random.default_rng(11)
+    npart = nx * ny * 4
+    X, Y = rng.uniform(0, nx, npart), rng.uniform(0, ny, npart)
+    vth = math.sqrt(1.0 / 511.0)
+    ux, uy = rng.normal(0, vth, npart), rng.normal(0, vth, npart)
+    w = np.full(npart, 0.1 / 4)
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    n_bg, _, _ = oracle.deposit(g, oracle.SINE, 1.9, X, Y, ux, uy, w)
+    sp = [dict(sign=-1, mass=1.0, T_keV=1.0, C=2.0, shape=oracle.SINE, DD=1.9, mobile=1, X=X, Y=Y, ux=ux, uy=uy, w=w),
+          dict(sign=+1, mass=1836.0, T_keV=0.0, mobile=0, shape=oracle.SINE, DD=1.9, n_fixed=n_bg)]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    e0 = o.energies()
+    hist = []
+    for _ in range(6):
+        o.step(50)
+        hist.append(o.energies()["W_total"])
+    drift = max(abs(h - e0["W_total"]) for h in hist) / e0["W_kin"][0]
+    assert drift < 3e-2, drift
+
+
+def test_count_and_charge_conserved_over_steps():
+    nx, ny, dx, dt = 16, 8, 0.05, 0.035
+    rng = np.random.default_rng(12)
+    npart = nx * ny * 4
+    X, Y = rng.uniform(0, nx, npart), rng.uniform(0, ny, npart)
+    ux, uy = rng.normal(0, 0.3, npart), rng.normal(0, 0.3, npart)       # fast: many wall hits
+    w = rng.uniform(0.01, 0.03, npart)
+    sp = [dict(sign=-1, mass=1.0, T_keV=1.0, C=2.0, shape=oracle.SINE, DD=1.9, mobile=1, X=X, Y=Y, ux=ux, uy=uy, w=w),
+          dict(sign=+1, mass=1836.0, T_keV=0.0, mobile=0, shape=oracle.SINE, DD=1.9,
+               n_fixed=np.full((nx + 1, ny), 0.08))]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    vol = np.ones((nx + 1, 1))
+    vol[0] = vol[-1] = 0.5
+    for _ in range(20):
+        o.step()
+        assert (o.moment(0, "n") * vol).sum() == pytest.approx(w.sum(), rel=1e-12)
+        assert ((o.sp[0]["X"] >= 0) & (o.sp[0]["X"] <= nx)).all()
+        assert ((o.sp[0]["Y"] >= 0) & (o.sp[0]["Y"] < ny)).all()
+    assert o.sp[0]["X"].size == npart

@@ -1,0 +1,401 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+Every check here compares the oracle with something other than itself: values printed by / derived
+from the paper's Eq. 13 (tests/golden/eq13_worked_values.txt), numerical quadrature of the shape
+density, textbook CIC/TSC weights, dense linear algebra, exact discrete eigenmodes, closed forms.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+SHAPES = [(oracle.CIC, 1.0), (oracle.TSC, 2.0), (oracle.SINE, 1.9), (oracle.SINE, 1.6), (oracle.SINE, 1.0)]
+
+
+# --------------------------------------------------------------------------------------------
+# O1: weights
+def test_P2_eq13_worked_values():
+    """Values that follow from Eq. 13 for a particle centred on a node."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "eq13_worked_values.txt")) if l.strip() and l[0] != "#"]
+    for DD, xp, node_offset, expected in rows:
+        DD, xp, node_offset, expected = float(DD), float(xp), int(node_offset), float(expected)
+        first, W = oracle.weights_1d(oracle.SINE, DD, xp)
+        k = int(round(xp)) + node_offset - first
+        got = W[k] if 0 <= k < len(W) else 0.0
+        assert got == pytest.approx(expected, abs=5e-6), (DD, xp, node_offset)
+
+
+@pytest.mark.parametrize("shape,DD", SHAPES)
+def test_P1_weights_sum_to_one(shape, DD):
+    rng = np.random.default_rng(1)
+    for xp in rng.uniform(3.0, 9.0, 200):
+        first, W = oracle.weights_1d(shape, DD, xp)
+        assert abs(W.sum() - 1.0) < 1e-14
+        assert (W >= 0).all()
+        # support: only nodes whose control volume overlaps the particle
+        for k, wk in enumerate(W):
+            node = first + k
+            overlap = min(node + 0.5, xp + DD / 2) - max(node - 0.5, xp - DD / 2)
+            assert (wk > 0) == (overlap > 1e-15)
+
+
+def _shape_density(shape, DD, s):
+    """Normalised 1-D particle density on s in [0, DD] (NOT the oracle's cumulative form)."""
+    s = np.asarray(s, dtype=np.float64)
+    inside = (s > 0) & (s < DD)
+    if shape == oracle.SINE:       # Eq. 12 per axis, normalised to unit integral (Q1)
+        d = (math.pi / (2 * DD)) * np.sin(math.pi * s / DD)
+    elif shape == oracle.CIC:
+        d = np.ones_like(s) / DD
+    else:                          # TSC: triangle of base 2 and unit area
+        d = np.where(s < 1.0, s, 2.0 - s)
+    return np.where(inside, d, 0.0)
+
+
+@pytest.mark.parametrize("shape,DD", SHAPES)
+def test_P3_weights_equal_quadrature_of_shape(shape, DD):
+    rng = np.random.default_rng(2)
+    for xp in rng.uniform(4.0, 6.0, 25):
+        first, W = oracle.weights_1d(shape, DD, xp)
+        for k, wk in enumerate(W):
+            node = first + k
+            # midpoint rule on the node's control volume [node-1/2, node+1/2]
+            m = 20000
+            x = node - 0.5 + (np.arange(m) + 0.5) / m
+            q = _shape_density(shape, DD, x - (xp - DD / 2)).sum() / m
+            # midpoint rule: O(1/m) at the CIC density jump, O(1/m^2) otherwise
+            assert wk == pytest.approx(q, abs=(1.1 / m if shape == oracle.CIC else 2e-8))
+
+
+def test_P4_cic_tsc_textbook():
+    rng = np.random.default_rng(3)
+    for xp in rng.uniform(2.0, 7.0, 200):
+        first, W = oracle.weights_1d(oracle.CIC, 1.0, xp)
+        i = math.floor(xp)
+        ref = {i: 1 - (xp - i), i + 1: xp - i}
+        for k, wk in enumerate(W):
+            assert wk == pytest.approx(ref.get(first + k, 0.0), abs=1e-14)
+        first, W = oracle.weights_1d(oracle.TSC, 2.0, xp)
+        c = math.floor(xp + 0.5)
+        d = xp - c
+        ref = {c - 1: 0.5 * (0.5 - d) ** 2, c: 0.75 - d * d, c + 1: 0.5 * (0.5 + d) ** 2}
+        for k, wk in enumerate(W):
+            assert wk == pytest.approx(ref.get(first + k, 0.0), abs=1e-14)
+
+
+# --------------------------------------------------------------------------------------------
+# O2: deposit
+def _brute_deposit(nx, ny, shape, DD, X, Y, w, q=None, m=400):
+    """Grid-point loop of Eq. 14 by 2-D quadrature of the product shape, with mirror particles at
+    the x walls (Q9) and periodic images in y.  Independent of orc_deposit / orc_weights_1d."""
+    q = np.ones_like(w) if q is None else q
+    out = np.zeros((nx + 1, ny))
+    sub = (np.arange(m) + 0.5) / m - 0.5
+    for i in range(nx + 1):
+        for j in range(ny):
+            # control volume clipped to the box in x; value = mass / clipped volume
+            xs = i + sub
+            xs_in = xs[(xs > 0) & (xs < nx)]
+            vol = len(xs_in) / m
+            acc = 0.0
+            for p in range(len(X)):
+                fx = 0.0
+                for xm in (X[p], -X[p], 2 * nx - X[p]):           # particle + wall mirrors
+                    fx = fx + _shape_density(shape, DD, xs_in - (xm - DD / 2)).sum() / m
+                fy = 0.0
+                for shift in (-ny, 0, ny):
+                    fy = fy + _shape_density(shape, DD, (j + sub) - (Y[p] + shift - DD / 2)).sum() / m
+                acc += w[p] * q[p] * fx * fy
+            out[i, j] = acc / vol
+    return out
+
+
+@pytest.mark.parametrize("shape,DD", [(oracle.CIC, 1.0), (oracle.TSC, 2.0), (oracle.SINE, 1.9)])
+def test_P3_brute_force_4x4(shape, DD):
+    nx = ny = 4
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    rng = np.random.default_rng(4)
+    X = np.concatenate([rng.uniform(0, nx, 5), [0.2, 3.9, 2.0]])      # incl. near both walls
+    Y = np.concatenate([rng.uniform(0, ny, 5), [3.8, 0.1, 2.5]])
+    w = rng.uniform(0.5, 1.5, X.size)
+    ux = rng.normal(0, 0.1, X.size)
+    uy = rng.normal(0, 0.1, X.size)
+    n, Px, Py = oracle.deposit(g, shape, DD, X, Y, ux, uy, w)
+    nb = _brute_deposit(nx, ny, shape, DD, X, Y, w)
+    assert np.abs(n - nb).max() < 2e-3 * np.abs(nb).max()            # quadrature-limited (kinks)
+    Pb = _brute_deposit(nx, ny, shape, DD, X, Y, w, ux)
+    assert np.abs(Px - Pb).max() < 2e-3 * np.abs(nb).max() * 0.3
+    Pb = _brute_deposit(nx, ny, shape, DD, X, Y, w, uy)
+    assert np.abs(Py - Pb).max() < 2e-3 * np.abs(nb).max() * 0.3
+
+
+def test_eq14_grid_loop_equals_particle_loop():
+    """Eq. 14 typed as printed (grid point as the loop variable, corner coordinates x1p..y2p of the
+    overlap rectangle in the particle's own frame) against the particle loop of P:L189."""
+    nx, ny, DD = 6, 8, 1.6
+    D = DD / 2
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    rng = np.random.default_rng(5)
+    X = rng.uniform(1.5, nx - 1.5, 40)          # interior: no wall terms in Eq. 14 as printed
+    Y = rng.uniform(0, ny, 40)
+    w = rng.uniform(0.5, 1.5, 40)
+    n, _, _ = oracle.deposit(g, oracle.SINE, DD, X, Y, np.zeros(40), np.zeros(40), w)
+    ref = np.zeros((nx + 1, ny))
+    for i in range(nx + 1):
+        for j in range(ny):
+            for p in range(40):
+                for sh in (-ny, 0, ny):
+                    x1 = max(i - 0.5, X[p] - D) - (X[p] - D)
+                    x2 = min(i + 0.5, X[p] + D) - (X[p] - D)
+                    y1 = max(j - 0.5, Y[p] + sh - D) - (Y[p] + sh - D)
+                    y2 = min(j + 0.5, Y[p] + sh + D) - (Y[p] + sh - D)
+                    if x2 > x1 and y2 > y1:
+                        c = math.pi / (2 * D)
+                        ref[i, j] += 0.25 * (math.cos(c * x1) - math.cos(c * x2)) * (math.cos(c * y1) - math.cos(c * y2)) * w[p]
+    assert np.abs(n - ref).max() < 1e-13
+
+
+@pytest.mark.parametrize("shape,DD", SHAPES)
+def test_P1_charge_conservation(shape, DD):
+    nx, ny = 12, 8
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    rng = np.random.default_rng(6)
+    X, Y = rng.uniform(0, nx, 500), rng.uniform(0, ny, 500)
+    w = rng.uniform(0.1, 1.0, 500)
+    ux, uy = rng.normal(0, 0.1, 500), rng.normal(0, 0.1, 500)
+    n, Px, Py = oracle.deposit(g, shape, DD, X, Y, ux, uy, w)
+    vol = np.ones((nx + 1, 1))
+    vol[0] = vol[-1] = 0.5
+    assert (n * vol).sum() == pytest.approx(w.sum(), rel=1e-13)
+    assert (Px * vol).sum() == pytest.approx((w * ux).sum(), rel=1e-11, abs=1e-13)
+    assert (Py * vol).sum() == pytest.approx((w * uy).sum(), rel=1e-11, abs=1e-13)
+
+
+def test_uniform_lattice_deposits_uniform_density():
+    """Mirror-particle wall treatment (Q9): an even lattice gives the same density on wall nodes as
+    inside (up to the lattice's own aliasing, which vanishes for DD = 2 and 2 particles/cell)."""
+    nx, ny = 8, 4
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    xs = (np.arange(nx * 4) + 0.5) / 4
+    ys = (np.arange(ny * 4) + 0.5) / 4
+    X, Y = [a.ravel() for a in np.meshgrid(xs, ys, indexing="ij")]
+    w = np.full(X.size, 0.3 / 16)
+    n, _, _ = oracle.deposit(g, oracle.TSC, 2.0, X, Y, 0 * X, 0 * X, w)
+    assert np.abs(n - 0.3).max() < 1e-14
+
+
+# --------------------------------------------------------------------------------------------
+# O7: gather
+@pytest.mark.parametrize("shape,DD", SHAPES)
+def test_gather_is_adjoint_of_deposit(shape, DD):
+    nx, ny = 6, 4
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    rng = np.random.default_rng(7)
+    Fx, Fy = rng.normal(size=(nx + 1, ny)), rng.normal(size=(nx + 1, ny))
+    vol = np.ones((nx + 1, 1))
+    vol[0] = vol[-1] = 0.5
+    for xp, yp in [(0.1, 0.2), (5.95, 3.9), (3.3, 2.2), (0.6, 0.0), (1.0, 1.0)]:
+        n1, _, _ = oracle.deposit(g, shape, DD, [xp], [yp], [0.0], [0.0], [1.0])
+        fx, fy = oracle.gather(g, shape, DD, xp, yp, Fx, Fy)
+        assert fx == pytest.approx((n1 * vol * Fx).sum(), abs=1e-13)
+        assert fy == pytest.approx((n1 * vol * Fy).sum(), abs=1e-13)
+
+
+def test_gather_linear_field_exact_for_cic_tsc():
+    nx, ny = 16, 8
+    g = oracle.make_grid(nx, ny, 0.05, 0.05, 0.035)
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+    Fx = 0.3 + 0.7 * i
+    Fy = -1.0 + 0.25 * i
+    for shape, DD in [(oracle.CIC, 1.0), (oracle.TSC, 2.0)]:
+        for xp in [3.3, 7.5, 9.01, 11.99]:
+            fx, fy = oracle.gather(g, shape, DD, xp, 4.2, Fx, Fy)
+            assert fx == pytest.approx(0.3 + 0.7 * xp, abs=1e-13)
+            assert fy == pytest.approx(-1.0 + 0.25 * xp, abs=1e-13)
+
+
+# --------------------------------------------------------------------------------------------
+# O8: push
+def test_P5_heun_exact_for_constant_force():
+    dt, dx = 0.035, 0.05
+    h = dt / (2 * dx)
+    x, u, F = 3.0, 0.02, -0.4
+    x0, u0 = x, u
+    for n in range(1, 101):
+        uh, xh = oracle.predictor(dt, h, x, u, F)
+        assert uh == pytest.approx(u + dt * F, abs=1e-16)
+        u, x = oracle.corrector(dt, h, x, u, uh, F)
+        t = n * dt
+        assert u == pytest.approx(u0 + F * t, abs=1e-14)
+        assert x == pytest.approx(x0 + (u0 * t + 0.5 * F * t * t) / dx, abs=1e-12)
+
+
+def test_heun_second_order_on_oscillator():
+    """F = -W^2 x, one step of Eqs. 17+19 from (x, u) = (1, 0), th = W dt, by hand:
+    u^ = -W th, x^ = 1 - th^2/2, u' = W(-th + th^3/4), x' = 1 - th^2/2 + th^4/8,
+    so x'^2 + (u'/W)^2 = 1 - th^6/16 + th^8/64 (the paper's variant is very slightly damped)."""
+    W, dx = 2.0, 1.0
+    for dt in (0.02, 0.01):
+        h = dt / (2 * dx)
+        th = W * dt
+        x, u = 1.0, 0.0
+        uh, xh = oracle.predictor(dt, h, x, u, -W * W * x)
+        un, xn = oracle.corrector(dt, h, x, u, uh, -W * W * xh)
+        assert xn == pytest.approx(1 - th ** 2 / 2 + th ** 4 / 8, abs=1e-15)
+        assert un == pytest.approx(W * (-th + th ** 3 / 4), abs=1e-15)
+        amp2 = xn ** 2 + (un / W) ** 2
+        assert amp2 == pytest.approx(1 - th ** 6 / 16 + th ** 8 / 64, abs=1e-14)
+        assert abs(xn - math.cos(th)) < th ** 4
+        assert abs(un + W * math.sin(th)) < W * th ** 3
+
+
+# --------------------------------------------------------------------------------------------
+# O5: Poisson
+def test_fft_equals_dft_and_numpy():
+    rng = np.random.default_rng(8)
+    for n in (2, 8, 64, 256):
+        re, im = rng.normal(size=n), rng.normal(size=n)
+        fr, fi = oracle.fft(re, im, -1)
+        dr, di = oracle.dft(re, im, -1)
+        ref = np.fft.fft(re + 1j * im)
+        assert np.abs(fr + 1j * fi - ref).max() < 1e-11
+        assert np.abs(dr + 1j * di - ref).max() < 1e-10
+        br, bi = oracle.fft(fr, fi, +1)
+        assert np.abs(br / n - re).max() < 1e-12
+
+
+def test_P9_poisson_eigenfunction():
+    nx, ny, dx, dy = 32, 16, 0.05, 0.07
+    g = oracle.make_grid(nx, ny, dx, dy, 0.035)
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+    for m, l in [(1, 0), (3, 2), (7, 5), (2, 8)]:
+        rho = np.sin(math.pi * m * i / nx) * np.cos(2 * math.pi * l * j / ny)
+        ky = 2 * math.pi * l / (ny * dy)
+        lam = -(4 / dx ** 2) * math.sin(math.pi * m / (2 * nx)) ** 2 - ky ** 2
+        phi = oracle.poisson(g, rho)
+        assert np.abs(phi - rho / lam).max() < 1e-12 * np.abs(rho / lam).max() + 1e-15
+        phi2 = oracle.poisson(g, rho, use_dft=True)
+        assert np.abs(phi2 - phi).max() < 1e-12
+
+
+def test_P9_poisson_dense_solve_8x8():
+    nx, ny, dx, dy = 8, 8, 0.05, 0.03
+    g = oracle.make_grid(nx, ny, dx, dy, 0.035)
+    rng = np.random.default_rng(9)
+    rho = rng.normal(size=(nx + 1, ny))
+    phi = oracle.poisson(g, rho)
+    # dense operator on interior rows i = 1..nx-1: second difference in x, spectral -ky^2 in y
+    l = np.fft.fftfreq(ny, d=1.0 / ny)
+    ky2 = (2 * math.pi * l / (ny * dy)) ** 2
+    F = np.fft.fft(np.eye(ny), axis=0)
+    Dyy = np.real(np.linalg.inv(F) @ np.diag(-ky2) @ F)
+    ni = nx - 1
+    Dxx = (np.diag(-2 * np.ones(ni)) + np.diag(np.ones(ni - 1), 1) + np.diag(np.ones(ni - 1), -1)) / dx ** 2
+    A = np.kron(Dxx, np.eye(ny)) + np.kron(np.eye(ni), Dyy)
+    ref = np.linalg.solve(A, rho[1:nx].ravel()).reshape(ni, ny)
+    assert np.abs(phi[1:nx] - ref).max() < 1e-12 * np.abs(ref).max()
+    assert np.abs(phi[0]).max() == 0 and np.abs(phi[nx]).max() == 0          # Q5
+
+
+def test_P10_efield_sign_and_staggering():
+    nx, ny, dx, dy = 8, 4, 0.05, 0.1
+    g = oracle.make_grid(nx, ny, dx, dy, 0.035)
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+    Ex, Ey = oracle.efield(g, 3.0 * i * dx + 0 * j)
+    assert np.abs(Ex + 3.0).max() < 1e-12 and np.abs(Ey).max() < 1e-12     # E = -grad phi (Q2)
+    phi = np.cos(2 * math.pi * j / ny) * (1.0 + 0 * i)
+    Ex, Ey = oracle.efield(g, phi)
+    ref = -(np.cos(2 * math.pi * (np.arange(ny) + 1) / ny) - np.cos(2 * math.pi * np.arange(ny) / ny)) / dy
+    assert np.abs(Ex).max() < 1e-12 and np.abs(Ey - ref[None, :]).max() < 1e-12
+
+
+# --------------------------------------------------------------------------------------------
+# O3 / O4: wave equation
+def _field_only_oracle(nx, ny, dx, dy, dt, ne, lasers=()):
+    sp = [dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, shape=oracle.CIC, DD=1.0,
+               n_fixed=np.full((nx + 1, ny), float(ne)))]
+    return oracle.Oracle(nx, ny, dx, dy, dt, sp, lasers)
+
+
+@pytest.mark.parametrize("ne,mx,my", [(0.0, 0, 1), (0.1, 0, 2), (0.25, 6, 1)])
+def test_P6_discrete_dispersion(ne, mx, my):
+    """An exact eigenmode of Eq. 6: sin^2(W dt/2)/dt^2 = sin^2(Kx dx/2)/dx^2 + sin^2(Ky dy/2)/dy^2 + pi^2 n_e."""
+    nx, ny, dx, dy, dt = 128, 16, 0.05, 0.05, 0.035
+    o = _field_only_oracle(nx, ny, dx, dy, dt, ne)
+    Kx, Ky = 2 * math.pi * mx / (nx * dx), 2 * math.pi * my / (ny * dy)
+    s2 = dt * dt * (math.sin(Kx * dx / 2) ** 2 / dx ** 2 + math.sin(Ky * dy / 2) ** 2 / dy ** 2 + math.pi ** 2 * ne)
+    W = 2 * math.asin(math.sqrt(s2)) / dt
+    # continuum limit w^2 = w_pe^2 + k^2 (in units of omega0: W/2pi)
+    w_cont = math.sqrt(ne + (Kx ** 2 + Ky ** 2) / (4 * math.pi ** 2))
+    assert W / (2 * math.pi) == pytest.approx(w_cont, rel=2e-2)
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+    mode = np.cos(Kx * i * dx) * np.cos(Ky * j * dy)
+    o.a_now[0][:] = mode
+    o.a_old[0][:] = mode * math.cos(W * dt)
+    c = nx // 2
+    for n in range(1, 41):          # boundary influence travels one node per step
+        o.step()
+        assert np.abs(o.a_now[0][c - 8:c + 9] - mode[c - 8:c + 9] * math.cos(W * n * dt)).max() < 1e-12
+
+
+def test_stability_bound_is_sharp():
+    """dt/dx < sqrt(2)/2: the checkerboard mode grows above it and stays bounded below."""
+    for ratio, stable in ((0.70, True), (0.72, False)):
+        nx, ny, dx = 32, 16, 0.05
+        o = _field_only_oracle(nx, ny, dx, dx, ratio * dx, 0.0)
+        i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+        o.a_now[0][:] = 1e-6 * (-1.0) ** (i + j)
+        o.a_old[0][:] = o.a_now[0]
+        o.step(200)
+        amp = np.abs(o.a_now[0][8:24]).max()
+        assert (amp < 1e-4) == stable
+
+
+def test_P7_absorbing_boundary_outgoing_pulse():
+    nx, ny, dx, dt = 400, 4, 0.05, 0.035
+    o = _field_only_oracle(nx, ny, dx, dx, dt, 0.0)
+    x = np.arange(nx + 1)[:, None] * dx + np.zeros((1, ny))
+    f = lambda s: np.exp(-((s - 6.0) / 1.0) ** 2) * np.cos(2 * math.pi * (s - 6.0))
+    o.a_now[0][:] = f(x)                # left-going: a(x, t) = f(x + t)
+    o.a_old[0][:] = f(x - dt)
+    e0 = (o.a_now[0] ** 2).sum()
+    o.step(int(14.0 / dt))
+    assert (o.a_now[0] ** 2).sum() < 1e-3 * e0
+    # right-going pulse through the right boundary
+    o = _field_only_oracle(nx, ny, dx, dx, dt, 0.0)
+    fr = lambda s: np.exp(-((s - 14.0) / 1.0) ** 2) * np.cos(2 * math.pi * (s - 14.0))
+    o.a_now[0][:] = fr(x)               # a(x, t) = f(x - t)
+    o.a_old[0][:] = fr(x + dt)
+    o.step(int(14.0 / dt))
+    assert (o.a_now[0] ** 2).sum() < 1e-3 * e0
+
+
+def test_P8_injection_amplitude_and_no_reflection():
+    nx, ny, dx, dt, a0 = 240, 4, 0.05, 0.035, 0.01
+    o = _field_only_oracle(nx, ny, dx, dx, dt, 0.0, [dict(a0=a0, t_rise=3.0)])
+    amp = np.zeros(nx + 1)
+    nsteps = int(24.0 / dt)
+    for n in range(nsteps):
+        o.step()
+        if n > nsteps - int(1.5 / dt):
+            amp = np.maximum(amp, np.abs(o.a_now[0][:, 0]))
+    # the box is 12 wavelengths; after 24 T0 it is filled with a pure right-going wave: flat envelope
+    assert np.abs(amp[5:-5] / a0 - 1.0).max() < 0.01
+    # and the analytic incident wave is reproduced (phase error of the 2nd-order stencil included)
+    t = nsteps * dt
+    xs = np.arange(nx + 1) * dx
+    Kd = 2 * math.asin(math.sin(math.pi * dt) * dx / dt) / dx          # discrete vacuum wavenumber
+    ref = a0 * np.cos(2 * math.pi * t - Kd * xs)
+    assert np.abs(o.a_now[0][:40, 0] - ref[:40]).max() < 0.02 * a0
+
+
+def test_gaussian_beam_envelope_eq4():
+    las = dict(a0=0.03, w0=2.0, y0=5.0, t_rise=0.0)
+    for y in (3.0, 5.0, 8.5):
+        v = oracle.a_inc(las, 0.0, y, 2.0)          # integer number of periods: cos = 1
+        assert v == pytest.approx(0.03 * math.exp(-((y - 5.0) / 2.0) ** 2), rel=1e-12)
+    assert oracle.a_inc(las, 0.25, 5.0, 1.0) == pytest.approx(0.03 * math.cos(2 * math.pi * 0.75), abs=1e-15)
