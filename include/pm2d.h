@@ -1,0 +1,183 @@
+/*
+ * pm2d.h -- C ABI of the B200-native PM2D particle-mesh library (libpm2d.so).
+ *
+ * One time step of PM2D (arXiv 2404.14293): deposit -> wave update + Poisson -> force grid ->
+ * gather + predictor -> deposit -> Poisson -> force grid -> gather + corrector (program flow,
+ * PAPER.md L229-238, Fig. 3).  Every step of that path runs in hand-written sm_100a kernels;
+ * there is no CPU fallback.  "P:Lnnn" below cites /root/reference/PAPER.md line nnn; "Qn" cites
+ * a reading listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Units: lengths in lambda0, times in T0 = lambda0/c; velocities in c; densities in
+ *     n_c; E in 2 pi c omega0 m_e / e; phi in the unit that makes Eq. 3 hold.
+ *   - Nodes (i, j), i = 0..nx, j = 0..ny-1 (y periodic, ny a power of two >= 8); nodal arrays
+ *     handed to / returned from the library are row-major float[(nx+1)][ny], index i*ny + j.
+ *   - Canonical particle position: x = (ix + fx) dx, y = (iy + fy) dy with integer cell
+ *     0 <= ix < nx, 0 <= iy < ny and fx, fy in [0,1) multiples of 2^-24 -- exact in double, so a
+ *     checker sees exactly the device state.
+ *   - Every call returns PM2D_OK (0) or a negative PM2D_E* code; pm2d_last_error() gives the
+ *     text of the last failure on the calling thread's context.  No exceptions, no abort, no
+ *     printing.  A ctx is not thread-safe.
+ *   - Ownership: the caller owns `dev_workspace` (device memory, e.g. a torch uint8 tensor) and
+ *     the CUDA stream for the life of the ctx.  The library carves every device array out of the
+ *     workspace and never allocates device memory on the hot path.  `host` pointers are host
+ *     memory owned by the caller (pinned memory makes the copies asynchronous-capable, pageable
+ *     works).  The ctx itself is a small host object freed by pm2d_free.
+ */
+#ifndef PM2D_H
+#define PM2D_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PM2D_OK 0
+#define PM2D_EINVAL (-1)  /* bad argument: ny not a power of two, dt above the stability bound, ... */
+#define PM2D_ENOMEM (-2)  /* workspace or host buffer too small */
+#define PM2D_ECUDA (-3)   /* a CUDA call or kernel failed */
+#define PM2D_ESTATE (-4)  /* call not valid in the current state (e.g. particle left the rebin range) */
+
+#define PM2D_MAX_SPECIES 4
+#define PM2D_MAX_LASERS 4
+#define PM2D_TILE 32 /* particles are binned by tiles of PM2D_TILE x PM2D_TILE cells */
+
+/* particle shape: 1-D cumulative weight G(s); weights are G differences over the control volumes
+ * [i-1/2, i+1/2] of the nodes.  SINE is the paper's cloud, Eq. 12-13. */
+enum { PM2D_CIC = 0, PM2D_TSC = 1, PM2D_SINE = 2 };
+/* particle loading: NONE = no particles generated (fixed background or
+ * particles supplied by pm2d_set_particles); LATTICE_COLD = even lattice, u = 0;
+ * RANDOM_MAXWELL = uniform-random offsets, Maxwellian u (BASELINE.json configs; Q7). */
+enum { PM2D_LOAD_NONE = 0, PM2D_LATTICE_COLD = 1, PM2D_RANDOM_MAXWELL = 2 };
+enum { PM2D_PROFILE_UNIFORM = 0, PM2D_PROFILE_LINEAR = 1, PM2D_PROFILE_EXP_CAPPED = 2 };
+/* fields for pm2d_get_fields / pm2d_set_fields */
+enum {
+    PM2D_FIELD_A = 0,      /* vector potential component `comp`, time level `level` (0 = n, 1 = n-1) */
+    PM2D_FIELD_PHI = 1,    /* electrostatic potential on nodes (Eq. 3), recomputed from the current densities */
+    PM2D_FIELD_ENODE = 2,  /* E averaged to nodes (Q3), comp 0 = x, 1 = y, from the current densities */
+    PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16), comp 0 = x, 1 = y, as last computed */
+};
+enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
+
+typedef struct pm2d_ctx pm2d_ctx; /* opaque */
+
+typedef struct {
+    int32_t nx, ny;        /* cells; nx >= 8, ny a power of two in [8, 8192]                          */
+    int32_t ncomp;         /* active components of a (Eq. 1): 1..3                                   */
+    int32_t rebin_every;   /* tile rebin period in steps, 1..32; 0 = never (tests)                   */
+    int32_t eager_moments; /* 1: deposit n, Px, Py at both RK stages as the flow chart says (P:L197,
+                              L229, L234); 0: deposit n only and build Px, Py when pm2d_get_moments
+                              asks (nothing in the step reads them)                                   */
+    int32_t track_ids;     /* 1: carry a particle id through the rebin (tests); costs 8 B/particle   */
+    double dx, dy, dt;     /* lambda0, lambda0, T0; dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1 */
+} pm2d_grid;
+
+typedef struct {
+    double mass;           /* m_s / m_e (electron 1, deuterium 3672)                                  */
+    double T_keV;          /* v_th = sqrt(T/511/mass)                                         */
+    double pressure_coeff; /* C in  -C v_th^2 grad(n)/n ; Eq. 2 prints 2 (Q8)               */
+    double DD;             /* side length of the cloud in cells: 1 for CIC, 2 for TSC, < 2 for SINE   */
+    int32_t sign;          /* -1 electron, +1 ion (Z = 1), 0 neutral (tests: pressure force alone)    */
+    int32_t shape;         /* PM2D_CIC | PM2D_TSC | PM2D_SINE                                         */
+    int32_t mobile;        /* 0: fixed neutralising background (Q13)                                  */
+    int32_t load;          /* PM2D_LOAD_*                                                             */
+    int32_t ppc_x, ppc_y;  /* N, M of P:L154                                                          */
+    int64_t capacity;      /* particle slots when load == NONE and mobile (pm2d_set_particles); else 0 */
+} pm2d_species;
+
+typedef struct {
+    int32_t kind;          /* PM2D_PROFILE_*                                                          */
+    int32_t taper_cells;   /* sin^2 edge taper at both x walls (Q9); 0 = none                         */
+    double p[4];           /* UNIFORM: n0. LINEAR: n(0), n(Lx). EXP_CAPPED: n0, Lx/L, cap    */
+} pm2d_profile;
+
+typedef struct {
+    double a0, omega;      /* amplitude; frequency in omega0 (Eq. 4)                        */
+    double y0, w0;         /* beam centre and width in lambda0; w0 <= 0: plane wave                   */
+    double t_rise;         /* sin^2 turn-on over t_rise (Q14); 0: none                                */
+    int32_t comp;          /* component of a that carries the beam                                    */
+    int32_t pad_;
+} pm2d_laser;
+
+typedef struct {
+    int64_t step;
+    double time;                        /* step * dt                                                  */
+    double W_es, W_int, W_em;           /* energy terms of DESIGN.md Q11, per dx*dy                   */
+    double W_kin[PM2D_MAX_SPECIES], W_th[PM2D_MAX_SPECIES];
+    double charge[PM2D_MAX_SPECIES];    /* sum over nodes of n_s * control volume (cells)            */
+    int64_t count[PM2D_MAX_SPECIES];    /* particles held                                             */
+    double W_total;
+} pm2d_diag;
+
+/* phases timed by the built-in CUDA-event profile (pm2d_profile_*) */
+enum { PM2D_PH_FIELD = 0, PM2D_PH_POISSON = 1, PM2D_PH_FORCE = 2, PM2D_PH_STAGE_A = 3,
+       PM2D_PH_STAGE_B = 4, PM2D_PH_REBIN = 5, PM2D_PH_COUNT = 6 };
+
+/* Bytes of device workspace pm2d_init needs for this problem; 0 on invalid arguments. */
+size_t pm2d_query_workspace(const pm2d_grid *grid, const pm2d_species *species, int nsp);
+
+/* Build a context: validates arguments, carves the workspace, zeroes the fields, loads the
+ * particles (profile x loader x seed, Philox-4x32-10), bins them by tile,
+ * deposits item (1) of the flow and fixes immobile backgrounds (Q13).  `cuda_stream` is
+ * a cudaStream_t (NULL = default stream).  Synchronises the stream before returning. */
+int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int nsp, const pm2d_profile *profile,
+              const pm2d_laser *lasers, int nlaser, uint64_t seed, void *dev_workspace, size_t bytes,
+              void *cuda_stream, pm2d_ctx **out);
+
+/* Advance `nsteps` time steps (items (1)-(8)).  Enqueues everything on the stream
+ * with no host round trip inside, then synchronises the stream once. */
+int pm2d_step(pm2d_ctx *ctx, int nsteps);
+/* Same, without the final synchronisation (the caller synchronises its stream). */
+int pm2d_step_async(pm2d_ctx *ctx, int nsteps);
+
+/* Replace the laser table (e.g. a time-varying drive); nlaser <= PM2D_MAX_LASERS. */
+int pm2d_set_lasers(pm2d_ctx *ctx, const pm2d_laser *lasers, int nlaser);
+
+/* Copy the window rows i0..i1-1, columns j0..j1-1 of a nodal field / moment into host[(i1-i0)*(j1-j0)].
+ * Returns the element count or a negative code; cap = capacity of `host` in elements. */
+int64_t pm2d_get_fields(pm2d_ctx *ctx, int field, int comp, int level, int i0, int i1, int j0, int j1,
+                        float *host, size_t cap);
+int64_t pm2d_get_moments(pm2d_ctx *ctx, int species, int moment, int i0, int i1, int j0, int j1,
+                         float *host, size_t cap);
+/* Write one full nodal array of `a` (component comp, level 0 = n, 1 = n-1) from host[(nx+1)*ny]. */
+int pm2d_set_fields(pm2d_ctx *ctx, int field, int comp, int level, const float *host);
+
+/* Particles first..first+count-1 of a species in storage order (tile-binned), canonical form.
+ * Any output pointer may be NULL.  `id` needs track_ids.  Returns the number written. */
+int64_t pm2d_get_particles(pm2d_ctx *ctx, int species, int64_t first, int64_t count, int32_t *ix, int32_t *iy,
+                           float *fx, float *fy, float *ux, float *uy, float *w, int64_t *id);
+/* Replace all particles of a mobile species (count <= capacity; any order; ids = 0..count-1 in
+ * the order given), bin them, re-deposit every moment.  If `refix_background` != 0 the immobile
+ * species of opposite sign are re-set to neutralise the new deposit (Q13). */
+int pm2d_set_particles(pm2d_ctx *ctx, int species, int64_t count, const int32_t *ix, const int32_t *iy,
+                       const float *fx, const float *fy, const float *ux, const float *uy, const float *w,
+                       int refix_background);
+/* Set the nodal density of an immobile species from host[(nx+1)*ny] (n_c). */
+int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
+
+/* Run the tile rebin now.  keys_out[count] (optional) receives, in the OLD storage order, the
+ * destination tile key of every particle; perm_out[count] (optional) receives for every NEW slot
+ * the OLD slot it came from.  The result equals a stable counting sort by key. */
+int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
+
+int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);
+int64_t pm2d_particle_count(pm2d_ctx *ctx, int species);
+
+/* CUDA-event profile of the step phases on the ctx's stream.  enable(1) starts recording one event
+ * pair per phase per step (no synchronisation added); get() synchronises and returns the summed
+ * milliseconds and kernel-launch counts per phase since enable(1), and the steps covered. */
+int pm2d_profile_enable(pm2d_ctx *ctx, int on);
+int pm2d_profile_get(pm2d_ctx *ctx, double ms[PM2D_PH_COUNT], int64_t launches[PM2D_PH_COUNT], int64_t *steps);
+/* Kernels launched by this ctx since init. */
+int64_t pm2d_launch_count(pm2d_ctx *ctx);
+
+void pm2d_free(pm2d_ctx *ctx);
+const char *pm2d_last_error(void);
+const char *pm2d_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PM2D_H */

@@ -1,0 +1,597 @@
+// pm2d_api.cu -- the C ABI of include/pm2d.h: argument checks, workspace carving, the host step
+// scheduler and the host<->device accessors.  No arithmetic of the method lives here
+// except the laser carrier phases handed to the boundary kernel (pm2d_fields.cu).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "pm2d_internal.h"
+
+static thread_local std::string g_err;
+void pm2d_set_error(const std::string &s) { g_err = s; }
+extern "C" const char *pm2d_last_error(void) { return g_err.c_str(); }
+extern "C" const char *pm2d_version(void) { return "pm2d-b200 0.1 (sm_100a)"; }
+
+static int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+
+namespace {
+
+__global__ void k_extract_comp(const float2 *src, int comp, float *dst, size_t n)
+{
+    size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) dst[k] = comp == 0 ? src[k].x : src[k].y;
+}
+
+struct Carver {
+    char *base;
+    size_t off;
+    template <class T>
+    T *take(size_t count)
+    {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+int64_t species_np(const pm2d_grid &g, const pm2d_species &s)
+{
+    if (!s.mobile) return 0;
+    if (s.load == PM2D_LOAD_NONE) return s.capacity;
+    return (int64_t)g.nx * g.ny * s.ppc_x * s.ppc_y;
+}
+
+int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
+{
+    if (!g || !sp) return fail(PM2D_EINVAL, "null argument");
+    if (nsp < 1 || nsp > PM2D_MAX_SPECIES) return fail(PM2D_EINVAL, "nsp out of range");
+    if (g->nx < 8 || g->nx > 32767) return fail(PM2D_EINVAL, "nx must be in [8, 32767]");
+    if (!is_pow2(g->ny) || g->ny < 8 || g->ny > 8192) return fail(PM2D_EINVAL, "ny must be a power of two in [8, 8192]");
+    if (g->ncomp < 1 || g->ncomp > 3) return fail(PM2D_EINVAL, "ncomp must be 1..3");
+    if (g->rebin_every < 0 || g->rebin_every > 32) return fail(PM2D_EINVAL, "rebin_every must be 0..32");
+    if (!(g->dx > 0) || !(g->dy > 0) || !(g->dt > 0)) return fail(PM2D_EINVAL, "dx, dy, dt must be positive");
+    if (g->dt / g->dx > 0.999 || g->dt / g->dy > 0.999)
+        return fail(PM2D_EINVAL, "dt/dx must be < 1: a particle may not cross more than one cell per step");
+    for (int s = 0; s < nsp; s++) {
+        const pm2d_species &q = sp[s];
+        if (!(q.mass > 0)) return fail(PM2D_EINVAL, "species mass must be positive");
+        if (q.sign < -1 || q.sign > 1) return fail(PM2D_EINVAL, "species sign must be -1, 0, +1");
+        if (q.shape == PM2D_CIC) { if (q.DD != 1.0) return fail(PM2D_EINVAL, "CIC needs DD = 1"); }
+        else if (q.shape == PM2D_TSC) { if (q.DD != 2.0) return fail(PM2D_EINVAL, "TSC needs DD = 2"); }
+        else if (q.shape == PM2D_SINE) { if (!(q.DD > 0.0) || q.DD > 2.0) return fail(PM2D_EINVAL, "SINE needs 0 < DD <= 2 (3-node footprint)"); }
+        else return fail(PM2D_EINVAL, "unknown shape");
+        if (q.load < PM2D_LOAD_NONE || q.load > PM2D_RANDOM_MAXWELL) return fail(PM2D_EINVAL, "unknown load");
+        if (q.load != PM2D_LOAD_NONE && (q.ppc_x < 1 || q.ppc_y < 1)) return fail(PM2D_EINVAL, "ppc_x, ppc_y must be >= 1");
+        if (q.load != PM2D_LOAD_NONE && !q.mobile) return fail(PM2D_EINVAL, "an immobile species is a fixed background: load must be NONE");
+        if (species_np(*g, q) < 0 || species_np(*g, q) > ((int64_t)1 << 31) - 1) return fail(PM2D_EINVAL, "particle count out of range");
+    }
+    return PM2D_OK;
+}
+
+// carve (or, with base == nullptr, just size) every device array
+size_t layout(pm2d_ctx *c, char *base)
+{
+    Carver cv{base, 0};
+    const pm2d_grid &g = c->g;
+    const size_t nn = (size_t)(g.nx + 1) * g.ny;
+    const int ntx = (g.nx + TILE - 1) / TILE, nty = (g.ny + TILE - 1) / TILE, ntiles = ntx * nty;
+    const int LP = g.ny / 2 + 2;
+    c->nn = (int64_t)nn; c->ntx = ntx; c->nty = nty; c->ntiles = ntiles; c->LP = LP;
+    const size_t ns = (size_t)(g.nx + 1) * LP;
+    for (int k = 0; k < 3; k++) c->a[k] = cv.take<float>(g.ncomp * nn);
+    c->rho_hat = cv.take<float2>(ns);
+    c->dtmp = cv.take<double2>(ns);
+    c->cp = cv.take<double>(ns);
+    c->ehx = cv.take<float2>(ns);
+    c->ehy = cv.take<float2>(ns);
+    c->Enode = cv.take<float2>(nn);
+    c->phi = cv.take<float>(nn);
+    c->twiddle = cv.take<float2>(g.ny / 2);
+    c->red = cv.take<double>(64);
+    c->flags = cv.take<int32_t>(4);
+    for (int s = 0; s < c->nsp; s++) {
+        SpeciesDev &S = c->sp[s];
+        S.nfix = cv.take<int32_t>(nn);
+        S.pxfix = S.pyfix = nullptr; S.F = nullptr;
+        S.np = S.cap = species_np(g, S.cfg);
+        if (!S.cfg.mobile) continue;
+        S.pxfix = cv.take<int32_t>(nn);
+        S.pyfix = cv.take<int32_t>(nn);
+        S.F = cv.take<float2>(nn);
+        const size_t cap = (size_t)std::max<int64_t>(S.cap, 1);
+        S.x = cv.take<uint32_t>(cap); S.y = cv.take<uint32_t>(cap);
+        S.ux = cv.take<float>(cap); S.uy = cv.take<float>(cap); S.w = cv.take<float>(cap);
+        S.uhx = cv.take<float>(cap); S.uhy = cv.take<float>(cap);
+        S.x2 = cv.take<uint32_t>(cap); S.y2 = cv.take<uint32_t>(cap); S.w2 = cv.take<float>(cap);
+        S.id = S.id2 = nullptr;
+        if (g.track_ids) { S.id = cv.take<int64_t>(cap); S.id2 = cv.take<int64_t>(cap); }
+        S.max_chunks = ntiles + (int32_t)(cap / CHUNK) + 1;
+        S.tile_off = cv.take<int64_t>(ntiles + 1);
+        S.tile_off2 = cv.take<int64_t>(ntiles + 1);
+        S.chunk_tile = cv.take<int32_t>(S.max_chunks);
+        S.chunk_beg = cv.take<int64_t>(S.max_chunks + 1);
+        S.chunk_cnt9 = cv.take<int32_t>((size_t)S.max_chunks * 9);
+        S.chunk_rel9 = cv.take<int64_t>((size_t)S.max_chunks * 9);
+        S.tile_first_chunk = cv.take<int32_t>(ntiles + 1);
+        S.tile_cnt = cv.take<int32_t>(ntiles);
+        S.nchunks_dev = cv.take<int32_t>(4);
+    }
+    return (cv.off + 255) & ~(size_t)255;
+}
+
+void phase_begin(pm2d_ctx *c, int ph)
+{
+    c->cur_phase = ph;
+    if (!c->prof_on) return;
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    cudaEventRecord(e, c->stream);
+    c->ev.push_back(e);
+    c->ev_phase.push_back(ph);
+}
+void phase_end(pm2d_ctx *c)
+{
+    if (c->prof_on) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        cudaEventRecord(e, c->stream);
+        c->ev.push_back(e);
+        c->ev_phase.push_back(-1);
+    }
+    c->cur_phase = -1;
+}
+
+int check_flags(pm2d_ctx *c)
+{
+    int32_t h[4];
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(h, c->flags, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    if (h[0]) return fail(PM2D_ESTATE, "a particle moved further than one tile between rebins (rebin_every too large)");
+    if (h[1]) return fail(PM2D_ESTATE, "chunk table overflow");
+    return PM2D_OK;
+}
+
+int zero_moments(pm2d_ctx *c, int s, bool density, bool momentum)
+{
+    SpeciesDev &S = c->sp[s];
+    const size_t bytes = (size_t)c->nn * sizeof(int32_t);
+    if (density) PM2D_CUDA_CHECK(cudaMemsetAsync(S.nfix, 0, bytes, c->stream));
+    if (momentum) {
+        PM2D_CUDA_CHECK(cudaMemsetAsync(S.pxfix, 0, bytes, c->stream));
+        PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
+    }
+    return PM2D_OK;
+}
+
+// deposit every moment of species s from its current particles (item (1) of the flow)
+int redeposit(pm2d_ctx *c, int s)
+{
+    int rc = zero_moments(c, s, true, true);
+    if (rc) return rc;
+    return launch_deposit_only(c, s, true, c->g.eager_moments != 0);
+}
+
+int refix_backgrounds(pm2d_ctx *c)
+{
+    for (int s = 0; s < c->nsp; s++)
+        if (!c->sp[s].cfg.mobile) {
+            int rc = launch_fix_background(c, s);
+            if (rc) return rc;
+        }
+    return PM2D_OK;
+}
+
+}  // namespace
+
+extern "C" size_t pm2d_query_workspace(const pm2d_grid *grid, const pm2d_species *species, int nsp)
+{
+    if (validate(grid, species, nsp) != PM2D_OK) return 0;
+    pm2d_ctx *c = new (std::nothrow) pm2d_ctx();
+    if (!c) return 0;
+    c->g = *grid;
+    c->nsp = nsp;
+    for (int s = 0; s < nsp; s++) c->sp[s].cfg = species[s];
+    size_t bytes = layout(c, nullptr);
+    delete c;
+    return bytes;
+}
+
+extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int nsp, const pm2d_profile *profile,
+                         const pm2d_laser *lasers, int nlaser, uint64_t seed, void *dev_workspace, size_t bytes,
+                         void *cuda_stream, pm2d_ctx **out)
+{
+    if (!out) return fail(PM2D_EINVAL, "null out");
+    *out = nullptr;
+    int rc = validate(grid, species, nsp);
+    if (rc) return rc;
+    if (!profile) return fail(PM2D_EINVAL, "null profile");
+    if (nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
+    for (int l = 0; l < nlaser; l++)
+        if (lasers[l].comp < 0 || lasers[l].comp >= grid->ncomp) return fail(PM2D_EINVAL, "laser component out of range");
+    if (profile->kind < PM2D_PROFILE_UNIFORM || profile->kind > PM2D_PROFILE_EXP_CAPPED) return fail(PM2D_EINVAL, "unknown profile");
+    double nmax;
+    if (profile->kind == PM2D_PROFILE_UNIFORM) nmax = profile->p[0];
+    else if (profile->kind == PM2D_PROFILE_LINEAR) nmax = std::max(profile->p[0], profile->p[1]);
+    else nmax = std::min(profile->p[0] * std::exp(std::max(profile->p[1], 0.0)), profile->p[2]);
+    if (!(nmax >= 0.0) || nmax > 1e3) return fail(PM2D_EINVAL, "profile density out of range");
+    // discrete stability of Eq. 6 with the plasma term (P:L120 and its bound with n_e)
+    {
+        const double PI = 3.14159265358979323846;
+        double s2 = grid->dt * grid->dt * (1.0 / (grid->dx * grid->dx) + 1.0 / (grid->dy * grid->dy) + PI * PI * nmax);
+        if (s2 > 1.0) return fail(PM2D_EINVAL, "dt violates the stability bound dt*sqrt(1/dx^2+1/dy^2+pi^2 n_max) <= 1 (P:L120)");
+    }
+    if (!dev_workspace) return fail(PM2D_EINVAL, "null workspace");
+    if (((uintptr_t)dev_workspace & 255) != 0) return fail(PM2D_EINVAL, "workspace must be 256-byte aligned");
+    pm2d_ctx *c = new (std::nothrow) pm2d_ctx();
+    if (!c) return fail(PM2D_ENOMEM, "host allocation failed");
+    c->g = *grid;
+    c->nsp = nsp;
+    c->nlaser = nlaser;
+    for (int s = 0; s < nsp; s++) {
+        c->sp[s].cfg = species[s];
+        c->sp[s].vth2 = species[s].T_keV / 511.0 / species[s].mass;
+    }
+    for (int l = 0; l < nlaser; l++) c->laser[l] = lasers[l];
+    c->profile = *profile;
+    c->seed = seed;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->step = 0;
+    c->prof_on = false;
+    c->cur_phase = -1;
+    c->launches = 0;
+    c->prof_steps = 0;
+    for (int p = 0; p < PM2D_PH_COUNT; p++) { c->prof_ms[p] = 0; c->prof_launch[p] = 0; }
+    const size_t need = layout(c, (char *)dev_workspace);
+    if (need > bytes) {
+        delete c;
+        return fail(PM2D_ENOMEM, "workspace too small");
+    }
+    // fixed-point scale: n_cap = power of two >= 8 n_max
+    {
+        double cap = 8.0 * (nmax > 0.0 ? nmax : 1.0);
+        int e = (int)std::ceil(std::log2(cap));
+        double ncap = std::ldexp(1.0, e);
+        c->nscale = (float)(2147483648.0 / ncap);
+        c->inv_nscale = (float)(ncap / 2147483648.0);
+        c->pscale = c->nscale * 8.0f;
+        c->inv_pscale = c->inv_nscale / 8.0f;
+    }
+#define INIT_CHECK(call)           \
+    do {                           \
+        int rc_ = (call);          \
+        if (rc_) {                 \
+            delete c;              \
+            return rc_;            \
+        }                          \
+    } while (0)
+#define INIT_CUDA(call)                                                          \
+    do {                                                                         \
+        cudaError_t e_ = (call);                                                 \
+        if (e_ != cudaSuccess) {                                                 \
+            delete c;                                                            \
+            return fail(PM2D_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+        }                                                                        \
+    } while (0)
+    INIT_CUDA(cudaMemsetAsync(dev_workspace, 0, need, c->stream));
+    INIT_CHECK(launch_poisson_init(c));
+    for (int s = 0; s < nsp; s++) {
+        SpeciesDev &S = c->sp[s];
+        if (!S.cfg.mobile) continue;
+        if (S.cfg.load != PM2D_LOAD_NONE) INIT_CHECK(launch_load_particles(c, s));
+        else {
+            S.np = 0;   // until pm2d_set_particles
+            INIT_CHECK(launch_build_chunks(c, s));   // all-zero tile_off -> zero chunks
+        }
+        INIT_CHECK(redeposit(c, s));
+    }
+    INIT_CHECK(refix_backgrounds(c));
+    INIT_CHECK(check_flags(c));
+#undef INIT_CHECK
+#undef INIT_CUDA
+    *out = c;
+    return PM2D_OK;
+}
+
+extern "C" void pm2d_free(pm2d_ctx *c)
+{
+    if (!c) return;
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    delete c;
+}
+
+extern "C" int pm2d_set_lasers(pm2d_ctx *c, const pm2d_laser *lasers, int nlaser)
+{
+    if (!c || nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
+    for (int l = 0; l < nlaser; l++)
+        if (lasers[l].comp < 0 || lasers[l].comp >= c->g.ncomp) return fail(PM2D_EINVAL, "laser component out of range");
+    for (int l = 0; l < nlaser; l++) c->laser[l] = lasers[l];
+    c->nlaser = nlaser;
+    return PM2D_OK;
+}
+
+// ---- the time step: items (1)-(8) of P:L229-238 --------------------------------------------------
+static int enqueue_step(pm2d_ctx *c)
+{
+    int rc;
+    const bool eager = c->g.eager_moments != 0;
+    // (2) a^{n+1} from a^n, a^{n-1}, n_e^n ; E^n from n_i^n - n_e^n
+    phase_begin(c, PM2D_PH_FIELD);
+    if ((rc = launch_field_step(c))) return rc;
+    phase_end(c);
+    for (int stage = 0; stage < 2; stage++) {
+        phase_begin(c, PM2D_PH_POISSON);
+        if ((rc = launch_poisson(c, false))) return rc;
+        phase_end(c);
+        // (3)/(7) force grid with a^n (stage A) or a^{n+1} (stage B)
+        phase_begin(c, PM2D_PH_FORCE);
+        for (int s = 0; s < c->nsp; s++)
+            if (c->sp[s].cfg.mobile && (rc = launch_force(c, s, stage == 0 ? c->a[1] : c->a[0]))) return rc;
+        phase_end(c);
+        // (3)-(5) gather, predictor, deposit / (7)-(8)+(1) gather, corrector, deposit
+        phase_begin(c, stage == 0 ? PM2D_PH_STAGE_A : PM2D_PH_STAGE_B);
+        for (int s = 0; s < c->nsp; s++) {
+            if (!c->sp[s].cfg.mobile) continue;
+            if ((rc = zero_moments(c, s, true, eager))) return rc;
+            if ((rc = launch_stage(c, s, stage))) return rc;
+        }
+        phase_end(c);
+    }
+    float *t = c->a[2];
+    c->a[2] = c->a[1];
+    c->a[1] = c->a[0];
+    c->a[0] = t;
+    c->step++;
+    if (c->prof_on) c->prof_steps++;
+    if (c->g.rebin_every > 0 && c->step % c->g.rebin_every == 0) {
+        phase_begin(c, PM2D_PH_REBIN);
+        for (int s = 0; s < c->nsp; s++)
+            if (c->sp[s].cfg.mobile && (rc = launch_rebin(c, s, nullptr, nullptr))) return rc;
+        phase_end(c);
+    }
+    return PM2D_OK;
+}
+
+extern "C" int pm2d_step_async(pm2d_ctx *c, int nsteps)
+{
+    if (!c || nsteps < 0) return fail(PM2D_EINVAL, "bad argument");
+    for (int n = 0; n < nsteps; n++) {
+        int rc = enqueue_step(c);
+        if (rc) return rc;
+    }
+    return PM2D_OK;
+}
+
+extern "C" int pm2d_step(pm2d_ctx *c, int nsteps)
+{
+    int rc = pm2d_step_async(c, nsteps);
+    if (rc) return rc;
+    return check_flags(c);
+}
+
+extern "C" int64_t pm2d_launch_count(pm2d_ctx *c) { return c ? c->launches : 0; }
+extern "C" int64_t pm2d_particle_count(pm2d_ctx *c, int s) { return (c && s >= 0 && s < c->nsp) ? c->sp[s].np : -1; }
+
+extern "C" int pm2d_profile_enable(pm2d_ctx *c, int on)
+{
+    if (!c) return fail(PM2D_EINVAL, "null ctx");
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    c->ev_phase.clear();
+    for (int p = 0; p < PM2D_PH_COUNT; p++) { c->prof_ms[p] = 0; c->prof_launch[p] = 0; }
+    c->prof_steps = 0;
+    c->prof_on = on != 0;
+    return PM2D_OK;
+}
+
+extern "C" int pm2d_profile_get(pm2d_ctx *c, double ms[PM2D_PH_COUNT], int64_t launches[PM2D_PH_COUNT], int64_t *steps)
+{
+    if (!c) return fail(PM2D_EINVAL, "null ctx");
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    for (size_t k = 0; k + 1 < c->ev.size(); k += 2) {
+        float t = 0.f;
+        PM2D_CUDA_CHECK(cudaEventElapsedTime(&t, c->ev[k], c->ev[k + 1]));
+        c->prof_ms[c->ev_phase[k]] += t;
+    }
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    c->ev_phase.clear();
+    for (int p = 0; p < PM2D_PH_COUNT; p++) {
+        if (ms) ms[p] = c->prof_ms[p];
+        if (launches) launches[p] = c->prof_launch[p];
+    }
+    if (steps) *steps = c->prof_steps;
+    return PM2D_OK;
+}
+
+// ---- accessors ---------------------------------------------------------------------------------
+static int64_t copy_window(pm2d_ctx *c, const float *dev, int i0, int i1, int j0, int j1, float *host, size_t cap)
+{
+    const int nx = c->g.nx, ny = c->g.ny;
+    if (i0 < 0 || i1 > nx + 1 || i0 >= i1 || j0 < 0 || j1 > ny || j0 >= j1 || !host) return fail(PM2D_EINVAL, "bad window");
+    const size_t cnt = (size_t)(i1 - i0) * (j1 - j0);
+    if (cnt > cap) return fail(PM2D_ENOMEM, "host buffer too small");
+    PM2D_CUDA_CHECK(cudaMemcpy2DAsync(host, (size_t)(j1 - j0) * sizeof(float), dev + (size_t)i0 * ny + j0, (size_t)ny * sizeof(float),
+                                      (size_t)(j1 - j0) * sizeof(float), (size_t)(i1 - i0), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return (int64_t)cnt;
+}
+
+extern "C" int64_t pm2d_get_fields(pm2d_ctx *c, int field, int comp, int level, int i0, int i1, int j0, int j1, float *host,
+                                   size_t cap)
+{
+    if (!c) return fail(PM2D_EINVAL, "null ctx");
+    const unsigned blocks = (unsigned)((c->nn + 255) / 256);
+    int rc;
+    switch (field) {
+    case PM2D_FIELD_A:
+        if (comp < 0 || comp >= c->g.ncomp || level < 0 || level > 1) return fail(PM2D_EINVAL, "bad comp/level");
+        return copy_window(c, c->a[1 + level] + (size_t)comp * c->nn, i0, i1, j0, j1, host, cap);
+    case PM2D_FIELD_PHI:
+        if ((rc = launch_poisson(c, true))) return rc;
+        return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
+    case PM2D_FIELD_ENODE:
+        if (comp < 0 || comp > 1) return fail(PM2D_EINVAL, "bad comp");
+        if ((rc = launch_poisson(c, false))) return rc;
+        k_extract_comp<<<blocks, 256, 0, c->stream>>>(c->Enode, comp, c->phi, (size_t)c->nn);
+        count_launch(c);
+        return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
+    case PM2D_FIELD_FORCE:
+        if (comp < 0 || comp > 1 || level < 0 || level >= c->nsp || !c->sp[level].cfg.mobile) return fail(PM2D_EINVAL, "bad comp/species");
+        k_extract_comp<<<blocks, 256, 0, c->stream>>>(c->sp[level].F, comp, c->phi, (size_t)c->nn);
+        count_launch(c);
+        return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
+    default:
+        return fail(PM2D_EINVAL, "unknown field");
+    }
+}
+
+extern "C" int64_t pm2d_get_moments(pm2d_ctx *c, int s, int moment, int i0, int i1, int j0, int j1, float *host, size_t cap)
+{
+    if (!c || s < 0 || s >= c->nsp) return fail(PM2D_EINVAL, "bad species");
+    SpeciesDev &S = c->sp[s];
+    int rc;
+    if (moment == PM2D_MOMENT_N) {
+        if ((rc = launch_fix_to_float(c, S.nfix, c->inv_nscale, c->phi))) return rc;
+    } else if (moment == PM2D_MOMENT_PX || moment == PM2D_MOMENT_PY) {
+        if (!S.cfg.mobile) return fail(PM2D_EINVAL, "immobile species has no momentum");
+        if (!c->g.eager_moments) {   // build P on demand from the current particles (Eq. 14)
+            if ((rc = zero_moments(c, s, false, true))) return rc;
+            if ((rc = launch_deposit_only(c, s, false, true))) return rc;
+        }
+        if ((rc = launch_fix_to_float(c, moment == PM2D_MOMENT_PX ? S.pxfix : S.pyfix, c->inv_pscale, c->phi))) return rc;
+    } else
+        return fail(PM2D_EINVAL, "unknown moment");
+    return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
+}
+
+extern "C" int pm2d_set_fields(pm2d_ctx *c, int field, int comp, int level, const float *host)
+{
+    if (!c || !host) return fail(PM2D_EINVAL, "null argument");
+    if (field != PM2D_FIELD_A || comp < 0 || comp >= c->g.ncomp || level < 0 || level > 1) return fail(PM2D_EINVAL, "only a (level 0/1) can be set");
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(c->a[1 + level] + (size_t)comp * c->nn, host, (size_t)c->nn * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return PM2D_OK;
+}
+
+extern "C" int pm2d_set_background(pm2d_ctx *c, int s, const float *host)
+{
+    if (!c || !host || s < 0 || s >= c->nsp || c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "not an immobile species");
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(c->phi, host, (size_t)c->nn * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    int rc = launch_float_to_fix(c, c->phi, c->nscale, c->sp[s].nfix);
+    if (rc) return rc;
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return PM2D_OK;
+}
+
+extern "C" int64_t pm2d_get_particles(pm2d_ctx *c, int s, int64_t first, int64_t count, int32_t *ix, int32_t *iy, float *fx, float *fy,
+                                      float *ux, float *uy, float *w, int64_t *id)
+{
+    if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
+    SpeciesDev &S = c->sp[s];
+    if (first < 0 || count < 0 || first > S.np) return fail(PM2D_EINVAL, "bad range");
+    count = std::min(count, S.np - first);
+    if (count == 0) return 0;
+    if (id && !S.id) return fail(PM2D_EINVAL, "ids need track_ids");
+    // canonical cell + offset of every particle into the (idle) rebin buffers
+    int32_t *dix = (int32_t *)S.x2, *diy = (int32_t *)S.y2;
+    float *dfx = S.w2, *dfy = S.uhx;
+    int rc = launch_unpack_particles(c, s, first, count, dix, diy, dfx, dfy);
+    if (rc) return rc;
+    auto d2h = [&](void *dst, const void *src, size_t esz) -> cudaError_t {
+        if (!dst) return cudaSuccess;
+        return cudaMemcpyAsync(dst, (const char *)src + (size_t)first * esz, (size_t)count * esz, cudaMemcpyDeviceToHost, c->stream);
+    };
+    PM2D_CUDA_CHECK(d2h(ix, dix, 4));
+    PM2D_CUDA_CHECK(d2h(iy, diy, 4));
+    PM2D_CUDA_CHECK(d2h(fx, dfx, 4));
+    PM2D_CUDA_CHECK(d2h(fy, dfy, 4));
+    PM2D_CUDA_CHECK(d2h(ux, S.ux, 4));
+    PM2D_CUDA_CHECK(d2h(uy, S.uy, 4));
+    PM2D_CUDA_CHECK(d2h(w, S.w, 4));
+    PM2D_CUDA_CHECK(d2h(id, S.id, 8));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return count;
+}
+
+extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32_t *ix, const int32_t *iy, const float *fx,
+                                  const float *fy, const float *ux, const float *uy, const float *w, int refix_background)
+{
+    if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
+    SpeciesDev &S = c->sp[s];
+    if (count < 0 || count > S.cap) return fail(PM2D_ENOMEM, "more particles than capacity");
+    if (count > 0 && (!ix || !iy || !fx || !fy || !ux || !uy || !w)) return fail(PM2D_EINVAL, "null particle array");
+    const int nx = c->g.nx, ny = c->g.ny, nty = c->nty, ntiles = c->ntiles;
+    // host-side stable counting sort by tile (test / restart path, not the hot path)
+    std::vector<int64_t> off(ntiles + 1, 0);
+    std::vector<int32_t> key((size_t)count);
+    for (int64_t p = 0; p < count; p++) {
+        if (ix[p] < 0 || ix[p] >= nx || iy[p] < 0 || iy[p] >= ny || !(fx[p] >= 0.f && fx[p] < 1.f) || !(fy[p] >= 0.f && fy[p] < 1.f))
+            return fail(PM2D_EINVAL, "particle outside the box or offset outside [0,1)");
+        key[p] = (ix[p] / TILE) * nty + iy[p] / TILE;
+        off[key[p] + 1]++;
+    }
+    for (int t = 0; t < ntiles; t++) off[t + 1] += off[t];
+    std::vector<int64_t> cur(off.begin(), off.end() - 1);
+    std::vector<uint32_t> hx((size_t)count), hy((size_t)count);
+    std::vector<float> hux((size_t)count), huy((size_t)count), hw((size_t)count);
+    std::vector<int64_t> hid(S.id ? (size_t)count : 0);
+    for (int64_t p = 0; p < count; p++) {
+        int64_t q = cur[key[p]]++;
+        int li = ix[p] % TILE, lj = iy[p] % TILE;
+        hx[q] = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fx[p] * 16777216.0);
+        hy[q] = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fy[p] * 16777216.0);
+        hux[q] = ux[p]; huy[q] = uy[p]; hw[q] = w[p];
+        if (S.id) hid[q] = p;
+    }
+    auto h2d = [&](void *dst, const void *src, size_t bytes) { return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream); };
+    if (count > 0) {
+        PM2D_CUDA_CHECK(h2d(S.x, hx.data(), (size_t)count * 4));
+        PM2D_CUDA_CHECK(h2d(S.y, hy.data(), (size_t)count * 4));
+        PM2D_CUDA_CHECK(h2d(S.ux, hux.data(), (size_t)count * 4));
+        PM2D_CUDA_CHECK(h2d(S.uy, huy.data(), (size_t)count * 4));
+        PM2D_CUDA_CHECK(h2d(S.w, hw.data(), (size_t)count * 4));
+        if (S.id) PM2D_CUDA_CHECK(h2d(S.id, hid.data(), (size_t)count * 8));
+    }
+    PM2D_CUDA_CHECK(h2d(S.tile_off, off.data(), (size_t)(ntiles + 1) * 8));
+    S.np = count;
+    int rc = launch_build_chunks(c, s);
+    if (rc) return rc;
+    if ((rc = redeposit(c, s))) return rc;
+    if (refix_background && (rc = refix_backgrounds(c))) return rc;
+    return check_flags(c);   // synchronises: the host vectors may now go
+}
+
+extern "C" int pm2d_rebin(pm2d_ctx *c, int s, int32_t *keys_out, int64_t *perm_out)
+{
+    if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
+    SpeciesDev &S = c->sp[s];
+    int32_t *dk = nullptr;
+    int64_t *dp = nullptr;
+    const size_t n = (size_t)std::max<int64_t>(S.np, 1);
+    if (keys_out) PM2D_CUDA_CHECK(cudaMalloc(&dk, n * sizeof(int32_t)));
+    if (perm_out) PM2D_CUDA_CHECK(cudaMalloc(&dp, n * sizeof(int64_t)));
+    int rc = launch_rebin(c, s, dk, dp);
+    if (!rc && keys_out) rc = cudaMemcpyAsync(keys_out, dk, (size_t)S.np * 4, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;
+    if (!rc && perm_out) rc = cudaMemcpyAsync(perm_out, dp, (size_t)S.np * 8, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;
+    if (!rc) rc = check_flags(c);
+    else cudaStreamSynchronize(c->stream);
+    cudaFree(dk);
+    cudaFree(dp);
+    return rc;
+}
+
+extern "C" int pm2d_diagnostics(pm2d_ctx *c, pm2d_diag *out)
+{
+    if (!c || !out) return fail(PM2D_EINVAL, "null argument");
+    int rc = launch_poisson(c, true);   // phi of the current densities, so every term is at one time level
+    if (rc) return rc;
+    return launch_diagnostics(c, out);
+}

@@ -1,0 +1,144 @@
+// pm2d_diag.cu -- energy / charge diagnostics as block reductions (Q11):
+//   W = sum_s sum_p (1/2) m_s w_p |u_p|^2 + 2 pi^2 sum |E|^2 + (1/2) sum n_e |a|^2
+//       + (1/8 pi^2) sum (|d_t a|^2 + |grad a|^2) + sum_s m_s C_s v_s^2 sum n_s ln n_s
+// float32 inputs, float64 accumulation, one atomicAdd(double) per CTA and quantity.
+#include "pm2d_internal.h"
+
+namespace {
+
+__device__ __forceinline__ void block_add(double v, double *dst)
+{
+    __shared__ double ws[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) ws[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        v = lane < (blockDim.x + 31) / 32 ? ws[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0 && v != 0.0) atomicAdd(dst, v);
+    }
+}
+
+struct GridDiag {
+    const float *phi, *a_now, *a_old;
+    const int32_t *ne[PM2D_MAX_SPECIES];
+    int ne_count;
+    int nx, ny, ncomp;
+    float inv_nscale, inv_dx, inv_dy, inv_dt;
+    double *red;
+};
+
+// one thread per node: cell (i, j) terms for i < nx, node terms for all i
+__global__ void __launch_bounds__(256) k_diag_grid(const GridDiag D)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    double es = 0.0, wint = 0.0, em = 0.0;
+    if (j < D.ny) {
+        const size_t nn = (size_t)(D.nx + 1) * D.ny;
+        const int jp = (j + 1) & (D.ny - 1);
+        const size_t k = (size_t)i * D.ny + j, ku = (size_t)i * D.ny + jp;
+        const double vol = (i == 0 || i == D.nx) ? 0.5 : 1.0;
+        if (i < D.nx) {
+            float p00 = D.phi[k], p01 = D.phi[ku], p10 = D.phi[k + D.ny], p11 = D.phi[ku + D.ny];
+            float ex = -0.5f * ((p11 - p01) + (p10 - p00)) * D.inv_dx;
+            float ey = -0.5f * ((p11 - p10) + (p01 - p00)) * D.inv_dy;
+            es = (double)ex * ex + (double)ey * ey;
+        }
+        int nv = 0;
+        for (int s = 0; s < D.ne_count; s++) nv += D.ne[s][k];
+        double a2 = 0.0;
+        for (int c = 0; c < D.ncomp; c++) {
+            float a = D.a_now[c * nn + k];
+            float at = (a - D.a_old[c * nn + k]) * D.inv_dt;
+            float ay = (D.a_now[c * nn + ku] - a) * D.inv_dy;
+            a2 += (double)a * a;
+            em += vol * ((double)at * at + (double)ay * ay);
+            if (i < D.nx) {
+                float ax = (D.a_now[c * nn + k + D.ny] - a) * D.inv_dx;
+                em += (double)ax * ax;
+            }
+        }
+        wint = 0.5 * vol * (double)nv * D.inv_nscale * a2;
+    }
+    block_add(es, &D.red[0]);
+    block_add(wint, &D.red[1]);
+    block_add(em, &D.red[2]);
+}
+
+__global__ void __launch_bounds__(256) k_diag_species_grid(const int32_t *nfix, int nx, int ny, float inv_nscale, double *red_th,
+                                                           double *red_charge)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    double th = 0.0, q = 0.0;
+    if (j < ny) {
+        const double vol = (i == 0 || i == nx) ? 0.5 : 1.0;
+        double n = (double)nfix[(size_t)i * ny + j] * inv_nscale;
+        q = vol * n;
+        if (n > 0.0) th = vol * n * log(n);
+    }
+    block_add(th, red_th);
+    block_add(q, red_charge);
+}
+
+__global__ void __launch_bounds__(256) k_diag_kinetic(const float *ux, const float *uy, const float *w, int64_t np, double *red)
+{
+    double s = 0.0;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += (int64_t)gridDim.x * blockDim.x)
+        s += (double)w[p] * ((double)ux[p] * ux[p] + (double)uy[p] * uy[p]);
+    block_add(s, red);
+}
+
+}  // namespace
+
+// expects c->phi to hold phi of the current densities (caller ran launch_poisson(c, true))
+int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out)
+{
+    const double PI = 3.14159265358979323846;
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->red, 0, 64 * sizeof(double), c->stream));
+    GridDiag D;
+    D.phi = c->phi; D.a_now = c->a[1]; D.a_old = c->a[2];
+    D.ne_count = 0;
+    for (int s = 0; s < c->nsp; s++)
+        if (c->sp[s].cfg.sign < 0) D.ne[D.ne_count++] = c->sp[s].nfix;
+    D.nx = c->g.nx; D.ny = c->g.ny; D.ncomp = c->g.ncomp;
+    D.inv_nscale = c->inv_nscale; D.inv_dx = (float)(1.0 / c->g.dx); D.inv_dy = (float)(1.0 / c->g.dy);
+    D.inv_dt = (float)(1.0 / c->g.dt);
+    D.red = c->red;
+    dim3 grid((c->g.ny + 255) / 256, c->g.nx + 1);
+    k_diag_grid<<<grid, 256, 0, c->stream>>>(D);
+    count_launch(c);
+    for (int s = 0; s < c->nsp; s++) {
+        SpeciesDev &S = c->sp[s];
+        k_diag_species_grid<<<grid, 256, 0, c->stream>>>(S.nfix, c->g.nx, c->g.ny, c->inv_nscale, c->red + 4 + 3 * s, c->red + 5 + 3 * s);
+        count_launch(c);
+        if (S.cfg.mobile && S.np > 0) {
+            k_diag_kinetic<<<592, 256, 0, c->stream>>>(S.ux, S.uy, S.w, S.np, c->red + 3 + 3 * s);
+            count_launch(c);
+        }
+    }
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    double h[64];
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(h, c->red, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    out->step = c->step;
+    out->time = c->step * c->g.dt;
+    out->W_es = 2.0 * PI * PI * h[0];
+    out->W_int = h[1];
+    out->W_em = h[2] / (8.0 * PI * PI);
+    out->W_total = out->W_es + out->W_int + out->W_em;
+    for (int s = 0; s < PM2D_MAX_SPECIES; s++) {
+        out->W_kin[s] = out->W_th[s] = out->charge[s] = 0.0;
+        out->count[s] = 0;
+    }
+    for (int s = 0; s < c->nsp; s++) {
+        SpeciesDev &S = c->sp[s];
+        out->W_kin[s] = 0.5 * S.cfg.mass * h[3 + 3 * s];
+        out->W_th[s] = S.cfg.mass * S.cfg.pressure_coeff * S.vth2 * h[4 + 3 * s];
+        out->charge[s] = h[5 + 3 * s];
+        out->count[s] = S.np;
+        out->W_total += out->W_kin[s] + out->W_th[s];
+    }
+    return PM2D_OK;
+}

@@ -1,0 +1,266 @@
+// pm2d_fields.cu -- mesh kernels of libpm2d.so (sm_100a):
+//   * wave equation, Eq. 6: x-marching register stencil, one thread per column j
+//   * x-boundary absorbing condition Eq. 8 with laser injection (Eq. 4)
+//   * nodal fluid force, Eq. 16 / 18
+//   * small conversions between the fixed-point deposit grids and float
+#include "pm2d_internal.h"
+
+namespace {
+
+constexpr float FOUR_PI2 = 39.47841760435743f;
+
+struct NeSrc {
+    const int32_t *n[PM2D_MAX_SPECIES];   // density grids of the negative species
+    int count;
+    float inv_nscale;
+};
+
+__device__ __forceinline__ float ne_at(const NeSrc &S, size_t k)
+{
+    int v = 0;
+    for (int s = 0; s < S.count; s++) v += S.n[s][k];
+    return (float)v * S.inv_nscale;
+}
+
+// Eq. 6.  CTA = 128 columns x ROWS rows; each thread marches along x keeping a[i-1], a[i], a[i+1]
+// in registers; the y neighbours come from the same cache lines through L1.
+constexpr int FCOLS = 128, FROWS = 32;
+__global__ void __launch_bounds__(FCOLS) k_wave(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap,
+                                                NeSrc ne, int nx, int ny, float cx, float cy, float dt2)
+{
+    const int j = blockIdx.x * FCOLS + threadIdx.x;
+    if (j >= ny) return;
+    const int i0 = 1 + blockIdx.y * FROWS, i1 = min(nx, i0 + FROWS);   // interior rows i0 .. i1-1
+    if (i0 >= i1) return;
+    const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
+    float lo = a[(size_t)(i0 - 1) * ny + j], mid = a[(size_t)i0 * ny + j];
+    for (int i = i0; i < i1; i++) {
+        const size_t row = (size_t)i * ny;
+        float hi = a[row + ny + j];
+        float l = a[row + jm], r = a[row + jp];
+        float lap = cx * (hi - 2.f * mid + lo) + cy * (r - 2.f * mid + l);
+        float src = FOUR_PI2 * ne_at(ne, row + j) * mid;
+        ap[row + j] = 2.f * mid - am[row + j] + dt2 * (lap - src);
+        lo = mid;
+        mid = hi;
+    }
+}
+
+struct BcParams {
+    float g[PM2D_MAX_LASERS][6];   // carrier*ramp at (x=0: t-dt, t, t+dt), (x=dx: t-dt, t, t+dt)
+    float y0[PM2D_MAX_LASERS], inv_w0[PM2D_MAX_LASERS];   // inv_w0 = 0: plane wave
+    int comp[PM2D_MAX_LASERS];
+    int nlaser;
+    float alpha, beta, gam, dy;
+};
+
+__device__ __forceinline__ float beam_env(const BcParams &B, int l, float y)
+{
+    float r = (y - B.y0[l]) * B.inv_w0[l];
+    return __expf(-r * r);
+}
+
+// Eq. 8 solved for the boundary node, both x walls, one thread per j.  Left wall: applied to the
+// scattered field s = a - a_inc and a_inc added back.
+__global__ void k_boundary(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap, BcParams B,
+                           int comp, int nx, int ny)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= ny) return;
+    const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
+    // incident wave at the 3 columns j-1, j, j+1: inc[col][x][t]
+    float inc[3][6];
+    for (int q = 0; q < 3; q++)
+        for (int k = 0; k < 6; k++) inc[q][k] = 0.f;
+    for (int l = 0; l < B.nlaser; l++) {
+        if (B.comp[l] != comp) continue;
+        const int cols[3] = {jm, j, jp};
+        for (int q = 0; q < 3; q++) {
+            float e = beam_env(B, l, cols[q] * B.dy);
+            for (int k = 0; k < 6; k++) inc[q][k] += e * B.g[l][k];
+        }
+    }
+    const float ab = 1.f / (B.alpha + B.beta);
+    {   // left wall: rows 0, 1
+        float s0 = a[j] - inc[1][1], s0m = am[j] - inc[1][0];
+        float s1 = a[ny + j] - inc[1][4], s1m = am[ny + j] - inc[1][3], s1p = ap[ny + j] - inc[1][5];
+        float D0 = (a[jp] - inc[2][1]) - 2.f * s0 + (a[jm] - inc[0][1]);
+        float D1 = (a[ny + jp] - inc[2][4]) - 2.f * s1 + (a[ny + jm] - inc[0][4]);
+        float s0p = (B.alpha * (s1p - s1m + s0m) - B.beta * (s1p + s1m + s0m - 2.f * s0 - 2.f * s1) + B.gam * (D0 + D1)) * ab;
+        ap[j] = s0p + inc[1][2];
+    }
+    {   // right wall: rows nx, nx-1, no incident wave
+        const size_t r0 = (size_t)nx * ny, r1 = (size_t)(nx - 1) * ny;
+        float E0 = a[r0 + jp] - 2.f * a[r0 + j] + a[r0 + jm];
+        float E1 = a[r1 + jp] - 2.f * a[r1 + j] + a[r1 + jm];
+        ap[r0 + j] = (B.alpha * (ap[r1 + j] - am[r1 + j] + am[r0 + j]) -
+                      B.beta * (ap[r1 + j] + am[r1 + j] + am[r0 + j] - 2.f * a[r0 + j] - 2.f * a[r1 + j]) + B.gam * (E0 + E1)) * ab;
+    }
+}
+
+// Eq. 16 / 18 on the nodes.  E arrives already averaged to the nodes (Q3; pm2d_poisson.cu).
+struct ForceParams {
+    const float2 *Enode;
+    const float *a;          // [ncomp][nn], the level the stage needs (n or n+1)
+    const int32_t *nfix;     // this species' density
+    float2 *F;
+    int nx, ny, ncomp;
+    float qE;                // -sign * 4 pi^2 / mass
+    float pond;              // 1 for electrons, 0 otherwise
+    float cv2;               // C * v_th^2
+    float inv_2dx, inv_2dy;
+};
+
+__device__ __forceinline__ float a2_at(const ForceParams &P, size_t k, size_t nn)
+{
+    float s = 0.f;
+    for (int c = 0; c < P.ncomp; c++) {
+        float v = P.a[c * nn + k];
+        s += v * v;
+    }
+    return s;
+}
+
+__global__ void __launch_bounds__(256) k_force(const ForceParams P)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y;
+    if (j >= P.ny) return;
+    const size_t nn = (size_t)(P.nx + 1) * P.ny;
+    const int jm = (j - 1) & (P.ny - 1), jp = (j + 1) & (P.ny - 1);
+    const int il = i > 0 ? i - 1 : 0, ih = i < P.nx ? i + 1 : P.nx;
+    const float sx = (il == i || ih == i) ? 2.f * P.inv_2dx : P.inv_2dx;     // one-sided at the walls
+    const size_t k = (size_t)i * P.ny + j, kl = (size_t)il * P.ny + j, kh = (size_t)ih * P.ny + j;
+    const size_t kd = (size_t)i * P.ny + jm, ku = (size_t)i * P.ny + jp;
+    float2 E = P.Enode[k];
+    float fx = P.qE * E.x, fy = P.qE * E.y;
+    if (P.pond != 0.f) {
+        fx -= 0.5f * sx * (a2_at(P, kh, nn) - a2_at(P, kl, nn));
+        fy -= 0.5f * P.inv_2dy * (a2_at(P, ku, nn) - a2_at(P, kd, nn));
+    }
+    const int n0 = P.nfix[k];
+    if (n0 > 0 && P.cv2 != 0.f) {
+        const float inv_n = 1.f / (float)n0;
+        fx -= P.cv2 * sx * (float)(P.nfix[kh] - P.nfix[kl]) * inv_n;
+        fy -= P.cv2 * P.inv_2dy * (float)(P.nfix[ku] - P.nfix[kd]) * inv_n;
+    }
+    P.F[k] = make_float2(fx, fy);
+}
+
+__global__ void k_fix_to_float(const int32_t *src, float scale, float *dst, size_t n)
+{
+    size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) dst[k] = (float)src[k] * scale;
+}
+__global__ void k_float_to_fix(const float *src, float scale, int32_t *dst, size_t n)
+{
+    size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) dst[k] = __float2int_rn(src[k] * scale);
+}
+__global__ void k_sum_fix(NeSrc S, int32_t *dst, size_t n)
+{
+    size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    int v = 0;
+    for (int s = 0; s < S.count; s++) v += S.n[s][k];
+    dst[k] = v;
+}
+
+}  // namespace
+
+// carrier * ramp of one laser at retarded time tau (double on the host: the phase 2 pi omega tau
+// grows without bound and must not be rounded to float)
+static double laser_g(const pm2d_laser &L, double tau)
+{
+    const double PI = 3.14159265358979323846;
+    if (tau <= 0.0) return 0.0;
+    double ramp = 1.0;
+    if (L.t_rise > 0.0 && tau < L.t_rise) {
+        double s = sin(0.5 * PI * tau / L.t_rise);
+        ramp = s * s;
+    }
+    return L.a0 * ramp * cos(2.0 * PI * L.omega * tau);
+}
+
+int launch_field_step(pm2d_ctx *c)
+{
+    const int nx = c->g.nx, ny = c->g.ny;
+    const double dx = c->g.dx, dy = c->g.dy, dt = c->g.dt, t_now = c->step * dt;
+    NeSrc ne;
+    ne.count = 0;
+    ne.inv_nscale = c->inv_nscale;
+    for (int s = 0; s < c->nsp; s++)
+        if (c->sp[s].cfg.sign < 0) ne.n[ne.count++] = c->sp[s].nfix;
+    BcParams B;
+    B.nlaser = c->nlaser;
+    for (int l = 0; l < c->nlaser; l++) {
+        const pm2d_laser &L = c->laser[l];
+        for (int xk = 0; xk < 2; xk++)
+            for (int tk = 0; tk < 3; tk++) B.g[l][xk * 3 + tk] = (float)laser_g(L, t_now + (tk - 1) * dt - xk * dx);
+        B.y0[l] = (float)L.y0;
+        B.inv_w0[l] = L.w0 > 0.0 ? (float)(1.0 / L.w0) : 0.f;
+        B.comp[l] = L.comp;
+    }
+    B.alpha = (float)(1.0 / (2.0 * dt * dx));
+    B.beta = (float)(1.0 / (2.0 * dt * dt));
+    B.gam = (float)(1.0 / (4.0 * dy * dy));
+    B.dy = (float)dy;
+    dim3 grid((ny + FCOLS - 1) / FCOLS, (nx - 1 + FROWS - 1) / FROWS);
+    for (int comp = 0; comp < c->g.ncomp; comp++) {
+        const size_t off = (size_t)comp * c->nn;
+        k_wave<<<grid, FCOLS, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, ne, nx, ny, (float)(1.0 / (dx * dx)),
+                                              (float)(1.0 / (dy * dy)), (float)(dt * dt));
+        k_boundary<<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, comp, nx, ny);
+        count_launch(c, 2);
+    }
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    return PM2D_OK;
+}
+
+int launch_force(pm2d_ctx *c, int s, const float *a_level)
+{
+    SpeciesDev &S = c->sp[s];
+    ForceParams P;
+    const double PI = 3.14159265358979323846;
+    P.Enode = c->Enode; P.a = a_level; P.nfix = S.nfix; P.F = S.F;
+    P.nx = c->g.nx; P.ny = c->g.ny; P.ncomp = c->g.ncomp;
+    P.qE = (float)(-(double)S.cfg.sign * 4.0 * PI * PI / S.cfg.mass);
+    P.pond = S.cfg.sign < 0 ? 1.f : 0.f;
+    P.cv2 = (float)(S.cfg.pressure_coeff * S.vth2);
+    P.inv_2dx = (float)(1.0 / (2.0 * c->g.dx));
+    P.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
+    dim3 grid((c->g.ny + 255) / 256, c->g.nx + 1);
+    k_force<<<grid, 256, 0, c->stream>>>(P);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    return PM2D_OK;
+}
+
+int launch_fix_background(pm2d_ctx *c, int s)
+{
+    NeSrc src;
+    src.count = 0;
+    src.inv_nscale = 1.f;
+    for (int t = 0; t < c->nsp; t++)
+        if (t != s && c->sp[t].cfg.mobile && c->sp[t].cfg.sign == -c->sp[s].cfg.sign) src.n[src.count++] = c->sp[t].nfix;
+    k_sum_fix<<<(unsigned)((c->nn + 255) / 256), 256, 0, c->stream>>>(src, c->sp[s].nfix, (size_t)c->nn);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    return PM2D_OK;
+}
+
+int launch_fix_to_float(pm2d_ctx *c, const int32_t *src, float scale, float *dst)
+{
+    k_fix_to_float<<<(unsigned)((c->nn + 255) / 256), 256, 0, c->stream>>>(src, scale, dst, (size_t)c->nn);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    return PM2D_OK;
+}
+
+int launch_float_to_fix(pm2d_ctx *c, const float *src, float scale, int32_t *dst)
+{
+    k_float_to_fix<<<(unsigned)((c->nn + 255) / 256), 256, 0, c->stream>>>(src, scale, dst, (size_t)c->nn);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    return PM2D_OK;
+}

@@ -1,0 +1,125 @@
+// pm2d_internal.h -- context layout and launcher prototypes shared by the .cu files of libpm2d.so.
+// Not part of the public ABI (include/pm2d.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/pm2d.h"
+
+// ---- geometry of the particle tiles -----------------------------------------------------------
+constexpr int TILE = PM2D_TILE;          // cells per tile side
+constexpr int HALO = 4;                  // window nodes beyond the tile on each side
+constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (41)
+constexpr int WPITCH = WIN;              // odd pitch: rows start on different banks
+constexpr int CHUNK = 8192;              // max particles per CTA work item
+constexpr int PTHREADS = 256;            // threads per particle CTA
+// fixed-point tile-relative position: (cell_rel + POS_BIAS) << 24 | frac24
+constexpr int POS_BIAS = 64;
+constexpr int POS_FRAC_BITS = 24;
+constexpr uint32_t POS_FRAC_MASK = (1u << POS_FRAC_BITS) - 1u;
+
+struct SpeciesDev {
+    // host copy of the parameters
+    pm2d_species cfg;
+    double vth2;
+    int64_t np;          // particles held (constant: walls reflect, y wraps)
+    int64_t cap;
+    // particle SoA (device)
+    uint32_t *x, *y;     // fixed-point tile-relative position
+    float *ux, *uy, *w;
+    float *uhx, *uhy;    // predictor velocity u^ (Eq. 17); scratch for the rebin
+    uint32_t *x2, *y2;   // rebin double buffers
+    float *w2;
+    int64_t *id, *id2;   // optional
+    // binning
+    int64_t *tile_off;   // [ntiles+1] first slot of each tile
+    int64_t *tile_off2;
+    int32_t *chunk_tile; // [max_chunks]
+    int64_t *chunk_beg;  // [max_chunks+1]
+    int32_t *chunk_cnt9; // [max_chunks][9] movers per direction (rebin)
+    int64_t *chunk_rel9; // [max_chunks][9] offset inside the destination tile
+    int32_t *tile_first_chunk; // [ntiles+1]
+    int32_t *tile_cnt;         // [ntiles] scratch: particles per tile after a rebin
+    int32_t *nchunks_dev;      // [1]
+    int32_t max_chunks;
+    int32_t nchunks;     // host copy (refreshed after a rebin)
+    // grids (device)
+    int32_t *nfix;       // density, fixed point, [(nx+1)*ny]
+    int32_t *pxfix, *pyfix;
+    float2 *F;           // nodal force (Eq. 16)
+};
+
+struct pm2d_ctx {
+    pm2d_grid g;
+    int nsp, nlaser;
+    SpeciesDev sp[PM2D_MAX_SPECIES];
+    pm2d_laser laser[PM2D_MAX_LASERS];
+    pm2d_profile profile;
+    uint64_t seed;
+    cudaStream_t stream;
+    int64_t step;
+    int64_t nn;          // nodes
+    int ntx, nty, ntiles;
+    int LP;              // pitch (complex elements) of spectral rows: ny/2 + 2
+    float nscale, inv_nscale; // density fixed point: n = fix * inv_nscale (power of two)
+    float pscale, inv_pscale; // momentum fixed point
+    // fields
+    float *a[3];         // ring of time levels, each [ncomp][nn]; a[0] = n+1 target, a[1] = n, a[2] = n-1
+    float2 *rho_hat;     // [(nx+1)][LP]
+    double2 *dtmp;       // [(nx+1)][LP] forward-sweep result
+    double *cp;          // [(nx+1)][LP] Thomas c' coefficients (right-hand-side independent)
+    float2 *ehx, *ehy;   // [(nx+1)][LP] spectra of nodal E (or phi^ in ehx for diagnostics)
+    float2 *Enode;       // [nn]
+    float *phi;          // [nn] (diagnostics only)
+    float2 *twiddle;     // [ny/2]
+    double *red;         // [64] reduction scratch
+    int32_t *flags;      // [4] device error flags
+    // profile
+    bool prof_on;
+    std::vector<cudaEvent_t> ev;   // 2 per phase per step, reused ring
+    std::vector<int> ev_phase;
+    double prof_ms[PM2D_PH_COUNT];
+    int64_t prof_launch[PM2D_PH_COUNT];
+    int64_t prof_steps;
+    int cur_phase;
+    int64_t launches;
+};
+
+void pm2d_set_error(const std::string &s);
+#define PM2D_CUDA_CHECK(call)                                                                  \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            pm2d_set_error(std::string(#call) + ": " + cudaGetErrorString(e_));                \
+            return PM2D_ECUDA;                                                                 \
+        }                                                                                      \
+    } while (0)
+
+static inline void count_launch(pm2d_ctx *c, int n = 1)
+{
+    c->launches += n;
+    if (c->prof_on && c->cur_phase >= 0) c->prof_launch[c->cur_phase] += n;
+}
+
+// ---- launchers (each enqueues on c->stream and returns a PM2D_* code) --------------------------
+// pm2d_particles.cu
+int launch_load_particles(pm2d_ctx *c, int s);
+int launch_stage(pm2d_ctx *c, int s, int stage);            // 0 = A (Eq. 17), 1 = B (Eq. 19)
+int launch_deposit_only(pm2d_ctx *c, int s, bool density, bool momentum);
+int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev);
+int launch_build_chunks(pm2d_ctx *c, int s);
+int launch_unpack_particles(pm2d_ctx *c, int s, int64_t first, int64_t count, int32_t *ix, int32_t *iy,
+                            float *fx, float *fy);
+// pm2d_fields.cu
+int launch_field_step(pm2d_ctx *c);
+int launch_force(pm2d_ctx *c, int s, const float *a_level);
+int launch_fix_background(pm2d_ctx *c, int s);
+int launch_fix_to_float(pm2d_ctx *c, const int32_t *src, float scale, float *dst);
+int launch_float_to_fix(pm2d_ctx *c, const float *src, float scale, int32_t *dst);
+// pm2d_poisson.cu
+int launch_poisson_init(pm2d_ctx *c);
+int launch_poisson(pm2d_ctx *c, bool want_phi);
+// pm2d_diag.cu
+int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out);

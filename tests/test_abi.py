@@ -1,0 +1,57 @@
+"""The C-ABI library loads and exports every symbol include/pm2d.h declares (no GPU needed)."""
+import os
+import re
+
+import paper_2404_14293_b200 as P
+from paper_2404_14293_b200 import build as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    txt = open(os.path.join(ROOT, "include", "pm2d.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(pm2d_[a-z_0-9]+)\s*\(", txt)))
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    B.build()
+    lib = P.load_library()
+    declared = _declared_symbols()
+    assert len(declared) >= 18
+    for name in declared:
+        assert hasattr(lib, name), name
+        assert name in P.SYMBOLS, f"binding does not type {name}"
+    assert sorted(P.SYMBOLS) == declared
+    assert b"sm_100a" in lib.pm2d_version()
+
+
+def test_argument_validation_needs_no_gpu():
+    import ctypes as C
+    import pm2d_inputs as I
+    from paper_2404_14293_b200.binding import make_structs
+
+    lib = P.load_library()
+    cfg = I.config("c1", nx=64, ny=32)
+    grid, sp, prof, las = make_structs(cfg)
+    assert lib.pm2d_query_workspace(C.byref(grid), sp, len(cfg["species"])) > 0
+    grid.ny = 48                                   # not a power of two
+    assert lib.pm2d_query_workspace(C.byref(grid), sp, len(cfg["species"])) == 0
+    assert b"power of two" in lib.pm2d_last_error()
+    grid.ny = 32
+    grid.dt = 0.06                                 # dt/dx > 1
+    assert lib.pm2d_query_workspace(C.byref(grid), sp, len(cfg["species"])) == 0
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2404_14293_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "pm2d_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_2404_14293_b200", txt, flags=re.M), f
+            assert not re.search(r"#include\s+\"[^\"]*(csrc|pm2d\.h|pm2d_internal)", txt), f

@@ -1,0 +1,261 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: deposited fields rel-L2 <= 1e-5 per step,
+particle phase space after 10 steps max relative error <= 1e-5, rebin bit-exact, energies 2 %."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import pm2d_inputs as I
+from helpers import oracle_from_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2404_14293_b200 as pkg
+    from paper_2404_14293_b200 import build
+    build.build()
+    return pkg
+
+
+def rel_l2(a, b):
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    d = np.sqrt(((a - b) ** 2).sum())
+    n = np.sqrt((b ** 2).sum())
+    return d / n if n > 0 else d
+
+
+def small_cfg(name, nx, ny, **over):
+    cfg = I.config(name, nx=nx, ny=ny)
+    cfg["grid"].update(over)
+    return cfg
+
+
+CASES = [("c1", 96, 64), ("c2", 80, 32), ("c3", 72, 64)]   # CIC / TSC / SINE(+mobile ions); ragged nx
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,nx,ny", CASES)
+def test_device_loader_equals_numpy_generator(P, name, nx, ny):
+    cfg = small_cfg(name, nx, ny)
+    sim = P.PM2D(cfg, track_ids=1)
+    for s, sp in enumerate(cfg["species"]):
+        if sp["load"] == I.LOAD_NONE:
+            continue
+        ref = I.generate_particles(cfg, s)
+        got = sim.get_particles(s, with_id=True)
+        assert got["id"].size == ref["id"].size == I.n_particles(cfg, s)
+        order = np.argsort(got["id"])
+        assert np.array_equal(got["id"][order], ref["id"])            # ref is in id order
+        for k in ("ix", "iy", "fx", "fy"):
+            assert np.array_equal(got[k][order], ref[k]), k
+        for k in ("ux", "uy", "w"):
+            a, b = got[k][order], ref[k]
+            ulp = np.abs(a.view(np.int32).astype(np.int64) - b.view(np.int32).astype(np.int64))
+            assert ulp.max() <= 1, (k, ulp.max())
+            assert (ulp > 0).mean() < 1e-3
+        # storage order is tile-major
+        key = (got["ix"] // P.TILE) * ((ny + P.TILE - 1) // P.TILE) + got["iy"] // P.TILE
+        assert (np.diff(key) >= 0).all()
+    sim.close()
+
+
+@pytest.mark.parametrize("name,nx,ny", CASES)
+def test_initial_deposit_parity(P, name, nx, ny):
+    cfg = small_cfg(name, nx, ny)
+    sim = P.PM2D(cfg, eager_moments=1)
+    orc, _ = oracle_from_config(cfg)
+    for s, sp in enumerate(cfg["species"]):
+        n = sim.get_moments(s, P.MOMENT_N)
+        assert rel_l2(n, orc.moment(s, "n")) < 1e-5
+        if sp["mobile"]:
+            for mom, key in ((P.MOMENT_PX, "Px"), (P.MOMENT_PY, "Py")):
+                ref = orc.moment(s, key)
+                if np.abs(ref).max() > 0:
+                    assert rel_l2(sim.get_moments(s, mom), ref) < 1e-5
+    d = sim.diagnostics()
+    vol = np.ones((nx + 1, 1)); vol[0] = vol[-1] = 0.5
+    for s in range(len(cfg["species"])):
+        assert d["charge"][s] == pytest.approx((orc.moment(s, "n") * vol).sum(), rel=1e-6)
+        assert d["count"][s] == I.n_particles(cfg, s)
+    sim.close()
+
+
+def test_lazy_momentum_equals_eager(P):
+    cfg = small_cfg("c3", 72, 64)
+    a, b = P.PM2D(cfg, eager_moments=1), P.PM2D(cfg, eager_moments=0)
+    a.step(3); b.step(3)
+    for mom in (P.MOMENT_N, P.MOMENT_PX, P.MOMENT_PY):
+        assert np.array_equal(a.get_moments(0, mom), b.get_moments(0, mom))      # integer deposit: bit-exact
+    pa, pb = a.get_particles(0), b.get_particles(0)
+    for k in pa:
+        assert np.array_equal(pa[k], pb[k])
+    a.close(); b.close()
+
+
+def test_deposit_is_bit_reproducible(P):
+    cfg = small_cfg("c3", 72, 64)
+    runs = []
+    for _ in range(2):
+        sim = P.PM2D(cfg)
+        sim.step(4)
+        runs.append((sim.get_moments(0, P.MOMENT_N), sim.get_fields(P.FIELD_A), sim.get_particles(0)))
+        sim.close()
+    assert np.array_equal(runs[0][0], runs[1][0]) and np.array_equal(runs[0][1], runs[1][1])
+    for k in runs[0][2]:
+        assert np.array_equal(runs[0][2][k], runs[1][2][k])
+
+
+# ---------------------------------------------------------------------------------------------
+def _compare_particles(sim, orc, cfg, s, vth):
+    got = sim.get_particles(s, with_id=True)
+    order = np.argsort(got["id"])
+    nx, ny = cfg["grid"]["nx"], cfg["grid"]["ny"]
+    X = got["ix"][order].astype(np.float64) + got["fx"][order]
+    Y = got["iy"][order].astype(np.float64) + got["fy"][order]
+    oX, oY = orc.sp[s]["X"], orc.sp[s]["Y"]
+    dX = np.abs(X - oX)
+    dY = np.abs(Y - oY)
+    dY = np.minimum(dY, ny - dY)
+    ex = (dX / np.maximum(np.abs(oX), 1.0)).max()
+    ey = (dY / np.maximum(np.abs(oY), 1.0)).max()
+    eu = max((np.abs(got["ux"][order] - orc.sp[s]["ux"]) / np.maximum(np.abs(orc.sp[s]["ux"]), vth)).max(),
+             (np.abs(got["uy"][order] - orc.sp[s]["uy"]) / np.maximum(np.abs(orc.sp[s]["uy"]), vth)).max())
+    return ex, ey, eu, max(dX.max(), dY.max())
+
+
+@pytest.mark.parametrize("name,nx,ny,rebin", [("c1", 96, 64, 0), ("c2", 80, 32, 3), ("c3", 72, 64, 1), ("c3", 64, 16, 4)])
+def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin):
+    cfg = small_cfg(name, nx, ny)
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=rebin)
+    orc, _ = oracle_from_config(cfg)
+    for step in range(10):
+        sim.step(1)
+        orc.step(1)
+        for s, sp in enumerate(cfg["species"]):
+            if not sp["mobile"]:
+                continue
+            assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < 1e-5, (step, s)
+            assert rel_l2(sim.get_moments(s, P.MOMENT_PX), orc.moment(s, "Px")) < 1e-5, (step, s)
+            assert rel_l2(sim.get_moments(s, P.MOMENT_PY), orc.moment(s, "Py")) < 1e-5, (step, s)
+        a = sim.get_fields(P.FIELD_A, 0, 0)
+        scale = max(np.abs(orc.a_now[0]).max(), 1e-30)
+        assert np.abs(a - orc.a_now[0]).max() < 2e-5 * scale + 1e-9, step
+    for s, sp in enumerate(cfg["species"]):
+        if not sp["mobile"]:
+            continue
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
+        assert ex < 1e-5 and ey < 1e-5 and eu < 1e-5, (s, ex, ey, eu)
+        assert dabs < 1e-4                                    # absolute, in cells
+    # the last force grid (Eq. 18) and the potential of the final densities
+    for s, sp in enumerate(cfg["species"]):
+        if sp["mobile"]:
+            fx = sim.get_fields(P.FIELD_FORCE, 0, s)
+            fy = sim.get_fields(P.FIELD_FORCE, 1, s)
+            ref = np.hypot(orc.moment(s, "Fx"), orc.moment(s, "Fy"))
+            err = np.hypot(fx - orc.moment(s, "Fx"), fy - orc.moment(s, "Fy"))
+            assert np.sqrt((err ** 2).sum()) < 2e-4 * np.sqrt((ref ** 2).sum()), s
+    orc.refresh_fields()
+    phi = sim.get_fields(P.FIELD_PHI)
+    assert rel_l2(phi, orc.phi.reshape(nx + 1, ny)) < 2e-4
+    sim.close()
+
+
+def test_rebin_is_a_stable_counting_sort(P):
+    cfg = small_cfg("c3", 136, 128, rebin_every=0)
+    for sp in cfg["species"]:
+        sp["T_keV"] *= 40.0                                   # fast particles: many tile crossings
+    sim = P.PM2D(cfg, track_ids=1, rebin_every=0)
+    nty = (128 + P.TILE - 1) // P.TILE
+    for rounds in range(3):
+        sim.step(3)
+        before = sim.get_particles(0, with_id=True)
+        key_ref = (before["ix"] // P.TILE) * nty + before["iy"] // P.TILE
+        keys, perm = sim.rebin(0)
+        assert np.array_equal(keys, key_ref.astype(np.int32))
+        perm_ref = np.argsort(key_ref, kind="stable")
+        assert np.array_equal(perm, perm_ref)
+        after = sim.get_particles(0, with_id=True)
+        for k in before:
+            assert np.array_equal(after[k], before[k][perm_ref]), k
+        hist = np.bincount(key_ref, minlength=nty * ((136 + P.TILE - 1) // P.TILE))
+        assert hist.sum() == before["ix"].size
+        assert (np.diff((after["ix"] // P.TILE) * nty + after["iy"] // P.TILE) >= 0).all()
+    sim.close()
+
+
+def test_set_particles_roundtrip_and_host_supplied_inputs(P):
+    """Particles supplied by the host (any order), incl. the degenerate cases: a particle exactly on a
+    node, at the first/last representable offset, next to both walls; empty species."""
+    nx, ny = 40, 16
+    cfg = small_cfg("c3", nx, ny)
+    cfg["species"][1]["load"] = I.LOAD_NONE                   # ions supplied by hand
+    cfg["species"][1]["capacity"] = 64
+    cfg["species"][0]["load"] = I.LOAD_NONE
+    cfg["species"][0]["capacity"] = 4096
+    cfg["lasers"] = []
+    sim = P.PM2D(cfg, track_ids=1, rebin_every=2)
+    assert sim.particle_count(0) == 0
+    sim.step(2)                                               # empty species: nothing to push, no crash
+    rng = np.random.default_rng(5)
+    n = 4000
+    parts = dict(ix=rng.integers(0, nx, n).astype(np.int32), iy=rng.integers(0, ny, n).astype(np.int32),
+                 fx=(rng.integers(0, 2 ** 24, n) / 2.0 ** 24).astype(np.float32),
+                 fy=(rng.integers(0, 2 ** 24, n) / 2.0 ** 24).astype(np.float32),
+                 ux=rng.normal(0, 0.08, n).astype(np.float32), uy=rng.normal(0, 0.08, n).astype(np.float32),
+                 w=rng.uniform(0.01, 0.03, n).astype(np.float32))
+    parts["ix"][:4] = [0, nx - 1, 5, 7]
+    parts["fx"][:4] = [0.0, 1.0 - 2.0 ** -24, 0.0, 0.5]
+    parts["ux"][:2] = [-0.3, 0.3]                             # into the walls
+    sim.set_particles(0, parts, refix_background=False)
+    ions = {k: v[:50].copy() for k, v in parts.items()}
+    ions["ux"] *= 0.01; ions["uy"] *= 0.01
+    sim.set_particles(1, ions, refix_background=False)
+    got = sim.get_particles(0, with_id=True)
+    order = np.argsort(got["id"])
+    for k in parts:
+        assert np.array_equal(got[k][order], parts[k]), k
+    osp = []
+    for s, pp in enumerate((parts, ions)):
+        sp = cfg["species"][s]
+        osp.append(dict(mass=sp["mass"], sign=sp["sign"], T_keV=sp["T_keV"], C=sp["pressure_coeff"], shape=sp["shape"], DD=sp["DD"],
+                        mobile=1, X=pp["ix"] + pp["fx"].astype(np.float64), Y=pp["iy"] + pp["fy"].astype(np.float64),
+                        ux=pp["ux"], uy=pp["uy"], w=pp["w"]))
+    g = cfg["grid"]
+    orc = oracle.Oracle(nx, ny, g["dx"], g["dy"], g["dt"], osp, [], 1)
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
+    sim.step(6)
+    orc.step(6)
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
+    assert rel_l2(sim.get_moments(1, P.MOMENT_N), orc.moment(1, "n")) < 1e-5
+    ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, 0, math.sqrt(3.0 / 511.0))
+    assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4
+    assert sim.particle_count(0) == n and sim.diagnostics()["count"][0] == n
+    sim.close()
+
+
+def test_energy_history_parity_c1(P):
+    """Config 1 in full (256x128, 131,072 electrons, 100 steps): every energy term within 2 %."""
+    cfg = I.config("c1")
+    sim = P.PM2D(cfg)
+    orc, _ = oracle_from_config(cfg)
+    for n in range(5):
+        sim.step(20)
+        orc.step(20)
+        d, e = sim.diagnostics(), orc.energies()
+        assert d["W_kin"][0] == pytest.approx(e["W_kin"][0], rel=1e-4)
+        assert d["W_th"][0] == pytest.approx(e["W_th"][0], rel=1e-4)
+        assert d["W_int"] == pytest.approx(e["W_int"], rel=0.02, abs=1e-12)
+        assert d["W_em"] == pytest.approx(e["W_em"], rel=0.02, abs=1e-12)
+        assert d["W_es"] == pytest.approx(e["W_es"], rel=0.02)
+        assert d["count"][0] == 131072
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
+    assert rel_l2(sim.get_fields(P.FIELD_A), orc.a_now[0]) < 1e-4
+    sim.close()
