@@ -1,0 +1,252 @@
+#!/usr/bin/env python
+"""bench.py -- whole-step throughput of the PM2D hot path on B200 (contract in the build brief).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl reference]
+
+One "step" = one pass of the whole hot path (field update, 2 Poisson solves, 2 force grids, fused
+gather-push-deposit stage A and B for every mobile species, periodic rebin) over the resident
+particle set.  N = 1 workload: BASELINE.json configs[2], the 8192x4096 SRS-scale slab the
+north_star target is quoted on (134 M electrons + 33.5 M deuterium ions, sine shape).  N > 1: the
+path does not shard without the paper's domain decomposition (out of scope: "only one GPU is
+used"), so every rank runs an independent replica -- weak scaling, no collective on the data path.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import pm2d_inputs as I  # noqa: E402
+
+BYTES_STAGE_A = 28   # read x, y, ux, uy, w (20 B), write u^ (8 B)            -- DESIGN.md section 7
+BYTES_STAGE_B = 44   # read x, y, ux, uy, w, u^ (28 B), write x, y, ux, uy (16 B)
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(self.rows))
+
+
+def time_oracle(cfg, steps, warmup):
+    """The CPU oracle as it stands (single thread, double precision) on a reduced copy of the workload."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import oracle
+    from helpers import oracle_from_config
+    oracle.build()
+    orc, parts = oracle_from_config(cfg)
+    nmob = sum(len(p["ix"]) for s, p in enumerate(parts) if p is not None and cfg["species"][s]["mobile"])
+    orc.step(warmup)
+    t0 = time.perf_counter()
+    orc.step(steps)
+    dt = time.perf_counter() - t0
+    return nmob * steps / dt, dt / steps, nmob
+
+
+def sample_config(name, nx, ny):
+    return I.config(name, nx=nx, ny=ny)
+
+
+def run_reference(args):
+    """--impl reference: the oracle on host cores, same metric/config keys; each step is a bounded
+    sample (a 512x256 copy of the workload: same dx, dt, particles per cell, profile, species, laser)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = sample_config(args.config, 512, 256)
+    value, sec_per_step, nmob = time_oracle(cfg, args.steps, args.warmup)
+    g = I.config(args.config)["grid"]
+    line = dict(impl="reference", metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=sec_per_step * 1e3, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} SRS-scale slab (BASELINE.json configs[2])",
+                            sample=f"{cfg['name']} reduced copy, {nmob} mobile particles"),
+                cpu_baseline=dict(value=value, unit="particle-steps/s", cores=1, kind="oracle",
+                                  sample=f"{cfg['name']}: {nmob} mobile particles x {args.steps} steps"),
+                e2e=dict(value=value, unit="particle-steps/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2404_14293_b200 as pkg
+    from paper_2404_14293_b200 import build
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        dist.barrier()
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    cfg = I.config(args.config)
+    cfg["seed"] = int(cfg["seed"]) + 1000 * rank          # independent replicas
+    g = cfg["grid"]
+    sim = pkg.PM2D(cfg, device=f"cuda:{local}", eager_moments=args.eager, rebin_every=args.rebin_every)
+    nmob = sum(sim.particle_count(s) for s, sp in enumerate(cfg["species"]) if sp["mobile"])
+    nodes = (g["nx"] + 1) * g["ny"]
+
+    # ---- device-timed region: K steps, inputs resident in HBM ---------------------------------
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    sim.profile_enable(True)
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    sim.step_async(args.steps)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    prof = sim.profile_get()
+    sim.profile_enable(False)
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = nmob * world * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers: per step the host sends the laser table
+    # (H2D, kernel arguments) and reads back the left-boundary probe column of a ----------
+    probe = np.empty((1, g["ny"]), np.float32)
+    lasers = cfg["lasers"]
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        sim.set_lasers(lasers)
+        sim.step(1)
+        sim.get_fields(pkg.FIELD_A, 0, 0, window=(0, 1, 0, g["ny"]), out=probe)
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = nmob * world * args.steps / float(t.item())
+
+    if rank == 0:
+        peak, peak_src = hbm_peak()
+        steps_p = max(prof["steps"], 1)
+        stage_ms = (prof["ms"]["stage_a"] + prof["ms"]["stage_b"]) / steps_p
+        alg_bytes = (BYTES_STAGE_A + BYTES_STAGE_B) * nmob
+        achieved = alg_bytes / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "stage_traffic_bytes.txt")
+        if os.path.exists(tp):
+            try:
+                traffic = float(open(tp).read().split()[0])
+            except Exception:
+                traffic = None
+        line = dict(metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=world, steps=args.steps,
+                    warmup=args.warmup, ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak",
+                    vs_baseline=None, dtype="f32", data="synthetic",
+                    config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU "
+                                         f"(BASELINE.json configs[{int(args.config[1]) - 1}])",
+                                shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
+                                eager_moments=bool(args.eager), rebin_every=sim.grid.rebin_every,
+                                l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
+                                parallelism="replicas only" if world > 1 else "1 GPU"),
+                    ns_per_particle_step=1e9 / value * world,
+                    cell_updates_per_s=nodes * g["ncomp"] * world * args.steps / (ms_max * 1e-3),
+                    field_kernel_node_updates_per_s=(nodes * g["ncomp"] / (prof["ms"]["field"] / steps_p * 1e-3)) if prof["ms"]["field"] > 0 else None,
+                    phases_ms_per_step={k: v / steps_p for k, v in prof["ms"].items()},
+                    clocks=clocks, gpu_launches=int(launches),
+                    e2e=dict(value=e2e_value, unit="particle-steps/s",
+                             h2d_bytes_per_step=int(len(lasers) * 48), d2h_bytes_per_step=int(g["ny"] * 4 + 16)),
+                    roofline=dict(bound="hbm", kernel="k_stage (fused gather-push-deposit, stage A + stage B, all mobile species)",
+                                  achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, peak_source=peak_src,
+                                  algorithmic_bytes_per_particle_step=BYTES_STAGE_A + BYTES_STAGE_B,
+                                  ms_per_step=stage_ms, traffic=traffic))
+        if world == 1 and not args.no_cpu_baseline:
+            scfg = sample_config(args.config, 1024, 512)
+            v, sec, n = time_oracle(scfg, 3, 1)
+            line["cpu_baseline"] = dict(value=v, unit="particle-steps/s", cores=1, kind="oracle",
+                                        sample=f"{scfg['name']} reduced copy of the workload: {n} mobile particles x 3 steps ({sec * 3:.1f} s)")
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--eager", type=int, default=1, help="1: deposit n, Px, Py at both stages (paper's flow); 0: n only")
+    ap.add_argument("--rebin-every", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -88,8 +88,15 @@ size_t layout(pm2d_ctx *c, char *base)
     const size_t ns = (size_t)(g.nx + 1) * LP;
     for (int k = 0; k < 3; k++) c->a[k] = cv.take<float>(g.ncomp * nn);
     c->rho_hat = cv.take<float2>(ns);
-    c->dtmp = cv.take<double2>(ns);
-    c->cp = cv.take<double>(ns);
+    {
+        const size_t P = (size_t)(g.nx + TRI_M - 1) / TRI_M;
+        c->tri_cp = cv.take<double>((size_t)2 * TRI_M * LP);
+        c->tri_V = cv.take<double>((size_t)2 * TRI_M * LP);
+        c->tri_W = cv.take<double>((size_t)2 * TRI_M * LP);
+        c->tri_sumV = cv.take<double2>(P * LP);
+        c->tri_sumW = cv.take<double2>(P * LP);
+        c->tri_g = cv.take<double2>((P + 1) * LP);
+    }
     c->ehx = cv.take<float2>(ns);
     c->ehy = cv.take<float2>(ns);
     c->Enode = cv.take<float2>(nn);

@@ -15,6 +15,7 @@ constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (41)
 constexpr int WPITCH = WIN;              // odd pitch: rows start on different banks
 constexpr int CHUNK = 8192;              // max particles per CTA work item
 constexpr int PTHREADS = 256;            // threads per particle CTA
+constexpr int TRI_M = 32;                // rows per x-partition of the tridiagonal solve
 // fixed-point tile-relative position: (cell_rel + POS_BIAS) << 24 | frac24
 constexpr int POS_BIAS = 64;
 constexpr int POS_FRAC_BITS = 24;
@@ -68,8 +69,10 @@ struct pm2d_ctx {
     // fields
     float *a[3];         // ring of time levels, each [ncomp][nn]; a[0] = n+1 target, a[1] = n, a[2] = n-1
     float2 *rho_hat;     // [(nx+1)][LP]
-    double2 *dtmp;       // [(nx+1)][LP] forward-sweep result
-    double *cp;          // [(nx+1)][LP] Thomas c' coefficients (right-hand-side independent)
+    // partitioned chasing method (pm2d_poisson.cu): tables [2][TRI_M][LP], sums [P][LP], g [P+1][LP]
+    double *tri_cp, *tri_V, *tri_W;
+    double2 *tri_sumV, *tri_sumW, *tri_g;
+    int tri_P, tri_mlast;
     float2 *ehx, *ehy;   // [(nx+1)][LP] spectra of nodal E (or phi^ in ehx for diagnostics)
     float2 *Enode;       // [nn]
     float *phi;          // [nn] (diagnostics only)

@@ -1,14 +1,22 @@
 // pm2d_poisson.cu -- the electrostatic module without cuFFT / cuSPARSE:
-//   k_fft_rho   : rho = sum_s sign_s n_s (exact integer difference of the fixed-point deposits),
-//                 radix-2 FFT along y in shared memory, one CTA per grid row          (Eq. 9-10)
-//   k_tridiag   : one thread per k_y: Thomas ("chasing") sweep along x in double with the
-//                 right-hand-side independent c' coefficients precomputed at init      (Eq. 11)
-//                 the back-substitution emits the spectrum of E already averaged to the nodes
-//   k_ifft_pair : one complex inverse FFT per row returns E_x (real part) and E_y (imaginary part)
+//   k_fft_rho     : rho = sum_s sign_s n_s (exact integer difference of the fixed-point deposits),
+//                   Stockham radix-4 FFT along y in shared memory, one CTA per grid row   (Eq. 9-10)
+//   k_tri_sums / k_tri_reduced / k_tri_local : the tridiagonal systems of Eq. 11, one per k_y,
+//                   solved exactly (to rounding) by the chasing method applied to x-partitions
+//                   of TRI_M rows so that (k_y, partition) pairs -- not just k_y -- run in parallel
+//   k_ifft        : one complex inverse FFT per row returns E_x (real part) and E_y (imaginary part)
+//
+// Partitioned chasing method.  Rows kM (k = 1..P-1) are interfaces with unknown values g_k.  Inside a
+// partition the solution is  phi = y + g_k V + g_{k+1} W, with y the local solve for zero interface
+// values and V, W the two homogeneous solutions (right-hand-side independent, tabulated at init).
+// By symmetry of the local matrix, y_1 = -sum_j V_j r_j and y_m = -sum_j W_j r_j, so the reduced
+// (P-1)-unknown tridiagonal system for g needs only two weighted column sums per partition
+// (k_tri_sums), is solved by one thread per k_y (k_tri_reduced), and then every partition is
+// solved ONCE with its true boundary values, entirely in registers, in double (k_tri_local).
 //
 // Why E leaves the solver in spectral form.  The paper differences phi in real space
-// and the force needs E on the nodes (Q3).  Both operations are shifts and sums along y and x, so
-// by the DFT shift theorem they are exact multipliers of each mode (theta = 2 pi l / ny):
+// and the force needs E on the nodes (Q3).  Both are shifts and sums along y and x, hence exact
+// multipliers of each mode by the DFT shift theorem (theta = 2 pi l / ny):
 //   E_x,node(i) = -cos^2(theta/2) (phi^_{i+1} - phi^_{i-1}) / (2 dx)
 //   E_y,node(i) = -i sin(theta) (phi^_{i-1} + 2 phi^_i + phi^_{i+1}) / (4 dy)
 // (walls: one-sided forms below).  Applying them to the double-precision phi^ avoids differencing
@@ -18,6 +26,7 @@
 namespace {
 
 constexpr int FFT_THREADS = 256;
+constexpr int M = TRI_M;
 
 struct RhoSrc {
     const int32_t *n[PM2D_MAX_SPECIES];
@@ -26,31 +35,58 @@ struct RhoSrc {
     float inv_nscale;
 };
 
-// in-place radix-2 decimation-in-time FFT of buf[0..n-1] (already in bit-reversed order);
-// tw[k] = exp(-2 pi i k / n); inverse uses the conjugate twiddles.
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// Stockham autosort FFT of n points held in shared memory (natural order in, natural order out).
+// x, y: ping-pong buffers; tw[t] = exp(-2 pi i t / n), t < n/2.  Returns the buffer with the result.
 template <bool INVERSE>
-__device__ void fft_shared(float2 *buf, const float2 *__restrict__ tw, int n, int log2n)
+__device__ float2 *fft_stockham(float2 *x, float2 *y, const float2 *__restrict__ tw, int n)
 {
-    for (int s = 1; s <= log2n; s++) {
-        const int h = 1 << (s - 1);
-        const int tstride = n >> s;
+    int Ns = 1;
+    while (Ns < n) {
         __syncthreads();
-        for (int b = threadIdx.x; b < n / 2; b += blockDim.x) {
-            int k = b & (h - 1);
-            int p = ((b >> (s - 1)) << s) + k, q = p + h;
-            float2 w = tw[k * tstride];
-            if (INVERSE) w.y = -w.y;
-            float2 u = buf[p], v = buf[q];
-            float2 t = make_float2(v.x * w.x - v.y * w.y, v.x * w.y + v.y * w.x);
-            buf[p] = make_float2(u.x + t.x, u.y + t.y);
-            buf[q] = make_float2(u.x - t.x, u.y - t.y);
+        if (n / Ns >= 4) {
+            const int q = n >> 2, tstep = n / (4 * Ns);
+            for (int j = threadIdx.x; j < q; j += blockDim.x) {
+                const int k = j & (Ns - 1);
+                float2 v0 = x[j], v1 = x[j + q], v2 = x[j + 2 * q], v3 = x[j + 3 * q];
+                if (Ns > 1) {
+                    float2 w1 = tw[k * tstep], w2 = tw[2 * k * tstep];
+                    if (INVERSE) { w1.y = -w1.y; w2.y = -w2.y; }
+                    float2 w3 = cmul(w1, w2);
+                    v1 = cmul(v1, w1); v2 = cmul(v2, w2); v3 = cmul(v3, w3);
+                }
+                float2 a0 = make_float2(v0.x + v2.x, v0.y + v2.y), a1 = make_float2(v0.x - v2.x, v0.y - v2.y);
+                float2 a2 = make_float2(v1.x + v3.x, v1.y + v3.y), d = make_float2(v1.x - v3.x, v1.y - v3.y);
+                float2 a3 = INVERSE ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);     // (+/- i) d
+                const int j0 = ((j - k) << 2) + k;
+                y[j0] = make_float2(a0.x + a2.x, a0.y + a2.y);
+                y[j0 + Ns] = make_float2(a1.x + a3.x, a1.y + a3.y);
+                y[j0 + 2 * Ns] = make_float2(a0.x - a2.x, a0.y - a2.y);
+                y[j0 + 3 * Ns] = make_float2(a1.x - a3.x, a1.y - a3.y);
+            }
+            Ns <<= 2;
+        } else {
+            const int h = n >> 1, tstep = n / (2 * Ns);
+            for (int j = threadIdx.x; j < h; j += blockDim.x) {
+                const int k = j & (Ns - 1);
+                float2 w = tw[k * tstep];
+                if (INVERSE) w.y = -w.y;
+                float2 a = x[j], b = cmul(x[j + h], w);
+                const int j0 = ((j - k) << 1) + k;
+                y[j0] = make_float2(a.x + b.x, a.y + b.y);
+                y[j0 + Ns] = make_float2(a.x - b.x, a.y - b.y);
+            }
+            Ns <<= 1;
         }
+        float2 *t = x; x = y; y = t;
     }
     __syncthreads();
+    return x;
 }
 
 __global__ void __launch_bounds__(FFT_THREADS) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw, float2 *__restrict__ rho_hat,
-                                                         int ny, int log2n, int LP)
+                                                         int ny, int LP)
 {
     extern __shared__ float2 buf[];
     const int i = blockIdx.x + 1;                     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
@@ -58,126 +94,17 @@ __global__ void __launch_bounds__(FFT_THREADS) k_fft_rho(RhoSrc S, const float2 
     for (int j = threadIdx.x; j < ny; j += blockDim.x) {
         int v = 0;
         for (int s = 0; s < S.count; s++) v += S.sign[s] * S.n[s][row + j];
-        buf[__brev((unsigned)j) >> (32 - log2n)] = make_float2((float)v * S.inv_nscale, 0.f);
+        buf[j] = make_float2((float)v * S.inv_nscale, 0.f);
     }
-    fft_shared<false>(buf, tw, ny, log2n);
-    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) rho_hat[(size_t)i * LP + l] = buf[l];
-}
-
-__global__ void k_cp_init(double *cp, int nx, int ny, int LP, double dx, double Ly)
-{
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l > ny / 2) return;
-    const double PI = 3.14159265358979323846;
-    const double ky = 2.0 * PI * (double)l / Ly;
-    const double b = -2.0 - ky * ky * dx * dx;
-    double c = 0.0;
-    for (int i = 1; i < nx; i++) {
-        c = 1.0 / (b - c);
-        cp[(size_t)i * LP + l] = c;
-    }
-}
-
-struct TriParams {
-    const float2 *rho_hat;
-    float2 *phi_hat;      // may alias rho_hat (row i is read before it is written); NULL: not wanted
-    const double *cp;
-    double2 *d;
-    float2 *ehx, *ehy;
-    int nx, ny, LP;
-    double dx2, inv_dx, inv_dy, inv_ny;
-};
-
-__global__ void __launch_bounds__(32) k_tridiag(const TriParams T)
-{
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
-    if (l > T.ny / 2) return;
-    const int nx = T.nx, LP = T.LP;
-    constexpr int B = 8;
-    // forward elimination: d_i = (dx^2 rho^_i - d_{i-1}) c'_i
-    double dr = 0.0, di = 0.0;
-    for (int i0 = 1; i0 < nx; i0 += B) {
-        float2 r[B];
-        double c[B];
-#pragma unroll
-        for (int k = 0; k < B; k++) {
-            int i = min(i0 + k, nx - 1);
-            r[k] = T.rho_hat[(size_t)i * LP + l];
-            c[k] = T.cp[(size_t)i * LP + l];
-        }
-#pragma unroll
-        for (int k = 0; k < B; k++) {
-            int i = i0 + k;
-            if (i < nx) {
-                dr = (T.dx2 * (double)r[k].x - dr) * c[k];
-                di = (T.dx2 * (double)r[k].y - di) * c[k];
-                T.d[(size_t)i * LP + l] = make_double2(dr, di);
-            }
-        }
-    }
-    // back substitution phi_i = d_i - c'_i phi_{i+1}, emitting the nodal-E spectrum of row i+1 as soon
-    // as phi_i is known
-    const double PI = 3.14159265358979323846;
-    const double theta = 2.0 * PI * (double)l / (double)T.ny;
-    const double c2 = cos(0.5 * theta) * cos(0.5 * theta), sn = sin(theta);
-    const double kx = -c2 * 0.5 * T.inv_dx * T.inv_ny;       // times (phi_{i+1} - phi_{i-1})
-    const double kyf = -sn * 0.25 * T.inv_dy * T.inv_ny;     // times i (phi_{i-1} + 2 phi_i + phi_{i+1})
-    double p2r = 0.0, p2i = 0.0;     // phi_{i+2}
-    double p1r = 0.0, p1i = 0.0;     // phi_{i+1}   (starts as phi_nx = 0)
-    for (int i1 = nx - 1; i1 >= 1; i1 -= B) {
-        double2 dd[B];
-        double c[B];
-#pragma unroll
-        for (int k = 0; k < B; k++) {
-            int i = max(i1 - k, 1);
-            dd[k] = T.d[(size_t)i * LP + l];
-            c[k] = T.cp[(size_t)i * LP + l];
-        }
-#pragma unroll
-        for (int k = 0; k < B; k++) {
-            int i = i1 - k;
-            if (i >= 1) {
-                double pr = dd[k].x - c[k] * p1r, pi = dd[k].y - c[k] * p1i;     // phi_i
-                // row i+1 now has both neighbours
-                int e = i + 1;
-                double ex_r, ex_i, ey_r, ey_i;
-                if (e == nx) {      // right wall: mean of the two cells at nx - 1/2
-                    ex_r = 2.0 * kx * (p1r - pr); ex_i = 2.0 * kx * (p1i - pi);
-                    ey_r = -2.0 * kyf * (pi + p1i); ey_i = 2.0 * kyf * (pr + p1r);
-                } else {
-                    ex_r = kx * (p2r - pr); ex_i = kx * (p2i - pi);
-                    double sr = pr + 2.0 * p1r + p2r, si = pi + 2.0 * p1i + p2i;
-                    ey_r = -kyf * si; ey_i = kyf * sr;                            // i * (sr + i si)
-                }
-                T.ehx[(size_t)e * LP + l] = make_float2((float)ex_r, (float)ex_i);
-                T.ehy[(size_t)e * LP + l] = make_float2((float)ey_r, (float)ey_i);
-                if (T.phi_hat) T.phi_hat[(size_t)i * LP + l] = make_float2((float)(pr * T.inv_ny), (float)(pi * T.inv_ny));
-                p2r = p1r; p2i = p1i;
-                p1r = pr; p1i = pi;
-            }
-        }
-    }
-    // rows 1 and 0: phi_0 = 0; p1 = phi_1, p2 = phi_2 (or phi_nx = 0 when nx == 2)
-    {
-        double ex_r = kx * (p2r - 0.0), ex_i = kx * (p2i - 0.0);
-        double sr = 0.0 + 2.0 * p1r + p2r, si = 0.0 + 2.0 * p1i + p2i;
-        T.ehx[(size_t)1 * LP + l] = make_float2((float)ex_r, (float)ex_i);
-        T.ehy[(size_t)1 * LP + l] = make_float2((float)(-kyf * si), (float)(kyf * sr));
-        // left wall: mean of the two cells at 1/2
-        T.ehx[l] = make_float2((float)(2.0 * kx * p1r), (float)(2.0 * kx * p1i));
-        T.ehy[l] = make_float2((float)(-2.0 * kyf * p1i), (float)(2.0 * kyf * p1r));
-        if (T.phi_hat) {
-            T.phi_hat[l] = make_float2(0.f, 0.f);
-            T.phi_hat[(size_t)nx * LP + l] = make_float2(0.f, 0.f);
-        }
-    }
+    float2 *r = fft_stockham<false>(buf, buf + ny, tw, ny);
+    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) rho_hat[(size_t)i * LP + l] = r[l];
 }
 
 // MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part)
 template <int MODE>
 __global__ void __launch_bounds__(FFT_THREADS) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
-                                                      float *__restrict__ phi, int ny, int log2n, int LP)
+                                                      float *__restrict__ phi, int ny, int LP)
 {
     extern __shared__ float2 buf[];
     const int i = blockIdx.x;
@@ -185,13 +112,13 @@ __global__ void __launch_bounds__(FFT_THREADS) k_ifft(const float2 *__restrict__
         float2 a = hx[(size_t)i * LP + l];
         float2 b = MODE == 0 ? hy[(size_t)i * LP + l] : make_float2(0.f, 0.f);
         // Z_l = a + i b ; Z_{ny-l} = conj(a) + i conj(b)
-        buf[__brev((unsigned)l) >> (32 - log2n)] = make_float2(a.x - b.y, a.y + b.x);
-        if (l > 0 && l < ny / 2) buf[__brev((unsigned)(ny - l)) >> (32 - log2n)] = make_float2(a.x + b.y, -a.y + b.x);
+        buf[l] = make_float2(a.x - b.y, a.y + b.x);
+        if (l > 0 && l < ny / 2) buf[ny - l] = make_float2(a.x + b.y, -a.y + b.x);
     }
-    fft_shared<true>(buf, tw, ny, log2n);
+    float2 *r = fft_stockham<true>(buf, buf + ny, tw, ny);
     for (int j = threadIdx.x; j < ny; j += blockDim.x) {
-        if (MODE == 0) Enode[(size_t)i * ny + j] = buf[j];
-        else phi[(size_t)i * ny + j] = buf[j].x;
+        if (MODE == 0) Enode[(size_t)i * ny + j] = r[j];
+        else phi[(size_t)i * ny + j] = r[j].x;
     }
 }
 
@@ -204,26 +131,224 @@ __global__ void k_twiddle_init(float2 *tw, int ny)
     tw[k] = make_float2((float)c, (float)s);
 }
 
-}  // namespace
+// ---- partitioned chasing method ---------------------------------------------------------------------
+// tables [cls][j][LP], cls 0 = full partition (m = M-1 interior rows), cls 1 = last partition (m_last)
+struct TriTables {
+    double *cp, *V, *W;     // local c', spikes V (1 at the left interface), W (1 at the right interface)
+};
 
-static int ilog2(int n)
+__global__ void k_tri_tables(TriTables T, int ny, int LP, int m_last, double dx, double Ly)
 {
-    int l = 0;
-    while ((1 << l) < n) l++;
-    return l;
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l > ny / 2) return;
+    const double PI = 3.14159265358979323846;
+    const double ky = 2.0 * PI * (double)l / Ly;
+    const double b = -2.0 - ky * ky * dx * dx;                   // Eq. 11 times dx^2
+    for (int cls = 0; cls < 2; cls++) {
+        const int m = cls == 0 ? M - 1 : m_last;
+        double *cp = T.cp + (size_t)cls * M * LP, *V = T.V + (size_t)cls * M * LP, *W = T.W + (size_t)cls * M * LP;
+        double c = 0.0;
+        for (int j = 1; j <= m; j++) {
+            c = 1.0 / (b - c);
+            cp[(size_t)j * LP + l] = c;
+        }
+        // V: local solve of A V = -e_1 ; W: A W = -e_m
+        double d = 0.0;
+        for (int j = 1; j <= m; j++) {
+            d = ((j == 1 ? -1.0 : 0.0) - d) * cp[(size_t)j * LP + l];
+            V[(size_t)j * LP + l] = d;                             // forward result, overwritten below
+        }
+        double v = 0.0;
+        for (int j = m; j >= 1; j--) {
+            v = V[(size_t)j * LP + l] - cp[(size_t)j * LP + l] * v;
+            V[(size_t)j * LP + l] = v;
+        }
+        double w = 0.0;
+        for (int j = m; j >= 1; j--) {
+            w = (j == m ? -cp[(size_t)j * LP + l] : 0.0) - cp[(size_t)j * LP + l] * w;
+            W[(size_t)j * LP + l] = w;
+        }
+    }
 }
+
+struct TriParams {
+    const float2 *rho_hat;
+    float2 *phi_hat;      // may alias rho_hat; NULL: not wanted
+    TriTables tab;
+    double2 *sumV, *sumW; // [P][LP]
+    double2 *g;           // [P+1][LP] interface values (g_0 = g_P = 0)
+    float2 *ehx, *ehy;
+    int nx, ny, LP, P, m_last;
+    double dx2, inv_dx, inv_dy, inv_ny, Ly;
+};
+
+// S_V = sum_j V_j r_j, S_W = sum_j W_j r_j over the interior rows of partition k (r = dx^2 rho^)
+__global__ void __launch_bounds__(128) k_tri_sums(const TriParams T)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+    if (l > T.ny / 2) return;
+    const int cls = (k == T.P - 1) ? 1 : 0, m = cls ? T.m_last : M - 1;
+    const double *V = T.tab.V + (size_t)cls * M * T.LP, *W = T.tab.W + (size_t)cls * M * T.LP;
+    double svr = 0.0, svi = 0.0, swr = 0.0, swi = 0.0;
+#pragma unroll 8
+    for (int j = 1; j <= m; j++) {
+        float2 r = T.rho_hat[(size_t)(k * M + j) * T.LP + l];
+        double v = V[(size_t)j * T.LP + l], w = W[(size_t)j * T.LP + l];
+        svr += v * (double)r.x; svi += v * (double)r.y;
+        swr += w * (double)r.x; swi += w * (double)r.y;
+    }
+    T.sumV[(size_t)k * T.LP + l] = make_double2(T.dx2 * svr, T.dx2 * svi);
+    T.sumW[(size_t)k * T.LP + l] = make_double2(T.dx2 * swr, T.dx2 * swi);
+}
+
+// reduced system for the interface values, one thread per k_y, chasing method in double
+__global__ void __launch_bounds__(32) k_tri_reduced(const TriParams T)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l > T.ny / 2) return;
+    const int LP = T.LP, P = T.P;
+    const double PI = 3.14159265358979323846;
+    const double ky = 2.0 * PI * (double)l / T.Ly;
+    const double b = -2.0 - ky * ky * T.dx2;
+    const double Vm = T.tab.V[(size_t)(M - 1) * LP + l], Wm = T.tab.W[(size_t)(M - 1) * LP + l];
+    const double V1 = T.tab.V[(size_t)1 * LP + l], W1 = T.tab.W[(size_t)1 * LP + l];
+    const double V1_last = T.m_last >= 1 ? T.tab.V[((size_t)M + 1) * LP + l] : 0.0;
+    T.g[l] = make_double2(0.0, 0.0);
+    T.g[(size_t)P * LP + l] = make_double2(0.0, 0.0);
+    if (P < 2) return;
+    // forward: row k: Vm g_{k-1} + (Wm + b + V1(k)) g_k + W1 g_{k+1} = r_{kM} + S_W(k-1) + S_V(k)
+    double cprev = 0.0, dr = 0.0, di = 0.0;
+    double2 *cd = T.g;                       // store d_k in g[k] and c'_k in sumV[k].x (free after read)
+    for (int k = 1; k <= P - 1; k++) {
+        float2 r = T.rho_hat[(size_t)(k * M) * LP + l];
+        double2 sw = T.sumW[(size_t)(k - 1) * LP + l], sv = T.sumV[(size_t)k * LP + l];
+        double diag = Wm + b + (k == P - 1 ? V1_last : V1);
+        double den = 1.0 / (diag - Vm * cprev);
+        double Rr = T.dx2 * (double)r.x + sw.x + sv.x, Ri = T.dx2 * (double)r.y + sw.y + sv.y;
+        dr = (Rr - Vm * dr) * den;
+        di = (Ri - Vm * di) * den;
+        cprev = W1 * den;
+        cd[(size_t)k * LP + l] = make_double2(dr, di);
+        T.sumV[(size_t)k * LP + l].x = cprev;
+    }
+    double gr = 0.0, gi = 0.0;
+    for (int k = P - 1; k >= 1; k--) {
+        double2 d = cd[(size_t)k * LP + l];
+        double c = T.sumV[(size_t)k * LP + l].x;
+        gr = d.x - c * gr;
+        gi = d.y - c * gi;
+        cd[(size_t)k * LP + l] = make_double2(gr, gi);
+    }
+}
+
+// one thread per (k_y, partition): local chasing solve in registers with the true interface values,
+// then the nodal-E spectra of rows kM .. kM+m (plus the wall row nx for the last partition)
+__global__ void __launch_bounds__(128) k_tri_local(const TriParams T)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+    if (l > T.ny / 2) return;
+    const int LP = T.LP;
+    const int cls = (k == T.P - 1) ? 1 : 0, m = cls ? T.m_last : M - 1;
+    const double *cp = T.tab.cp + (size_t)cls * M * LP;
+    const size_t row0 = (size_t)k * M;
+    const double2 gl = T.g[(size_t)k * LP + l], gr = T.g[(size_t)(k + 1) * LP + l];
+    double dr[M], di[M];
+    // forward elimination with the interface values folded into rows 1 and m
+    {
+        double pr = 0.0, pi = 0.0;
+#pragma unroll
+        for (int j = 1; j < M; j++) {
+            if (j <= m) {
+                float2 r = T.rho_hat[(row0 + j) * LP + l];
+                double c = cp[(size_t)j * LP + l];
+                double rr = T.dx2 * (double)r.x, ri = T.dx2 * (double)r.y;
+                if (j == 1) { rr -= gl.x; ri -= gl.y; }
+                if (j == m) { rr -= gr.x; ri -= gr.y; }
+                pr = (rr - pr) * c;
+                pi = (ri - pi) * c;
+            }
+            dr[j] = pr; di[j] = pi;
+        }
+    }
+    const double PI = 3.14159265358979323846;
+    const double theta = 2.0 * PI * (double)l / (double)T.ny;
+    const double ch = cos(0.5 * theta), sn = sin(theta);
+    const double kx = -ch * ch * 0.5 * T.inv_dx * T.inv_ny;     // times (phi_{e+1} - phi_{e-1})
+    const double kyf = -sn * 0.25 * T.inv_dy * T.inv_ny;        // times i (phi_{e-1} + 2 phi_e + phi_{e+1})
+    // back substitution from row m down to 1; p1 = phi_{j+1}, p2 = phi_{j+2}
+    double p2r = 0.0, p2i = 0.0, p1r = gr.x, p1i = gr.y;
+    const bool right_wall = (k == T.P - 1);    // then gr = g_P = 0 = phi_nx
+#pragma unroll
+    for (int j = M - 1; j >= 1; j--) {
+        if (j <= m) {
+            double c = cp[(size_t)j * LP + l];
+            // phi_j; the right boundary value is already folded into d_m
+            double pr = dr[j] - (j == m ? 0.0 : c * p1r), pi = di[j] - (j == m ? 0.0 : c * p1i);
+            const size_t e = row0 + j + 1;                           // row j+1 now has both neighbours
+            if (j == m) {
+                if (right_wall) {    // e == nx: mean of the two cells at nx - 1/2
+                    T.ehx[e * LP + l] = make_float2((float)(-2.0 * kx * pr), (float)(-2.0 * kx * pi));
+                    T.ehy[e * LP + l] = make_float2((float)(-2.0 * kyf * pi), (float)(2.0 * kyf * pr));
+                }   // else: row e is the next partition's interface row, emitted there
+            } else {
+                double sr = pr + 2.0 * p1r + p2r, si = pi + 2.0 * p1i + p2i;
+                T.ehx[e * LP + l] = make_float2((float)(kx * (p2r - pr)), (float)(kx * (p2i - pi)));
+                T.ehy[e * LP + l] = make_float2((float)(-kyf * si), (float)(kyf * sr));
+            }
+            if (T.phi_hat) T.phi_hat[(row0 + j) * LP + l] = make_float2((float)(pr * T.inv_ny), (float)(pi * T.inv_ny));
+            p2r = p1r; p2i = p1i;
+            p1r = pr; p1i = pi;
+        }
+    }
+    // now p1 = phi_1 and p2 = phi_2 (or the right boundary value); m == 0: p1 = right boundary value
+    if (m >= 1) {        // row kM+1: left neighbour is the interface value
+        double sr = gl.x + 2.0 * p1r + p2r, si = gl.y + 2.0 * p1i + p2i;
+        const size_t e = row0 + 1;
+        T.ehx[e * LP + l] = make_float2((float)(kx * (p2r - gl.x)), (float)(kx * (p2i - gl.y)));
+        T.ehy[e * LP + l] = make_float2((float)(-kyf * si), (float)(kyf * sr));
+    } else if (right_wall) {   // empty last partition: the wall row nx is this interface's right neighbour
+        const size_t e = row0 + 1;
+        T.ehx[e * LP + l] = make_float2((float)(-2.0 * kx * gl.x), (float)(-2.0 * kx * gl.y));
+        T.ehy[e * LP + l] = make_float2((float)(-2.0 * kyf * gl.y), (float)(2.0 * kyf * gl.x));
+    }
+    // interface row kM itself
+    if (k == 0) {        // left wall: mean of the two cells at 1/2, phi_0 = 0
+        T.ehx[l] = make_float2((float)(2.0 * kx * p1r), (float)(2.0 * kx * p1i));
+        T.ehy[l] = make_float2((float)(-2.0 * kyf * p1i), (float)(2.0 * kyf * p1r));
+        if (T.phi_hat) {
+            T.phi_hat[l] = make_float2(0.f, 0.f);
+            T.phi_hat[(size_t)T.nx * LP + l] = make_float2(0.f, 0.f);
+        }
+    } else {
+        // phi_{kM-1} from the interface equation: phi_{kM-1} + b g_k + phi_{kM+1} = dx^2 rho^_{kM}
+        const double kyc = 2.0 * PI * (double)l / T.Ly;
+        const double b = -2.0 - kyc * kyc * T.dx2;
+        float2 r = T.rho_hat[row0 * LP + l];
+        double lr = T.dx2 * (double)r.x - b * gl.x - p1r, li = T.dx2 * (double)r.y - b * gl.y - p1i;
+        double sr = lr + 2.0 * gl.x + p1r, si = li + 2.0 * gl.y + p1i;
+        T.ehx[row0 * LP + l] = make_float2((float)(kx * (p1r - lr)), (float)(kx * (p1i - li)));
+        T.ehy[row0 * LP + l] = make_float2((float)(-kyf * si), (float)(kyf * sr));
+        if (T.phi_hat) T.phi_hat[row0 * LP + l] = make_float2((float)(gl.x * T.inv_ny), (float)(gl.y * T.inv_ny));
+    }
+}
+
+}  // namespace
 
 int launch_poisson_init(pm2d_ctx *c)
 {
-    const int ny = c->g.ny;
+    const int ny = c->g.ny, nx = c->g.nx;
+    c->tri_P = (nx + M - 1) / M;
+    c->tri_mlast = nx - (c->tri_P - 1) * M - 1;
     k_twiddle_init<<<(ny / 2 + 127) / 128, 128, 0, c->stream>>>(c->twiddle, ny);
-    k_cp_init<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(c->cp, c->g.nx, ny, c->LP, c->g.dx, ny * c->g.dy);
+    TriTables T{c->tri_cp, c->tri_V, c->tri_W};
+    k_tri_tables<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T, ny, c->LP, c->tri_mlast, c->g.dx, ny * c->g.dy);
     count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
-    if (ny * sizeof(float2) > 48 * 1024) {
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ny * sizeof(float2))));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ny * sizeof(float2))));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ny * sizeof(float2))));
+    const int smem = 2 * ny * (int)sizeof(float2);
+    if (smem > 48 * 1024) {
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     }
     return PM2D_OK;
 }
@@ -231,8 +356,8 @@ int launch_poisson_init(pm2d_ctx *c)
 // rho from the current density grids -> nodal E (and phi if wanted, for diagnostics)
 int launch_poisson(pm2d_ctx *c, bool want_phi)
 {
-    const int nx = c->g.nx, ny = c->g.ny, log2n = ilog2(ny);
-    const size_t smem = ny * sizeof(float2);
+    const int nx = c->g.nx, ny = c->g.ny;
+    const size_t smem = 2 * ny * sizeof(float2);
     RhoSrc S;
     S.count = 0;
     S.inv_nscale = c->inv_nscale;
@@ -242,16 +367,21 @@ int launch_poisson(pm2d_ctx *c, bool want_phi)
             S.sign[S.count] = c->sp[s].cfg.sign;
             S.count++;
         }
-    if (nx >= 2) k_fft_rho<<<nx - 1, FFT_THREADS, smem, c->stream>>>(S, c->twiddle, c->rho_hat, ny, log2n, c->LP);
+    k_fft_rho<<<nx - 1, FFT_THREADS, smem, c->stream>>>(S, c->twiddle, c->rho_hat, ny, c->LP);
     TriParams T;
-    T.rho_hat = c->rho_hat; T.phi_hat = want_phi ? c->rho_hat : nullptr; T.cp = c->cp; T.d = c->dtmp;
-    T.ehx = c->ehx; T.ehy = c->ehy; T.nx = nx; T.ny = ny; T.LP = c->LP;
-    T.dx2 = c->g.dx * c->g.dx; T.inv_dx = 1.0 / c->g.dx; T.inv_dy = 1.0 / c->g.dy; T.inv_ny = 1.0 / ny;
-    k_tridiag<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
-    k_ifft<0><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, log2n, c->LP);
-    count_launch(c, 3);
+    T.rho_hat = c->rho_hat; T.phi_hat = want_phi ? c->rho_hat : nullptr;
+    T.tab = TriTables{c->tri_cp, c->tri_V, c->tri_W};
+    T.sumV = c->tri_sumV; T.sumW = c->tri_sumW; T.g = c->tri_g;
+    T.ehx = c->ehx; T.ehy = c->ehy; T.nx = nx; T.ny = ny; T.LP = c->LP; T.P = c->tri_P; T.m_last = c->tri_mlast;
+    T.dx2 = c->g.dx * c->g.dx; T.inv_dx = 1.0 / c->g.dx; T.inv_dy = 1.0 / c->g.dy; T.inv_ny = 1.0 / ny; T.Ly = ny * c->g.dy;
+    dim3 grid((ny / 2 + 1 + 127) / 128, c->tri_P);
+    k_tri_sums<<<grid, 128, 0, c->stream>>>(T);
+    k_tri_reduced<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
+    k_tri_local<<<grid, 128, 0, c->stream>>>(T);
+    k_ifft<0><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP);
+    count_launch(c, 5);
     if (want_phi) {
-        k_ifft<1><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, log2n, c->LP);
+        k_ifft<1><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP);
         count_launch(c);
     }
     PM2D_CUDA_CHECK(cudaGetLastError());

@@ -259,3 +259,30 @@ def test_energy_history_parity_c1(P):
     assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
     assert rel_l2(sim.get_fields(P.FIELD_A), orc.a_now[0]) < 1e-4
     sim.close()
+
+
+@pytest.mark.parametrize("nx", [24, 33, 65, 100])
+def test_poisson_partition_edge_cases(P, nx):
+    """x-partitioned chasing method: single partition, empty last partition (nx = 1 mod 32), ragged last one."""
+    ny = 16
+    cfg = small_cfg("c3", nx, ny)
+    sim = P.PM2D(cfg, eager_moments=1)
+    orc, _ = oracle_from_config(cfg)
+    for _ in range(2):
+        orc.refresh_fields()
+        assert rel_l2(sim.get_fields(P.FIELD_PHI), orc.phi.reshape(nx + 1, ny)) < 1e-5
+        # E on the nodes (Q3): mean of the adjacent cell-centred values of the oracle
+        Ex, Ey = orc.Ex.reshape(nx, ny), orc.Ey.reshape(nx, ny)
+        def to_nodes(E):
+            Ec = 0.5 * (E + np.roll(E, 1, axis=1))
+            out = np.empty((nx + 1, ny))
+            out[1:nx] = 0.5 * (Ec[:-1] + Ec[1:])
+            out[0], out[nx] = Ec[0], Ec[-1]
+            return out
+        for comp, E in ((0, Ex), (1, Ey)):
+            ref = to_nodes(E)
+            got = sim.get_fields(P.FIELD_ENODE, comp)
+            assert np.abs(got - ref).max() < 1e-5 * np.abs(np.concatenate([Ex, Ey])).max(), (nx, comp)
+        sim.step(1)
+        orc.step(1)
+    sim.close()
