@@ -57,7 +57,7 @@ enum {
     PM2D_FIELD_A = 0,      /* vector potential component `comp`, time level `level` (0 = n, 1 = n-1) */
     PM2D_FIELD_PHI = 1,    /* electrostatic potential on nodes (Eq. 3), recomputed from the current densities */
     PM2D_FIELD_ENODE = 2,  /* E averaged to nodes (Q3), comp 0 = x, 1 = y, from the current densities */
-    PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16), comp 0 = x, 1 = y, as last computed */
+    PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16) for the current E, a^n, n^n; comp 0 = x, 1 = y */
 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 

@@ -288,6 +288,14 @@ class Oracle:
     def refresh_fields(self):
         lib().orc_refresh_fields(C.byref(self.st))
 
+    def force_now(self, s):
+        """Eq. 16 for the current state: E of the current densities, a^n, n^n  -> (Fx, Fy)."""
+        self.refresh_fields()
+        Fx, Fy = np.zeros(self.nn), np.zeros(self.nn)
+        lib().orc_force(C.byref(self.g), C.byref(self._sp[s]), self.st.a_now, _p(self.Ex), _p(self.Ey), _p(Fx), _p(Fy))
+        sh = (self.g.nx + 1, self.g.ny)
+        return Fx.reshape(sh), Fy.reshape(sh)
+
     def energies(self):
         self.refresh_fields()
         out = np.zeros(3 + 2 * len(self.sp))

@@ -104,12 +104,17 @@ size_t layout(pm2d_ctx *c, char *base)
     c->twiddle = cv.take<float2>(g.ny / 2);
     c->red = cv.take<double>(64);
     c->flags = cv.take<int32_t>(4);
+    c->ovf_cap = 1 << 20;
+    c->ovf_p = cv.take<int64_t>(c->ovf_cap);
+    c->ovf_tile = cv.take<int32_t>(c->ovf_cap);
+    c->ovf_count = cv.take<int32_t>(4);
     for (int s = 0; s < c->nsp; s++) {
         SpeciesDev &S = c->sp[s];
         S.nfix = cv.take<int32_t>(nn);
         S.pxfix = S.pyfix = nullptr; S.F = nullptr;
         S.np = S.cap = species_np(g, S.cfg);
         if (!S.cfg.mobile) continue;
+        S.nfix2 = cv.take<int32_t>(nn);
         S.pxfix = cv.take<int32_t>(nn);
         S.pyfix = cv.take<int32_t>(nn);
         S.F = cv.take<float2>(nn);
@@ -163,6 +168,7 @@ int check_flags(pm2d_ctx *c)
     PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     if (h[0]) return fail(PM2D_ESTATE, "a particle moved further than one tile between rebins (rebin_every too large)");
     if (h[1]) return fail(PM2D_ESTATE, "chunk table overflow");
+    if (h[2]) return fail(PM2D_ESTATE, "too many particles outside their tile window (rebin_every too large)");
     return PM2D_OK;
 }
 
@@ -328,7 +334,6 @@ extern "C" int pm2d_set_lasers(pm2d_ctx *c, const pm2d_laser *lasers, int nlaser
 static int enqueue_step(pm2d_ctx *c)
 {
     int rc;
-    const bool eager = c->g.eager_moments != 0;
     // (2) a^{n+1} from a^n, a^{n-1}, n_e^n ; E^n from n_i^n - n_e^n
     phase_begin(c, PM2D_PH_FIELD);
     if ((rc = launch_field_step(c))) return rc;
@@ -337,18 +342,11 @@ static int enqueue_step(pm2d_ctx *c)
         phase_begin(c, PM2D_PH_POISSON);
         if ((rc = launch_poisson(c, false))) return rc;
         phase_end(c);
-        // (3)/(7) force grid with a^n (stage A) or a^{n+1} (stage B)
-        phase_begin(c, PM2D_PH_FORCE);
-        for (int s = 0; s < c->nsp; s++)
-            if (c->sp[s].cfg.mobile && (rc = launch_force(c, s, stage == 0 ? c->a[1] : c->a[0]))) return rc;
-        phase_end(c);
-        // (3)-(5) gather, predictor, deposit / (7)-(8)+(1) gather, corrector, deposit
+        // (3)-(5) force of Eq. 16 with a^n built per tile, gather, predictor, deposit /
+        // (7)-(8)+(1) force of Eq. 18 with a^{n+1}, gather, corrector, deposit -- one fused kernel
         phase_begin(c, stage == 0 ? PM2D_PH_STAGE_A : PM2D_PH_STAGE_B);
-        for (int s = 0; s < c->nsp; s++) {
-            if (!c->sp[s].cfg.mobile) continue;
-            if ((rc = zero_moments(c, s, true, eager))) return rc;
-            if ((rc = launch_stage(c, s, stage))) return rc;
-        }
+        for (int s = 0; s < c->nsp; s++)
+            if (c->sp[s].cfg.mobile && (rc = launch_stage(c, s, stage))) return rc;
         phase_end(c);
     }
     float *t = c->a[2];
@@ -452,6 +450,10 @@ extern "C" int64_t pm2d_get_fields(pm2d_ctx *c, int field, int comp, int level, 
         return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
     case PM2D_FIELD_FORCE:
         if (comp < 0 || comp > 1 || level < 0 || level >= c->nsp || !c->sp[level].cfg.mobile) return fail(PM2D_EINVAL, "bad comp/species");
+        // Eq. 16 for the current state: E of the current densities, a^n, n^n (diagnostic grid;
+        // the step itself builds the force per tile inside the fused particle kernel)
+        if ((rc = launch_poisson(c, false))) return rc;
+        if ((rc = launch_force(c, level, c->a[1]))) return rc;
         k_extract_comp<<<blocks, 256, 0, c->stream>>>(c->sp[level].F, comp, c->phi, (size_t)c->nn);
         count_launch(c);
         return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);

@@ -28,9 +28,18 @@ struct PartParams {
     const int64_t *tile_off;
     const int32_t *nchunks;
     // grids
-    const float2 *F;
+    const float2 *F;          // materialised force grid (slow path / diagnostics); may be NULL
+    const float2 *Enode;      // nodal E of the last Poisson solve
+    const float *a;           // [ncomp][nn], level n (stage A) or n+1 (stage B)
+    int ncomp;
+    float qE, pond, cv2;      // -sign 4 pi^2 / m ; 1 for electrons ; C v_th^2
+    float inv_2dx, inv_2dy;
+    const int32_t *nfix_in;   // density the force is built from (n^n or n^); the deposit goes to nfix
     int32_t *nfix, *pxfix, *pyfix;
     int32_t *flags;
+    int64_t *ovf_p;           // overflow list: particles whose gather footprint left the tile window
+    int32_t *ovf_tile, *ovf_count;
+    int ovf_cap;
     int nx, ny, nty;
     float dt, hx, hy;        // hx = dt / (2 dx): cells per unit (u' + u)
     float nscale, pscale;
@@ -42,6 +51,7 @@ __device__ __forceinline__ int fold_x(int i, int nx)
 {
     if (i < 0) i = -i;
     if (i > nx) i = 2 * nx - i;
+    if (i < 0) i = 0;          // rows more than nx beyond a wall (tiny boxes) are never touched by a particle
     return i;
 }
 
@@ -134,15 +144,49 @@ __device__ __noinline__ void deposit_global(const PartParams &P, int gx0, int gy
     }
 }
 
+// Eq. 16 at one global node (slow path only)
+__device__ __forceinline__ float2 force_at_node(const PartParams &P, int gi, int gj)
+{
+    const size_t nn = (size_t)(P.nx + 1) * P.ny;
+    const int il = gi > 0 ? gi - 1 : 0, ih = gi < P.nx ? gi + 1 : P.nx;
+    const float sx = (il == gi || ih == gi) ? 2.f * P.inv_2dx : P.inv_2dx;
+    const int jm = (gj - 1) & (P.ny - 1), jp = (gj + 1) & (P.ny - 1);
+    const size_t k = (size_t)gi * P.ny + gj, kl = (size_t)il * P.ny + gj, kh = (size_t)ih * P.ny + gj;
+    const size_t kd = (size_t)gi * P.ny + jm, ku = (size_t)gi * P.ny + jp;
+    float2 E = P.Enode[k];
+    float fx = P.qE * E.x, fy = P.qE * E.y;
+    if (P.pond != 0.f) {
+        float ah = 0.f, al = 0.f, au = 0.f, ad = 0.f;
+        for (int c = 0; c < P.ncomp; c++) {
+            float v;
+            v = P.a[c * nn + kh]; ah += v * v;
+            v = P.a[c * nn + kl]; al += v * v;
+            v = P.a[c * nn + ku]; au += v * v;
+            v = P.a[c * nn + kd]; ad += v * v;
+        }
+        fx -= 0.5f * sx * (ah - al);
+        fy -= 0.5f * P.inv_2dy * (au - ad);
+    }
+    const int n0 = P.nfix_in[k];
+    if (n0 > 0 && P.cv2 != 0.f) {
+        const float inv_n = 1.f / (float)n0;
+        fx -= P.cv2 * sx * (float)(P.nfix_in[kh] - P.nfix_in[kl]) * inv_n;
+        fy -= P.cv2 * P.inv_2dy * (float)(P.nfix_in[ku] - P.nfix_in[kd]) * inv_n;
+    }
+    return make_float2(fx, fy);
+}
+
 __device__ __noinline__ float2 gather_global(const PartParams &P, int gx0, int gy0, int cx, int cy, const float Wx[3],
                                              const float Wy[3])
 {
     float fx = 0.f, fy = 0.f;
+#pragma unroll 1
     for (int a = 0; a < 3; a++) {
         int gi = fold_x(gx0 + cx - 1 + a, P.nx);
+#pragma unroll 1
         for (int b = 0; b < 3; b++) {
             int gj = (gy0 + cy - 1 + b) & (P.ny - 1);
-            float2 f = P.F[(size_t)gi * P.ny + gj];
+            float2 f = force_at_node(P, gi, gj);
             float ww = Wx[a] * Wy[b];
             fx += ww * f.x;
             fy += ww * f.y;
@@ -175,13 +219,142 @@ __device__ __forceinline__ float2 gather_window(const float2 *Fs, int cx, int cy
     return make_float2(fx, fy);
 }
 
-// STAGE 0: predictor (Eq. 17); STAGE 1: corrector (Eq. 19) + particle boundaries; STAGE 2: deposit only.
-// QMASK bit 0: density, bit 1: momentum.
+
+// Eq. 16 / 18 evaluated for the nodes of the tile window, straight into shared memory:
+//   F = qE E_node - (1/2) grad(sum_c a_c^2) [electrons] - C v_th^2 grad(n)/n
+// central differences, one-sided on the wall rows, pressure term 0 where n = 0 (Q10).  Window rows
+// beyond a wall hold F of the mirror node (Q9: the gather folds indices), whose x-difference runs
+// the other way in window coordinates.  a2s / ns: scratch of (WIN+2)^2 values (window + 1 ring).
+constexpr int WF = WIN + 2;
+__device__ __forceinline__ void build_force_window(const PartParams &P, int gx0, int gy0, float *a2s, int32_t *ns, float2 *Fs)
+{
+    const size_t nn = (size_t)(P.nx + 1) * P.ny;
+#pragma unroll 2
+    for (int e = threadIdx.x; e < WF * WF; e += PTHREADS) {
+        int r = e / WF, cidx = e - r * WF;
+        int gi = fold_x(gx0 + r - HALO - 1, P.nx);
+        int gj = (gy0 + cidx - HALO - 1) & (P.ny - 1);
+        size_t k = (size_t)gi * P.ny + gj;
+        float s2 = 0.f;
+        if (P.pond != 0.f)
+            for (int c = 0; c < P.ncomp; c++) {
+                float v = P.a[c * nn + k];
+                s2 += v * v;
+            }
+        a2s[e] = s2;
+        ns[e] = P.nfix_in[k];
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int e = threadIdx.x; e < WIN * WIN; e += PTHREADS) {
+        int r = e / WIN, cidx = e - r * WIN;
+        int raw = gx0 + r - HALO;
+        int gi = fold_x(raw, P.nx);
+        int gj = (gy0 + cidx - HALO) & (P.ny - 1);
+        const int c0 = (r + 1) * WF + (cidx + 1);
+        // x-difference in window coordinates -> difference at the (possibly mirrored) node
+        int lo = c0 - WF, hi = c0 + WF;
+        float sx = P.inv_2dx;
+        if (raw < 0 || raw > P.nx) sx = -sx;
+        if (gi == 0) { lo = c0; hi = (raw == 0) ? c0 + WF : c0 - WF; sx = 2.f * P.inv_2dx; }
+        else if (gi == P.nx) { hi = c0; lo = (raw == P.nx) ? c0 - WF : c0 + WF; sx = 2.f * P.inv_2dx; }
+        float2 E = P.Enode[(size_t)gi * P.ny + gj];
+        float fx = P.qE * E.x, fy = P.qE * E.y;
+        if (P.pond != 0.f) {
+            fx -= 0.5f * sx * (a2s[hi] - a2s[lo]);
+            fy -= 0.5f * P.inv_2dy * (a2s[c0 + 1] - a2s[c0 - 1]);
+        }
+        const int n0 = ns[c0];
+        if (n0 > 0 && P.cv2 != 0.f) {
+            const float inv_n = 1.f / (float)n0;
+            fx -= P.cv2 * sx * (float)(ns[hi] - ns[lo]) * inv_n;
+            fy -= P.cv2 * P.inv_2dy * (float)(ns[c0 + 1] - ns[c0 - 1]) * inv_n;
+        }
+        Fs[r * WPITCH + cidx] = make_float2(fx, fy);
+    }
+    __syncthreads();
+}
+
+// One particle through one stage.  STAGE 0: predictor (Eq. 17); STAGE 1: corrector (Eq. 19) + particle
+// boundaries; STAGE 2: deposit only.  QMASK bit 0: density, bit 1: momentum.
+// WINDOWED: gather from / deposit into the CTA's shared windows; returns false (nothing done) when the
+// gather footprint lies outside the window -- the caller defers the particle to k_stage_overflow, which
+// runs the same code with WINDOWED = false straight on the global grids.
+template <int SHAPE, int STAGE, int QMASK, bool WINDOWED>
+__device__ __forceinline__ bool process_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+{
+    uint32_t xf = P.x[p], yf = P.y[p];
+    float ux = P.ux[p], uy = P.uy[p];
+    float Wx[3], Wy[3];
+    int cx, cy;
+    float dx_, dy_;
+    if (STAGE == 0) {
+        decode(xf, cx, dx_);
+        decode(yf, cy, dy_);
+        if (WINDOWED && !in_window(cx, cy)) return false;
+        weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
+        weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
+        float2 f = WINDOWED ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
+        float uhx = __fmaf_rn(P.dt, f.x, ux), uhy = __fmaf_rn(P.dt, f.y, uy);     // Eq. 17
+        P.uhx[p] = uhx;
+        P.uhy[p] = uhy;
+        xf = advance(xf, P.hx, __fadd_rn(uhx, ux));
+        yf = advance(yf, P.hy, __fadd_rn(uhy, uy));
+        ux = uhx;
+        uy = uhy;
+    } else if (STAGE == 1) {
+        const float uhx = P.uhx[p], uhy = P.uhy[p];
+        uint32_t xh = advance(xf, P.hx, __fadd_rn(uhx, ux));                      // x^ of Eq. 17 again
+        uint32_t yh = advance(yf, P.hy, __fadd_rn(uhy, uy));
+        decode(xh, cx, dx_);
+        decode(yh, cy, dy_);
+        if (WINDOWED && !in_window(cx, cy)) return false;
+        weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
+        weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
+        float2 f = WINDOWED ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
+        float unx = __fmaf_rn(0.5f * P.dt, f.x, 0.5f * __fadd_rn(uhx, ux));       // Eq. 19
+        float uny = __fmaf_rn(0.5f * P.dt, f.y, 0.5f * __fadd_rn(uhy, uy));
+        xf = advance(xf, P.hx, __fadd_rn(unx, ux));
+        yf = advance(yf, P.hy, __fadd_rn(uny, uy));
+        // x walls reflect (Q9); y is periodic and needs nothing until the rebin
+        int64_t gx = (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS) + (int64_t)xf;
+        const int64_t wall = (int64_t)P.nx << POS_FRAC_BITS;
+        if (gx < 0) {
+            gx = -gx;
+            unx = -unx;
+        } else if (gx >= wall) {
+            gx = 2 * wall - gx;
+            if (gx >= wall) gx = wall - 1;
+            unx = -unx;
+        }
+        xf = (uint32_t)(gx - (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS));
+        P.x[p] = xf;
+        P.y[p] = yf;
+        P.ux[p] = unx;
+        P.uy[p] = uny;
+        ux = unx;
+        uy = uny;
+    }
+    decode(xf, cx, dx_);
+    decode(yf, cy, dy_);
+    weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
+    weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
+    const float w = P.w[p];
+    const float qn = w * P.nscale, qx = w * ux * P.pscale, qy = w * uy * P.pscale;
+    if (WINDOWED && in_window(cx, cy))
+        deposit_window<QMASK>(dep, cx, cy, Wx, Wy, qn, qx, qy, SHAPE == PM2D_CIC);
+    else
+        deposit_global<QMASK>(P, gx0, gy0, cx, cy, Wx, Wy, qn, qx, qy);
+    return true;
+}
+
 template <int SHAPE, int STAGE, int QMASK>
-__global__ void __launch_bounds__(PTHREADS) k_stage(const PartParams P)
+__global__ void __launch_bounds__(PTHREADS, 4) k_stage(const PartParams P)
 {
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
-    __shared__ int32_t dep[NQ * WIN * WPITCH];
+    // dep doubles as the scratch of build_force_window (2 (WIN+2)^2 words) before it is zeroed
+    constexpr int DEPW = (STAGE < 2 && NQ * WIN * WPITCH < 2 * WF * WF) ? 2 * WF * WF : NQ * WIN * WPITCH;
+    __shared__ int32_t dep[DEPW];
     __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
     const int chunk = blockIdx.x;
     if (chunk >= *P.nchunks) return;
@@ -194,78 +367,20 @@ __global__ void __launch_bounds__(PTHREADS) k_stage(const PartParams P)
     }
     const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
 
+    if (STAGE < 2) build_force_window(P, gx0, gy0, reinterpret_cast<float *>(dep), dep + WF * WF, Fs);
     for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += PTHREADS) dep[e] = 0;
-    if (STAGE < 2) {
-        for (int e = threadIdx.x; e < WIN * WIN; e += PTHREADS) {
-            int r = e / WIN, cidx = e - r * WIN;
-            int gi = fold_x(gx0 + r - HALO, P.nx);
-            int gj = (gy0 + cidx - HALO) & (P.ny - 1);
-            Fs[r * WPITCH + cidx] = P.F[(size_t)gi * P.ny + gj];
-        }
-    }
     __syncthreads();
 
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
-        uint32_t xf = P.x[p], yf = P.y[p];
-        float ux = P.ux[p], uy = P.uy[p];
-        const float w = P.w[p];
-        float Wx[3], Wy[3];
-        int cx, cy;
-        float dx_, dy_;
-        if (STAGE == 0) {
-            decode(xf, cx, dx_);
-            decode(yf, cy, dy_);
-            weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-            weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-            float2 f = in_window(cx, cy) ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
-            float uhx = __fmaf_rn(P.dt, f.x, ux), uhy = __fmaf_rn(P.dt, f.y, uy);     // Eq. 17
-            P.uhx[p] = uhx;
-            P.uhy[p] = uhy;
-            xf = advance(xf, P.hx, __fadd_rn(uhx, ux));
-            yf = advance(yf, P.hy, __fadd_rn(uhy, uy));
-            ux = uhx;
-            uy = uhy;
-        } else if (STAGE == 1) {
-            const float uhx = P.uhx[p], uhy = P.uhy[p];
-            uint32_t xh = advance(xf, P.hx, __fadd_rn(uhx, ux));                      // x^ of Eq. 17 again
-            uint32_t yh = advance(yf, P.hy, __fadd_rn(uhy, uy));
-            decode(xh, cx, dx_);
-            decode(yh, cy, dy_);
-            weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-            weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-            float2 f = in_window(cx, cy) ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
-            float unx = __fmaf_rn(0.5f * P.dt, f.x, 0.5f * __fadd_rn(uhx, ux));       // Eq. 19
-            float uny = __fmaf_rn(0.5f * P.dt, f.y, 0.5f * __fadd_rn(uhy, uy));
-            xf = advance(xf, P.hx, __fadd_rn(unx, ux));
-            yf = advance(yf, P.hy, __fadd_rn(uny, uy));
-            // x walls reflect (Q9); y is periodic and needs nothing until the rebin
-            int64_t gx = (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS) + (int64_t)xf;
-            const int64_t wall = (int64_t)P.nx << POS_FRAC_BITS;
-            if (gx < 0) {
-                gx = -gx;
-                unx = -unx;
-            } else if (gx >= wall) {
-                gx = 2 * wall - gx;
-                if (gx >= wall) gx = wall - 1;
-                unx = -unx;
-            }
-            xf = (uint32_t)(gx - (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS));
-            P.x[p] = xf;
-            P.y[p] = yf;
-            P.ux[p] = unx;
-            P.uy[p] = uny;
-            ux = unx;
-            uy = uny;
+        if (!process_particle<SHAPE, STAGE, QMASK, true>(P, p, gx0, gy0, Fs, dep)) {
+            // drifted more than HALO - 1/2 cells out of its tile since the last rebin: rare; deferred
+            int slot = atomicAdd(P.ovf_count, 1);
+            if (slot < P.ovf_cap) {
+                P.ovf_p[slot] = p;
+                P.ovf_tile[slot] = tile;
+            } else
+                P.flags[2] = 1;
         }
-        decode(xf, cx, dx_);
-        decode(yf, cy, dy_);
-        weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-        weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-        const float qn = w * P.nscale, qx = w * ux * P.pscale, qy = w * uy * P.pscale;
-        if (in_window(cx, cy))
-            deposit_window<QMASK>(dep, cx, cy, Wx, Wy, qn, qx, qy, SHAPE == PM2D_CIC);
-        else
-            deposit_global<QMASK>(P, gx0, gy0, cx, cy, Wx, Wy, qn, qx, qy);
     }
     __syncthreads();
 
@@ -283,10 +398,21 @@ __global__ void __launch_bounds__(PTHREADS) k_stage(const PartParams P)
             if (v) atomicAdd(&P.nfix[k], fac * v);
         }
         if (QMASK & 2) {
-            int vx = dep[((QMASK & 1) ? 1 : 1) * WIN * WPITCH + se], vy = dep[2 * WIN * WPITCH + se];
+            int vx = dep[WIN * WPITCH + se], vy = dep[2 * WIN * WPITCH + se];
             if (vx) atomicAdd(&P.pxfix[k], fac * vx);
             if (vy) atomicAdd(&P.pyfix[k], fac * vy);
         }
+    }
+}
+
+// the deferred particles of k_stage: same arithmetic, global grids only
+template <int SHAPE, int STAGE, int QMASK>
+__global__ void __launch_bounds__(128) k_stage_overflow(const PartParams P)
+{
+    const int n = min(*P.ovf_count, P.ovf_cap);
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
+        const int tile = P.ovf_tile[k];
+        process_particle<SHAPE, STAGE, QMASK, false>(P, P.ovf_p[k], (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr, nullptr);
     }
 }
 
@@ -663,13 +789,20 @@ __global__ void __launch_bounds__(PTHREADS) k_unpack(const uint32_t *x, const ui
 
 // =================================================================================================
 // host launchers
-static PartParams make_part_params(pm2d_ctx *c, int s)
+static PartParams make_part_params(pm2d_ctx *c, int s, const float *a_level)
 {
     SpeciesDev &S = c->sp[s];
     PartParams P;
     P.x = S.x; P.y = S.y; P.ux = S.ux; P.uy = S.uy; P.uhx = S.uhx; P.uhy = S.uhy; P.w = S.w;
     P.chunk_tile = S.chunk_tile; P.chunk_beg = S.chunk_beg; P.tile_off = S.tile_off; P.nchunks = S.nchunks_dev;
-    P.F = S.F; P.nfix = S.nfix; P.pxfix = S.pxfix; P.pyfix = S.pyfix; P.flags = c->flags;
+    P.F = S.F; P.Enode = c->Enode; P.a = a_level; P.ncomp = c->g.ncomp;
+    P.qE = (float)(-(double)S.cfg.sign * 4.0 * 3.14159265358979323846 * 3.14159265358979323846 / S.cfg.mass);
+    P.pond = S.cfg.sign < 0 ? 1.f : 0.f;
+    P.cv2 = (float)(S.cfg.pressure_coeff * S.vth2);
+    P.inv_2dx = (float)(1.0 / (2.0 * c->g.dx));
+    P.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
+    P.nfix_in = S.nfix; P.nfix = S.nfix; P.pxfix = S.pxfix; P.pyfix = S.pyfix; P.flags = c->flags;
+    P.ovf_p = c->ovf_p; P.ovf_tile = c->ovf_tile; P.ovf_count = c->ovf_count; P.ovf_cap = c->ovf_cap;
     P.nx = c->g.nx; P.ny = c->g.ny; P.nty = c->nty;
     P.dt = (float)c->g.dt;
     P.hx = (float)(c->g.dt / (2.0 * c->g.dx));
@@ -683,7 +816,11 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
 template <int SHAPE>
 static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, cudaStream_t st)
 {
-#define PM2D_LAUNCH(ST, Q) k_stage<SHAPE, ST, Q><<<grid, PTHREADS, 0, st>>>(P)
+#define PM2D_LAUNCH(ST, Q)                                        \
+    do {                                                          \
+        k_stage<SHAPE, ST, Q><<<grid, PTHREADS, 0, st>>>(P);      \
+        if (ST < 2) k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P); \
+    } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }
     else if (stage == 1) { if (qmask == 3) PM2D_LAUNCH(1, 3); else PM2D_LAUNCH(1, 1); }
     else { if (qmask == 3) PM2D_LAUNCH(2, 3); else if (qmask == 2) PM2D_LAUNCH(2, 2); else PM2D_LAUNCH(2, 1); }
@@ -694,13 +831,25 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
 {
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
-    PartParams P = make_part_params(c, s);
+    PartParams P = make_part_params(c, s, stage == 0 ? c->a[1] : c->a[0]);
     const int grid = S.max_chunks;
+    if (stage < 2) {
+        // the force window reads n_s while other CTAs already deposit: ping-pong the density grid
+        const size_t bytes = (size_t)c->nn * sizeof(int32_t);
+        P.nfix = S.nfix2;
+        PM2D_CUDA_CHECK(cudaMemsetAsync(c->ovf_count, 0, sizeof(int32_t), c->stream));
+        PM2D_CUDA_CHECK(cudaMemsetAsync(S.nfix2, 0, bytes, c->stream));
+        if (qmask & 2) {
+            PM2D_CUDA_CHECK(cudaMemsetAsync(S.pxfix, 0, bytes, c->stream));
+            PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
+        }
+    }
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, grid, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, grid, c->stream);
     else launch_stage_shape<PM2D_SINE>(P, stage, qmask, grid, c->stream);
-    count_launch(c);
+    count_launch(c, stage < 2 ? 2 : 1);
     PM2D_CUDA_CHECK(cudaGetLastError());
+    if (stage < 2) std::swap(S.nfix, S.nfix2);
     return PM2D_OK;
 }
 

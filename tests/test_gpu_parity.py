@@ -154,13 +154,14 @@ def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin):
         ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
         assert ex < 1e-5 and ey < 1e-5 and eu < 1e-5, (s, ex, ey, eu)
         assert dabs < 1e-4                                    # absolute, in cells
-    # the last force grid (Eq. 18) and the potential of the final densities
+    # the force grid of Eq. 16 for the final state and the potential of the final densities
     for s, sp in enumerate(cfg["species"]):
         if sp["mobile"]:
             fx = sim.get_fields(P.FIELD_FORCE, 0, s)
             fy = sim.get_fields(P.FIELD_FORCE, 1, s)
-            ref = np.hypot(orc.moment(s, "Fx"), orc.moment(s, "Fy"))
-            err = np.hypot(fx - orc.moment(s, "Fx"), fy - orc.moment(s, "Fy"))
+            rx, ry = orc.force_now(s)
+            ref = np.hypot(rx, ry)
+            err = np.hypot(fx - rx, fy - ry)
             assert np.sqrt((err ** 2).sum()) < 2e-4 * np.sqrt((ref ** 2).sum()), s
     orc.refresh_fields()
     phi = sim.get_fields(P.FIELD_PHI)
