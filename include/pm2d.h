@@ -144,7 +144,8 @@ int64_t pm2d_get_moments(pm2d_ctx *ctx, int species, int moment, int i0, int i1,
 /* Write one full nodal array of `a` (component comp, level 0 = n, 1 = n-1) from host[(nx+1)*ny]. */
 int pm2d_set_fields(pm2d_ctx *ctx, int field, int comp, int level, const float *host);
 
-/* Particles first..first+count-1 of a species in storage order (tile-binned), canonical form.
+/* Particles first..first+count-1 of a species in storage order (binned by tile, then by cell as of the last
+ * rebin), canonical form.
  * Any output pointer may be NULL.  `id` needs track_ids.  Returns the number written. */
 int64_t pm2d_get_particles(pm2d_ctx *ctx, int species, int64_t first, int64_t count, int32_t *ix, int32_t *iy,
                            float *fx, float *fy, float *ux, float *uy, float *w, int64_t *id);
@@ -157,9 +158,10 @@ int pm2d_set_particles(pm2d_ctx *ctx, int species, int64_t count, const int32_t 
 /* Set the nodal density of an immobile species from host[(nx+1)*ny] (n_c). */
 int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
 
-/* Run the tile rebin now.  keys_out[count] (optional) receives, in the OLD storage order, the
- * destination tile key of every particle; perm_out[count] (optional) receives for every NEW slot
- * the OLD slot it came from.  The result equals a stable counting sort by key. */
+/* Run the rebin now.  keys_out[count] (optional, host) receives, in the OLD storage order, the
+ * destination key of every particle, key = tile * PM2D_TILE^2 + (ix % PM2D_TILE) * PM2D_TILE + iy % PM2D_TILE
+ * with tile = (ix / PM2D_TILE) * ceil(ny / PM2D_TILE) + iy / PM2D_TILE; perm_out[count] (optional, host)
+ * receives for every NEW slot the OLD slot it came from.  The result equals a stable counting sort by key. */
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);

@@ -119,10 +119,10 @@ size_t layout(pm2d_ctx *c, char *base)
         S.pyfix = cv.take<int32_t>(nn);
         S.F = cv.take<float2>(nn);
         const size_t cap = (size_t)std::max<int64_t>(S.cap, 1);
-        S.x = cv.take<uint32_t>(cap); S.y = cv.take<uint32_t>(cap);
-        S.ux = cv.take<float>(cap); S.uy = cv.take<float>(cap); S.w = cv.take<float>(cap);
-        S.uhx = cv.take<float>(cap); S.uhy = cv.take<float>(cap);
-        S.x2 = cv.take<uint32_t>(cap); S.y2 = cv.take<uint32_t>(cap); S.w2 = cv.take<float>(cap);
+        S.pv = cv.take<PV>(cap); S.pv2 = cv.take<PV>(cap);
+        S.uh = cv.take<float2>(cap);
+        S.w = cv.take<float>(cap); S.w2 = cv.take<float>(cap);
+        S.cell_off = cv.take<int32_t>((size_t)ntiles * CPITCH);
         S.id = S.id2 = nullptr;
         if (g.track_ids) { S.id = cv.take<int64_t>(cap); S.id2 = cv.take<int64_t>(cap); }
         S.max_chunks = ntiles + (int32_t)(cap / CHUNK) + 1;
@@ -358,7 +358,7 @@ static int enqueue_step(pm2d_ctx *c)
     if (c->g.rebin_every > 0 && c->step % c->g.rebin_every == 0) {
         phase_begin(c, PM2D_PH_REBIN);
         for (int s = 0; s < c->nsp; s++)
-            if (c->sp[s].cfg.mobile && (rc = launch_rebin(c, s, nullptr, nullptr))) return rc;
+            if (c->sp[s].cfg.mobile && (rc = launch_rebin(c, s, nullptr, nullptr, nullptr))) return rc;
         phase_end(c);
     }
     return PM2D_OK;
@@ -509,10 +509,13 @@ extern "C" int64_t pm2d_get_particles(pm2d_ctx *c, int s, int64_t first, int64_t
     count = std::min(count, S.np - first);
     if (count == 0) return 0;
     if (id && !S.id) return fail(PM2D_EINVAL, "ids need track_ids");
-    // canonical cell + offset of every particle into the (idle) rebin buffers
-    int32_t *dix = (int32_t *)S.x2, *diy = (int32_t *)S.y2;
-    float *dfx = S.w2, *dfy = S.uhx;
-    int rc = launch_unpack_particles(c, s, first, count, dix, diy, dfx, dfy);
+    // canonical cell + offset and velocity of every particle as separate arrays in the (idle) rebin and
+    // predictor buffers: pv2 holds 4 arrays of cap words, uh holds 2
+    const size_t capw = (size_t)std::max<int64_t>(S.cap, 1);
+    int32_t *dix = (int32_t *)S.pv2, *diy = dix + capw;
+    float *dfx = (float *)(diy + capw), *dfy = dfx + capw;
+    float *dux = (float *)S.uh, *duy = dux + capw;
+    int rc = launch_unpack_particles(c, s, dix, diy, dfx, dfy, dux, duy);
     if (rc) return rc;
     auto d2h = [&](void *dst, const void *src, size_t esz) -> cudaError_t {
         if (!dst) return cudaSuccess;
@@ -522,8 +525,8 @@ extern "C" int64_t pm2d_get_particles(pm2d_ctx *c, int s, int64_t first, int64_t
     PM2D_CUDA_CHECK(d2h(iy, diy, 4));
     PM2D_CUDA_CHECK(d2h(fx, dfx, 4));
     PM2D_CUDA_CHECK(d2h(fy, dfy, 4));
-    PM2D_CUDA_CHECK(d2h(ux, S.ux, 4));
-    PM2D_CUDA_CHECK(d2h(uy, S.uy, 4));
+    PM2D_CUDA_CHECK(d2h(ux, dux, 4));
+    PM2D_CUDA_CHECK(d2h(uy, duy, 4));
     PM2D_CUDA_CHECK(d2h(w, S.w, 4));
     PM2D_CUDA_CHECK(d2h(id, S.id, 8));
     PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
@@ -538,38 +541,45 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
     if (count < 0 || count > S.cap) return fail(PM2D_ENOMEM, "more particles than capacity");
     if (count > 0 && (!ix || !iy || !fx || !fy || !ux || !uy || !w)) return fail(PM2D_EINVAL, "null particle array");
     const int nx = c->g.nx, ny = c->g.ny, nty = c->nty, ntiles = c->ntiles;
-    // host-side stable counting sort by tile (test / restart path, not the hot path)
+    // host-side stable counting sort by (tile, cell) (test / restart path, not the hot path)
     std::vector<int64_t> off(ntiles + 1, 0);
-    std::vector<int32_t> key((size_t)count);
+    std::vector<int32_t> coff((size_t)ntiles * CPITCH, 0);
+    std::vector<int64_t> key((size_t)count);
     for (int64_t p = 0; p < count; p++) {
         if (ix[p] < 0 || ix[p] >= nx || iy[p] < 0 || iy[p] >= ny || !(fx[p] >= 0.f && fx[p] < 1.f) || !(fy[p] >= 0.f && fy[p] < 1.f))
             return fail(PM2D_EINVAL, "particle outside the box or offset outside [0,1)");
-        key[p] = (ix[p] / TILE) * nty + iy[p] / TILE;
-        off[key[p] + 1]++;
+        const int t = (ix[p] / TILE) * nty + iy[p] / TILE, cl = (ix[p] % TILE) * TILE + iy[p] % TILE;
+        key[p] = (int64_t)t * CPITCH + cl;
+        off[t + 1]++;
+        coff[key[p] + 1]++;      // count of cell cl lands in slot cl+1 of the same tile (slot TCELLS = last cell)
     }
     for (int t = 0; t < ntiles; t++) off[t + 1] += off[t];
-    std::vector<int64_t> cur(off.begin(), off.end() - 1);
-    std::vector<uint32_t> hx((size_t)count), hy((size_t)count);
-    std::vector<float> hux((size_t)count), huy((size_t)count), hw((size_t)count);
+    std::vector<int64_t> cur((size_t)ntiles * CPITCH);
+    for (int t = 0; t < ntiles; t++) {
+        int32_t *co = coff.data() + (size_t)t * CPITCH;
+        co[0] = 0;
+        for (int cl = 0; cl < TCELLS; cl++) co[cl + 1] += co[cl];       // exclusive scan: co[cl] = first slot of cell cl
+        for (int cl = 0; cl < TCELLS; cl++) cur[(size_t)t * CPITCH + cl] = off[t] + co[cl];
+    }
+    std::vector<PV> hpv((size_t)count);
+    std::vector<float> hw((size_t)count);
     std::vector<int64_t> hid(S.id ? (size_t)count : 0);
     for (int64_t p = 0; p < count; p++) {
         int64_t q = cur[key[p]]++;
         int li = ix[p] % TILE, lj = iy[p] % TILE;
-        hx[q] = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fx[p] * 16777216.0);
-        hy[q] = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fy[p] * 16777216.0);
-        hux[q] = ux[p]; huy[q] = uy[p]; hw[q] = w[p];
+        hpv[q].x = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fx[p] * 16777216.0);
+        hpv[q].y = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fy[p] * 16777216.0);
+        hpv[q].ux = ux[p]; hpv[q].uy = uy[p]; hw[q] = w[p];
         if (S.id) hid[q] = p;
     }
     auto h2d = [&](void *dst, const void *src, size_t bytes) { return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream); };
     if (count > 0) {
-        PM2D_CUDA_CHECK(h2d(S.x, hx.data(), (size_t)count * 4));
-        PM2D_CUDA_CHECK(h2d(S.y, hy.data(), (size_t)count * 4));
-        PM2D_CUDA_CHECK(h2d(S.ux, hux.data(), (size_t)count * 4));
-        PM2D_CUDA_CHECK(h2d(S.uy, huy.data(), (size_t)count * 4));
+        PM2D_CUDA_CHECK(h2d(S.pv, hpv.data(), (size_t)count * sizeof(PV)));
         PM2D_CUDA_CHECK(h2d(S.w, hw.data(), (size_t)count * 4));
         if (S.id) PM2D_CUDA_CHECK(h2d(S.id, hid.data(), (size_t)count * 8));
     }
     PM2D_CUDA_CHECK(h2d(S.tile_off, off.data(), (size_t)(ntiles + 1) * 8));
+    PM2D_CUDA_CHECK(h2d(S.cell_off, coff.data(), coff.size() * 4));
     S.np = count;
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
@@ -583,17 +593,19 @@ extern "C" int pm2d_rebin(pm2d_ctx *c, int s, int32_t *keys_out, int64_t *perm_o
     if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
     SpeciesDev &S = c->sp[s];
     int32_t *dk = nullptr;
-    int64_t *dp = nullptr;
+    int64_t *dp = nullptr, *dt = nullptr;
     const size_t n = (size_t)std::max<int64_t>(S.np, 1);
     if (keys_out) PM2D_CUDA_CHECK(cudaMalloc(&dk, n * sizeof(int32_t)));
     if (perm_out) PM2D_CUDA_CHECK(cudaMalloc(&dp, n * sizeof(int64_t)));
-    int rc = launch_rebin(c, s, dk, dp);
+    if (keys_out || perm_out) PM2D_CUDA_CHECK(cudaMalloc(&dt, n * sizeof(int64_t)));
+    int rc = launch_rebin(c, s, dk, dp, dt);
     if (!rc && keys_out) rc = cudaMemcpyAsync(keys_out, dk, (size_t)S.np * 4, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;
     if (!rc && perm_out) rc = cudaMemcpyAsync(perm_out, dp, (size_t)S.np * 8, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;
     if (!rc) rc = check_flags(c);
     else cudaStreamSynchronize(c->stream);
     cudaFree(dk);
     cudaFree(dp);
+    cudaFree(dt);
     return rc;
 }
 

@@ -82,11 +82,13 @@ __global__ void __launch_bounds__(256) k_diag_species_grid(const int32_t *nfix, 
     block_add(q, red_charge);
 }
 
-__global__ void __launch_bounds__(256) k_diag_kinetic(const float *ux, const float *uy, const float *w, int64_t np, double *red)
+__global__ void __launch_bounds__(256) k_diag_kinetic(const PV *pv, const float *w, int64_t np, double *red)
 {
     double s = 0.0;
-    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += (int64_t)gridDim.x * blockDim.x)
-        s += (double)w[p] * ((double)ux[p] * ux[p] + (double)uy[p] * uy[p]);
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < np; p += (int64_t)gridDim.x * blockDim.x) {
+        const PV me = pv[p];
+        s += (double)w[p] * ((double)me.ux * me.ux + (double)me.uy * me.uy);
+    }
     block_add(s, red);
 }
 
@@ -114,7 +116,7 @@ int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out)
         k_diag_species_grid<<<grid, 256, 0, c->stream>>>(S.nfix, c->g.nx, c->g.ny, c->inv_nscale, c->red + 4 + 3 * s, c->red + 5 + 3 * s);
         count_launch(c);
         if (S.cfg.mobile && S.np > 0) {
-            k_diag_kinetic<<<592, 256, 0, c->stream>>>(S.ux, S.uy, S.w, S.np, c->red + 3 + 3 * s);
+            k_diag_kinetic<<<592, 256, 0, c->stream>>>(S.pv, S.w, S.np, c->red + 3 + 3 * s);
             count_launch(c);
         }
     }

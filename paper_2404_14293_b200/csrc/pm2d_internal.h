@@ -13,13 +13,21 @@ constexpr int TILE = PM2D_TILE;          // cells per tile side
 constexpr int HALO = 4;                  // window nodes beyond the tile on each side
 constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (41)
 constexpr int WPITCH = WIN;              // odd pitch: rows start on different banks
-constexpr int CHUNK = 8192;              // max particles per CTA work item
-constexpr int PTHREADS = 256;            // threads per particle CTA
+constexpr int CHUNK = 8192;              // max particles per CTA work item (loader, tile rebin, unpack)
+constexpr int PTHREADS = 256;            // threads per CTA of the chunk kernels
+constexpr int TCELLS = TILE * TILE;      // cells per tile
+constexpr int CPITCH = TCELLS + 1;       // ints per tile in cell_off (last = particles in the tile)
 constexpr int TRI_M = 32;                // rows per x-partition of the tridiagonal solve
 // fixed-point tile-relative position: (cell_rel + POS_BIAS) << 24 | frac24
 constexpr int POS_BIAS = 64;
 constexpr int POS_FRAC_BITS = 24;
 constexpr uint32_t POS_FRAC_MASK = (1u << POS_FRAC_BITS) - 1u;
+
+// one particle: fixed-point tile-relative position and velocity, 16 bytes (one 128-bit access)
+struct __align__(16) PV {
+    uint32_t x, y;
+    float ux, uy;
+};
 
 struct SpeciesDev {
     // host copy of the parameters
@@ -27,13 +35,14 @@ struct SpeciesDev {
     double vth2;
     int64_t np;          // particles held (constant: walls reflect, y wraps)
     int64_t cap;
-    // particle SoA (device)
-    uint32_t *x, *y;     // fixed-point tile-relative position
-    float *ux, *uy, *w;
-    float *uhx, *uhy;    // predictor velocity u^ (Eq. 17); scratch for the rebin
-    uint32_t *x2, *y2;   // rebin double buffers
+    // particles (device), stored tile by tile and, inside a tile, cell by cell (as of the last rebin)
+    PV *pv;              // position + velocity
+    float *w;            // density weight
+    float2 *uh;          // predictor velocity u^ (Eq. 17); scratch outside a step
+    PV *pv2;             // rebin double buffers
     float *w2;
     int64_t *id, *id2;   // optional
+    int32_t *cell_off;   // [ntiles][CPITCH] first slot (relative to the tile) of each cell's run
     // binning
     int64_t *tile_off;   // [ntiles+1] first slot of each tile
     int64_t *tile_off2;
@@ -115,10 +124,10 @@ static inline void count_launch(pm2d_ctx *c, int n = 1)
 int launch_load_particles(pm2d_ctx *c, int s);
 int launch_stage(pm2d_ctx *c, int s, int stage);            // 0 = A (Eq. 17), 1 = B (Eq. 19)
 int launch_deposit_only(pm2d_ctx *c, int s, bool density, bool momentum);
-int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev);
+int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64_t *perm_tmp_dev);
+int launch_set_cell_offsets_uniform(pm2d_ctx *c, int s);
 int launch_build_chunks(pm2d_ctx *c, int s);
-int launch_unpack_particles(pm2d_ctx *c, int s, int64_t first, int64_t count, int32_t *ix, int32_t *iy,
-                            float *fx, float *fy);
+int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float *fx, float *fy, float *ux, float *uy);
 // pm2d_fields.cu
 int launch_field_step(pm2d_ctx *c);
 int launch_force(pm2d_ctx *c, int s, const float *a_level);

@@ -1,34 +1,45 @@
 // pm2d_particles.cu -- particle kernels of libpm2d.so (sm_100a):
 //   * fused gather + push + deposit, stage A (Eq. 17) and stage B (Eq. 19)      [P:L191-221]
 //   * deposit-only pass (initial item (1) of the flow, lazy momentum grids)       [Eq. 14, P:L187]
-//   * counter-based particle loader (Philox-4x32-10; DESIGN.md section 5)         [P:L154-162]
-//   * stable tile rebin (counting sort specialised to neighbour moves)            [DESIGN.md 6.4]
+//   * counter-based particle loader (Philox-4x32-10; DESIGN.md section 4)         [P:L154-162]
+//   * stable rebin by (tile, cell): tile pass specialised to neighbour moves, then a counting
+//     sort by cell inside every tile                                              [DESIGN.md 6.4]
 //
-// Data layout.  Particles are SoA, stored tile by tile (PM2D_TILE x PM2D_TILE cells); a particle's
-// position is a pair of 32-bit fixed-point numbers relative to its tile's origin,
+// Data layout.  A particle is a 16-byte record PV {x, y, ux, uy} plus a weight w and, between the
+// two stages of a step, the predictor velocity u^ (float2).  Particles are stored tile by tile
+// (PM2D_TILE x PM2D_TILE cells) and inside a tile cell by cell (row-major cells, as of the last
+// rebin); cell_off gives every cell's run.  A position is a pair of 32-bit fixed-point numbers
+// relative to the tile's origin,
 //     xfix = (cell_rel + POS_BIAS) << 24 | frac24,
 // so the in-cell offset carries 24 bits whatever the size of the box, the push is an exact integer
 // add of a rounded displacement, and the canonical (ix, fx) of include/pm2d.h is read off exactly.
-// A CTA owns one chunk (<= CHUNK particles of one tile): it stages the force of the tile + halo in
-// shared memory, accumulates the deposit of its particles in a shared int32 fixed-point window
-// (native ATOMS.ADD; float atomics in shared memory are CAS loops on sm_100a) and flushes the
-// window once with global integer reductions.  Integer accumulation makes the deposited grids
-// independent of the order of the atomics (bit-reproducible) and n_i - n_e exact.
+//
+// Fused stage kernel.  A CTA owns one tile: it builds the force of the tile + halo in shared memory
+// (Eq. 16/18), and every thread owns a strip of S consecutive cells of one cell row.  While the
+// thread walks the particles of a cell it keeps, in registers, the force on the 4 x 4 nodes around
+// that cell and the deposit those particles make on the same 16 nodes: a particle that is still
+// within half a cell of its rebin-time cell gathers and deposits entirely in registers (weights of
+// the four nodes per axis from three evaluations of the cumulative shape G, Eq. 13).  Moving to the
+// next cell slides the patch one column: the oldest column is rounded to fixed point and added to
+// the tile's shared int32 window with 4 x 3 conflict-free ATOMS (lanes = rows, odd pitch), the new
+// force column is read with 4 LDS.64.  Particles that drifted further take the same arithmetic on
+// the shared windows directly (3 x 3 nodes around the nearest node), and those outside the window
+// go to an overflow list handled on the global grids.  The window is flushed once with global
+// integer reductions.  Integer accumulation makes the grids independent of the order of the
+// atomics (bit-reproducible) and n_i - n_e exact.
 #include "pm2d_internal.h"
 
 namespace {
 
 struct PartParams {
     // particles
-    uint32_t *x, *y;
-    float *ux, *uy, *uhx, *uhy;
+    PV *pv;
+    float2 *uh;
     const float *w;
-    const int32_t *chunk_tile;
-    const int64_t *chunk_beg;
     const int64_t *tile_off;
-    const int32_t *nchunks;
+    const int32_t *cell_off;
     // grids
-    const float2 *F;          // materialised force grid (slow path / diagnostics); may be NULL
+    const float2 *F;          // materialised force grid (diagnostics only); may be NULL
     const float2 *Enode;      // nodal E of the last Poisson solve
     const float *a;           // [ncomp][nn], level n (stage A) or n+1 (stage B)
     int ncomp;
@@ -44,7 +55,8 @@ struct PartParams {
     float dt, hx, hy;        // hx = dt / (2 dx): cells per unit (u' + u)
     float nscale, pscale;
     float half_dd;           // DD / 2
-    float shape_k;           // 0.5 / DD  (sine: G(s) = sinpi(s * shape_k)^2)
+    float dd;                // DD
+    float k_rad;             // pi / DD  (sine: G(t) = 1/2 - 1/2 cos(k_rad t))
 };
 
 __device__ __forceinline__ int fold_x(int i, int nx)
@@ -55,32 +67,55 @@ __device__ __forceinline__ int fold_x(int i, int nx)
     return i;
 }
 
-// O1 / Eq. 13: weights of the three nodes c-1, c, c+1 around the nearest node c for a particle at
-// offset d in [-1/2, 1/2) from it.  With s measured from the particle's left edge, the control-
-// volume faces c-1/2 and c+1/2 sit at s0 = DD/2 - 1/2 - d and s1 = s0 + 1, and
-//   W[c-1] = G(s0), W[c] = G(s1) - G(s0), W[c+1] = 1 - G(s1),  G clamped to [0, DD].
+// O1 / Eq. 13: cumulative shape G(t), t already clamped to [0, DD].  SINE: G = 1/2 - 1/2 cos(pi t/DD)
+// (Q1) through MUFU.COS (abs. error < 5e-7); TSC, CIC: textbook (ref. [42]).
 template <int SHAPE>
-__device__ __forceinline__ void weights3(float d, float half_dd, float shape_k, float W[3])
+__device__ __forceinline__ float shape_G(float t, float k_rad)
 {
+    if (SHAPE == PM2D_SINE) return fmaf(-0.5f, __cosf(t * k_rad), 0.5f);
     if (SHAPE == PM2D_TSC) {
-        float a = 0.5f - d, b = 0.5f + d;
-        W[0] = 0.5f * a * a;
-        W[2] = 0.5f * b * b;
-        W[1] = 0.75f - d * d;
-    } else if (SHAPE == PM2D_CIC) {
-        W[0] = fmaxf(-d, 0.f);
-        W[2] = fmaxf(d, 0.f);
-        W[1] = 1.f - fabsf(d);
+        float u = fminf(t, 2.f - t), h = 0.5f * u * u;
+        return t < 1.f ? h : 1.f - h;
+    }
+    return t;   // CIC, DD = 1
+}
+
+// weights of the three nodes c-1, c, c+1 around the nearest node c for a particle at offset d in
+// [-1/2, 1/2) from it: control-volume faces c-1/2, c+1/2 at t0 = DD/2 - 1/2 - d, t1 = t0 + 1 from the
+// particle's left edge;  W[c-1] = G(t0), W[c] = G(t1) - G(t0), W[c+1] = 1 - G(t1).
+template <int SHAPE>
+__device__ __forceinline__ void weights3(float d, const PartParams &P, float W[3])
+{
+    float t0 = fminf(fmaxf(P.half_dd - 0.5f - d, 0.f), P.dd);
+    float t1 = fminf(fmaxf(P.half_dd + 0.5f - d, 0.f), P.dd);
+    float g0 = shape_G<SHAPE>(t0, P.k_rad), g1 = shape_G<SHAPE>(t1, P.k_rad);
+    W[0] = g0;
+    W[1] = g1 - g0;
+    W[2] = 1.f - g1;
+}
+
+// weights of the four nodes c-1 .. c+2 around cell c for a particle at offset f in [-1/2, 3/2) from
+// the cell's origin: faces c-1/2, c+1/2, c+3/2 at t_k = DD/2 + k - 1/2 - f; the outer faces c-3/2 and
+// c+5/2 lie outside the cloud (G = 0, 1) because DD <= 2.
+template <int SHAPE>
+__device__ __forceinline__ void weights4(float f, const PartParams &P, float W[4])
+{
+    const float b = P.half_dd - 0.5f - f;
+    float t0 = fminf(fmaxf(b, 0.f), P.dd);
+    float t1 = fminf(fmaxf(b + 1.f, 0.f), P.dd);
+    float t2 = fminf(fmaxf(b + 2.f, 0.f), P.dd);
+    if (SHAPE == PM2D_SINE) {
+        float c0 = __cosf(t0 * P.k_rad), c1 = __cosf(t1 * P.k_rad), c2 = __cosf(t2 * P.k_rad);
+        W[0] = fmaf(-0.5f, c0, 0.5f);
+        W[1] = 0.5f * (c0 - c1);
+        W[2] = 0.5f * (c1 - c2);
+        W[3] = fmaf(0.5f, c2, 0.5f);
     } else {
-        float dd = 2.f * half_dd;
-        float s0 = fminf(fmaxf(half_dd - 0.5f - d, 0.f), dd);
-        float s1 = fminf(fmaxf(half_dd + 0.5f - d, 0.f), dd);
-        float g0 = sinpif(s0 * shape_k), g1 = sinpif(s1 * shape_k);
-        g0 *= g0;
-        g1 *= g1;
+        float g0 = shape_G<SHAPE>(t0, P.k_rad), g1 = shape_G<SHAPE>(t1, P.k_rad), g2 = shape_G<SHAPE>(t2, P.k_rad);
         W[0] = g0;
         W[1] = g1 - g0;
-        W[2] = 1.f - g1;
+        W[2] = g2 - g1;
+        W[3] = 1.f - g2;
     }
 }
 
@@ -101,36 +136,64 @@ __device__ __forceinline__ uint32_t advance(uint32_t f, float h, float usum)
     return f + (uint32_t)__float2int_rn(disp);
 }
 
-template <int QMASK>
-__device__ __forceinline__ void deposit_window(int32_t *dep, int cx, int cy, const float Wx[3], const float Wy[3],
-                                               float qn, float qx, float qy, bool skip_zero)
+// x walls reflect (Q9); y is periodic and needs nothing until the rebin
+__device__ __forceinline__ void reflect_x(uint32_t &xf, float &ux, int gx0, int nx)
 {
-    const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-#pragma unroll
-        for (int b = 0; b < 3; b++) {
-            float ww = Wx[a] * Wy[b];
-            if (skip_zero && ww == 0.f) continue;
-            int e = base + a * WPITCH + b;
-            if (QMASK & 1) atomicAdd(&dep[e], __float2int_rn(ww * qn));
-            if (QMASK & 2) {
-                atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(ww * qx));
-                atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(ww * qy));
-            }
-        }
-    }
+    const int64_t org = ((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS;
+    int64_t gx = org + (int64_t)xf;
+    const int64_t wall = (int64_t)nx << POS_FRAC_BITS;
+    if (gx < 0) {
+        gx = -gx;
+        ux = -ux;
+    } else if (gx >= wall) {
+        gx = 2 * wall - gx;
+        if (gx >= wall) gx = wall - 1;
+        ux = -ux;
+    } else
+        return;
+    xf = (uint32_t)(gx - org);
 }
 
-// slow path: footprint outside the shared window (a particle that drifted more than HALO - 1/2
-// cells from its tile since the last rebin) -> straight to the global grids
-template <int QMASK>
-__device__ __noinline__ void deposit_global(const PartParams &P, int gx0, int gy0, int cx, int cy, const float Wx[3],
-                                            const float Wy[3], float qn, float qx, float qy)
+__device__ __forceinline__ bool in_window(int cx, int cy)
 {
+    return cx - 1 >= -HALO && cx + 1 <= TILE + HALO && cy - 1 >= -HALO && cy + 1 <= TILE + HALO;
+}
+
+// ---- deposit of one particle outside the register patch: 3 x 3 nodes around the nearest node, into the
+// shared window when it covers them, else straight to the global grids (particle far from its tile)
+template <int SHAPE, int QMASK, bool WINDOWED>
+__device__ __forceinline__ void deposit_direct(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, float ux, float uy,
+                                               float w, int32_t *dep)
+{
+    int cx, cy;
+    float dx_, dy_, Wx[3], Wy[3];
+    decode(xf, cx, dx_);
+    decode(yf, cy, dy_);
+    weights3<SHAPE>(dx_, P, Wx);
+    weights3<SHAPE>(dy_, P, Wy);
+    const float qn = w * P.nscale, qx = w * ux * P.pscale, qy = w * uy * P.pscale;
+    if (WINDOWED && in_window(cx, cy)) {
+        const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                float ww = Wx[a] * Wy[b];
+                if (ww == 0.f) continue;
+                int e = base + a * WPITCH + b;
+                if (QMASK & 1) atomicAdd(&dep[e], __float2int_rn(ww * qn));
+                if (QMASK & 2) {
+                    atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(ww * qx));
+                    atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(ww * qy));
+                }
+            }
+        return;
+    }
+#pragma unroll 1
     for (int a = 0; a < 3; a++) {
         int gi = fold_x(gx0 + cx - 1 + a, P.nx);
         int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
+#pragma unroll 1
         for (int b = 0; b < 3; b++) {
             int gj = (gy0 + cy - 1 + b) & (P.ny - 1);
             float ww = Wx[a] * Wy[b];
@@ -144,7 +207,7 @@ __device__ __noinline__ void deposit_global(const PartParams &P, int gx0, int gy
     }
 }
 
-// Eq. 16 at one global node (slow path only)
+// Eq. 16 at one global node (overflow path only)
 __device__ __forceinline__ float2 force_at_node(const PartParams &P, int gi, int gj)
 {
     const size_t nn = (size_t)(P.nx + 1) * P.ny;
@@ -176,49 +239,111 @@ __device__ __forceinline__ float2 force_at_node(const PartParams &P, int gi, int
     return make_float2(fx, fy);
 }
 
-__device__ __noinline__ float2 gather_global(const PartParams &P, int gx0, int gy0, int cx, int cy, const float Wx[3],
-                                             const float Wy[3])
+// Eq. 15 on 3 x 3 nodes around the nearest node: from the shared force window, or (overflow path)
+// from forces evaluated on the global grids
+template <int SHAPE, bool WINDOWED>
+__device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, const float2 *Fs, bool &ok)
 {
+    int cx, cy;
+    float dx_, dy_, Wx[3], Wy[3];
+    decode(xf, cx, dx_);
+    decode(yf, cy, dy_);
+    ok = !WINDOWED || in_window(cx, cy);
+    if (!ok) return make_float2(0.f, 0.f);
+    weights3<SHAPE>(dx_, P, Wx);
+    weights3<SHAPE>(dy_, P, Wy);
     float fx = 0.f, fy = 0.f;
+    if (WINDOWED) {
+        const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float rx = 0.f, ry = 0.f;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                float2 f = Fs[base + a * WPITCH + b];
+                rx += Wy[b] * f.x;
+                ry += Wy[b] * f.y;
+            }
+            fx += Wx[a] * rx;
+            fy += Wx[a] * ry;
+        }
+    } else {
 #pragma unroll 1
-    for (int a = 0; a < 3; a++) {
-        int gi = fold_x(gx0 + cx - 1 + a, P.nx);
+        for (int a = 0; a < 3; a++) {
+            int gi = fold_x(gx0 + cx - 1 + a, P.nx);
 #pragma unroll 1
-        for (int b = 0; b < 3; b++) {
-            int gj = (gy0 + cy - 1 + b) & (P.ny - 1);
-            float2 f = force_at_node(P, gi, gj);
-            float ww = Wx[a] * Wy[b];
-            fx += ww * f.x;
-            fy += ww * f.y;
+            for (int b = 0; b < 3; b++) {
+                int gj = (gy0 + cy - 1 + b) & (P.ny - 1);
+                float2 f = force_at_node(P, gi, gj);
+                float ww = Wx[a] * Wy[b];
+                fx += ww * f.x;
+                fy += ww * f.y;
+            }
         }
     }
     return make_float2(fx, fy);
 }
 
-__device__ __forceinline__ bool in_window(int cx, int cy)
+// One particle through one stage outside the register patch.  STAGE 0: predictor (Eq. 17); STAGE 1:
+// corrector (Eq. 19) + particle boundaries; STAGE 2: deposit only.  QMASK bit 0: density, bit 1: momentum.
+// WINDOWED: shared windows; returns false (nothing done) when the gather footprint lies outside the
+// window -- the caller defers the particle to k_stage_overflow (WINDOWED = false, global grids).
+template <int SHAPE, int STAGE, int QMASK, bool WINDOWED>
+__device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
 {
-    return cx - 1 >= -HALO && cx + 1 <= TILE + HALO && cy - 1 >= -HALO && cy + 1 <= TILE + HALO;
-}
-
-__device__ __forceinline__ float2 gather_window(const float2 *Fs, int cx, int cy, const float Wx[3], const float Wy[3])
-{
-    const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
-    float fx = 0.f, fy = 0.f;
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-        float rx = 0.f, ry = 0.f;
-#pragma unroll
-        for (int b = 0; b < 3; b++) {
-            float2 f = Fs[base + a * WPITCH + b];
-            rx += Wy[b] * f.x;
-            ry += Wy[b] * f.y;
-        }
-        fx += Wx[a] * rx;
-        fy += Wx[a] * ry;
+    PV me = P.pv[p];
+    uint32_t xf = me.x, yf = me.y;
+    float ux = me.ux, uy = me.uy;
+    if (STAGE == 0) {
+        bool ok;
+        float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xf, yf, Fs, ok);
+        if (!ok) return false;
+        float uhx = __fmaf_rn(P.dt, f.x, ux), uhy = __fmaf_rn(P.dt, f.y, uy);     // Eq. 17
+        P.uh[p] = make_float2(uhx, uhy);
+        xf = advance(xf, P.hx, __fadd_rn(uhx, ux));
+        yf = advance(yf, P.hy, __fadd_rn(uhy, uy));
+        ux = uhx;
+        uy = uhy;
+    } else if (STAGE == 1) {
+        const float2 uh = P.uh[p];
+        uint32_t xh = advance(xf, P.hx, __fadd_rn(uh.x, ux));                      // x^ of Eq. 17 again
+        uint32_t yh = advance(yf, P.hy, __fadd_rn(uh.y, uy));
+        bool ok;
+        float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xh, yh, Fs, ok);
+        if (!ok) return false;
+        float unx = __fmaf_rn(0.5f * P.dt, f.x, 0.5f * __fadd_rn(uh.x, ux));       // Eq. 19
+        float uny = __fmaf_rn(0.5f * P.dt, f.y, 0.5f * __fadd_rn(uh.y, uy));
+        xf = advance(xf, P.hx, __fadd_rn(unx, ux));
+        yf = advance(yf, P.hy, __fadd_rn(uny, uy));
+        reflect_x(xf, unx, gx0, P.nx);
+        me.x = xf; me.y = yf; me.ux = unx; me.uy = uny;
+        P.pv[p] = me;
+        ux = unx;
+        uy = uny;
     }
-    return make_float2(fx, fy);
+    deposit_direct<SHAPE, QMASK, WINDOWED>(P, gx0, gy0, xf, yf, ux, uy, P.w[p], dep);
+    return true;
 }
 
+template <int SHAPE, int STAGE, int QMASK>
+__device__ __noinline__ void slow_particle(const PartParams &P, int64_t p, int tile, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+{
+    if (!process_direct<SHAPE, STAGE, QMASK, true>(P, p, gx0, gy0, Fs, dep)) {
+        int slot = atomicAdd(P.ovf_count, 1);
+        if (slot < P.ovf_cap) {
+            P.ovf_p[slot] = p;
+            P.ovf_tile[slot] = tile;
+        } else
+            P.flags[2] = 1;
+    }
+}
+
+template <int SHAPE, int QMASK>
+__device__ __noinline__ void slow_deposit(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, float ux, float uy, float w,
+                                          int32_t *dep)
+{
+    deposit_direct<SHAPE, QMASK, true>(P, gx0, gy0, xf, yf, ux, uy, w, dep);
+}
 
 // Eq. 16 / 18 evaluated for the nodes of the tile window, straight into shared memory:
 //   F = qE E_node - (1/2) grad(sum_c a_c^2) [electrons] - C v_th^2 grad(n)/n
@@ -230,7 +355,7 @@ __device__ __forceinline__ void build_force_window(const PartParams &P, int gx0,
 {
     const size_t nn = (size_t)(P.nx + 1) * P.ny;
 #pragma unroll 2
-    for (int e = threadIdx.x; e < WF * WF; e += PTHREADS) {
+    for (int e = threadIdx.x; e < WF * WF; e += blockDim.x) {
         int r = e / WF, cidx = e - r * WF;
         int gi = fold_x(gx0 + r - HALO - 1, P.nx);
         int gj = (gy0 + cidx - HALO - 1) & (P.ny - 1);
@@ -246,7 +371,7 @@ __device__ __forceinline__ void build_force_window(const PartParams &P, int gx0,
     }
     __syncthreads();
 #pragma unroll 1
-    for (int e = threadIdx.x; e < WIN * WIN; e += PTHREADS) {
+    for (int e = threadIdx.x; e < WIN * WIN; e += blockDim.x) {
         int r = e / WIN, cidx = e - r * WIN;
         int raw = gx0 + r - HALO;
         int gi = fold_x(raw, P.nx);
@@ -275,121 +400,245 @@ __device__ __forceinline__ void build_force_window(const PartParams &P, int gx0,
     __syncthreads();
 }
 
-// One particle through one stage.  STAGE 0: predictor (Eq. 17); STAGE 1: corrector (Eq. 19) + particle
-// boundaries; STAGE 2: deposit only.  QMASK bit 0: density, bit 1: momentum.
-// WINDOWED: gather from / deposit into the CTA's shared windows; returns false (nothing done) when the
-// gather footprint lies outside the window -- the caller defers the particle to k_stage_overflow, which
-// runs the same code with WINDOWED = false straight on the global grids.
-template <int SHAPE, int STAGE, int QMASK, bool WINDOWED>
-__device__ __forceinline__ bool process_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+// ---- register patch of a strip thread: force on, and deposit to, the 4 x 4 nodes around its current cell.
+// Logical column b (node column j-1+b of cell column j) lives in physical column (b + ROT) & 3, so sliding
+// to the next cell renames columns instead of moving registers.
+struct Patch {
+    float Fx[4][4], Fy[4][4];
+    float dn[4][4], dpx[4][4], dpy[4][4];
+};
+
+__device__ __forceinline__ bool in_patch(int rel) { return (uint32_t)(rel + (1 << 23)) < (1u << 25); }   // offset in [-1/2, 3/2)
+
+template <int SHAPE, int STAGE, int QMASK, int ROT>
+__device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, const PV me, const float wme, const float2 uhme,
+                                               const int64_t p, const uint32_t ax_fix, const uint32_t ay_fix, const int tile,
+                                               const int gx0, const int gy0, const float2 *Fs, int32_t *dep)
 {
-    uint32_t xf = P.x[p], yf = P.y[p];
-    float ux = P.ux[p], uy = P.uy[p];
-    float Wx[3], Wy[3];
-    int cx, cy;
-    float dx_, dy_;
-    if (STAGE == 0) {
-        decode(xf, cx, dx_);
-        decode(yf, cy, dy_);
-        if (WINDOWED && !in_window(cx, cy)) return false;
-        weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-        weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-        float2 f = WINDOWED ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
-        float uhx = __fmaf_rn(P.dt, f.x, ux), uhy = __fmaf_rn(P.dt, f.y, uy);     // Eq. 17
-        P.uhx[p] = uhx;
-        P.uhy[p] = uhy;
-        xf = advance(xf, P.hx, __fadd_rn(uhx, ux));
-        yf = advance(yf, P.hy, __fadd_rn(uhy, uy));
-        ux = uhx;
-        uy = uhy;
-    } else if (STAGE == 1) {
-        const float uhx = P.uhx[p], uhy = P.uhy[p];
-        uint32_t xh = advance(xf, P.hx, __fadd_rn(uhx, ux));                      // x^ of Eq. 17 again
-        uint32_t yh = advance(yf, P.hy, __fadd_rn(uhy, uy));
-        decode(xh, cx, dx_);
-        decode(yh, cy, dy_);
-        if (WINDOWED && !in_window(cx, cy)) return false;
-        weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-        weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-        float2 f = WINDOWED ? gather_window(Fs, cx, cy, Wx, Wy) : gather_global(P, gx0, gy0, cx, cy, Wx, Wy);
-        float unx = __fmaf_rn(0.5f * P.dt, f.x, 0.5f * __fadd_rn(uhx, ux));       // Eq. 19
-        float uny = __fmaf_rn(0.5f * P.dt, f.y, 0.5f * __fadd_rn(uhy, uy));
-        xf = advance(xf, P.hx, __fadd_rn(unx, ux));
-        yf = advance(yf, P.hy, __fadd_rn(uny, uy));
-        // x walls reflect (Q9); y is periodic and needs nothing until the rebin
-        int64_t gx = (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS) + (int64_t)xf;
-        const int64_t wall = (int64_t)P.nx << POS_FRAC_BITS;
-        if (gx < 0) {
-            gx = -gx;
-            unx = -unx;
-        } else if (gx >= wall) {
-            gx = 2 * wall - gx;
-            if (gx >= wall) gx = wall - 1;
-            unx = -unx;
+    constexpr float INV24 = 1.0f / 16777216.0f;
+    float ux = me.ux, uy = me.uy;
+    uint32_t xd = me.x, yd = me.y;                        // deposit position
+    float Wx[4], Wy[4];
+    if (STAGE < 2) {
+        uint32_t xg = me.x, yg = me.y;                    // gather position: x^n (stage A), x^ (stage B, Q4)
+        if (STAGE == 1) {
+            xg = advance(me.x, P.hx, __fadd_rn(uhme.x, ux));
+            yg = advance(me.y, P.hy, __fadd_rn(uhme.y, uy));
         }
-        xf = (uint32_t)(gx - (((int64_t)gx0 - POS_BIAS) << POS_FRAC_BITS));
-        P.x[p] = xf;
-        P.y[p] = yf;
-        P.ux[p] = unx;
-        P.uy[p] = uny;
-        ux = unx;
-        uy = uny;
+        const int rx = (int)(xg - ax_fix), ry = (int)(yg - ay_fix);
+        if (!in_patch(rx) || !in_patch(ry)) {
+            slow_particle<SHAPE, STAGE, QMASK>(P, p, tile, gx0, gy0, Fs, dep);
+            return;
+        }
+        weights4<SHAPE>((float)rx * INV24, P, Wx);
+        weights4<SHAPE>((float)ry * INV24, P, Wy);
+        float fx = 0.f, fy = 0.f;                         // Eq. 15
+#pragma unroll
+        for (int a = 0; a < 4; a++) {
+            float sx = 0.f, sy = 0.f;
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                sx = fmaf(Wy[b], pt.Fx[a][(b + ROT) & 3], sx);
+                sy = fmaf(Wy[b], pt.Fy[a][(b + ROT) & 3], sy);
+            }
+            fx = fmaf(Wx[a], sx, fx);
+            fy = fmaf(Wx[a], sy, fy);
+        }
+        if (STAGE == 0) {
+            const float uhx = __fmaf_rn(P.dt, fx, ux), uhy = __fmaf_rn(P.dt, fy, uy);       // Eq. 17
+            P.uh[p] = make_float2(uhx, uhy);
+            xd = advance(me.x, P.hx, __fadd_rn(uhx, ux));
+            yd = advance(me.y, P.hy, __fadd_rn(uhy, uy));
+            ux = uhx;
+            uy = uhy;
+        } else {
+            float unx = __fmaf_rn(0.5f * P.dt, fx, 0.5f * __fadd_rn(uhme.x, ux));             // Eq. 19
+            float uny = __fmaf_rn(0.5f * P.dt, fy, 0.5f * __fadd_rn(uhme.y, uy));
+            xd = advance(me.x, P.hx, __fadd_rn(unx, ux));
+            yd = advance(me.y, P.hy, __fadd_rn(uny, uy));
+            reflect_x(xd, unx, gx0, P.nx);
+            PV out;
+            out.x = xd; out.y = yd; out.ux = unx; out.uy = uny;
+            P.pv[p] = out;
+            ux = unx;
+            uy = uny;
+        }
     }
-    decode(xf, cx, dx_);
-    decode(yf, cy, dy_);
-    weights3<SHAPE>(dx_, P.half_dd, P.shape_k, Wx);
-    weights3<SHAPE>(dy_, P.half_dd, P.shape_k, Wy);
-    const float w = P.w[p];
-    const float qn = w * P.nscale, qx = w * ux * P.pscale, qy = w * uy * P.pscale;
-    if (WINDOWED && in_window(cx, cy))
-        deposit_window<QMASK>(dep, cx, cy, Wx, Wy, qn, qx, qy, SHAPE == PM2D_CIC);
-    else
-        deposit_global<QMASK>(P, gx0, gy0, cx, cy, Wx, Wy, qn, qx, qy);
-    return true;
+    const int rx = (int)(xd - ax_fix), ry = (int)(yd - ay_fix);
+    if (!in_patch(rx) || !in_patch(ry)) {
+        slow_deposit<SHAPE, QMASK>(P, gx0, gy0, xd, yd, ux, uy, wme, dep);
+        return;
+    }
+    weights4<SHAPE>((float)rx * INV24, P, Wx);
+    weights4<SHAPE>((float)ry * INV24, P, Wy);
+    const float q = wme * P.nscale;                       // Eq. 14 in fixed-point units
+    const float pr = P.pscale / P.nscale;
+    const float qux = ux * pr, quy = uy * pr;
+#pragma unroll
+    for (int a = 0; a < 4; a++) {
+        const float qa = Wx[a] * q;
+        if (QMASK & 1) {
+#pragma unroll
+            for (int b = 0; b < 4; b++) pt.dn[a][(b + ROT) & 3] = fmaf(qa, Wy[b], pt.dn[a][(b + ROT) & 3]);
+        }
+        if (QMASK & 2) {
+            const float qxa = qa * qux, qya = qa * quy;
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                pt.dpx[a][(b + ROT) & 3] = fmaf(qxa, Wy[b], pt.dpx[a][(b + ROT) & 3]);
+                pt.dpy[a][(b + ROT) & 3] = fmaf(qya, Wy[b], pt.dpy[a][(b + ROT) & 3]);
+            }
+        }
+    }
 }
 
-template <int SHAPE, int STAGE, int QMASK>
-__global__ void __launch_bounds__(PTHREADS, 4) k_stage(const PartParams P)
+// flush physical column PC of the deposit patch into window column wc, rows wr0 .. wr0+3, and clear it
+template <int QMASK, int PC>
+__device__ __forceinline__ void flush_column(Patch &pt, int32_t *dep, int wr0, int wc)
 {
+#pragma unroll
+    for (int a = 0; a < 4; a++) {
+        const int e = (wr0 + a) * WPITCH + wc;
+        if (QMASK & 1) {
+            atomicAdd(&dep[e], __float2int_rn(pt.dn[a][PC]));
+            pt.dn[a][PC] = 0.f;
+        }
+        if (QMASK & 2) {
+            atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(pt.dpx[a][PC]));
+            atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(pt.dpy[a][PC]));
+            pt.dpx[a][PC] = 0.f;
+            pt.dpy[a][PC] = 0.f;
+        }
+    }
+}
+
+template <int PC>
+__device__ __forceinline__ void load_force_column(Patch &pt, const float2 *Fs, int wr0, int wc)
+{
+#pragma unroll
+    for (int a = 0; a < 4; a++) {
+        const float2 f = Fs[(wr0 + a) * WPITCH + wc];
+        pt.Fx[a][PC] = f.x;
+        pt.Fy[a][PC] = f.y;
+    }
+}
+
+constexpr int COPITCH = TILE + 1;   // odd pitch of the shared copy of the tile's cell offsets
+
+// walking state of a strip thread
+struct StripCtx {
+    int64_t p, strip_end, t0;
+    const int32_t *coff_row;     // shared: start of every cell of this thread's row; [j+1] = end of cell j
+    uint32_t ax_fix;
+    int wr0, tile, gx0, gy0;
+    const float2 *Fs;
+    int32_t *dep;
+    PV cur;                      // prefetched particle p
+    float wcur;
+    float2 uhcur;
+};
+
+// all particles of cell column j, then slide the patch to column j+1 (physical column ROT is renamed)
+template <int SHAPE, int STAGE, int QMASK, int ROT>
+__device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, StripCtx &c, const int j)
+{
+    const int64_t end = c.t0 + c.coff_row[j + 1];
+    const uint32_t ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
+    while (c.p < end) {
+        const PV me = c.cur;
+        const float wme = c.wcur;
+        const float2 uhme = c.uhcur;
+        if (c.p + 1 < c.strip_end) {
+            c.cur = P.pv[c.p + 1];
+            c.wcur = P.w[c.p + 1];
+            if (STAGE == 1) c.uhcur = P.uh[c.p + 1];
+        }
+        strip_particle<SHAPE, STAGE, QMASK, ROT>(P, pt, me, wme, uhme, c.p, c.ax_fix, ay_fix, c.tile, c.gx0, c.gy0, c.Fs, c.dep);
+        c.p++;
+    }
+    flush_column<QMASK, ROT>(pt, c.dep, c.wr0, j - 1 + HALO);              // node column j-1 is complete for this strip
+    if (STAGE < 2) load_force_column<ROT>(pt, c.Fs, c.wr0, j + 3 + HALO);
+}
+
+template <int SHAPE, int STAGE, int QMASK, int S>
+__global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const PartParams P)
+{
+    static_assert(S % 4 == 0 && TILE % S == 0, "strip length");
+    constexpr int NT = TCELLS / S;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
     // dep doubles as the scratch of build_force_window (2 (WIN+2)^2 words) before it is zeroed
     constexpr int DEPW = (STAGE < 2 && NQ * WIN * WPITCH < 2 * WF * WF) ? 2 * WF * WF : NQ * WIN * WPITCH;
     __shared__ int32_t dep[DEPW];
     __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
-    const int chunk = blockIdx.x;
-    if (chunk >= *P.nchunks) return;
-    const int tile = P.chunk_tile[chunk];
-    const int64_t beg = P.chunk_beg[chunk];
-    int64_t end = beg + CHUNK;
-    {
-        int64_t te = P.tile_off[tile + 1];
-        if (te < end) end = te;
-    }
+    __shared__ int32_t coff[TILE * COPITCH];
+    const int tile = blockIdx.x;
+    const int64_t t0 = P.tile_off[tile];
+    if (P.tile_off[tile + 1] == t0) return;
     const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
 
+    {
+        const int32_t *co = P.cell_off + (size_t)tile * CPITCH;
+        for (int e = threadIdx.x; e <= TCELLS; e += NT) {
+            const int32_t v = co[e];
+            if (e < TCELLS) coff[(e >> 5) * COPITCH + (e & 31)] = v;
+            if ((e & 31) == 0 && e > 0) coff[((e >> 5) - 1) * COPITCH + TILE] = v;   // end of the previous row
+        }
+    }
     if (STAGE < 2) build_force_window(P, gx0, gy0, reinterpret_cast<float *>(dep), dep + WF * WF, Fs);
-    for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += PTHREADS) dep[e] = 0;
+    for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
     __syncthreads();
 
-    for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
-        if (!process_particle<SHAPE, STAGE, QMASK, true>(P, p, gx0, gy0, Fs, dep)) {
-            // drifted more than HALO - 1/2 cells out of its tile since the last rebin: rare; deferred
-            int slot = atomicAdd(P.ovf_count, 1);
-            if (slot < P.ovf_cap) {
-                P.ovf_p[slot] = p;
-                P.ovf_tile[slot] = tile;
-            } else
-                P.flags[2] = 1;
-        }
+    const int r = threadIdx.x & 31, j0 = (threadIdx.x >> 5) * S;          // cell row, first cell column of the strip
+    const int wr0 = r - 1 + HALO;                                        // window row of node row r-1
+    const uint32_t ax_fix = (uint32_t)(r + POS_BIAS) << POS_FRAC_BITS;
+    // cell (r, j) -> coff[r * COPITCH + j]; its end is coff[r * COPITCH + j + 1] (slot TILE = end of the row)
+    const int cbase = r * COPITCH + j0;
+    int64_t p = t0 + coff[cbase];
+    const int64_t strip_end = t0 + coff[cbase + S];
+    Patch pt;
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) pt.dn[a][b] = pt.dpx[a][b] = pt.dpy[a][b] = pt.Fx[a][b] = pt.Fy[a][b] = 0.f;
+    if (STAGE < 2) {
+        load_force_column<0>(pt, Fs, wr0, j0 - 1 + HALO);
+        load_force_column<1>(pt, Fs, wr0, j0 + HALO);
+        load_force_column<2>(pt, Fs, wr0, j0 + 1 + HALO);
+        load_force_column<3>(pt, Fs, wr0, j0 + 2 + HALO);
+    }
+    StripCtx ctx;
+    ctx.p = p; ctx.strip_end = strip_end; ctx.t0 = t0;
+    ctx.coff_row = coff + r * COPITCH;
+    ctx.ax_fix = ax_fix; ctx.wr0 = wr0; ctx.tile = tile; ctx.gx0 = gx0; ctx.gy0 = gy0;
+    ctx.Fs = Fs; ctx.dep = dep;
+    ctx.cur = PV{0u, 0u, 0.f, 0.f};
+    ctx.wcur = 0.f;
+    ctx.uhcur = make_float2(0.f, 0.f);
+    if (p < strip_end) {
+        ctx.cur = P.pv[p];
+        ctx.wcur = P.w[p];
+        if (STAGE == 1) ctx.uhcur = P.uh[p];
+    }
+#pragma unroll 1
+    for (int kk = 0; kk < S; kk += 4) {
+        strip_cell<SHAPE, STAGE, QMASK, 0>(P, pt, ctx, j0 + kk);
+        strip_cell<SHAPE, STAGE, QMASK, 1>(P, pt, ctx, j0 + kk + 1);
+        strip_cell<SHAPE, STAGE, QMASK, 2>(P, pt, ctx, j0 + kk + 2);
+        strip_cell<SHAPE, STAGE, QMASK, 3>(P, pt, ctx, j0 + kk + 3);
+    }
+    {   // node columns j0+S-1 .. j0+S+1 (logical columns 0..2 of the cell after the strip)
+        flush_column<QMASK, 0>(pt, dep, wr0, j0 + S - 1 + HALO);
+        flush_column<QMASK, 1>(pt, dep, wr0, j0 + S + HALO);
+        flush_column<QMASK, 2>(pt, dep, wr0, j0 + S + 1 + HALO);
     }
     __syncthreads();
 
     // flush: one global integer reduction per touched window node; wall columns hold half a
     // control volume and count twice (Q9); rows beyond a wall fold back (mirror particles)
-    for (int e = threadIdx.x; e < WIN * WIN; e += PTHREADS) {
-        int r = e / WIN, cidx = e - r * WIN;
-        int se = r * WPITCH + cidx;
-        int gi = fold_x(gx0 + r - HALO, P.nx);
+    for (int e = threadIdx.x; e < WIN * WIN; e += NT) {
+        int rr = e / WIN, cidx = e - rr * WIN;
+        int se = rr * WPITCH + cidx;
+        int gi = fold_x(gx0 + rr - HALO, P.nx);
         int gj = (gy0 + cidx - HALO) & (P.ny - 1);
         int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
         size_t k = (size_t)gi * P.ny + gj;
@@ -412,7 +661,7 @@ __global__ void __launch_bounds__(128) k_stage_overflow(const PartParams P)
     const int n = min(*P.ovf_count, P.ovf_cap);
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
         const int tile = P.ovf_tile[k];
-        process_particle<SHAPE, STAGE, QMASK, false>(P, P.ovf_p[k], (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr, nullptr);
+        process_direct<SHAPE, STAGE, QMASK, false>(P, P.ovf_p[k], (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr, nullptr);
     }
 }
 
@@ -438,8 +687,8 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 struct LoadParams {
-    uint32_t *x, *y;
-    float *ux, *uy, *w;
+    PV *pv;
+    float *w;
     int64_t *id;
     const int32_t *chunk_tile;
     const int64_t *chunk_beg;
@@ -470,7 +719,8 @@ __device__ double profile_density(const LoadParams &L, int i)
     return n;
 }
 
-// one CTA per chunk; slot s of a tile with wx*wy cells holds particle k = s / cells of cell s % cells
+// one CTA per chunk; a tile with wx*wy cells stores its cells row-major, ppc particles each:
+// slot s holds particle k = s % ppc of the (s / ppc)-th cell
 __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
 {
     const double PI = 3.14159265358979323846;
@@ -482,11 +732,11 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
     int64_t end = beg + CHUNK;
     if (L.tile_off[tile + 1] < end) end = L.tile_off[tile + 1];
     const int gx0 = (tile / L.nty) * TILE, gy0 = (tile % L.nty) * TILE;
-    const int wx = min(TILE, L.nx - gx0), wy = min(TILE, L.ny - gy0);
-    const int cells = wx * wy, ppc = L.ppc_x * L.ppc_y;
+    const int wy = min(TILE, L.ny - gy0);
+    const int ppc = L.ppc_x * L.ppc_y;
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
         int s = (int)(p - t0);
-        int k = s / cells, lc = s - k * cells;
+        int lc = s / ppc, k = s - lc * ppc;
         int li = lc / wy, lj = lc - li * wy;
         int64_t cell = (int64_t)(gx0 + li) * L.ny + (gy0 + lj);
         int64_t pid = (int64_t)k * ((int64_t)L.nx * L.ny) + cell;
@@ -505,13 +755,28 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
             ux = (float)(R * cos(2.0 * PI * U2));
             uy = (float)(R * sin(2.0 * PI * U2));
         }
-        L.x[p] = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | fx24;
-        L.y[p] = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | fy24;
-        L.ux[p] = ux;
-        L.uy[p] = uy;
+        PV out;
+        out.x = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | fx24;
+        out.y = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | fy24;
+        out.ux = ux;
+        out.uy = uy;
+        L.pv[p] = out;
         L.w[p] = (float)(profile_density(L, gx0 + li) / (double)ppc);
         if (L.id) L.id[p] = pid;
     }
+}
+
+// cell offsets of the loader's order: ppc particles in every cell that exists
+__global__ void k_uniform_cell_off(int32_t *cell_off, int ntiles, int nty, int nx, int ny, int ppc)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (int64_t)ntiles * CPITCH) return;
+    const int t = (int)(e / CPITCH), c = (int)(e - (int64_t)t * CPITCH);
+    const int gx0 = (t / nty) * TILE, gy0 = (t % nty) * TILE;
+    const int wx = min(TILE, nx - gx0), wy = min(TILE, ny - gy0);
+    const int li = c >> 5, lj = c & 31;                 // c == TCELLS: li = 32
+    const int before = li < wx ? li * wy + min(lj, wy) : wx * wy;
+    cell_off[e] = ppc * before;
 }
 
 // ---- single-CTA scans over tiles ----------------------------------------------------------------
@@ -598,13 +863,13 @@ __global__ void k_uniform_tile_counts(int32_t *cnt, int ntx, int nty, int nx, in
     cnt[t] = ppc * min(TILE, nx - gx0) * min(TILE, ny - gy0);
 }
 
-// ---- rebin ---------------------------------------------------------------------------------------
+// ---- rebin, pass 1: stable move between neighbouring tiles ------------------------------------------
 struct RebinParams {
-    const uint32_t *x, *y;
-    const float *ux, *uy, *w;
+    const PV *pv;
+    const float *w;
     const int64_t *id;
-    uint32_t *x2, *y2;
-    float *ux2, *uy2, *w2;
+    PV *pv2;
+    float *w2;
     int64_t *id2;
     const int32_t *chunk_tile;
     const int64_t *chunk_beg;
@@ -616,8 +881,7 @@ struct RebinParams {
     int64_t *rel9;
     int32_t *newcount;
     int32_t *flags;
-    int32_t *keys_out;
-    int64_t *perm_out;
+    int64_t *perm1;        // optional: for every slot after pass 1, the slot before it
     int nx, ny, ntx, nty;
 };
 
@@ -654,7 +918,8 @@ __global__ void __launch_bounds__(PTHREADS) k_rebin_count(const RebinParams R)
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
         int dti, dtj;
         bool bad;
-        int slot = rebin_slot(R, gx0, gy0, R.x[p], R.y[p], dti, dtj, bad);
+        const uint2 xy = *reinterpret_cast<const uint2 *>(&R.pv[p]);
+        int slot = rebin_slot(R, gx0, gy0, xy.x, xy.y, dti, dtj, bad);
         anybad |= bad;
 #pragma unroll
         for (int s = 0; s < 9; s++) local[s] += (slot == s);
@@ -671,7 +936,7 @@ __global__ void __launch_bounds__(PTHREADS) k_rebin_count(const RebinParams R)
 }
 
 // one thread per destination tile: walk its (<= 9) source tiles in ascending key order, chunk by
-// chunk, handing out offsets -> the new order is the stable counting sort of the old array by key
+// chunk, handing out offsets -> the new order is the stable counting sort of the old array by tile
 __global__ void k_rebin_offsets(const RebinParams R)
 {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -722,12 +987,11 @@ __global__ void __launch_bounds__(PTHREADS) k_rebin_scatter(const RebinParams R)
         const int64_t p = base + threadIdx.x;
         const bool live = p < end;
         int slot = 9, dti = 0, dtj = 0;
-        uint32_t xf = 0, yf = 0;
+        PV me = {0u, 0u, 0.f, 0.f};
         bool bad = false;
         if (live) {
-            xf = R.x[p];
-            yf = R.y[p];
-            slot = rebin_slot(R, gx0, gy0, xf, yf, dti, dtj, bad);
+            me = R.pv[p];
+            slot = rebin_slot(R, gx0, gy0, me.x, me.y, dti, dtj, bad);
         }
         if (lane < 10) wcnt[wid][lane] = 0;
         __syncthreads();
@@ -744,14 +1008,12 @@ __global__ void __launch_bounds__(PTHREADS) k_rebin_scatter(const RebinParams R)
             int dest = ti * R.nty + tj;
             int64_t q = R.tile_off2[dest] + off;
             if (bad) q = p;   // flagged by k_rebin_count; keep memory safe
-            R.x2[q] = xf - ((uint32_t)(dti * TILE) << POS_FRAC_BITS);
-            R.y2[q] = yf - ((uint32_t)(dtj * th) << POS_FRAC_BITS);
-            R.ux2[q] = R.ux[p];
-            R.uy2[q] = R.uy[p];
+            me.x -= (uint32_t)(dti * TILE) << POS_FRAC_BITS;
+            me.y -= (uint32_t)(dtj * th) << POS_FRAC_BITS;
+            R.pv2[q] = me;
             R.w2[q] = R.w[p];
             if (R.id) R.id2[q] = R.id[p];
-            if (R.keys_out) R.keys_out[p] = dest;
-            if (R.perm_out) R.perm_out[q] = p;
+            if (R.perm1) R.perm1[q] = p;
         }
         __syncthreads();
         if (threadIdx.x < 9) {
@@ -763,11 +1025,116 @@ __global__ void __launch_bounds__(PTHREADS) k_rebin_scatter(const RebinParams R)
     }
 }
 
-// canonical (ix, iy, fx, fy) of the particles of each chunk
-__global__ void __launch_bounds__(PTHREADS) k_unpack(const uint32_t *x, const uint32_t *y, const int32_t *chunk_tile,
-                                                     const int64_t *chunk_beg, const int64_t *tile_off,
-                                                     const int32_t *nchunks, int nty, int ny, int32_t *ix, int32_t *iy,
-                                                     float *fx, float *fy)
+// ---- rebin, pass 2: stable counting sort by cell inside every tile -----------------------------------
+// One CTA per tile.  Each warp owns a contiguous part of the tile's list; per-warp histograms, one scan
+// over (cell, warp), then every warp ranks its particles batch by batch with match_any -- the result is
+// the stable sort by cell of the pass-1 order, hence (with pass 1) the stable sort by (tile, cell).
+struct CellSortParams {
+    const PV *src;
+    const float *wsrc;
+    const int64_t *idsrc;
+    PV *dst;
+    float *wdst;
+    int64_t *iddst;
+    const int64_t *tile_off;   // offsets of the pass-1 order (= of the result)
+    int32_t *cell_off;
+    const int64_t *perm1;      // optional (tests)
+    int32_t *keys_out;         // optional: destination key of every particle, in the order before pass 1
+    int64_t *perm_out;         // optional: for every final slot the slot before pass 1
+};
+
+constexpr int CS_WARPS = 8;
+
+__device__ __forceinline__ int cell_of(uint32_t xf, uint32_t yf)
+{
+    int cx = (int)(xf >> POS_FRAC_BITS) - POS_BIAS, cy = (int)(yf >> POS_FRAC_BITS) - POS_BIAS;
+    cx = max(0, min(TILE - 1, cx));
+    cy = max(0, min(TILE - 1, cy));
+    return cx * TILE + cy;
+}
+
+__global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams C)
+{
+    __shared__ int32_t hist[CS_WARPS * TCELLS];
+    __shared__ int32_t wsum[CS_WARPS];
+    const int tile = blockIdx.x;
+    const int64_t t0 = C.tile_off[tile];
+    const int64_t n = C.tile_off[tile + 1] - t0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int32_t *co = C.cell_off + (size_t)tile * CPITCH;
+    for (int e = threadIdx.x; e < CS_WARPS * TCELLS; e += CS_WARPS * 32) hist[e] = 0;
+    __syncthreads();
+    int64_t per = (n + CS_WARPS - 1) / CS_WARPS;
+    per = (per + 31) & ~(int64_t)31;
+    const int64_t beg = min(n, wid * per), end = min(n, beg + per);
+    int32_t *myhist = hist + wid * TCELLS;
+    for (int64_t i = beg + lane; i < end; i += 32) {
+        const uint2 xy = *reinterpret_cast<const uint2 *>(&C.src[t0 + i]);
+        atomicAdd(&myhist[cell_of(xy.x, xy.y)], 1);
+    }
+    __syncthreads();
+    {   // exclusive scan over (cell, warp): thread t owns cells 4t .. 4t+3
+        const int c0 = threadIdx.x * (TCELLS / (CS_WARPS * 32));
+        int s = 0;
+        for (int c = c0; c < c0 + TCELLS / (CS_WARPS * 32); c++)
+            for (int w = 0; w < CS_WARPS; w++) s += hist[w * TCELLS + c];
+        int incl = s;
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) wsum[wid] = incl;
+        __syncthreads();
+        int run = incl - s;
+        for (int w = 0; w < wid; w++) run += wsum[w];
+        for (int c = c0; c < c0 + TCELLS / (CS_WARPS * 32); c++) {
+            co[c] = run;
+            for (int w = 0; w < CS_WARPS; w++) {
+                int v = hist[w * TCELLS + c];
+                hist[w * TCELLS + c] = run;
+                run += v;
+            }
+        }
+        if (threadIdx.x == CS_WARPS * 32 - 1) co[TCELLS] = run;
+    }
+    __syncthreads();
+    for (int64_t base = beg; base < end; base += 32) {
+        const int64_t i = base + lane;
+        const bool live = i < end;
+        PV me = {0u, 0u, 0.f, 0.f};
+        int c = TCELLS + lane;                       // dead lanes: unique keys
+        if (live) {
+            me = C.src[t0 + i];
+            c = cell_of(me.x, me.y);
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
+        const int rank = __popc(peers & ((1u << lane) - 1u));
+        const int leader = __ffs(peers) - 1;
+        int b = 0;
+        if (live && lane == leader) {
+            b = myhist[c];
+            myhist[c] = b + __popc(peers);
+        }
+        b = __shfl_sync(0xffffffffu, b, leader);
+        __syncwarp();
+        if (live) {
+            const int64_t q = t0 + b + rank;
+            C.dst[q] = me;
+            C.wdst[q] = C.wsrc[t0 + i];
+            if (C.idsrc) C.iddst[q] = C.idsrc[t0 + i];
+            if (C.perm1) {
+                const int64_t old = C.perm1[t0 + i];
+                if (C.keys_out) C.keys_out[old] = tile * TCELLS + c;
+                if (C.perm_out) C.perm_out[q] = old;
+            }
+        }
+    }
+}
+
+// canonical (ix, iy, fx, fy) and velocity of the particles of each chunk, as separate arrays
+__global__ void __launch_bounds__(PTHREADS) k_unpack(const PV *pv, const int32_t *chunk_tile, const int64_t *chunk_beg,
+                                                     const int64_t *tile_off, const int32_t *nchunks, int nty, int ny, int32_t *ix,
+                                                     int32_t *iy, float *fx, float *fy, float *ux, float *uy)
 {
     const int chunk = blockIdx.x;
     if (chunk >= *nchunks) return;
@@ -777,11 +1144,13 @@ __global__ void __launch_bounds__(PTHREADS) k_unpack(const uint32_t *x, const ui
     if (tile_off[tile + 1] < end) end = tile_off[tile + 1];
     const int gx0 = (tile / nty) * TILE, gy0 = (tile % nty) * TILE;
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
-        uint32_t xf = x[p], yf = y[p];
-        ix[p] = gx0 + (int)(xf >> POS_FRAC_BITS) - POS_BIAS;
-        iy[p] = (gy0 + (int)(yf >> POS_FRAC_BITS) - POS_BIAS) & (ny - 1);
-        fx[p] = (float)(xf & POS_FRAC_MASK) * (1.0f / 16777216.0f);
-        fy[p] = (float)(yf & POS_FRAC_MASK) * (1.0f / 16777216.0f);
+        const PV me = pv[p];
+        ix[p] = gx0 + (int)(me.x >> POS_FRAC_BITS) - POS_BIAS;
+        iy[p] = (gy0 + (int)(me.y >> POS_FRAC_BITS) - POS_BIAS) & (ny - 1);
+        fx[p] = (float)(me.x & POS_FRAC_MASK) * (1.0f / 16777216.0f);
+        fy[p] = (float)(me.y & POS_FRAC_MASK) * (1.0f / 16777216.0f);
+        ux[p] = me.ux;
+        uy[p] = me.uy;
     }
 }
 
@@ -793,8 +1162,8 @@ static PartParams make_part_params(pm2d_ctx *c, int s, const float *a_level)
 {
     SpeciesDev &S = c->sp[s];
     PartParams P;
-    P.x = S.x; P.y = S.y; P.ux = S.ux; P.uy = S.uy; P.uhx = S.uhx; P.uhy = S.uhy; P.w = S.w;
-    P.chunk_tile = S.chunk_tile; P.chunk_beg = S.chunk_beg; P.tile_off = S.tile_off; P.nchunks = S.nchunks_dev;
+    P.pv = S.pv; P.uh = S.uh; P.w = S.w;
+    P.tile_off = S.tile_off; P.cell_off = S.cell_off;
     P.F = S.F; P.Enode = c->Enode; P.a = a_level; P.ncomp = c->g.ncomp;
     P.qE = (float)(-(double)S.cfg.sign * 4.0 * 3.14159265358979323846 * 3.14159265358979323846 / S.cfg.mass);
     P.pond = S.cfg.sign < 0 ? 1.f : 0.f;
@@ -809,17 +1178,20 @@ static PartParams make_part_params(pm2d_ctx *c, int s, const float *a_level)
     P.hy = (float)(c->g.dt / (2.0 * c->g.dy));
     P.nscale = c->nscale; P.pscale = c->pscale;
     P.half_dd = (float)(0.5 * S.cfg.DD);
-    P.shape_k = (float)(0.5 / S.cfg.DD);
+    P.dd = (float)S.cfg.DD;
+    P.k_rad = (float)(3.14159265358979323846 / S.cfg.DD);
     return P;
 }
+
+constexpr int STRIP = 8;   // cells per strip thread: 128 threads per tile
 
 template <int SHAPE>
 static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, cudaStream_t st)
 {
-#define PM2D_LAUNCH(ST, Q)                                        \
-    do {                                                          \
-        k_stage<SHAPE, ST, Q><<<grid, PTHREADS, 0, st>>>(P);      \
-        if (ST < 2) k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P); \
+#define PM2D_LAUNCH(ST, Q)                                                         \
+    do {                                                                           \
+        k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);          \
+        if (ST < 2) k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P);        \
     } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }
     else if (stage == 1) { if (qmask == 3) PM2D_LAUNCH(1, 3); else PM2D_LAUNCH(1, 1); }
@@ -832,7 +1204,6 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
     PartParams P = make_part_params(c, s, stage == 0 ? c->a[1] : c->a[0]);
-    const int grid = S.max_chunks;
     if (stage < 2) {
         // the force window reads n_s while other CTAs already deposit: ping-pong the density grid
         const size_t bytes = (size_t)c->nn * sizeof(int32_t);
@@ -844,9 +1215,9 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
             PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
         }
     }
-    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, grid, c->stream);
-    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, grid, c->stream);
-    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, grid, c->stream);
+    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, c->stream);
+    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, c->stream);
+    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, c->stream);
     count_launch(c, stage < 2 ? 2 : 1);
     PM2D_CUDA_CHECK(cudaGetLastError());
     if (stage < 2) std::swap(S.nfix, S.nfix2);
@@ -881,11 +1252,13 @@ int launch_load_particles(pm2d_ctx *c, int s)
     const int ppc = S.cfg.ppc_x * S.cfg.ppc_y;
     k_uniform_tile_counts<<<(c->ntiles + 255) / 256, 256, 0, c->stream>>>(S.tile_cnt, c->ntx, c->nty, c->g.nx, c->g.ny, ppc);
     k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off);
-    count_launch(c, 2);
+    const int64_t ncell = (int64_t)c->ntiles * CPITCH;
+    k_uniform_cell_off<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>(S.cell_off, c->ntiles, c->nty, c->g.nx, c->g.ny, ppc);
+    count_launch(c, 3);
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
     LoadParams L;
-    L.x = S.x; L.y = S.y; L.ux = S.ux; L.uy = S.uy; L.w = S.w; L.id = S.id;
+    L.pv = S.pv; L.w = S.w; L.id = S.id;
     L.chunk_tile = S.chunk_tile; L.chunk_beg = S.chunk_beg; L.tile_off = S.tile_off; L.nchunks = S.nchunks_dev;
     L.nx = c->g.nx; L.ny = c->g.ny; L.nty = c->nty;
     L.ppc_x = S.cfg.ppc_x; L.ppc_y = S.cfg.ppc_y; L.load = S.cfg.load; L.species = s;
@@ -899,40 +1272,42 @@ int launch_load_particles(pm2d_ctx *c, int s)
     return PM2D_OK;
 }
 
-int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev)
+// keys_dev / perm_dev: optional outputs of the test entry point pm2d_rebin; perm_tmp_dev: scratch of np
+// int64, required when either is given
+int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64_t *perm_tmp_dev)
 {
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
     RebinParams R;
-    R.x = S.x; R.y = S.y; R.ux = S.ux; R.uy = S.uy; R.w = S.w; R.id = S.id;
-    R.x2 = S.x2; R.y2 = S.y2; R.ux2 = S.uhx; R.uy2 = S.uhy; R.w2 = S.w2; R.id2 = S.id2;
+    R.pv = S.pv; R.w = S.w; R.id = S.id;
+    R.pv2 = S.pv2; R.w2 = S.w2; R.id2 = S.id2;
     R.chunk_tile = S.chunk_tile; R.chunk_beg = S.chunk_beg; R.tile_off = S.tile_off; R.tile_off2 = S.tile_off2;
     R.nchunks = S.nchunks_dev; R.tile_first_chunk = S.tile_first_chunk;
     R.cnt9 = S.chunk_cnt9; R.rel9 = S.chunk_rel9; R.newcount = S.tile_cnt; R.flags = c->flags;
-    R.keys_out = keys_dev; R.perm_out = perm_dev;
+    R.perm1 = (keys_dev || perm_dev) ? perm_tmp_dev : nullptr;
     R.nx = c->g.nx; R.ny = c->g.ny; R.ntx = c->ntx; R.nty = c->nty;
     k_rebin_count<<<S.max_chunks, PTHREADS, 0, c->stream>>>(R);
     k_rebin_offsets<<<(c->ntiles + 127) / 128, 128, 0, c->stream>>>(R);
     k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off2);
     k_rebin_scatter<<<S.max_chunks, PTHREADS, 0, c->stream>>>(R);
-    count_launch(c, 4);
+    CellSortParams C;
+    C.src = S.pv2; C.wsrc = S.w2; C.idsrc = S.id ? S.id2 : nullptr;
+    C.dst = S.pv; C.wdst = S.w; C.iddst = S.id;
+    C.tile_off = S.tile_off2; C.cell_off = S.cell_off;
+    C.perm1 = R.perm1; C.keys_out = keys_dev; C.perm_out = perm_dev;
+    k_cellsort<<<c->ntiles, CS_WARPS * 32, 0, c->stream>>>(C);
+    count_launch(c, 5);
     PM2D_CUDA_CHECK(cudaGetLastError());
-    std::swap(S.x, S.x2);
-    std::swap(S.y, S.y2);
-    std::swap(S.w, S.w2);
-    std::swap(S.ux, S.uhx);
-    std::swap(S.uy, S.uhy);
-    std::swap(S.id, S.id2);
     std::swap(S.tile_off, S.tile_off2);
     return launch_build_chunks(c, s);
 }
 
-int launch_unpack_particles(pm2d_ctx *c, int s, int64_t, int64_t, int32_t *ix, int32_t *iy, float *fx, float *fy)
+int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float *fx, float *fy, float *ux, float *uy)
 {
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
-    k_unpack<<<S.max_chunks, PTHREADS, 0, c->stream>>>(S.x, S.y, S.chunk_tile, S.chunk_beg, S.tile_off, S.nchunks_dev, c->nty,
-                                                        c->g.ny, ix, iy, fx, fy);
+    k_unpack<<<S.max_chunks, PTHREADS, 0, c->stream>>>(S.pv, S.chunk_tile, S.chunk_beg, S.tile_off, S.nchunks_dev, c->nty, c->g.ny,
+                                                        ix, iy, fx, fy, ux, uy);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;

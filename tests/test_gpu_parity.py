@@ -170,15 +170,23 @@ def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin):
 
 
 def test_rebin_is_a_stable_counting_sort(P):
+    """Rebin as a pure function of the device's own state (Q12): key = (tile, cell in tile),
+    permutation = the stable counting sort by that key; both bit-exact."""
     cfg = small_cfg("c3", 136, 128, rebin_every=0)
     for sp in cfg["species"]:
-        sp["T_keV"] *= 40.0                                   # fast particles: many tile crossings
+        sp["T_keV"] *= 40.0                                   # fast particles: many tile and cell crossings
     sim = P.PM2D(cfg, track_ids=1, rebin_every=0)
-    nty = (128 + P.TILE - 1) // P.TILE
+    T = P.TILE
+    nty = (128 + T - 1) // T
+    ntx = (136 + T - 1) // T
+
+    def key_of(pp):
+        return ((pp["ix"] // T) * nty + pp["iy"] // T).astype(np.int64) * (T * T) + (pp["ix"] % T) * T + pp["iy"] % T
+
     for rounds in range(3):
         sim.step(3)
         before = sim.get_particles(0, with_id=True)
-        key_ref = (before["ix"] // P.TILE) * nty + before["iy"] // P.TILE
+        key_ref = key_of(before)
         keys, perm = sim.rebin(0)
         assert np.array_equal(keys, key_ref.astype(np.int32))
         perm_ref = np.argsort(key_ref, kind="stable")
@@ -186,9 +194,12 @@ def test_rebin_is_a_stable_counting_sort(P):
         after = sim.get_particles(0, with_id=True)
         for k in before:
             assert np.array_equal(after[k], before[k][perm_ref]), k
-        hist = np.bincount(key_ref, minlength=nty * ((136 + P.TILE - 1) // P.TILE))
+        hist = np.bincount(key_ref // (T * T), minlength=nty * ntx)
         assert hist.sum() == before["ix"].size
-        assert (np.diff((after["ix"] // P.TILE) * nty + after["iy"] // P.TILE) >= 0).all()
+        assert (np.diff(key_of(after)) >= 0).all()
+    # a second rebin of an already sorted state is the identity
+    keys, perm = sim.rebin(0)
+    assert np.array_equal(perm, np.arange(perm.size))
     sim.close()
 
 
