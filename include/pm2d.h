@@ -174,6 +174,10 @@ int pm2d_profile_enable(pm2d_ctx *ctx, int on);
 int pm2d_profile_get(pm2d_ctx *ctx, double ms[PM2D_PH_COUNT], int64_t launches[PM2D_PH_COUNT], int64_t *steps);
 /* Kernels launched by this ctx since init. */
 int64_t pm2d_launch_count(pm2d_ctx *ctx);
+/* Statistics: particle-stage visits, since the last call, that were not served from a strip thread's
+ * register patch (the particle had drifted more than half a cell from its cell of the last rebin) but
+ * from the tile's shared windows or the global grids.  Synchronises the stream; resets the counter. */
+int64_t pm2d_stray_count(pm2d_ctx *ctx);
 
 void pm2d_free(pm2d_ctx *ctx);
 const char *pm2d_last_error(void);

@@ -75,6 +75,7 @@ SYMBOLS = {
     "pm2d_profile_enable": (C.c_int, [_vp, C.c_int]),
     "pm2d_profile_get": (C.c_int, [_vp, C.POINTER(C.c_double), _lp, _lp]),
     "pm2d_launch_count": (C.c_int64, [_vp]),
+    "pm2d_stray_count": (C.c_int64, [_vp]),
     "pm2d_free": (None, [_vp]),
     "pm2d_last_error": (C.c_char_p, []),
     "pm2d_version": (C.c_char_p, []),
@@ -262,3 +263,6 @@ class PM2D:
 
     def launch_count(self):
         return int(self.lib.pm2d_launch_count(self.ctx))
+
+    def stray_count(self):
+        return int(_check(self.lib.pm2d_stray_count(self.ctx)))

@@ -3,6 +3,7 @@
 // except the laser carrier phases handed to the boundary kernel (pm2d_fields.cu).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -104,6 +105,7 @@ size_t layout(pm2d_ctx *c, char *base)
     c->twiddle = cv.take<float2>(g.ny / 2);
     c->red = cv.take<double>(64);
     c->flags = cv.take<int32_t>(4);
+    c->stray_total = cv.take<unsigned long long>(1);
     c->ovf_cap = 1 << 20;
     c->ovf_p = cv.take<int64_t>(c->ovf_cap);
     c->ovf_tile = cv.take<int32_t>(c->ovf_cap);
@@ -114,7 +116,6 @@ size_t layout(pm2d_ctx *c, char *base)
         S.pxfix = S.pyfix = nullptr; S.F = nullptr;
         S.np = S.cap = species_np(g, S.cfg);
         if (!S.cfg.mobile) continue;
-        S.nfix2 = cv.take<int32_t>(nn);
         S.pxfix = cv.take<int32_t>(nn);
         S.pyfix = cv.take<int32_t>(nn);
         S.F = cv.take<float2>(nn);
@@ -257,6 +258,8 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     c->seed = seed;
     c->stream = (cudaStream_t)cuda_stream;
     c->step = 0;
+    c->cap_extra = 0;
+    if (const char *e = getenv("PM2D_CAP_EXTRA")) c->cap_extra = atoi(e);
     c->prof_on = false;
     c->cur_phase = -1;
     c->launches = 0;
@@ -342,8 +345,12 @@ static int enqueue_step(pm2d_ctx *c)
         phase_begin(c, PM2D_PH_POISSON);
         if ((rc = launch_poisson(c, false))) return rc;
         phase_end(c);
-        // (3)-(5) force of Eq. 16 with a^n built per tile, gather, predictor, deposit /
-        // (7)-(8)+(1) force of Eq. 18 with a^{n+1}, gather, corrector, deposit -- one fused kernel
+        // (3) / (7): nodal force of Eq. 16 with a^n, n^n, E^n / of Eq. 18 with a^{n+1}, n^, E^
+        phase_begin(c, PM2D_PH_FORCE);
+        for (int s = 0; s < c->nsp; s++)
+            if (c->sp[s].cfg.mobile && c->sp[s].np > 0 && (rc = launch_force(c, s, stage == 0 ? c->a[1] : c->a[0]))) return rc;
+        phase_end(c);
+        // (3)-(5) gather, predictor, deposit / (7)-(8)+(1) gather, corrector, deposit -- one fused kernel
         phase_begin(c, stage == 0 ? PM2D_PH_STAGE_A : PM2D_PH_STAGE_B);
         for (int s = 0; s < c->nsp; s++)
             if (c->sp[s].cfg.mobile && (rc = launch_stage(c, s, stage))) return rc;
@@ -382,6 +389,16 @@ extern "C" int pm2d_step(pm2d_ctx *c, int nsteps)
 }
 
 extern "C" int64_t pm2d_launch_count(pm2d_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int64_t pm2d_stray_count(pm2d_ctx *c)
+{
+    if (!c) return fail(PM2D_EINVAL, "null ctx");
+    unsigned long long h = 0;
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(&h, c->stray_total, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->stray_total, 0, sizeof(h), c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return (int64_t)h;
+}
 extern "C" int64_t pm2d_particle_count(pm2d_ctx *c, int s) { return (c && s >= 0 && s < c->nsp) ? c->sp[s].np : -1; }
 
 extern "C" int pm2d_profile_enable(pm2d_ctx *c, int on)

@@ -121,30 +121,40 @@ __device__ __forceinline__ float a2_at(const ForceParams &P, size_t k, size_t nn
     return s;
 }
 
-__global__ void __launch_bounds__(256) k_force(const ForceParams P)
+// CTA = 128 columns x GROWS rows; each thread marches along x keeping |a|^2 and n of rows i-1, i, i+1 in
+// registers (central x-differences, one-sided on the wall rows); the y neighbours come through L1.
+constexpr int GCOLS = 128, GROWS = 32;
+__global__ void __launch_bounds__(GCOLS) k_force(const ForceParams P)
 {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    const int i = blockIdx.y;
+    const int j = blockIdx.x * GCOLS + threadIdx.x;
     if (j >= P.ny) return;
+    const int i0 = blockIdx.y * GROWS, i1 = min(P.nx + 1, i0 + GROWS);
     const size_t nn = (size_t)(P.nx + 1) * P.ny;
     const int jm = (j - 1) & (P.ny - 1), jp = (j + 1) & (P.ny - 1);
-    const int il = i > 0 ? i - 1 : 0, ih = i < P.nx ? i + 1 : P.nx;
-    const float sx = (il == i || ih == i) ? 2.f * P.inv_2dx : P.inv_2dx;     // one-sided at the walls
-    const size_t k = (size_t)i * P.ny + j, kl = (size_t)il * P.ny + j, kh = (size_t)ih * P.ny + j;
-    const size_t kd = (size_t)i * P.ny + jm, ku = (size_t)i * P.ny + jp;
-    float2 E = P.Enode[k];
-    float fx = P.qE * E.x, fy = P.qE * E.y;
-    if (P.pond != 0.f) {
-        fx -= 0.5f * sx * (a2_at(P, kh, nn) - a2_at(P, kl, nn));
-        fy -= 0.5f * P.inv_2dy * (a2_at(P, ku, nn) - a2_at(P, kd, nn));
+    const bool pond = P.pond != 0.f, press = P.cv2 != 0.f;
+    const size_t rlo = (size_t)(i0 > 0 ? i0 - 1 : 0) * P.ny, r0 = (size_t)i0 * P.ny;
+    float a_lo = pond ? a2_at(P, rlo + j, nn) : 0.f, a_mid = pond ? a2_at(P, r0 + j, nn) : 0.f;
+    int n_lo = P.nfix[rlo + j], n_mid = P.nfix[r0 + j];
+    for (int i = i0; i < i1; i++) {
+        const size_t row = (size_t)i * P.ny, rhi = (size_t)(i < P.nx ? i + 1 : P.nx) * P.ny;
+        const float a_hi = pond ? a2_at(P, rhi + j, nn) : 0.f;
+        const int n_hi = P.nfix[rhi + j];
+        const float sx = (i == 0 || i == P.nx) ? 2.f * P.inv_2dx : P.inv_2dx;     // one-sided at the walls
+        const float2 E = P.Enode[row + j];
+        float fx = P.qE * E.x, fy = P.qE * E.y;
+        if (pond) {
+            fx -= 0.5f * sx * (a_hi - a_lo);
+            fy -= 0.5f * P.inv_2dy * (a2_at(P, row + jp, nn) - a2_at(P, row + jm, nn));
+        }
+        if (n_mid > 0 && press) {
+            const float inv_n = 1.f / (float)n_mid;
+            fx -= P.cv2 * sx * (float)(n_hi - n_lo) * inv_n;
+            fy -= P.cv2 * P.inv_2dy * (float)(P.nfix[row + jp] - P.nfix[row + jm]) * inv_n;
+        }
+        P.F[row + j] = make_float2(fx, fy);
+        a_lo = a_mid; a_mid = a_hi;
+        n_lo = n_mid; n_mid = n_hi;
     }
-    const int n0 = P.nfix[k];
-    if (n0 > 0 && P.cv2 != 0.f) {
-        const float inv_n = 1.f / (float)n0;
-        fx -= P.cv2 * sx * (float)(P.nfix[kh] - P.nfix[kl]) * inv_n;
-        fy -= P.cv2 * P.inv_2dy * (float)(P.nfix[ku] - P.nfix[kd]) * inv_n;
-    }
-    P.F[k] = make_float2(fx, fy);
 }
 
 __global__ void k_fix_to_float(const int32_t *src, float scale, float *dst, size_t n)
@@ -229,8 +239,8 @@ int launch_force(pm2d_ctx *c, int s, const float *a_level)
     P.cv2 = (float)(S.cfg.pressure_coeff * S.vth2);
     P.inv_2dx = (float)(1.0 / (2.0 * c->g.dx));
     P.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
-    dim3 grid((c->g.ny + 255) / 256, c->g.nx + 1);
-    k_force<<<grid, 256, 0, c->stream>>>(P);
+    dim3 grid((c->g.ny + GCOLS - 1) / GCOLS, (c->g.nx + 1 + GROWS - 1) / GROWS);
+    k_force<<<grid, GCOLS, 0, c->stream>>>(P);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;

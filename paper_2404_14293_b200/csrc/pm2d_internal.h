@@ -57,7 +57,6 @@ struct SpeciesDev {
     int32_t nchunks;     // host copy (refreshed after a rebin)
     // grids (device)
     int32_t *nfix;       // density, fixed point, [(nx+1)*ny] (current)
-    int32_t *nfix2;      // the other half of the ping-pong (mobile species)
     int32_t *pxfix, *pyfix;
     float2 *F;           // nodal force (Eq. 16)
 };
@@ -89,9 +88,11 @@ struct pm2d_ctx {
     float2 *twiddle;     // [ny/2]
     double *red;         // [64] reduction scratch
     int32_t *flags;      // [4] device error flags
+    unsigned long long *stray_total; // [1] statistics
     int64_t *ovf_p;      // [ovf_cap] particles deferred by k_stage (footprint outside the tile window)
     int32_t *ovf_tile, *ovf_count;
     int ovf_cap;
+    int cap_extra;       // tuning: see PartParams::cap_extra
     // profile
     bool prof_on;
     std::vector<cudaEvent_t> ev;   // 2 per phase per step, reused ring

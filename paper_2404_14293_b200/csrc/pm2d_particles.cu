@@ -39,15 +39,10 @@ struct PartParams {
     const int64_t *tile_off;
     const int32_t *cell_off;
     // grids
-    const float2 *F;          // materialised force grid (diagnostics only); may be NULL
-    const float2 *Enode;      // nodal E of the last Poisson solve
-    const float *a;           // [ncomp][nn], level n (stage A) or n+1 (stage B)
-    int ncomp;
-    float qE, pond, cv2;      // -sign 4 pi^2 / m ; 1 for electrons ; C v_th^2
-    float inv_2dx, inv_2dy;
-    const int32_t *nfix_in;   // density the force is built from (n^n or n^); the deposit goes to nfix
+    const float2 *F;          // nodal force of this species, Eq. 16 (stage A) / Eq. 18 (stage B)
     int32_t *nfix, *pxfix, *pyfix;
     int32_t *flags;
+    unsigned long long *stray_total;   // statistics: particles served outside the register patch
     int64_t *ovf_p;           // overflow list: particles whose gather footprint left the tile window
     int32_t *ovf_tile, *ovf_count;
     int ovf_cap;
@@ -57,6 +52,7 @@ struct PartParams {
     float half_dd;           // DD / 2
     float dd;                // DD
     float k_rad;             // pi / DD  (sine: G(t) = 1/2 - 1/2 cos(k_rad t))
+    int cap_extra;           // cell_cap = ceil(mean particles per cell of the tile) + cap_extra
 };
 
 __device__ __forceinline__ int fold_x(int i, int nx)
@@ -207,38 +203,6 @@ __device__ __forceinline__ void deposit_direct(const PartParams &P, int gx0, int
     }
 }
 
-// Eq. 16 at one global node (overflow path only)
-__device__ __forceinline__ float2 force_at_node(const PartParams &P, int gi, int gj)
-{
-    const size_t nn = (size_t)(P.nx + 1) * P.ny;
-    const int il = gi > 0 ? gi - 1 : 0, ih = gi < P.nx ? gi + 1 : P.nx;
-    const float sx = (il == gi || ih == gi) ? 2.f * P.inv_2dx : P.inv_2dx;
-    const int jm = (gj - 1) & (P.ny - 1), jp = (gj + 1) & (P.ny - 1);
-    const size_t k = (size_t)gi * P.ny + gj, kl = (size_t)il * P.ny + gj, kh = (size_t)ih * P.ny + gj;
-    const size_t kd = (size_t)gi * P.ny + jm, ku = (size_t)gi * P.ny + jp;
-    float2 E = P.Enode[k];
-    float fx = P.qE * E.x, fy = P.qE * E.y;
-    if (P.pond != 0.f) {
-        float ah = 0.f, al = 0.f, au = 0.f, ad = 0.f;
-        for (int c = 0; c < P.ncomp; c++) {
-            float v;
-            v = P.a[c * nn + kh]; ah += v * v;
-            v = P.a[c * nn + kl]; al += v * v;
-            v = P.a[c * nn + ku]; au += v * v;
-            v = P.a[c * nn + kd]; ad += v * v;
-        }
-        fx -= 0.5f * sx * (ah - al);
-        fy -= 0.5f * P.inv_2dy * (au - ad);
-    }
-    const int n0 = P.nfix_in[k];
-    if (n0 > 0 && P.cv2 != 0.f) {
-        const float inv_n = 1.f / (float)n0;
-        fx -= P.cv2 * sx * (float)(P.nfix_in[kh] - P.nfix_in[kl]) * inv_n;
-        fy -= P.cv2 * P.inv_2dy * (float)(P.nfix_in[ku] - P.nfix_in[kd]) * inv_n;
-    }
-    return make_float2(fx, fy);
-}
-
 // Eq. 15 on 3 x 3 nodes around the nearest node: from the shared force window, or (overflow path)
 // from forces evaluated on the global grids
 template <int SHAPE, bool WINDOWED>
@@ -274,7 +238,7 @@ __device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, in
 #pragma unroll 1
             for (int b = 0; b < 3; b++) {
                 int gj = (gy0 + cy - 1 + b) & (P.ny - 1);
-                float2 f = force_at_node(P, gi, gj);
+                float2 f = P.F[(size_t)gi * P.ny + gj];
                 float ww = Wx[a] * Wy[b];
                 fx += ww * f.x;
                 fy += ww * f.y;
@@ -286,25 +250,37 @@ __device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, in
 
 // One particle through one stage outside the register patch.  STAGE 0: predictor (Eq. 17); STAGE 1:
 // corrector (Eq. 19) + particle boundaries; STAGE 2: deposit only.  QMASK bit 0: density, bit 1: momentum.
-// WINDOWED: shared windows; returns false (nothing done) when the gather footprint lies outside the
-// window -- the caller defers the particle to k_stage_overflow (WINDOWED = false, global grids).
+// dep_only: the strip thread already gathered and pushed this particle (u^ resp. the new state is stored);
+// only its deposit is left.  WINDOWED: shared windows; returns false (nothing done) when the gather
+// footprint lies outside the window -- the caller defers the particle to k_stage_overflow (WINDOWED =
+// false, global grids).  The force window is a copy of the global force grid and the deposits are integer
+// sums, so all three routes (register patch, window, global) give identical grids.
 template <int SHAPE, int STAGE, int QMASK, bool WINDOWED>
-__device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+__device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, bool dep_only, int gx0, int gy0, const float2 *Fs,
+                                               int32_t *dep)
 {
     PV me = P.pv[p];
     uint32_t xf = me.x, yf = me.y;
     float ux = me.ux, uy = me.uy;
     if (STAGE == 0) {
-        bool ok;
-        float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xf, yf, Fs, ok);
-        if (!ok) return false;
-        float uhx = __fmaf_rn(P.dt, f.x, ux), uhy = __fmaf_rn(P.dt, f.y, uy);     // Eq. 17
-        P.uh[p] = make_float2(uhx, uhy);
+        float uhx, uhy;
+        if (dep_only) {
+            const float2 uh = P.uh[p];
+            uhx = uh.x;
+            uhy = uh.y;
+        } else {
+            bool ok;
+            float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xf, yf, Fs, ok);
+            if (!ok) return false;
+            uhx = __fmaf_rn(P.dt, f.x, ux);                                        // Eq. 17
+            uhy = __fmaf_rn(P.dt, f.y, uy);
+            P.uh[p] = make_float2(uhx, uhy);
+        }
         xf = advance(xf, P.hx, __fadd_rn(uhx, ux));
         yf = advance(yf, P.hy, __fadd_rn(uhy, uy));
         ux = uhx;
         uy = uhy;
-    } else if (STAGE == 1) {
+    } else if (STAGE == 1 && !dep_only) {
         const float2 uh = P.uh[p];
         uint32_t xh = advance(xf, P.hx, __fadd_rn(uh.x, ux));                      // x^ of Eq. 17 again
         uint32_t yh = advance(yf, P.hy, __fadd_rn(uh.y, uy));
@@ -325,79 +301,52 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, i
     return true;
 }
 
-template <int SHAPE, int STAGE, int QMASK>
-__device__ __noinline__ void slow_particle(const PartParams &P, int64_t p, int tile, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+// particles a strip thread cannot serve from its register patch are listed per CTA and processed by all
+// threads after the strips (no divergence inside the strip loops); a full list spills to the global one
+constexpr int STRAY_CAP = 2048;
+constexpr uint32_t STRAY_DEP = 0x80000000u;            // flag: deposit only
+constexpr int64_t OVF_DEP = (int64_t)1 << 62;
+
+__device__ __forceinline__ void push_overflow(const PartParams &P, int64_t p, int tile, bool dep_only)
 {
-    if (!process_direct<SHAPE, STAGE, QMASK, true>(P, p, gx0, gy0, Fs, dep)) {
-        int slot = atomicAdd(P.ovf_count, 1);
-        if (slot < P.ovf_cap) {
-            P.ovf_p[slot] = p;
-            P.ovf_tile[slot] = tile;
-        } else
-            P.flags[2] = 1;
-    }
+    int slot = atomicAdd(P.ovf_count, 1);
+    if (slot < P.ovf_cap) {
+        P.ovf_p[slot] = p | (dep_only ? OVF_DEP : 0);
+        P.ovf_tile[slot] = tile;
+    } else
+        P.flags[2] = 1;
 }
 
-template <int SHAPE, int QMASK>
-__device__ __noinline__ void slow_deposit(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, float ux, float uy, float w,
-                                          int32_t *dep)
+__device__ __forceinline__ void defer_stray(const PartParams &P, uint32_t *slist, int *scount, int64_t p, int64_t t0, int tile,
+                                            bool dep_only)
 {
-    deposit_direct<SHAPE, QMASK, true>(P, gx0, gy0, xf, yf, ux, uy, w, dep);
+    int slot = atomicAdd(scount, 1);
+    if (slot < STRAY_CAP) slist[slot] = (uint32_t)(p - t0) | (dep_only ? STRAY_DEP : 0u);
+    else push_overflow(P, p, tile, dep_only);
 }
 
-// Eq. 16 / 18 evaluated for the nodes of the tile window, straight into shared memory:
-//   F = qE E_node - (1/2) grad(sum_c a_c^2) [electrons] - C v_th^2 grad(n)/n
-// central differences, one-sided on the wall rows, pressure term 0 where n = 0 (Q10).  Window rows
-// beyond a wall hold F of the mirror node (Q9: the gather folds indices), whose x-difference runs
-// the other way in window coordinates.  a2s / ns: scratch of (WIN+2)^2 values (window + 1 ring).
-constexpr int WF = WIN + 2;
-__device__ __forceinline__ void build_force_window(const PartParams &P, int gx0, int gy0, float *a2s, int32_t *ns, float2 *Fs)
+// The nodal force of Eq. 16 / 18 (k_force, pm2d_fields.cu) for the nodes of the tile window -> shared
+// memory.  Window rows beyond a wall hold F of the mirror node (Q9: the gather folds indices), window
+// columns wrap (y periodic).  All loads of a thread are issued before the first store.
+template <int NT>
+__device__ __forceinline__ void load_force_window(const PartParams &P, int gx0, int gy0, float2 *Fs)
 {
-    const size_t nn = (size_t)(P.nx + 1) * P.ny;
-#pragma unroll 2
-    for (int e = threadIdx.x; e < WF * WF; e += blockDim.x) {
-        int r = e / WF, cidx = e - r * WF;
-        int gi = fold_x(gx0 + r - HALO - 1, P.nx);
-        int gj = (gy0 + cidx - HALO - 1) & (P.ny - 1);
-        size_t k = (size_t)gi * P.ny + gj;
-        float s2 = 0.f;
-        if (P.pond != 0.f)
-            for (int c = 0; c < P.ncomp; c++) {
-                float v = P.a[c * nn + k];
-                s2 += v * v;
-            }
-        a2s[e] = s2;
-        ns[e] = P.nfix_in[k];
+    constexpr int IT = (WIN * WIN + NT - 1) / NT;
+    float2 v[IT];
+#pragma unroll
+    for (int k = 0; k < IT; k++) {
+        const int e = threadIdx.x + k * NT;
+        const int r = e / WIN, cidx = e - r * WIN;
+        const int gi = fold_x(gx0 + r - HALO, P.nx);
+        const int gj = (gy0 + cidx - HALO) & (P.ny - 1);
+        v[k] = (e < WIN * WIN) ? P.F[(size_t)gi * P.ny + gj] : make_float2(0.f, 0.f);
     }
-    __syncthreads();
-#pragma unroll 1
-    for (int e = threadIdx.x; e < WIN * WIN; e += blockDim.x) {
-        int r = e / WIN, cidx = e - r * WIN;
-        int raw = gx0 + r - HALO;
-        int gi = fold_x(raw, P.nx);
-        int gj = (gy0 + cidx - HALO) & (P.ny - 1);
-        const int c0 = (r + 1) * WF + (cidx + 1);
-        // x-difference in window coordinates -> difference at the (possibly mirrored) node
-        int lo = c0 - WF, hi = c0 + WF;
-        float sx = P.inv_2dx;
-        if (raw < 0 || raw > P.nx) sx = -sx;
-        if (gi == 0) { lo = c0; hi = (raw == 0) ? c0 + WF : c0 - WF; sx = 2.f * P.inv_2dx; }
-        else if (gi == P.nx) { hi = c0; lo = (raw == P.nx) ? c0 - WF : c0 + WF; sx = 2.f * P.inv_2dx; }
-        float2 E = P.Enode[(size_t)gi * P.ny + gj];
-        float fx = P.qE * E.x, fy = P.qE * E.y;
-        if (P.pond != 0.f) {
-            fx -= 0.5f * sx * (a2s[hi] - a2s[lo]);
-            fy -= 0.5f * P.inv_2dy * (a2s[c0 + 1] - a2s[c0 - 1]);
-        }
-        const int n0 = ns[c0];
-        if (n0 > 0 && P.cv2 != 0.f) {
-            const float inv_n = 1.f / (float)n0;
-            fx -= P.cv2 * sx * (float)(ns[hi] - ns[lo]) * inv_n;
-            fy -= P.cv2 * P.inv_2dy * (float)(ns[c0 + 1] - ns[c0 - 1]) * inv_n;
-        }
-        Fs[r * WPITCH + cidx] = make_float2(fx, fy);
+#pragma unroll
+    for (int k = 0; k < IT; k++) {
+        const int e = threadIdx.x + k * NT;
+        const int r = e / WIN, cidx = e - r * WIN;
+        if (e < WIN * WIN) Fs[r * WPITCH + cidx] = v[k];
     }
-    __syncthreads();
 }
 
 // ---- register patch of a strip thread: force on, and deposit to, the 4 x 4 nodes around its current cell.
@@ -413,7 +362,7 @@ __device__ __forceinline__ bool in_patch(int rel) { return (uint32_t)(rel + (1 <
 template <int SHAPE, int STAGE, int QMASK, int ROT>
 __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, const PV me, const float wme, const float2 uhme,
                                                const int64_t p, const uint32_t ax_fix, const uint32_t ay_fix, const int tile,
-                                               const int gx0, const int gy0, const float2 *Fs, int32_t *dep)
+                                               const int gx0, const int64_t t0, uint32_t *slist, int *scount)
 {
     constexpr float INV24 = 1.0f / 16777216.0f;
     float ux = me.ux, uy = me.uy;
@@ -427,7 +376,7 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
         }
         const int rx = (int)(xg - ax_fix), ry = (int)(yg - ay_fix);
         if (!in_patch(rx) || !in_patch(ry)) {
-            slow_particle<SHAPE, STAGE, QMASK>(P, p, tile, gx0, gy0, Fs, dep);
+            defer_stray(P, slist, scount, p, t0, tile, false);
             return;
         }
         weights4<SHAPE>((float)rx * INV24, P, Wx);
@@ -466,7 +415,7 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
     }
     const int rx = (int)(xd - ax_fix), ry = (int)(yd - ay_fix);
     if (!in_patch(rx) || !in_patch(ry)) {
-        slow_deposit<SHAPE, QMASK>(P, gx0, gy0, xd, yd, ux, uy, wme, dep);
+        defer_stray(P, slist, scount, p, t0, tile, true);
         return;
     }
     weights4<SHAPE>((float)rx * INV24, P, Wx);
@@ -533,6 +482,9 @@ struct StripCtx {
     int wr0, tile, gx0, gy0;
     const float2 *Fs;
     int32_t *dep;
+    uint32_t *slist;             // shared stray list of the CTA
+    int *scount;
+    int cell_cap;                // particles per cell served from the patch
     PV cur;                      // prefetched particle p
     float wcur;
     float2 uhcur;
@@ -544,18 +496,30 @@ __device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, Strip
 {
     const int64_t end = c.t0 + c.coff_row[j + 1];
     const uint32_t ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
-    while (c.p < end) {
-        const PV me = c.cur;
-        const float wme = c.wcur;
-        const float2 uhme = c.uhcur;
-        if (c.p + 1 < c.strip_end) {
-            c.cur = P.pv[c.p + 1];
-            c.wcur = P.w[c.p + 1];
-            if (STAGE == 1) c.uhcur = P.uh[c.p + 1];
+    // the lanes of a warp walk their cells in lockstep: a cell much fuller than the tile's mean would stall
+    // the other 31 lanes, so only its first cell_cap particles go through the patch, the rest to the stray list
+    const int64_t fast_end = min(end, c.p + c.cell_cap);
+    // warp-uniform loop: the lanes reconverge at every particle (vote) instead of drifting apart in the
+    // unrolled copies of this function
+    for (;;) {
+        const bool act = c.p < fast_end;
+        if (!__any_sync(0xffffffffu, act)) break;
+        if (act) {
+            const PV me = c.cur;
+            const float wme = c.wcur;
+            const float2 uhme = c.uhcur;
+            const int64_t nxt = (c.p + 1 == fast_end) ? end : c.p + 1;          // the next particle this thread serves
+            if (nxt < c.strip_end) {
+                c.cur = P.pv[nxt];
+                c.wcur = P.w[nxt];
+                if (STAGE == 1) c.uhcur = P.uh[nxt];
+            }
+            strip_particle<SHAPE, STAGE, QMASK, ROT>(P, pt, me, wme, uhme, c.p, c.ax_fix, ay_fix, c.tile, c.gx0, c.t0, c.slist, c.scount);
+            c.p++;
         }
-        strip_particle<SHAPE, STAGE, QMASK, ROT>(P, pt, me, wme, uhme, c.p, c.ax_fix, ay_fix, c.tile, c.gx0, c.gy0, c.Fs, c.dep);
-        c.p++;
     }
+    for (; c.p < end; c.p++) defer_stray(P, c.slist, c.scount, c.p, c.t0, c.tile, false);
+    __syncwarp();
     flush_column<QMASK, ROT>(pt, c.dep, c.wr0, j - 1 + HALO);              // node column j-1 is complete for this strip
     if (STAGE < 2) load_force_column<ROT>(pt, c.Fs, c.wr0, j + 3 + HALO);
 }
@@ -566,11 +530,11 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     static_assert(S % 4 == 0 && TILE % S == 0, "strip length");
     constexpr int NT = TCELLS / S;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
-    // dep doubles as the scratch of build_force_window (2 (WIN+2)^2 words) before it is zeroed
-    constexpr int DEPW = (STAGE < 2 && NQ * WIN * WPITCH < 2 * WF * WF) ? 2 * WF * WF : NQ * WIN * WPITCH;
-    __shared__ int32_t dep[DEPW];
+    __shared__ int32_t dep[NQ * WIN * WPITCH];
     __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
     __shared__ int32_t coff[TILE * COPITCH];
+    __shared__ uint32_t slist[STRAY_CAP];
+    __shared__ int scount;
     const int tile = blockIdx.x;
     const int64_t t0 = P.tile_off[tile];
     if (P.tile_off[tile + 1] == t0) return;
@@ -578,14 +542,23 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 
     {
         const int32_t *co = P.cell_off + (size_t)tile * CPITCH;
-        for (int e = threadIdx.x; e <= TCELLS; e += NT) {
-            const int32_t v = co[e];
-            if (e < TCELLS) coff[(e >> 5) * COPITCH + (e & 31)] = v;
-            if ((e & 31) == 0 && e > 0) coff[((e >> 5) - 1) * COPITCH + TILE] = v;   // end of the previous row
+        constexpr int IT = (TCELLS + NT) / NT;
+        int32_t v[IT];
+#pragma unroll
+        for (int k = 0; k < IT; k++) {
+            const int e = threadIdx.x + k * NT;
+            v[k] = e <= TCELLS ? co[e] : 0;
+        }
+        if (STAGE < 2) load_force_window<NT>(P, gx0, gy0, Fs);
+#pragma unroll
+        for (int k = 0; k < IT; k++) {
+            const int e = threadIdx.x + k * NT;
+            if (e < TCELLS) coff[(e >> 5) * COPITCH + (e & 31)] = v[k];
+            if ((e & 31) == 0 && e > 0 && e <= TCELLS) coff[((e >> 5) - 1) * COPITCH + TILE] = v[k];   // end of the previous row
         }
     }
-    if (STAGE < 2) build_force_window(P, gx0, gy0, reinterpret_cast<float *>(dep), dep + WF * WF, Fs);
     for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
+    if (threadIdx.x == 0) scount = 0;
     __syncthreads();
 
     const int r = threadIdx.x & 31, j0 = (threadIdx.x >> 5) * S;          // cell row, first cell column of the strip
@@ -610,7 +583,8 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     ctx.p = p; ctx.strip_end = strip_end; ctx.t0 = t0;
     ctx.coff_row = coff + r * COPITCH;
     ctx.ax_fix = ax_fix; ctx.wr0 = wr0; ctx.tile = tile; ctx.gx0 = gx0; ctx.gy0 = gy0;
-    ctx.Fs = Fs; ctx.dep = dep;
+    ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
+    ctx.cell_cap = (int)min((int64_t)0x3fffffff, (P.tile_off[tile + 1] - t0 + TCELLS - 1) / TCELLS + P.cap_extra);
     ctx.cur = PV{0u, 0u, 0.f, 0.f};
     ctx.wcur = 0.f;
     ctx.uhcur = make_float2(0.f, 0.f);
@@ -632,25 +606,33 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
         flush_column<QMASK, 2>(pt, dep, wr0, j0 + S + 1 + HALO);
     }
     __syncthreads();
+    {   // strays: 3 x 3 nodes around the nearest node, straight on the shared windows
+        const int ns = min(scount, STRAY_CAP);
+        if (threadIdx.x == 0 && scount > 0) atomicAdd(P.stray_total, (unsigned long long)scount);
+        for (int e = threadIdx.x; e < ns; e += NT) {
+            const uint32_t ent = slist[e];
+            const int64_t p = t0 + (int64_t)(ent & ~STRAY_DEP);
+            const bool dep_only = (ent & STRAY_DEP) != 0;
+            if (!process_direct<SHAPE, STAGE, QMASK, true>(P, p, dep_only, gx0, gy0, Fs, dep)) push_overflow(P, p, tile, dep_only);
+        }
+        if (ns > 0) __syncthreads();
+    }
 
     // flush: one global integer reduction per touched window node; wall columns hold half a
     // control volume and count twice (Q9); rows beyond a wall fold back (mirror particles)
     for (int e = threadIdx.x; e < WIN * WIN; e += NT) {
-        int rr = e / WIN, cidx = e - rr * WIN;
-        int se = rr * WPITCH + cidx;
-        int gi = fold_x(gx0 + rr - HALO, P.nx);
-        int gj = (gy0 + cidx - HALO) & (P.ny - 1);
-        int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
-        size_t k = (size_t)gi * P.ny + gj;
-        if (QMASK & 1) {
-            int v = dep[se];
-            if (v) atomicAdd(&P.nfix[k], fac * v);
-        }
-        if (QMASK & 2) {
-            int vx = dep[WIN * WPITCH + se], vy = dep[2 * WIN * WPITCH + se];
-            if (vx) atomicAdd(&P.pxfix[k], fac * vx);
-            if (vy) atomicAdd(&P.pyfix[k], fac * vy);
-        }
+        const int rr = e / WIN, cidx = e - rr * WIN;
+        const int se = rr * WPITCH + cidx;
+        const int v = (QMASK & 1) ? dep[se] : 0;
+        const int vx = (QMASK & 2) ? dep[WIN * WPITCH + se] : 0, vy = (QMASK & 2) ? dep[2 * WIN * WPITCH + se] : 0;
+        if ((v | vx | vy) == 0) continue;
+        const int gi = fold_x(gx0 + rr - HALO, P.nx);
+        const int gj = (gy0 + cidx - HALO) & (P.ny - 1);
+        const int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
+        const size_t k = (size_t)gi * P.ny + gj;
+        if (v) atomicAdd(&P.nfix[k], fac * v);
+        if (vx) atomicAdd(&P.pxfix[k], fac * vx);
+        if (vy) atomicAdd(&P.pyfix[k], fac * vy);
     }
 }
 
@@ -661,7 +643,9 @@ __global__ void __launch_bounds__(128) k_stage_overflow(const PartParams P)
     const int n = min(*P.ovf_count, P.ovf_cap);
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
         const int tile = P.ovf_tile[k];
-        process_direct<SHAPE, STAGE, QMASK, false>(P, P.ovf_p[k], (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr, nullptr);
+        const int64_t ent = P.ovf_p[k];
+        process_direct<SHAPE, STAGE, QMASK, false>(P, ent & ~OVF_DEP, (ent & OVF_DEP) != 0, (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr,
+                                                   nullptr);
     }
 }
 
@@ -1158,19 +1142,15 @@ __global__ void __launch_bounds__(PTHREADS) k_unpack(const PV *pv, const int32_t
 
 // =================================================================================================
 // host launchers
-static PartParams make_part_params(pm2d_ctx *c, int s, const float *a_level)
+static PartParams make_part_params(pm2d_ctx *c, int s)
 {
     SpeciesDev &S = c->sp[s];
     PartParams P;
     P.pv = S.pv; P.uh = S.uh; P.w = S.w;
     P.tile_off = S.tile_off; P.cell_off = S.cell_off;
-    P.F = S.F; P.Enode = c->Enode; P.a = a_level; P.ncomp = c->g.ncomp;
-    P.qE = (float)(-(double)S.cfg.sign * 4.0 * 3.14159265358979323846 * 3.14159265358979323846 / S.cfg.mass);
-    P.pond = S.cfg.sign < 0 ? 1.f : 0.f;
-    P.cv2 = (float)(S.cfg.pressure_coeff * S.vth2);
-    P.inv_2dx = (float)(1.0 / (2.0 * c->g.dx));
-    P.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
-    P.nfix_in = S.nfix; P.nfix = S.nfix; P.pxfix = S.pxfix; P.pyfix = S.pyfix; P.flags = c->flags;
+    P.F = S.F;
+    P.nfix = S.nfix; P.pxfix = S.pxfix; P.pyfix = S.pyfix; P.flags = c->flags;
+    P.stray_total = c->stray_total;
     P.ovf_p = c->ovf_p; P.ovf_tile = c->ovf_tile; P.ovf_count = c->ovf_count; P.ovf_cap = c->ovf_cap;
     P.nx = c->g.nx; P.ny = c->g.ny; P.nty = c->nty;
     P.dt = (float)c->g.dt;
@@ -1180,6 +1160,7 @@ static PartParams make_part_params(pm2d_ctx *c, int s, const float *a_level)
     P.half_dd = (float)(0.5 * S.cfg.DD);
     P.dd = (float)S.cfg.DD;
     P.k_rad = (float)(3.14159265358979323846 / S.cfg.DD);
+    P.cap_extra = c->cap_extra;
     return P;
 }
 
@@ -1191,7 +1172,7 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
 #define PM2D_LAUNCH(ST, Q)                                                         \
     do {                                                                           \
         k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);          \
-        if (ST < 2) k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P);        \
+        k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P);                    \
     } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }
     else if (stage == 1) { if (qmask == 3) PM2D_LAUNCH(1, 3); else PM2D_LAUNCH(1, 1); }
@@ -1199,17 +1180,17 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
 #undef PM2D_LAUNCH
 }
 
+// stage 0 / 1: the caller has put the nodal force of the stage into S.F (launch_force), which also was
+// the last reader of the density grid the deposit now overwrites
 static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
 {
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
-    PartParams P = make_part_params(c, s, stage == 0 ? c->a[1] : c->a[0]);
+    PartParams P = make_part_params(c, s);
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->ovf_count, 0, sizeof(int32_t), c->stream));
     if (stage < 2) {
-        // the force window reads n_s while other CTAs already deposit: ping-pong the density grid
         const size_t bytes = (size_t)c->nn * sizeof(int32_t);
-        P.nfix = S.nfix2;
-        PM2D_CUDA_CHECK(cudaMemsetAsync(c->ovf_count, 0, sizeof(int32_t), c->stream));
-        PM2D_CUDA_CHECK(cudaMemsetAsync(S.nfix2, 0, bytes, c->stream));
+        PM2D_CUDA_CHECK(cudaMemsetAsync(S.nfix, 0, bytes, c->stream));
         if (qmask & 2) {
             PM2D_CUDA_CHECK(cudaMemsetAsync(S.pxfix, 0, bytes, c->stream));
             PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
@@ -1218,9 +1199,8 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, c->stream);
     else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, c->stream);
-    count_launch(c, stage < 2 ? 2 : 1);
+    count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
-    if (stage < 2) std::swap(S.nfix, S.nfix2);
     return PM2D_OK;
 }
 
