@@ -304,6 +304,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
 // particles a strip thread cannot serve from its register patch are listed per CTA and processed by all
 // threads after the strips (no divergence inside the strip loops); a full list spills to the global one
 constexpr int STRAY_CAP = 2048;
+constexpr bool SHIFT_PATCH = true;   // one copy of the particle loop (instruction cache) at the price of register moves per cell
 constexpr uint32_t STRAY_DEP = 0x80000000u;            // flag: deposit only
 constexpr int64_t OVF_DEP = (int64_t)1 << 62;
 
@@ -350,8 +351,10 @@ __device__ __forceinline__ void load_force_window(const PartParams &P, int gx0, 
 }
 
 // ---- register patch of a strip thread: force on, and deposit to, the 4 x 4 nodes around its current cell.
-// Logical column b (node column j-1+b of cell column j) lives in physical column (b + ROT) & 3, so sliding
-// to the next cell renames columns instead of moving registers.
+// A strip runs along x (rows of cells); the 32 lanes of a warp hold the 32 cell columns of the tile, so at
+// every row the warp reads one contiguous piece of the cell-sorted particle arrays and its shared-memory
+// accesses fall into consecutive banks.  Logical patch row a (node row i-1+a of cell row i) lives in
+// physical row (a + ROT) & 3, so sliding to the next cell row renames rows instead of moving registers.
 struct Patch {
     float Fx[4][4], Fy[4][4];
     float dn[4][4], dpx[4][4], dpy[4][4];
@@ -359,10 +362,27 @@ struct Patch {
 
 __device__ __forceinline__ bool in_patch(int rel) { return (uint32_t)(rel + (1 << 23)) < (1u << 25); }   // offset in [-1/2, 3/2)
 
+// walking state of a strip thread
+struct StripCtx {
+    int64_t t0;                  // first slot of the tile
+    int32_t n_tile;              // particles in the tile
+    const int32_t *coff;         // shared: coff[c] = first slot (tile-relative) of cell c = row * TILE + column
+    uint32_t ay_fix;
+    int j, wc0, tile, gx0;
+    const float2 *Fs;
+    int32_t *dep;
+    uint32_t *slist;             // shared stray list of the CTA
+    int *scount;
+    int cell_cap;                // particles per cell served from the patch
+    int32_t q;                   // tile-relative slot of the prefetched particle
+    PV cur;                      // prefetched particle q
+    float wcur;
+    float2 uhcur;
+};
+
 template <int SHAPE, int STAGE, int QMASK, int ROT>
-__device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, const PV me, const float wme, const float2 uhme,
-                                               const int64_t p, const uint32_t ax_fix, const uint32_t ay_fix, const int tile,
-                                               const int gx0, const int64_t t0, uint32_t *slist, int *scount)
+__device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, const StripCtx &c, const PV me, const float wme,
+                                               const float2 uhme, const int64_t p, const uint32_t ax_fix)
 {
     constexpr float INV24 = 1.0f / 16777216.0f;
     float ux = me.ux, uy = me.uy;
@@ -374,9 +394,9 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
             xg = advance(me.x, P.hx, __fadd_rn(uhme.x, ux));
             yg = advance(me.y, P.hy, __fadd_rn(uhme.y, uy));
         }
-        const int rx = (int)(xg - ax_fix), ry = (int)(yg - ay_fix);
+        const int rx = (int)(xg - ax_fix), ry = (int)(yg - c.ay_fix);
         if (!in_patch(rx) || !in_patch(ry)) {
-            defer_stray(P, slist, scount, p, t0, tile, false);
+            defer_stray(P, c.slist, c.scount, p, c.t0, c.tile, false);
             return;
         }
         weights4<SHAPE>((float)rx * INV24, P, Wx);
@@ -387,8 +407,8 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
             float sx = 0.f, sy = 0.f;
 #pragma unroll
             for (int b = 0; b < 4; b++) {
-                sx = fmaf(Wy[b], pt.Fx[a][(b + ROT) & 3], sx);
-                sy = fmaf(Wy[b], pt.Fy[a][(b + ROT) & 3], sy);
+                sx = fmaf(Wy[b], pt.Fx[(a + ROT) & 3][b], sx);
+                sy = fmaf(Wy[b], pt.Fy[(a + ROT) & 3][b], sy);
             }
             fx = fmaf(Wx[a], sx, fx);
             fy = fmaf(Wx[a], sy, fy);
@@ -405,7 +425,7 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
             float uny = __fmaf_rn(0.5f * P.dt, fy, 0.5f * __fadd_rn(uhme.y, uy));
             xd = advance(me.x, P.hx, __fadd_rn(unx, ux));
             yd = advance(me.y, P.hy, __fadd_rn(uny, uy));
-            reflect_x(xd, unx, gx0, P.nx);
+            reflect_x(xd, unx, c.gx0, P.nx);
             PV out;
             out.x = xd; out.y = yd; out.ux = unx; out.uy = uny;
             P.pv[p] = out;
@@ -413,9 +433,9 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
             uy = uny;
         }
     }
-    const int rx = (int)(xd - ax_fix), ry = (int)(yd - ay_fix);
+    const int rx = (int)(xd - ax_fix), ry = (int)(yd - c.ay_fix);
     if (!in_patch(rx) || !in_patch(ry)) {
-        defer_stray(P, slist, scount, p, t0, tile, true);
+        defer_stray(P, c.slist, c.scount, p, c.t0, c.tile, true);
         return;
     }
     weights4<SHAPE>((float)rx * INV24, P, Wx);
@@ -428,100 +448,106 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
         const float qa = Wx[a] * q;
         if (QMASK & 1) {
 #pragma unroll
-            for (int b = 0; b < 4; b++) pt.dn[a][(b + ROT) & 3] = fmaf(qa, Wy[b], pt.dn[a][(b + ROT) & 3]);
+            for (int b = 0; b < 4; b++) pt.dn[(a + ROT) & 3][b] = fmaf(qa, Wy[b], pt.dn[(a + ROT) & 3][b]);
         }
         if (QMASK & 2) {
             const float qxa = qa * qux, qya = qa * quy;
 #pragma unroll
             for (int b = 0; b < 4; b++) {
-                pt.dpx[a][(b + ROT) & 3] = fmaf(qxa, Wy[b], pt.dpx[a][(b + ROT) & 3]);
-                pt.dpy[a][(b + ROT) & 3] = fmaf(qya, Wy[b], pt.dpy[a][(b + ROT) & 3]);
+                pt.dpx[(a + ROT) & 3][b] = fmaf(qxa, Wy[b], pt.dpx[(a + ROT) & 3][b]);
+                pt.dpy[(a + ROT) & 3][b] = fmaf(qya, Wy[b], pt.dpy[(a + ROT) & 3][b]);
             }
         }
     }
 }
 
-// flush physical column PC of the deposit patch into window column wc, rows wr0 .. wr0+3, and clear it
-template <int QMASK, int PC>
-__device__ __forceinline__ void flush_column(Patch &pt, int32_t *dep, int wr0, int wc)
+// flush physical row PR of the deposit patch into window row wr, columns wc0 .. wc0+3, and clear it
+template <int QMASK, int PR>
+__device__ __forceinline__ void flush_row(Patch &pt, int32_t *dep, int wr, int wc0)
 {
 #pragma unroll
-    for (int a = 0; a < 4; a++) {
-        const int e = (wr0 + a) * WPITCH + wc;
+    for (int b = 0; b < 4; b++) {
+        const int e = wr * WPITCH + wc0 + b;
         if (QMASK & 1) {
-            atomicAdd(&dep[e], __float2int_rn(pt.dn[a][PC]));
-            pt.dn[a][PC] = 0.f;
+            atomicAdd(&dep[e], __float2int_rn(pt.dn[PR][b]));
+            pt.dn[PR][b] = 0.f;
         }
         if (QMASK & 2) {
-            atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(pt.dpx[a][PC]));
-            atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(pt.dpy[a][PC]));
-            pt.dpx[a][PC] = 0.f;
-            pt.dpy[a][PC] = 0.f;
+            atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(pt.dpx[PR][b]));
+            atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(pt.dpy[PR][b]));
+            pt.dpx[PR][b] = 0.f;
+            pt.dpy[PR][b] = 0.f;
         }
     }
 }
 
-template <int PC>
-__device__ __forceinline__ void load_force_column(Patch &pt, const float2 *Fs, int wr0, int wc)
+template <int PR>
+__device__ __forceinline__ void load_force_row(Patch &pt, const float2 *Fs, int wr, int wc0)
 {
 #pragma unroll
-    for (int a = 0; a < 4; a++) {
-        const float2 f = Fs[(wr0 + a) * WPITCH + wc];
-        pt.Fx[a][PC] = f.x;
-        pt.Fy[a][PC] = f.y;
+    for (int b = 0; b < 4; b++) {
+        const float2 f = Fs[wr * WPITCH + wc0 + b];
+        pt.Fx[PR][b] = f.x;
+        pt.Fy[PR][b] = f.y;
     }
 }
 
-constexpr int COPITCH = TILE + 1;   // odd pitch of the shared copy of the tile's cell offsets
-
-// walking state of a strip thread
-struct StripCtx {
-    int64_t p, strip_end, t0;
-    const int32_t *coff_row;     // shared: start of every cell of this thread's row; [j+1] = end of cell j
-    uint32_t ax_fix;
-    int wr0, tile, gx0, gy0;
-    const float2 *Fs;
-    int32_t *dep;
-    uint32_t *slist;             // shared stray list of the CTA
-    int *scount;
-    int cell_cap;                // particles per cell served from the patch
-    PV cur;                      // prefetched particle p
-    float wcur;
-    float2 uhcur;
-};
-
-// all particles of cell column j, then slide the patch to column j+1 (physical column ROT is renamed)
-template <int SHAPE, int STAGE, int QMASK, int ROT>
-__device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, StripCtx &c, const int j)
+// all particles of cell (i, j), then slide the patch to cell row i+1: physical row ROT is renamed (4 unrolled
+// copies, ROT = 0..3), or, with SHIFT, the registers move and one copy serves every row (ROT = 0)
+template <int SHAPE, int STAGE, int QMASK, int ROT, bool SHIFT>
+__device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, StripCtx &c, const int i)
 {
-    const int64_t end = c.t0 + c.coff_row[j + 1];
-    const uint32_t ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
+    const int cell = i * TILE + c.j;
+    const int32_t beg = c.coff[cell], end = c.coff[cell + 1];
+    const int32_t next_beg = c.coff[min(cell + TILE, TCELLS)];          // where this thread reads next
+    const uint32_t ax_fix = (uint32_t)(i + POS_BIAS) << POS_FRAC_BITS;
     // the lanes of a warp walk their cells in lockstep: a cell much fuller than the tile's mean would stall
     // the other 31 lanes, so only its first cell_cap particles go through the patch, the rest to the stray list
-    const int64_t fast_end = min(end, c.p + c.cell_cap);
+    const int32_t fast_end = min(end, beg + c.cell_cap);
+    int32_t q = beg;
+    if (beg < fast_end && c.q != beg) {                                  // no prefetch in flight (strip start, after empty cells)
+        c.cur = P.pv[c.t0 + beg];
+        c.wcur = P.w[c.t0 + beg];
+        if (STAGE == 1) c.uhcur = P.uh[c.t0 + beg];
+        c.q = beg;
+    }
     // warp-uniform loop: the lanes reconverge at every particle (vote) instead of drifting apart in the
     // unrolled copies of this function
     for (;;) {
-        const bool act = c.p < fast_end;
+        const bool act = q < fast_end;
         if (!__any_sync(0xffffffffu, act)) break;
         if (act) {
             const PV me = c.cur;
             const float wme = c.wcur;
             const float2 uhme = c.uhcur;
-            const int64_t nxt = (c.p + 1 == fast_end) ? end : c.p + 1;          // the next particle this thread serves
-            if (nxt < c.strip_end) {
-                c.cur = P.pv[nxt];
-                c.wcur = P.w[nxt];
-                if (STAGE == 1) c.uhcur = P.uh[nxt];
+            const int32_t nxt = (q + 1 < fast_end) ? q + 1 : next_beg;
+            if (nxt < c.n_tile) {
+                c.cur = P.pv[c.t0 + nxt];
+                c.wcur = P.w[c.t0 + nxt];
+                if (STAGE == 1) c.uhcur = P.uh[c.t0 + nxt];
             }
-            strip_particle<SHAPE, STAGE, QMASK, ROT>(P, pt, me, wme, uhme, c.p, c.ax_fix, ay_fix, c.tile, c.gx0, c.t0, c.slist, c.scount);
-            c.p++;
+            c.q = nxt;
+            strip_particle<SHAPE, STAGE, QMASK, ROT>(P, pt, c, me, wme, uhme, c.t0 + q, ax_fix);
+            q++;
         }
     }
-    for (; c.p < end; c.p++) defer_stray(P, c.slist, c.scount, c.p, c.t0, c.tile, false);
+    for (; q < end; q++) defer_stray(P, c.slist, c.scount, c.t0 + q, c.t0, c.tile, false);
     __syncwarp();
-    flush_column<QMASK, ROT>(pt, c.dep, c.wr0, j - 1 + HALO);              // node column j-1 is complete for this strip
-    if (STAGE < 2) load_force_column<ROT>(pt, c.Fs, c.wr0, j + 3 + HALO);
+    flush_row<QMASK, ROT>(pt, c.dep, i - 1 + HALO, c.wc0);                // node row i-1 is complete for this strip
+    if (SHIFT) {                                                          // one copy of the loop body: move the patch up one row
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                if (QMASK & 1) pt.dn[a][b] = pt.dn[a + 1][b];
+                if (QMASK & 2) { pt.dpx[a][b] = pt.dpx[a + 1][b]; pt.dpy[a][b] = pt.dpy[a + 1][b]; }
+                if (STAGE < 2) { pt.Fx[a][b] = pt.Fx[a + 1][b]; pt.Fy[a][b] = pt.Fy[a + 1][b]; }
+            }
+#pragma unroll
+        for (int b = 0; b < 4; b++) pt.dn[3][b] = pt.dpx[3][b] = pt.dpy[3][b] = 0.f;
+        if (STAGE < 2) load_force_row<3>(pt, c.Fs, i + 3 + HALO, c.wc0);
+    } else if (STAGE < 2)
+        load_force_row<ROT>(pt, c.Fs, i + 3 + HALO, c.wc0);
 }
 
 template <int SHAPE, int STAGE, int QMASK, int S>
@@ -532,7 +558,7 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
     __shared__ int32_t dep[NQ * WIN * WPITCH];
     __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
-    __shared__ int32_t coff[TILE * COPITCH];
+    __shared__ int32_t coff[TCELLS + 1];
     __shared__ uint32_t slist[STRAY_CAP];
     __shared__ int scount;
     const int tile = blockIdx.x;
@@ -553,57 +579,53 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 #pragma unroll
         for (int k = 0; k < IT; k++) {
             const int e = threadIdx.x + k * NT;
-            if (e < TCELLS) coff[(e >> 5) * COPITCH + (e & 31)] = v[k];
-            if ((e & 31) == 0 && e > 0 && e <= TCELLS) coff[((e >> 5) - 1) * COPITCH + TILE] = v[k];   // end of the previous row
+            if (e <= TCELLS) coff[e] = v[k];
         }
     }
     for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
     if (threadIdx.x == 0) scount = 0;
     __syncthreads();
 
-    const int r = threadIdx.x & 31, j0 = (threadIdx.x >> 5) * S;          // cell row, first cell column of the strip
-    const int wr0 = r - 1 + HALO;                                        // window row of node row r-1
-    const uint32_t ax_fix = (uint32_t)(r + POS_BIAS) << POS_FRAC_BITS;
-    // cell (r, j) -> coff[r * COPITCH + j]; its end is coff[r * COPITCH + j + 1] (slot TILE = end of the row)
-    const int cbase = r * COPITCH + j0;
-    int64_t p = t0 + coff[cbase];
-    const int64_t strip_end = t0 + coff[cbase + S];
+    const int j = threadIdx.x & 31, i0 = (threadIdx.x >> 5) * S;          // cell column, first cell row of the strip
+    StripCtx ctx;
+    ctx.t0 = t0;
+    ctx.n_tile = coff[TCELLS];
+    ctx.coff = coff;
+    ctx.ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
+    ctx.j = j; ctx.wc0 = j - 1 + HALO; ctx.tile = tile; ctx.gx0 = gx0;
+    ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
+    ctx.cell_cap = min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + P.cap_extra);
+    ctx.q = -1;
+    ctx.cur = PV{0u, 0u, 0.f, 0.f};
+    ctx.wcur = 0.f;
+    ctx.uhcur = make_float2(0.f, 0.f);
     Patch pt;
 #pragma unroll
     for (int a = 0; a < 4; a++)
 #pragma unroll
         for (int b = 0; b < 4; b++) pt.dn[a][b] = pt.dpx[a][b] = pt.dpy[a][b] = pt.Fx[a][b] = pt.Fy[a][b] = 0.f;
     if (STAGE < 2) {
-        load_force_column<0>(pt, Fs, wr0, j0 - 1 + HALO);
-        load_force_column<1>(pt, Fs, wr0, j0 + HALO);
-        load_force_column<2>(pt, Fs, wr0, j0 + 1 + HALO);
-        load_force_column<3>(pt, Fs, wr0, j0 + 2 + HALO);
+        load_force_row<0>(pt, Fs, i0 - 1 + HALO, ctx.wc0);
+        load_force_row<1>(pt, Fs, i0 + HALO, ctx.wc0);
+        load_force_row<2>(pt, Fs, i0 + 1 + HALO, ctx.wc0);
+        load_force_row<3>(pt, Fs, i0 + 2 + HALO, ctx.wc0);
     }
-    StripCtx ctx;
-    ctx.p = p; ctx.strip_end = strip_end; ctx.t0 = t0;
-    ctx.coff_row = coff + r * COPITCH;
-    ctx.ax_fix = ax_fix; ctx.wr0 = wr0; ctx.tile = tile; ctx.gx0 = gx0; ctx.gy0 = gy0;
-    ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
-    ctx.cell_cap = (int)min((int64_t)0x3fffffff, (P.tile_off[tile + 1] - t0 + TCELLS - 1) / TCELLS + P.cap_extra);
-    ctx.cur = PV{0u, 0u, 0.f, 0.f};
-    ctx.wcur = 0.f;
-    ctx.uhcur = make_float2(0.f, 0.f);
-    if (p < strip_end) {
-        ctx.cur = P.pv[p];
-        ctx.wcur = P.w[p];
-        if (STAGE == 1) ctx.uhcur = P.uh[p];
-    }
+    if (SHIFT_PATCH) {
 #pragma unroll 1
-    for (int kk = 0; kk < S; kk += 4) {
-        strip_cell<SHAPE, STAGE, QMASK, 0>(P, pt, ctx, j0 + kk);
-        strip_cell<SHAPE, STAGE, QMASK, 1>(P, pt, ctx, j0 + kk + 1);
-        strip_cell<SHAPE, STAGE, QMASK, 2>(P, pt, ctx, j0 + kk + 2);
-        strip_cell<SHAPE, STAGE, QMASK, 3>(P, pt, ctx, j0 + kk + 3);
+        for (int k = 0; k < S; k++) strip_cell<SHAPE, STAGE, QMASK, 0, true>(P, pt, ctx, i0 + k);
+    } else {
+#pragma unroll 1
+        for (int kk = 0; kk < S; kk += 4) {
+            strip_cell<SHAPE, STAGE, QMASK, 0, false>(P, pt, ctx, i0 + kk);
+            strip_cell<SHAPE, STAGE, QMASK, 1, false>(P, pt, ctx, i0 + kk + 1);
+            strip_cell<SHAPE, STAGE, QMASK, 2, false>(P, pt, ctx, i0 + kk + 2);
+            strip_cell<SHAPE, STAGE, QMASK, 3, false>(P, pt, ctx, i0 + kk + 3);
+        }
     }
-    {   // node columns j0+S-1 .. j0+S+1 (logical columns 0..2 of the cell after the strip)
-        flush_column<QMASK, 0>(pt, dep, wr0, j0 + S - 1 + HALO);
-        flush_column<QMASK, 1>(pt, dep, wr0, j0 + S + HALO);
-        flush_column<QMASK, 2>(pt, dep, wr0, j0 + S + 1 + HALO);
+    {   // node rows i0+S-1 .. i0+S+1 (logical rows 0..2 of the cell row after the strip)
+        flush_row<QMASK, 0>(pt, dep, i0 + S - 1 + HALO, ctx.wc0);
+        flush_row<QMASK, 1>(pt, dep, i0 + S + HALO, ctx.wc0);
+        flush_row<QMASK, 2>(pt, dep, i0 + S + 1 + HALO, ctx.wc0);
     }
     __syncthreads();
     {   // strays: 3 x 3 nodes around the nearest node, straight on the shared windows
