@@ -49,9 +49,11 @@ struct PartParams {
     int nx, ny, nty;
     float dt, hx, hy;        // hx = dt / (2 dx): cells per unit (u' + u)
     float nscale, pscale;
+    float pratio;            // pscale / nscale
     float half_dd;           // DD / 2
     float dd;                // DD
     float k_rad;             // pi / DD  (sine: G(t) = 1/2 - 1/2 cos(k_rad t))
+    float w4_slope, w4_off;  // sine weights4: cosine argument = rel * w4_slope + w4_off
     int cap_extra;           // cell_cap = ceil(mean particles per cell of the tile) + cap_extra
 };
 
@@ -90,23 +92,32 @@ __device__ __forceinline__ void weights3(float d, const PartParams &P, float W[3
     W[2] = 1.f - g1;
 }
 
-// weights of the four nodes c-1 .. c+2 around cell c for a particle at offset f in [-1/2, 3/2) from
-// the cell's origin: faces c-1/2, c+1/2, c+3/2 at t_k = DD/2 + k - 1/2 - f; the outer faces c-3/2 and
-// c+5/2 lie outside the cloud (G = 0, 1) because DD <= 2.
+// weights of the four nodes c-1 .. c+2 around cell c for a particle whose offset from the cell's origin is
+// rel * 2^-24 in [-1/2, 3/2): faces c-1/2, c+1/2, c+3/2 at t_k = DD/2 + k - 1/2 - f; the outer faces c-3/2
+// and c+5/2 lie outside the cloud (G = 0, 1) because DD <= 2.  Returns W4_SCALE<SHAPE> * weight: for the sine
+// cloud the factor 1/2 of G = (1 - cos)/2 is left to the caller (folded into dt and the deposit scale).
 template <int SHAPE>
-__device__ __forceinline__ void weights4(float f, const PartParams &P, float W[4])
+struct W4Scale { static constexpr float value = SHAPE == PM2D_SINE ? 2.f : 1.f; };
+
+template <int SHAPE>
+__device__ __forceinline__ void weights4(int rel, const PartParams &P, float W[4])
 {
-    const float b = P.half_dd - 0.5f - f;
-    float t0 = fminf(fmaxf(b, 0.f), P.dd);
-    float t1 = fminf(fmaxf(b + 1.f, 0.f), P.dd);
-    float t2 = fminf(fmaxf(b + 2.f, 0.f), P.dd);
     if (SHAPE == PM2D_SINE) {
-        float c0 = __cosf(t0 * P.k_rad), c1 = __cosf(t1 * P.k_rad), c2 = __cosf(t2 * P.k_rad);
-        W[0] = fmaf(-0.5f, c0, 0.5f);
-        W[1] = 0.5f * (c0 - c1);
-        W[2] = 0.5f * (c1 - c2);
-        W[3] = fmaf(0.5f, c2, 0.5f);
+        // everything in radians of the cosine argument: b = (DD/2 - 1/2 - f) pi/DD, clamped to [0, pi]
+        const float b = fmaf((float)rel, P.w4_slope, P.w4_off);
+        const float t0 = fminf(fmaxf(b, 0.f), 3.14159265358979f);
+        const float t1 = fminf(fmaxf(b + P.k_rad, 0.f), 3.14159265358979f);
+        const float t2 = fminf(fmaxf(b + 2.f * P.k_rad, 0.f), 3.14159265358979f);
+        const float c0 = __cosf(t0), c1 = __cosf(t1), c2 = __cosf(t2);
+        W[0] = 1.f - c0;
+        W[1] = c0 - c1;
+        W[2] = c1 - c2;
+        W[3] = 1.f + c2;
     } else {
+        const float b = P.half_dd - 0.5f - (float)rel * (1.0f / 16777216.0f);
+        float t0 = fminf(fmaxf(b, 0.f), P.dd);
+        float t1 = fminf(fmaxf(b + 1.f, 0.f), P.dd);
+        float t2 = fminf(fmaxf(b + 2.f, 0.f), P.dd);
         float g0 = shape_G<SHAPE>(t0, P.k_rad), g1 = shape_G<SHAPE>(t1, P.k_rad), g2 = shape_G<SHAPE>(t2, P.k_rad);
         W[0] = g0;
         W[1] = g1 - g0;
@@ -304,6 +315,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
 // particles a strip thread cannot serve from its register patch are listed per CTA and processed by all
 // threads after the strips (no divergence inside the strip loops); a full list spills to the global one
 constexpr int STRAY_CAP = 2048;
+constexpr int PF_ROWS = 2;            // L2 prefetch distance of the strips, in cell rows
 constexpr bool SHIFT_PATCH = true;   // one copy of the particle loop (instruction cache) at the price of register moves per cell
 constexpr uint32_t STRAY_DEP = 0x80000000u;            // flag: deposit only
 constexpr int64_t OVF_DEP = (int64_t)1 << 62;
@@ -356,9 +368,12 @@ __device__ __forceinline__ void load_force_window(const PartParams &P, int gx0, 
 // accesses fall into consecutive banks.  Logical patch row a (node row i-1+a of cell row i) lives in
 // physical row (a + ROT) & 3, so sliding to the next cell row renames rows instead of moving registers.
 struct Patch {
-    float Fx[4][4], Fy[4][4];
-    float dn[4][4], dpx[4][4], dpy[4][4];
+    float2 F[4][4];      // (Fx, Fy)
+    float2 dn[4][2];     // density deposit, columns (0,1) and (2,3)
+    float2 dp[4][4];     // momentum deposit (Px, Py)
 };
+
+__device__ __forceinline__ float2 dup2(float v) { return make_float2(v, v); }
 
 __device__ __forceinline__ bool in_patch(int rel) { return (uint32_t)(rel + (1 << 23)) < (1u << 25); }   // offset in [-1/2, 3/2)
 
@@ -384,7 +399,7 @@ template <int SHAPE, int STAGE, int QMASK, int ROT>
 __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, const StripCtx &c, const PV me, const float wme,
                                                const float2 uhme, const int64_t p, const uint32_t ax_fix)
 {
-    constexpr float INV24 = 1.0f / 16777216.0f;
+    constexpr float GS = 1.f / (W4Scale<SHAPE>::value * W4Scale<SHAPE>::value);   // undoes the scale of weights4
     float ux = me.ux, uy = me.uy;
     uint32_t xd = me.x, yd = me.y;                        // deposit position
     float Wx[4], Wy[4];
@@ -399,30 +414,29 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
             defer_stray(P, c.slist, c.scount, p, c.t0, c.tile, false);
             return;
         }
-        weights4<SHAPE>((float)rx * INV24, P, Wx);
-        weights4<SHAPE>((float)ry * INV24, P, Wy);
-        float fx = 0.f, fy = 0.f;                         // Eq. 15
+        weights4<SHAPE>(rx, P, Wx);
+        weights4<SHAPE>(ry, P, Wy);
+        float2 f = make_float2(0.f, 0.f);                 // Eq. 15, both components at once (FFMA2)
+        const float2 wy0 = dup2(Wy[0]), wy1 = dup2(Wy[1]), wy2 = dup2(Wy[2]), wy3 = dup2(Wy[3]);
 #pragma unroll
         for (int a = 0; a < 4; a++) {
-            float sx = 0.f, sy = 0.f;
-#pragma unroll
-            for (int b = 0; b < 4; b++) {
-                sx = fmaf(Wy[b], pt.Fx[(a + ROT) & 3][b], sx);
-                sy = fmaf(Wy[b], pt.Fy[(a + ROT) & 3][b], sy);
-            }
-            fx = fmaf(Wx[a], sx, fx);
-            fy = fmaf(Wx[a], sy, fy);
+            const int pa = (a + ROT) & 3;
+            float2 sa = __fmul2_rn(wy0, pt.F[pa][0]);
+            sa = __ffma2_rn(wy1, pt.F[pa][1], sa);
+            sa = __ffma2_rn(wy2, pt.F[pa][2], sa);
+            sa = __ffma2_rn(wy3, pt.F[pa][3], sa);
+            f = __ffma2_rn(dup2(Wx[a]), sa, f);
         }
         if (STAGE == 0) {
-            const float uhx = __fmaf_rn(P.dt, fx, ux), uhy = __fmaf_rn(P.dt, fy, uy);       // Eq. 17
+            const float uhx = __fmaf_rn(GS * P.dt, f.x, ux), uhy = __fmaf_rn(GS * P.dt, f.y, uy);   // Eq. 17
             P.uh[p] = make_float2(uhx, uhy);
             xd = advance(me.x, P.hx, __fadd_rn(uhx, ux));
             yd = advance(me.y, P.hy, __fadd_rn(uhy, uy));
             ux = uhx;
             uy = uhy;
         } else {
-            float unx = __fmaf_rn(0.5f * P.dt, fx, 0.5f * __fadd_rn(uhme.x, ux));             // Eq. 19
-            float uny = __fmaf_rn(0.5f * P.dt, fy, 0.5f * __fadd_rn(uhme.y, uy));
+            float unx = __fmaf_rn(0.5f * GS * P.dt, f.x, 0.5f * __fadd_rn(uhme.x, ux));             // Eq. 19
+            float uny = __fmaf_rn(0.5f * GS * P.dt, f.y, 0.5f * __fadd_rn(uhme.y, uy));
             xd = advance(me.x, P.hx, __fadd_rn(unx, ux));
             yd = advance(me.y, P.hy, __fadd_rn(uny, uy));
             reflect_x(xd, unx, c.gx0, P.nx);
@@ -438,25 +452,26 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
         defer_stray(P, c.slist, c.scount, p, c.t0, c.tile, true);
         return;
     }
-    weights4<SHAPE>((float)rx * INV24, P, Wx);
-    weights4<SHAPE>((float)ry * INV24, P, Wy);
-    const float q = wme * P.nscale;                       // Eq. 14 in fixed-point units
-    const float pr = P.pscale / P.nscale;
-    const float qux = ux * pr, quy = uy * pr;
+    weights4<SHAPE>(rx, P, Wx);
+    weights4<SHAPE>(ry, P, Wy);
+    const float q = wme * (GS * P.nscale);                // Eq. 14 in fixed-point units
+    const float2 qu = make_float2(ux * P.pratio, uy * P.pratio);
+    const float2 wy01 = make_float2(Wy[0], Wy[1]), wy23 = make_float2(Wy[2], Wy[3]);
+    const float2 wy0 = dup2(Wy[0]), wy1 = dup2(Wy[1]), wy2 = dup2(Wy[2]), wy3 = dup2(Wy[3]);
 #pragma unroll
     for (int a = 0; a < 4; a++) {
-        const float qa = Wx[a] * q;
+        const int pa = (a + ROT) & 3;
+        const float2 qa = dup2(Wx[a] * q);
         if (QMASK & 1) {
-#pragma unroll
-            for (int b = 0; b < 4; b++) pt.dn[(a + ROT) & 3][b] = fmaf(qa, Wy[b], pt.dn[(a + ROT) & 3][b]);
+            pt.dn[pa][0] = __ffma2_rn(qa, wy01, pt.dn[pa][0]);
+            pt.dn[pa][1] = __ffma2_rn(qa, wy23, pt.dn[pa][1]);
         }
         if (QMASK & 2) {
-            const float qxa = qa * qux, qya = qa * quy;
-#pragma unroll
-            for (int b = 0; b < 4; b++) {
-                pt.dpx[(a + ROT) & 3][b] = fmaf(qxa, Wy[b], pt.dpx[(a + ROT) & 3][b]);
-                pt.dpy[(a + ROT) & 3][b] = fmaf(qya, Wy[b], pt.dpy[(a + ROT) & 3][b]);
-            }
+            const float2 qp = __fmul2_rn(qa, qu);
+            pt.dp[pa][0] = __ffma2_rn(qp, wy0, pt.dp[pa][0]);
+            pt.dp[pa][1] = __ffma2_rn(qp, wy1, pt.dp[pa][1]);
+            pt.dp[pa][2] = __ffma2_rn(qp, wy2, pt.dp[pa][2]);
+            pt.dp[pa][3] = __ffma2_rn(qp, wy3, pt.dp[pa][3]);
         }
     }
 }
@@ -465,18 +480,20 @@ __device__ __forceinline__ void strip_particle(const PartParams &P, Patch &pt, c
 template <int QMASK, int PR>
 __device__ __forceinline__ void flush_row(Patch &pt, int32_t *dep, int wr, int wc0)
 {
+    const int e = wr * WPITCH + wc0;
+    if (QMASK & 1) {
+        atomicAdd(&dep[e], __float2int_rn(pt.dn[PR][0].x));
+        atomicAdd(&dep[e + 1], __float2int_rn(pt.dn[PR][0].y));
+        atomicAdd(&dep[e + 2], __float2int_rn(pt.dn[PR][1].x));
+        atomicAdd(&dep[e + 3], __float2int_rn(pt.dn[PR][1].y));
+        pt.dn[PR][0] = pt.dn[PR][1] = make_float2(0.f, 0.f);
+    }
+    if (QMASK & 2) {
 #pragma unroll
-    for (int b = 0; b < 4; b++) {
-        const int e = wr * WPITCH + wc0 + b;
-        if (QMASK & 1) {
-            atomicAdd(&dep[e], __float2int_rn(pt.dn[PR][b]));
-            pt.dn[PR][b] = 0.f;
-        }
-        if (QMASK & 2) {
-            atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(pt.dpx[PR][b]));
-            atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(pt.dpy[PR][b]));
-            pt.dpx[PR][b] = 0.f;
-            pt.dpy[PR][b] = 0.f;
+        for (int b = 0; b < 4; b++) {
+            atomicAdd(&dep[WIN * WPITCH + e + b], __float2int_rn(pt.dp[PR][b].x));
+            atomicAdd(&dep[2 * WIN * WPITCH + e + b], __float2int_rn(pt.dp[PR][b].y));
+            pt.dp[PR][b] = make_float2(0.f, 0.f);
         }
     }
 }
@@ -485,10 +502,20 @@ template <int PR>
 __device__ __forceinline__ void load_force_row(Patch &pt, const float2 *Fs, int wr, int wc0)
 {
 #pragma unroll
-    for (int b = 0; b < 4; b++) {
-        const float2 f = Fs[wr * WPITCH + wc0 + b];
-        pt.Fx[PR][b] = f.x;
-        pt.Fy[PR][b] = f.y;
+    for (int b = 0; b < 4; b++) pt.F[PR][b] = Fs[wr * WPITCH + wc0 + b];
+}
+
+__device__ __forceinline__ void prefetch_l2(const void *ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
+
+// DRAM -> L2 ahead of the strip: the particles of cell c of this thread's column
+template <int STAGE>
+__device__ __forceinline__ void prefetch_cell(const PartParams &P, const StripCtx &c, int cell)
+{
+    const int32_t q = c.coff[min(cell, TCELLS - 1)];
+    if (q < c.n_tile) {
+        prefetch_l2(P.pv + c.t0 + q);
+        prefetch_l2(P.w + c.t0 + q);
+        if (STAGE == 1) prefetch_l2(P.uh + c.t0 + q);
     }
 }
 
@@ -505,6 +532,7 @@ __device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, Strip
     // the other 31 lanes, so only its first cell_cap particles go through the patch, the rest to the stray list
     const int32_t fast_end = min(end, beg + c.cell_cap);
     int32_t q = beg;
+    prefetch_cell<STAGE>(P, c, cell + PF_ROWS * TILE);
     if (beg < fast_end && c.q != beg) {                                  // no prefetch in flight (strip start, after empty cells)
         c.cur = P.pv[c.t0 + beg];
         c.wcur = P.w[c.t0 + beg];
@@ -539,12 +567,15 @@ __device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, Strip
         for (int a = 0; a < 3; a++)
 #pragma unroll
             for (int b = 0; b < 4; b++) {
-                if (QMASK & 1) pt.dn[a][b] = pt.dn[a + 1][b];
-                if (QMASK & 2) { pt.dpx[a][b] = pt.dpx[a + 1][b]; pt.dpy[a][b] = pt.dpy[a + 1][b]; }
-                if (STAGE < 2) { pt.Fx[a][b] = pt.Fx[a + 1][b]; pt.Fy[a][b] = pt.Fy[a + 1][b]; }
+                if ((QMASK & 1) && b < 2) pt.dn[a][b] = pt.dn[a + 1][b];
+                if (QMASK & 2) pt.dp[a][b] = pt.dp[a + 1][b];
+                if (STAGE < 2) pt.F[a][b] = pt.F[a + 1][b];
             }
 #pragma unroll
-        for (int b = 0; b < 4; b++) pt.dn[3][b] = pt.dpx[3][b] = pt.dpy[3][b] = 0.f;
+        for (int b = 0; b < 4; b++) {
+            if (b < 2) pt.dn[3][b] = make_float2(0.f, 0.f);
+            pt.dp[3][b] = make_float2(0.f, 0.f);
+        }
         if (STAGE < 2) load_force_row<3>(pt, c.Fs, i + 3 + HALO, c.wc0);
     } else if (STAGE < 2)
         load_force_row<ROT>(pt, c.Fs, i + 3 + HALO, c.wc0);
@@ -603,7 +634,12 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 #pragma unroll
     for (int a = 0; a < 4; a++)
 #pragma unroll
-        for (int b = 0; b < 4; b++) pt.dn[a][b] = pt.dpx[a][b] = pt.dpy[a][b] = pt.Fx[a][b] = pt.Fy[a][b] = 0.f;
+        for (int b = 0; b < 4; b++) {
+            pt.F[a][b] = pt.dp[a][b] = make_float2(0.f, 0.f);
+            if (b < 2) pt.dn[a][b] = make_float2(0.f, 0.f);
+        }
+#pragma unroll
+    for (int k = 0; k < PF_ROWS; k++) prefetch_cell<STAGE>(P, ctx, (i0 + k) * TILE + j);
     if (STAGE < 2) {
         load_force_row<0>(pt, Fs, i0 - 1 + HALO, ctx.wc0);
         load_force_row<1>(pt, Fs, i0 + HALO, ctx.wc0);
@@ -1179,10 +1215,13 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
     P.hx = (float)(c->g.dt / (2.0 * c->g.dx));
     P.hy = (float)(c->g.dt / (2.0 * c->g.dy));
     P.nscale = c->nscale; P.pscale = c->pscale;
+    P.pratio = c->pscale / c->nscale;
     P.half_dd = (float)(0.5 * S.cfg.DD);
     P.dd = (float)S.cfg.DD;
     P.k_rad = (float)(3.14159265358979323846 / S.cfg.DD);
     P.cap_extra = c->cap_extra;
+    P.w4_slope = (float)(-3.14159265358979323846 / S.cfg.DD / 16777216.0);
+    P.w4_off = (float)((0.5 * S.cfg.DD - 0.5) * 3.14159265358979323846 / S.cfg.DD);
     return P;
 }
 
