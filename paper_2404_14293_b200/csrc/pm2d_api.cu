@@ -342,13 +342,10 @@ static int enqueue_step(pm2d_ctx *c)
     if ((rc = launch_field_step(c))) return rc;
     phase_end(c);
     for (int stage = 0; stage < 2; stage++) {
+        // E^n from n^n resp. E^ from n^ (Eqs. 9-11), and in the epilogue of the inverse transform the nodal
+        // force of (3) / (7): Eq. 16 with a^n, n^n / Eq. 18 with a^{n+1}, n^
         phase_begin(c, PM2D_PH_POISSON);
-        if ((rc = launch_poisson(c, false))) return rc;
-        phase_end(c);
-        // (3) / (7): nodal force of Eq. 16 with a^n, n^n, E^n / of Eq. 18 with a^{n+1}, n^, E^
-        phase_begin(c, PM2D_PH_FORCE);
-        for (int s = 0; s < c->nsp; s++)
-            if (c->sp[s].cfg.mobile && c->sp[s].np > 0 && (rc = launch_force(c, s, stage == 0 ? c->a[1] : c->a[0]))) return rc;
+        if ((rc = launch_poisson(c, false, stage == 0 ? c->a[1] : c->a[0]))) return rc;
         phase_end(c);
         // (3)-(5) gather, predictor, deposit / (7)-(8)+(1) gather, corrector, deposit -- one fused kernel
         phase_begin(c, stage == 0 ? PM2D_PH_STAGE_A : PM2D_PH_STAGE_B);

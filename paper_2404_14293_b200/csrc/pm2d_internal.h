@@ -137,6 +137,6 @@ int launch_fix_to_float(pm2d_ctx *c, const int32_t *src, float scale, float *dst
 int launch_float_to_fix(pm2d_ctx *c, const float *src, float scale, int32_t *dst);
 // pm2d_poisson.cu
 int launch_poisson_init(pm2d_ctx *c);
-int launch_poisson(pm2d_ctx *c, bool want_phi);
+int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a = nullptr);
 // pm2d_diag.cu
 int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out);

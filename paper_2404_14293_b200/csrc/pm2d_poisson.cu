@@ -85,40 +85,225 @@ __device__ float2 *fft_stockham(float2 *x, float2 *y, const float2 *__restrict__
     return x;
 }
 
-__global__ void __launch_bounds__(FFT_THREADS) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw, float2 *__restrict__ rho_hat,
-                                                         int ny, int LP)
+// ---- register-blocked FFT for n >= 512 ----------------------------------------------------------------
+// n/16 threads; every thread holds 16 points.  A pass reads the points of its radix-R butterflies (R = 16,
+// last pass 8 / 4 / 2) from shared memory into registers, transforms them there and writes them back in
+// Stockham order, so n = 4096 takes three passes and two exchanges through shared memory instead of six.
+// The buffer is padded by one element per 16 (index i -> i + i/16) against bank conflicts of the strided
+// writes.
+__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
+
+template <int IDX>
+__device__ __forceinline__ constexpr float cos16()
 {
-    extern __shared__ float2 buf[];
-    const int i = blockIdx.x + 1;                     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
-    const size_t row = (size_t)i * ny;
-    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
-        int v = 0;
-        for (int s = 0; s < S.count; s++) v += S.sign[s] * S.n[s][row + j];
-        buf[j] = make_float2((float)v * S.inv_nscale, 0.f);
-    }
-    float2 *r = fft_stockham<false>(buf, buf + ny, tw, ny);
-    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) rho_hat[(size_t)i * LP + l] = r[l];
+    return IDX == 0 ? 1.f : IDX == 1 ? 0.9238795325112867f : IDX == 2 ? 0.7071067811865476f : IDX == 3 ? 0.3826834323650898f
+         : IDX == 4 ? 0.f : IDX == 5 ? -0.3826834323650898f : IDX == 6 ? -0.7071067811865476f : -0.9238795325112867f;
+}
+template <int IDX>
+__device__ __forceinline__ constexpr float sin16()
+{
+    return IDX == 0 ? 0.f : IDX == 1 ? 0.3826834323650898f : IDX == 2 ? 0.7071067811865476f : IDX == 3 ? 0.9238795325112867f
+         : IDX == 4 ? 1.f : IDX == 5 ? 0.9238795325112867f : IDX == 6 ? 0.7071067811865476f : 0.3826834323650898f;
 }
 
-// MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part)
-template <int MODE>
-__global__ void __launch_bounds__(FFT_THREADS) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
+// o * exp(-/+ 2 pi i IDX / 16)
+template <int IDX, bool INV>
+__device__ __forceinline__ float2 mul_w16(float2 o)
+{
+    if (IDX == 0) return o;
+    if (IDX == 4) return INV ? make_float2(-o.y, o.x) : make_float2(o.y, -o.x);
+    const float c = cos16<IDX>(), sn = INV ? sin16<IDX>() : -sin16<IDX>();
+    return make_float2(o.x * c - o.y * sn, o.x * sn + o.y * c);
+}
+
+template <int R, bool INV, int K>
+struct DftCombine {
+    static __device__ __forceinline__ void run(float2 *v, const float2 *e, const float2 *o)
+    {
+        const float2 t = mul_w16<K * (16 / R), INV>(o[K]);
+        v[K] = make_float2(e[K].x + t.x, e[K].y + t.y);
+        v[K + R / 2] = make_float2(e[K].x - t.x, e[K].y - t.y);
+        if (K + 1 < R / 2) DftCombine<R, INV, (K + 1 < R / 2) ? K + 1 : K>::run(v, e, o);
+    }
+};
+
+// DFT of R points in registers, natural order in and out (radix-2 decimation in time, fully unrolled)
+template <int R, bool INV>
+__device__ __forceinline__ void dft_reg(float2 *v)
+{
+    if (R == 1) return;
+    float2 e[R / 2 > 0 ? R / 2 : 1], o[R / 2 > 0 ? R / 2 : 1];
+#pragma unroll
+    for (int k = 0; k < R / 2; k++) {
+        e[k] = v[2 * k];
+        o[k] = v[2 * k + 1];
+    }
+    dft_reg<(R > 1 ? R / 2 : 1), INV>(e);
+    dft_reg<(R > 1 ? R / 2 : 1), INV>(o);
+    DftCombine<(R > 1 ? R : 2), INV, 0>::run(v, e, o);
+}
+
+template <int R, bool INV>
+__device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict__ tw, int n, int Ns)
+{
+    constexpr int NB = 16 / R;
+    const int T = blockDim.x, q = n / R;
+    float2 v[NB][R];
+#pragma unroll
+    for (int b = 0; b < NB; b++) {
+        const int j = threadIdx.x + b * T;
+#pragma unroll
+        for (int r = 0; r < R; r++) v[b][r] = buf[pad16(j + r * q)];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < NB; b++) {
+        const int j = threadIdx.x + b * T, k = j & (Ns - 1);
+        if (Ns > 1) {
+            const int step = n / (Ns * R), h = n >> 1;
+#pragma unroll
+            for (int r = 1; r < R; r++) {
+                const int t = r * k * step;
+                float2 w = t < h ? tw[t] : tw[t - h];
+                if (t >= h) { w.x = -w.x; w.y = -w.y; }
+                if (INV) w.y = -w.y;
+                v[b][r] = cmul(v[b][r], w);
+            }
+        }
+        dft_reg<R, INV>(v[b]);
+        const int j0 = (j - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; r++) buf[pad16(j0 + r * Ns)] = v[b][r];
+    }
+    __syncthreads();
+}
+
+// in place on the padded buffer; blockDim.x == n / 16, n a power of two >= 512; callers synchronise before
+template <bool INV>
+__device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n)
+{
+    int Ns = 1;
+    while (n / Ns >= 16) {
+        fft16_pass<16, INV>(buf, tw, n, Ns);
+        Ns <<= 4;
+    }
+    const int rem = n / Ns;
+    if (rem == 8) fft16_pass<8, INV>(buf, tw, n, Ns);
+    else if (rem == 4) fft16_pass<4, INV>(buf, tw, n, Ns);
+    else if (rem == 2) fft16_pass<2, INV>(buf, tw, n, Ns);
+}
+
+// Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
+// rho^_b = (Z_l - conj Z_{n-l}) / 2i.  BIG: register-blocked FFT on the padded buffer (ny >= 512).
+template <bool BIG>
+__global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
+                                                                     float2 *__restrict__ rho_hat, int nx, int ny, int LP)
+{
+    extern __shared__ float2 buf[];
+    const int ia = 1 + 2 * blockIdx.x, ib = ia + 1;     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
+    const bool has_b = ib <= nx - 1;
+    const size_t rowa = (size_t)ia * ny, rowb = (size_t)ib * ny;
+    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+        int va = 0, vb = 0;
+        for (int s = 0; s < S.count; s++) {
+            va += S.sign[s] * S.n[s][rowa + j];
+            if (has_b) vb += S.sign[s] * S.n[s][rowb + j];
+        }
+        buf[BIG ? pad16(j) : j] = make_float2((float)va * S.inv_nscale, (float)vb * S.inv_nscale);
+    }
+    float2 *r = buf;
+    if (BIG) {
+        __syncthreads();
+        fft16_inplace<false>(buf, tw, ny);
+    } else
+        r = fft_stockham<false>(buf, buf + ny, tw, ny);
+    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) {
+        const int lc = (ny - l) & (ny - 1);
+        const float2 z = r[BIG ? pad16(l) : l], zc = r[BIG ? pad16(lc) : lc];
+        rho_hat[(size_t)ia * LP + l] = make_float2(0.5f * (z.x + zc.x), 0.5f * (z.y - zc.y));
+        if (has_b) rho_hat[(size_t)ib * LP + l] = make_float2(0.5f * (z.y + zc.y), 0.5f * (zc.x - z.x));
+    }
+}
+
+// nodal force of every mobile species, Eq. 16 / 18, evaluated in the epilogue of the inverse
+// transform of E (E enters the force only at the node itself):
+//   F = qE E_node - (1/2) grad(sum_c a_c^2) [electrons] - C v_th^2 grad(n)/n
+// central differences, one-sided on the wall rows, pressure term 0 where n = 0 (Q10)
+struct ForceOut {
+    const int32_t *nfix[PM2D_MAX_SPECIES];
+    float2 *F[PM2D_MAX_SPECIES];
+    float qE[PM2D_MAX_SPECIES], pond[PM2D_MAX_SPECIES], cv2[PM2D_MAX_SPECIES];
+    int count;
+    const float *a;          // [ncomp][nn], the level the stage needs (n or n+1)
+    int ncomp, nx;
+    float inv_2dx, inv_2dy;
+};
+
+// MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part);
+// MODE 2: Z = ehx + i ehy -> F_s of every mobile species (ForceOut)
+template <int MODE, bool BIG>
+__global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
-                                                      float *__restrict__ phi, int ny, int LP)
+                                                      float *__restrict__ phi, int ny, int LP, const ForceOut FO)
 {
     extern __shared__ float2 buf[];
     const int i = blockIdx.x;
     for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) {
         float2 a = hx[(size_t)i * LP + l];
-        float2 b = MODE == 0 ? hy[(size_t)i * LP + l] : make_float2(0.f, 0.f);
+        float2 b = MODE != 1 ? hy[(size_t)i * LP + l] : make_float2(0.f, 0.f);
         // Z_l = a + i b ; Z_{ny-l} = conj(a) + i conj(b)
-        buf[l] = make_float2(a.x - b.y, a.y + b.x);
-        if (l > 0 && l < ny / 2) buf[ny - l] = make_float2(a.x + b.y, -a.y + b.x);
+        buf[BIG ? pad16(l) : l] = make_float2(a.x - b.y, a.y + b.x);
+        if (l > 0 && l < ny / 2) buf[BIG ? pad16(ny - l) : ny - l] = make_float2(a.x + b.y, -a.y + b.x);
     }
-    float2 *r = fft_stockham<true>(buf, buf + ny, tw, ny);
+    float2 *r = buf;
+    if (BIG) {
+        __syncthreads();
+        fft16_inplace<true>(buf, tw, ny);
+    } else
+        r = fft_stockham<true>(buf, buf + ny, tw, ny);
+    if (MODE == 2) {
+        const size_t nn = (size_t)(FO.nx + 1) * ny;
+        const int il = i > 0 ? i - 1 : 0, ih = i < FO.nx ? i + 1 : FO.nx;
+        const float sx = (il == i || ih == i) ? 2.f * FO.inv_2dx : FO.inv_2dx;     // one-sided at the walls
+        const size_t row = (size_t)i * ny, rl = (size_t)il * ny, rh = (size_t)ih * ny;
+        bool any_pond = false;
+        for (int s = 0; s < FO.count; s++) any_pond |= FO.pond[s] != 0.f;
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
+            const float2 E = r[BIG ? pad16(j) : j];
+            float px = 0.f, py = 0.f;
+            if (any_pond) {
+                float ah = 0.f, al = 0.f, au = 0.f, ad = 0.f;
+                for (int c = 0; c < FO.ncomp; c++) {
+                    const float *ac = FO.a + c * nn;
+                    float v;
+                    v = ac[rh + j]; ah += v * v;
+                    v = ac[rl + j]; al += v * v;
+                    v = ac[row + jp]; au += v * v;
+                    v = ac[row + jm]; ad += v * v;
+                }
+                px = 0.5f * sx * (ah - al);
+                py = 0.5f * FO.inv_2dy * (au - ad);
+            }
+            for (int s = 0; s < FO.count; s++) {
+                float fx = FO.qE[s] * E.x, fy = FO.qE[s] * E.y;
+                if (FO.pond[s] != 0.f) { fx -= px; fy -= py; }
+                const int32_t *n = FO.nfix[s];
+                const int n0 = n[row + j];
+                if (n0 > 0 && FO.cv2[s] != 0.f) {
+                    const float inv_n = 1.f / (float)n0;
+                    fx -= FO.cv2[s] * sx * (float)(n[rh + j] - n[rl + j]) * inv_n;
+                    fy -= FO.cv2[s] * FO.inv_2dy * (float)(n[row + jp] - n[row + jm]) * inv_n;
+                }
+                FO.F[s][row + j] = make_float2(fx, fy);
+            }
+        }
+        return;
+    }
     for (int j = threadIdx.x; j < ny; j += blockDim.x) {
-        if (MODE == 0) Enode[(size_t)i * ny + j] = r[j];
-        else phi[(size_t)i * ny + j] = r[j].x;
+        const float2 z = r[BIG ? pad16(j) : j];
+        if (MODE == 0) Enode[(size_t)i * ny + j] = z;
+        else phi[(size_t)i * ny + j] = z.x;
     }
 }
 
@@ -344,20 +529,26 @@ int launch_poisson_init(pm2d_ctx *c)
     k_tri_tables<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T, ny, c->LP, c->tri_mlast, c->g.dx, ny * c->g.dy);
     count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
-    const int smem = 2 * ny * (int)sizeof(float2);
-    if (smem > 48 * 1024) {
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    const int smem = 2 * ny * (int)sizeof(float2);       // small-n path only (ny < 512): 8 KB at most
+    (void)smem;
+    {
+        const int big_smem = (8192 + 8192 / 16) * (int)sizeof(float2);
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
     }
     return PM2D_OK;
 }
 
-// rho from the current density grids -> nodal E (and phi if wanted, for diagnostics)
-int launch_poisson(pm2d_ctx *c, bool want_phi)
+// rho from the current density grids -> nodal E (and phi if wanted, for diagnostics); with force_a (a time
+// level of the vector potential) the nodal force of every mobile species instead of E
+int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
 {
     const int nx = c->g.nx, ny = c->g.ny;
-    const size_t smem = 2 * ny * sizeof(float2);
+    const bool big = ny >= 512;
+    const size_t smem = big ? (size_t)(ny + ny / 16) * sizeof(float2) : 2 * (size_t)ny * sizeof(float2);
+    const int fft_threads = big ? ny / 16 : FFT_THREADS;
     RhoSrc S;
     S.count = 0;
     S.inv_nscale = c->inv_nscale;
@@ -367,7 +558,8 @@ int launch_poisson(pm2d_ctx *c, bool want_phi)
             S.sign[S.count] = c->sp[s].cfg.sign;
             S.count++;
         }
-    k_fft_rho<<<nx - 1, FFT_THREADS, smem, c->stream>>>(S, c->twiddle, c->rho_hat, ny, c->LP);
+    if (big) k_fft_rho<true><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else k_fft_rho<false><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
     TriParams T;
     T.rho_hat = c->rho_hat; T.phi_hat = want_phi ? c->rho_hat : nullptr;
     T.tab = TriTables{c->tri_cp, c->tri_V, c->tri_W};
@@ -378,10 +570,31 @@ int launch_poisson(pm2d_ctx *c, bool want_phi)
     k_tri_sums<<<grid, 128, 0, c->stream>>>(T);
     k_tri_reduced<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
     k_tri_local<<<grid, 128, 0, c->stream>>>(T);
-    k_ifft<0><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP);
+    ForceOut FO;
+    FO.count = 0;
+    if (force_a) {
+        const double PI = 3.14159265358979323846;
+        for (int s = 0; s < c->nsp; s++) {
+            SpeciesDev &Q = c->sp[s];
+            if (!Q.cfg.mobile || Q.np == 0) continue;
+            const int k = FO.count++;
+            FO.nfix[k] = Q.nfix; FO.F[k] = Q.F;
+            FO.qE[k] = (float)(-(double)Q.cfg.sign * 4.0 * PI * PI / Q.cfg.mass);
+            FO.pond[k] = Q.cfg.sign < 0 ? 1.f : 0.f;
+            FO.cv2[k] = (float)(Q.cfg.pressure_coeff * Q.vth2);
+        }
+        FO.a = force_a; FO.ncomp = c->g.ncomp; FO.nx = nx;
+        FO.inv_2dx = (float)(1.0 / (2.0 * c->g.dx)); FO.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
+        if (big) k_ifft<2, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else k_ifft<2, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+    } else if (big)
+        k_ifft<0, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
+    else
+        k_ifft<0, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
     count_launch(c, 5);
     if (want_phi) {
-        k_ifft<1><<<nx + 1, FFT_THREADS, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP);
+        if (big) k_ifft<1, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
+        else k_ifft<1, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
         count_launch(c);
     }
     PM2D_CUDA_CHECK(cudaGetLastError());

@@ -273,10 +273,11 @@ def test_energy_history_parity_c1(P):
     sim.close()
 
 
-@pytest.mark.parametrize("nx", [24, 33, 65, 100])
-def test_poisson_partition_edge_cases(P, nx):
-    """x-partitioned chasing method: single partition, empty last partition (nx = 1 mod 32), ragged last one."""
-    ny = 16
+@pytest.mark.parametrize("nx,ny", [(24, 16), (33, 16), (65, 16), (100, 16), (24, 512), (17, 1024), (24, 2048), (17, 4096), (9, 8192)])
+def test_poisson_partition_edge_cases(P, nx, ny):
+    """x-partitioned chasing method: single partition, empty last partition (nx = 1 mod 32), ragged last one;
+    ny >= 512: the register-blocked FFT with every last-pass radix (512: 2, 1024: 4, 2048: 8, 4096: none, 8192: 2)
+    and an odd number of interior rows (two real rows share one complex transform)."""
     cfg = small_cfg("c3", nx, ny)
     sim = P.PM2D(cfg, eager_moments=1)
     orc, _ = oracle_from_config(cfg)
