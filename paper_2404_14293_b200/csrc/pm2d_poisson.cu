@@ -203,6 +203,7 @@ __global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_fft_rho(RhoSrc S, c
     const int ia = 1 + 2 * blockIdx.x, ib = ia + 1;     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
     const bool has_b = ib <= nx - 1;
     const size_t rowa = (size_t)ia * ny, rowb = (size_t)ib * ny;
+#pragma unroll 4
     for (int j = threadIdx.x; j < ny; j += blockDim.x) {
         int va = 0, vb = 0;
         for (int s = 0; s < S.count; s++) {
@@ -248,6 +249,7 @@ __global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_ifft(const float2 *
 {
     extern __shared__ float2 buf[];
     const int i = blockIdx.x;
+#pragma unroll 4
     for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) {
         float2 a = hx[(size_t)i * LP + l];
         float2 b = MODE != 1 ? hy[(size_t)i * LP + l] : make_float2(0.f, 0.f);
@@ -268,35 +270,67 @@ __global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_ifft(const float2 *
         const size_t row = (size_t)i * ny, rl = (size_t)il * ny, rh = (size_t)ih * ny;
         bool any_pond = false;
         for (int s = 0; s < FO.count; s++) any_pond |= FO.pond[s] != 0.f;
-        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
-            const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
-            const float2 E = r[BIG ? pad16(j) : j];
-            float px = 0.f, py = 0.f;
+        // four nodes per thread at a time, all loads of a batch issued before the arithmetic
+        constexpr int NB = 2;
+        for (int jb = threadIdx.x; jb < ny; jb += NB * blockDim.x) {
+            int jj[NB], jm[NB], jp[NB];
+            float px[NB], py[NB];
+#pragma unroll
+            for (int u = 0; u < NB; u++) {
+                jj[u] = min(jb + u * (int)blockDim.x, ny - 1);           // clamped duplicates are not stored
+                jm[u] = (jj[u] - 1) & (ny - 1);
+                jp[u] = (jj[u] + 1) & (ny - 1);
+                px[u] = py[u] = 0.f;
+            }
+            int n0[PM2D_MAX_SPECIES][NB], nh[PM2D_MAX_SPECIES][NB], nl[PM2D_MAX_SPECIES][NB], nu[PM2D_MAX_SPECIES][NB],
+                nd[PM2D_MAX_SPECIES][NB];
+#pragma unroll
+            for (int s = 0; s < PM2D_MAX_SPECIES; s++)
+                if (s < FO.count) {
+                    const int32_t *n = FO.nfix[s];
+#pragma unroll
+                    for (int u = 0; u < NB; u++) {
+                        n0[s][u] = n[row + jj[u]];
+                        nh[s][u] = n[rh + jj[u]];
+                        nl[s][u] = n[rl + jj[u]];
+                        nu[s][u] = n[row + jp[u]];
+                        nd[s][u] = n[row + jm[u]];
+                    }
+                }
             if (any_pond) {
-                float ah = 0.f, al = 0.f, au = 0.f, ad = 0.f;
                 for (int c = 0; c < FO.ncomp; c++) {
                     const float *ac = FO.a + c * nn;
-                    float v;
-                    v = ac[rh + j]; ah += v * v;
-                    v = ac[rl + j]; al += v * v;
-                    v = ac[row + jp]; au += v * v;
-                    v = ac[row + jm]; ad += v * v;
+                    float vh[NB], vl[NB], vu[NB], vd[NB];
+#pragma unroll
+                    for (int u = 0; u < NB; u++) {
+                        vh[u] = ac[rh + jj[u]];
+                        vl[u] = ac[rl + jj[u]];
+                        vu[u] = ac[row + jp[u]];
+                        vd[u] = ac[row + jm[u]];
+                    }
+#pragma unroll
+                    for (int u = 0; u < NB; u++) {
+                        px[u] += 0.5f * sx * (vh[u] * vh[u] - vl[u] * vl[u]);
+                        py[u] += 0.5f * FO.inv_2dy * (vu[u] * vu[u] - vd[u] * vd[u]);
+                    }
                 }
-                px = 0.5f * sx * (ah - al);
-                py = 0.5f * FO.inv_2dy * (au - ad);
             }
-            for (int s = 0; s < FO.count; s++) {
-                float fx = FO.qE[s] * E.x, fy = FO.qE[s] * E.y;
-                if (FO.pond[s] != 0.f) { fx -= px; fy -= py; }
-                const int32_t *n = FO.nfix[s];
-                const int n0 = n[row + j];
-                if (n0 > 0 && FO.cv2[s] != 0.f) {
-                    const float inv_n = 1.f / (float)n0;
-                    fx -= FO.cv2[s] * sx * (float)(n[rh + j] - n[rl + j]) * inv_n;
-                    fy -= FO.cv2[s] * FO.inv_2dy * (float)(n[row + jp] - n[row + jm]) * inv_n;
+#pragma unroll
+            for (int s = 0; s < PM2D_MAX_SPECIES; s++)
+                if (s < FO.count) {
+#pragma unroll
+                    for (int u = 0; u < NB; u++) {
+                        const float2 E = r[BIG ? pad16(jj[u]) : jj[u]];
+                        float fx = FO.qE[s] * E.x, fy = FO.qE[s] * E.y;
+                        if (FO.pond[s] != 0.f) { fx -= px[u]; fy -= py[u]; }
+                        if (n0[s][u] > 0 && FO.cv2[s] != 0.f) {
+                            const float inv_n = 1.f / (float)n0[s][u];
+                            fx -= FO.cv2[s] * sx * (float)(nh[s][u] - nl[s][u]) * inv_n;
+                            fy -= FO.cv2[s] * FO.inv_2dy * (float)(nu[s][u] - nd[s][u]) * inv_n;
+                        }
+                        if (jb + u * (int)blockDim.x < ny) FO.F[s][row + jj[u]] = make_float2(fx, fy);
+                    }
                 }
-                FO.F[s][row + j] = make_float2(fx, fy);
-            }
         }
         return;
     }
@@ -404,25 +438,51 @@ __global__ void __launch_bounds__(32) k_tri_reduced(const TriParams T)
     // forward: row k: Vm g_{k-1} + (Wm + b + V1(k)) g_k + W1 g_{k+1} = r_{kM} + S_W(k-1) + S_V(k)
     double cprev = 0.0, dr = 0.0, di = 0.0;
     double2 *cd = T.g;                       // store d_k in g[k] and c'_k in sumV[k].x (free after read)
-    for (int k = 1; k <= P - 1; k++) {
-        float2 r = T.rho_hat[(size_t)(k * M) * LP + l];
-        double2 sw = T.sumW[(size_t)(k - 1) * LP + l], sv = T.sumV[(size_t)k * LP + l];
-        double diag = Wm + b + (k == P - 1 ? V1_last : V1);
-        double den = 1.0 / (diag - Vm * cprev);
-        double Rr = T.dx2 * (double)r.x + sw.x + sv.x, Ri = T.dx2 * (double)r.y + sw.y + sv.y;
-        dr = (Rr - Vm * dr) * den;
-        di = (Ri - Vm * di) * den;
-        cprev = W1 * den;
-        cd[(size_t)k * LP + l] = make_double2(dr, di);
-        T.sumV[(size_t)k * LP + l].x = cprev;
+    constexpr int CH = 8;                    // the inputs of CH rows are loaded before their (serial) elimination
+    for (int k0 = 1; k0 <= P - 1; k0 += CH) {
+        float2 r[CH];
+        double2 sw[CH], sv[CH];
+#pragma unroll
+        for (int u = 0; u < CH; u++) {
+            const int k = min(k0 + u, P - 1);
+            r[u] = T.rho_hat[(size_t)(k * M) * LP + l];
+            sw[u] = T.sumW[(size_t)(k - 1) * LP + l];
+            sv[u] = T.sumV[(size_t)k * LP + l];
+        }
+#pragma unroll
+        for (int u = 0; u < CH; u++) {
+            const int k = k0 + u;
+            if (k <= P - 1) {
+                double diag = Wm + b + (k == P - 1 ? V1_last : V1);
+                double den = 1.0 / (diag - Vm * cprev);
+                double Rr = T.dx2 * (double)r[u].x + sw[u].x + sv[u].x, Ri = T.dx2 * (double)r[u].y + sw[u].y + sv[u].y;
+                dr = (Rr - Vm * dr) * den;
+                di = (Ri - Vm * di) * den;
+                cprev = W1 * den;
+                cd[(size_t)k * LP + l] = make_double2(dr, di);
+                T.sumV[(size_t)k * LP + l].x = cprev;
+            }
+        }
     }
     double gr = 0.0, gi = 0.0;
-    for (int k = P - 1; k >= 1; k--) {
-        double2 d = cd[(size_t)k * LP + l];
-        double c = T.sumV[(size_t)k * LP + l].x;
-        gr = d.x - c * gr;
-        gi = d.y - c * gi;
-        cd[(size_t)k * LP + l] = make_double2(gr, gi);
+    for (int k0 = P - 1; k0 >= 1; k0 -= CH) {
+        double2 d[CH];
+        double cc[CH];
+#pragma unroll
+        for (int u = 0; u < CH; u++) {
+            const int k = max(k0 - u, 1);
+            d[u] = cd[(size_t)k * LP + l];
+            cc[u] = T.sumV[(size_t)k * LP + l].x;
+        }
+#pragma unroll
+        for (int u = 0; u < CH; u++) {
+            const int k = k0 - u;
+            if (k >= 1) {
+                gr = d[u].x - cc[u] * gr;
+                gi = d[u].y - cc[u] * gi;
+                cd[(size_t)k * LP + l] = make_double2(gr, gi);
+            }
+        }
     }
 }
 
