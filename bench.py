@@ -32,6 +32,18 @@ BYTES_STAGE_A = 28   # read x, y, ux, uy, w (20 B), write u^ (8 B)            --
 BYTES_STAGE_B = 44   # read x, y, ux, uy, w, u^ (28 B), write x, y, ux, uy (16 B)
 
 
+def job_throughput(units_per_rank, steps, ms_local, world=1, device=None):
+    """Whole-job throughput: the units all ranks processed divided by the slowest rank's device time
+    (max over ranks; the path does not shard, so ranks are independent replicas)."""
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return units_per_rank * world * steps / (ms_max * 1e-3), ms_max
+
+
 def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -147,6 +159,7 @@ def run_cuda(args):
 
     # ---- device-timed region: K steps, inputs resident in HBM ---------------------------------
     sim.step(args.warmup)
+    sim.stray_count()
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
@@ -163,11 +176,8 @@ def run_cuda(args):
     prof = sim.profile_get()
     sim.profile_enable(False)
     clocks = sampler.stop() if sampler else None
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = nmob * world * args.steps / (ms_max * 1e-3)
+    strays = sim.stray_count()
+    value, ms_max = job_throughput(nmob, args.steps, ms, world, dev)
 
     # ---- end to end through the C ABI with host buffers: per step the host sends the laser table
     # (H2D, kernel arguments) and reads back the left-boundary probe column of a ----------
@@ -181,10 +191,7 @@ def run_cuda(args):
         sim.get_fields(pkg.FIELD_A, 0, 0, window=(0, 1, 0, g["ny"]), out=probe)
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = nmob * world * args.steps / float(t.item())
+    e2e_value, _ = job_throughput(nmob, args.steps, e2e_s * 1e3, world, dev)
 
     if rank == 0:
         peak, peak_src = hbm_peak()
@@ -212,10 +219,11 @@ def run_cuda(args):
                     cell_updates_per_s=nodes * g["ncomp"] * world * args.steps / (ms_max * 1e-3),
                     field_kernel_node_updates_per_s=(nodes * g["ncomp"] / (prof["ms"]["field"] / steps_p * 1e-3)) if prof["ms"]["field"] > 0 else None,
                     phases_ms_per_step={k: v / steps_p for k, v in prof["ms"].items()},
+                    stray_fraction=strays / max(2.0 * nmob * args.steps, 1.0),
                     clocks=clocks, gpu_launches=int(launches),
                     e2e=dict(value=e2e_value, unit="particle-steps/s",
                              h2d_bytes_per_step=int(len(lasers) * 48), d2h_bytes_per_step=int(g["ny"] * 4 + 16)),
-                    roofline=dict(bound="hbm", kernel="k_stage (fused gather-push-deposit, stage A + stage B, all mobile species)",
+                    roofline=dict(bound="hbm", kernel="k_stage (fused gather-push-deposit; per step: stage A + stage B launches of every mobile species)",
                                   achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, peak_source=peak_src,
                                   algorithmic_bytes_per_particle_step=BYTES_STAGE_A + BYTES_STAGE_B,
                                   ms_per_step=stage_ms, traffic=traffic))

@@ -625,7 +625,8 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     ctx.ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
     ctx.j = j; ctx.wc0 = j - 1 + HALO; ctx.tile = tile; ctx.gx0 = gx0;
     ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
-    ctx.cell_cap = min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + P.cap_extra);
+    // ceil(mean particles per cell); sparse tiles (mean <= 1.5) get one more, or a third of them would stray
+    ctx.cell_cap = min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + (2 * ctx.n_tile <= 3 * TCELLS ? 1 : 0) + P.cap_extra);
     ctx.q = -1;
     ctx.cur = PV{0u, 0u, 0.f, 0.f};
     ctx.wcur = 0.f;
