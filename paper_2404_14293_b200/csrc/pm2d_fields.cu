@@ -24,7 +24,7 @@ __device__ __forceinline__ float ne_at(const NeSrc &S, size_t k)
 
 // Eq. 6.  CTA = 128 columns x ROWS rows; each thread marches along x keeping a[i-1], a[i], a[i+1]
 // in registers; the y neighbours come from the same cache lines through L1.
-constexpr int FCOLS = 128, FROWS = 32;
+constexpr int FCOLS = 128, FROWS = 32, FBATCH = 4;
 __global__ void __launch_bounds__(FCOLS) k_wave(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap,
                                                 NeSrc ne, int nx, int ny, float cx, float cy, float dt2)
 {
@@ -34,15 +34,29 @@ __global__ void __launch_bounds__(FCOLS) k_wave(const float *__restrict__ a, con
     if (i0 >= i1) return;
     const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
     float lo = a[(size_t)(i0 - 1) * ny + j], mid = a[(size_t)i0 * ny + j];
-    for (int i = i0; i < i1; i++) {
-        const size_t row = (size_t)i * ny;
-        float hi = a[row + ny + j];
-        float l = a[row + jm], r = a[row + jp];
-        float lap = cx * (hi - 2.f * mid + lo) + cy * (r - 2.f * mid + l);
-        float src = FOUR_PI2 * ne_at(ne, row + j) * mid;
-        ap[row + j] = 2.f * mid - am[row + j] + dt2 * (lap - src);
-        lo = mid;
-        mid = hi;
+    for (int ib = i0; ib < i1; ib += FBATCH) {
+        // the loads of FBATCH rows are issued together: the march itself is a chain of dependent rows
+        float hi[FBATCH], l[FBATCH], r[FBATCH], old[FBATCH], den[FBATCH];
+#pragma unroll
+        for (int u = 0; u < FBATCH; u++) {
+            const size_t row = (size_t)min(ib + u, i1 - 1) * ny;
+            hi[u] = a[row + ny + j];
+            l[u] = a[row + jm];
+            r[u] = a[row + jp];
+            old[u] = am[row + j];
+            den[u] = ne_at(ne, row + j);
+        }
+#pragma unroll
+        for (int u = 0; u < FBATCH; u++) {
+            if (ib + u < i1) {
+                const size_t row = (size_t)(ib + u) * ny;
+                float lap = cx * (hi[u] - 2.f * mid + lo) + cy * (r[u] - 2.f * mid + l[u]);
+                float src = FOUR_PI2 * den[u] * mid;
+                ap[row + j] = 2.f * mid - old[u] + dt2 * (lap - src);
+                lo = mid;
+                mid = hi[u];
+            }
+        }
     }
 }
 

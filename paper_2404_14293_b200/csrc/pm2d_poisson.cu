@@ -203,14 +203,37 @@ __global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_fft_rho(RhoSrc S, c
     const int ia = 1 + 2 * blockIdx.x, ib = ia + 1;     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
     const bool has_b = ib <= nx - 1;
     const size_t rowa = (size_t)ia * ny, rowb = (size_t)ib * ny;
-#pragma unroll 4
-    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
-        int va = 0, vb = 0;
+    if (BIG) {
+        // blockDim.x == ny / 16: every thread owns 16 columns; all loads are issued before the first use
+        int va[16], vb[16];
+#pragma unroll
+        for (int k = 0; k < 16; k++) va[k] = vb[k] = 0;
         for (int s = 0; s < S.count; s++) {
-            va += S.sign[s] * S.n[s][rowa + j];
-            if (has_b) vb += S.sign[s] * S.n[s][rowb + j];
+            const int32_t *na = S.n[s] + rowa, *nb = S.n[s] + (has_b ? rowb : rowa);
+            int ta[16], tb[16];
+#pragma unroll
+            for (int k = 0; k < 16; k++) {
+                ta[k] = na[threadIdx.x + k * blockDim.x];
+                tb[k] = nb[threadIdx.x + k * blockDim.x];
+            }
+#pragma unroll
+            for (int k = 0; k < 16; k++) {
+                va[k] += S.sign[s] * ta[k];
+                vb[k] += S.sign[s] * tb[k];
+            }
         }
-        buf[BIG ? pad16(j) : j] = make_float2((float)va * S.inv_nscale, (float)vb * S.inv_nscale);
+#pragma unroll
+        for (int k = 0; k < 16; k++)
+            buf[pad16(threadIdx.x + k * blockDim.x)] = make_float2((float)va[k] * S.inv_nscale, has_b ? (float)vb[k] * S.inv_nscale : 0.f);
+    } else {
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            int va = 0, vb = 0;
+            for (int s = 0; s < S.count; s++) {
+                va += S.sign[s] * S.n[s][rowa + j];
+                if (has_b) vb += S.sign[s] * S.n[s][rowb + j];
+            }
+            buf[j] = make_float2((float)va * S.inv_nscale, (float)vb * S.inv_nscale);
+        }
     }
     float2 *r = buf;
     if (BIG) {
