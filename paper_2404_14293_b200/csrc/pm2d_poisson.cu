@@ -195,8 +195,8 @@ __device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n)
 
 // Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
 // rho^_b = (Z_l - conj Z_{n-l}) / 2i.  BIG: register-blocked FFT on the padded buffer (ny >= 512).
-template <bool BIG>
-__global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
+template <int BIG>
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
                                                                      float2 *__restrict__ rho_hat, int nx, int ny, int LP)
 {
     extern __shared__ float2 buf[];
@@ -263,10 +263,11 @@ struct ForceOut {
     float inv_2dx, inv_2dy;
 };
 
+// BIG: 0 = radix-4 Stockham (ny < 512), 1 = register-blocked FFT with ny/16 <= 256 threads, 2 = with 512 threads (ny = 8192).
 // MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part);
 // MODE 2: Z = ehx + i ehy -> F_s of every mobile species (ForceOut)
-template <int MODE, bool BIG>
-__global__ void __launch_bounds__(BIG ? 512 : FFT_THREADS) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
+template <int MODE, int BIG>
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
                                                       float *__restrict__ phi, int ny, int LP, const ForceOut FO)
 {
@@ -616,10 +617,14 @@ int launch_poisson_init(pm2d_ctx *c)
     (void)smem;
     {
         const int big_smem = (8192 + 8192 / 16) * (int)sizeof(float2);
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
-        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
     }
     return PM2D_OK;
 }
@@ -629,7 +634,7 @@ int launch_poisson_init(pm2d_ctx *c)
 int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
 {
     const int nx = c->g.nx, ny = c->g.ny;
-    const bool big = ny >= 512;
+    const int big = ny >= 8192 ? 2 : (ny >= 512 ? 1 : 0);
     const size_t smem = big ? (size_t)(ny + ny / 16) * sizeof(float2) : 2 * (size_t)ny * sizeof(float2);
     const int fft_threads = big ? ny / 16 : FFT_THREADS;
     RhoSrc S;
@@ -641,8 +646,9 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
             S.sign[S.count] = c->sp[s].cfg.sign;
             S.count++;
         }
-    if (big) k_fft_rho<true><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
-    else k_fft_rho<false><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    if (big == 2) k_fft_rho<2><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else if (big == 1) k_fft_rho<1><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else k_fft_rho<0><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
     TriParams T;
     T.rho_hat = c->rho_hat; T.phi_hat = want_phi ? c->rho_hat : nullptr;
     T.tab = TriTables{c->tri_cp, c->tri_V, c->tri_W};
@@ -668,16 +674,20 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
         }
         FO.a = force_a; FO.ncomp = c->g.ncomp; FO.nx = nx;
         FO.inv_2dx = (float)(1.0 / (2.0 * c->g.dx)); FO.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
-        if (big) k_ifft<2, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
-        else k_ifft<2, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
-    } else if (big)
-        k_ifft<0, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
+        if (big == 2) k_ifft<2, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (big == 1) k_ifft<2, 1><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else k_ifft<2, 0><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+    } else if (big == 2)
+        k_ifft<0, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
+    else if (big == 1)
+        k_ifft<0, 1><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
     else
-        k_ifft<0, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
+        k_ifft<0, 0><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, c->Enode, nullptr, ny, c->LP, FO);
     count_launch(c, 5);
     if (want_phi) {
-        if (big) k_ifft<1, true><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
-        else k_ifft<1, false><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
+        if (big == 2) k_ifft<1, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
+        else if (big == 1) k_ifft<1, 1><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
+        else k_ifft<1, 0><<<nx + 1, fft_threads, smem, c->stream>>>(c->rho_hat, nullptr, c->twiddle, nullptr, c->phi, ny, c->LP, FO);
         count_launch(c);
     }
     PM2D_CUDA_CHECK(cudaGetLastError());
