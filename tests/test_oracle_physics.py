@@ -165,3 +165,44 @@ def test_count_and_charge_conserved_over_steps():
         assert ((o.sp[0]["X"] >= 0) & (o.sp[0]["X"] <= nx)).all()
         assert ((o.sp[0]["Y"] >= 0) & (o.sp[0]["Y"] < ny)).all()
     assert o.sp[0]["X"].size == npart
+
+
+def _quiet_maxwellian_mode(T_keV, nsteps, nx=64, ny=2, ppc=32, n0=0.01, dx=0.05, dt=0.035, eps=0.05):
+    """Lattice in x with the ppc quantiles of a Maxwellian in every cell (bit-reversed over the slots: a
+    'quiet start', no shot noise in the long modes), pressure term off (C = 0): kinetic electrons."""
+    from statistics import NormalDist
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    xs, ys = (np.arange(nx * ppc) + 0.5) / ppc, np.arange(ny) + 0.5
+    X0, Y0 = [a.ravel() for a in np.meshgrid(xs, ys, indexing="ij")]
+    w = np.full(X0.size, n0 / ppc)
+    n_bg, _, _ = oracle.deposit(g, oracle.SINE, 1.9, X0, Y0, 0 * X0, 0 * X0, w)
+    q = np.array([NormalDist().inv_cdf((k + 0.5) / ppc) for k in range(ppc)])
+    bits = int(math.log2(ppc))
+    rev = np.array([int(format(k, f"0{bits}b")[::-1], 2) for k in range(ppc)])
+    ux = np.repeat(math.sqrt(T_keV / 511.0) * q[rev[np.arange(nx * ppc) % ppc]], ny)
+    K = 2 * math.pi / nx
+    sp = [dict(sign=-1, mass=1.0, T_keV=T_keV, C=0.0, shape=oracle.SINE, DD=1.9, mobile=1,
+               X=X0 + eps * np.sin(K * X0), Y=Y0, ux=ux, uy=0 * X0, w=w),
+          dict(sign=1, mass=1836.0, T_keV=0.0, mobile=0, shape=oracle.SINE, DD=1.9, n_fixed=n_bg)]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    basis = np.cos(K * np.arange(nx + 1))[:, None]
+    t, amp = [], []
+    for n in range(nsteps):
+        amp.append(((o.moment(0, "n") - n_bg) * basis).sum())
+        t.append(n * dt)
+        o.step()
+    return np.array(t), np.array(amp)
+
+
+def test_P12b_bohm_gross_maxwellian_load():
+    """Kinetic electrons (Maxwellian momenta, C = 0): omega^2 = omega_pe^2 + 3 k^2 v_th^2 (BASELINE.json's
+    Bohm-Gross check), measured from the mode amplitude against the cold run of the same grid so that grid
+    and shape corrections cancel.  k lambda_D = 0.2: Bohm-Gross 1.0583, exact kinetic root 1.0640; the
+    fluid closure of Eq. 2 (coefficient 2, P12a) would give 1.0392."""
+    n0, kl = 0.01, 0.2
+    vth = kl * math.sqrt(n0) / (1.0 / (64 * 0.05))            # k v_th / omega_pe = kl, both per 2 pi
+    tc, ac = _quiet_maxwellian_mode(0.0, 1500)
+    tw, aw = _quiet_maxwellian_mode(vth * vth * 511.0, 1500)
+    ratio = _period_from_zero_crossings(tc, ac) / _period_from_zero_crossings(tw, aw)
+    assert ratio == pytest.approx(math.sqrt(1.0 + 3.0 * kl * kl), abs=0.008)
+    assert ratio > math.sqrt(1.0 + 2.0 * kl * kl) + 0.012
