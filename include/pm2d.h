@@ -49,9 +49,11 @@ extern "C" {
 enum { PM2D_CIC = 0, PM2D_TSC = 1, PM2D_SINE = 2 };
 /* particle loading: NONE = no particles generated (fixed background or
  * particles supplied by pm2d_set_particles); LATTICE_COLD = even lattice, u = 0;
- * RANDOM_MAXWELL = uniform-random offsets, Maxwellian u (BASELINE.json configs; Q7). */
-enum { PM2D_LOAD_NONE = 0, PM2D_LATTICE_COLD = 1, PM2D_RANDOM_MAXWELL = 2 };
-enum { PM2D_PROFILE_UNIFORM = 0, PM2D_PROFILE_LINEAR = 1, PM2D_PROFILE_EXP_CAPPED = 2 };
+ * RANDOM_MAXWELL = uniform-random offsets, Maxwellian u (BASELINE.json configs; Q7);
+ * NUMBER_WEIGHTED = equal weights p[0]/(ppc_x ppc_y), the number of particles of a cell follows the profile
+ * (floor(ppc * taper(i) * filament(j) + dither), BASELINE.json config 5); needs `capacity` >= the total. */
+enum { PM2D_LOAD_NONE = 0, PM2D_LATTICE_COLD = 1, PM2D_RANDOM_MAXWELL = 2, PM2D_NUMBER_WEIGHTED = 3 };
+enum { PM2D_PROFILE_UNIFORM = 0, PM2D_PROFILE_LINEAR = 1, PM2D_PROFILE_EXP_CAPPED = 2, PM2D_PROFILE_FILAMENT_Y = 3 };
 /* fields for pm2d_get_fields / pm2d_set_fields */
 enum {
     PM2D_FIELD_A = 0,      /* vector potential component `comp`, time level `level` (0 = n, 1 = n-1) */
@@ -84,13 +86,14 @@ typedef struct {
     int32_t mobile;        /* 0: fixed neutralising background (Q13)                                  */
     int32_t load;          /* PM2D_LOAD_*                                                             */
     int32_t ppc_x, ppc_y;  /* N, M of P:L154                                                          */
-    int64_t capacity;      /* particle slots when load == NONE and mobile (pm2d_set_particles); else 0 */
+    int64_t capacity;      /* particle slots when load == NONE (pm2d_set_particles) or NUMBER_WEIGHTED; else 0 */
 } pm2d_species;
 
 typedef struct {
     int32_t kind;          /* PM2D_PROFILE_*                                                          */
     int32_t taper_cells;   /* sin^2 edge taper at both x walls (Q9); 0 = none                         */
-    double p[4];           /* UNIFORM: n0. LINEAR: n(0), n(Lx). EXP_CAPPED: n0, Lx/L, cap    */
+    double p[4];           /* UNIFORM: n0. LINEAR: n(0), n(Lx). EXP_CAPPED: n0, Lx/L, cap.
+                              FILAMENT_Y: mean n0, amplitude A, sigma in cells: n(j) ~ 1 + A exp(-(y-Ly/2)^2/2 sigma^2) */
 } pm2d_profile;
 
 typedef struct {

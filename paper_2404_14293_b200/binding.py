@@ -16,8 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libpm2d.so")
 
 MAX_SPECIES, MAX_LASERS, TILE = 4, 4, 32
 CIC, TSC, SINE = 0, 1, 2
-LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL = 0, 1, 2
-PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED = 0, 1, 2
+LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
+PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
 FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
 PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")

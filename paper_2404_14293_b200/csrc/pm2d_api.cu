@@ -46,7 +46,7 @@ bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 int64_t species_np(const pm2d_grid &g, const pm2d_species &s)
 {
     if (!s.mobile) return 0;
-    if (s.load == PM2D_LOAD_NONE) return s.capacity;
+    if (s.load == PM2D_LOAD_NONE || s.load == PM2D_NUMBER_WEIGHTED) return s.capacity;
     return (int64_t)g.nx * g.ny * s.ppc_x * s.ppc_y;
 }
 
@@ -69,7 +69,7 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
         else if (q.shape == PM2D_TSC) { if (q.DD != 2.0) return fail(PM2D_EINVAL, "TSC needs DD = 2"); }
         else if (q.shape == PM2D_SINE) { if (!(q.DD > 0.0) || q.DD > 2.0) return fail(PM2D_EINVAL, "SINE needs 0 < DD <= 2 (3-node footprint)"); }
         else return fail(PM2D_EINVAL, "unknown shape");
-        if (q.load < PM2D_LOAD_NONE || q.load > PM2D_RANDOM_MAXWELL) return fail(PM2D_EINVAL, "unknown load");
+        if (q.load < PM2D_LOAD_NONE || q.load > PM2D_NUMBER_WEIGHTED) return fail(PM2D_EINVAL, "unknown load");
         if (q.load != PM2D_LOAD_NONE && (q.ppc_x < 1 || q.ppc_y < 1)) return fail(PM2D_EINVAL, "ppc_x, ppc_y must be >= 1");
         if (q.load != PM2D_LOAD_NONE && !q.mobile) return fail(PM2D_EINVAL, "an immobile species is a fixed background: load must be NONE");
         if (species_np(*g, q) < 0 || species_np(*g, q) > ((int64_t)1 << 31) - 1) return fail(PM2D_EINVAL, "particle count out of range");
@@ -105,6 +105,8 @@ size_t layout(pm2d_ctx *c, char *base)
     c->twiddle = cv.take<float2>(g.ny / 2);
     c->red = cv.take<double>(64);
     c->flags = cv.take<int32_t>(4);
+    c->shape_y = cv.take<double>(g.ny);
+    c->taper_x = cv.take<double>(g.nx);
     c->stray_total = cv.take<unsigned long long>(1);
     c->ovf_cap = 1 << 20;
     c->ovf_p = cv.take<int64_t>(c->ovf_cap);
@@ -230,11 +232,14 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     if (nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
     for (int l = 0; l < nlaser; l++)
         if (lasers[l].comp < 0 || lasers[l].comp >= grid->ncomp) return fail(PM2D_EINVAL, "laser component out of range");
-    if (profile->kind < PM2D_PROFILE_UNIFORM || profile->kind > PM2D_PROFILE_EXP_CAPPED) return fail(PM2D_EINVAL, "unknown profile");
+    if (profile->kind < PM2D_PROFILE_UNIFORM || profile->kind > PM2D_PROFILE_FILAMENT_Y) return fail(PM2D_EINVAL, "unknown profile");
     double nmax;
     if (profile->kind == PM2D_PROFILE_UNIFORM) nmax = profile->p[0];
     else if (profile->kind == PM2D_PROFILE_LINEAR) nmax = std::max(profile->p[0], profile->p[1]);
-    else nmax = std::min(profile->p[0] * std::exp(std::max(profile->p[1], 0.0)), profile->p[2]);
+    else if (profile->kind == PM2D_PROFILE_FILAMENT_Y) {
+        if (!(profile->p[2] > 0.0) || !(profile->p[1] >= 0.0)) return fail(PM2D_EINVAL, "filament needs sigma > 0, A >= 0");
+        nmax = profile->p[0] * (1.0 + profile->p[1]);
+    } else nmax = std::min(profile->p[0] * std::exp(std::max(profile->p[1], 0.0)), profile->p[2]);
     if (!(nmax >= 0.0) || nmax > 1e3) return fail(PM2D_EINVAL, "profile density out of range");
     // discrete stability of Eq. 6 with the plasma term (P:L120 and its bound with n_e)
     {
@@ -270,16 +275,6 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
         delete c;
         return fail(PM2D_ENOMEM, "workspace too small");
     }
-    // fixed-point scale: n_cap = power of two >= 8 n_max
-    {
-        double cap = 8.0 * (nmax > 0.0 ? nmax : 1.0);
-        int e = (int)std::ceil(std::log2(cap));
-        double ncap = std::ldexp(1.0, e);
-        c->nscale = (float)(2147483648.0 / ncap);
-        c->inv_nscale = (float)(ncap / 2147483648.0);
-        c->pscale = c->nscale * 8.0f;
-        c->inv_pscale = c->inv_nscale / 8.0f;
-    }
 #define INIT_CHECK(call)           \
     do {                           \
         int rc_ = (call);          \
@@ -298,6 +293,41 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     } while (0)
     INIT_CUDA(cudaMemsetAsync(dev_workspace, 0, need, c->stream));
     INIT_CHECK(launch_poisson_init(c));
+    {   // relative density of the cell columns (filament) and the x taper, for the number-weighted loader
+        std::vector<double> sy(grid->ny, 1.0), tx(grid->nx, 1.0);
+        const double PI = 3.14159265358979323846;
+        if (profile->kind == PM2D_PROFILE_FILAMENT_Y) {
+            double sum = 0.0;
+            for (int j = 0; j < grid->ny; j++) {
+                const double r = ((double)j + 0.5 - 0.5 * grid->ny) / profile->p[2];
+                sy[j] = 1.0 + profile->p[1] * std::exp(-0.5 * r * r);
+                sum += sy[j];
+            }
+            for (int j = 0; j < grid->ny; j++) sy[j] /= sum / grid->ny;
+        }
+        if (profile->taper_cells > 0)
+            for (int i = 0; i < grid->nx; i++) {
+                const double d = std::min((double)i + 0.5, (double)grid->nx - 0.5 - (double)i);
+                if (d < (double)profile->taper_cells) {
+                    const double sn = std::sin(0.5 * PI * d / (double)profile->taper_cells);
+                    tx[i] = sn * sn;
+                }
+            }
+        if (profile->kind == PM2D_PROFILE_FILAMENT_Y) nmax = profile->p[0] * *std::max_element(sy.begin(), sy.end());
+        INIT_CUDA(cudaMemcpyAsync(c->shape_y, sy.data(), sy.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        INIT_CUDA(cudaMemcpyAsync(c->taper_x, tx.data(), tx.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        INIT_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    // fixed-point scale: n_cap = power of two >= 8 n_max
+    {
+        double cap = 8.0 * (nmax > 0.0 ? nmax : 1.0);
+        int e = (int)std::ceil(std::log2(cap));
+        double ncap = std::ldexp(1.0, e);
+        c->nscale = (float)(2147483648.0 / ncap);
+        c->inv_nscale = (float)(ncap / 2147483648.0);
+        c->pscale = c->nscale * 16.0f;            // |n u| <= n_cap / 16 = n_max / 2
+        c->inv_pscale = c->inv_nscale / 16.0f;
+    }
     for (int s = 0; s < nsp; s++) {
         SpeciesDev &S = c->sp[s];
         if (!S.cfg.mobile) continue;

@@ -88,6 +88,7 @@ struct pm2d_ctx {
     float2 *twiddle;     // [ny/2]
     double *red;         // [64] reduction scratch
     int32_t *flags;      // [4] device error flags
+    double *shape_y, *taper_x;   // [ny], [nx] relative density tables of the number-weighted loader
     unsigned long long *stray_total; // [1] statistics
     int64_t *ovf_p;      // [ovf_cap] particles deferred by k_stage (footprint outside the tile window)
     int32_t *ovf_tile, *ovf_count;

@@ -743,6 +743,7 @@ struct LoadParams {
     double vth;
     int prof_kind, taper_cells;
     double p0, p1, p2;
+    const int32_t *cell_off;     // NUMBER_WEIGHTED: the tile's cell runs give (cell, k) of a slot
 };
 
 __device__ double profile_density(const LoadParams &L, int i)
@@ -779,8 +780,20 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
     const int ppc = L.ppc_x * L.ppc_y;
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
         int s = (int)(p - t0);
-        int lc = s / ppc, k = s - lc * ppc;
-        int li = lc / wy, lj = lc - li * wy;
+        int li, lj, k;
+        if (L.load == PM2D_NUMBER_WEIGHTED) {      // last cell whose run starts at or before slot s
+            const int32_t *co = L.cell_off + (size_t)tile * CPITCH;
+            int lo = 0, hi = TCELLS - 1;
+            while (lo < hi) {
+                int mid = (lo + hi + 1) >> 1;
+                if (co[mid] <= s) lo = mid; else hi = mid - 1;
+            }
+            li = lo >> 5; lj = lo & 31; k = s - co[lo];
+        } else {
+            int lc = s / ppc;
+            k = s - lc * ppc;
+            li = lc / wy; lj = lc - li * wy;
+        }
         int64_t cell = (int64_t)(gx0 + li) * L.ny + (gy0 + lj);
         int64_t pid = (int64_t)k * ((int64_t)L.nx * L.ny) + cell;
         uint32_t r[4];
@@ -804,7 +817,7 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
         out.ux = ux;
         out.uy = uy;
         L.pv[p] = out;
-        L.w[p] = (float)(profile_density(L, gx0 + li) / (double)ppc);
+        L.w[p] = L.load == PM2D_NUMBER_WEIGHTED ? (float)(L.p0 / (double)ppc) : (float)(profile_density(L, gx0 + li) / (double)ppc);
         if (L.id) L.id[p] = pid;
     }
 }
@@ -820,6 +833,50 @@ __global__ void k_uniform_cell_off(int32_t *cell_off, int ntiles, int nty, int n
     const int li = c >> 5, lj = c & 31;                 // c == TCELLS: li = 32
     const int before = li < wx ? li * wy + min(lj, wy) : wx * wy;
     cell_off[e] = ppc * before;
+}
+
+// NUMBER_WEIGHTED: particles per cell = floor(ppc * taper(i) * filament(j) + U), U a Philox uniform of the cell
+// (dithered rounding); one CTA per tile writes the tile's cell_off and its total
+__global__ void __launch_bounds__(256) k_weighted_cell_off(int32_t *cell_off, int32_t *tile_cnt, const double *shape_y,
+                                                           const double *taper_x, int nty, int nx, int ny, double ppc, int species,
+                                                           uint32_t seed_lo, uint32_t seed_hi)
+{
+    __shared__ int32_t wsum[8];
+    const int t = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int gx0 = (t / nty) * TILE, gy0 = (t % nty) * TILE;
+    int cnt[4], s = 0;
+#pragma unroll
+    for (int u = 0; u < 4; u++) {
+        const int c = threadIdx.x * 4 + u, gi = gx0 + (c >> 5), gj = gy0 + (c & 31);
+        cnt[u] = 0;
+        if (gi < nx && gj < ny) {
+            const int64_t cell = (int64_t)gi * ny + gj;
+            uint32_t r[4];
+            philox4x32_10((uint32_t)(cell & 0xFFFFFFFF), (uint32_t)(cell >> 32), (uint32_t)species, 1u, seed_lo, seed_hi, r);
+            const double lam = __dmul_rn(__dmul_rn(ppc, taper_x[gi]), shape_y[gj]);
+            cnt[u] = (int)floor(__dadd_rn(lam, (double)r[0] * (1.0 / 4294967296.0)));
+        }
+        s += cnt[u];
+    }
+    int incl = s;
+    for (int o = 1; o < 32; o <<= 1) {
+        int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    int run = incl - s;
+    for (int w = 0; w < wid; w++) run += wsum[w];
+    int32_t *co = cell_off + (size_t)t * CPITCH;
+#pragma unroll
+    for (int u = 0; u < 4; u++) {
+        co[threadIdx.x * 4 + u] = run;
+        run += cnt[u];
+    }
+    if (threadIdx.x == 255) {
+        co[TCELLS] = run;
+        tile_cnt[t] = run;
+    }
 }
 
 // ---- single-CTA scans over tiles ----------------------------------------------------------------
@@ -1292,11 +1349,26 @@ int launch_load_particles(pm2d_ctx *c, int s)
 {
     SpeciesDev &S = c->sp[s];
     const int ppc = S.cfg.ppc_x * S.cfg.ppc_y;
-    k_uniform_tile_counts<<<(c->ntiles + 255) / 256, 256, 0, c->stream>>>(S.tile_cnt, c->ntx, c->nty, c->g.nx, c->g.ny, ppc);
-    k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off);
-    const int64_t ncell = (int64_t)c->ntiles * CPITCH;
-    k_uniform_cell_off<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>(S.cell_off, c->ntiles, c->nty, c->g.nx, c->g.ny, ppc);
-    count_launch(c, 3);
+    if (S.cfg.load == PM2D_NUMBER_WEIGHTED) {
+        k_weighted_cell_off<<<c->ntiles, 256, 0, c->stream>>>(S.cell_off, S.tile_cnt, c->shape_y, c->taper_x, c->nty, c->g.nx, c->g.ny,
+                                                              (double)ppc, s, (uint32_t)(c->seed & 0xFFFFFFFFu), (uint32_t)(c->seed >> 32));
+        k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off);
+        count_launch(c, 2);
+        int64_t total = 0;
+        PM2D_CUDA_CHECK(cudaMemcpyAsync(&total, S.tile_off + c->ntiles, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
+        PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        if (total > S.cap) {
+            pm2d_set_error("NUMBER_WEIGHTED: capacity is smaller than the number of particles the profile asks for");
+            return PM2D_ENOMEM;
+        }
+        S.np = total;
+    } else {
+        k_uniform_tile_counts<<<(c->ntiles + 255) / 256, 256, 0, c->stream>>>(S.tile_cnt, c->ntx, c->nty, c->g.nx, c->g.ny, ppc);
+        k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off);
+        const int64_t ncell = (int64_t)c->ntiles * CPITCH;
+        k_uniform_cell_off<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>(S.cell_off, c->ntiles, c->nty, c->g.nx, c->g.ny, ppc);
+        count_launch(c, 3);
+    }
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
     LoadParams L;
@@ -1308,6 +1380,7 @@ int launch_load_particles(pm2d_ctx *c, int s)
     L.vth = sqrt(S.cfg.T_keV / 511.0 / S.cfg.mass);
     L.prof_kind = c->profile.kind; L.taper_cells = c->profile.taper_cells;
     L.p0 = c->profile.p[0]; L.p1 = c->profile.p[1]; L.p2 = c->profile.p[2];
+    L.cell_off = S.cell_off;
     k_load<<<S.max_chunks, PTHREADS, 0, c->stream>>>(L);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());

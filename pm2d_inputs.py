@@ -18,6 +18,10 @@ Loader recipe:
                      ux = vth*sqrt(-2 ln U1)*cos(2 pi U2), uy = vth*sqrt(-2 ln U1)*sin(2 pi U2)
                      evaluated in double, rounded once to float32
      w = profile(x at cell centre) * taper / (ppc_x*ppc_y), double rounded once to float32     (Q17)
+     NUMBER_WEIGHTED (config c5): equal weights w = n0/ppc; the NUMBER of particles of a cell follows the
+                     profile: count(i, j) = floor(ppc * shape(i, j) + U), shape = taper(i) * filament(j) with
+                     mean 1 over j, U = philox(counter=(cell_lo, cell_hi, species, 1))[0] * 2^-32 (a
+                     dithered rounding, so the expected count is exact); offsets and momenta as RANDOM_MAXWELL
 """
 from __future__ import annotations
 
@@ -28,8 +32,8 @@ import numpy as np
 
 # enums shared with include/pm2d.h (values only; no code shared)
 CIC, TSC, SINE = 0, 1, 2
-LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL = 0, 1, 2
-PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED = 0, 1, 2
+LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
+PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
 
 _M0, _M1 = np.uint64(0xD2511F53), np.uint64(0xCD9E8D57)
 _W0, _W1 = 0x9E3779B9, 0xBB67AE85
@@ -63,6 +67,8 @@ def profile_density(profile: dict, nx: int, i_cell):
         n = p[0] + (p[1] - p[0]) * xc
     elif kind == PROFILE_EXP_CAPPED:                                  # n0 exp(x/L) capped
         n = np.minimum(p[0] * np.exp(xc * p[1]), p[2])                # p[1] = Lx/L
+    elif kind == PROFILE_FILAMENT_Y:                                  # uniform in x; the y-dependence is in filament_shape
+        n = np.full_like(xc, p[0])
     else:
         raise ValueError(kind)
     tc = int(profile.get("taper_cells", 0))
@@ -73,10 +79,32 @@ def profile_density(profile: dict, nx: int, i_cell):
     return n
 
 
+def taper_factor(profile: dict, nx: int, i_cell):
+    """sin^2 edge taper (Q9) alone, float64."""
+    i = np.asarray(i_cell, dtype=np.float64)
+    tc = int(profile.get("taper_cells", 0))
+    if tc <= 0:
+        return np.ones_like(i)
+    d = np.minimum(i + 0.5, nx - 0.5 - i)
+    return np.where(d < tc, np.sin(0.5 * math.pi * d / tc) ** 2, 1.0)
+
+
+def filament_shape(profile: dict, ny: int):
+    """Relative density of the cells of column index j (mean 1 over j): a Gaussian filament along x centred
+    in y, 1 + A exp(-(y - Ly/2)^2 / 2 sigma^2), normalised; p = [n0, A, sigma in cells].  float64[ny]."""
+    A, sig = float(profile["p"][1]), float(profile["p"][2])
+    yc = np.arange(ny, dtype=np.float64) + 0.5
+    r = (yc - 0.5 * ny) / sig
+    g = 1.0 + A * np.exp(-0.5 * r * r)
+    return g / (g.sum() / ny)
+
+
 def profile_max(profile: dict) -> float:
     kind, p = profile["kind"], profile["p"]
     if kind == PROFILE_UNIFORM:
         return float(p[0])
+    if kind == PROFILE_FILAMENT_Y:
+        return float(p[0]) * (1.0 + float(p[1]))
     if kind == PROFILE_LINEAR:
         return float(max(p[0], p[1]))
     return float(min(p[0] * math.exp(max(p[1], 0.0)), p[2]))
@@ -91,8 +119,14 @@ def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None
     ppc = sp["ppc_x"] * sp["ppc_y"]
     ii, jj = np.meshgrid(np.arange(i_lo, i_hi, dtype=np.int64), np.arange(ny, dtype=np.int64), indexing="ij")
     cell = (ii * ny + jj).ravel()
-    k = np.repeat(np.arange(ppc, dtype=np.int64), cell.size)
-    cell = np.tile(cell, ppc)
+    if sp["load"] == NUMBER_WEIGHTED:
+        cnt = cell_counts(cfg, s)[i_lo:i_hi].ravel()
+        kmax = int(cnt.max()) if cnt.size else 0
+        k = np.concatenate([np.full(int((cnt > kk).sum()), kk, dtype=np.int64) for kk in range(kmax)]) if kmax else np.zeros(0, np.int64)
+        cell = np.concatenate([cell[cnt > kk] for kk in range(kmax)]) if kmax else np.zeros(0, np.int64)
+    else:
+        k = np.repeat(np.arange(ppc, dtype=np.int64), cell.size)
+        cell = np.tile(cell, ppc)
     pid = k * (nx * ny) + cell
     ix = (cell // ny).astype(np.int32)
     iy = (cell % ny).astype(np.int32)
@@ -104,7 +138,7 @@ def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None
         fy = (((k % sp["ppc_y"]) + 0.5) / sp["ppc_y"]).astype(np.float32)
         ux = np.zeros(pid.size, np.float32)
         uy = np.zeros(pid.size, np.float32)
-    elif sp["load"] == RANDOM_MAXWELL:
+    elif sp["load"] in (RANDOM_MAXWELL, NUMBER_WEIGHTED):
         fx = ((r0 >> np.uint32(8)).astype(np.float64) * 2.0 ** -24).astype(np.float32)
         fy = ((r1 >> np.uint32(8)).astype(np.float64) * 2.0 ** -24).astype(np.float32)
         vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
@@ -115,8 +149,27 @@ def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None
         uy = (R * np.sin(2.0 * math.pi * U2)).astype(np.float32)
     else:
         raise ValueError(sp["load"])
-    w = (profile_density(cfg["profile"], nx, ix) / ppc).astype(np.float32)
+    if sp["load"] == NUMBER_WEIGHTED:
+        w = np.full(pid.size, np.float32(cfg["profile"]["p"][0] / ppc), np.float32)
+    else:
+        w = (profile_density(cfg["profile"], nx, ix) / ppc).astype(np.float32)
     return dict(id=pid, ix=ix, iy=iy, fx=fx, fy=fy, ux=ux, uy=uy, w=w)
+
+
+def cell_counts(cfg: dict, s: int):
+    """NUMBER_WEIGHTED: particles per cell, int64[nx][ny] (see the module docstring)."""
+    g, sp = cfg["grid"], cfg["species"][s]
+    nx, ny = g["nx"], g["ny"]
+    ppc = float(sp["ppc_x"] * sp["ppc_y"])
+    shape_y = filament_shape(cfg["profile"], ny) if cfg["profile"]["kind"] == PROFILE_FILAMENT_Y else np.ones(ny)
+    tap = taper_factor(cfg["profile"], nx, np.arange(nx))
+    cell = np.arange(nx * ny, dtype=np.int64)
+    seed = int(cfg["seed"])
+    r0, _, _, _ = philox4x32_10(cell & 0xFFFFFFFF, cell >> 32, np.full_like(cell, s), np.ones_like(cell),
+                                seed & 0xFFFFFFFF, seed >> 32)
+    u = r0.astype(np.float64) * 2.0 ** -32
+    lam = (ppc * tap)[:, None] * shape_y[None, :]
+    return np.floor(lam + u.reshape(nx, ny)).astype(np.int64)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -138,7 +191,7 @@ def _base(nx, ny, dt, steps, seed, rebin_every=8):
 
 
 def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
-    """BASELINE.json configs 'c1'..'c4'.  nx/ny override the grid size to make
+    """BASELINE.json configs 'c1'..'c5'.  nx/ny override the grid size to make
     a reduced copy (same dx, dt, particles per cell, profile shape over the box, species, laser)."""
     if name == "c1":      # tiny slab: 256x128, CFL 0.5, uniform 0.1 n_c, 4 e/cell 1 keV, CIC, a0=0.01
         c = _base(256, 128, 0.5 * _DX, 100, 0)
@@ -164,6 +217,12 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
         c["species"] = [_species(-1, 1.0, 3.0, 2, 1, SINE, 1.9),
                         _species(+1, 3672.0, 1.0, 1, 1, SINE, 1.9)]
         c["lasers"] = [_laser(0.03, w0=0.3, y0=0.5)]     # w0, y0 in units of Ly, resolved below
+    elif name == "c5":    # stress: 4096x4096, ~60 e/cell (1.0e9), 5 keV, Gaussian filament in y (peak 20x mean, sigma 64 cells)
+        c = _base(4096, 4096, 0.035, 50, 4)
+        c["profile"] = dict(kind=PROFILE_FILAMENT_Y, p=[0.01, 87.7, 64.0, 0])
+        c["species"] = [_species(-1, 1.0, 5.0, 10, 6, SINE, 1.9, load=NUMBER_WEIGHTED),
+                        _species(+1, 1836.0, 0.0, 0, 0, SINE, 1.9, mobile=0, load=LOAD_NONE)]
+        c["lasers"] = [_laser(0.01)]
     else:
         raise ValueError(name)
     if nx is not None:
@@ -173,6 +232,13 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     g = c["grid"]
     c["name"] = name if (nx is None and ny is None) else f"{name}@{g['nx']}x{g['ny']}"
     c["profile"]["taper_cells"] = g["nx"] // 16          # Q9
+    if name == "c5":                                      # sigma = ny/64 cells, amplitude A such that peak = 20 x mean
+        sig = g["ny"] / 64.0
+        c["profile"]["p"][2] = sig
+        c["profile"]["p"][1] = 19.0 / (1.0 - 20.0 * sig * math.sqrt(2.0 * math.pi) / g["ny"])
+    for sp in c["species"]:
+        if sp["load"] == NUMBER_WEIGHTED:                 # slots: an upper bound of the dithered counts
+            sp["capacity"] = g["nx"] * g["ny"] * sp["ppc_x"] * sp["ppc_y"] + 4096
     if name == "c4":
         Ly = g["ny"] * g["dy"]
         c["lasers"][0]["w0"] *= Ly
@@ -184,4 +250,6 @@ def n_particles(cfg: dict, s: int) -> int:
     sp = cfg["species"][s]
     if sp["load"] == LOAD_NONE:
         return 0
+    if sp["load"] == NUMBER_WEIGHTED:
+        return int(cell_counts(cfg, s).sum())
     return cfg["grid"]["nx"] * cfg["grid"]["ny"] * sp["ppc_x"] * sp["ppc_y"]

@@ -37,7 +37,7 @@ def small_cfg(name, nx, ny, **over):
     return cfg
 
 
-CASES = [("c1", 96, 64), ("c2", 80, 32), ("c3", 72, 64)]   # CIC / TSC / SINE(+mobile ions); ragged nx
+CASES = [("c1", 96, 64), ("c2", 80, 32), ("c3", 72, 64), ("c5", 48, 64)]   # CIC / TSC / SINE(+mobile ions) / filament; ragged nx
 
 
 # ---------------------------------------------------------------------------------------------
@@ -130,7 +130,7 @@ def _compare_particles(sim, orc, cfg, s, vth):
     return ex, ey, eu, max(dX.max(), dY.max())
 
 
-@pytest.mark.parametrize("name,nx,ny,rebin", [("c1", 96, 64, 0), ("c2", 80, 32, 3), ("c3", 72, 64, 1), ("c3", 64, 16, 4)])
+@pytest.mark.parametrize("name,nx,ny,rebin", [("c1", 96, 64, 0), ("c2", 80, 32, 3), ("c3", 72, 64, 1), ("c3", 64, 16, 4), ("c5", 48, 64, 2)])
 def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin):
     cfg = small_cfg(name, nx, ny)
     sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=rebin)
