@@ -201,7 +201,7 @@ def run_cuda(args):
         achieved = alg_bytes / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
         traffic = None
         tp = os.path.join(ROOT, "profiles", "stage_traffic_bytes.txt")
-        if os.path.exists(tp):
+        if os.path.exists(tp) and args.config == "c3" and world == 1:      # measured for c3 only
             try:
                 traffic = float(open(tp).read().split()[0])
             except Exception:

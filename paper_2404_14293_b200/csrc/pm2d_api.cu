@@ -108,7 +108,11 @@ size_t layout(pm2d_ctx *c, char *base)
     c->shape_y = cv.take<double>(g.ny);
     c->taper_x = cv.take<double>(g.nx);
     c->stray_total = cv.take<unsigned long long>(1);
-    c->ovf_cap = 1 << 20;
+    {   // overflow list of the stage kernels: a quarter of the largest species, at least 2^20 entries
+        int64_t most = 0;
+        for (int s = 0; s < c->nsp; s++) most = std::max<int64_t>(most, species_np(g, c->sp[s].cfg));
+        c->ovf_cap = (int)std::min<int64_t>(std::max<int64_t>((int64_t)1 << 20, most / 4), (int64_t)1 << 30);
+    }
     c->ovf_p = cv.take<int64_t>(c->ovf_cap);
     c->ovf_tile = cv.take<int32_t>(c->ovf_cap);
     c->ovf_count = cv.take<int32_t>(4);

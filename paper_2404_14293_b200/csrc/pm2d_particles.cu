@@ -625,8 +625,11 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     ctx.ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
     ctx.j = j; ctx.wc0 = j - 1 + HALO; ctx.tile = tile; ctx.gx0 = gx0;
     ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
-    // ceil(mean particles per cell); sparse tiles (mean <= 1.5) get one more, or a third of them would stray
-    ctx.cell_cap = min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + (2 * ctx.n_tile <= 3 * TCELLS ? 1 : 0) + P.cap_extra);
+    // ceil(mean particles per cell); sparse tiles (mean <= 1.5) get one more, or a third of them would stray;
+    // dense tiles (mean >= 16: relative fluctuations are small, gradients across the tile are not) take no cap
+    ctx.cell_cap = ctx.n_tile >= 16 * TCELLS
+                       ? 0x3fffffff
+                       : min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + (2 * ctx.n_tile <= 3 * TCELLS ? 1 : 0) + P.cap_extra);
     ctx.q = -1;
     ctx.cur = PV{0u, 0u, 0.f, 0.f};
     ctx.wcur = 0.f;
@@ -1291,7 +1294,7 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
 #define PM2D_LAUNCH(ST, Q)                                                         \
     do {                                                                           \
         k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);          \
-        k_stage_overflow<SHAPE, ST, Q><<<148, 128, 0, st>>>(P);                    \
+        k_stage_overflow<SHAPE, ST, Q><<<148 * 8, 128, 0, st>>>(P);                    \
     } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }
     else if (stage == 1) { if (qmask == 3) PM2D_LAUNCH(1, 3); else PM2D_LAUNCH(1, 1); }
