@@ -27,6 +27,8 @@
 // go to an overflow list handled on the global grids.  The window is flushed once with global
 // integer reductions.  Integer accumulation makes the grids independent of the order of the
 // atomics (bit-reproducible) and n_i - n_e exact.
+#include <cstdlib>
+
 #include "pm2d_internal.h"
 
 namespace {
@@ -54,6 +56,7 @@ struct PartParams {
     float dd;                // DD
     float k_rad;             // pi / DD  (sine: G(t) = 1/2 - 1/2 cos(k_rad t))
     float w4_slope, w4_off;  // sine weights4: cosine argument = rel * w4_slope + w4_off
+    int sparse_cap;          // cell_cap of sparse tiles (mean <= 1.5 per cell)
     int cap_extra;           // cell_cap = ceil(mean particles per cell of the tile) + cap_extra
 };
 
@@ -629,7 +632,7 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     // dense tiles (mean >= 16: relative fluctuations are small, gradients across the tile are not) take no cap
     ctx.cell_cap = ctx.n_tile >= 16 * TCELLS
                        ? 0x3fffffff
-                       : min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + (2 * ctx.n_tile <= 3 * TCELLS ? 1 : 0) + P.cap_extra);
+                       : (2 * ctx.n_tile <= 3 * TCELLS ? P.sparse_cap : min(0x3fffffff, (ctx.n_tile + TCELLS - 1) / TCELLS + P.cap_extra));
     ctx.q = -1;
     ctx.cur = PV{0u, 0u, 0.f, 0.f};
     ctx.wcur = 0.f;
@@ -1281,6 +1284,7 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
     P.dd = (float)S.cfg.DD;
     P.k_rad = (float)(3.14159265358979323846 / S.cfg.DD);
     P.cap_extra = c->cap_extra;
+    P.sparse_cap = 2;
     P.w4_slope = (float)(-3.14159265358979323846 / S.cfg.DD / 16777216.0);
     P.w4_off = (float)((0.5 * S.cfg.DD - 0.5) * 3.14159265358979323846 / S.cfg.DD);
     return P;
