@@ -20,6 +20,8 @@ static int fail(int code, const std::string &msg)
     return code;
 }
 
+static void destroy_ctx(pm2d_ctx *c);
+
 namespace {
 
 __global__ void k_extract_comp(const float2 *src, int comp, float *dst, size_t n)
@@ -124,6 +126,9 @@ size_t layout(pm2d_ctx *c, char *base)
         if (!S.cfg.mobile) continue;
         S.pxfix = cv.take<int32_t>(nn);
         S.pyfix = cv.take<int32_t>(nn);
+        S.nhat = cv.take<int32_t>(nn);
+        S.pxhat = cv.take<int32_t>(nn);
+        S.pyhat = cv.take<int32_t>(nn);
         S.F = cv.take<float2>(nn);
         const size_t cap = (size_t)std::max<int64_t>(S.cap, 1);
         S.pv = cv.take<PV>(cap); S.pv2 = cv.take<PV>(cap);
@@ -188,6 +193,26 @@ int zero_moments(pm2d_ctx *c, int s, bool density, bool momentum)
         PM2D_CUDA_CHECK(cudaMemsetAsync(S.pxfix, 0, bytes, c->stream));
         PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
     }
+    return PM2D_OK;
+}
+
+// The deposit set `which` (0: n, Px, Py of stage B; 1: those of stage A) has had its last reader enqueued on
+// the main stream: zero it on the side stream, concurrently with whatever the main stream does next.
+int zero_set_async(pm2d_ctx *c, int which)
+{
+    PM2D_CUDA_CHECK(cudaEventRecord(c->ev_free[which], c->stream));
+    PM2D_CUDA_CHECK(cudaStreamWaitEvent(c->zstream, c->ev_free[which], 0));
+    const size_t bytes = (size_t)c->nn * sizeof(int32_t);
+    for (int s = 0; s < c->nsp; s++) {
+        SpeciesDev &S = c->sp[s];
+        if (!S.cfg.mobile || S.np == 0) continue;
+        PM2D_CUDA_CHECK(cudaMemsetAsync(which ? S.nhat : S.nfix, 0, bytes, c->zstream));
+        if (c->g.eager_moments) {
+            PM2D_CUDA_CHECK(cudaMemsetAsync(which ? S.pxhat : S.pxfix, 0, bytes, c->zstream));
+            PM2D_CUDA_CHECK(cudaMemsetAsync(which ? S.pyhat : S.pyfix, 0, bytes, c->zstream));
+        }
+    }
+    PM2D_CUDA_CHECK(cudaEventRecord(c->ev_zero[which], c->zstream));
     return PM2D_OK;
 }
 
@@ -266,6 +291,8 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     c->profile = *profile;
     c->seed = seed;
     c->stream = (cudaStream_t)cuda_stream;
+    c->zstream = nullptr;
+    for (int k = 0; k < 2; k++) c->ev_free[k] = c->ev_zero[k] = nullptr;
     c->step = 0;
     c->cap_extra = 0;
     if (const char *e = getenv("PM2D_CAP_EXTRA")) c->cap_extra = atoi(e);
@@ -276,14 +303,14 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     for (int p = 0; p < PM2D_PH_COUNT; p++) { c->prof_ms[p] = 0; c->prof_launch[p] = 0; }
     const size_t need = layout(c, (char *)dev_workspace);
     if (need > bytes) {
-        delete c;
+        destroy_ctx(c);
         return fail(PM2D_ENOMEM, "workspace too small");
     }
 #define INIT_CHECK(call)           \
     do {                           \
         int rc_ = (call);          \
         if (rc_) {                 \
-            delete c;              \
+            destroy_ctx(c);              \
             return rc_;            \
         }                          \
     } while (0)
@@ -291,11 +318,17 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     do {                                                                         \
         cudaError_t e_ = (call);                                                 \
         if (e_ != cudaSuccess) {                                                 \
-            delete c;                                                            \
+            destroy_ctx(c);                                                            \
             return fail(PM2D_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
         }                                                                        \
     } while (0)
     INIT_CUDA(cudaMemsetAsync(dev_workspace, 0, need, c->stream));
+    INIT_CUDA(cudaStreamCreateWithFlags(&c->zstream, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; k++) {
+        INIT_CUDA(cudaEventCreateWithFlags(&c->ev_free[k], cudaEventDisableTiming));
+        INIT_CUDA(cudaEventCreateWithFlags(&c->ev_zero[k], cudaEventDisableTiming));
+        INIT_CUDA(cudaEventRecord(c->ev_zero[k], c->stream));     // both deposit sets start zeroed
+    }
     INIT_CHECK(launch_poisson_init(c));
     {   // relative density of the cell columns (filament) and the x taper, for the number-weighted loader
         std::vector<double> sy(grid->ny, 1.0), tx(grid->nx, 1.0);
@@ -350,12 +383,22 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     return PM2D_OK;
 }
 
-extern "C" void pm2d_free(pm2d_ctx *c)
+static void destroy_ctx(pm2d_ctx *c)
 {
     if (!c) return;
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    if (c->zstream) {
+        cudaStreamSynchronize(c->zstream);
+        cudaStreamDestroy(c->zstream);
+    }
+    for (int k = 0; k < 2; k++) {
+        if (c->ev_free[k]) cudaEventDestroy(c->ev_free[k]);
+        if (c->ev_zero[k]) cudaEventDestroy(c->ev_zero[k]);
+    }
     delete c;
 }
+
+extern "C" void pm2d_free(pm2d_ctx *c) { destroy_ctx(c); }
 
 extern "C" int pm2d_set_lasers(pm2d_ctx *c, const pm2d_laser *lasers, int nlaser)
 {
@@ -379,8 +422,12 @@ static int enqueue_step(pm2d_ctx *c)
         // E^n from n^n resp. E^ from n^ (Eqs. 9-11), and in the epilogue of the inverse transform the nodal
         // force of (3) / (7): Eq. 16 with a^n, n^n / Eq. 18 with a^{n+1}, n^
         phase_begin(c, PM2D_PH_POISSON);
-        if ((rc = launch_poisson(c, false, stage == 0 ? c->a[1] : c->a[0]))) return rc;
+        if ((rc = launch_poisson(c, false, stage == 0 ? c->a[1] : c->a[0], stage == 1))) return rc;
         phase_end(c);
+        // the set just read (n^n resp. n^) is the target of the stage after next: zero it on the side stream now;
+        // the target of this stage was zeroed while the previous stage ran
+        if ((rc = zero_set_async(c, stage))) return rc;
+        PM2D_CUDA_CHECK(cudaStreamWaitEvent(c->stream, c->ev_zero[1 - stage], 0));
         // (3)-(5) gather, predictor, deposit / (7)-(8)+(1) gather, corrector, deposit -- one fused kernel
         phase_begin(c, stage == 0 ? PM2D_PH_STAGE_A : PM2D_PH_STAGE_B);
         for (int s = 0; s < c->nsp; s++)

@@ -10,8 +10,8 @@
 
 // ---- geometry of the particle tiles -----------------------------------------------------------
 constexpr int TILE = PM2D_TILE;          // cells per tile side
-constexpr int HALO = 4;                  // window nodes beyond the tile on each side
-constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (41)
+constexpr int HALO = 3;                  // window nodes beyond the tile on each side
+constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (39)
 constexpr int WPITCH = WIN;              // odd pitch: rows start on different banks
 constexpr int CHUNK = 8192;              // max particles per CTA work item (loader, tile rebin, unpack)
 constexpr int PTHREADS = 256;            // threads per CTA of the chunk kernels
@@ -58,6 +58,7 @@ struct SpeciesDev {
     // grids (device)
     int32_t *nfix;       // density, fixed point, [(nx+1)*ny] (current)
     int32_t *pxfix, *pyfix;
+    int32_t *nhat, *pxhat, *pyhat; // second set: deposits of stage A (x^, u^); zeroed on the side stream
     float2 *F;           // nodal force (Eq. 16)
 };
 
@@ -69,6 +70,8 @@ struct pm2d_ctx {
     pm2d_profile profile;
     uint64_t seed;
     cudaStream_t stream;
+    cudaStream_t zstream;            // side stream: zeroes the idle deposit set while a stage kernel runs
+    cudaEvent_t ev_free[2], ev_zero[2];   // [0] main set (n^n, stage B target), [1] hat set (stage A target)
     int64_t step;
     int64_t nn;          // nodes
     int ntx, nty, ntiles;
@@ -138,6 +141,6 @@ int launch_fix_to_float(pm2d_ctx *c, const int32_t *src, float scale, float *dst
 int launch_float_to_fix(pm2d_ctx *c, const float *src, float scale, int32_t *dst);
 // pm2d_poisson.cu
 int launch_poisson_init(pm2d_ctx *c);
-int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a = nullptr);
+int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a = nullptr, bool use_hat = false);
 // pm2d_diag.cu
 int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out);

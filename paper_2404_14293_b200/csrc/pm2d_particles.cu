@@ -1306,21 +1306,15 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
 #undef PM2D_LAUNCH
 }
 
-// stage 0 / 1: the caller has put the nodal force of the stage into S.F (launch_force), which also was
-// the last reader of the density grid the deposit now overwrites
+// stage 0 / 1: the caller has put the nodal force of the stage into S.F and zeroed the target deposit set
 static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
 {
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
     PartParams P = make_part_params(c, s);
     PM2D_CUDA_CHECK(cudaMemsetAsync(c->ovf_count, 0, sizeof(int32_t), c->stream));
-    if (stage < 2) {
-        const size_t bytes = (size_t)c->nn * sizeof(int32_t);
-        PM2D_CUDA_CHECK(cudaMemsetAsync(S.nfix, 0, bytes, c->stream));
-        if (qmask & 2) {
-            PM2D_CUDA_CHECK(cudaMemsetAsync(S.pxfix, 0, bytes, c->stream));
-            PM2D_CUDA_CHECK(cudaMemsetAsync(S.pyfix, 0, bytes, c->stream));
-        }
+    if (stage == 0) {          // stage A deposits (x^, u^) into the second set (zeroed by the caller's side stream)
+        P.nfix = S.nhat; P.pxfix = S.pxhat; P.pyfix = S.pyhat;
     }
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, c->stream);

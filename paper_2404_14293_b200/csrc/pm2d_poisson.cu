@@ -631,7 +631,7 @@ int launch_poisson_init(pm2d_ctx *c)
 
 // rho from the current density grids -> nodal E (and phi if wanted, for diagnostics); with force_a (a time
 // level of the vector potential) the nodal force of every mobile species instead of E
-int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
+int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a, bool use_hat)
 {
     const int nx = c->g.nx, ny = c->g.ny;
     const int big = ny >= 8192 ? 2 : (ny >= 512 ? 1 : 0);
@@ -642,7 +642,7 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
     S.inv_nscale = c->inv_nscale;
     for (int s = 0; s < c->nsp; s++)
         if (c->sp[s].cfg.sign != 0) {
-            S.n[S.count] = c->sp[s].nfix;
+            S.n[S.count] = (use_hat && c->sp[s].cfg.mobile) ? c->sp[s].nhat : c->sp[s].nfix;
             S.sign[S.count] = c->sp[s].cfg.sign;
             S.count++;
         }
@@ -667,7 +667,7 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a)
             SpeciesDev &Q = c->sp[s];
             if (!Q.cfg.mobile || Q.np == 0) continue;
             const int k = FO.count++;
-            FO.nfix[k] = Q.nfix; FO.F[k] = Q.F;
+            FO.nfix[k] = use_hat ? Q.nhat : Q.nfix; FO.F[k] = Q.F;
             FO.qE[k] = (float)(-(double)Q.cfg.sign * 4.0 * PI * PI / Q.cfg.mass);
             FO.pond[k] = Q.cfg.sign < 0 ? 1.f : 0.f;
             FO.cv2[k] = (float)(Q.cfg.pressure_coeff * Q.vth2);
