@@ -10,8 +10,8 @@
 
 // ---- geometry of the particle tiles -----------------------------------------------------------
 constexpr int TILE = PM2D_TILE;          // cells per tile side
-constexpr int HALO = 3;                  // window nodes beyond the tile on each side
-constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (39)
+constexpr int HALO = 2;                  // window nodes beyond the tile on each side
+constexpr int WIN = TILE + 2 * HALO + 1; // window nodes per side (37)
 constexpr int WPITCH = WIN;              // odd pitch: rows start on different banks
 constexpr int CHUNK = 8192;              // max particles per CTA work item (loader, tile rebin, unpack)
 constexpr int PTHREADS = 256;            // threads per CTA of the chunk kernels
