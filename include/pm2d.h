@@ -114,7 +114,8 @@ typedef struct {
     double W_total;
 } pm2d_diag;
 
-/* phases timed by the built-in CUDA-event profile (pm2d_profile_*) */
+/* phases timed by the built-in CUDA-event profile (pm2d_profile_*); the nodal force is evaluated in the epilogue
+ * of the Poisson solve, so PM2D_PH_FORCE stays 0 during steps */
 enum { PM2D_PH_FIELD = 0, PM2D_PH_POISSON = 1, PM2D_PH_FORCE = 2, PM2D_PH_STAGE_A = 3,
        PM2D_PH_STAGE_B = 4, PM2D_PH_REBIN = 5, PM2D_PH_COUNT = 6 };
 

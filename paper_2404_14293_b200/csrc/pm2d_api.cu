@@ -295,7 +295,6 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     for (int k = 0; k < 2; k++) c->ev_free[k] = c->ev_zero[k] = nullptr;
     c->step = 0;
     c->cap_extra = 0;
-    if (const char *e = getenv("PM2D_CAP_EXTRA")) c->cap_extra = atoi(e);
     c->prof_on = false;
     c->cur_phase = -1;
     c->launches = 0;
