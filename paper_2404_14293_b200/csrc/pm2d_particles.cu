@@ -701,6 +701,43 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     }
 }
 
+// Sparse species (about one particle per cell or fewer): a register patch would be slid once per particle, so
+// the CTA walks the tile's particles one per thread instead (coalesced records; in the cell-sorted order the
+// lanes of a warp sit in neighbouring cells of one row, so the 3 x 3 shared accesses fall in nearby banks) and
+// gathers from / deposits into the shared windows directly.  Same arithmetic as the stray pass of k_stage.
+template <int SHAPE, int STAGE, int QMASK>
+__global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
+{
+    constexpr int NT = 256;
+    constexpr int NQ = (QMASK & 2) ? 3 : 1;
+    __shared__ int32_t dep[NQ * WIN * WPITCH];
+    __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
+    const int tile = blockIdx.x;
+    const int64_t t0 = P.tile_off[tile], t1 = P.tile_off[tile + 1];
+    if (t1 == t0) return;
+    const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
+    if (STAGE < 2) load_force_window<NT>(P, gx0, gy0, Fs);
+    for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
+    __syncthreads();
+    for (int64_t p = t0 + threadIdx.x; p < t1; p += NT)
+        if (!process_direct<SHAPE, STAGE, QMASK, true>(P, p, false, gx0, gy0, Fs, dep)) push_overflow(P, p, tile, false);
+    __syncthreads();
+    for (int e = threadIdx.x; e < WIN * WIN; e += NT) {
+        const int rr = e / WIN, cidx = e - rr * WIN;
+        const int se = rr * WPITCH + cidx;
+        const int v = (QMASK & 1) ? dep[se] : 0;
+        const int vx = (QMASK & 2) ? dep[WIN * WPITCH + se] : 0, vy = (QMASK & 2) ? dep[2 * WIN * WPITCH + se] : 0;
+        if ((v | vx | vy) == 0) continue;
+        const int gi = fold_x(gx0 + rr - HALO, P.nx);
+        const int gj = (gy0 + cidx - HALO) & (P.ny - 1);
+        const int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
+        const size_t k = (size_t)gi * P.ny + gj;
+        if (v) atomicAdd(&P.nfix[k], fac * v);
+        if (vx) atomicAdd(&P.pxfix[k], fac * vx);
+        if (vy) atomicAdd(&P.pyfix[k], fac * vy);
+    }
+}
+
 // the deferred particles of k_stage: same arithmetic, global grids only
 template <int SHAPE, int STAGE, int QMASK>
 __global__ void __launch_bounds__(128) k_stage_overflow(const PartParams P)
@@ -1293,11 +1330,12 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
 constexpr int STRIP = 8;   // cells per strip thread: 128 threads per tile
 
 template <int SHAPE>
-static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, cudaStream_t st)
+static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, bool sparse, cudaStream_t st)
 {
 #define PM2D_LAUNCH(ST, Q)                                                         \
     do {                                                                           \
-        k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);          \
+        if (sparse) k_stage_direct<SHAPE, ST, Q><<<grid, 256, 0, st>>>(P);         \
+        else k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);     \
         k_stage_overflow<SHAPE, ST, Q><<<148 * 8, 128, 0, st>>>(P);                    \
     } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }
@@ -1316,9 +1354,11 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     if (stage == 0) {          // stage A deposits (x^, u^) into the second set (zeroed by the caller's side stream)
         P.nfix = S.nhat; P.pxfix = S.pxhat; P.pyfix = S.pyhat;
     }
-    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, c->stream);
-    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, c->stream);
-    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, c->stream);
+    // sparse species: at most 1.5 particles per cell on average
+    const bool sparse = 2 * S.np <= 3 * (int64_t)c->g.nx * c->g.ny;
+    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, c->stream);
+    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, c->stream);
+    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, c->stream);
     count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;
