@@ -701,7 +701,7 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     }
 }
 
-// Sparse species (about one particle per cell or fewer): a register patch would be slid once per particle, so
+// Sparse species (up to ~2 particles per cell): a register patch would be slid once per particle or two, so
 // the CTA walks the tile's particles one per thread instead (coalesced records; in the cell-sorted order the
 // lanes of a warp sit in neighbouring cells of one row, so the 3 x 3 shared accesses fall in nearby banks) and
 // gathers from / deposits into the shared windows directly.  Same arithmetic as the stray pass of k_stage.
@@ -1354,8 +1354,9 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     if (stage == 0) {          // stage A deposits (x^, u^) into the second set (zeroed by the caller's side stream)
         P.nfix = S.nhat; P.pxfix = S.pxhat; P.pyfix = S.pyhat;
     }
-    // sparse species: at most 1.5 particles per cell on average
-    const bool sparse = 2 * S.np <= 3 * (int64_t)c->g.nx * c->g.ny;
+    // sparse species: at most 2.5 particles per cell on average (measured: the direct kernel wins at 1 and 2 per
+    // cell, ties at 4, loses stage A at 8)
+    const bool sparse = 2 * S.np <= 5 * (int64_t)c->g.nx * c->g.ny;
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, c->stream);
     else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, c->stream);
