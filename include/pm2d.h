@@ -61,6 +61,11 @@ enum {
     PM2D_FIELD_ENODE = 2,  /* E averaged to nodes (Q3), comp 0 = x, 1 = y, from the current densities */
     PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16) for the current E, a^n, n^n; comp 0 = x, 1 = y */
 };
+/* Storage order of a species inside a tile (as of the last rebin).  CELL_MAJOR: (cell, rank in cell), walked by
+ * strip threads with register accumulation (dense species).  LAYERED: (min(rank, 16), cell, rank): 32 consecutive
+ * particles lie in 32 different cells, walked one particle per thread.  AUTO: LAYERED up to 16 particles per cell on
+ * average (and never for PM2D_NUMBER_WEIGHTED), else CELL_MAJOR. */
+enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 
 typedef struct pm2d_ctx pm2d_ctx; /* opaque */
@@ -73,6 +78,8 @@ typedef struct {
                               L229, L234); 0: deposit n only and build Px, Py when pm2d_get_moments
                               asks (nothing in the step reads them)                                   */
     int32_t track_ids;     /* 1: carry a particle id through the rebin (tests); costs 8 B/particle   */
+    int32_t particle_order; /* PM2D_ORDER_*: storage order inside a tile and the stage kernel that goes with it */
+    int32_t pad_;
     double dx, dy, dt;     /* lambda0, lambda0, T0; dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1 */
 } pm2d_grid;
 
@@ -165,7 +172,9 @@ int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
 /* Run the rebin now.  keys_out[count] (optional, host) receives, in the OLD storage order, the
  * destination key of every particle, key = tile * PM2D_TILE^2 + (ix % PM2D_TILE) * PM2D_TILE + iy % PM2D_TILE
  * with tile = (ix / PM2D_TILE) * ceil(ny / PM2D_TILE) + iy / PM2D_TILE; perm_out[count] (optional, host)
- * receives for every NEW slot the OLD slot it came from.  The result equals a stable counting sort by key. */
+ * receives for every NEW slot the OLD slot it came from.  CELL_MAJOR species: the result equals a stable counting
+ * sort by key.  LAYERED species: with r = the rank of a particle among those of equal key in the old order, the
+ * result is sorted by (tile, min(r, 16), cell, r). */
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);

@@ -20,12 +20,13 @@ LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
 PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
 FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
+ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, LAYERS = 0, 1, 2, 16
 PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 
 
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("rebin_every", C.c_int32),
-                ("eager_moments", C.c_int32), ("track_ids", C.c_int32),
+                ("eager_moments", C.c_int32), ("track_ids", C.c_int32), ("particle_order", C.c_int32), ("pad_", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -117,11 +118,11 @@ def _ptr(a, ctype):
     return None if a is None else a.ctypes.data_as(C.POINTER(ctype))
 
 
-def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None):
+def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, particle_order=0):
     """Translate a pm2d_inputs-style config dict into the C structs."""
     g = cfg["grid"]
     grid = Grid(g["nx"], g["ny"], g.get("ncomp", 1), g.get("rebin_every", 8) if rebin_every is None else rebin_every,
-                int(eager_moments), int(track_ids), g["dx"], g["dy"], g["dt"])
+                int(eager_moments), int(track_ids), int(particle_order), 0, g["dx"], g["dy"], g["dt"])
     sp = (Species * len(cfg["species"]))()
     for k, s in enumerate(cfg["species"]):
         sp[k] = Species(s["mass"], s["T_keV"], s["pressure_coeff"], s["DD"], s["sign"], s["shape"], s["mobile"], s["load"],
@@ -137,7 +138,7 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None):
 class PM2D:
     """One simulation context.  Method names mirror the C ABI (pm2d_step -> .step, ...)."""
 
-    def __init__(self, cfg: dict, device="cuda:0", eager_moments=1, track_ids=0, rebin_every=None, stream=None):
+    def __init__(self, cfg: dict, device="cuda:0", eager_moments=1, track_ids=0, rebin_every=None, stream=None, particle_order=0):
         import torch
 
         self.lib = load_library()
@@ -145,7 +146,7 @@ class PM2D:
             raise RuntimeError("pm2d needs a CUDA device (sm_100a); there is no CPU fallback")
         self.cfg = cfg
         self.device = torch.device(device)
-        self.grid, self.species, self.profile, self.lasers = make_structs(cfg, eager_moments, track_ids, rebin_every)
+        self.grid, self.species, self.profile, self.lasers = make_structs(cfg, eager_moments, track_ids, rebin_every, particle_order)
         self.nsp, self.nlaser = len(cfg["species"]), len(cfg["lasers"])
         self.nx, self.ny = self.grid.nx, self.grid.ny
         nbytes = self.lib.pm2d_query_workspace(C.byref(self.grid), self.species, self.nsp)

@@ -60,6 +60,7 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (!is_pow2(g->ny) || g->ny < 8 || g->ny > 8192) return fail(PM2D_EINVAL, "ny must be a power of two in [8, 8192]");
     if (g->ncomp < 1 || g->ncomp > 3) return fail(PM2D_EINVAL, "ncomp must be 1..3");
     if (g->rebin_every < 0 || g->rebin_every > 32) return fail(PM2D_EINVAL, "rebin_every must be 0..32");
+    if (g->particle_order < PM2D_ORDER_AUTO || g->particle_order > PM2D_ORDER_LAYERED) return fail(PM2D_EINVAL, "unknown particle_order");
     if (!(g->dx > 0) || !(g->dy > 0) || !(g->dt > 0)) return fail(PM2D_EINVAL, "dx, dy, dt must be positive");
     if (g->dt / g->dx > 0.999 || g->dt / g->dy > 0.999)
         return fail(PM2D_EINVAL, "dt/dx must be < 1: a particle may not cross more than one cell per step");
@@ -123,7 +124,13 @@ size_t layout(pm2d_ctx *c, char *base)
         S.nfix = cv.take<int32_t>(nn);
         S.pxfix = S.pyfix = nullptr; S.F = nullptr;
         S.np = S.cap = species_np(g, S.cfg);
+        S.layered = false;
         if (!S.cfg.mobile) continue;
+        // layered order + thread-per-particle kernel up to 16 particles per cell on average; the number-weighted
+        // loader fills cell runs, so it stays cell-major
+        if (S.cfg.load != PM2D_NUMBER_WEIGHTED)
+            S.layered = g.particle_order == PM2D_ORDER_LAYERED ||
+                        (g.particle_order == PM2D_ORDER_AUTO && S.cap <= (int64_t)PM2D_LAYERS * g.nx * g.ny);
         S.pxfix = cv.take<int32_t>(nn);
         S.pyfix = cv.take<int32_t>(nn);
         S.nhat = cv.take<int32_t>(nn);
@@ -658,8 +665,28 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
     std::vector<PV> hpv((size_t)count);
     std::vector<float> hw((size_t)count);
     std::vector<int64_t> hid(S.id ? (size_t)count : 0);
+    std::vector<int64_t> slot_of((size_t)count);          // cell-major slot of every particle (stable)
+    for (int64_t p = 0; p < count; p++) slot_of[p] = cur[key[p]]++;
+    if (S.layered) {
+        // (min(rank, LAYERS), cell, rank) inside every tile: remap the cell-major slots
+        std::vector<int64_t> remap((size_t)count);
+        for (int t = 0; t < ntiles; t++) {
+            const int32_t *co = coff.data() + (size_t)t * CPITCH;
+            if (co[TCELLS] == 0) continue;
+            int64_t run = off[t];
+            for (int r = 0; r <= PM2D_LAYERS; r++)
+                for (int cl = 0; cl < TCELLS; cl++) {
+                    const int cnt = co[cl + 1] - co[cl];
+                    if (r < PM2D_LAYERS) {
+                        if (cnt > r) remap[(size_t)(off[t] + co[cl] + r)] = run++;
+                    } else
+                        for (int q = PM2D_LAYERS; q < cnt; q++) remap[(size_t)(off[t] + co[cl] + q)] = run++;
+                }
+        }
+        for (int64_t p = 0; p < count; p++) slot_of[p] = remap[(size_t)slot_of[p]];
+    }
     for (int64_t p = 0; p < count; p++) {
-        int64_t q = cur[key[p]]++;
+        const int64_t q = slot_of[p];
         int li = ix[p] % TILE, lj = iy[p] % TILE;
         hpv[q].x = ((uint32_t)(li + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fx[p] * 16777216.0);
         hpv[q].y = ((uint32_t)(lj + POS_BIAS) << POS_FRAC_BITS) | (uint32_t)std::floor((double)fy[p] * 16777216.0);

@@ -17,6 +17,7 @@ constexpr int CHUNK = 8192;              // max particles per CTA work item (loa
 constexpr int PTHREADS = 256;            // threads per CTA of the chunk kernels
 constexpr int TCELLS = TILE * TILE;      // cells per tile
 constexpr int CPITCH = TCELLS + 1;       // ints per tile in cell_off (last = particles in the tile)
+constexpr int PM2D_LAYERS = 16;          // layered order: ranks >= PM2D_LAYERS form a cell-major tail
 constexpr int TRI_M = 32;                // rows per x-partition of the tridiagonal solve
 // fixed-point tile-relative position: (cell_rel + POS_BIAS) << 24 | frac24
 constexpr int POS_BIAS = 64;
@@ -35,6 +36,8 @@ struct SpeciesDev {
     double vth2;
     int64_t np;          // particles held (constant: walls reflect, y wraps)
     int64_t cap;
+    bool layered;        // storage order inside a tile: (rank in cell, cell) + thread-per-particle stage kernel;
+                         // else (cell, rank) + strip kernel
     // particles (device), stored tile by tile and, inside a tile, cell by cell (as of the last rebin)
     PV *pv;              // position + velocity
     float *w;            // density weight

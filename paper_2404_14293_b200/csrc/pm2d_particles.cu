@@ -787,6 +787,7 @@ struct LoadParams {
     int prof_kind, taper_cells;
     double p0, p1, p2;
     const int32_t *cell_off;     // NUMBER_WEIGHTED: the tile's cell runs give (cell, k) of a slot
+    int layered;                 // storage order inside a tile: (rank in cell, cell) instead of (cell, rank)
 };
 
 __device__ double profile_density(const LoadParams &L, int i)
@@ -832,6 +833,11 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
                 if (co[mid] <= s) lo = mid; else hi = mid - 1;
             }
             li = lo >> 5; lj = lo & 31; k = s - co[lo];
+        } else if (L.layered) {                    // layer-major: the k-th particles of all cells are contiguous
+            const int cells = min(TILE, L.nx - gx0) * wy;
+            k = s / cells;
+            int lc = s - k * cells;
+            li = lc / wy; lj = lc - li * wy;
         } else {
             int lc = s / ppc;
             k = s - lc * ppc;
@@ -1196,9 +1202,23 @@ __device__ __forceinline__ int cell_of(uint32_t xf, uint32_t yf)
     return cx * TILE + cy;
 }
 
+// LAYERED: inside the tile the particles are ordered by (rank in their cell, cell) instead of (cell, rank): 32
+// consecutive particles then lie in 32 different, consecutive cells, which is what the thread-per-particle stage
+// kernel wants (its shared atomics spread over the banks instead of piling up on the nodes of one cell).  Ranks
+// >= LAYERS form a cell-major tail.  Shared memory: hist | cb[LAYERS][TCELLS] (uint16) | cellbeg | tb | small.
+constexpr int LAYERS = PM2D_LAYERS;
+constexpr size_t CELLSORT_LAYERED_SMEM = (size_t)CS_WARPS * TCELLS * 4 + (size_t)LAYERS * TCELLS * 2 + (size_t)(TCELLS + 1) * 4 +
+                                         (size_t)TCELLS * 4 + 64 * 4;
+
+template <bool LAYERED>
 __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams C)
 {
-    __shared__ int32_t hist[CS_WARPS * TCELLS];
+    extern __shared__ int32_t cs_smem[];
+    int32_t *hist = cs_smem;                                                  // [CS_WARPS][TCELLS]
+    uint16_t *cb = reinterpret_cast<uint16_t *>(hist + CS_WARPS * TCELLS);    // [LAYERS][TCELLS] (LAYERED)
+    int32_t *cellbeg = LAYERED ? reinterpret_cast<int32_t *>(cb + LAYERS * TCELLS) : hist + CS_WARPS * TCELLS;   // [TCELLS+1]
+    int32_t *tb = cellbeg + TCELLS + 1;                                       // [TCELLS] (LAYERED)
+    int32_t *lay = LAYERED ? tb + TCELLS : cellbeg + TCELLS + 1;              // [LAYERS+2] layer offsets, tail offset
     __shared__ int32_t wsum[CS_WARPS];
     const int tile = blockIdx.x;
     const int64_t t0 = C.tile_off[tile];
@@ -1232,15 +1252,89 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
         for (int w = 0; w < wid; w++) run += wsum[w];
         for (int c = c0; c < c0 + TCELLS / (CS_WARPS * 32); c++) {
             co[c] = run;
+            cellbeg[c] = run;
             for (int w = 0; w < CS_WARPS; w++) {
                 int v = hist[w * TCELLS + c];
                 hist[w * TCELLS + c] = run;
                 run += v;
             }
         }
-        if (threadIdx.x == CS_WARPS * 32 - 1) co[TCELLS] = run;
+        if (threadIdx.x == CS_WARPS * 32 - 1) {
+            co[TCELLS] = run;
+            cellbeg[TCELLS] = run;
+        }
     }
     __syncthreads();
+    if (LAYERED) {
+        // cb[r][c] = cells before c that hold more than r particles; lay[r] = first slot of layer r;
+        // tb[c] = particles of rank >= LAYERS in the cells before c; lay[LAYERS] = first slot of that tail.
+        // All LAYERS + 1 prefix sums run in one block scan: four 64-bit words carry 16-bit counters of four layers each.
+        static_assert(LAYERS == 16 && TCELLS <= 65535, "packing of the layer counters");
+        constexpr int PER = TCELLS / (CS_WARPS * 32);
+        __shared__ unsigned long long wsum64[CS_WARPS][4];
+        __shared__ int32_t wsumt[CS_WARPS];
+        const int c0 = threadIdx.x * PER;
+        int cnt[PER];
+        unsigned long long loc[4] = {0ull, 0ull, 0ull, 0ull};
+        int loct = 0;
+#pragma unroll
+        for (int u = 0; u < PER; u++) {
+            cnt[u] = cellbeg[c0 + u + 1] - cellbeg[c0 + u];
+#pragma unroll
+            for (int r = 0; r < LAYERS; r++) loc[r >> 2] += (unsigned long long)(cnt[u] > r ? 1 : 0) << (16 * (r & 3));
+            loct += max(cnt[u] - LAYERS, 0);
+        }
+        unsigned long long inc[4] = {loc[0], loc[1], loc[2], loc[3]};
+        int inct = loct;
+        for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+            for (int m = 0; m < 4; m++) {
+                unsigned long long t = __shfl_up_sync(0xffffffffu, inc[m], o);
+                if (lane >= o) inc[m] += t;
+            }
+            int t = __shfl_up_sync(0xffffffffu, inct, o);
+            if (lane >= o) inct += t;
+        }
+        if (lane == 31) {
+#pragma unroll
+            for (int m = 0; m < 4; m++) wsum64[wid][m] = inc[m];
+            wsumt[wid] = inct;
+        }
+        __syncthreads();
+        unsigned long long run[4], tot[4] = {0ull, 0ull, 0ull, 0ull};
+        int runt = inct - loct, tott = 0;
+#pragma unroll
+        for (int m = 0; m < 4; m++) run[m] = inc[m] - loc[m];
+        for (int w = 0; w < CS_WARPS; w++) {
+#pragma unroll
+            for (int m = 0; m < 4; m++) {
+                if (w < wid) run[m] += wsum64[w][m];
+                tot[m] += wsum64[w][m];
+            }
+            if (w < wid) runt += wsumt[w];
+            tott += wsumt[w];
+        }
+#pragma unroll
+        for (int u = 0; u < PER; u++) {
+#pragma unroll
+            for (int r = 0; r < LAYERS; r++) {
+                cb[r * TCELLS + c0 + u] = (uint16_t)((run[r >> 2] >> (16 * (r & 3))) & 0xFFFFu);
+                run[r >> 2] += (unsigned long long)(cnt[u] > r ? 1 : 0) << (16 * (r & 3));
+            }
+            tb[c0 + u] = runt;
+            runt += max(cnt[u] - LAYERS, 0);
+        }
+        if (threadIdx.x == 0) {
+            int slot = 0;
+            for (int r = 0; r < LAYERS; r++) {
+                lay[r] = slot;
+                slot += (int)((tot[r >> 2] >> (16 * (r & 3))) & 0xFFFFu);
+            }
+            lay[LAYERS] = slot;
+        }
+        (void)tott;
+        __syncthreads();
+    }
     for (int64_t base = beg; base < end; base += 32) {
         const int64_t i = base + lane;
         const bool live = i < end;
@@ -1261,7 +1355,11 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
         b = __shfl_sync(0xffffffffu, b, leader);
         __syncwarp();
         if (live) {
-            const int64_t q = t0 + b + rank;
+            int64_t q = t0 + b + rank;                 // cell-major slot
+            if (LAYERED) {
+                const int r = b + rank - cellbeg[c];   // stable rank of the particle in its cell
+                q = t0 + (r < LAYERS ? lay[r] + (int)cb[r * TCELLS + c] : lay[LAYERS] + tb[c] + (r - LAYERS));
+            }
             C.dst[q] = me;
             C.wdst[q] = C.wsrc[t0 + i];
             if (C.idsrc) C.iddst[q] = C.idsrc[t0 + i];
@@ -1354,9 +1452,8 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     if (stage == 0) {          // stage A deposits (x^, u^) into the second set (zeroed by the caller's side stream)
         P.nfix = S.nhat; P.pxfix = S.pxhat; P.pyfix = S.pyhat;
     }
-    // sparse species: at most 2.5 particles per cell on average (measured: the direct kernel wins at 1 and 2 per
-    // cell, ties at 4, loses stage A at 8)
-    const bool sparse = 2 * S.np <= 5 * (int64_t)c->g.nx * c->g.ny;
+    // layered species take the thread-per-particle kernel, cell-major ones the strip kernel
+    const bool sparse = S.layered;
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, c->stream);
     else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, c->stream);
@@ -1423,6 +1520,7 @@ int launch_load_particles(pm2d_ctx *c, int s)
     L.prof_kind = c->profile.kind; L.taper_cells = c->profile.taper_cells;
     L.p0 = c->profile.p[0]; L.p1 = c->profile.p[1]; L.p2 = c->profile.p[2];
     L.cell_off = S.cell_off;
+    L.layered = S.layered ? 1 : 0;
     k_load<<<S.max_chunks, PTHREADS, 0, c->stream>>>(L);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());
@@ -1452,7 +1550,9 @@ int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64
     C.dst = S.pv; C.wdst = S.w; C.iddst = S.id;
     C.tile_off = S.tile_off2; C.cell_off = S.cell_off;
     C.perm1 = R.perm1; C.keys_out = keys_dev; C.perm_out = perm_dev;
-    k_cellsort<<<c->ntiles, CS_WARPS * 32, 0, c->stream>>>(C);
+    if (S.layered) PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_cellsort<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CELLSORT_LAYERED_SMEM));
+    if (S.layered) k_cellsort<true><<<c->ntiles, CS_WARPS * 32, CELLSORT_LAYERED_SMEM, c->stream>>>(C);
+    else k_cellsort<false><<<c->ntiles, CS_WARPS * 32, (size_t)CS_WARPS * TCELLS * 4 + (TCELLS + 1) * 4 + 64 * 4, c->stream>>>(C);
     count_launch(c, 5);
     PM2D_CUDA_CHECK(cudaGetLastError());
     std::swap(S.tile_off, S.tile_off2);
