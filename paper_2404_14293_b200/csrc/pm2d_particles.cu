@@ -344,7 +344,7 @@ __device__ __forceinline__ void defer_stray(const PartParams &P, uint32_t *slist
 // The nodal force of Eq. 16 / 18 (k_force, pm2d_fields.cu) for the nodes of the tile window -> shared
 // memory.  Window rows beyond a wall hold F of the mirror node (Q9: the gather folds indices), window
 // columns wrap (y periodic).  All loads of a thread are issued before the first store.
-template <int NT>
+template <int NT, int PITCH = WPITCH>
 __device__ __forceinline__ void load_force_window(const PartParams &P, int gx0, int gy0, float2 *Fs)
 {
     constexpr int IT = (WIN * WIN + NT - 1) / NT;
@@ -361,7 +361,7 @@ __device__ __forceinline__ void load_force_window(const PartParams &P, int gx0, 
     for (int k = 0; k < IT; k++) {
         const int e = threadIdx.x + k * NT;
         const int r = e / WIN, cidx = e - r * WIN;
-        if (e < WIN * WIN) Fs[r * WPITCH + cidx] = v[k];
+        if (e < WIN * WIN) Fs[r * PITCH + cidx] = v[k];
     }
 }
 
@@ -701,32 +701,129 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     }
 }
 
-// Sparse species (up to ~2 particles per cell): a register patch would be slid once per particle or two, so
-// the CTA walks the tile's particles one per thread instead (coalesced records; in the cell-sorted order the
-// lanes of a warp sit in neighbouring cells of one row, so the 3 x 3 shared accesses fall in nearby banks) and
-// gathers from / deposits into the shared windows directly.  Same arithmetic as the stray pass of k_stage.
+// ---- thread-per-particle stage kernel for layered species ------------------------------------------------------
+// In the layered order the 32 lanes of a warp hold particles of 32 different, consecutive cells of (mostly) one
+// cell row.  To make their shared accesses conflict-free the footprint is taken as 3 nodes around the nearest node
+// in x and the 4 nodes around the CELL in y (the lane direction): the window column then depends on the cell only,
+// and with a window pitch that is a multiple of 32 words the bank is the column, whatever the row.  12 nodes: 12
+// LDS.64 for the gather, 12 x 3 ATOMS for the deposit, one wavefront each.
+constexpr int DPITCH = 64;
+
 template <int SHAPE, int STAGE, int QMASK>
+__device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
+{
+    constexpr float GY = 1.f / W4Scale<SHAPE>::value;             // undoes the scale of weights4 (y only)
+    PV me = P.pv[p];
+    const float w = P.w[p];
+    float ux = me.ux, uy = me.uy;
+    uint32_t xd = me.x, yd = me.y;
+    float Wx[3], Wy[4];
+    if (STAGE < 2) {
+        float2 uh = make_float2(0.f, 0.f);
+        uint32_t xg = me.x, yg = me.y;
+        if (STAGE == 1) {
+            uh = P.uh[p];
+            xg = advance(me.x, P.hx, __fadd_rn(uh.x, ux));
+            yg = advance(me.y, P.hy, __fadd_rn(uh.y, uy));
+        }
+        int cx;
+        float dx_;
+        decode(xg, cx, dx_);
+        const int cyc = (int)(yg >> POS_FRAC_BITS) - POS_BIAS;    // cell, not nearest node
+        if (cx - 1 < -HALO || cx + 1 > TILE + HALO || cyc - 1 < -HALO || cyc + 2 > TILE + HALO) return false;
+        weights3<SHAPE>(dx_, P, Wx);
+        weights4<SHAPE>((int)(yg & POS_FRAC_MASK), P, Wy);
+        const float2 *fw = Fs + (cx - 1 + HALO) * DPITCH + (cyc - 1 + HALO);
+        float2 f = make_float2(0.f, 0.f);
+        const float2 wy0 = dup2(Wy[0]), wy1 = dup2(Wy[1]), wy2 = dup2(Wy[2]), wy3 = dup2(Wy[3]);
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float2 sa = __fmul2_rn(wy0, fw[a * DPITCH]);
+            sa = __ffma2_rn(wy1, fw[a * DPITCH + 1], sa);
+            sa = __ffma2_rn(wy2, fw[a * DPITCH + 2], sa);
+            sa = __ffma2_rn(wy3, fw[a * DPITCH + 3], sa);
+            f = __ffma2_rn(dup2(Wx[a]), sa, f);
+        }
+        if (STAGE == 0) {
+            const float uhx = __fmaf_rn(GY * P.dt, f.x, ux), uhy = __fmaf_rn(GY * P.dt, f.y, uy);       // Eq. 17
+            P.uh[p] = make_float2(uhx, uhy);
+            xd = advance(me.x, P.hx, __fadd_rn(uhx, ux));
+            yd = advance(me.y, P.hy, __fadd_rn(uhy, uy));
+            ux = uhx;
+            uy = uhy;
+        } else {
+            float unx = __fmaf_rn(0.5f * GY * P.dt, f.x, 0.5f * __fadd_rn(uh.x, ux));                   // Eq. 19
+            const float uny = __fmaf_rn(0.5f * GY * P.dt, f.y, 0.5f * __fadd_rn(uh.y, uy));
+            xd = advance(me.x, P.hx, __fadd_rn(unx, ux));
+            yd = advance(me.y, P.hy, __fadd_rn(uny, uy));
+            reflect_x(xd, unx, gx0, P.nx);
+            me.x = xd; me.y = yd; me.ux = unx; me.uy = uny;
+            P.pv[p] = me;
+            ux = unx;
+            uy = uny;
+        }
+    }
+    int cx;
+    float dx_;
+    decode(xd, cx, dx_);
+    const int cyc = (int)(yd >> POS_FRAC_BITS) - POS_BIAS;
+    if (cx - 1 < -HALO || cx + 1 > TILE + HALO || cyc - 1 < -HALO || cyc + 2 > TILE + HALO) {
+        // off the window (far from its tile): 3 x 3 nodes on the global grids, like the overflow pass
+        deposit_direct<SHAPE, QMASK, false>(P, gx0, gy0, xd, yd, ux, uy, w, nullptr);
+        return true;
+    }
+    weights3<SHAPE>(dx_, P, Wx);
+    weights4<SHAPE>((int)(yd & POS_FRAC_MASK), P, Wy);
+    const float q = w * (GY * P.nscale);
+    const float2 qu = make_float2(ux * P.pratio, uy * P.pratio);
+    int32_t *dw = dep + (cx - 1 + HALO) * DPITCH + (cyc - 1 + HALO);
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const float qa = Wx[a] * q;
+#pragma unroll
+        for (int b = 0; b < 4; b++) {
+            const float qn = qa * Wy[b];
+            if (QMASK & 1) atomicAdd(&dw[a * DPITCH + b], __float2int_rn(qn));
+            if (QMASK & 2) {
+                const float2 qp = __fmul2_rn(dup2(qn), qu);
+                atomicAdd(&dw[WIN * DPITCH + a * DPITCH + b], __float2int_rn(qp.x));
+                atomicAdd(&dw[2 * WIN * DPITCH + a * DPITCH + b], __float2int_rn(qp.y));
+            }
+        }
+    }
+    return true;
+}
+
+// ANCH: the cell-anchored 3 x 4 footprint above (conflict-free as long as the particles sit in the cells they were
+// sorted into: species that hardly move between rebins, e.g. ions); else the 3 x 3 nodes around the nearest node
+// on the odd-pitch windows (process_direct), whose conflicts do not depend on the drift.
+template <int SHAPE, int STAGE, int QMASK, bool ANCH>
 __global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
 {
     constexpr int NT = 256;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
-    __shared__ int32_t dep[NQ * WIN * WPITCH];
-    __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
+    constexpr int PITCH = ANCH ? DPITCH : WPITCH;
+    extern __shared__ int32_t direct_smem[];
+    int32_t *dep = direct_smem;                                                      // [NQ][WIN][PITCH]
+    float2 *Fs = reinterpret_cast<float2 *>(direct_smem + ((NQ * WIN * PITCH + 1) & ~1));   // [WIN][PITCH]
     const int tile = blockIdx.x;
     const int64_t t0 = P.tile_off[tile], t1 = P.tile_off[tile + 1];
     if (t1 == t0) return;
     const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
-    if (STAGE < 2) load_force_window<NT>(P, gx0, gy0, Fs);
-    for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
+    if (STAGE < 2) load_force_window<NT, PITCH>(P, gx0, gy0, Fs);
+    for (int e = threadIdx.x; e < NQ * WIN * PITCH; e += NT) dep[e] = 0;
     __syncthreads();
-    for (int64_t p = t0 + threadIdx.x; p < t1; p += NT)
-        if (!process_direct<SHAPE, STAGE, QMASK, true>(P, p, false, gx0, gy0, Fs, dep)) push_overflow(P, p, tile, false);
+    for (int64_t p = t0 + threadIdx.x; p < t1; p += NT) {
+        const bool ok = ANCH ? direct_particle<SHAPE, STAGE, QMASK>(P, p, gx0, gy0, Fs, dep)
+                             : process_direct<SHAPE, STAGE, QMASK, true>(P, p, false, gx0, gy0, Fs, dep);
+        if (!ok) push_overflow(P, p, tile, false);
+    }
     __syncthreads();
     for (int e = threadIdx.x; e < WIN * WIN; e += NT) {
         const int rr = e / WIN, cidx = e - rr * WIN;
-        const int se = rr * WPITCH + cidx;
+        const int se = rr * PITCH + cidx;
         const int v = (QMASK & 1) ? dep[se] : 0;
-        const int vx = (QMASK & 2) ? dep[WIN * WPITCH + se] : 0, vy = (QMASK & 2) ? dep[2 * WIN * WPITCH + se] : 0;
+        const int vx = (QMASK & 2) ? dep[WIN * PITCH + se] : 0, vy = (QMASK & 2) ? dep[2 * WIN * PITCH + se] : 0;
         if ((v | vx | vy) == 0) continue;
         const int gi = fold_x(gx0 + rr - HALO, P.nx);
         const int gj = (gy0 + cidx - HALO) & (P.ny - 1);
@@ -736,6 +833,13 @@ __global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
         if (vx) atomicAdd(&P.pxfix[k], fac * vx);
         if (vy) atomicAdd(&P.pyfix[k], fac * vy);
     }
+}
+
+template <int STAGE, int QMASK, bool ANCH>
+constexpr size_t direct_smem_bytes()
+{
+    return (size_t)(((((QMASK & 2) ? 3 : 1) * WIN * (ANCH ? DPITCH : WPITCH)) + 1) & ~1) * 4 +
+           (STAGE < 2 ? (size_t)WIN * (ANCH ? DPITCH : WPITCH) * 8 : 0);
 }
 
 // the deferred particles of k_stage: same arithmetic, global grids only
@@ -1428,11 +1532,15 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
 constexpr int STRIP = 8;   // cells per strip thread: 128 threads per tile
 
 template <int SHAPE>
-static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, bool sparse, cudaStream_t st)
+static void launch_stage_shape(const PartParams &P, int stage, int qmask, int grid, bool sparse, bool anch, cudaStream_t st)
 {
 #define PM2D_LAUNCH(ST, Q)                                                         \
     do {                                                                           \
-        if (sparse) k_stage_direct<SHAPE, ST, Q><<<grid, 256, 0, st>>>(P);         \
+        if (sparse && anch) {                                                      \
+            cudaFuncSetAttribute(k_stage_direct<SHAPE, ST, Q, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)direct_smem_bytes<ST, Q, true>()); \
+            k_stage_direct<SHAPE, ST, Q, true><<<grid, 256, direct_smem_bytes<ST, Q, true>(), st>>>(P); \
+        } else if (sparse)                                                         \
+            k_stage_direct<SHAPE, ST, Q, false><<<grid, 256, direct_smem_bytes<ST, Q, false>(), st>>>(P); \
         else k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);     \
         k_stage_overflow<SHAPE, ST, Q><<<148 * 8, 128, 0, st>>>(P);                    \
     } while (0)
@@ -1454,9 +1562,12 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     }
     // layered species take the thread-per-particle kernel, cell-major ones the strip kernel
     const bool sparse = S.layered;
-    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, c->stream);
-    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, c->stream);
-    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, c->stream);
+    // thermal drift between two rebins, in cells: below a tenth of a cell the particles are (almost all) still in the
+    // cells they were sorted into
+    const bool anch = sqrt(S.vth2) * c->g.dt / fmin(c->g.dx, c->g.dy) * (double)(c->g.rebin_every > 0 ? c->g.rebin_every : 32) < 0.1;
+    if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);
+    else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);
+    else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);
     count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;
