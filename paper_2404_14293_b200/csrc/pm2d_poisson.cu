@@ -266,8 +266,9 @@ struct ForceOut {
 // BIG: 0 = radix-4 Stockham (ny < 512), 1 = register-blocked FFT with ny/16 <= 256 threads, 2 = with 512 threads (ny = 8192).
 // MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part);
 // MODE 2: Z = ehx + i ehy -> F_s of every mobile species (ForceOut)
-template <int MODE, int BIG>
-__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
+// NS: species slots of the force epilogue (2 covers electrons + one ion species with fewer registers)
+template <int MODE, int BIG, int NS = PM2D_MAX_SPECIES>
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <= 2 ? 3 : 2) : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
                                                       float *__restrict__ phi, int ny, int LP, const ForceOut FO)
 {
@@ -306,10 +307,9 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1
                 jp[u] = (jj[u] + 1) & (ny - 1);
                 px[u] = py[u] = 0.f;
             }
-            int n0[PM2D_MAX_SPECIES][NB], nh[PM2D_MAX_SPECIES][NB], nl[PM2D_MAX_SPECIES][NB], nu[PM2D_MAX_SPECIES][NB],
-                nd[PM2D_MAX_SPECIES][NB];
+            int n0[NS][NB], nh[NS][NB], nl[NS][NB], nu[NS][NB], nd[NS][NB];
 #pragma unroll
-            for (int s = 0; s < PM2D_MAX_SPECIES; s++)
+            for (int s = 0; s < NS; s++)
                 if (s < FO.count) {
                     const int32_t *n = FO.nfix[s];
 #pragma unroll
@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1
                 }
             }
 #pragma unroll
-            for (int s = 0; s < PM2D_MAX_SPECIES; s++)
+            for (int s = 0; s < NS; s++)
                 if (s < FO.count) {
 #pragma unroll
                     for (int u = 0; u < NB; u++) {
@@ -621,6 +621,7 @@ int launch_poisson_init(pm2d_ctx *c)
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
@@ -675,6 +676,7 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a, bool use_ha
         FO.a = force_a; FO.ncomp = c->g.ncomp; FO.nx = nx;
         FO.inv_2dx = (float)(1.0 / (2.0 * c->g.dx)); FO.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
         if (big == 2) k_ifft<2, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (big == 1 && FO.count <= 2) k_ifft<2, 1, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
         else if (big == 1) k_ifft<2, 1><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
         else k_ifft<2, 0><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
     } else if (big == 2)
