@@ -196,7 +196,7 @@ __device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n)
 // Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
 // rho^_b = (Z_l - conj Z_{n-l}) / 2i.  BIG: register-blocked FFT on the padded buffer (ny >= 512).
 template <int BIG>
-__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
                                                                      float2 *__restrict__ rho_hat, int nx, int ny, int LP)
 {
     extern __shared__ float2 buf[];
@@ -204,27 +204,32 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 2 : 1
     const bool has_b = ib <= nx - 1;
     const size_t rowa = (size_t)ia * ny, rowb = (size_t)ib * ny;
     if (BIG) {
-        // blockDim.x == ny / 16: every thread owns 16 columns; all loads are issued before the first use
-        int va[16], vb[16];
+        // blockDim.x == ny / 16: every thread owns 16 columns, taken in two halves of 8 (registers); the loads of a
+        // half are issued before their first use
 #pragma unroll
-        for (int k = 0; k < 16; k++) va[k] = vb[k] = 0;
-        for (int s = 0; s < S.count; s++) {
-            const int32_t *na = S.n[s] + rowa, *nb = S.n[s] + (has_b ? rowb : rowa);
-            int ta[16], tb[16];
+        for (int half = 0; half < 2; half++) {
+            int va[8], vb[8];
 #pragma unroll
-            for (int k = 0; k < 16; k++) {
-                ta[k] = na[threadIdx.x + k * blockDim.x];
-                tb[k] = nb[threadIdx.x + k * blockDim.x];
+            for (int k = 0; k < 8; k++) va[k] = vb[k] = 0;
+            for (int s = 0; s < S.count; s++) {
+                const int32_t *na = S.n[s] + rowa, *nb = S.n[s] + (has_b ? rowb : rowa);
+                int ta[8], tb[8];
+#pragma unroll
+                for (int k = 0; k < 8; k++) {
+                    ta[k] = na[threadIdx.x + (half * 8 + k) * blockDim.x];
+                    tb[k] = nb[threadIdx.x + (half * 8 + k) * blockDim.x];
+                }
+#pragma unroll
+                for (int k = 0; k < 8; k++) {
+                    va[k] += S.sign[s] * ta[k];
+                    vb[k] += S.sign[s] * tb[k];
+                }
             }
 #pragma unroll
-            for (int k = 0; k < 16; k++) {
-                va[k] += S.sign[s] * ta[k];
-                vb[k] += S.sign[s] * tb[k];
-            }
+            for (int k = 0; k < 8; k++)
+                buf[pad16(threadIdx.x + (half * 8 + k) * blockDim.x)] =
+                    make_float2((float)va[k] * S.inv_nscale, has_b ? (float)vb[k] * S.inv_nscale : 0.f);
         }
-#pragma unroll
-        for (int k = 0; k < 16; k++)
-            buf[pad16(threadIdx.x + k * blockDim.x)] = make_float2((float)va[k] * S.inv_nscale, has_b ? (float)vb[k] * S.inv_nscale : 0.f);
     } else {
         for (int j = threadIdx.x; j < ny; j += blockDim.x) {
             int va = 0, vb = 0;
