@@ -2,31 +2,31 @@
 //   * fused gather + push + deposit, stage A (Eq. 17) and stage B (Eq. 19)      [P:L191-221]
 //   * deposit-only pass (initial item (1) of the flow, lazy momentum grids)       [Eq. 14, P:L187]
 //   * counter-based particle loader (Philox-4x32-10)         [P:L154-162]
-//   * stable rebin by (tile, cell): tile pass specialised to neighbour moves, then a counting
-//     sort by cell inside every tile                                              [DESIGN.md 6.4]
+//   * deterministic stable rebin: tile pass specialised to neighbour moves, then a sort inside
+//     every tile by (layer, cell) or by cell                                      [DESIGN.md 6.4]
 //
-// Data layout.  A particle is a 16-byte record PV {x, y, ux, uy} plus a weight w and, between the
-// two stages of a step, the predictor velocity u^ (float2).  Particles are stored tile by tile
-// (PM2D_TILE x PM2D_TILE cells) and inside a tile cell by cell (row-major cells, as of the last
-// rebin); cell_off gives every cell's run.  A position is a pair of 32-bit fixed-point numbers
+// Data layout.  A particle is a 16-byte record PV {x, y, ux, uy} plus a weight w
+// and, between the two stages of a step, the predictor velocity u^ (float2).  Particles are stored
+// tile by tile (PM2D_TILE x PM2D_TILE cells); inside a tile, as of the last rebin, either LAYERED
+// (by rank in the cell, then by cell: 32 consecutive particles lie in 32 different cells) or
+// CELL-MAJOR (cell_off gives every cell's run).  A position is a pair of 32-bit fixed-point numbers
 // relative to the tile's origin,
 //     xfix = (cell_rel + POS_BIAS) << 24 | frac24,
 // so the in-cell offset carries 24 bits whatever the size of the box, the push is an exact integer
 // add of a rounded displacement, and the canonical (ix, fx) of include/pm2d.h is read off exactly.
 //
-// Fused stage kernel.  A CTA owns one tile: it builds the force of the tile + halo in shared memory
-// (Eq. 16/18), and every thread owns a strip of S consecutive cells of one cell row.  While the
-// thread walks the particles of a cell it keeps, in registers, the force on the 4 x 4 nodes around
-// that cell and the deposit those particles make on the same 16 nodes: a particle that is still
-// within half a cell of its rebin-time cell gathers and deposits entirely in registers (weights of
-// the four nodes per axis from three evaluations of the cumulative shape G, Eq. 13).  Moving to the
-// next cell slides the patch one column: the oldest column is rounded to fixed point and added to
-// the tile's shared int32 window with 4 x 3 conflict-free ATOMS (lanes = rows, odd pitch), the new
-// force column is read with 4 LDS.64.  Particles that drifted further take the same arithmetic on
-// the shared windows directly (3 x 3 nodes around the nearest node), and those outside the window
-// go to an overflow list handled on the global grids.  The window is flushed once with global
-// integer reductions.  Integer accumulation makes the grids independent of the order of the
-// atomics (bit-reproducible) and n_i - n_e exact.
+// Fused stage kernels.  A CTA owns one tile: it copies the nodal force of the tile +
+// halo into shared memory, its particles gather from that window, are pushed, and deposit into a
+// shared int32 fixed-point window that is flushed once with global integer reductions.  Integer
+// accumulation makes the grids independent of the order of the atomics (bit-reproducible) and
+// n_i - n_e exact.
+//   k_stage_direct (layered species): one particle per thread, shared atomics per particle;
+//   k_stage        (cell-major species): every thread owns a strip of S cells of one cell column and
+//                  keeps, in registers, the force on and the deposit to the 4 x 4 nodes around its
+//                  current cell; sliding to the next cell row adds the finished node row to the
+//                  window with 4 x 3 conflict-free ATOMS.  Particles outside the patch ("strays")
+//                  are listed and served with the per-particle code after the strips;
+//   k_stage_overflow: particles whose footprint left the tile's window, on the global grids.
 #include <cstdlib>
 
 #include "pm2d_internal.h"
