@@ -356,3 +356,47 @@ def test_srs_growth_rate_parity(P):
     rg, ro = backscatter_growth_rate(t, sg - inc), backscatter_growth_rate(t, so - inc)
     assert rg == pytest.approx(ro, rel=0.07), (rg, ro)
     sim.close()
+
+
+def test_full_size_c2_deposit_parity_and_conservation(P):
+    """BASELINE.json config 2 at full size (2048 x 1024, 16.8 M electrons, TSC), in the launch configuration bench.py
+    times: after 3 steps the deposited n, Px, Py of the device's own particles equal the oracle's deposit of the same
+    particles (rel. L2 <= 1e-5 over all 2.1 M nodes), the particle count and the total charge are conserved."""
+    cfg = I.config("c2")
+    g = cfg["grid"]
+    sim = P.PM2D(cfg, eager_moments=1)
+    n0 = sim.particle_count(0)
+    q0 = sim.diagnostics()["charge"][0]
+    sim.step(3)
+    parts = sim.get_particles(0)
+    assert parts["ix"].size == n0 == I.n_particles(cfg, 0)
+    grid = oracle.make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"])
+    sp = cfg["species"][0]
+    n, px, py = oracle.deposit(grid, sp["shape"], sp["DD"], parts["ix"] + parts["fx"].astype(np.float64),
+                               parts["iy"] + parts["fy"].astype(np.float64), parts["ux"], parts["uy"], parts["w"])
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), n) < 1e-5
+    assert rel_l2(sim.get_moments(0, P.MOMENT_PX), px) < 1e-5
+    assert rel_l2(sim.get_moments(0, P.MOMENT_PY), py) < 1e-5
+    d = sim.diagnostics()
+    assert d["count"][0] == n0
+    assert d["charge"][0] == pytest.approx(q0, rel=1e-6)
+    assert d["charge"][0] == pytest.approx(float(parts["w"].astype(np.float64).sum()), rel=1e-6)
+    sim.close()
+
+
+def test_full_size_c3_conservation_across_a_rebin(P):
+    """BASELINE.json config 3 at full size (8192 x 4096, 134 M electrons + 33.6 M ions): 17 steps (one rebin) keep
+    the particle counts and both species' total charge (properties that hold at any size); nothing strays to the
+    overflow path in numbers that matter; sampled field values are finite."""
+    cfg = I.config("c3")
+    sim = P.PM2D(cfg, eager_moments=1)
+    d0 = sim.diagnostics()
+    sim.step(17)
+    d1 = sim.diagnostics()
+    for s in (0, 1):
+        assert d1["count"][s] == d0["count"][s] == I.n_particles(cfg, s)
+        assert d1["charge"][s] == pytest.approx(d0["charge"][s], rel=1e-6)
+    assert np.isfinite(d1["W_total"]) and d1["W_kin"][0] > 0
+    a = sim.get_fields(P.FIELD_A, 0, 0, window=(0, 64, 0, 64))
+    assert np.isfinite(a).all() and np.abs(a).max() > 0
+    sim.close()
