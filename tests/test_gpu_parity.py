@@ -400,3 +400,29 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     a = sim.get_fields(P.FIELD_A, 0, 0, window=(0, 64, 0, 64))
     assert np.isfinite(a).all() and np.abs(a).max() > 0
     sim.close()
+
+
+def test_three_components_two_beams_gaussian_parity(P):
+    """All three components of a (Eq. 1 is the same equation for a_x, a_y, a_z; the ponderomotive force takes the
+    sum of their squares, Eq. 16), two beams on different components, one of them Gaussian (Eq. 4) and detuned
+    (P:L380): 10 steps of the reduced c4 config against the oracle."""
+    cfg = small_cfg("c4", 64, 64, ncomp=3)
+    Ly = 64 * cfg["grid"]["dy"]
+    cfg["lasers"] = [dict(a0=0.03, omega=1.0, y0=0.5 * Ly, w0=0.3 * Ly, alpha=0.0, comp=0, t_rise=0.2),
+                     dict(a0=0.02, omega=1.0 / 0.9995, y0=0.0, w0=0.0, alpha=0.0, comp=2, t_rise=0.0)]
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=4)
+    orc, _ = oracle_from_config(cfg)
+    for step in range(10):
+        sim.step(1)
+        orc.step(1)
+    for comp in range(3):
+        a = sim.get_fields(P.FIELD_A, comp, 0)
+        ref = orc.a_now[comp]
+        assert np.abs(a - ref).max() < 2e-5 * max(np.abs(orc.a_now).max(), 1e-30) + 1e-9, comp
+    assert np.abs(orc.a_now[0]).max() > 1e-3 and np.abs(orc.a_now[2]).max() > 1e-3 and np.abs(orc.a_now[1]).max() == 0.0
+    for s, sp in enumerate(cfg["species"]):
+        assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < 1e-5
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
+        assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4, (s, ex, ey, eu, dabs)
+    sim.close()
