@@ -143,9 +143,12 @@ __device__ __forceinline__ void dft_reg(float2 *v)
     DftCombine<(R > 1 ? R : 2), INV, 0>::run(v, e, o);
 }
 
+// plain_out: the pass writes its results unpadded (index i instead of pad16(i)): the last pass of a transform
+// whose consumer reads runs of consecutive points (k_ifft's force epilogue)
 template <int R, bool INV>
-__device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict__ tw, int n, int Ns)
+__device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict__ tw, int n, int Ns, bool plain_out = false)
 {
+    const int pad_mask = plain_out ? 0 : -1;
     constexpr int NB = 16 / R;
     const int T = blockDim.x, q = n / R;
     float2 v[NB][R];
@@ -160,37 +163,45 @@ __device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict
     for (int b = 0; b < NB; b++) {
         const int j = threadIdx.x + b * T, k = j & (Ns - 1);
         if (Ns > 1) {
-            const int step = n / (Ns * R), h = n >> 1;
+            // twiddles w^r, r < R, of w = exp(-/+ 2 pi i k / (Ns R)): one table load (k step < n / R), the powers by
+            // a product tree of depth log2 R (w^r = w^p w^(r-p), p the largest power of two <= r) -- R - 1 gathers
+            // with up to 32 cache lines per warp each cost far more than R - 2 complex products
+            const int step = n / (Ns * R);
+            float2 w[R];
+            w[1] = tw[k * step];
+            if (INV) w[1].y = -w[1].y;
 #pragma unroll
-            for (int r = 1; r < R; r++) {
-                const int t = r * k * step;
-                float2 w = t < h ? tw[t] : tw[t - h];
-                if (t >= h) { w.x = -w.x; w.y = -w.y; }
-                if (INV) w.y = -w.y;
-                v[b][r] = cmul(v[b][r], w);
+            for (int r = 2; r < R; r++) {
+                const int p = r >= 8 ? 8 : (r >= 4 ? 4 : 2);
+                w[r] = (r == p) ? cmul(w[r / 2], w[r / 2]) : cmul(w[p], w[r - p]);
             }
+#pragma unroll
+            for (int r = 1; r < R; r++) v[b][r] = cmul(v[b][r], w[r]);
         }
         dft_reg<R, INV>(v[b]);
         const int j0 = (j - k) * R + k;
 #pragma unroll
-        for (int r = 0; r < R; r++) buf[pad16(j0 + r * Ns)] = v[b][r];
+        for (int r = 0; r < R; r++) {
+            const int o = j0 + r * Ns;
+            buf[o + ((o >> 4) & pad_mask)] = v[b][r];
+        }
     }
     __syncthreads();
 }
 
 // in place on the padded buffer; blockDim.x == n / 16, n a power of two >= 512; callers synchronise before
 template <bool INV>
-__device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n)
+__device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n, bool plain_out = false)
 {
     int Ns = 1;
     while (n / Ns >= 16) {
-        fft16_pass<16, INV>(buf, tw, n, Ns);
+        fft16_pass<16, INV>(buf, tw, n, Ns, plain_out && n / Ns == 16);
         Ns <<= 4;
     }
     const int rem = n / Ns;
-    if (rem == 8) fft16_pass<8, INV>(buf, tw, n, Ns);
-    else if (rem == 4) fft16_pass<4, INV>(buf, tw, n, Ns);
-    else if (rem == 2) fft16_pass<2, INV>(buf, tw, n, Ns);
+    if (rem == 8) fft16_pass<8, INV>(buf, tw, n, Ns, plain_out);
+    else if (rem == 4) fft16_pass<4, INV>(buf, tw, n, Ns, plain_out);
+    else if (rem == 2) fft16_pass<2, INV>(buf, tw, n, Ns, plain_out);
 }
 
 // Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
@@ -290,9 +301,83 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <
     float2 *r = buf;
     if (BIG) {
         __syncthreads();
-        fft16_inplace<true>(buf, tw, ny);
+        fft16_inplace<true>(buf, tw, ny, MODE == 2);
     } else
         r = fft_stockham<true>(buf, buf + ny, tw, ny);
+    if (MODE == 2 && BIG) {
+        // four consecutive nodes per thread: 128-bit loads of the density and vector-potential rows, E from the
+        // unpadded buffer as two LDS.128 (lanes 4..7 of every quarter-warp take the two halves in the other order:
+        // no bank conflicts), two 128-bit stores of F per species
+        const size_t nn = (size_t)(FO.nx + 1) * ny;
+        const int il = i > 0 ? i - 1 : 0, ih = i < FO.nx ? i + 1 : FO.nx;
+        const float sx = (il == i || ih == i) ? 2.f * FO.inv_2dx : FO.inv_2dx;     // one-sided at the walls
+        const size_t row = (size_t)i * ny, rl = (size_t)il * ny, rh = (size_t)ih * ny;
+        bool any_pond = false;
+        for (int s = 0; s < FO.count; s++) any_pond |= FO.pond[s] != 0.f;
+        const int swz = (threadIdx.x >> 2) & 1;
+#pragma unroll 1
+        for (int g = threadIdx.x; g < ny / 4; g += blockDim.x) {
+            const int j0 = 4 * g, jm = (j0 - 1) & (ny - 1), jp = (j0 + 4) & (ny - 1);
+            int4 n0[NS], nh[NS], nl[NS];
+            int nd[NS], nu[NS];
+#pragma unroll
+            for (int s = 0; s < NS; s++)
+                if (s < FO.count) {
+                    const int32_t *n = FO.nfix[s];
+                    n0[s] = *reinterpret_cast<const int4 *>(n + row + j0);
+                    nh[s] = *reinterpret_cast<const int4 *>(n + rh + j0);
+                    nl[s] = *reinterpret_cast<const int4 *>(n + rl + j0);
+                    nd[s] = n[row + jm];
+                    nu[s] = n[row + jp];
+                }
+            float px[4] = {0.f, 0.f, 0.f, 0.f}, py[4] = {0.f, 0.f, 0.f, 0.f};
+            if (any_pond) {
+                for (int c = 0; c < FO.ncomp; c++) {
+                    const float *ac = FO.a + c * nn;
+                    const float4 vh = *reinterpret_cast<const float4 *>(ac + rh + j0);
+                    const float4 vl = *reinterpret_cast<const float4 *>(ac + rl + j0);
+                    const float4 v0 = *reinterpret_cast<const float4 *>(ac + row + j0);
+                    const float vd = ac[row + jm], vu = ac[row + jp];
+                    const float hx = 0.5f * sx, hy = 0.5f * FO.inv_2dy;
+                    px[0] += hx * (vh.x * vh.x - vl.x * vl.x);
+                    px[1] += hx * (vh.y * vh.y - vl.y * vl.y);
+                    px[2] += hx * (vh.z * vh.z - vl.z * vl.z);
+                    px[3] += hx * (vh.w * vh.w - vl.w * vl.w);
+                    py[0] += hy * (v0.y * v0.y - vd * vd);
+                    py[1] += hy * (v0.z * v0.z - v0.x * v0.x);
+                    py[2] += hy * (v0.w * v0.w - v0.y * v0.y);
+                    py[3] += hy * (vu * vu - v0.z * v0.z);
+                }
+            }
+            const float4 *rb = reinterpret_cast<const float4 *>(r) + 2 * g;
+            const float4 ea = rb[swz], eb = rb[swz ^ 1];
+            const float4 e01 = swz ? eb : ea, e23 = swz ? ea : eb;
+            const float Ex[4] = {e01.x, e01.z, e23.x, e23.z}, Ey[4] = {e01.y, e01.w, e23.y, e23.w};
+#pragma unroll
+            for (int s = 0; s < NS; s++)
+                if (s < FO.count) {
+                    const int c0[4] = {n0[s].x, n0[s].y, n0[s].z, n0[s].w};
+                    const int dxn[4] = {nh[s].x - nl[s].x, nh[s].y - nl[s].y, nh[s].z - nl[s].z, nh[s].w - nl[s].w};
+                    const int dyn[4] = {n0[s].y - nd[s], n0[s].z - n0[s].x, n0[s].w - n0[s].y, nu[s] - n0[s].z};
+                    float fx[4], fy[4];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        fx[u] = FO.qE[s] * Ex[u];
+                        fy[u] = FO.qE[s] * Ey[u];
+                        if (FO.pond[s] != 0.f) { fx[u] -= px[u]; fy[u] -= py[u]; }
+                        if (c0[u] > 0 && FO.cv2[s] != 0.f) {
+                            const float inv_n = 1.f / (float)c0[u];
+                            fx[u] -= FO.cv2[s] * sx * (float)dxn[u] * inv_n;
+                            fy[u] -= FO.cv2[s] * FO.inv_2dy * (float)dyn[u] * inv_n;
+                        }
+                    }
+                    float4 *out = reinterpret_cast<float4 *>(FO.F[s] + row + j0);
+                    out[0] = make_float4(fx[0], fy[0], fx[1], fy[1]);
+                    out[1] = make_float4(fx[2], fy[2], fx[3], fy[3]);
+                }
+        }
+        return;
+    }
     if (MODE == 2) {
         const size_t nn = (size_t)(FO.nx + 1) * ny;
         const int il = i > 0 ? i - 1 : 0, ih = i < FO.nx ? i + 1 : FO.nx;
@@ -517,15 +602,41 @@ __global__ void __launch_bounds__(32) k_tri_reduced(const TriParams T)
 
 // one thread per (k_y, partition): local chasing solve in registers with the true interface values,
 // then the nodal-E spectra of rows kM .. kM+m (plus the wall row nx for the last partition)
-__global__ void __launch_bounds__(128) k_tri_local(const TriParams T)
+// The thread's column of rho^ (rows kM .. kM+m) and of the elimination table go to shared memory by
+// cp.async first -- 2 M independent copies in flight per thread, no registers held -- because the
+// chasing recurrence itself is serial and would otherwise meet one DRAM latency per row.  Every thread
+// reads back only what it copied itself: cp.async.wait_all is the only synchronisation needed.
+constexpr int TL_THREADS = 128;
+constexpr size_t TL_SMEM = (size_t)M * TL_THREADS * (sizeof(float2) + sizeof(double));
+
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src)
 {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+
+__global__ void __launch_bounds__(TL_THREADS) k_tri_local(const TriParams T)
+{
+    extern __shared__ __align__(16) unsigned char tl_smem[];
+    float2 *rs = reinterpret_cast<float2 *>(tl_smem) + threadIdx.x;                                  // [M][TL_THREADS]
+    double *cs = reinterpret_cast<double *>(tl_smem + (size_t)M * TL_THREADS * sizeof(float2)) + threadIdx.x;
     const int l = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
     if (l > T.ny / 2) return;
     const int LP = T.LP;
     const int cls = (k == T.P - 1) ? 1 : 0, m = cls ? T.m_last : M - 1;
-    const double *cp = T.tab.cp + (size_t)cls * M * LP;
     const size_t row0 = (size_t)k * M;
+    {
+        const double *cp = T.tab.cp + (size_t)cls * M * LP;
+        cp_async8(rs, T.rho_hat + row0 * LP + l);
+#pragma unroll
+        for (int j = 1; j < M; j++)
+            if (j <= m) {
+                cp_async8(rs + j * TL_THREADS, T.rho_hat + (row0 + j) * LP + l);
+                cp_async8(cs + j * TL_THREADS, cp + (size_t)j * LP + l);
+            }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     const double2 gl = T.g[(size_t)k * LP + l], gr = T.g[(size_t)(k + 1) * LP + l];
+    asm volatile("cp.async.wait_all;" ::: "memory");
     double dr[M], di[M];
     // forward elimination with the interface values folded into rows 1 and m
     {
@@ -533,8 +644,8 @@ __global__ void __launch_bounds__(128) k_tri_local(const TriParams T)
 #pragma unroll
         for (int j = 1; j < M; j++) {
             if (j <= m) {
-                float2 r = T.rho_hat[(row0 + j) * LP + l];
-                double c = cp[(size_t)j * LP + l];
+                float2 r = rs[j * TL_THREADS];
+                double c = cs[j * TL_THREADS];
                 double rr = T.dx2 * (double)r.x, ri = T.dx2 * (double)r.y;
                 if (j == 1) { rr -= gl.x; ri -= gl.y; }
                 if (j == m) { rr -= gr.x; ri -= gr.y; }
@@ -555,7 +666,7 @@ __global__ void __launch_bounds__(128) k_tri_local(const TriParams T)
 #pragma unroll
     for (int j = M - 1; j >= 1; j--) {
         if (j <= m) {
-            double c = cp[(size_t)j * LP + l];
+            double c = cs[j * TL_THREADS];
             // phi_j; the right boundary value is already folded into d_m
             double pr = dr[j] - (j == m ? 0.0 : c * p1r), pi = di[j] - (j == m ? 0.0 : c * p1i);
             const size_t e = row0 + j + 1;                           // row j+1 now has both neighbours
@@ -597,7 +708,7 @@ __global__ void __launch_bounds__(128) k_tri_local(const TriParams T)
         // phi_{kM-1} from the interface equation: phi_{kM-1} + b g_k + phi_{kM+1} = dx^2 rho^_{kM}
         const double kyc = 2.0 * PI * (double)l / T.Ly;
         const double b = -2.0 - kyc * kyc * T.dx2;
-        float2 r = T.rho_hat[row0 * LP + l];
+        float2 r = rs[0];
         double lr = T.dx2 * (double)r.x - b * gl.x - p1r, li = T.dx2 * (double)r.y - b * gl.y - p1i;
         double sr = lr + 2.0 * gl.x + p1r, si = li + 2.0 * gl.y + p1i;
         T.ehx[row0 * LP + l] = make_float2((float)(kx * (p1r - lr)), (float)(kx * (p1i - li)));
@@ -622,6 +733,7 @@ int launch_poisson_init(pm2d_ctx *c)
     (void)smem;
     {
         const int big_smem = (8192 + 8192 / 16) * (int)sizeof(float2);
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_tri_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL_SMEM));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
@@ -664,7 +776,7 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a, bool use_ha
     dim3 grid((ny / 2 + 1 + 127) / 128, c->tri_P);
     k_tri_sums<<<grid, 128, 0, c->stream>>>(T);
     k_tri_reduced<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
-    k_tri_local<<<grid, 128, 0, c->stream>>>(T);
+    k_tri_local<<<grid, TL_THREADS, TL_SMEM, c->stream>>>(T);
     ForceOut FO;
     FO.count = 0;
     if (force_a) {
