@@ -97,6 +97,7 @@ size_t layout(pm2d_ctx *c, char *base)
         c->tri_cp = cv.take<double>((size_t)2 * TRI_M * LP);
         c->tri_V = cv.take<double>((size_t)2 * TRI_M * LP);
         c->tri_W = cv.take<double>((size_t)2 * TRI_M * LP);
+        c->tri_den = cv.take<double>(P * LP);
         c->tri_sumV = cv.take<double2>(P * LP);
         c->tri_sumW = cv.take<double2>(P * LP);
         c->tri_g = cv.take<double2>((P + 1) * LP);

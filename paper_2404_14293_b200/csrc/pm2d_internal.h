@@ -85,7 +85,7 @@ struct pm2d_ctx {
     float *a[3];         // ring of time levels, each [ncomp][nn]; a[0] = n+1 target, a[1] = n, a[2] = n-1
     float2 *rho_hat;     // [(nx+1)][LP]
     // partitioned chasing method (pm2d_poisson.cu): tables [2][TRI_M][LP], sums [P][LP], g [P+1][LP]
-    double *tri_cp, *tri_V, *tri_W;
+    double *tri_cp, *tri_V, *tri_W, *tri_den;
     double2 *tri_sumV, *tri_sumW, *tri_g;
     int tri_P, tri_mlast;
     float2 *ehx, *ehy;   // [(nx+1)][LP] spectra of nodal E (or phi^ in ehx for diagnostics)

@@ -145,12 +145,14 @@ __device__ __forceinline__ void dft_reg(float2 *v)
 
 // plain_out: the pass writes its results unpadded (index i instead of pad16(i)): the last pass of a transform
 // whose consumer reads runs of consecutive points (k_ifft's force epilogue)
-template <int R, bool INV>
+// NY != 0: the transform length is the compile-time constant NY (n and Ns then fold into immediate offsets)
+template <int R, bool INV, int NY = 0>
 __device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict__ tw, int n, int Ns, bool plain_out = false)
 {
+    if (NY) n = NY;
     const int pad_mask = plain_out ? 0 : -1;
     constexpr int NB = 16 / R;
-    const int T = blockDim.x, q = n / R;
+    const int T = NY ? NY / 16 : (int)blockDim.x, q = n / R;
     float2 v[NB][R];
 #pragma unroll
     for (int b = 0; b < NB; b++) {
@@ -190,9 +192,19 @@ __device__ __forceinline__ void fft16_pass(float2 *buf, const float2 *__restrict
 }
 
 // in place on the padded buffer; blockDim.x == n / 16, n a power of two >= 512; callers synchronise before
-template <bool INV>
-__device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n, bool plain_out = false)
+template <bool INV, int NY = 0>
+__device__ __forceinline__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n, bool plain_out = false)
 {
+    if (NY) {       // constant length: every pass is its own, fully folded copy
+        constexpr int L16 = NY >= 65536 ? 4 : (NY >= 4096 ? 3 : (NY >= 256 ? 2 : 1));      // radix-16 passes
+        constexpr int REM = NY >> (4 * L16);
+#pragma unroll
+        for (int ps = 0; ps < L16; ps++) fft16_pass<16, INV, NY>(buf, tw, NY, 1 << (4 * ps), plain_out && REM == 1 && ps == L16 - 1);
+        if (REM == 8) fft16_pass<8, INV, NY>(buf, tw, NY, 1 << (4 * L16), plain_out);
+        else if (REM == 4) fft16_pass<4, INV, NY>(buf, tw, NY, 1 << (4 * L16), plain_out);
+        else if (REM == 2) fft16_pass<2, INV, NY>(buf, tw, NY, 1 << (4 * L16), plain_out);
+        return;
+    }
     int Ns = 1;
     while (n / Ns >= 16) {
         fft16_pass<16, INV>(buf, tw, n, Ns, plain_out && n / Ns == 16);
@@ -206,16 +218,17 @@ __device__ void fft16_inplace(float2 *buf, const float2 *__restrict__ tw, int n,
 
 // Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
 // rho^_b = (Z_l - conj Z_{n-l}) / 2i.  BIG: register-blocked FFT on the padded buffer (ny >= 512).
-template <int BIG>
+template <int BIG, int NY = 0>
 __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
-                                                                     float2 *__restrict__ rho_hat, int nx, int ny, int LP)
+                                                                     float2 *__restrict__ rho_hat, int nx, int ny_, int LP)
 {
     extern __shared__ float2 buf[];
+    const int ny = NY ? NY : ny_, bdim = NY ? NY / 16 : (int)blockDim.x;
     const int ia = 1 + 2 * blockIdx.x, ib = ia + 1;     // rows 1 .. nx-1 (phi = 0 on the walls, Q5)
     const bool has_b = ib <= nx - 1;
     const size_t rowa = (size_t)ia * ny, rowb = (size_t)ib * ny;
     if (BIG) {
-        // blockDim.x == ny / 16: every thread owns 16 columns, taken in two halves of 8 (registers); the loads of a
+        // bdim == ny / 16: every thread owns 16 columns, taken in two halves of 8 (registers); the loads of a
         // half are issued before their first use
 #pragma unroll
         for (int half = 0; half < 2; half++) {
@@ -227,8 +240,8 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1
                 int ta[8], tb[8];
 #pragma unroll
                 for (int k = 0; k < 8; k++) {
-                    ta[k] = na[threadIdx.x + (half * 8 + k) * blockDim.x];
-                    tb[k] = nb[threadIdx.x + (half * 8 + k) * blockDim.x];
+                    ta[k] = na[threadIdx.x + (half * 8 + k) * bdim];
+                    tb[k] = nb[threadIdx.x + (half * 8 + k) * bdim];
                 }
 #pragma unroll
                 for (int k = 0; k < 8; k++) {
@@ -238,11 +251,11 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1
             }
 #pragma unroll
             for (int k = 0; k < 8; k++)
-                buf[pad16(threadIdx.x + (half * 8 + k) * blockDim.x)] =
+                buf[pad16(threadIdx.x + (half * 8 + k) * bdim)] =
                     make_float2((float)va[k] * S.inv_nscale, has_b ? (float)vb[k] * S.inv_nscale : 0.f);
         }
     } else {
-        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+        for (int j = threadIdx.x; j < ny; j += bdim) {
             int va = 0, vb = 0;
             for (int s = 0; s < S.count; s++) {
                 va += S.sign[s] * S.n[s][rowa + j];
@@ -254,10 +267,10 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1
     float2 *r = buf;
     if (BIG) {
         __syncthreads();
-        fft16_inplace<false>(buf, tw, ny);
+        fft16_inplace<false, NY>(buf, tw, ny);
     } else
         r = fft_stockham<false>(buf, buf + ny, tw, ny);
-    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) {
+    for (int l = threadIdx.x; l <= ny / 2; l += bdim) {
         const int lc = (ny - l) & (ny - 1);
         const float2 z = r[BIG ? pad16(l) : l], zc = r[BIG ? pad16(lc) : lc];
         rho_hat[(size_t)ia * LP + l] = make_float2(0.5f * (z.x + zc.x), 0.5f * (z.y - zc.y));
@@ -283,15 +296,16 @@ struct ForceOut {
 // MODE 0: Z = ehx + i ehy -> Enode (float2);  MODE 1: Z = phi^ -> phi (float, real part);
 // MODE 2: Z = ehx + i ehy -> F_s of every mobile species (ForceOut)
 // NS: species slots of the force epilogue (2 covers electrons + one ion species with fewer registers)
-template <int MODE, int BIG, int NS = PM2D_MAX_SPECIES>
+template <int MODE, int BIG, int NS = PM2D_MAX_SPECIES, int NY = 0>
 __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <= 2 ? 3 : 2) : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
-                                                      float *__restrict__ phi, int ny, int LP, const ForceOut FO)
+                                                      float *__restrict__ phi, int ny_, int LP, const ForceOut FO)
 {
     extern __shared__ float2 buf[];
+    const int ny = NY ? NY : ny_, bdim = NY ? NY / 16 : (int)blockDim.x;
     const int i = blockIdx.x;
 #pragma unroll 4
-    for (int l = threadIdx.x; l <= ny / 2; l += blockDim.x) {
+    for (int l = threadIdx.x; l <= ny / 2; l += bdim) {
         float2 a = hx[(size_t)i * LP + l];
         float2 b = MODE != 1 ? hy[(size_t)i * LP + l] : make_float2(0.f, 0.f);
         // Z_l = a + i b ; Z_{ny-l} = conj(a) + i conj(b)
@@ -301,7 +315,7 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <
     float2 *r = buf;
     if (BIG) {
         __syncthreads();
-        fft16_inplace<true>(buf, tw, ny, MODE == 2);
+        fft16_inplace<true, NY>(buf, tw, ny, MODE == 2);
     } else
         r = fft_stockham<true>(buf, buf + ny, tw, ny);
     if (MODE == 2 && BIG) {
@@ -316,7 +330,7 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <
         for (int s = 0; s < FO.count; s++) any_pond |= FO.pond[s] != 0.f;
         const int swz = (threadIdx.x >> 2) & 1;
 #pragma unroll 1
-        for (int g = threadIdx.x; g < ny / 4; g += blockDim.x) {
+        for (int g = threadIdx.x; g < ny / 4; g += bdim) {
             const int j0 = 4 * g, jm = (j0 - 1) & (ny - 1), jp = (j0 + 4) & (ny - 1);
             int4 n0[NS], nh[NS], nl[NS];
             int nd[NS], nu[NS];
@@ -387,12 +401,12 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <
         for (int s = 0; s < FO.count; s++) any_pond |= FO.pond[s] != 0.f;
         // four nodes per thread at a time, all loads of a batch issued before the arithmetic
         constexpr int NB = 2;
-        for (int jb = threadIdx.x; jb < ny; jb += NB * blockDim.x) {
+        for (int jb = threadIdx.x; jb < ny; jb += NB * bdim) {
             int jj[NB], jm[NB], jp[NB];
             float px[NB], py[NB];
 #pragma unroll
             for (int u = 0; u < NB; u++) {
-                jj[u] = min(jb + u * (int)blockDim.x, ny - 1);           // clamped duplicates are not stored
+                jj[u] = min(jb + u * (int)bdim, ny - 1);           // clamped duplicates are not stored
                 jm[u] = (jj[u] - 1) & (ny - 1);
                 jp[u] = (jj[u] + 1) & (ny - 1);
                 px[u] = py[u] = 0.f;
@@ -442,13 +456,13 @@ __global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <
                             fx -= FO.cv2[s] * sx * (float)(nh[s][u] - nl[s][u]) * inv_n;
                             fy -= FO.cv2[s] * FO.inv_2dy * (float)(nu[s][u] - nd[s][u]) * inv_n;
                         }
-                        if (jb + u * (int)blockDim.x < ny) FO.F[s][row + jj[u]] = make_float2(fx, fy);
+                        if (jb + u * (int)bdim < ny) FO.F[s][row + jj[u]] = make_float2(fx, fy);
                     }
                 }
         }
         return;
     }
-    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+    for (int j = threadIdx.x; j < ny; j += bdim) {
         const float2 z = r[BIG ? pad16(j) : j];
         if (MODE == 0) Enode[(size_t)i * ny + j] = z;
         else phi[(size_t)i * ny + j] = z.x;
@@ -468,9 +482,10 @@ __global__ void k_twiddle_init(float2 *tw, int ny)
 // tables [cls][j][LP], cls 0 = full partition (m = M-1 interior rows), cls 1 = last partition (m_last)
 struct TriTables {
     double *cp, *V, *W;     // local c', spikes V (1 at the left interface), W (1 at the right interface)
+    double *den;            // [P][LP]: 1 / pivot of row k of the reduced (interface) system, k = 1 .. P-1
 };
 
-__global__ void k_tri_tables(TriTables T, int ny, int LP, int m_last, double dx, double Ly)
+__global__ void k_tri_tables(TriTables T, int ny, int LP, int m_last, int P, double dx, double Ly)
 {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l > ny / 2) return;
@@ -501,6 +516,17 @@ __global__ void k_tri_tables(TriTables T, int ny, int LP, int m_last, double dx,
             w = (j == m ? -cp[(size_t)j * LP + l] : 0.0) - cp[(size_t)j * LP + l] * w;
             W[(size_t)j * LP + l] = w;
         }
+    }
+    // pivots of the reduced system (right-hand-side independent): row k is
+    //   Vm g_{k-1} + (Wm + b + V1(k)) g_k + W1 g_{k+1} = ...
+    const double Vm = T.V[(size_t)(M - 1) * LP + l], Wm = T.W[(size_t)(M - 1) * LP + l];
+    const double V1 = T.V[(size_t)1 * LP + l], W1 = T.W[(size_t)1 * LP + l];
+    const double V1_last = m_last >= 1 ? T.V[((size_t)M + 1) * LP + l] : 0.0;
+    double cprev = 0.0;
+    for (int k = 1; k <= P - 1; k++) {
+        const double den = 1.0 / (Wm + b + (k == P - 1 ? V1_last : V1) - Vm * cprev);
+        cprev = W1 * den;
+        T.den[(size_t)k * LP + l] = den;
     }
 }
 
@@ -597,6 +623,68 @@ __global__ void __launch_bounds__(32) k_tri_reduced(const TriParams T)
                 cd[(size_t)k * LP + l] = make_double2(gr, gi);
             }
         }
+    }
+}
+
+// The same solve with every input of the thread -- r, S_W, S_V and the tabulated pivots of all P-1 rows -- copied to
+// shared memory by cp.async first: the two recurrences then run at arithmetic latency instead of meeting a memory
+// round trip per chunk of rows.  Few threads per CTA (the staged column of one k_y is 48 (P-1) bytes).
+constexpr int TR_THREADS = 8;
+__host__ __device__ constexpr size_t tri_reduced_smem(int P) { return (size_t)(P - 1) * TR_THREADS * 48; }
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async8r(void *smem_dst, const void *gmem_src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+
+__global__ void __launch_bounds__(TR_THREADS) k_tri_reduced_staged(const TriParams T)
+{
+    extern __shared__ __align__(16) unsigned char tr_smem[];
+    const int LP = T.LP, P = T.P, nk = P - 1;
+    const int l = blockIdx.x * TR_THREADS + threadIdx.x;
+    if (l > T.ny / 2) return;
+    T.g[l] = make_double2(0.0, 0.0);
+    T.g[(size_t)P * LP + l] = make_double2(0.0, 0.0);
+    if (P < 2) return;
+    double2 *sws = reinterpret_cast<double2 *>(tr_smem) + threadIdx.x;                                   // [nk][TR_THREADS]; later d_k
+    double2 *svs = reinterpret_cast<double2 *>(tr_smem) + (size_t)nk * TR_THREADS + threadIdx.x;
+    double *dens = reinterpret_cast<double *>(tr_smem + (size_t)nk * TR_THREADS * 32) + threadIdx.x;
+    float2 *rs = reinterpret_cast<float2 *>(tr_smem + (size_t)nk * TR_THREADS * 40) + threadIdx.x;
+    for (int k = 1; k <= nk; k++) {
+        const int e = (k - 1) * TR_THREADS;
+        cp_async16(sws + e, T.sumW + (size_t)(k - 1) * LP + l);
+        cp_async16(svs + e, T.sumV + (size_t)k * LP + l);
+        cp_async8r(dens + e, T.tab.den + (size_t)k * LP + l);
+        cp_async8r(rs + e, T.rho_hat + (size_t)(k * M) * LP + l);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const double Vm = T.tab.V[(size_t)(M - 1) * LP + l], W1 = T.tab.W[(size_t)1 * LP + l];
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    double dr = 0.0, di = 0.0;
+#pragma unroll 4
+    for (int k = 1; k <= nk; k++) {
+        const int e = (k - 1) * TR_THREADS;
+        const double den = dens[e];
+        const double2 sw = sws[e], sv = svs[e];
+        const float2 r = rs[e];
+        const double Rr = T.dx2 * (double)r.x + sw.x + sv.x, Ri = T.dx2 * (double)r.y + sw.y + sv.y;
+        dr = (Rr - Vm * dr) * den;
+        di = (Ri - Vm * di) * den;
+        sws[e] = make_double2(dr, di);
+    }
+    double gr = 0.0, gi = 0.0;
+#pragma unroll 4
+    for (int k = nk; k >= 1; k--) {
+        const int e = (k - 1) * TR_THREADS;
+        const double cc = W1 * dens[e];
+        const double2 d = sws[e];
+        gr = d.x - cc * gr;
+        gi = d.y - cc * gi;
+        T.g[(size_t)k * LP + l] = make_double2(gr, gi);
     }
 }
 
@@ -725,8 +813,10 @@ int launch_poisson_init(pm2d_ctx *c)
     c->tri_P = (nx + M - 1) / M;
     c->tri_mlast = nx - (c->tri_P - 1) * M - 1;
     k_twiddle_init<<<(ny / 2 + 127) / 128, 128, 0, c->stream>>>(c->twiddle, ny);
-    TriTables T{c->tri_cp, c->tri_V, c->tri_W};
-    k_tri_tables<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T, ny, c->LP, c->tri_mlast, c->g.dx, ny * c->g.dy);
+    TriTables T{c->tri_cp, c->tri_V, c->tri_W, c->tri_den};
+    k_tri_tables<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T, ny, c->LP, c->tri_mlast, c->tri_P, c->g.dx, ny * c->g.dy);
+    if (c->tri_P >= 2 && tri_reduced_smem(c->tri_P) <= 100 * 1024)
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_tri_reduced_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tri_reduced_smem(c->tri_P)));
     count_launch(c, 2);
     PM2D_CUDA_CHECK(cudaGetLastError());
     const int smem = 2 * ny * (int)sizeof(float2);       // small-n path only (ny < 512): 8 KB at most
@@ -740,6 +830,8 @@ int launch_poisson_init(pm2d_ctx *c)
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_fft_rho<2, 8192>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
+        PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 2, PM2D_MAX_SPECIES, 8192>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
         PM2D_CUDA_CHECK(cudaFuncSetAttribute(k_ifft<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem));
@@ -764,18 +856,25 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a, bool use_ha
             S.sign[S.count] = c->sp[s].cfg.sign;
             S.count++;
         }
-    if (big == 2) k_fft_rho<2><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    if (ny == 8192) k_fft_rho<2, 8192><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else if (ny == 4096) k_fft_rho<1, 4096><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else if (ny == 2048) k_fft_rho<1, 2048><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else if (ny == 1024) k_fft_rho<1, 1024><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
+    else if (big == 2) k_fft_rho<2><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
     else if (big == 1) k_fft_rho<1><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
     else k_fft_rho<0><<<nx / 2, fft_threads, smem, c->stream>>>(S, c->twiddle, c->rho_hat, nx, ny, c->LP);
     TriParams T;
     T.rho_hat = c->rho_hat; T.phi_hat = want_phi ? c->rho_hat : nullptr;
-    T.tab = TriTables{c->tri_cp, c->tri_V, c->tri_W};
+    T.tab = TriTables{c->tri_cp, c->tri_V, c->tri_W, c->tri_den};
     T.sumV = c->tri_sumV; T.sumW = c->tri_sumW; T.g = c->tri_g;
     T.ehx = c->ehx; T.ehy = c->ehy; T.nx = nx; T.ny = ny; T.LP = c->LP; T.P = c->tri_P; T.m_last = c->tri_mlast;
     T.dx2 = c->g.dx * c->g.dx; T.inv_dx = 1.0 / c->g.dx; T.inv_dy = 1.0 / c->g.dy; T.inv_ny = 1.0 / ny; T.Ly = ny * c->g.dy;
     dim3 grid((ny / 2 + 1 + 127) / 128, c->tri_P);
     k_tri_sums<<<grid, 128, 0, c->stream>>>(T);
-    k_tri_reduced<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
+    if (c->tri_P >= 2 && tri_reduced_smem(c->tri_P) <= 100 * 1024)
+        k_tri_reduced_staged<<<(ny / 2 + 1 + TR_THREADS - 1) / TR_THREADS, TR_THREADS, tri_reduced_smem(c->tri_P), c->stream>>>(T);
+    else
+        k_tri_reduced<<<(ny / 2 + 1 + 31) / 32, 32, 0, c->stream>>>(T);
     k_tri_local<<<grid, TL_THREADS, TL_SMEM, c->stream>>>(T);
     ForceOut FO;
     FO.count = 0;
@@ -792,7 +891,11 @@ int launch_poisson(pm2d_ctx *c, bool want_phi, const float *force_a, bool use_ha
         }
         FO.a = force_a; FO.ncomp = c->g.ncomp; FO.nx = nx;
         FO.inv_2dx = (float)(1.0 / (2.0 * c->g.dx)); FO.inv_2dy = (float)(1.0 / (2.0 * c->g.dy));
-        if (big == 2) k_ifft<2, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        if (ny == 8192) k_ifft<2, 2, PM2D_MAX_SPECIES, 8192><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (ny == 4096 && FO.count <= 2) k_ifft<2, 1, 2, 4096><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (ny == 2048 && FO.count <= 2) k_ifft<2, 1, 2, 2048><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (ny == 1024 && FO.count <= 2) k_ifft<2, 1, 2, 1024><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
+        else if (big == 2) k_ifft<2, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
         else if (big == 1 && FO.count <= 2) k_ifft<2, 1, 2><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
         else if (big == 1) k_ifft<2, 1><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
         else k_ifft<2, 0><<<nx + 1, fft_threads, smem, c->stream>>>(c->ehx, c->ehy, c->twiddle, nullptr, nullptr, ny, c->LP, FO);
