@@ -153,7 +153,8 @@ def run_cuda(args):
     cfg = I.config(args.config)
     cfg["seed"] = int(cfg["seed"]) + 1000 * rank          # independent replicas
     g = cfg["grid"]
-    sim = pkg.PM2D(cfg, device=f"cuda:{local}", eager_moments=args.eager, rebin_every=args.rebin_every)
+    order = {"auto": pkg.ORDER_AUTO, "cellmajor": pkg.ORDER_CELL_MAJOR, "layered": pkg.ORDER_LAYERED, "random": pkg.ORDER_RANDOM}[args.order]
+    sim = pkg.PM2D(cfg, device=f"cuda:{local}", eager_moments=args.eager, rebin_every=args.rebin_every, particle_order=order)
     nmob = sum(sim.particle_count(s) for s, sp in enumerate(cfg["species"]) if sp["mobile"])
     nodes = (g["nx"] + 1) * g["ny"]
 
@@ -197,7 +198,8 @@ def run_cuda(args):
         peak, peak_src = hbm_peak()
         steps_p = max(prof["steps"], 1)
         stage_ms = (prof["ms"]["stage_a"] + prof["ms"]["stage_b"]) / steps_p
-        alg_bytes = (BYTES_STAGE_A + BYTES_STAGE_B) * nmob
+        per_particle = BYTES_STAGE_A + BYTES_STAGE_B + (8 if args.order == "random" else 0)   # random order: + the tile index, read at both stages
+        alg_bytes = per_particle * nmob
         achieved = alg_bytes / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
         traffic = None
         tp = os.path.join(ROOT, "profiles", "stage_traffic_bytes.txt")
@@ -212,7 +214,7 @@ def run_cuda(args):
                     config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU "
                                          f"(BASELINE.json configs[{int(args.config[1]) - 1}])",
                                 shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
-                                eager_moments=bool(args.eager), rebin_every=sim.grid.rebin_every,
+                                eager_moments=bool(args.eager), rebin_every=sim.grid.rebin_every, particle_order=args.order,
                                 l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
                                 parallelism="replicas only" if world > 1 else "1 GPU"),
                     ns_per_particle_step=1e9 / value * world,
@@ -225,7 +227,7 @@ def run_cuda(args):
                              h2d_bytes_per_step=int(len(lasers) * 48), d2h_bytes_per_step=int(g["ny"] * 4 + 16)),
                     roofline=dict(bound="hbm", kernel="k_stage (fused gather-push-deposit; per step: stage A + stage B launches of every mobile species)",
                                   achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, peak_source=peak_src,
-                                  algorithmic_bytes_per_particle_step=BYTES_STAGE_A + BYTES_STAGE_B,
+                                  algorithmic_bytes_per_particle_step=per_particle,
                                   ms_per_step=stage_ms, traffic=traffic))
         if world == 1 and not args.no_cpu_baseline:
             scfg = sample_config(args.config, 1024, 512)
@@ -247,6 +249,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--eager", type=int, default=1, help="1: deposit n, Px, Py at both stages (paper's flow); 0: n only")
     ap.add_argument("--rebin-every", type=int, default=None)
+    ap.add_argument("--order", default="auto", choices=["auto", "cellmajor", "layered", "random"],
+                    help="particle storage order; random = BASELINE config 5 run A (no tile staging, global atomics, no rebin)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

@@ -64,8 +64,13 @@ enum {
 /* Storage order of a species inside a tile (as of the last rebin).  CELL_MAJOR: (cell, rank in cell), walked by
  * strip threads with register accumulation (dense species).  LAYERED: (min(rank, 16), cell, rank): 32 consecutive
  * particles lie in 32 different cells, walked one particle per thread.  AUTO: LAYERED up to 16 particles per cell on
- * average (and never for PM2D_NUMBER_WEIGHTED), else CELL_MAJOR. */
-enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2 };
+ * average (and never for PM2D_NUMBER_WEIGHTED), else CELL_MAJOR.
+ * RANDOM (BASELINE.json config 5, "particles stored in random order"): the loader's particles are stored in a
+ * pseudo-random permutation with an explicit tile index each (+4 B per particle); no tile is staged: every particle
+ * gathers from the global force grid and deposits with integer atomics on the global grids (L2).  No rebin (the
+ * positions stay relative to the tile a particle was loaded into: a run may drift at most 64 cells from it, else
+ * PM2D_ESTATE), pm2d_rebin and pm2d_set_particles return PM2D_ESTATE.  It exists to measure what the sort buys. */
+enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2, PM2D_ORDER_RANDOM = 3 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 
 typedef struct pm2d_ctx pm2d_ctx; /* opaque */

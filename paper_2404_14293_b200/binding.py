@@ -20,7 +20,7 @@ LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
 PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
 FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
-ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, LAYERS = 0, 1, 2, 16
+ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, ORDER_RANDOM, LAYERS = 0, 1, 2, 3, 16
 PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 
 

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpm2d.so")
 SOURCES = ["pm2d_api.cu", "pm2d_particles.cu", "pm2d_fields.cu", "pm2d_poisson.cu", "pm2d_diag.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-diag-suppress", "128", "-Wno-deprecated-gpu-targets", "--use_fast_math=false"]
 
 
 def _stale() -> bool:

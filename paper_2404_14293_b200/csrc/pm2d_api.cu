@@ -60,7 +60,7 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (!is_pow2(g->ny) || g->ny < 8 || g->ny > 8192) return fail(PM2D_EINVAL, "ny must be a power of two in [8, 8192]");
     if (g->ncomp < 1 || g->ncomp > 3) return fail(PM2D_EINVAL, "ncomp must be 1..3");
     if (g->rebin_every < 0 || g->rebin_every > 32) return fail(PM2D_EINVAL, "rebin_every must be 0..32");
-    if (g->particle_order < PM2D_ORDER_AUTO || g->particle_order > PM2D_ORDER_LAYERED) return fail(PM2D_EINVAL, "unknown particle_order");
+    if (g->particle_order < PM2D_ORDER_AUTO || g->particle_order > PM2D_ORDER_RANDOM) return fail(PM2D_EINVAL, "unknown particle_order");
     if (!(g->dx > 0) || !(g->dy > 0) || !(g->dt > 0)) return fail(PM2D_EINVAL, "dx, dy, dt must be positive");
     if (g->dt / g->dx > 0.999 || g->dt / g->dy > 0.999)
         return fail(PM2D_EINVAL, "dt/dx must be < 1: a particle may not cross more than one cell per step");
@@ -126,7 +126,10 @@ size_t layout(pm2d_ctx *c, char *base)
         S.pxfix = S.pyfix = nullptr; S.F = nullptr;
         S.np = S.cap = species_np(g, S.cfg);
         S.layered = false;
+        S.random = false;
+        S.ptile = nullptr;
         if (!S.cfg.mobile) continue;
+        S.random = g.particle_order == PM2D_ORDER_RANDOM;
         // layered order + thread-per-particle kernel up to 16 particles per cell on average; the number-weighted
         // loader fills cell runs, so it stays cell-major
         if (S.cfg.load != PM2D_NUMBER_WEIGHTED)
@@ -143,6 +146,7 @@ size_t layout(pm2d_ctx *c, char *base)
         S.uh = cv.take<float2>(cap);
         S.w = cv.take<float>(cap); S.w2 = cv.take<float>(cap);
         S.cell_off = cv.take<int32_t>((size_t)ntiles * CPITCH);
+        if (S.random) S.ptile = cv.take<int32_t>(cap);
         S.id = S.id2 = nullptr;
         if (g.track_ids) { S.id = cv.take<int64_t>(cap); S.id2 = cv.take<int64_t>(cap); }
         S.max_chunks = ntiles + (int32_t)(cap / CHUNK) + 1;
@@ -375,8 +379,10 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     for (int s = 0; s < nsp; s++) {
         SpeciesDev &S = c->sp[s];
         if (!S.cfg.mobile) continue;
-        if (S.cfg.load != PM2D_LOAD_NONE) INIT_CHECK(launch_load_particles(c, s));
-        else {
+        if (S.cfg.load != PM2D_LOAD_NONE) {
+            INIT_CHECK(launch_load_particles(c, s));
+            if (S.random) INIT_CHECK(launch_shuffle_random(c, s));
+        } else {
             S.np = 0;   // until pm2d_set_particles
             INIT_CHECK(launch_build_chunks(c, s));   // all-zero tile_off -> zero chunks
         }
@@ -450,7 +456,7 @@ static int enqueue_step(pm2d_ctx *c)
     if (c->g.rebin_every > 0 && c->step % c->g.rebin_every == 0) {
         phase_begin(c, PM2D_PH_REBIN);
         for (int s = 0; s < c->nsp; s++)
-            if (c->sp[s].cfg.mobile && (rc = launch_rebin(c, s, nullptr, nullptr, nullptr))) return rc;
+            if (c->sp[s].cfg.mobile && !c->sp[s].random && (rc = launch_rebin(c, s, nullptr, nullptr, nullptr))) return rc;
         phase_end(c);
     }
     return PM2D_OK;
@@ -640,6 +646,7 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
 {
     if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
     SpeciesDev &S = c->sp[s];
+    if (S.random) return fail(PM2D_ESTATE, "PM2D_ORDER_RANDOM takes its particles from the loader only");
     if (count < 0 || count > S.cap) return fail(PM2D_ENOMEM, "more particles than capacity");
     if (count > 0 && (!ix || !iy || !fx || !fy || !ux || !uy || !w)) return fail(PM2D_EINVAL, "null particle array");
     const int nx = c->g.nx, ny = c->g.ny, nty = c->nty, ntiles = c->ntiles;
@@ -714,6 +721,7 @@ extern "C" int pm2d_rebin(pm2d_ctx *c, int s, int32_t *keys_out, int64_t *perm_o
 {
     if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile) return fail(PM2D_EINVAL, "bad species");
     SpeciesDev &S = c->sp[s];
+    if (S.random) return fail(PM2D_ESTATE, "PM2D_ORDER_RANDOM has no rebin");
     int32_t *dk = nullptr;
     int64_t *dp = nullptr, *dt = nullptr;
     const size_t n = (size_t)std::max<int64_t>(S.np, 1);

@@ -36,6 +36,8 @@ struct SpeciesDev {
     double vth2;
     int64_t np;          // particles held (constant: walls reflect, y wraps)
     int64_t cap;
+    bool random;         // PM2D_ORDER_RANDOM: permuted storage + ptile, global gather / deposit, no rebin
+    int32_t *ptile;      // [cap] tile of every particle (random order only)
     bool layered;        // storage order inside a tile: (rank in cell, cell) + thread-per-particle stage kernel;
                          // else (cell, rank) + strip kernel
     // particles (device), stored tile by tile and, inside a tile, cell by cell (as of the last rebin)
@@ -130,6 +132,7 @@ static inline void count_launch(pm2d_ctx *c, int n = 1)
 // ---- launchers (each enqueues on c->stream and returns a PM2D_* code) --------------------------
 // pm2d_particles.cu
 int launch_load_particles(pm2d_ctx *c, int s);
+int launch_shuffle_random(pm2d_ctx *c, int s);
 int launch_stage(pm2d_ctx *c, int s, int stage);            // 0 = A (Eq. 17), 1 = B (Eq. 19)
 int launch_deposit_only(pm2d_ctx *c, int s, bool density, bool momentum);
 int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64_t *perm_tmp_dev);

@@ -855,6 +855,21 @@ __global__ void __launch_bounds__(128) k_stage_overflow(const PartParams P)
     }
 }
 
+// ---- PM2D_ORDER_RANDOM: no tile staging at all (BASELINE config 5, run A) -------------------------------------------
+// one particle per thread in storage order; gather from the global force grid, integer atomics on the global grids
+template <int SHAPE, int STAGE, int QMASK>
+__global__ void __launch_bounds__(256) k_stage_random(const PartParams P, const int32_t *__restrict__ ptile, int64_t np)
+{
+    for (int64_t p = (int64_t)blockIdx.x * 256 + threadIdx.x; p < np; p += (int64_t)gridDim.x * 256) {
+        const int tile = ptile[p];
+        process_direct<SHAPE, STAGE, QMASK, false>(P, p, false, (tile / P.nty) * TILE, (tile % P.nty) * TILE, nullptr, nullptr);
+        if (STAGE == 1) {     // the tile-relative fixed point covers cells -64 .. 191 of the loading tile
+            const uint32_t cx = P.pv[p].x >> POS_FRAC_BITS, cy = P.pv[p].y >> POS_FRAC_BITS;
+            if (cx < 4u || cx > 250u || cy < 4u || cy > 250u) P.flags[2] = 1;
+        }
+    }
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -1476,19 +1491,62 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
     }
 }
 
+// A pseudo-random bijection of [0, n): four Feistel rounds on 2 * hb bits, walked until the image is < n.
+__device__ __forceinline__ uint32_t mix32(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352du;
+    x ^= x >> 15; x *= 0x846ca68bu;
+    x ^= x >> 16;
+    return x;
+}
+__device__ __forceinline__ int64_t feistel_perm(int64_t q, int64_t n, int hb, uint32_t key)
+{
+    const uint32_t mask = (1u << hb) - 1u;
+    do {
+        uint32_t L = (uint32_t)(q >> hb) & mask, R = (uint32_t)q & mask;
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            const uint32_t t = L ^ (mix32(R * 0x9E3779B1u + key + 0x632BE5ABu * (uint32_t)r) & mask);
+            L = R;
+            R = t;
+        }
+        q = ((int64_t)L << hb) | R;
+    } while (q >= n);
+    return q;
+}
+
+// slot q takes the particle of slot perm(q) of the tile-ordered arrays, and remembers its tile
+__global__ void __launch_bounds__(256) k_shuffle_random(const PV *pv, const float *w, const int64_t *id, PV *pv2, float *w2, int64_t *id2,
+                                                        int32_t *ptile, const int64_t *tile_off, int ntiles, int64_t np, int hb, uint32_t key)
+{
+    for (int64_t q = (int64_t)blockIdx.x * 256 + threadIdx.x; q < np; q += (int64_t)gridDim.x * 256) {
+        const int64_t src = feistel_perm(q, np, hb, key);
+        int lo = 0, hi = ntiles;                 // last tile with tile_off[tile] <= src
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (tile_off[mid] <= src) lo = mid; else hi = mid;
+        }
+        pv2[q] = pv[src];
+        w2[q] = w[src];
+        if (id) id2[q] = id[src];
+        ptile[q] = lo;
+    }
+}
+
 // canonical (ix, iy, fx, fy) and velocity of the particles of each chunk, as separate arrays
 __global__ void __launch_bounds__(PTHREADS) k_unpack(const PV *pv, const int32_t *chunk_tile, const int64_t *chunk_beg,
                                                      const int64_t *tile_off, const int32_t *nchunks, int nty, int ny, int32_t *ix,
-                                                     int32_t *iy, float *fx, float *fy, float *ux, float *uy)
+                                                     int32_t *iy, float *fx, float *fy, float *ux, float *uy, const int32_t *ptile)
 {
     const int chunk = blockIdx.x;
     if (chunk >= *nchunks) return;
-    const int tile = chunk_tile[chunk];
+    const int ctile = chunk_tile[chunk];
     const int64_t beg = chunk_beg[chunk];
     int64_t end = beg + CHUNK;
-    if (tile_off[tile + 1] < end) end = tile_off[tile + 1];
-    const int gx0 = (tile / nty) * TILE, gy0 = (tile % nty) * TILE;
+    if (tile_off[ctile + 1] < end) end = tile_off[ctile + 1];
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
+        const int tile = ptile ? ptile[p] : ctile;      // random order: the slots of a chunk hold particles of any tile
+        const int gx0 = (tile / nty) * TILE, gy0 = (tile % nty) * TILE;
         const PV me = pv[p];
         ix[p] = gx0 + (int)(me.x >> POS_FRAC_BITS) - POS_BIAS;
         iy[p] = (gy0 + (int)(me.y >> POS_FRAC_BITS) - POS_BIAS) & (ny - 1);
@@ -1559,6 +1617,26 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     PM2D_CUDA_CHECK(cudaMemsetAsync(c->ovf_count, 0, sizeof(int32_t), c->stream));
     if (stage == 0) {          // stage A deposits (x^, u^) into the second set (zeroed by the caller's side stream)
         P.nfix = S.nhat; P.pxfix = S.pxhat; P.pyfix = S.pyhat;
+    }
+    if (S.random) {
+        const int grid = (int)std::min<int64_t>((S.np + 255) / 256, (int64_t)148 * 64);
+#define PM2D_LAUNCH_R(SH)                                                                                              \
+        do {                                                                                                           \
+            if (stage == 0) { if (qmask == 3) k_stage_random<SH, 0, 3><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np); \
+                              else k_stage_random<SH, 0, 1><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np); }          \
+            else if (stage == 1) { if (qmask == 3) k_stage_random<SH, 1, 3><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np); \
+                                   else k_stage_random<SH, 1, 1><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np); }     \
+            else if (qmask == 3) k_stage_random<SH, 2, 3><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np);              \
+            else if (qmask == 2) k_stage_random<SH, 2, 2><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np);              \
+            else k_stage_random<SH, 2, 1><<<grid, 256, 0, c->stream>>>(P, S.ptile, S.np);                              \
+        } while (0)
+        if (S.cfg.shape == PM2D_CIC) PM2D_LAUNCH_R(PM2D_CIC);
+        else if (S.cfg.shape == PM2D_TSC) PM2D_LAUNCH_R(PM2D_TSC);
+        else PM2D_LAUNCH_R(PM2D_SINE);
+#undef PM2D_LAUNCH_R
+        count_launch(c, 1);
+        PM2D_CUDA_CHECK(cudaGetLastError());
+        return PM2D_OK;
     }
     // layered species take the thread-per-particle kernel, cell-major ones the strip kernel
     const bool sparse = S.layered;
@@ -1638,6 +1716,25 @@ int launch_load_particles(pm2d_ctx *c, int s)
     return PM2D_OK;
 }
 
+// PM2D_ORDER_RANDOM: permute the freshly loaded (tile-ordered) arrays into the second buffers and make those current
+int launch_shuffle_random(pm2d_ctx *c, int s)
+{
+    SpeciesDev &S = c->sp[s];
+    if (S.np == 0) return PM2D_OK;
+    int bits = 1;
+    while (((int64_t)1 << bits) < S.np) bits++;
+    const int hb = (bits + 1) / 2;
+    const int grid = (int)std::min<int64_t>((S.np + 255) / 256, (int64_t)148 * 64);
+    k_shuffle_random<<<grid, 256, 0, c->stream>>>(S.pv, S.w, S.id, S.pv2, S.w2, S.id2, S.ptile, S.tile_off, c->ntiles, S.np, hb,
+                                                  (uint32_t)(c->seed * 0x9E3779B97F4A7C15ull >> 32) + (uint32_t)s);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    std::swap(S.pv, S.pv2);
+    std::swap(S.w, S.w2);
+    std::swap(S.id, S.id2);
+    return PM2D_OK;
+}
+
 // keys_dev / perm_dev: optional outputs of the test entry point pm2d_rebin; perm_tmp_dev: scratch of np
 // int64, required when either is given
 int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64_t *perm_tmp_dev)
@@ -1675,7 +1772,7 @@ int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float 
     SpeciesDev &S = c->sp[s];
     if (S.np == 0) return PM2D_OK;
     k_unpack<<<S.max_chunks, PTHREADS, 0, c->stream>>>(S.pv, S.chunk_tile, S.chunk_beg, S.tile_off, S.nchunks_dev, c->nty, c->g.ny,
-                                                        ix, iy, fx, fy, ux, uy);
+                                                        ix, iy, fx, fy, ux, uy, S.random ? S.ptile : nullptr);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;

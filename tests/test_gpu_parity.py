@@ -130,11 +130,12 @@ def _compare_particles(sim, orc, cfg, s, vth):
     return ex, ey, eu, max(dX.max(), dY.max())
 
 
-@pytest.mark.parametrize("order", [0, 1], ids=["auto", "cellmajor"])
+@pytest.mark.parametrize("order", [0, 1, 3], ids=["auto", "cellmajor", "random"])
 @pytest.mark.parametrize("name,nx,ny,rebin", [("c1", 96, 64, 0), ("c2", 80, 32, 3), ("c3", 72, 64, 1), ("c3", 64, 16, 4), ("c5", 48, 64, 2)])
 def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin, order):
     """order auto: layered storage + thread-per-particle stage kernel for c1-c3, cell-major + strip kernel for c5;
-    order cell-major: the strip kernel for every config."""
+    order cell-major: the strip kernel for every config; order random (BASELINE config 5, run A): permuted storage,
+    gather and deposit on the global grids, no rebin."""
     if name == "c5" and order == 1:
         pytest.skip("c5 is cell-major already")
     cfg = small_cfg(name, nx, ny)
@@ -171,6 +172,27 @@ def test_ten_step_trajectory_and_field_parity(P, name, nx, ny, rebin, order):
     orc.refresh_fields()
     phi = sim.get_fields(P.FIELD_PHI)
     assert rel_l2(phi, orc.phi.reshape(nx + 1, ny)) < 2e-4
+    sim.close()
+
+
+def test_random_order_storage(P):
+    """PM2D_ORDER_RANDOM: the loader's particles, all of them and unchanged, in a storage order that is not tile-major;
+    rebin and host-supplied particles are refused."""
+    cfg = small_cfg("c5", 64, 64)
+    sim = P.PM2D(cfg, track_ids=1, particle_order=P.ORDER_RANDOM)
+    ref = I.generate_particles(cfg, 0)
+    got = sim.get_particles(0, with_id=True)
+    order = np.argsort(got["id"])
+    assert np.array_equal(got["id"][order], ref["id"])
+    for k in ("ix", "iy", "fx", "fy", "w"):
+        assert np.array_equal(got[k][order], ref[k]), k
+    key = (got["ix"] // P.TILE) * (64 // P.TILE) + got["iy"] // P.TILE
+    assert (np.diff(key) < 0).mean() > 0.2                    # four tiles: a sorted order would have none
+    assert np.abs(np.corrcoef(np.arange(key.size), got["id"])[0, 1]) < 0.05
+    with pytest.raises(P.PM2DError):
+        sim.rebin(0)
+    with pytest.raises(P.PM2DError):
+        sim.set_particles(0, {k: got[k][:4] for k in ("ix", "iy", "fx", "fy", "ux", "uy", "w")})
     sim.close()
 
 
