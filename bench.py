@@ -231,9 +231,9 @@ def run_cuda(args):
                                   ms_per_step=stage_ms, traffic=traffic))
         if world == 1 and not args.no_cpu_baseline:
             scfg = sample_config(args.config, 1024, 512)
-            v, sec, n = time_oracle(scfg, 3, 1)
+            v, sec, n = time_oracle(scfg, 8, 1)         # about 12 s of CPU work
             line["cpu_baseline"] = dict(value=v, unit="particle-steps/s", cores=1, kind="oracle",
-                                        sample=f"{scfg['name']} reduced copy of the workload: {n} mobile particles x 3 steps ({sec * 3:.1f} s)")
+                                        sample=f"{scfg['name']} reduced copy of the workload: {n} mobile particles x 8 steps ({sec * 8:.1f} s)")
         print(json.dumps(line))
     sim.close()
     if world > 1:

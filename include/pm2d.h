@@ -73,6 +73,11 @@ enum {
 enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2, PM2D_ORDER_RANDOM = 3 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 
+/* The edge taper ends at 1 % of the profile: macro-particles of neighbouring cells must not differ in weight by
+ * orders of magnitude, or a light particle that wanders next to heavy ones sees grad(n)/n ~ (n_heavy/n_light)/dx in
+ * the pressure term of Eq. 16 and runs away (Q20). */
+#define PM2D_TAPER_FLOOR 0.01
+
 typedef struct pm2d_ctx pm2d_ctx; /* opaque */
 
 typedef struct {
@@ -103,7 +108,9 @@ typedef struct {
 
 typedef struct {
     int32_t kind;          /* PM2D_PROFILE_*                                                          */
-    int32_t taper_cells;   /* sin^2 edge taper at both x walls (Q9); 0 = none                         */
+    int32_t taper_cells;   /* edge taper at both x walls (Q9): within taper_cells of a wall the profile is
+                              multiplied by PM2D_TAPER_FLOOR + (1 - PM2D_TAPER_FLOOR) sin^2(pi d / 2 taper_cells),
+                              d = distance of the cell centre from the wall in cells; 0 = none           */
     double p[4];           /* UNIFORM: n0. LINEAR: n(0), n(Lx). EXP_CAPPED: n0, Lx/L, cap.
                               FILAMENT_Y: mean n0, amplitude A, sigma in cells: n(j) ~ 1 + A exp(-(y-Ly/2)^2/2 sigma^2) */
 } pm2d_profile;

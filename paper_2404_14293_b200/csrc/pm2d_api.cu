@@ -358,7 +358,7 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
                 const double d = std::min((double)i + 0.5, (double)grid->nx - 0.5 - (double)i);
                 if (d < (double)profile->taper_cells) {
                     const double sn = std::sin(0.5 * PI * d / (double)profile->taper_cells);
-                    tx[i] = sn * sn;
+                    tx[i] = PM2D_TAPER_FLOOR + (1.0 - PM2D_TAPER_FLOOR) * (sn * sn);
                 }
             }
         if (profile->kind == PM2D_PROFILE_FILAMENT_Y) nmax = profile->p[0] * *std::max_element(sy.begin(), sy.end());

@@ -920,7 +920,7 @@ __device__ double profile_density(const LoadParams &L, int i)
         double d = fmin((double)i + 0.5, (double)L.nx - 0.5 - (double)i);
         if (d < (double)L.taper_cells) {
             double s = sin(0.5 * PI * d / (double)L.taper_cells);
-            n = n * (s * s);
+            n = n * (PM2D_TAPER_FLOOR + (1.0 - PM2D_TAPER_FLOOR) * (s * s));
         }
     }
     return n;

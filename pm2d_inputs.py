@@ -71,22 +71,21 @@ def profile_density(profile: dict, nx: int, i_cell):
         n = np.full_like(xc, p[0])
     else:
         raise ValueError(kind)
-    tc = int(profile.get("taper_cells", 0))
-    if tc > 0:                                                        # Q9: sin^2 edge taper
-        d = np.minimum(np.asarray(i_cell, dtype=np.float64) + 0.5, nx - 0.5 - np.asarray(i_cell, dtype=np.float64))
-        t = np.where(d < tc, np.sin(0.5 * math.pi * d / tc) ** 2, 1.0)
-        n = n * t
-    return n
+    return n * taper_factor(profile, nx, i_cell)
+
+
+TAPER_FLOOR = 0.01   # the edge taper ends at 1 % of the profile, not at 0 (Q9 / Q20)
 
 
 def taper_factor(profile: dict, nx: int, i_cell):
-    """sin^2 edge taper (Q9) alone, float64."""
+    """Edge taper (Q9) alone, float64: FLOOR + (1 - FLOOR) sin^2(pi d / 2 tc) within tc cells of an x wall."""
     i = np.asarray(i_cell, dtype=np.float64)
     tc = int(profile.get("taper_cells", 0))
     if tc <= 0:
         return np.ones_like(i)
     d = np.minimum(i + 0.5, nx - 0.5 - i)
-    return np.where(d < tc, np.sin(0.5 * math.pi * d / tc) ** 2, 1.0)
+    sn = np.sin(0.5 * math.pi * d / tc)
+    return np.where(d < tc, TAPER_FLOOR + (1.0 - TAPER_FLOOR) * (sn * sn), 1.0)
 
 
 def filament_shape(profile: dict, ny: int):

@@ -424,6 +424,29 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     sim.close()
 
 
+def test_full_length_c2_run_stays_bounded(P):
+    """BASELINE.json config 2 over its full 1000 steps (Q20: with an edge taper that ran to zero, particles
+    of the outermost cells were kicked to |u| >> 1 by the pressure term around step 378 and the run ended in
+    PM2D_ESTATE): the run completes, no particle is faster than the depth of the edge's pressure well plus the thermal
+    tail allows, count and charge are conserved, the energy terms are finite and the kinetic energy changes by < 3 %."""
+    cfg = I.config("c2")
+    sim = P.PM2D(cfg, eager_moments=1)
+    d0 = sim.diagnostics()
+    sim.step(cfg["steps"])
+    d1 = sim.diagnostics()
+    assert d1["step"] == cfg["steps"] == 1000
+    parts = sim.get_particles(0)
+    u = np.hypot(parts["ux"], parts["uy"])
+    vth = math.sqrt(cfg["species"][0]["T_keV"] / 511.0)
+    well = math.sqrt(2.0 * 2.0 * vth ** 2 * math.log(1.0 / I.TAPER_FLOOR))        # u^2/2 = C v_th^2 ln(n_bulk / n_edge)
+    assert u.max() < well + 6.0 * vth, (float(u.max()), well, vth)
+    assert d1["count"][0] == d0["count"][0] == I.n_particles(cfg, 0)
+    assert d1["charge"][0] == pytest.approx(d0["charge"][0], rel=1e-6)
+    assert all(np.isfinite(d1[k]) for k in ("W_es", "W_em", "W_int", "W_total"))
+    assert d1["W_kin"][0] == pytest.approx(d0["W_kin"][0], rel=0.03)
+    sim.close()
+
+
 def test_three_components_two_beams_gaussian_parity(P):
     """All three components of a (Eq. 1 is the same equation for a_x, a_y, a_z; the ponderomotive force takes the
     sum of their squares, Eq. 16), two beams on different components, one of them Gaussian (Eq. 4) and detuned
