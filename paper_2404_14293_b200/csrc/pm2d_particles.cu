@@ -171,7 +171,7 @@ __device__ __forceinline__ bool in_window(int cx, int cy)
 
 // ---- deposit of one particle outside the register patch: 3 x 3 nodes around the nearest node, into the
 // shared window when it covers them, else straight to the global grids (particle far from its tile)
-template <int SHAPE, int QMASK, bool WINDOWED>
+template <int SHAPE, int QMASK, bool WINDOWED, int PITCH = WPITCH>
 __device__ __forceinline__ void deposit_direct(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, float ux, float uy,
                                                float w, int32_t *dep)
 {
@@ -183,18 +183,18 @@ __device__ __forceinline__ void deposit_direct(const PartParams &P, int gx0, int
     weights3<SHAPE>(dy_, P, Wy);
     const float qn = w * P.nscale, qx = w * ux * P.pscale, qy = w * uy * P.pscale;
     if (WINDOWED && in_window(cx, cy)) {
-        const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
+        const int base = (cx - 1 + HALO) * PITCH + (cy - 1 + HALO);
 #pragma unroll
         for (int a = 0; a < 3; a++)
 #pragma unroll
             for (int b = 0; b < 3; b++) {
                 float ww = Wx[a] * Wy[b];
                 if (ww == 0.f) continue;
-                int e = base + a * WPITCH + b;
+                int e = base + a * PITCH + b;
                 if (QMASK & 1) atomicAdd(&dep[e], __float2int_rn(ww * qn));
                 if (QMASK & 2) {
-                    atomicAdd(&dep[WIN * WPITCH + e], __float2int_rn(ww * qx));
-                    atomicAdd(&dep[2 * WIN * WPITCH + e], __float2int_rn(ww * qy));
+                    atomicAdd(&dep[WIN * PITCH + e], __float2int_rn(ww * qx));
+                    atomicAdd(&dep[2 * WIN * PITCH + e], __float2int_rn(ww * qy));
                 }
             }
         return;
@@ -219,7 +219,7 @@ __device__ __forceinline__ void deposit_direct(const PartParams &P, int gx0, int
 
 // Eq. 15 on 3 x 3 nodes around the nearest node: from the shared force window, or (overflow path)
 // from forces evaluated on the global grids
-template <int SHAPE, bool WINDOWED>
+template <int SHAPE, bool WINDOWED, int PITCH = WPITCH>
 __device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, int gy0, uint32_t xf, uint32_t yf, const float2 *Fs, bool &ok)
 {
     int cx, cy;
@@ -232,13 +232,13 @@ __device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, in
     weights3<SHAPE>(dy_, P, Wy);
     float fx = 0.f, fy = 0.f;
     if (WINDOWED) {
-        const int base = (cx - 1 + HALO) * WPITCH + (cy - 1 + HALO);
+        const int base = (cx - 1 + HALO) * PITCH + (cy - 1 + HALO);
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             float rx = 0.f, ry = 0.f;
 #pragma unroll
             for (int b = 0; b < 3; b++) {
-                float2 f = Fs[base + a * WPITCH + b];
+                float2 f = Fs[base + a * PITCH + b];
                 rx += Wy[b] * f.x;
                 ry += Wy[b] * f.y;
             }
@@ -269,7 +269,7 @@ __device__ __forceinline__ float2 gather_direct(const PartParams &P, int gx0, in
 // footprint lies outside the window -- the caller defers the particle to k_stage_overflow (WINDOWED =
 // false, global grids).  The force window is a copy of the global force grid and the deposits are integer
 // sums, so all three routes (register patch, window, global) give identical grids.
-template <int SHAPE, int STAGE, int QMASK, bool WINDOWED>
+template <int SHAPE, int STAGE, int QMASK, bool WINDOWED, int PITCH = WPITCH, int FPITCH = PITCH>
 __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, bool dep_only, int gx0, int gy0, const float2 *Fs,
                                                int32_t *dep)
 {
@@ -284,7 +284,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
             uhy = uh.y;
         } else {
             bool ok;
-            float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xf, yf, Fs, ok);
+            float2 f = gather_direct<SHAPE, WINDOWED, FPITCH>(P, gx0, gy0, xf, yf, Fs, ok);
             if (!ok) return false;
             uhx = __fmaf_rn(P.dt, f.x, ux);                                        // Eq. 17
             uhy = __fmaf_rn(P.dt, f.y, uy);
@@ -299,7 +299,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
         uint32_t xh = advance(xf, P.hx, __fadd_rn(uh.x, ux));                      // x^ of Eq. 17 again
         uint32_t yh = advance(yf, P.hy, __fadd_rn(uh.y, uy));
         bool ok;
-        float2 f = gather_direct<SHAPE, WINDOWED>(P, gx0, gy0, xh, yh, Fs, ok);
+        float2 f = gather_direct<SHAPE, WINDOWED, FPITCH>(P, gx0, gy0, xh, yh, Fs, ok);
         if (!ok) return false;
         float unx = __fmaf_rn(0.5f * P.dt, f.x, 0.5f * __fadd_rn(uh.x, ux));       // Eq. 19
         float uny = __fmaf_rn(0.5f * P.dt, f.y, 0.5f * __fadd_rn(uh.y, uy));
@@ -311,7 +311,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
         ux = unx;
         uy = uny;
     }
-    deposit_direct<SHAPE, QMASK, WINDOWED>(P, gx0, gy0, xf, yf, ux, uy, P.w[p], dep);
+    deposit_direct<SHAPE, QMASK, WINDOWED, PITCH>(P, gx0, gy0, xf, yf, ux, uy, P.w[p], dep);
     return true;
 }
 
@@ -708,6 +708,10 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 // and with a window pitch that is a multiple of 32 words the bank is the column, whatever the row.  12 nodes: 12
 // LDS.64 for the gather, 12 x 3 ATOMS for the deposit, one wavefront each.
 constexpr int DPITCH = 64;
+constexpr int NNPITCH = 64;   // deposit-window pitch of the nearest-node variant
+// its force-window pitch: 64 costs a fifth resident CTA in stage A (48 registers), stage B (4 CTAs by registers) takes it
+template <int STAGE>
+struct NNFPitch { static constexpr int value = STAGE == 1 ? 64 : WPITCH; };
 
 template <int SHAPE, int STAGE, int QMASK>
 __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
@@ -802,7 +806,8 @@ __global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
 {
     constexpr int NT = 256;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
-    constexpr int PITCH = ANCH ? DPITCH : WPITCH;
+    constexpr int PITCH = ANCH ? DPITCH : NNPITCH;
+    constexpr int FPITCH = ANCH ? DPITCH : NNFPitch<STAGE>::value;
     extern __shared__ int32_t direct_smem[];
     int32_t *dep = direct_smem;                                                      // [NQ][WIN][PITCH]
     float2 *Fs = reinterpret_cast<float2 *>(direct_smem + ((NQ * WIN * PITCH + 1) & ~1));   // [WIN][PITCH]
@@ -810,12 +815,12 @@ __global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
     const int64_t t0 = P.tile_off[tile], t1 = P.tile_off[tile + 1];
     if (t1 == t0) return;
     const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
-    if (STAGE < 2) load_force_window<NT, PITCH>(P, gx0, gy0, Fs);
+    if (STAGE < 2) load_force_window<NT, FPITCH>(P, gx0, gy0, Fs);
     for (int e = threadIdx.x; e < NQ * WIN * PITCH; e += NT) dep[e] = 0;
     __syncthreads();
     for (int64_t p = t0 + threadIdx.x; p < t1; p += NT) {
         const bool ok = ANCH ? direct_particle<SHAPE, STAGE, QMASK>(P, p, gx0, gy0, Fs, dep)
-                             : process_direct<SHAPE, STAGE, QMASK, true>(P, p, false, gx0, gy0, Fs, dep);
+                             : process_direct<SHAPE, STAGE, QMASK, true, NNPITCH, NNFPitch<STAGE>::value>(P, p, false, gx0, gy0, Fs, dep);
         if (!ok) push_overflow(P, p, tile, false);
     }
     __syncthreads();
@@ -838,8 +843,8 @@ __global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
 template <int STAGE, int QMASK, bool ANCH>
 constexpr size_t direct_smem_bytes()
 {
-    return (size_t)(((((QMASK & 2) ? 3 : 1) * WIN * (ANCH ? DPITCH : WPITCH)) + 1) & ~1) * 4 +
-           (STAGE < 2 ? (size_t)WIN * (ANCH ? DPITCH : WPITCH) * 8 : 0);
+    return (size_t)(((((QMASK & 2) ? 3 : 1) * WIN * (ANCH ? DPITCH : NNPITCH)) + 1) & ~1) * 4 +
+           (STAGE < 2 ? (size_t)WIN * (ANCH ? DPITCH : NNFPitch<STAGE>::value) * 8 : 0);
 }
 
 // the deferred particles of k_stage: same arithmetic, global grids only
