@@ -676,20 +676,26 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
     std::vector<int64_t> slot_of((size_t)count);          // cell-major slot of every particle (stable)
     for (int64_t p = 0; p < count; p++) slot_of[p] = cur[key[p]]++;
     if (S.layered) {
-        // (min(rank, LAYERS), cell, rank) inside every tile: remap the cell-major slots
+        // the layered order of k_cellsort inside every tile: layer r < LAYERS = particle r of every cell with more than r
+        // particles, by (rank of the cell among the occupied cells of its column, column); then the cell-major tail
         std::vector<int64_t> remap((size_t)count);
         for (int t = 0; t < ntiles; t++) {
             const int32_t *co = coff.data() + (size_t)t * CPITCH;
             if (co[TCELLS] == 0) continue;
             int64_t run = off[t];
-            for (int r = 0; r <= PM2D_LAYERS; r++)
-                for (int cl = 0; cl < TCELLS; cl++) {
-                    const int cnt = co[cl + 1] - co[cl];
-                    if (r < PM2D_LAYERS) {
-                        if (cnt > r) remap[(size_t)(off[t] + co[cl] + r)] = run++;
-                    } else
-                        for (int q = PM2D_LAYERS; q < cnt; q++) remap[(size_t)(off[t] + co[cl] + q)] = run++;
+            for (int r = 0; r < PM2D_LAYERS; r++) {
+                int rows[TILE][TILE], nocc[TILE];
+                for (int j = 0; j < TILE; j++) {
+                    nocc[j] = 0;
+                    for (int i = 0; i < TILE; i++)
+                        if (co[i * TILE + j + 1] - co[i * TILE + j] > r) rows[j][nocc[j]++] = i;
                 }
+                for (int k = 0; k < TILE; k++)
+                    for (int j = 0; j < TILE; j++)
+                        if (k < nocc[j]) remap[(size_t)(off[t] + co[rows[j][k] * TILE + j] + r)] = run++;
+            }
+            for (int cl = 0; cl < TCELLS; cl++)
+                for (int q = PM2D_LAYERS; q < co[cl + 1] - co[cl]; q++) remap[(size_t)(off[t] + co[cl] + q)] = run++;
         }
         for (int64_t p = 0; p < count; p++) slot_of[p] = remap[(size_t)slot_of[p]];
     }

@@ -1331,18 +1331,20 @@ __device__ __forceinline__ int cell_of(uint32_t xf, uint32_t yf)
 // kernel wants (its shared atomics spread over the banks instead of piling up on the nodes of one cell).  Ranks
 // >= LAYERS form a cell-major tail.  Shared memory: hist | cb[LAYERS][TCELLS] (uint16) | cellbeg | tb | small.
 constexpr int LAYERS = PM2D_LAYERS;
-constexpr size_t CELLSORT_LAYERED_SMEM = (size_t)CS_WARPS * TCELLS * 4 + (size_t)LAYERS * TCELLS * 2 + (size_t)(TCELLS + 1) * 4 +
-                                         (size_t)TCELLS * 4 + 64 * 4;
+constexpr size_t CELLSORT_LAYERED_SMEM = (size_t)CS_WARPS * TCELLS * 4 + (size_t)LAYERS * TCELLS + (size_t)(TCELLS + 1) * 4 +
+                                         (size_t)TCELLS * 4 + (LAYERS + 2) * 4 + (size_t)LAYERS * (TILE + 1) * 4 + (size_t)LAYERS * TILE * 4 + 64;
 
 template <bool LAYERED>
 __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams C)
 {
     extern __shared__ int32_t cs_smem[];
     int32_t *hist = cs_smem;                                                  // [CS_WARPS][TCELLS]
-    uint16_t *cb = reinterpret_cast<uint16_t *>(hist + CS_WARPS * TCELLS);    // [LAYERS][TCELLS] (LAYERED)
-    int32_t *cellbeg = LAYERED ? reinterpret_cast<int32_t *>(cb + LAYERS * TCELLS) : hist + CS_WARPS * TCELLS;   // [TCELLS+1]
+    uint8_t *cr = reinterpret_cast<uint8_t *>(hist + CS_WARPS * TCELLS);      // [LAYERS][TCELLS] (LAYERED)
+    int32_t *cellbeg = LAYERED ? reinterpret_cast<int32_t *>(cr + LAYERS * TCELLS) : hist + CS_WARPS * TCELLS;   // [TCELLS+1]
     int32_t *tb = cellbeg + TCELLS + 1;                                       // [TCELLS] (LAYERED)
     int32_t *lay = LAYERED ? tb + TCELLS : cellbeg + TCELLS + 1;              // [LAYERS+2] layer offsets, tail offset
+    int32_t *Tt = lay + LAYERS + 2;                                           // [LAYERS][TILE+1] (LAYERED)
+    uint32_t *Mm = reinterpret_cast<uint32_t *>(Tt + LAYERS * (TILE + 1));    // [LAYERS][TILE] (LAYERED)
     __shared__ int32_t wsum[CS_WARPS];
     const int tile = blockIdx.x;
     const int64_t t0 = C.tile_off[tile];
@@ -1390,73 +1392,69 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
     }
     __syncthreads();
     if (LAYERED) {
-        // cb[r][c] = cells before c that hold more than r particles; lay[r] = first slot of layer r;
-        // tb[c] = particles of rank >= LAYERS in the cells before c; lay[LAYERS] = first slot of that tail.
-        // All LAYERS + 1 prefix sums run in one block scan: four 64-bit words carry 16-bit counters of four layers each.
-        static_assert(LAYERS == 16 && TCELLS <= 65535, "packing of the layer counters");
-        constexpr int PER = TCELLS / (CS_WARPS * 32);
-        __shared__ unsigned long long wsum64[CS_WARPS][4];
+        // Layer r (r < LAYERS) holds one particle of every cell with more than r particles, ordered by (k, j): j the
+        // cell's column (the lane direction of the stage kernel), k the rank of the cell among the occupied cells of
+        // its column.  Any 32 consecutive slots of a layer then lie in (almost always) 32 different columns, also in
+        // the sparse upper layers; a full layer is simply row-major.  Tables:
+        //   cr[r][c]  = k of cell c in layer r          occ (implicit)  = occupied cells of column j in layer r
+        //   T[r][k]   = slots of layer r with rank < k = sum_j min(occ_j, k)
+        //   M[r][k]   = bit j set: column j has more than k occupied cells
+        //   lay[r]    = first slot of layer r; lay[LAYERS] = first slot of the cell-major tail, tb[c] its cell offsets
+        static_assert(LAYERS == 16 && TILE == 32 && CS_WARPS * 32 * 2 == LAYERS * TILE, "two (layer, column) tasks per thread");
+        __shared__ uint8_t occ[LAYERS][TILE];
         __shared__ int32_t wsumt[CS_WARPS];
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+            const int task = threadIdx.x + t * CS_WARPS * 32, r = task >> 5, j = task & 31;
+            int run = 0;
+            for (int i = 0; i < TILE; i++) {
+                const int c = i * TILE + j;
+                if (cellbeg[c + 1] - cellbeg[c] > r) cr[r * TCELLS + c] = (uint8_t)run++;
+            }
+            occ[r][j] = (uint8_t)run;
+        }
+        constexpr int PER = TCELLS / (CS_WARPS * 32);
         const int c0 = threadIdx.x * PER;
-        int cnt[PER];
-        unsigned long long loc[4] = {0ull, 0ull, 0ull, 0ull};
         int loct = 0;
 #pragma unroll
-        for (int u = 0; u < PER; u++) {
-            cnt[u] = cellbeg[c0 + u + 1] - cellbeg[c0 + u];
-#pragma unroll
-            for (int r = 0; r < LAYERS; r++) loc[r >> 2] += (unsigned long long)(cnt[u] > r ? 1 : 0) << (16 * (r & 3));
-            loct += max(cnt[u] - LAYERS, 0);
-        }
-        unsigned long long inc[4] = {loc[0], loc[1], loc[2], loc[3]};
+        for (int u = 0; u < PER; u++) loct += max(cellbeg[c0 + u + 1] - cellbeg[c0 + u] - LAYERS, 0);
         int inct = loct;
         for (int o = 1; o < 32; o <<= 1) {
-#pragma unroll
-            for (int m = 0; m < 4; m++) {
-                unsigned long long t = __shfl_up_sync(0xffffffffu, inc[m], o);
-                if (lane >= o) inc[m] += t;
-            }
             int t = __shfl_up_sync(0xffffffffu, inct, o);
             if (lane >= o) inct += t;
         }
-        if (lane == 31) {
+        if (lane == 31) wsumt[wid] = inct;
+        __syncthreads();
+        for (int task = threadIdx.x; task < LAYERS * (TILE + 1); task += CS_WARPS * 32) {
+            const int r = task / (TILE + 1), k = task - r * (TILE + 1);
+            int sum = 0;
+            uint32_t mask = 0u;
+            for (int j = 0; j < TILE; j++) {
+                const int o = occ[r][j];
+                sum += min(o, k);
+                if (o > k) mask |= 1u << j;
+            }
+            Tt[r * (TILE + 1) + k] = sum;
+            if (k < TILE) Mm[r * TILE + k] = mask;
+        }
+        {
+            int runt = inct - loct;
+            for (int w = 0; w < wid; w++) runt += wsumt[w];
 #pragma unroll
-            for (int m = 0; m < 4; m++) wsum64[wid][m] = inc[m];
-            wsumt[wid] = inct;
+            for (int u = 0; u < PER; u++) {
+                tb[c0 + u] = runt;
+                runt += max(cellbeg[c0 + u + 1] - cellbeg[c0 + u] - LAYERS, 0);
+            }
         }
         __syncthreads();
-        unsigned long long run[4], tot[4] = {0ull, 0ull, 0ull, 0ull};
-        int runt = inct - loct, tott = 0;
-#pragma unroll
-        for (int m = 0; m < 4; m++) run[m] = inc[m] - loc[m];
-        for (int w = 0; w < CS_WARPS; w++) {
-#pragma unroll
-            for (int m = 0; m < 4; m++) {
-                if (w < wid) run[m] += wsum64[w][m];
-                tot[m] += wsum64[w][m];
-            }
-            if (w < wid) runt += wsumt[w];
-            tott += wsumt[w];
-        }
-#pragma unroll
-        for (int u = 0; u < PER; u++) {
-#pragma unroll
-            for (int r = 0; r < LAYERS; r++) {
-                cb[r * TCELLS + c0 + u] = (uint16_t)((run[r >> 2] >> (16 * (r & 3))) & 0xFFFFu);
-                run[r >> 2] += (unsigned long long)(cnt[u] > r ? 1 : 0) << (16 * (r & 3));
-            }
-            tb[c0 + u] = runt;
-            runt += max(cnt[u] - LAYERS, 0);
-        }
         if (threadIdx.x == 0) {
             int slot = 0;
             for (int r = 0; r < LAYERS; r++) {
                 lay[r] = slot;
-                slot += (int)((tot[r >> 2] >> (16 * (r & 3))) & 0xFFFFu);
+                slot += Tt[r * (TILE + 1) + TILE];
             }
             lay[LAYERS] = slot;
         }
-        (void)tott;
         __syncthreads();
     }
     for (int64_t base = beg; base < end; base += 32) {
@@ -1482,7 +1480,11 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
             int64_t q = t0 + b + rank;                 // cell-major slot
             if (LAYERED) {
                 const int r = b + rank - cellbeg[c];   // stable rank of the particle in its cell
-                q = t0 + (r < LAYERS ? lay[r] + (int)cb[r * TCELLS + c] : lay[LAYERS] + tb[c] + (r - LAYERS));
+                if (r < LAYERS) {
+                    const int k = cr[r * TCELLS + c], j = c & (TILE - 1);
+                    q = t0 + lay[r] + Tt[r * (TILE + 1) + k] + __popc(Mm[r * TILE + k] & ((1u << j) - 1u));
+                } else
+                    q = t0 + lay[LAYERS] + tb[c] + (r - LAYERS);
             }
             C.dst[q] = me;
             C.wdst[q] = C.wsrc[t0 + i];

@@ -200,7 +200,8 @@ def test_random_order_storage(P):
 def test_rebin_is_a_stable_counting_sort(P, order):
     """Rebin as a pure function of the device's own state (Q12): key = (tile, cell in tile), both bit-exact.
     Cell-major species: permutation = the stable counting sort by key.  Layered species: with r the rank of a
-    particle among those of equal key in the old order, sorted by (tile, min(r, 16), cell, r)."""
+    particle among those of equal key in the old order, layer min(r, 16); layers below 16 sorted by (rank of the cell
+    among the cells of its tile column that reach the layer, column), the tail (r >= 16) by (cell, r)."""
     cfg = small_cfg("c3", 136, 128, rebin_every=0)
     for sp in cfg["species"]:
         sp["T_keV"] *= 40.0                                   # fast particles: many tile and cell crossings
@@ -221,7 +222,20 @@ def test_rebin_is_a_stable_counting_sort(P, order):
         start = np.r_[0, np.flatnonzero(np.diff(ks)) + 1]
         rank = np.arange(ks.size) - np.repeat(start, np.diff(np.r_[start, ks.size]))      # rank in (tile, cell), old order
         tile, cell = ks // (T * T), ks % (T * T)
-        o = np.lexsort((rank, cell, np.minimum(rank, P.LAYERS), tile))
+        layer = np.minimum(rank, P.LAYERS)
+        # rank of the cell among the cells of its tile column (same tile, same iy) that hold more than `layer` particles:
+        # the members of a layer < LAYERS are one per occupied cell, so that is the rank of the particle in
+        # (tile, layer, column) by row
+        col, row = cell % T, cell // T
+        g = np.lexsort((row, col, layer, tile))
+        grp = (tile[g] * (P.LAYERS + 1) + layer[g]) * T + col[g]
+        gstart = np.r_[0, np.flatnonzero(np.diff(grp)) + 1]
+        colrank = np.empty(ks.size, np.int64)
+        colrank[g] = np.arange(ks.size) - np.repeat(gstart, np.diff(np.r_[gstart, ks.size]))
+        lay = layer < P.LAYERS
+        k1 = np.where(lay, colrank, cell)              # layers: (colrank, column); tail: (cell, rank)
+        k2 = np.where(lay, col, rank)
+        o = np.lexsort((k2, k1, layer, tile))
         return stable[o]
 
     for rounds in range(3):
