@@ -1357,9 +1357,14 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
     per = (per + 31) & ~(int64_t)31;
     const int64_t beg = min(n, wid * per), end = min(n, beg + per);
     int32_t *myhist = hist + wid * TCELLS;
-    for (int64_t i = beg + lane; i < end; i += 32) {
-        const uint2 xy = *reinterpret_cast<const uint2 *>(&C.src[t0 + i]);
-        atomicAdd(&myhist[cell_of(xy.x, xy.y)], 1);
+    for (int64_t i0 = beg + lane; i0 < end; i0 += 4 * 32) {      // four loads in flight per lane
+        uint2 xy[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+            if (i0 + 32 * u < end) xy[u] = *reinterpret_cast<const uint2 *>(&C.src[t0 + i0 + 32 * u]);
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+            if (i0 + 32 * u < end) atomicAdd(&myhist[cell_of(xy[u].x, xy[u].y)], 1);
     }
     __syncthreads();
     {   // exclusive scan over (cell, warp): thread t owns cells 4t .. 4t+3
@@ -1457,42 +1462,56 @@ __global__ void __launch_bounds__(CS_WARPS * 32) k_cellsort(const CellSortParams
         }
         __syncthreads();
     }
-    for (int64_t base = beg; base < end; base += 32) {
-        const int64_t i = base + lane;
-        const bool live = i < end;
-        PV me = {0u, 0u, 0.f, 0.f};
-        int c = TCELLS + lane;                       // dead lanes: unique keys
-        if (live) {
-            me = C.src[t0 + i];
-            c = cell_of(me.x, me.y);
-        }
-        const unsigned peers = __match_any_sync(0xffffffffu, c);
-        const int rank = __popc(peers & ((1u << lane) - 1u));
-        const int leader = __ffs(peers) - 1;
-        int b = 0;
-        if (live && lane == leader) {
-            b = myhist[c];
-            myhist[c] = b + __popc(peers);
-        }
-        b = __shfl_sync(0xffffffffu, b, leader);
-        __syncwarp();
-        if (live) {
-            int64_t q = t0 + b + rank;                 // cell-major slot
-            if (LAYERED) {
-                const int r = b + rank - cellbeg[c];   // stable rank of the particle in its cell
-                if (r < LAYERS) {
-                    const int k = cr[r * TCELLS + c], j = c & (TILE - 1);
-                    q = t0 + lay[r] + Tt[r * (TILE + 1) + k] + __popc(Mm[r * TILE + k] & ((1u << j) - 1u));
-                } else
-                    q = t0 + lay[LAYERS] + tb[c] + (r - LAYERS);
+    for (int64_t base0 = beg; base0 < end; base0 += 4 * 32) {    // the records of four batches are loaded ahead of their ranking
+        PV mv[4];
+        float wv[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int64_t i = base0 + 32 * u + lane;
+            mv[u] = PV{0u, 0u, 0.f, 0.f};
+            wv[u] = 0.f;
+            if (i < end) {
+                mv[u] = C.src[t0 + i];
+                wv[u] = C.wsrc[t0 + i];
             }
-            C.dst[q] = me;
-            C.wdst[q] = C.wsrc[t0 + i];
-            if (C.idsrc) C.iddst[q] = C.idsrc[t0 + i];
-            if (C.perm1) {
-                const int64_t old = C.perm1[t0 + i];
-                if (C.keys_out) C.keys_out[old] = tile * TCELLS + c;
-                if (C.perm_out) C.perm_out[q] = old;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int64_t base = base0 + 32 * u;
+            if (base >= end) break;                      // warp-uniform
+            const int64_t i = base + lane;
+            const bool live = i < end;
+            const PV me = mv[u];
+            int c = TCELLS + lane;                       // dead lanes: unique keys
+            if (live) c = cell_of(me.x, me.y);
+            const unsigned peers = __match_any_sync(0xffffffffu, c);
+            const int rank = __popc(peers & ((1u << lane) - 1u));
+            const int leader = __ffs(peers) - 1;
+            int b = 0;
+            if (live && lane == leader) {
+                b = myhist[c];
+                myhist[c] = b + __popc(peers);
+            }
+            b = __shfl_sync(0xffffffffu, b, leader);
+            __syncwarp();
+            if (live) {
+                int64_t q = t0 + b + rank;                 // cell-major slot
+                if (LAYERED) {
+                    const int r = b + rank - cellbeg[c];   // stable rank of the particle in its cell
+                    if (r < LAYERS) {
+                        const int k = cr[r * TCELLS + c], j = c & (TILE - 1);
+                        q = t0 + lay[r] + Tt[r * (TILE + 1) + k] + __popc(Mm[r * TILE + k] & ((1u << j) - 1u));
+                    } else
+                        q = t0 + lay[LAYERS] + tb[c] + (r - LAYERS);
+                }
+                C.dst[q] = me;
+                C.wdst[q] = wv[u];
+                if (C.idsrc) C.iddst[q] = C.idsrc[t0 + i];
+                if (C.perm1) {
+                    const int64_t old = C.perm1[t0 + i];
+                    if (C.keys_out) C.keys_out[old] = tile * TCELLS + c;
+                    if (C.perm_out) C.perm_out[q] = old;
+                }
             }
         }
     }
