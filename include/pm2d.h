@@ -62,9 +62,11 @@ enum {
     PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16) for the current E, a^n, n^n; comp 0 = x, 1 = y */
 };
 /* Storage order of a species inside a tile (as of the last rebin).  CELL_MAJOR: (cell, rank in cell), walked by
- * strip threads with register accumulation (dense species).  LAYERED: (min(rank, 16), cell, rank): 32 consecutive
- * particles lie in 32 different cells, walked one particle per thread.  AUTO: LAYERED up to 16 particles per cell on
- * average (and never for PM2D_NUMBER_WEIGHTED), else CELL_MAJOR.
+ * strip threads with register accumulation (dense species).  LAYERED: layer r < 16 holds particle number r of every
+ * cell with more than r particles, its cells ordered by (rank of the cell among those cells of its tile column iy,
+ * iy); particles of rank >= 16 follow cell-major.  32 consecutive particles then lie in 32 different cells of 32
+ * different columns (a full layer is simply row-major); walked one particle per thread.  AUTO: LAYERED up to 16
+ * particles per cell on average (and never for PM2D_NUMBER_WEIGHTED), else CELL_MAJOR.
  * RANDOM (BASELINE.json config 5, "particles stored in random order"): the loader's particles are stored in a
  * pseudo-random permutation with an explicit tile index each (+4 B per particle); no tile is staged: every particle
  * gathers from the global force grid and deposits with integer atomics on the global grids (L2).  No rebin (the
@@ -186,7 +188,8 @@ int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
  * with tile = (ix / PM2D_TILE) * ceil(ny / PM2D_TILE) + iy / PM2D_TILE; perm_out[count] (optional, host)
  * receives for every NEW slot the OLD slot it came from.  CELL_MAJOR species: the result equals a stable counting
  * sort by key.  LAYERED species: with r = the rank of a particle among those of equal key in the old order, the
- * result is sorted by (tile, min(r, 16), cell, r). */
+ * result is sorted by tile, then layer min(r, 16); inside a layer below 16 by (rank of the cell among the cells of
+ * the same tile and the same iy that hold more than r particles, in ix order; iy), inside the tail by (cell, r). */
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);

@@ -8,7 +8,8 @@
 // Data layout.  A particle is a 16-byte record PV {x, y, ux, uy} plus a weight w
 // and, between the two stages of a step, the predictor velocity u^ (float2).  Particles are stored
 // tile by tile (PM2D_TILE x PM2D_TILE cells); inside a tile, as of the last rebin, either LAYERED
-// (by rank in the cell, then by cell: 32 consecutive particles lie in 32 different cells) or
+// (by rank in the cell, then by the cell's rank in its column, then by column: 32 consecutive particles lie in 32
+// different cells of 32 different columns) or
 // CELL-MAJOR (cell_off gives every cell's run).  A position is a pair of 32-bit fixed-point numbers
 // relative to the tile's origin,
 //     xfix = (cell_rel + POS_BIAS) << 24 | frac24,
@@ -1326,10 +1327,11 @@ __device__ __forceinline__ int cell_of(uint32_t xf, uint32_t yf)
     return cx * TILE + cy;
 }
 
-// LAYERED: inside the tile the particles are ordered by (rank in their cell, cell) instead of (cell, rank): 32
-// consecutive particles then lie in 32 different, consecutive cells, which is what the thread-per-particle stage
-// kernel wants (its shared atomics spread over the banks instead of piling up on the nodes of one cell).  Ranks
-// >= LAYERS form a cell-major tail.  Shared memory: hist | cb[LAYERS][TCELLS] (uint16) | cellbeg | tb | small.
+// LAYERED: inside the tile the particles are ordered by (rank in their cell; rank of the cell among the cells of its
+// column that reach this rank; column) instead of (cell, rank): 32 consecutive particles then lie in 32 different
+// cells of 32 different columns, which is what the thread-per-particle stage kernel wants (with the deposit windows
+// on pitch 64 the bank of a node is its column: the shared atomics of a warp spread over the banks).  Ranks
+// >= LAYERS form a cell-major tail.  Shared memory: hist | cr[LAYERS][TCELLS] (uint8) | cellbeg | tb | lay | T | M.
 constexpr int LAYERS = PM2D_LAYERS;
 constexpr size_t CELLSORT_LAYERED_SMEM = (size_t)CS_WARPS * TCELLS * 4 + (size_t)LAYERS * TCELLS + (size_t)(TCELLS + 1) * 4 +
                                          (size_t)TCELLS * 4 + (LAYERS + 2) * 4 + (size_t)LAYERS * (TILE + 1) * 4 + (size_t)LAYERS * TILE * 4 + 64;
