@@ -712,7 +712,7 @@ constexpr int DPITCH = 64;
 constexpr int NNPITCH = 64;   // deposit-window pitch of the nearest-node variant
 // its force-window pitch: 64 costs a fifth resident CTA in stage A (48 registers), stage B (4 CTAs by registers) takes it
 template <int STAGE>
-struct NNFPitch { static constexpr int value = STAGE == 1 ? 64 : WPITCH; };
+struct NNFPitch { static constexpr int value = WPITCH; };
 
 template <int SHAPE, int STAGE, int QMASK>
 __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
@@ -803,7 +803,7 @@ __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, 
 // sorted into: species that hardly move between rebins, e.g. ions); else the 3 x 3 nodes around the nearest node
 // on the odd-pitch windows (process_direct), whose conflicts do not depend on the drift.
 template <int SHAPE, int STAGE, int QMASK, bool ANCH>
-__global__ void __launch_bounds__(256, 4) k_stage_direct(const PartParams P)
+__global__ void __launch_bounds__(256, ANCH ? 4 : 5) k_stage_direct(const PartParams P)
 {
     constexpr int NT = 256;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
