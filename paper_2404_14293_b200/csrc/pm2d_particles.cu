@@ -709,6 +709,7 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 // and with a window pitch that is a multiple of 32 words the bank is the column, whatever the row.  12 nodes: 12
 // LDS.64 for the gather, 12 x 3 ATOMS for the deposit, one wavefront each.
 constexpr int DPITCH = 64;
+constexpr int DFPITCH = 48;   // force window of the anchored variant: 48 float2 = 96 words, a multiple of 32 as well
 constexpr int NNPITCH = 64;   // deposit-window pitch of the nearest-node variant
 // its force-window pitch: 64 costs a fifth resident CTA in stage A (48 registers), stage B (4 CTAs by registers) takes it
 template <int STAGE>
@@ -738,15 +739,15 @@ __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, 
         if (cx - 1 < -HALO || cx + 1 > TILE + HALO || cyc - 1 < -HALO || cyc + 2 > TILE + HALO) return false;
         weights3<SHAPE>(dx_, P, Wx);
         weights4<SHAPE>((int)(yg & POS_FRAC_MASK), P, Wy);
-        const float2 *fw = Fs + (cx - 1 + HALO) * DPITCH + (cyc - 1 + HALO);
+        const float2 *fw = Fs + (cx - 1 + HALO) * DFPITCH + (cyc - 1 + HALO);
         float2 f = make_float2(0.f, 0.f);
         const float2 wy0 = dup2(Wy[0]), wy1 = dup2(Wy[1]), wy2 = dup2(Wy[2]), wy3 = dup2(Wy[3]);
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            float2 sa = __fmul2_rn(wy0, fw[a * DPITCH]);
-            sa = __ffma2_rn(wy1, fw[a * DPITCH + 1], sa);
-            sa = __ffma2_rn(wy2, fw[a * DPITCH + 2], sa);
-            sa = __ffma2_rn(wy3, fw[a * DPITCH + 3], sa);
+            float2 sa = __fmul2_rn(wy0, fw[a * DFPITCH]);
+            sa = __ffma2_rn(wy1, fw[a * DFPITCH + 1], sa);
+            sa = __ffma2_rn(wy2, fw[a * DFPITCH + 2], sa);
+            sa = __ffma2_rn(wy3, fw[a * DFPITCH + 3], sa);
             f = __ffma2_rn(dup2(Wx[a]), sa, f);
         }
         if (STAGE == 0) {
@@ -803,12 +804,12 @@ __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, 
 // sorted into: species that hardly move between rebins, e.g. ions); else the 3 x 3 nodes around the nearest node
 // on the odd-pitch windows (process_direct), whose conflicts do not depend on the drift.
 template <int SHAPE, int STAGE, int QMASK, bool ANCH>
-__global__ void __launch_bounds__(256, ANCH ? 4 : 5) k_stage_direct(const PartParams P)
+__global__ void __launch_bounds__(256, 5) k_stage_direct(const PartParams P)
 {
     constexpr int NT = 256;
     constexpr int NQ = (QMASK & 2) ? 3 : 1;
     constexpr int PITCH = ANCH ? DPITCH : NNPITCH;
-    constexpr int FPITCH = ANCH ? DPITCH : NNFPitch<STAGE>::value;
+    constexpr int FPITCH = ANCH ? DFPITCH : NNFPitch<STAGE>::value;
     extern __shared__ int32_t direct_smem[];
     int32_t *dep = direct_smem;                                                      // [NQ][WIN][PITCH]
     float2 *Fs = reinterpret_cast<float2 *>(direct_smem + ((NQ * WIN * PITCH + 1) & ~1));   // [WIN][PITCH]
@@ -845,7 +846,7 @@ template <int STAGE, int QMASK, bool ANCH>
 constexpr size_t direct_smem_bytes()
 {
     return (size_t)(((((QMASK & 2) ? 3 : 1) * WIN * (ANCH ? DPITCH : NNPITCH)) + 1) & ~1) * 4 +
-           (STAGE < 2 ? (size_t)WIN * (ANCH ? DPITCH : NNFPitch<STAGE>::value) * 8 : 0);
+           (STAGE < 2 ? (size_t)WIN * (ANCH ? DFPITCH : NNFPitch<STAGE>::value) * 8 : 0);
 }
 
 // the deferred particles of k_stage: same arithmetic, global grids only
