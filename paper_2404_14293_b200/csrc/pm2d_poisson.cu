@@ -297,7 +297,7 @@ struct ForceOut {
 // MODE 2: Z = ehx + i ehy -> F_s of every mobile species (ForceOut)
 // NS: species slots of the force epilogue (2 covers electrons + one ion species with fewer registers)
 template <int MODE, int BIG, int NS = PM2D_MAX_SPECIES, int NY = 0>
-__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <= 2 ? 3 : 2) : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? (NS <= 2 ? 4 : 2) : 1) k_ifft(const float2 *__restrict__ hx, const float2 *__restrict__ hy,
                                                       const float2 *__restrict__ tw, float2 *__restrict__ Enode,
                                                       float *__restrict__ phi, int ny_, int LP, const ForceOut FO)
 {
