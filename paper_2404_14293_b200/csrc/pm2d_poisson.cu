@@ -219,7 +219,7 @@ __device__ __forceinline__ void fft16_inplace(float2 *buf, const float2 *__restr
 // Two real rows per complex transform: z = rho_a + i rho_b, then rho^_a = (Z_l + conj Z_{n-l}) / 2 and
 // rho^_b = (Z_l - conj Z_{n-l}) / 2i.  BIG: register-blocked FFT on the padded buffer (ny >= 512).
 template <int BIG, int NY = 0>
-__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 3 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
+__global__ void __launch_bounds__(BIG == 2 ? 512 : FFT_THREADS, BIG == 1 ? 4 : 1) k_fft_rho(RhoSrc S, const float2 *__restrict__ tw,
                                                                      float2 *__restrict__ rho_hat, int nx, int ny_, int LP)
 {
     extern __shared__ float2 buf[];
