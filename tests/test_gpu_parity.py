@@ -438,6 +438,49 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     sim.close()
 
 
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_full_size_c4_c5_sampled_deposit_parity(P, name):
+    """BASELINE.json configs 4 (16384 x 8192, 403 M particles, Gaussian beam, ny = 8192 FFT path) and 5 (4096 x 4096,
+    9.4e8 number-weighted electrons in a filament, cell-major order + strip kernel) at full size, in the launch
+    configuration bench.py times.  After 3 steps: counts and charge conserved, and on a sample of the grid -- 17 node
+    rows in the middle of the box, every column -- the deposited n, Px, Py equal the oracle's deposit of the device's
+    own particles.  The storage is tile-major and no rebin has run, so the two tile rows around the sample are one
+    contiguous range of slots; the sampled rows receive deposits only from particles within 1.5 cells, all of which
+    are in that range (the particles drift less than a cell in 3 steps)."""
+    cfg = I.config(name)
+    g = cfg["grid"]
+    nx, ny = g["nx"], g["ny"]
+    T = P.TILE
+    sim = P.PM2D(cfg, eager_moments=1)
+    d0 = sim.diagnostics()
+    sim.step(3)
+    d1 = sim.diagnostics()
+    mobile = [s for s, sp in enumerate(cfg["species"]) if sp["mobile"]]
+    for s in mobile:
+        assert d1["count"][s] == d0["count"][s] == I.n_particles(cfg, s)
+        assert d1["charge"][s] == pytest.approx(d0["charge"][s], rel=1e-6)
+    x0 = (nx // T // 2) * T                                        # first cell row of the two tile rows taken
+    sub = oracle.make_grid(4 * T, ny, g["dx"], g["dy"], g["dt"])   # cells x0 - T .. x0 + 3 T: no wall near the sample
+    for s in mobile:
+        sp = cfg["species"][s]
+        if sp["load"] == I.NUMBER_WEIGHTED:
+            cc = I.cell_counts(cfg, s)
+            first, count = int(cc[:x0].sum()), int(cc[x0:x0 + 2 * T].sum())
+        else:
+            ppc = sp["ppc_x"] * sp["ppc_y"]
+            first, count = x0 * ny * ppc, 2 * T * ny * ppc
+        parts = sim.get_particles(s, first=first, count=count)
+        assert parts["ix"].size == count
+        assert x0 - 4 <= parts["ix"].min() and parts["ix"].max() < x0 + 2 * T + 4          # those two tile rows, drifted a little
+        n, px, py = oracle.deposit(sub, sp["shape"], sp["DD"], parts["ix"] - (x0 - T) + parts["fx"].astype(np.float64),
+                                   parts["iy"] + parts["fy"].astype(np.float64), parts["ux"], parts["uy"], parts["w"])
+        lo = x0 + T - 8                                             # node rows lo .. lo + 16 straddle the two tile rows
+        for moment, ref in ((P.MOMENT_N, n), (P.MOMENT_PX, px), (P.MOMENT_PY, py)):
+            got = sim.get_moments(s, moment, window=(lo, lo + 17, 0, ny))
+            assert rel_l2(got, ref[lo - (x0 - T):lo - (x0 - T) + 17]) < 1e-5, (name, s, moment)
+    sim.close()
+
+
 def test_full_length_c2_run_stays_bounded(P):
     """BASELINE.json config 2 over its full 1000 steps (Q20: with an edge taper that ran to zero, particles
     of the outermost cells were kicked to |u| >> 1 by the pressure term around step 378 and the run ended in
