@@ -711,9 +711,10 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
 constexpr int DPITCH = 64;
 constexpr int DFPITCH = 48;   // force window of the anchored variant: 48 float2 = 96 words, a multiple of 32 as well
 constexpr int NNPITCH = 64;   // deposit-window pitch of the nearest-node variant
-// its force-window pitch: 64 costs a fifth resident CTA in stage A (48 registers), stage B (4 CTAs by registers) takes it
+// its force-window pitch: 48 float2 = 96 words (the 16 lanes of an LDS.64 half-warp fall on 16 different bank pairs
+// when they hold 16 consecutive columns); 42.6 KB per CTA with the deposit windows: five resident CTAs
 template <int STAGE>
-struct NNFPitch { static constexpr int value = WPITCH; };
+struct NNFPitch { static constexpr int value = 48; };
 
 template <int SHAPE, int STAGE, int QMASK>
 __device__ __forceinline__ bool direct_particle(const PartParams &P, int64_t p, int gx0, int gy0, const float2 *Fs, int32_t *dep)
