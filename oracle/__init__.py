@@ -30,7 +30,7 @@ def build(force: bool = False) -> str:
 
 
 class _Grid(C.Structure):
-    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("pad_", C.c_int32),
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("subcycle", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -48,7 +48,7 @@ class _Species(C.Structure):
 
 class _Laser(C.Structure):
     _fields_ = [("a0", C.c_double), ("omega", C.c_double), ("y0", C.c_double), ("w0", C.c_double),
-                ("t_rise", C.c_double), ("comp", C.c_int32), ("pad_", C.c_int32)]
+                ("t_rise", C.c_double), ("alpha", C.c_double), ("comp", C.c_int32), ("pad_", C.c_int32)]
 
 
 class _State(C.Structure):
@@ -74,7 +74,7 @@ def lib():
         L.orc_gather.restype = None
         L.orc_gather.argtypes = [C.POINTER(_Grid), C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
         L.orc_a_inc.restype = C.c_double
-        L.orc_a_inc.argtypes = [C.POINTER(_Laser), C.c_double, C.c_double, C.c_double]
+        L.orc_a_inc.argtypes = [C.POINTER(_Laser), C.c_double, C.c_double, C.c_double, C.c_double]
         L.orc_field_step.restype = None
         L.orc_field_step.argtypes = [C.POINTER(_State), _dp, C.c_double]
         L.orc_fft.restype = None
@@ -130,8 +130,8 @@ def weights_1d(shape: int, DD: float, xp: float):
     return first, W[: cnt.value]
 
 
-def make_grid(nx, ny, dx, dy, dt, ncomp=1):
-    return _Grid(nx, ny, ncomp, 0, dx, dy, dt)
+def make_grid(nx, ny, dx, dy, dt, ncomp=1, subcycle=1):
+    return _Grid(nx, ny, ncomp, subcycle, dx, dy, dt)
 
 
 def deposit(g: _Grid, shape, DD, X, Y, ux, uy, w):
@@ -190,10 +190,10 @@ def corrector(dt, h, x, u, uh, Fh):
     return un.value, xn.value
 
 
-def a_inc(laser: dict, x, y, t):
+def a_inc(laser: dict, x, y, t, Ly=1.0):
     L = _Laser(laser["a0"], laser.get("omega", 1.0), laser.get("y0", 0.0), laser.get("w0", 0.0),
-               laser.get("t_rise", 0.0), laser.get("comp", 0), 0)
-    return lib().orc_a_inc(C.byref(L), x, y, t)
+               laser.get("t_rise", 0.0), laser.get("alpha", 0.0), laser.get("comp", 0), 0)
+    return lib().orc_a_inc(C.byref(L), x, y, t, Ly)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -202,11 +202,12 @@ class Oracle:
 
     species: list of dicts with keys mass, sign, T_keV, C (pressure_coeff), shape, DD, mobile and
     particle arrays X, Y (cell units), ux, uy, w; an immobile species may instead give ``n_fixed``
-    (nodal density, shape (nx+1, ny)).  lasers: list of dicts (a0, omega, y0, w0, t_rise, comp).
+    (nodal density, shape (nx+1, ny)).  lasers: list of dicts (a0, omega, y0, w0, t_rise, alpha [rad], comp).
+    subcycle: wave-equation steps of dt per particle step (Q21).
     """
 
-    def __init__(self, nx, ny, dx, dy, dt, species, lasers=(), ncomp=1):
-        self.g = make_grid(nx, ny, dx, dy, dt, ncomp)
+    def __init__(self, nx, ny, dx, dy, dt, species, lasers=(), ncomp=1, subcycle=1):
+        self.g = make_grid(nx, ny, dx, dy, dt, ncomp, subcycle)
         self.nn = nn = (nx + 1) * ny
         self.a = [np.zeros(ncomp * nn) for _ in range(3)]       # new, now, old
         self.rho, self.phi = np.zeros(nn), np.zeros(nn)
@@ -241,7 +242,7 @@ class Oracle:
         self._las = (_Laser * max(len(lasers), 1))()
         for k, l in enumerate(lasers):
             self._las[k] = _Laser(l["a0"], l.get("omega", 1.0), l.get("y0", 0.0), l.get("w0", 0.0),
-                                  l.get("t_rise", 0.0), l.get("comp", 0), 0)
+                                  l.get("t_rise", 0.0), l.get("alpha", 0.0), l.get("comp", 0), 0)
         self.st = _State(self.g, len(species), len(lasers), self._sp, self._las,
                          _p(self.a[0]), _p(self.a[1]), _p(self.a[2]),
                          _p(self.rho), _p(self.phi), _p(self.Ex), _p(self.Ey), 0)

@@ -31,8 +31,8 @@ enum { ORC_CIC = 0, ORC_TSC = 1, ORC_SINE = 2 };
 typedef struct {
     int32_t nx, ny;      /* cells; nodes are (nx+1) x ny */
     int32_t ncomp;       /* active components of a (1..3) */
-    int32_t pad_;
-    double dx, dy, dt;
+    int32_t subcycle;    /* S: the particle step is S wave-equation steps long (Q21); 0, 1 = none */
+    double dx, dy, dt;   /* dt: time step of the wave equation */
 } orc_grid;
 
 typedef struct {
@@ -53,6 +53,7 @@ typedef struct {
 
 typedef struct {
     double a0, omega, y0, w0, t_rise;
+    double alpha;        /* angle of incidence in radians, Eq. 5 (Q22) */
     int32_t comp, pad_;
 } orc_laser;
 
@@ -177,23 +178,40 @@ void orc_gather(const orc_grid *g, int shape, double DD, double Xp, double Yp, c
     *fy = sy;
 }
 
-/* Incident wave, Eq. 4 at normal incidence: a = a0 env(y) cos(omega t - k x), k = omega
- * in vacuum, time in T0 and x in lambda0 so the phase is 2 pi omega (t - x).  Turn-on (Q14):
- * ramp(tau) = sin^2(pi tau / (2 t_rise)) of the retarded time tau = t - x; t_rise = 0 is the
- * paper's literal substitution.  w0 <= 0: plane wave.                                  */
-double orc_a_inc(const orc_laser *L, double x, double y, double t)
+/* Incident wave, Eq. 4: a = a0 env(y) cos(omega t - k x), k = omega in vacuum, time in
+ * T0 and x in lambda0 so the phase is 2 pi omega (t - x).  Turn-on (Q14): ramp(tau) =
+ * sin^2(pi tau / (2 t_rise)) of the retarded time tau = t - x; t_rise = 0 is the paper's literal
+ * substitution.  w0 <= 0: plane wave.
+ * Oblique incidence, Eq. 5: (x, y) here are the box coordinates (the paper's x', y');
+ * the beam coordinates that go into Eq. 4 are  xb = x cos(alpha) - y' sin(alpha),
+ * yb = x sin(alpha) + y' cos(alpha), with y' measured from the beam centre y0 so that y0 stays
+ * the centre of the beam on the boundary, and taken at the nearest periodic image (y is periodic
+ * with period Ly) -- Q22.  The turn-on front is the plane t - xb = (Ly/2)|sin(alpha)|, the earliest
+ * one that leaves the whole box field-free at t = 0 (the boundary reaches back to xb =
+ * -(Ly/2)|sin(alpha)|); the carrier keeps the phase of Eq. 4.  alpha = 0 is the normal incidence of
+ * P:L93, untouched.                                                                              */
+double orc_a_inc(const orc_laser *L, double x, double y, double t, double Ly)
 {
-    double tau = t - x, env = 1.0, ramp = 1.0;
+    double xb = x, yb = y - L->y0, tau, phase, env = 1.0, ramp = 1.0, lead = 0.0;
+    if (L->alpha != 0.0) {
+        double d = y - L->y0;
+        d -= Ly * floor(d / Ly + 0.5);
+        xb = x * cos(L->alpha) - d * sin(L->alpha);       /* Eq. 5 */
+        yb = x * sin(L->alpha) + d * cos(L->alpha);
+        lead = 0.5 * Ly * fabs(sin(L->alpha));
+    }
+    phase = t - xb;
+    tau = phase - lead;
     if (tau <= 0.0) return 0.0;
     if (L->w0 > 0.0) {
-        double r = (y - L->y0) / L->w0;
+        double r = yb / L->w0;
         env = exp(-r * r);
     }
     if (L->t_rise > 0.0 && tau < L->t_rise) {
         double s = sin(0.5 * ORC_PI * tau / L->t_rise);
         ramp = s * s;
     }
-    return L->a0 * env * ramp * cos(2.0 * ORC_PI * L->omega * tau);
+    return L->a0 * env * ramp * cos(2.0 * ORC_PI * L->omega * phase);
 }
 
 static double a_inc_sum(const orc_state *S, int comp, double x, double y, double t)
@@ -201,7 +219,7 @@ static double a_inc_sum(const orc_state *S, int comp, double x, double y, double
     double s = 0.0;
     int l;
     for (l = 0; l < S->nlaser; l++)
-        if (S->laser[l].comp == comp) s += orc_a_inc(&S->laser[l], x, y, t);
+        if (S->laser[l].comp == comp) s += orc_a_inc(&S->laser[l], x, y, t, S->g.ny * S->g.dy);
     return s;
 }
 
@@ -491,10 +509,13 @@ void orc_step(orc_state *S)
     const orc_grid *g = &S->g;
     const int nx = g->nx, ny = g->ny;
     const int64_t nn = (int64_t)(nx + 1) * ny;
-    const double dt = g->dt, t_now = S->step * g->dt;
+    /* Q21: the particles advance with dt = S dt_wave; the wave equation takes S steps of
+     * dt_wave per particle step with the electron density of item (1) held fixed                 */
+    const int nsub = g->subcycle > 1 ? g->subcycle : 1;
+    const double dt = nsub * g->dt;
     const double hx = dt / (2.0 * g->dx), hy = dt / (2.0 * g->dy);   /* cells per unit u */
-    double *Xh = NULL, *Yh = NULL, *ne;
-    int s;
+    double *Xh = NULL, *Yh = NULL, *ne, *a_n;
+    int s, sub;
     int64_t p, k;
 
     /* electron density for the wave source: sum over negative species */
@@ -503,8 +524,17 @@ void orc_step(orc_state *S)
         if (S->sp[s].sign < 0)
             for (k = 0; k < nn; k++) ne[k] += S->sp[s].n[k];
 
-    /* (2) a^{n+1} from a^n, a^{n-1}, n_e^n (Eq. 6, 8); E^n from n_i^n - n_e^n (Eqs. 9-11) */
-    orc_field_step(S, ne, t_now);
+    /* (2) a^{n+1} from a^n, a^{n-1}, n_e^n (Eq. 6, 8): S wave steps, a^n kept for item (3);
+     * E^n from n_i^n - n_e^n (Eqs. 9-11) */
+    a_n = (double *)malloc(sizeof(double) * g->ncomp * nn);
+    memcpy(a_n, S->a_now, sizeof(double) * g->ncomp * nn);
+    for (sub = 0; sub < nsub; sub++) {
+        orc_field_step(S, ne, (double)(S->step * nsub + sub) * g->dt);
+        if (sub + 1 < nsub) {
+            double *t = S->a_old;
+            S->a_old = S->a_now; S->a_now = S->a_new; S->a_new = t;
+        }
+    }
     charge_density(S, S->rho);
     orc_poisson(g, S->rho, S->phi, 0);
     orc_efield(g, S->phi, S->Ex, S->Ey);
@@ -513,8 +543,9 @@ void orc_step(orc_state *S)
     for (s = 0; s < S->nsp; s++) {
         orc_species *q = &S->sp[s];
         if (!q->mobile) continue;
-        orc_force(g, q, S->a_now, S->Ex, S->Ey, q->Fx, q->Fy);
+        orc_force(g, q, a_n, S->Ex, S->Ey, q->Fx, q->Fy);
     }
+    free(a_n);
     for (s = 0; s < S->nsp; s++) {
         orc_species *q = &S->sp[s];
         if (!q->mobile) continue;

@@ -1,0 +1,167 @@
+"""Pins of the S§8(f).1 widening of the oracle: oblique incidence (Eq. 5; Q22) and particle
+sub-cycling (Q21).  Closed forms and invariants only; no GPU."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+
+
+def _vacuum_oracle(nx, ny, dx, dt, lasers, subcycle=1):
+    sp = [dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, shape=oracle.CIC, DD=1.0, n_fixed=np.zeros((nx + 1, ny)))]
+    return oracle.Oracle(nx, ny, dx, dx, dt, sp, lasers, subcycle=subcycle)
+
+
+# ---- Eq. 5 -------------------------------------------------------------------------------------------
+def test_P15_eq5_rotation_worked_values():
+    """Eq. 5 substituted into Eq. 4 by hand: box point (x', y') -> beam point (x, y), y' from the beam centre."""
+    al = math.radians(15.0)
+    las = dict(a0=0.008, w0=30.0, y0=50.0, t_rise=0.0, omega=1.0 / 0.9995, alpha=al)     # beam 2 of P:L380
+    Ly = 400.0
+    lead = 0.5 * Ly * math.sin(al)            # turn-on front (Q22): 51.76 T0 here
+    hit = 0
+    for xq, yq, t in ((0.0, 50.0, 3.0), (0.0, 50.0, 53.0), (0.0, 62.0, 60.0), (0.05, 31.5, 80.0), (0.05, 50.0 - 7.25, 47.3),
+                      (0.05, 50.0 - 7.25, 97.3)):
+        d = yq - 50.0
+        xb = xq * math.cos(al) - d * math.sin(al)
+        yb = xq * math.sin(al) + d * math.cos(al)
+        on = t - xb > lead
+        hit += on
+        ref = 0.008 * math.exp(-(yb / 30.0) ** 2) * math.cos(2 * math.pi / 0.9995 * (t - xb)) if on else 0.0
+        assert oracle.a_inc(las, xq, yq, t, Ly) == pytest.approx(ref, abs=1e-15)
+    assert hit == 4
+    # nearest periodic image of the beam centre: y' and y' + Ly are the same boundary point
+    assert oracle.a_inc(las, 0.0, 60.0 - Ly, 70.0, Ly) == pytest.approx(oracle.a_inc(las, 0.0, 60.0, 70.0, Ly), abs=1e-15)
+    assert oracle.a_inc(las, 0.0, 60.0, 70.0, Ly) != 0.0
+    # alpha = 0 is Eq. 4 at normal incidence, whatever Ly
+    l0 = dict(las, alpha=0.0)
+    assert oracle.a_inc(l0, 0.05, 62.0, 40.0, Ly) == oracle.a_inc(l0, 0.05, 62.0, 40.0, 1.0)
+
+
+def test_P15_oblique_plane_wave_fills_vacuum_box():
+    """A plane wave injected at an angle that fits the periodic box (omega sin(alpha) Ly = m) fills a vacuum box
+    with a0 cos(2 pi (t - x' cos(alpha) + y' sin(alpha))): amplitude a0, transverse mode exactly -m (the sign of
+    Eq. 5 as printed: the beam axis is (cos alpha, -sin alpha) in box coordinates), longitudinal wavenumber
+    cos(alpha) up to the dispersion of the stencil, nothing coming back from either wall."""
+    nx, ny, dx, dt, a0, m = 240, 256, 0.05, 0.035, 0.01, 3
+    Ly = ny * dx
+    al = math.asin(m / Ly)
+    o = _vacuum_oracle(nx, ny, dx, dt, [dict(a0=a0, t_rise=3.0, alpha=al)])
+    nsteps = int(26.0 / dt)
+    o.step(nsteps)
+    a = o.a_now[0]                                   # (nx+1, ny)
+    A = np.fft.fft(a, axis=1) / ny                   # transverse modes, row by row
+    rows = slice(10, nx - 10)
+    power = (np.abs(A[rows]) ** 2).sum(axis=0)
+    # a real field cos(.. + 2 pi m y / Ly) has modes +m and -m of equal size; the direction sits in the x phase
+    assert set(np.argsort(power)[-2:]) == {m, ny - m}
+    assert power[[m, ny - m]].sum() / power.sum() > 0.9995
+    # a = Re[a0 exp(i(2 pi t - kx x' + 2 pi m y'/Ly))]: the coefficient of exp(+i 2 pi m y'/Ly) is (a0/2) exp(i(2 pi t - kx x'))
+    c = A[:, m]
+    assert np.abs(2 * np.abs(c[rows]) / a0 - 1.0).max() < 0.015
+    ph = np.unwrap(np.angle(c[rows]))
+    kx = -np.polyfit(np.arange(nx + 1)[rows] * dx, ph, 1)[0] / (2 * math.pi)
+    # discrete dispersion of Eq. 6 in vacuum: sin^2(pi dt)/dt^2 = sin^2(kx' dx/2)/dx^2 + sin^2(ky' dx/2)/dx^2
+    ky = m / Ly
+    kx_d = math.asin(math.sqrt((math.sin(math.pi * dt) / dt) ** 2 - (math.sin(math.pi * ky * dx) / dx) ** 2) * dx) / (math.pi * dx)
+    assert kx == pytest.approx(kx_d, rel=2e-3)
+    assert kx == pytest.approx(math.cos(al), rel=1e-2)
+    # with the opposite sign of alpha the wave goes the other way in y: conj pattern, i.e. the phase of mode +m
+    # now decreases with -x'... checked through the mode that carries exp(-i kx x')
+    o2 = _vacuum_oracle(nx, ny, dx, dt, [dict(a0=a0, t_rise=3.0, alpha=-al)])
+    o2.step(nsteps)
+    c2 = (np.fft.fft(o2.a_now[0], axis=1) / ny)[:, ny - m]
+    ph2 = np.unwrap(np.angle(c2[rows]))
+    assert -np.polyfit(np.arange(nx + 1)[rows] * dx, ph2, 1)[0] / (2 * math.pi) == pytest.approx(kx_d, rel=2e-3)
+
+
+def test_P15_oblique_gaussian_beam_axis():
+    """The centre of a Gaussian beam injected at alpha moves along (cos alpha, -sin alpha): at depth x' the
+    centroid of the cycle-averaged a^2 sits at y0 - x' tan(alpha)."""
+    nx, ny, dx, dt = 200, 256, 0.05, 0.035
+    al, y0, w0 = math.radians(15.0), 7.0, 1.5
+    o = _vacuum_oracle(nx, ny, dx, dt, [dict(a0=0.01, t_rise=2.0, alpha=al, y0=y0, w0=w0)])
+    o.step(int(16.0 / dt))
+    acc = np.zeros((nx + 1, ny))
+    per = int(round(1.0 / dt))
+    for _ in range(per):
+        o.step()
+        acc += o.a_now[0] ** 2
+    y = np.arange(ny) * dx
+    for i in (20, 100, 180):
+        cen = (acc[i] * y).sum() / acc[i].sum()
+        shift = i * dx * math.tan(al)
+        # one cell + 4 % of the shift: Eq. 4 prescribes a flat phase front on a boundary that cuts the beam obliquely,
+        # so a beam this narrow (w0 = 1.5 lambda0) steers slightly; a wrong sign or a sin/cos swap is off by > 100 %
+        assert cen == pytest.approx(y0 - shift, abs=0.05 + 0.04 * shift)
+    # width across the beam axis stays w0 (Rayleigh length pi w0^2 = 7 lambda0: mild spreading allowed)
+    i = 20
+    var = (acc[i] * (y - (acc[i] * y).sum() / acc[i].sum()) ** 2).sum() / acc[i].sum()
+    # a^2 ~ exp(-2 yb^2 / w0^2), yb = (y' - centre) cos(alpha)  =>  var(y') = w0^2 / (4 cos^2 alpha)
+    assert math.sqrt(var) == pytest.approx(w0 / (2 * math.cos(al)), rel=0.05)
+
+
+# ---- sub-cycling ----------------------------------------------------------------------------------------
+def test_P16_subcycled_wave_steps_equal_plain_steps_without_plasma():
+    """Without plasma the particle step plays no part: N particle steps of S wave steps are S N plain steps,
+    bit for bit (pins the time of every sub-step that goes into the boundary condition)."""
+    nx, ny, dx, dt, S = 96, 16, 0.05, 0.035, 5
+    las = [dict(a0=0.02, t_rise=1.0, w0=0.3, y0=0.4)]
+    o1 = _vacuum_oracle(nx, ny, dx, dt, las)
+    o5 = _vacuum_oracle(nx, ny, dx, dt, las, subcycle=S)
+    o1.step(12 * S)
+    o5.step(12)
+    assert np.abs(o1.a_now[0]).max() > 0.01
+    assert np.array_equal(o1.a_now[0], o5.a_now[0])
+    assert np.array_equal(o1.a_old[0], o5.a_old[0])
+
+
+def test_P16_subcycled_free_streaming_and_constant_force():
+    """A neutral pressure-free particle moves by u S dt per step (exact); Heun's step is exact for a constant
+    force, so a uniform E = -grad(phi) cannot be built here -- the free flight pins dt_p = S dt in Eq. 17/19."""
+    nx, ny, dx, dt, S = 32, 8, 0.05, 0.035, 5
+    X, Y = np.array([10.25]), np.array([3.5])
+    sp = [dict(sign=0, mass=1.0, T_keV=0.0, C=0.0, shape=oracle.SINE, DD=1.9, mobile=1, X=X, Y=Y,
+               ux=np.array([0.02]), uy=np.array([-0.03]), w=np.array([0.1]))]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp, subcycle=S)
+    o.step(7)
+    assert o.sp[0]["X"][0] == pytest.approx(10.25 + 0.02 * 7 * S * dt / dx, abs=1e-12)
+    assert o.sp[0]["Y"][0] == pytest.approx(3.5 - 0.03 * 7 * S * dt / dx, abs=1e-12)
+
+
+def test_P16_subcycled_plasma_oscillation_period():
+    """Cold plasma oscillation with S = 5: the period, on the time axis t = step S dt, is 1/sqrt(n0) T0 up to the
+    phase error of Heun's method at omega_pe dt_p (the same pin as P11 at five times the step)."""
+    nx, ny, dx, dt, S, n0, px = 64, 2, 0.05, 0.035, 5, 0.1, 8
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    xs = (np.arange(nx * px) + 0.5) / px
+    X0, Y0 = [a.ravel() for a in np.meshgrid(xs, np.arange(ny) + 0.5, indexing="ij")]
+    w = np.full(X0.size, n0 / px)
+    n_bg, _, _ = oracle.deposit(g, oracle.TSC, 2.0, X0, Y0, 0 * X0, 0 * X0, w)
+    K = 2 * math.pi * 2 / nx
+    X = X0 + 0.02 * np.sin(K * X0)
+    sp = [dict(sign=-1, mass=1.0, T_keV=0.0, C=0.0, shape=oracle.TSC, DD=2.0, mobile=1, X=X, Y=Y0, ux=0 * X, uy=0 * X, w=w),
+          dict(sign=1, mass=1836.0, T_keV=0.0, mobile=0, shape=oracle.TSC, DD=2.0, n_fixed=n_bg)]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp, subcycle=S)
+    i = np.arange(nx + 1)[:, None]
+    amp, t = [], []
+    for n in range(120):
+        amp.append((o.moment(0, "n") * np.cos(K * i)).sum())
+        t.append(n * S * dt)
+        o.step()
+    y = np.asarray(amp) - np.mean(amp)
+    s = np.sign(y)
+    idx = np.where(s[:-1] * s[1:] < 0)[0]
+    t = np.asarray(t)
+    tc = t[idx] - y[idx] * (t[idx + 1] - t[idx]) / (y[idx + 1] - y[idx])
+    period = 2.0 * (tc[-1] - tc[0]) / (len(tc) - 1)
+    th = 2 * math.pi * math.sqrt(n0) * S * dt                      # omega_pe dt_p
+    # one step of Eqs. 17, 19 on x'' = -omega^2 x is the matrix [[1 - th^2/2 + th^4/8, th - th^3/4], [-th + th^3/4,
+    # 1 - th^2/2]] in (x, u/omega): phase per step phi = arccos(trace / (2 sqrt(det))) = th (1 - th^2/12 + ...)
+    tr, det = 2 - th * th + th ** 4 / 8, 1 - th ** 4 / 8
+    phi = math.acos(tr / (2 * math.sqrt(det)))
+    assert phi / th == pytest.approx(1 - th * th / 12, abs=2e-4)
+    # the finite-grid factors of mode 2 on 64 cells (TSC smoothing, differenced E) lengthen the period by 0.6 %
+    assert period == pytest.approx(1.0 / math.sqrt(n0) * th / phi, rel=0.01)
+    # a push with dt instead of S dt would give a period S times longer on this time axis
