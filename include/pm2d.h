@@ -91,8 +91,12 @@ typedef struct {
                               asks (nothing in the step reads them)                                   */
     int32_t track_ids;     /* 1: carry a particle id through the rebin (tests); costs 8 B/particle   */
     int32_t particle_order; /* PM2D_ORDER_*: storage order inside a tile and the stage kernel that goes with it */
-    int32_t pad_;
-    double dx, dy, dt;     /* lambda0, lambda0, T0; dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1 */
+    int32_t subcycle;      /* S in 0..16 (0, 1 = none): the particle step is S wave-equation steps long, "the time step
+                              for updating the particle motion is five times larger" (Q21).
+                              One pm2d_step is then S steps of Eq. 6/8 with n_e held, and Eqs. 17/19 with S*dt;
+                              S*dt/min(dx,dy) <= 4                                                    */
+    double dx, dy, dt;     /* lambda0, lambda0, T0; dt = step of the wave equation,
+                              dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1                     */
 } pm2d_grid;
 
 typedef struct {
@@ -121,6 +125,10 @@ typedef struct {
     double a0, omega;      /* amplitude; frequency in omega0 (Eq. 4)                        */
     double y0, w0;         /* beam centre and width in lambda0; w0 <= 0: plane wave                   */
     double t_rise;         /* sin^2 turn-on over t_rise (Q14); 0: none                                */
+    double alpha;          /* angle of incidence in radians, |alpha| <= 1 (Eq. 5; Q22): the
+                              beam axis is (cos alpha, -sin alpha) in box coordinates and crosses the boundary at y0.
+                              A plane wave (w0 <= 0) at alpha != 0 must fit the periodic box:
+                              omega*sin(alpha)*Ly an integer, else PM2D_EINVAL                       */
     int32_t comp;          /* component of a that carries the beam                                    */
     int32_t pad_;
 } pm2d_laser;

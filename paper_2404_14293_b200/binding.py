@@ -26,7 +26,7 @@ PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("rebin_every", C.c_int32),
-                ("eager_moments", C.c_int32), ("track_ids", C.c_int32), ("particle_order", C.c_int32), ("pad_", C.c_int32),
+                ("eager_moments", C.c_int32), ("track_ids", C.c_int32), ("particle_order", C.c_int32), ("subcycle", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -42,7 +42,7 @@ class Profile(C.Structure):
 
 class Laser(C.Structure):
     _fields_ = [("a0", C.c_double), ("omega", C.c_double), ("y0", C.c_double), ("w0", C.c_double),
-                ("t_rise", C.c_double), ("comp", C.c_int32), ("pad_", C.c_int32)]
+                ("t_rise", C.c_double), ("alpha", C.c_double), ("comp", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Diag(C.Structure):
@@ -122,7 +122,7 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, part
     """Translate a pm2d_inputs-style config dict into the C structs."""
     g = cfg["grid"]
     grid = Grid(g["nx"], g["ny"], g.get("ncomp", 1), g.get("rebin_every", 8) if rebin_every is None else rebin_every,
-                int(eager_moments), int(track_ids), int(particle_order), 0, g["dx"], g["dy"], g["dt"])
+                int(eager_moments), int(track_ids), int(particle_order), int(g.get("subcycle", 1)), g["dx"], g["dy"], g["dt"])
     sp = (Species * len(cfg["species"]))()
     for k, s in enumerate(cfg["species"]):
         sp[k] = Species(s["mass"], s["T_keV"], s["pressure_coeff"], s["DD"], s["sign"], s["shape"], s["mobile"], s["load"],
@@ -131,7 +131,7 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, part
     prof = Profile(p["kind"], p.get("taper_cells", 0), (C.c_double * 4)(*[float(v) for v in p["p"]]))
     las = (Laser * max(len(cfg["lasers"]), 1))()
     for k, l in enumerate(cfg["lasers"]):
-        las[k] = Laser(l["a0"], l["omega"], l["y0"], l["w0"], l["t_rise"], l["comp"], 0)
+        las[k] = Laser(l["a0"], l["omega"], l["y0"], l["w0"], l["t_rise"], l.get("alpha", 0.0), l["comp"], 0)
     return grid, sp, prof, las
 
 
@@ -183,7 +183,7 @@ class PM2D:
     def set_lasers(self, lasers):
         las = (Laser * max(len(lasers), 1))()
         for k, l in enumerate(lasers):
-            las[k] = Laser(l["a0"], l["omega"], l["y0"], l["w0"], l["t_rise"], l["comp"], 0)
+            las[k] = Laser(l["a0"], l["omega"], l["y0"], l["w0"], l["t_rise"], l.get("alpha", 0.0), l["comp"], 0)
         _check(self.lib.pm2d_set_lasers(self.ctx, las, len(lasers)))
 
     # -- grids ---------------------------------------------------------------------------------

@@ -52,6 +52,17 @@ int64_t species_np(const pm2d_grid &g, const pm2d_species &s)
     return (int64_t)g.nx * g.ny * s.ppc_x * s.ppc_y;
 }
 
+// Eq. 5 on a y-periodic box (Q22): a plane wave must come back to itself after Ly
+int validate_laser_angle(const pm2d_laser &L, double Ly)
+{
+    if (!(std::fabs(L.alpha) <= 1.0)) return fail(PM2D_EINVAL, "laser alpha must be within [-1, 1] rad");
+    if (L.alpha != 0.0 && !(L.w0 > 0.0)) {
+        const double m = L.omega * std::sin(L.alpha) * Ly;
+        if (std::fabs(m - std::nearbyint(m)) > 1e-6) return fail(PM2D_EINVAL, "oblique plane wave: omega*sin(alpha)*Ly must be an integer (y is periodic)");
+    }
+    return PM2D_OK;
+}
+
 int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
 {
     if (!g || !sp) return fail(PM2D_EINVAL, "null argument");
@@ -64,6 +75,9 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (!(g->dx > 0) || !(g->dy > 0) || !(g->dt > 0)) return fail(PM2D_EINVAL, "dx, dy, dt must be positive");
     if (g->dt / g->dx > 0.999 || g->dt / g->dy > 0.999)
         return fail(PM2D_EINVAL, "dt/dx must be < 1: a particle may not cross more than one cell per step");
+    if (g->subcycle < 0 || g->subcycle > 16) return fail(PM2D_EINVAL, "subcycle must be 0..16");
+    if (g->subcycle > 1 && (g->subcycle * g->dt / g->dx > 4.0 || g->subcycle * g->dt / g->dy > 4.0))
+        return fail(PM2D_EINVAL, "subcycle*dt/dx must be <= 4");
     for (int s = 0; s < nsp; s++) {
         const pm2d_species &q = sp[s];
         if (!(q.mass > 0)) return fail(PM2D_EINVAL, "species mass must be positive");
@@ -254,6 +268,8 @@ extern "C" size_t pm2d_query_workspace(const pm2d_grid *grid, const pm2d_species
     pm2d_ctx *c = new (std::nothrow) pm2d_ctx();
     if (!c) return 0;
     c->g = *grid;
+    c->nsub = grid->subcycle > 1 ? grid->subcycle : 1;
+    c->dtp = c->nsub * grid->dt;
     c->nsp = nsp;
     for (int s = 0; s < nsp; s++) c->sp[s].cfg = species[s];
     size_t bytes = layout(c, nullptr);
@@ -272,7 +288,10 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     if (!profile) return fail(PM2D_EINVAL, "null profile");
     if (nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
     for (int l = 0; l < nlaser; l++)
+    {
         if (lasers[l].comp < 0 || lasers[l].comp >= grid->ncomp) return fail(PM2D_EINVAL, "laser component out of range");
+        if ((rc = validate_laser_angle(lasers[l], grid->ny * grid->dy))) return rc;
+    }
     if (profile->kind < PM2D_PROFILE_UNIFORM || profile->kind > PM2D_PROFILE_FILAMENT_Y) return fail(PM2D_EINVAL, "unknown profile");
     double nmax;
     if (profile->kind == PM2D_PROFILE_UNIFORM) nmax = profile->p[0];
@@ -293,6 +312,8 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     pm2d_ctx *c = new (std::nothrow) pm2d_ctx();
     if (!c) return fail(PM2D_ENOMEM, "host allocation failed");
     c->g = *grid;
+    c->nsub = grid->subcycle > 1 ? grid->subcycle : 1;
+    c->dtp = c->nsub * grid->dt;
     c->nsp = nsp;
     c->nlaser = nlaser;
     for (int s = 0; s < nsp; s++) {
@@ -416,6 +437,10 @@ extern "C" void pm2d_free(pm2d_ctx *c) { destroy_ctx(c); }
 extern "C" int pm2d_set_lasers(pm2d_ctx *c, const pm2d_laser *lasers, int nlaser)
 {
     if (!c || nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
+    for (int l = 0; l < nlaser; l++) {
+        int rc = validate_laser_angle(lasers[l], c->g.ny * c->g.dy);
+        if (rc) return rc;
+    }
     for (int l = 0; l < nlaser; l++)
         if (lasers[l].comp < 0 || lasers[l].comp >= c->g.ncomp) return fail(PM2D_EINVAL, "laser component out of range");
     for (int l = 0; l < nlaser; l++) c->laser[l] = lasers[l];
@@ -428,15 +453,32 @@ static int enqueue_step(pm2d_ctx *c)
 {
     int rc;
     // (2) a^{n+1} from a^n, a^{n-1}, n_e^n ; E^n from n_i^n - n_e^n
-    phase_begin(c, PM2D_PH_FIELD);
-    if ((rc = launch_field_step(c))) return rc;
-    phase_end(c);
+    if (c->nsub == 1) {
+        phase_begin(c, PM2D_PH_FIELD);
+        if ((rc = launch_field_step(c, 0))) return rc;
+        phase_end(c);
+    }
     for (int stage = 0; stage < 2; stage++) {
         // E^n from n^n resp. E^ from n^ (Eqs. 9-11), and in the epilogue of the inverse transform the nodal
         // force of (3) / (7): Eq. 16 with a^n, n^n / Eq. 18 with a^{n+1}, n^
         phase_begin(c, PM2D_PH_POISSON);
         if ((rc = launch_poisson(c, false, stage == 0 ? c->a[1] : c->a[0], stage == 1))) return rc;
         phase_end(c);
+        if (stage == 0 && c->nsub > 1) {
+            // sub-cycling (Q21): the force of (3) has taken a^n; now S wave steps with n_e^n held (it is zeroed
+            // only below), the ring turning after each but the last, so that a[0] = a^{n+1} for stage B
+            phase_begin(c, PM2D_PH_FIELD);
+            for (int sub = 0; sub < c->nsub; sub++) {
+                if ((rc = launch_field_step(c, sub))) return rc;
+                if (sub + 1 < c->nsub) {
+                    float *t = c->a[2];
+                    c->a[2] = c->a[1];
+                    c->a[1] = c->a[0];
+                    c->a[0] = t;
+                }
+            }
+            phase_end(c);
+        }
         // the set just read (n^n resp. n^) is the target of the stage after next: zero it on the side stream now;
         // the target of this stage was zeroed while the previous stage ran
         if ((rc = zero_set_async(c, stage))) return rc;

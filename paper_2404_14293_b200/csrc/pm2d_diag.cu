@@ -125,7 +125,7 @@ int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out)
     PM2D_CUDA_CHECK(cudaMemcpyAsync(h, c->red, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     out->step = c->step;
-    out->time = c->step * c->g.dt;
+    out->time = c->step * c->dtp;
     out->W_es = 2.0 * PI * PI * h[0];
     out->W_int = h[1];
     out->W_em = h[2] / (8.0 * PI * PI);

@@ -74,24 +74,72 @@ __device__ __forceinline__ float beam_env(const BcParams &B, int l, float y)
     return __expf(-r * r);
 }
 
+// Oblique incidence (Eq. 5; Q22): envelope and carrier no longer separate, so the incident wave
+// is evaluated per boundary node and time level, in double (the phase 2 pi omega (t - xb) grows without bound).
+struct ObLaser {
+    double a0, omega2, y0, inv_w0, inv_2rise, sa, ca, lead;   // omega2 = 2 omega; inv_2rise = 1 / (2 t_rise) or 0
+    int comp, oblique;
+};
+struct ObParams {
+    ObLaser L[PM2D_MAX_LASERS];
+    double t_now, dt, dx, Ly, inv_Ly;
+};
+
+// Eq. 4 in the beam's coordinates; (x, y) are box coordinates, y' = y - y0 at the nearest periodic image
+__device__ double oblique_inc(const ObLaser &L, double x, double y, double t, double Ly, double inv_Ly)
+{
+    double xb = x, yb = y - L.y0, lead = 0.0;
+    if (L.oblique) {
+        double d = y - L.y0;
+        d -= Ly * floor(d * inv_Ly + 0.5);
+        xb = x * L.ca - d * L.sa;                 // Eq. 5
+        yb = x * L.sa + d * L.ca;
+        lead = L.lead;
+    }
+    const double phase = t - xb, tau = phase - lead;
+    if (tau <= 0.0) return 0.0;
+    double v = L.a0 * cospi(L.omega2 * phase);
+    if (L.inv_w0 > 0.0) {
+        const double r = yb * L.inv_w0;
+        v *= exp(-r * r);
+    }
+    if (L.inv_2rise > 0.0 && tau * L.inv_2rise < 0.5) {
+        const double sr = sinpi(tau * L.inv_2rise);
+        v *= sr * sr;
+    }
+    return v;
+}
+
 // Eq. 8 solved for the boundary node, both x walls, one thread per j.  Left wall: applied to the
-// scattered field s = a - a_inc and a_inc added back.
+// scattered field s = a - a_inc and a_inc added back.  OBLIQUE: some beam has alpha != 0.
+template <bool OBLIQUE>
 __global__ void k_boundary(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap, BcParams B,
-                           int comp, int nx, int ny)
+                           ObParams O, int comp, int nx, int ny)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= ny) return;
     const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
     // incident wave at the 3 columns j-1, j, j+1: inc[col][x][t]
     float inc[3][6];
-    for (int q = 0; q < 3; q++)
-        for (int k = 0; k < 6; k++) inc[q][k] = 0.f;
-    for (int l = 0; l < B.nlaser; l++) {
-        if (B.comp[l] != comp) continue;
-        const int cols[3] = {jm, j, jp};
-        for (int q = 0; q < 3; q++) {
-            float e = beam_env(B, l, cols[q] * B.dy);
-            for (int k = 0; k < 6; k++) inc[q][k] += e * B.g[l][k];
+    const int cols[3] = {jm, j, jp};
+    if (OBLIQUE) {
+        for (int q = 0; q < 3; q++)
+            for (int k = 0; k < 6; k++) {
+                double v = 0.0;
+                for (int l = 0; l < B.nlaser; l++)
+                    if (B.comp[l] == comp)
+                        v += oblique_inc(O.L[l], (k / 3) * O.dx, cols[q] * (double)B.dy, O.t_now + (k % 3 - 1) * O.dt, O.Ly, O.inv_Ly);
+                inc[q][k] = (float)v;
+            }
+    } else {
+        for (int q = 0; q < 3; q++)
+            for (int k = 0; k < 6; k++) inc[q][k] = 0.f;
+        for (int l = 0; l < B.nlaser; l++) {
+            if (B.comp[l] != comp) continue;
+            for (int q = 0; q < 3; q++) {
+                float e = beam_env(B, l, cols[q] * B.dy);
+                for (int k = 0; k < 6; k++) inc[q][k] += e * B.g[l][k];
+            }
         }
     }
     const float ab = 1.f / (B.alpha + B.beta);
@@ -206,10 +254,11 @@ static double laser_g(const pm2d_laser &L, double tau)
     return L.a0 * ramp * cos(2.0 * PI * L.omega * tau);
 }
 
-int launch_field_step(pm2d_ctx *c)
+// one step of Eq. 6 + Eq. 8: a[0] <- a[1], a[2]; sub = index of the wave step inside the particle step (Q21)
+int launch_field_step(pm2d_ctx *c, int sub)
 {
     const int nx = c->g.nx, ny = c->g.ny;
-    const double dx = c->g.dx, dy = c->g.dy, dt = c->g.dt, t_now = c->step * dt;
+    const double dx = c->g.dx, dy = c->g.dy, dt = c->g.dt, t_now = (double)(c->step * c->nsub + sub) * dt;
     NeSrc ne;
     ne.count = 0;
     ne.inv_nscale = c->inv_nscale;
@@ -229,12 +278,28 @@ int launch_field_step(pm2d_ctx *c)
     B.beta = (float)(1.0 / (2.0 * dt * dt));
     B.gam = (float)(1.0 / (4.0 * dy * dy));
     B.dy = (float)dy;
+    ObParams O;
+    bool oblique = false;
+    for (int l = 0; l < c->nlaser; l++) {
+        const pm2d_laser &L = c->laser[l];
+        ObLaser &Q = O.L[l];
+        Q.a0 = L.a0; Q.omega2 = 2.0 * L.omega; Q.y0 = L.y0;
+        Q.inv_w0 = L.w0 > 0.0 ? 1.0 / L.w0 : 0.0;
+        Q.inv_2rise = L.t_rise > 0.0 ? 0.5 / L.t_rise : 0.0;
+        Q.sa = sin(L.alpha); Q.ca = cos(L.alpha);
+        Q.lead = 0.5 * ny * dy * fabs(Q.sa);
+        Q.comp = L.comp;
+        Q.oblique = L.alpha != 0.0;
+        oblique = oblique || Q.oblique;
+    }
+    O.t_now = t_now; O.dt = dt; O.dx = dx; O.Ly = ny * dy; O.inv_Ly = 1.0 / (ny * dy);
     dim3 grid((ny + FCOLS - 1) / FCOLS, (nx - 1 + FROWS - 1) / FROWS);
     for (int comp = 0; comp < c->g.ncomp; comp++) {
         const size_t off = (size_t)comp * c->nn;
         k_wave<<<grid, FCOLS, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, ne, nx, ny, (float)(1.0 / (dx * dx)),
                                               (float)(1.0 / (dy * dy)), (float)(dt * dt));
-        k_boundary<<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, comp, nx, ny);
+        if (oblique) k_boundary<true><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
+        else k_boundary<false><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
         count_launch(c, 2);
     }
     PM2D_CUDA_CHECK(cudaGetLastError());

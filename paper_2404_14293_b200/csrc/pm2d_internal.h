@@ -77,7 +77,9 @@ struct pm2d_ctx {
     cudaStream_t stream;
     cudaStream_t zstream;            // side stream: zeroes the idle deposit set while a stage kernel runs
     cudaEvent_t ev_free[2], ev_zero[2];   // [0] main set (n^n, stage B target), [1] hat set (stage A target)
-    int64_t step;
+    int64_t step;        // particle steps taken
+    int nsub;            // wave-equation steps per particle step (Q21)
+    double dtp;          // particle time step = nsub * g.dt
     int64_t nn;          // nodes
     int ntx, nty, ntiles;
     int LP;              // pitch (complex elements) of spectral rows: ny/2 + 2
@@ -140,7 +142,7 @@ int launch_set_cell_offsets_uniform(pm2d_ctx *c, int s);
 int launch_build_chunks(pm2d_ctx *c, int s);
 int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float *fx, float *fy, float *ux, float *uy);
 // pm2d_fields.cu
-int launch_field_step(pm2d_ctx *c);
+int launch_field_step(pm2d_ctx *c, int sub);
 int launch_force(pm2d_ctx *c, int s, const float *a_level);
 int launch_fix_background(pm2d_ctx *c, int s);
 int launch_fix_to_float(pm2d_ctx *c, const int32_t *src, float scale, float *dst);

@@ -1602,9 +1602,9 @@ static PartParams make_part_params(pm2d_ctx *c, int s)
     P.stray_total = c->stray_total;
     P.ovf_p = c->ovf_p; P.ovf_tile = c->ovf_tile; P.ovf_count = c->ovf_count; P.ovf_cap = c->ovf_cap;
     P.nx = c->g.nx; P.ny = c->g.ny; P.nty = c->nty;
-    P.dt = (float)c->g.dt;
-    P.hx = (float)(c->g.dt / (2.0 * c->g.dx));
-    P.hy = (float)(c->g.dt / (2.0 * c->g.dy));
+    P.dt = (float)c->dtp;                                   // particle step: S wave steps (Q21)
+    P.hx = (float)(c->dtp / (2.0 * c->g.dx));
+    P.hy = (float)(c->dtp / (2.0 * c->g.dy));
     P.nscale = c->nscale; P.pscale = c->pscale;
     P.pratio = c->pscale / c->nscale;
     P.half_dd = (float)(0.5 * S.cfg.DD);
@@ -1672,7 +1672,7 @@ static int launch_stage_any(pm2d_ctx *c, int s, int stage, int qmask)
     const bool sparse = S.layered;
     // thermal drift between two rebins, in cells: below a tenth of a cell the particles are (almost all) still in the
     // cells they were sorted into
-    const bool anch = sqrt(S.vth2) * c->g.dt / fmin(c->g.dx, c->g.dy) * (double)(c->g.rebin_every > 0 ? c->g.rebin_every : 32) < 0.1;
+    const bool anch = sqrt(S.vth2) * c->dtp / fmin(c->g.dx, c->g.dy) * (double)(c->g.rebin_every > 0 ? c->g.rebin_every : 32) < 0.1;
     if (S.cfg.shape == PM2D_CIC) launch_stage_shape<PM2D_CIC>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);
     else if (S.cfg.shape == PM2D_TSC) launch_stage_shape<PM2D_TSC>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);
     else launch_stage_shape<PM2D_SINE>(P, stage, qmask, c->ntiles, sparse, anch, c->stream);

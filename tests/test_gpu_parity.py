@@ -1,6 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Tolerances are BASELINE.json's: deposited fields rel-L2 <= 1e-5 per step,
 particle phase space after 10 steps max relative error <= 1e-5, rebin bit-exact, energies 2 %."""
+import copy
 import math
 
 import numpy as np
@@ -527,4 +528,93 @@ def test_three_components_two_beams_gaussian_parity(P):
         vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
         ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
         assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4, (s, ex, ey, eu, dabs)
+    sim.close()
+
+
+# ---- S§8(f).1: oblique incidence (Eq. 5) and particle sub-cycling -------------------------------------
+def _cbet_cfg(nx, ny, subcycle):
+    """Reduced copy of the paper's CBET set-up: two Gaussian beams at +15 and -15 degrees with wavelengths
+    lambda0 and 0.9995 lambda0 on the same component, electrons at 1 keV and mobile ions at 200 eV, DD = 1.85 dx,
+    particle step = `subcycle` wave steps."""
+    cfg = small_cfg("c3", nx, ny, subcycle=subcycle)
+    Ly = ny * cfg["grid"]["dy"]
+    for sp, T in zip(cfg["species"], (1.0, 0.2)):
+        sp["T_keV"], sp["DD"] = T, 1.85
+    al = math.radians(15.0)
+    cfg["lasers"] = [dict(a0=0.03, omega=1.0, y0=0.35 * Ly, w0=0.15 * Ly, alpha=al, comp=0, t_rise=0.5),
+                     dict(a0=0.03, omega=1.0 / 0.9995, y0=0.65 * Ly, w0=0.15 * Ly, alpha=-al, comp=0, t_rise=0.5)]
+    return cfg
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("subcycle", [1, 5])
+def test_cbet_like_oblique_beams_subcycled_parity(P, subcycle):
+    cfg = _cbet_cfg(72, 64, subcycle)
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=2)
+    orc, _ = oracle_from_config(cfg)
+    nsteps = 10 if subcycle > 1 else 40
+    for step in range(nsteps):
+        sim.step(1)
+        orc.step(1)
+        if step % 3 == 0 or step == nsteps - 1:
+            a = sim.get_fields(P.FIELD_A, 0, 0)
+            scale = max(np.abs(orc.a_now[0]).max(), 1e-30)
+            assert np.abs(a - orc.a_now[0]).max() < 2e-5 * scale + 1e-9, step
+            for s in (0, 1):
+                assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < 1e-5, (step, s)
+    assert np.abs(orc.a_now[0]).max() > 0.01                       # both beams are in the box
+    d = sim.diagnostics()
+    assert d["step"] == nsteps and d["time"] == pytest.approx(nsteps * subcycle * cfg["grid"]["dt"], rel=1e-12)
+    for s, sp in enumerate(cfg["species"]):
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
+        assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4, (s, ex, ey, eu, dabs)
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_oblique_plane_wave_long_run_parity(P):
+    """An oblique plane wave that fits the periodic box (omega sin(alpha) Ly = 1) driving the c1 slab for 300 steps:
+    the boundary condition with Eq. 5 stays with the oracle while the wave crosses the box and leaves on the right."""
+    cfg = small_cfg("c1", 96, 64)
+    Ly = 64 * cfg["grid"]["dy"]
+    cfg["lasers"] = [dict(a0=0.01, omega=1.0, y0=0.0, w0=0.0, alpha=-math.asin(1.0 / Ly), comp=0, t_rise=2.0)]
+    sim = P.PM2D(cfg, eager_moments=1, rebin_every=8)
+    orc, _ = oracle_from_config(cfg)
+    for blk in range(6):
+        sim.step(50)
+        orc.step(50)
+        a = sim.get_fields(P.FIELD_A, 0, 0)
+        scale = max(np.abs(orc.a_now[0]).max(), 1e-30)
+        assert np.abs(a - orc.a_now[0]).max() < 5e-5 * scale + 1e-9, blk
+    # the wave carries transverse mode 1 (the noisy slab scatters a few per cent into its neighbours)
+    A = np.abs(np.fft.rfft(a[8:-8], axis=1)).sum(axis=0)
+    assert A[1] > 0.9 * A.sum()
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_oblique_and_subcycle_arguments_are_validated(P):
+    cfg = small_cfg("c1", 96, 64)
+    bad = copy.deepcopy(cfg)
+    bad["lasers"][0]["alpha"] = 0.2                                 # plane wave that does not fit the periodic box
+    with pytest.raises(P.PM2DError):
+        P.PM2D(bad)
+    bad = copy.deepcopy(cfg)
+    bad["lasers"][0]["alpha"] = 1.5
+    bad["lasers"][0]["w0"] = 1.0
+    with pytest.raises(P.PM2DError):
+        P.PM2D(bad)
+    bad = small_cfg("c1", 96, 64, subcycle=17)
+    with pytest.raises(P.PM2DError):
+        P.PM2D(bad)
+    ok = copy.deepcopy(cfg)
+    ok["lasers"][0]["alpha"] = 0.2                                  # a Gaussian beam may come in at any angle
+    ok["lasers"][0]["w0"] = 0.5
+    ok["lasers"][0]["y0"] = 1.6
+    sim = P.PM2D(ok)
+    sim.step(2)
+    with pytest.raises(P.PM2DError):
+        sim.set_lasers([dict(ok["lasers"][0], w0=0.0)])
     sim.close()
