@@ -216,14 +216,15 @@ def run_cuda(args):
                     warmup=args.warmup, ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak",
                     vs_baseline=None, dtype="f32", data="synthetic",
                     config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU "
-                                         f"(BASELINE.json configs[{int(args.config[1]) - 1}])",
+                                         + (f"(BASELINE.json configs[{int(args.config[1]) - 1}])" if args.config != "cbet" else
+                                            "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)"),
                                 shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
-                                eager_moments=bool(args.eager), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
+                                eager_moments=bool(args.eager), subcycle=int(g.get("subcycle", 1)), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
                                 l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
                                 parallelism="replicas only" if world > 1 else "1 GPU"),
                     ns_per_particle_step=1e9 / value * world,
-                    cell_updates_per_s=nodes * g["ncomp"] * world * args.steps / (ms_max * 1e-3),
-                    field_kernel_node_updates_per_s=(nodes * g["ncomp"] / (prof["ms"]["field"] / steps_p * 1e-3)) if prof["ms"]["field"] > 0 else None,
+                    cell_updates_per_s=nodes * g["ncomp"] * max(int(g.get("subcycle", 1)), 1) * world * args.steps / (ms_max * 1e-3),
+                    field_kernel_node_updates_per_s=(nodes * g["ncomp"] * max(int(g.get("subcycle", 1)), 1) / (prof["ms"]["field"] / steps_p * 1e-3)) if prof["ms"]["field"] > 0 else None,
                     phases_ms_per_step={k: v / steps_p for k, v in prof["ms"].items()},
                     stray_fraction=strays / max(2.0 * nmob * args.steps, 1.0),
                     clocks=clocks, gpu_launches=int(launches),
@@ -249,7 +250,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "cbet"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--eager", type=int, default=1, help="1: deposit n, Px, Py at both stages (paper's flow); 0: n only")
     ap.add_argument("--rebin-every", type=int, default=None)

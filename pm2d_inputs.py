@@ -222,6 +222,18 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
         c["species"] = [_species(-1, 1.0, 5.0, 10, 6, SINE, 1.9, load=NUMBER_WEIGHTED),
                         _species(+1, 1836.0, 0.0, 0, 0, SINE, 1.9, mobile=0, load=LOAD_NONE)]
         c["lasers"] = [_laser(0.01)]
+    elif name == "cbet":  # S§8(f).1, the paper's CBET run: 8000x8000 there, 8192x8192 here (ny a power of two);
+        # 0.4 n_c hydrogen slab (the standard edge taper stands in for the 20 lambda0 vacuum margins), 1 e + 1 ion per
+        # cell, 1 keV / 200 eV, DD = 1.85 dx, two beams a0 = 0.008 at +-15 degrees, lambda0 and 0.9995 lambda0, centres
+        # -+50 lambda0 from the axis, w0 = 30 lambda0, particle step = 5 wave steps
+        c = _base(8192, 8192, 0.035, 200, 5, rebin_every=4)
+        c["grid"]["subcycle"] = 5
+        c["profile"] = dict(kind=PROFILE_UNIFORM, p=[0.4, 0, 0, 0])
+        c["species"] = [_species(-1, 1.0, 1.0, 1, 1, SINE, 1.85),
+                        _species(+1, 1836.0, 0.2, 1, 1, SINE, 1.85)]
+        al = math.radians(15.0)
+        c["lasers"] = [dict(_laser(0.008, w0=30.0 / 409.6, y0=0.5 - 50.0 / 409.6), alpha=al),
+                       dict(_laser(0.008, w0=30.0 / 409.6, y0=0.5 + 50.0 / 409.6, omega=1.0 / 0.9995), alpha=-al)]
     else:
         raise ValueError(name)
     if nx is not None:
@@ -238,10 +250,11 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     for sp in c["species"]:
         if sp["load"] == NUMBER_WEIGHTED:                 # slots: an upper bound of the dithered counts
             sp["capacity"] = g["nx"] * g["ny"] * sp["ppc_x"] * sp["ppc_y"] + 4096
-    if name == "c4":
+    if name in ("c4", "cbet"):
         Ly = g["ny"] * g["dy"]
-        c["lasers"][0]["w0"] *= Ly
-        c["lasers"][0]["y0"] *= Ly
+        for las in c["lasers"]:
+            las["w0"] *= Ly
+            las["y0"] *= Ly
     return copy.deepcopy(c)
 
 

@@ -618,3 +618,25 @@ def test_oblique_and_subcycle_arguments_are_validated(P):
     with pytest.raises(P.PM2DError):
         sim.set_lasers([dict(ok["lasers"][0], w0=0.0)])
     sim.close()
+
+
+@pytest.mark.gpu
+def test_cbet_bench_config_reduced_parity(P):
+    """pm2d_inputs.config("cbet") (bench.py --config cbet) on a reduced box: 6 particle steps = 30 wave steps."""
+    cfg = small_cfg("cbet", 80, 64)
+    assert cfg["grid"]["subcycle"] == 5 and cfg["lasers"][0]["alpha"] == -cfg["lasers"][1]["alpha"] != 0.0
+    for las in cfg["lasers"]:
+        las["t_rise"] = 0.3                    # the reduced box is 3.2 lambda0 wide: let the beams in within the run
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1)
+    orc, _ = oracle_from_config(cfg)
+    sim.step(6)
+    orc.step(6)
+    a = sim.get_fields(P.FIELD_A, 0, 0)
+    assert np.abs(orc.a_now[0]).max() > 1e-3
+    assert np.abs(a - orc.a_now[0]).max() < 2e-5 * np.abs(orc.a_now[0]).max() + 1e-9
+    for s, sp in enumerate(cfg["species"]):
+        assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < 1e-5
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
+        assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4, (s, ex, ey, eu, dabs)
+    sim.close()

@@ -165,3 +165,34 @@ def test_P16_subcycled_plasma_oscillation_period():
     # the finite-grid factors of mode 2 on 64 cells (TSC smoothing, differenced E) lengthen the period by 0.6 %
     assert period == pytest.approx(1.0 / math.sqrt(n0) * th / phi, rel=0.01)
     # a push with dt instead of S dt would give a period S times longer on this time axis
+
+
+def test_P15_oblique_turning_point_cos2_theta():
+    """"the propagation of the incident laser beam is stopped when n_e = cos^2(theta) n_c".  A plane wave at
+    theta = asin(1/3.2) = 18.2 degrees in a fixed linear ramp n_e = x'/L_n (L_n = 10 lambda0) is an Airy pattern
+    Ai((x' - x_t)/l) with x_t = L_n cos^2(theta) = 9.02 lambda0 (10 lambda0 at normal incidence) and l =
+    (L_n/k0^2)^(1/3) = 0.633 lambda0: last maximum of the cycle-averaged a^2 at x_t - 1.0188 l, evanescent beyond."""
+    nx, ny, dx, dt, Ln = 240, 64, 0.05, 0.035, 10.0
+    Ly = ny * dx
+    ne = np.repeat((np.arange(nx + 1) * dx / Ln)[:, None], ny, axis=1)
+    ell = (Ln / (2 * math.pi) ** 2) ** (1.0 / 3.0)
+    xs = np.arange(nx + 1) * dx
+    found = {}
+    for name, al in (("normal", 0.0), ("oblique", math.asin(1.0 / Ly))):
+        sp = [dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, shape=oracle.CIC, DD=1.0, n_fixed=ne)]
+        o = oracle.Oracle(nx, ny, dx, dx, dt, sp, [dict(a0=0.01, t_rise=3.0, alpha=al)])
+        o.step(int(34.0 / dt))                     # in, back, and a few periods to settle
+        acc = np.zeros(nx + 1)
+        per = int(round(2.0 / dt))
+        for _ in range(per):
+            o.step()
+            acc += (o.a_now[0] ** 2).mean(axis=1)
+        # last interior maximum of the standing pattern, refined by a parabola through its neighbours
+        i = max(k for k in range(2, nx - 1) if acc[k] > acc[k - 1] and acc[k] >= acc[k + 1] and acc[k] > 0.2 * acc.max())
+        off = 0.5 * (acc[i - 1] - acc[i + 1]) / (acc[i - 1] - 2 * acc[i] + acc[i + 1])
+        found[name] = (i + off) * dx
+        xt = Ln * math.cos(al) ** 2
+        assert found[name] == pytest.approx(xt - 1.0188 * ell, abs=0.12)
+        beyond = acc[xs > xt + 2.0 * ell]
+        assert beyond.max() < 0.02 * acc.max()
+    assert found["normal"] - found["oblique"] == pytest.approx(Ln * (1.0 / Ly) ** 2, abs=0.1)      # L_n sin^2(theta)
