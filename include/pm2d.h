@@ -42,6 +42,7 @@ extern "C" {
 
 #define PM2D_MAX_SPECIES 4
 #define PM2D_MAX_LASERS 4
+#define PM2D_MAX_MODES 16
 #define PM2D_TILE 32 /* particles are binned by tiles of PM2D_TILE x PM2D_TILE cells */
 
 /* particle shape: 1-D cumulative weight G(s); weights are G differences over the control volumes
@@ -201,6 +202,14 @@ int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);
+
+/* Fourier-mode amplitudes of a species' current nodal density (the k-spectra of Figs. 7 and 14,
+ * P:L356, are |A|^2 of delta n_e):
+ *     A(m_x, m_y) = sum_{i=0..nx} sum_{j<ny} v_i n_s(i,j) exp(-2 pi i (m_x i / nx + m_y j / ny)),
+ * v_i = 1/2 on the wall columns i = 0, nx (half control volumes, Q9), 1 elsewhere; in units of n_c * cells.
+ * mx, my: host int32[nmodes] (any sign), 1 <= nmodes <= PM2D_MAX_MODES; re, im: host double[nmodes].
+ * float32/fixed-point input, float64 accumulation; synchronises the stream. */
+int pm2d_mode_amplitudes(pm2d_ctx *ctx, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re, double *im);
 int64_t pm2d_particle_count(pm2d_ctx *ctx, int species);
 
 /* CUDA-event profile of the step phases on the ctx's stream.  enable(1) starts recording one event

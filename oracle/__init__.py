@@ -196,6 +196,21 @@ def a_inc(laser: dict, x, y, t, Ly=1.0):
     return lib().orc_a_inc(C.byref(L), x, y, t, Ly)
 
 
+def mode_amplitudes(n, mx, my):
+    """O9: Fourier-mode amplitudes of a nodal density n[(nx+1), ny], written out as the sum that
+    defines them: A(mx, my) = sum_i sum_j v_i n[i, j] exp(-2 pi i (mx i/nx + my j/ny)), v_i = 1/2 on the wall columns
+    (half control volumes, Q9).  The k-spectra of Figs. 7 and 14 are |A|^2 of delta n_e."""
+    n = np.asarray(n, np.float64)
+    nx, ny = n.shape[0] - 1, n.shape[1]
+    v = np.ones(nx + 1)
+    v[0] = v[nx] = 0.5
+    i, j = np.arange(nx + 1)[:, None], np.arange(ny)[None, :]
+    out = np.zeros(len(mx), complex)
+    for k, (a, b) in enumerate(zip(mx, my)):
+        out[k] = (v[:, None] * n * np.exp(-2j * np.pi * (a * i / nx + b * j / ny))).sum()
+    return out
+
+
 # ---------------------------------------------------------------------------------------------
 class Oracle:
     """The whole step (O8) over numpy-owned arrays.

@@ -72,6 +72,7 @@ SYMBOLS = {
     "pm2d_set_background": (C.c_int, [_vp, C.c_int, _fp]),
     "pm2d_rebin": (C.c_int, [_vp, C.c_int, _ip, _lp]),
     "pm2d_diagnostics": (C.c_int, [_vp, C.POINTER(Diag)]),
+    "pm2d_mode_amplitudes": (C.c_int, [_vp, C.c_int, C.c_int, _ip, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pm2d_particle_count": (C.c_int64, [_vp, C.c_int]),
     "pm2d_profile_enable": (C.c_int, [_vp, C.c_int]),
     "pm2d_profile_get": (C.c_int, [_vp, C.POINTER(C.c_double), _lp, _lp]),
@@ -251,6 +252,15 @@ class PM2D:
         return dict(step=d.step, time=d.time, W_es=d.W_es, W_int=d.W_int, W_em=d.W_em, W_total=d.W_total,
                     W_kin=list(d.W_kin)[: self.nsp], W_th=list(d.W_th)[: self.nsp], charge=list(d.charge)[: self.nsp],
                     count=list(d.count)[: self.nsp])
+
+    def mode_amplitudes(self, species, mx, my):
+        """complex A(m_x, m_y) of the species' nodal density for the mode pairs (mx[k], my[k])  [pm2d_mode_amplitudes]"""
+        mx, my = np.ascontiguousarray(mx, np.int32), np.ascontiguousarray(my, np.int32)
+        re, im = np.zeros(mx.size), np.zeros(mx.size)
+        _dp = C.POINTER(C.c_double)
+        _check(self.lib.pm2d_mode_amplitudes(self.ctx, int(species), int(mx.size), mx.ctypes.data_as(_ip), my.ctypes.data_as(_ip),
+                                             re.ctypes.data_as(_dp), im.ctypes.data_as(_dp)))
+        return re + 1j * im
 
     def profile_enable(self, on=True):
         _check(self.lib.pm2d_profile_enable(self.ctx, int(on)))

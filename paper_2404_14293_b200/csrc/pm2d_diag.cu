@@ -92,7 +92,78 @@ __global__ void __launch_bounds__(256) k_diag_kinetic(const PV *pv, const float 
     block_add(s, red);
 }
 
+// a8: Fourier-mode amplitudes of a nodal density.  Grid-stride over the nodes, every thread keeps the running sums
+// of all modes in double; the phase m_x i / nx + m_y j / ny is reduced mod 1 in integers before sincospi.
+struct ModeParams {
+    const int32_t *nfix;
+    int nx, ny, nmodes;
+    int mx[PM2D_MAX_MODES], my[PM2D_MAX_MODES];
+    double inv_nscale;
+    double *red;          // [2 * nmodes]: re, im interleaved
+};
+
+__global__ void __launch_bounds__(256) k_diag_modes(const ModeParams M)
+{
+    double re[PM2D_MAX_MODES], im[PM2D_MAX_MODES];
+#pragma unroll
+    for (int m = 0; m < PM2D_MAX_MODES; m++) re[m] = im[m] = 0.0;
+    const int64_t nn = (int64_t)(M.nx + 1) * M.ny;
+    const double inv_nx = 1.0 / M.nx, inv_ny = 1.0 / M.ny;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nn; k += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(k / M.ny), j = (int)(k - (int64_t)i * M.ny);
+        const int v = M.nfix[k];
+        if (v == 0) continue;
+        const double n = ((i == 0 || i == M.nx) ? 0.5 : 1.0) * (double)v * M.inv_nscale;
+#pragma unroll
+        for (int m = 0; m < PM2D_MAX_MODES; m++) {
+            if (m >= M.nmodes) break;
+            const int64_t px = ((int64_t)M.mx[m] * i) % M.nx, py = ((int64_t)M.my[m] * j) % M.ny;
+            double sn, cs;
+            sincospi(-2.0 * ((double)px * inv_nx + (double)py * inv_ny), &sn, &cs);
+            re[m] += n * cs;
+            im[m] += n * sn;
+        }
+    }
+#pragma unroll
+    for (int m = 0; m < PM2D_MAX_MODES; m++) {
+        if (m >= M.nmodes) break;
+        block_add(re[m], &M.red[2 * m]);
+        block_add(im[m], &M.red[2 * m + 1]);
+    }
+}
+
 }  // namespace
+
+extern "C" int pm2d_mode_amplitudes(pm2d_ctx *c, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re,
+                                    double *im)
+{
+    if (!c || species < 0 || species >= c->nsp || nmodes < 1 || nmodes > PM2D_MAX_MODES || !mx || !my || !re || !im)
+    {
+        pm2d_set_error("pm2d_mode_amplitudes: bad argument (species, 1 <= nmodes <= PM2D_MAX_MODES, non-null arrays)");
+        return PM2D_EINVAL;
+    }
+    ModeParams M;
+    M.nfix = c->sp[species].nfix;
+    M.nx = c->g.nx; M.ny = c->g.ny; M.nmodes = nmodes;
+    for (int m = 0; m < PM2D_MAX_MODES; m++) {
+        M.mx[m] = m < nmodes ? mx[m] : 0;
+        M.my[m] = m < nmodes ? my[m] : 0;
+    }
+    M.inv_nscale = (double)c->inv_nscale;
+    M.red = c->red;
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->red, 0, 64 * sizeof(double), c->stream));
+    k_diag_modes<<<592, 256, 0, c->stream>>>(M);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    double h[2 * PM2D_MAX_MODES];
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(h, c->red, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    for (int m = 0; m < nmodes; m++) {
+        re[m] = h[2 * m];
+        im[m] = h[2 * m + 1];
+    }
+    return PM2D_OK;
+}
 
 // expects c->phi to hold phi of the current densities (caller ran launch_poisson(c, true))
 int launch_diagnostics(pm2d_ctx *c, pm2d_diag *out)

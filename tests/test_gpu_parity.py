@@ -640,3 +640,26 @@ def test_cbet_bench_config_reduced_parity(P):
         ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
         assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4, (s, ex, ey, eu, dabs)
     sim.close()
+
+
+@pytest.mark.gpu
+def test_mode_amplitudes_parity(P):
+    """a8: Fourier-mode amplitudes of n_e and n_i (pm2d_mode_amplitudes) against the oracle's defining sum on the
+    oracle's own density after 5 steps of the reduced c3 config (ragged nx, walls included)."""
+    cfg = small_cfg("c3", 72, 64)
+    sim = P.PM2D(cfg, eager_moments=1, rebin_every=2)
+    orc, _ = oracle_from_config(cfg)
+    sim.step(5)
+    orc.step(5)
+    mx = [0, 1, 0, 3, -2, 7, 36, 71, 5, 1, 2, 3, 4, 5, 6, 9]
+    my = [0, 0, 1, 2, 5, -3, 32, 63, 31, 1, 1, 1, 1, 1, 1, 9]
+    for s in (0, 1):
+        ref = oracle.mode_amplitudes(orc.moment(s, "n"), mx, my)
+        got = sim.mode_amplitudes(s, mx, my)
+        assert got.shape == ref.shape
+        scale = np.abs(ref[0])                                    # the (0, 0) amplitude: total charge
+        assert np.abs(got - ref).max() < 1e-5 * scale, (s, np.abs(got - ref).max() / scale)
+        assert np.abs(ref[1:]).max() > 1e-4 * scale               # the profile and the noise give the other modes a size
+    with pytest.raises(P.PM2DError):
+        sim.mode_amplitudes(0, list(range(17)), list(range(17)))
+    sim.close()

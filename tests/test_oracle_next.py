@@ -196,3 +196,31 @@ def test_P15_oblique_turning_point_cos2_theta():
         beyond = acc[xs > xt + 2.0 * ell]
         assert beyond.max() < 0.02 * acc.max()
     assert found["normal"] - found["oblique"] == pytest.approx(Ln * (1.0 / Ly) ** 2, abs=0.1)      # L_n sin^2(theta)
+
+
+# ---- a8: Fourier-mode amplitudes ---------------------------------------------------------------------------
+def test_P17_mode_amplitudes_closed_form_and_fft():
+    """A single cosine product has the closed-form amplitude eps nx ny / 4 in its four modes and nx ny in (0, 0);
+    for any field the wall-halved sum over i = 0..nx is the periodic DFT of the field with its two wall columns
+    averaged into one (numpy's fft2 as the independent routine)."""
+    nx, ny, m, l, eps = 24, 16, 3, 2, 0.25
+    i, j = np.arange(nx + 1)[:, None], np.arange(ny)[None, :]
+    n = 1.0 + eps * np.cos(2 * np.pi * m * i / nx) * np.cos(2 * np.pi * l * j / ny)
+    A = oracle.mode_amplitudes(n, [0, m, -m, m, 1, m], [0, l, l, -l, l, 0])
+    assert A[0] == pytest.approx(nx * ny, abs=1e-9)
+    for k in (1, 2, 3):
+        assert A[k] == pytest.approx(eps * nx * ny / 4, abs=1e-9)
+    assert abs(A[4]) < 1e-9 and abs(A[5]) < 1e-9
+    # a phase: n = sin(2 pi (m i/nx + l j/ny)) has A(m, l) = nx ny / (2i), A(-m, -l) = -nx ny / (2i)
+    n2 = np.sin(2 * np.pi * (m * i / nx + l * j / ny))
+    B = oracle.mode_amplitudes(n2, [m, -m], [l, -l])
+    assert B[0] == pytest.approx(nx * ny / 2j, abs=1e-9) and B[1] == pytest.approx(-nx * ny / 2j, abs=1e-9)
+    rng = np.random.default_rng(7)
+    r = rng.random((nx + 1, ny))
+    per = r[:nx].copy()
+    per[0] = 0.5 * (r[0] + r[nx])
+    F = np.fft.fft2(per)
+    mxs, mys = [0, 1, 5, -2, 11], [0, 3, -1, 7, 8]
+    C = oracle.mode_amplitudes(r, mxs, mys)
+    for k in range(len(mxs)):
+        assert C[k] == pytest.approx(F[mxs[k] % nx, mys[k] % ny], abs=1e-9)
