@@ -43,6 +43,7 @@ extern "C" {
 #define PM2D_MAX_SPECIES 4
 #define PM2D_MAX_LASERS 4
 #define PM2D_MAX_MODES 16
+#define PM2D_MAX_BINS 1024
 #define PM2D_TILE 32 /* particles are binned by tiles of PM2D_TILE x PM2D_TILE cells */
 
 /* particle shape: 1-D cumulative weight G(s); weights are G differences over the control volumes
@@ -209,6 +210,14 @@ int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);
  * v_i = 1/2 on the wall columns i = 0, nx (half control volumes, Q9), 1 elsewhere; in units of n_c * cells.
  * mx, my: host int32[nmodes] (any sign), 1 <= nmodes <= PM2D_MAX_MODES; re, im: host double[nmodes].
  * float32/fixed-point input, float64 accumulation; synchronises the stream. */
+/* Velocity distribution of a species inside a sub-box (Fig. 9): hist[b] = sum of the weights
+ * w_p of the particles whose cell (ix, iy) lies in [i0, i1) x [j0, j1) and whose velocity component u (comp 0 = u_x,
+ * 1 = u_y, in c) falls into bin b = floor((u - umin) * (nbins / (umax - umin))) evaluated in float32 (u, umin and the
+ * scale rounded to float32 first); particles outside [umin, umax) are not counted.  hist: host double[nbins],
+ * 1 <= nbins <= PM2D_MAX_BINS.  Synchronises the stream.  Sums in float64; the order of the additions is not fixed. */
+int pm2d_velocity_histogram(pm2d_ctx *ctx, int species, int i0, int i1, int j0, int j1, int comp, double umin, double umax,
+                            int nbins, double *hist);
+
 int pm2d_mode_amplitudes(pm2d_ctx *ctx, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re, double *im);
 int64_t pm2d_particle_count(pm2d_ctx *ctx, int species);
 

@@ -196,6 +196,24 @@ def a_inc(laser: dict, x, y, t, Ly=1.0):
     return lib().orc_a_inc(C.byref(L), x, y, t, Ly)
 
 
+def velocity_histogram(X, Y, u, w, box, umin, umax, nbins):
+    """SURVEY 8f.4 (Fig. 9): weighted distribution of one velocity component over the particles whose cell
+    (floor X, floor Y) lies in box = (i0, i1, j0, j1).  The bin is an integer decided by floating point, so it is
+    taken in the kernel's precision (float32: u, umin and the scale nbins/(umax-umin) rounded first, then subtract,
+    multiply, floor); the sums are float64."""
+    X, Y, w = np.asarray(X, np.float64), np.asarray(Y, np.float64), np.asarray(w, np.float64)
+    i0, i1, j0, j1 = box
+    ix, iy = np.floor(X).astype(np.int64), np.floor(Y).astype(np.int64)
+    inside = (ix >= i0) & (ix < i1) & (iy >= j0) & (iy < j1)
+    u32 = np.asarray(u).astype(np.float32)
+    scale = np.float32(float(nbins) / (float(umax) - float(umin)))
+    t = np.floor((u32 - np.float32(umin)) * scale)
+    ok = inside & (t >= 0) & (t < nbins)
+    h = np.zeros(nbins)
+    np.add.at(h, t[ok].astype(np.int64), w[ok])
+    return h
+
+
 def mode_amplitudes(n, mx, my):
     """O9: Fourier-mode amplitudes of a nodal density n[(nx+1), ny], written out as the sum that
     defines them: A(mx, my) = sum_i sum_j v_i n[i, j] exp(-2 pi i (mx i/nx + my j/ny)), v_i = 1/2 on the wall columns

@@ -72,6 +72,8 @@ SYMBOLS = {
     "pm2d_set_background": (C.c_int, [_vp, C.c_int, _fp]),
     "pm2d_rebin": (C.c_int, [_vp, C.c_int, _ip, _lp]),
     "pm2d_diagnostics": (C.c_int, [_vp, C.POINTER(Diag)]),
+    "pm2d_velocity_histogram": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                         C.POINTER(C.c_double)]),
     "pm2d_mode_amplitudes": (C.c_int, [_vp, C.c_int, C.c_int, _ip, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pm2d_particle_count": (C.c_int64, [_vp, C.c_int]),
     "pm2d_profile_enable": (C.c_int, [_vp, C.c_int]),
@@ -252,6 +254,15 @@ class PM2D:
         return dict(step=d.step, time=d.time, W_es=d.W_es, W_int=d.W_int, W_em=d.W_em, W_total=d.W_total,
                     W_kin=list(d.W_kin)[: self.nsp], W_th=list(d.W_th)[: self.nsp], charge=list(d.charge)[: self.nsp],
                     count=list(d.count)[: self.nsp])
+
+    def velocity_histogram(self, species, box, comp, umin, umax, nbins):
+        """weighted histogram of u_x (comp 0) or u_y (comp 1) of the particles in the cells box = (i0, i1, j0, j1)
+        [pm2d_velocity_histogram]"""
+        h = np.zeros(int(nbins))
+        i0, i1, j0, j1 = box
+        _check(self.lib.pm2d_velocity_histogram(self.ctx, int(species), int(i0), int(i1), int(j0), int(j1), int(comp), float(umin),
+                                                float(umax), int(nbins), h.ctypes.data_as(C.POINTER(C.c_double))))
+        return h
 
     def mode_amplitudes(self, species, mx, my):
         """complex A(m_x, m_y) of the species' nodal density for the mode pairs (mx[k], my[k])  [pm2d_mode_amplitudes]"""

@@ -122,6 +122,7 @@ size_t layout(pm2d_ctx *c, char *base)
     c->phi = cv.take<float>(nn);
     c->twiddle = cv.take<float2>(g.ny / 2);
     c->red = cv.take<double>(64);
+    c->hist = cv.take<double>(PM2D_MAX_BINS);
     c->flags = cv.take<int32_t>(4);
     c->shape_y = cv.take<double>(g.ny);
     c->taper_x = cv.take<double>(g.nx);

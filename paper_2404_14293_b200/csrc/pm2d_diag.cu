@@ -132,7 +132,72 @@ __global__ void __launch_bounds__(256) k_diag_modes(const ModeParams M)
     }
 }
 
+// 8f.4: weighted velocity histogram of the particles of a sub-box; one CTA per chunk of a tile's particle list
+struct HistParams {
+    const PV *pv;
+    const float *w;
+    const int32_t *chunk_tile, *nchunks, *ptile;
+    const int64_t *chunk_beg, *tile_off;
+    int nty, ny, i0, i1, j0, j1, comp, nbins;
+    float umin, scale;
+    double *hist;
+};
+
+__global__ void __launch_bounds__(PTHREADS) k_diag_vhist(const HistParams H)
+{
+    __shared__ double sh[PM2D_MAX_BINS];
+    const int chunk = blockIdx.x;
+    if (chunk >= *H.nchunks) return;
+    for (int b = threadIdx.x; b < H.nbins; b += PTHREADS) sh[b] = 0.0;
+    __syncthreads();
+    const int ctile = H.chunk_tile[chunk];
+    const int64_t beg = H.chunk_beg[chunk];
+    int64_t end = beg + CHUNK;
+    if (H.tile_off[ctile + 1] < end) end = H.tile_off[ctile + 1];
+    for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
+        const int tile = H.ptile ? H.ptile[p] : ctile;
+        const PV me = H.pv[p];
+        const int ix = (tile / H.nty) * TILE + (int)(me.x >> POS_FRAC_BITS) - POS_BIAS;
+        const int iy = ((tile % H.nty) * TILE + (int)(me.y >> POS_FRAC_BITS) - POS_BIAS) & (H.ny - 1);
+        if (ix < H.i0 || ix >= H.i1 || iy < H.j0 || iy >= H.j1) continue;
+        const float u = H.comp ? me.uy : me.ux;
+        const float t = floorf(__fmul_rn(__fsub_rn(u, H.umin), H.scale));
+        if (!(t >= 0.f) || !(t < (float)H.nbins)) continue;
+        atomicAdd(&sh[(int)t], (double)H.w[p]);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < H.nbins; b += PTHREADS)
+        if (sh[b] != 0.0) atomicAdd(&H.hist[b], sh[b]);
+}
+
 }  // namespace
+
+extern "C" int pm2d_velocity_histogram(pm2d_ctx *c, int species, int i0, int i1, int j0, int j1, int comp, double umin, double umax,
+                                       int nbins, double *hist)
+{
+    if (!c || species < 0 || species >= c->nsp || !hist || nbins < 1 || nbins > PM2D_MAX_BINS || comp < 0 || comp > 1 ||
+        !(umax > umin) || i0 < 0 || i1 > c->g.nx || i0 >= i1 || j0 < 0 || j1 > c->g.ny || j0 >= j1) {
+        pm2d_set_error("pm2d_velocity_histogram: bad argument");
+        return PM2D_EINVAL;
+    }
+    SpeciesDev &S = c->sp[species];
+    for (int b = 0; b < nbins; b++) hist[b] = 0.0;
+    if (!S.cfg.mobile || S.np == 0) return PM2D_OK;
+    HistParams H;
+    H.pv = S.pv; H.w = S.w; H.chunk_tile = S.chunk_tile; H.nchunks = S.nchunks_dev; H.ptile = S.random ? S.ptile : nullptr;
+    H.chunk_beg = S.chunk_beg; H.tile_off = S.tile_off;
+    H.nty = c->nty; H.ny = c->g.ny; H.i0 = i0; H.i1 = i1; H.j0 = j0; H.j1 = j1; H.comp = comp; H.nbins = nbins;
+    H.umin = (float)umin;
+    H.scale = (float)((double)nbins / (umax - umin));
+    H.hist = c->hist;
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->hist, 0, (size_t)nbins * sizeof(double), c->stream));
+    k_diag_vhist<<<S.max_chunks, PTHREADS, 0, c->stream>>>(H);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(hist, c->hist, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return PM2D_OK;
+}
 
 extern "C" int pm2d_mode_amplitudes(pm2d_ctx *c, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re,
                                     double *im)

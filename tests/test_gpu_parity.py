@@ -663,3 +663,34 @@ def test_mode_amplitudes_parity(P):
     with pytest.raises(P.PM2DError):
         sim.mode_amplitudes(0, list(range(17)), list(range(17)))
     sim.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("order", [0, 3], ids=["auto", "random"])
+def test_velocity_histogram_parity(P, order):
+    """8f.4: pm2d_velocity_histogram against the oracle's definition.  (1) On the device's own particles (canonical
+    form read back) every bin decision is the same float32 expression: sums agree to rounding.  (2) Against the
+    oracle's particles after 5 steps of the reduced c3 config: velocities differ by ~1e-7 relative, so only
+    particles within that distance of an edge may change bins."""
+    cfg = small_cfg("c3", 72, 64)
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=2, particle_order=order)
+    orc, _ = oracle_from_config(cfg)
+    sim.step(5)
+    orc.step(5)
+    box = (8, 60, 5, 50)
+    for s, (lo, hi, nb) in enumerate([(-0.3, 0.3, 128), (-4e-3, 4e-3, 1000)]):
+        for comp, key in ((0, "ux"), (1, "uy")):
+            h = sim.velocity_histogram(s, box, comp, lo, hi, nb)
+            got = sim.get_particles(s)
+            own = oracle.velocity_histogram(got["ix"] + got["fx"].astype(np.float64), got["iy"] + got["fy"].astype(np.float64),
+                                            got[key], got["w"], box, lo, hi, nb)
+            assert np.abs(h - own).max() <= 1e-12 * max(own.max(), 1e-30), (s, comp)
+            assert own.sum() > 0
+            d = orc.sp[s]
+            ref = oracle.velocity_histogram(d["X"], d["Y"], d[key], d["w"], box, lo, hi, nb)
+            assert np.abs(h - ref).sum() <= 2e-3 * ref.sum(), (s, comp, np.abs(h - ref).sum() / ref.sum())
+    with pytest.raises(P.PM2DError):
+        sim.velocity_histogram(0, box, 0, 0.1, 0.1, 16)
+    with pytest.raises(P.PM2DError):
+        sim.velocity_histogram(0, box, 0, -1.0, 1.0, 2000)
+    sim.close()

@@ -224,3 +224,31 @@ def test_P17_mode_amplitudes_closed_form_and_fft():
     C = oracle.mode_amplitudes(r, mxs, mys)
     for k in range(len(mxs)):
         assert C[k] == pytest.approx(F[mxs[k] % nx, mys[k] % ny], abs=1e-9)
+
+
+def test_P18_velocity_histogram_of_a_maxwellian_and_a_box():
+    """The histogram of 4e5 seeded normal velocities follows the Gaussian bin integrals within counting noise; the
+    box selects by cell; the total weight inside [umin, umax) is conserved; numpy's histogram agrees where no value
+    sits on a float32 bin edge."""
+    rng = np.random.default_rng(3)
+    N, vth = 400000, 0.05
+    X, Y = rng.random(N) * 40, rng.random(N) * 16
+    u = (vth * rng.standard_normal(N)).astype(np.float32)
+    w = np.full(N, 0.25)
+    nb, lo, hi = 64, -0.2, 0.2
+    h = oracle.velocity_histogram(X, Y, u, w, (0, 40, 0, 16), lo, hi, nb)
+    assert h.sum() == pytest.approx(0.25 * ((u >= lo) & (u < hi)).sum(), rel=1e-12)
+    edges = np.linspace(lo, hi, nb + 1)
+    cdf = np.array([0.5 * (1 + math.erf(e / (vth * math.sqrt(2)))) for e in edges])
+    expect = N * 0.25 * np.diff(cdf)
+    big = expect > 200
+    assert np.abs(h[big] / expect[big] - 1).max() < 5 * np.sqrt(1.0 / (4 * expect[big].min()))
+    ref, _ = np.histogram(u.astype(np.float64), bins=nb, range=(lo, hi), weights=w)
+    assert np.abs(h - ref).sum() <= 0.25 * 4                      # at most a few values on a rounded edge
+    sub = oracle.velocity_histogram(X, Y, u, w, (10, 20, 4, 8), lo, hi, nb)
+    sel = (np.floor(X) >= 10) & (np.floor(X) < 20) & (np.floor(Y) >= 4) & (np.floor(Y) < 8) & (u >= lo) & (u < hi)
+    assert sub.sum() == pytest.approx(0.25 * sel.sum(), rel=1e-12)
+    # a single particle: bin 3 of 8 on [0, 0.8) holds u = 0.35
+    one = oracle.velocity_histogram([1.5], [2.5], [0.35], [2.0], (1, 2, 2, 3), 0.0, 0.8, 8)
+    assert list(one) == [0, 0, 0, 2.0, 0, 0, 0, 0]
+    assert oracle.velocity_histogram([1.5], [2.5], [0.35], [2.0], (2, 3, 2, 3), 0.0, 0.8, 8).sum() == 0.0
