@@ -15,44 +15,62 @@ struct NeSrc {
     float inv_nscale;
 };
 
-__device__ __forceinline__ float ne_at(const NeSrc &S, size_t k)
+// Eq. 6.  CTA = 128 threads x 4 columns x FROWS rows; each thread marches along x keeping a[i-1], a[i], a[i+1] of its
+// four columns in registers (128-bit loads and stores); the two outer y neighbours come from the same cache lines
+// through L1.  ny is a power of two >= 8, so a thread's four columns never wrap.
+constexpr int FCOLS = 128, FVEC = 4, FROWS = 32, FBATCH = 2;
+
+__device__ __forceinline__ float4 ne_at4(const NeSrc &S, size_t k)
 {
-    int v = 0;
-    for (int s = 0; s < S.count; s++) v += S.n[s][k];
-    return (float)v * S.inv_nscale;
+    int4 v = make_int4(0, 0, 0, 0);
+    for (int s = 0; s < S.count; s++) {
+        const int4 t = *reinterpret_cast<const int4 *>(S.n[s] + k);
+        v.x += t.x; v.y += t.y; v.z += t.z; v.w += t.w;
+    }
+    return make_float4((float)v.x * S.inv_nscale, (float)v.y * S.inv_nscale, (float)v.z * S.inv_nscale, (float)v.w * S.inv_nscale);
 }
 
-// Eq. 6.  CTA = 128 columns x ROWS rows; each thread marches along x keeping a[i-1], a[i], a[i+1]
-// in registers; the y neighbours come from the same cache lines through L1.
-constexpr int FCOLS = 128, FROWS = 32, FBATCH = 4;
+__device__ __forceinline__ float wave_node(float hi, float mid, float lo, float l, float r, float old, float den, float cx, float cy,
+                                           float dt2)
+{
+    const float lap = cx * (hi - 2.f * mid + lo) + cy * (r - 2.f * mid + l);
+    const float src = FOUR_PI2 * den * mid;
+    return 2.f * mid - old + dt2 * (lap - src);
+}
+
 __global__ void __launch_bounds__(FCOLS) k_wave(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap,
                                                 NeSrc ne, int nx, int ny, float cx, float cy, float dt2)
 {
-    const int j = blockIdx.x * FCOLS + threadIdx.x;
+    const int j = (blockIdx.x * FCOLS + threadIdx.x) * FVEC;
     if (j >= ny) return;
     const int i0 = 1 + blockIdx.y * FROWS, i1 = min(nx, i0 + FROWS);   // interior rows i0 .. i1-1
     if (i0 >= i1) return;
-    const int jm = (j - 1) & (ny - 1), jp = (j + 1) & (ny - 1);
-    float lo = a[(size_t)(i0 - 1) * ny + j], mid = a[(size_t)i0 * ny + j];
+    const int jm = (j - 1) & (ny - 1), jp = (j + FVEC) & (ny - 1);
+    float4 lo = *reinterpret_cast<const float4 *>(a + (size_t)(i0 - 1) * ny + j);
+    float4 mid = *reinterpret_cast<const float4 *>(a + (size_t)i0 * ny + j);
     for (int ib = i0; ib < i1; ib += FBATCH) {
         // the loads of FBATCH rows are issued together: the march itself is a chain of dependent rows
-        float hi[FBATCH], l[FBATCH], r[FBATCH], old[FBATCH], den[FBATCH];
+        float4 hi[FBATCH], old[FBATCH], den[FBATCH];
+        float l[FBATCH], r[FBATCH];
 #pragma unroll
         for (int u = 0; u < FBATCH; u++) {
             const size_t row = (size_t)min(ib + u, i1 - 1) * ny;
-            hi[u] = a[row + ny + j];
+            hi[u] = *reinterpret_cast<const float4 *>(a + row + ny + j);
             l[u] = a[row + jm];
             r[u] = a[row + jp];
-            old[u] = am[row + j];
-            den[u] = ne_at(ne, row + j);
+            old[u] = *reinterpret_cast<const float4 *>(am + row + j);
+            den[u] = ne_at4(ne, row + j);
         }
 #pragma unroll
         for (int u = 0; u < FBATCH; u++) {
             if (ib + u < i1) {
                 const size_t row = (size_t)(ib + u) * ny;
-                float lap = cx * (hi[u] - 2.f * mid + lo) + cy * (r[u] - 2.f * mid + l[u]);
-                float src = FOUR_PI2 * den[u] * mid;
-                ap[row + j] = 2.f * mid - old[u] + dt2 * (lap - src);
+                float4 o;
+                o.x = wave_node(hi[u].x, mid.x, lo.x, l[u], mid.y, old[u].x, den[u].x, cx, cy, dt2);
+                o.y = wave_node(hi[u].y, mid.y, lo.y, mid.x, mid.z, old[u].y, den[u].y, cx, cy, dt2);
+                o.z = wave_node(hi[u].z, mid.z, lo.z, mid.y, mid.w, old[u].z, den[u].z, cx, cy, dt2);
+                o.w = wave_node(hi[u].w, mid.w, lo.w, mid.z, r[u], old[u].w, den[u].w, cx, cy, dt2);
+                *reinterpret_cast<float4 *>(ap + row + j) = o;
                 lo = mid;
                 mid = hi[u];
             }
@@ -293,7 +311,7 @@ int launch_field_step(pm2d_ctx *c, int sub)
         oblique = oblique || Q.oblique;
     }
     O.t_now = t_now; O.dt = dt; O.dx = dx; O.Ly = ny * dy; O.inv_Ly = 1.0 / (ny * dy);
-    dim3 grid((ny + FCOLS - 1) / FCOLS, (nx - 1 + FROWS - 1) / FROWS);
+    dim3 grid((ny + FCOLS * FVEC - 1) / (FCOLS * FVEC), (nx - 1 + FROWS - 1) / FROWS);
     for (int comp = 0; comp < c->g.ncomp; comp++) {
         const size_t off = (size_t)comp * c->nn;
         k_wave<<<grid, FCOLS, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, ne, nx, ny, (float)(1.0 / (dx * dx)),
