@@ -439,9 +439,10 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     sim.close()
 
 
-@pytest.mark.parametrize("name", ["c4", "c5"])
+@pytest.mark.parametrize("name", ["c4", "c5", "cbet"])
 def test_full_size_c4_c5_sampled_deposit_parity(P, name):
-    """BASELINE.json configs 4 (16384 x 8192, 403 M particles, Gaussian beam, ny = 8192 FFT path) and 5 (4096 x 4096,
+    """(cbet: the second workload of bench.py, 8192 x 8192, particle step = 5 wave steps, same checks.)
+    BASELINE.json configs 4 (16384 x 8192, 403 M particles, Gaussian beam, ny = 8192 FFT path) and 5 (4096 x 4096,
     9.4e8 number-weighted electrons in a filament, cell-major order + strip kernel) at full size, in the launch
     configuration bench.py times.  After 3 steps: counts and charge conserved, and on a sample of the grid -- 17 node
     rows in the middle of the box, every column -- the deposited n, Px, Py equal the oracle's deposit of the device's
