@@ -362,9 +362,9 @@ def test_poisson_partition_edge_cases(P, nx, ny):
 def test_srs_growth_rate_parity(P):
     """Run-level parity (BASELINE.json: 'the linear SRS growth rate'): the quasi-1D SRS slab of the paper's
     section 6.1 on the GPU and in the oracle from identical particles; the backscatter envelope at the left
-    boundary must rise at the same rate.  The instability amplifies the fp32 / fp64 rounding difference of
-    the seed, so the two envelopes are shifted in time by ~1 T0 and their fitted rates agree to a few per cent,
-    not to BJ's 2 % (measured 2.5-5 %): asserted 7 %."""
+    boundary must rise at the same rate, within BJ's 2 % (measured 0.6 %: 0.1311 against 0.1319 per T0; the
+    two envelopes cross 1e-3 within 0.1 T0 of each other).  The run is deterministic on the device (integer deposits,
+    stable rebin), so the figure does not vary from run to run."""
     from helpers import srs_slab, srs_oracle, backscatter_growth_rate
     nx, ny, nsteps, dt, dx = 1600, 8, 6400, 0.035, 0.05
     parts = srs_slab(nx, ny)
@@ -391,7 +391,7 @@ def test_srs_growth_rate_parity(P):
     early = slice(0, int(100 / dt))
     assert np.abs(sg[early] - so[early]).max() < 2e-4 * 0.06
     rg, ro = backscatter_growth_rate(t, sg - inc), backscatter_growth_rate(t, so - inc)
-    assert rg == pytest.approx(ro, rel=0.07), (rg, ro)
+    assert rg == pytest.approx(ro, rel=0.02), (rg, ro)
     sim.close()
 
 
