@@ -31,6 +31,7 @@ def build(force: bool = False) -> str:
 
 class _Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("subcycle", C.c_int32),
+                ("bc_y", C.c_int32), ("pad_", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -130,8 +131,8 @@ def weights_1d(shape: int, DD: float, xp: float):
     return first, W[: cnt.value]
 
 
-def make_grid(nx, ny, dx, dy, dt, ncomp=1, subcycle=1):
-    return _Grid(nx, ny, ncomp, subcycle, dx, dy, dt)
+def make_grid(nx, ny, dx, dy, dt, ncomp=1, subcycle=1, bc_y=0):
+    return _Grid(nx, ny, ncomp, subcycle, bc_y, 0, dx, dy, dt)
 
 
 def deposit(g: _Grid, shape, DD, X, Y, ux, uy, w):
@@ -236,11 +237,11 @@ class Oracle:
     species: list of dicts with keys mass, sign, T_keV, C (pressure_coeff), shape, DD, mobile and
     particle arrays X, Y (cell units), ux, uy, w; an immobile species may instead give ``n_fixed``
     (nodal density, shape (nx+1, ny)).  lasers: list of dicts (a0, omega, y0, w0, t_rise, alpha [rad], comp).
-    subcycle: wave-equation steps of dt per particle step (Q21).
+    subcycle: wave-equation steps of dt per particle step (Q21).  bc_y: 0 periodic, 1 absorbing y walls for a (Q23).
     """
 
-    def __init__(self, nx, ny, dx, dy, dt, species, lasers=(), ncomp=1, subcycle=1):
-        self.g = make_grid(nx, ny, dx, dy, dt, ncomp, subcycle)
+    def __init__(self, nx, ny, dx, dy, dt, species, lasers=(), ncomp=1, subcycle=1, bc_y=0):
+        self.g = make_grid(nx, ny, dx, dy, dt, ncomp, subcycle, bc_y)
         self.nn = nn = (nx + 1) * ny
         self.a = [np.zeros(ncomp * nn) for _ in range(3)]       # new, now, old
         self.rho, self.phi = np.zeros(nn), np.zeros(nn)

@@ -32,6 +32,8 @@ typedef struct {
     int32_t nx, ny;      /* cells; nodes are (nx+1) x ny */
     int32_t ncomp;       /* active components of a (1..3) */
     int32_t subcycle;    /* S: the particle step is S wave-equation steps long (Q21); 0, 1 = none */
+    int32_t bc_y;        /* boundary condition of a at the y walls: 0 periodic (BJ configs), 1 absorbing (Q23) */
+    int32_t pad_;
     double dx, dy, dt;   /* dt: time step of the wave equation */
 } orc_grid;
 
@@ -271,6 +273,29 @@ void orc_field_step(orc_state *S, const double *ne, double t_now)
                 ap[r0 + j] = (alpha * (ap[r1 + j] - am[r1 + j] + am[r0 + j]) -
                               beta * (ap[r1 + j] + am[r1 + j] + am[r0 + j] - 2.0 * a[r0 + j] - 2.0 * a[r1 + j]) +
                               gam * (E0 + E1)) / (alpha + beta);
+            }
+        }
+        if (S->g.bc_y == 1) {
+            /* "the second-order absorbing boundary condition ... on all of four boundaries": Eq. 8 with the
+             * roles of x and y exchanged on the walls j = 0 and j = ny-1 (no incident wave there), for i = 1..nx-1;
+             * it overwrites what the periodic stencil and the x-wall loop above left in those two columns.  The
+             * corners are not treated by the paper: first-order outgoing condition along the diagonal (Q23).   */
+            const double alpha_y = 1.0 / (2.0 * dt * dy), gam_x = 1.0 / (4.0 * dx * dx);
+            const double hd = sqrt(dx * dx + dy * dy), kap = (dt - hd) / (dt + hd);
+            int side;
+            for (side = 0; side < 2; side++) {
+                const int j0 = side ? ny - 1 : 0, j1 = side ? ny - 2 : 1;
+                for (i = 1; i < nx; i++) {
+                    int64_t k0 = (int64_t)i * ny + j0, k1 = (int64_t)i * ny + j1;
+                    double D0 = a[k0 + ny] - 2.0 * a[k0] + a[k0 - ny];
+                    double D1 = a[k1 + ny] - 2.0 * a[k1] + a[k1 - ny];
+                    ap[k0] = (alpha_y * (ap[k1] - am[k1] + am[k0]) -
+                              beta * (ap[k1] + am[k1] + am[k0] - 2.0 * a[k0] - 2.0 * a[k1]) + gam_x * (D0 + D1)) /
+                             (alpha_y + beta);
+                }
+                /* corners: a_c^{n+1} = a_d^n + kappa (a_d^{n+1} - a_c^n), d the diagonal neighbour */
+                ap[j0] = a[ny + j1] + kap * (ap[ny + j1] - a[j0]);
+                ap[(int64_t)nx * ny + j0] = a[(int64_t)(nx - 1) * ny + j1] + kap * (ap[(int64_t)(nx - 1) * ny + j1] - a[(int64_t)nx * ny + j0]);
             }
         }
     }

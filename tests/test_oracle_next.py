@@ -252,3 +252,52 @@ def test_P18_velocity_histogram_of_a_maxwellian_and_a_box():
     one = oracle.velocity_histogram([1.5], [2.5], [0.35], [2.0], (1, 2, 2, 3), 0.0, 0.8, 8)
     assert list(one) == [0, 0, 0, 2.0, 0, 0, 0, 0]
     assert oracle.velocity_histogram([1.5], [2.5], [0.35], [2.0], (2, 3, 2, 3), 0.0, 0.8, 8).sum() == 0.0
+
+
+# ---- S§8(f).2: absorbing y walls for a ("on all of four boundaries"; Q23) ------------------------------
+def _vac(nx, ny, dx, dt, bc_y, lasers=()):
+    sp = [dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, shape=oracle.CIC, DD=1.0, n_fixed=np.zeros((nx + 1, ny)))]
+    return oracle.Oracle(nx, ny, dx, dx, dt, sp, lasers, bc_y=bc_y)
+
+
+def test_P19_four_absorbing_walls_let_a_ring_out():
+    """A wave packet at rest in the middle of a square vacuum box splits into an outgoing ring.  With absorbing y
+    walls it leaves through all four sides and the corners: under 0.5 % of the field energy is left once the ring
+    has passed the corners; in the y-periodic box the part that crossed the y walls comes back in and stays."""
+    nx, ny, dx, dt = 127, 128, 0.05, 0.035                 # 128 x 128 nodes (ny: a power of two for the Poisson FFT)
+    x = np.arange(nx + 1)[:, None] * dx
+    y = np.arange(ny)[None, :] * dx
+    r2 = (x - 3.175) ** 2 + (y - 3.175) ** 2
+    blob = np.exp(-r2 / 0.6 ** 2) * np.cos(2 * math.pi * np.sqrt(r2))
+    left = {}
+    for bc in (0, 1):
+        o = _vac(nx, ny, dx, dt, bc)
+        o.a_now[0][:] = blob
+        o.a_old[0][:] = blob
+        e0 = o.energies()["W_em"]
+        o.step(int(7.5 / dt))                    # half diagonal 4.5 + packet
+        left[bc] = o.energies()["W_em"] / e0
+    assert left[1] < 5e-3
+    assert left[0] > 0.2
+
+
+def test_P19_y_wall_transmits_an_oblique_beam():
+    """A Gaussian beam aimed at the lower y wall (alpha = +30 degrees: axis (cos, -sin)) crosses it: with the absorbing
+    wall the upper half of the box stays dark (reflection coefficient of the second-order condition at 60 degrees
+    from the wall normal: ((1 - cos 60)/(1 + cos 60))^2 = 1/9 in amplitude, 1.2 % in energy; measured against the
+    periodic box, where the beam re-enters through the upper wall)."""
+    nx, ny, dx, dt = 200, 128, 0.05, 0.035
+    las = [dict(a0=0.01, t_rise=2.0, alpha=math.radians(30.0), y0=2.2, w0=0.9)]
+    up = {}
+    for bc in (0, 1):
+        o = _vac(nx, ny, dx, dt, bc, las)
+        o.step(int(20.0 / dt))
+        acc = np.zeros((nx + 1, ny))
+        for _ in range(int(round(1.0 / dt))):
+            o.step()
+            acc += o.a_now[0] ** 2
+        # the beam meets the wall y = 0 near x' = 2.2 / tan(30) = 3.8; beyond x' = 5 everything above mid-height is
+        # either reflected or re-entered light
+        up[bc] = acc[100:, ny // 2:].sum() / acc.sum()
+    assert up[0] > 0.2                      # periodic: the beam comes back in from above
+    assert up[1] < 0.02                     # absorbing: only the reflected part
