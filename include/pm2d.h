@@ -75,6 +75,7 @@ enum {
  * positions stay relative to the tile a particle was loaded into: a run may drift at most 64 cells from it, else
  * PM2D_ESTATE), pm2d_rebin and pm2d_set_particles return PM2D_ESTATE.  It exists to measure what the sort buys. */
 enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2, PM2D_ORDER_RANDOM = 3 };
+enum { PM2D_BC_Y_PERIODIC = 0, PM2D_BC_Y_ABSORB = 1 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 
 /* The edge taper ends at 1 % of the profile: macro-particles of neighbouring cells must not differ in weight by
@@ -97,6 +98,12 @@ typedef struct {
                               for updating the particle motion is five times larger" (Q21).
                               One pm2d_step is then S steps of Eq. 6/8 with n_e held, and Eqs. 17/19 with S*dt;
                               S*dt/min(dx,dy) <= 4                                                    */
+    int32_t bc_y;          /* PM2D_BC_Y_PERIODIC (BASELINE.json configs) | PM2D_BC_Y_ABSORB: "the second-order absorbing
+                              boundary condition ... on all of four boundaries": Eq. 8 with x and
+                              y exchanged on the walls j = 0 and j = ny-1 of `a`, first-order outgoing condition along
+                              the diagonal at the four corners (Q23).  Particles, densities, Poisson and the
+                              force grid stay periodic in y                                           */
+    int32_t reserved;      /* must be 0                                                               */
     double dx, dy, dt;     /* lambda0, lambda0, T0; dt = step of the wave equation,
                               dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1                     */
 } pm2d_grid;

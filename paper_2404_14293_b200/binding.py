@@ -20,6 +20,7 @@ LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
 PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
 FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
+BC_Y_PERIODIC, BC_Y_ABSORB = 0, 1
 ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, ORDER_RANDOM, LAYERS = 0, 1, 2, 3, 16
 PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 
@@ -27,6 +28,7 @@ PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("rebin_every", C.c_int32),
                 ("eager_moments", C.c_int32), ("track_ids", C.c_int32), ("particle_order", C.c_int32), ("subcycle", C.c_int32),
+                ("bc_y", C.c_int32), ("reserved", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -125,7 +127,8 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, part
     """Translate a pm2d_inputs-style config dict into the C structs."""
     g = cfg["grid"]
     grid = Grid(g["nx"], g["ny"], g.get("ncomp", 1), g.get("rebin_every", 8) if rebin_every is None else rebin_every,
-                int(eager_moments), int(track_ids), int(particle_order), int(g.get("subcycle", 1)), g["dx"], g["dy"], g["dt"])
+                int(eager_moments), int(track_ids), int(particle_order), int(g.get("subcycle", 1)),
+                int(g.get("bc_y", 0)), 0, g["dx"], g["dy"], g["dt"])
     sp = (Species * len(cfg["species"]))()
     for k, s in enumerate(cfg["species"]):
         sp[k] = Species(s["mass"], s["T_keV"], s["pressure_coeff"], s["DD"], s["sign"], s["shape"], s["mobile"], s["load"],

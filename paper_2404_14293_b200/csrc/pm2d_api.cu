@@ -78,6 +78,8 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (g->subcycle < 0 || g->subcycle > 16) return fail(PM2D_EINVAL, "subcycle must be 0..16");
     if (g->subcycle > 1 && (g->subcycle * g->dt / g->dx > 4.0 || g->subcycle * g->dt / g->dy > 4.0))
         return fail(PM2D_EINVAL, "subcycle*dt/dx must be <= 4");
+    if (g->bc_y != PM2D_BC_Y_PERIODIC && g->bc_y != PM2D_BC_Y_ABSORB) return fail(PM2D_EINVAL, "unknown bc_y");
+    if (g->reserved != 0) return fail(PM2D_EINVAL, "pm2d_grid.reserved must be 0");
     for (int s = 0; s < nsp; s++) {
         const pm2d_species &q = sp[s];
         if (!(q.mass > 0)) return fail(PM2D_EINVAL, "species mass must be positive");

@@ -1,6 +1,7 @@
 // pm2d_fields.cu -- mesh kernels of libpm2d.so (sm_100a):
 //   * wave equation, Eq. 6: x-marching register stencil, one thread per column j
 //   * x-boundary absorbing condition Eq. 8 with laser injection (Eq. 4)
+//   * optional absorbing y walls and corners (Q23)
 //   * nodal fluid force, Eq. 16 / 18
 //   * small conversions between the fixed-point deposit grids and float
 #include "pm2d_internal.h"
@@ -178,6 +179,34 @@ __global__ void k_boundary(const float *__restrict__ a, const float *__restrict_
     }
 }
 
+// Absorbing y walls (pm2d_grid.bc_y = PM2D_BC_Y_ABSORB; "on all of four boundaries", Q23): Eq. 8 with
+// the roles of x and y exchanged on the wall columns j = 0 and j = ny-1, rows 1..nx-1, no incident wave; then the four
+// corners by the first-order outgoing condition along the diagonal.  Runs after k_wave and k_boundary and overwrites
+// what their periodic stencils left in the two wall columns.  One thread per (row, wall); the wall columns are ny
+// floats apart, so every access is its own sector: 2 (nx-1) nodes x 14 sectors, microseconds at any BJ size.
+struct BcYParams {
+    float alpha_y, beta, gam_x, kap;   // 1/(2 dt dy), 1/(2 dt^2), 1/(4 dx^2), (dt - hd)/(dt + hd), hd = sqrt(dx^2 + dy^2)
+};
+__global__ void k_boundary_y(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap, BcYParams B, int nx,
+                             int ny)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 0..nx
+    const int side = blockIdx.y;
+    if (i > nx) return;
+    const int j0 = side ? ny - 1 : 0, j1 = side ? ny - 2 : 1;
+    if (i == 0 || i == nx) {
+        // corner c, diagonal neighbour d: a_c^{n+1} = a_d^n + kappa (a_d^{n+1} - a_c^n)
+        const size_t kc = (size_t)i * ny + j0, kd = (size_t)(i == 0 ? 1 : nx - 1) * ny + j1;
+        ap[kc] = a[kd] + B.kap * (ap[kd] - a[kc]);
+        return;
+    }
+    const size_t k0 = (size_t)i * ny + j0, k1 = (size_t)i * ny + j1;
+    const float D0 = a[k0 + ny] - 2.f * a[k0] + a[k0 - ny];
+    const float D1 = a[k1 + ny] - 2.f * a[k1] + a[k1 - ny];
+    ap[k0] = (B.alpha_y * (ap[k1] - am[k1] + am[k0]) - B.beta * (ap[k1] + am[k1] + am[k0] - 2.f * a[k0] - 2.f * a[k1]) +
+              B.gam_x * (D0 + D1)) / (B.alpha_y + B.beta);
+}
+
 // Eq. 16 / 18 on the nodes.  E arrives already averaged to the nodes (Q3; pm2d_poisson.cu).
 struct ForceParams {
     const float2 *Enode;
@@ -319,6 +348,16 @@ int launch_field_step(pm2d_ctx *c, int sub)
         if (oblique) k_boundary<true><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
         else k_boundary<false><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
         count_launch(c, 2);
+        if (c->g.bc_y == PM2D_BC_Y_ABSORB) {
+            BcYParams Y;
+            const double hd = sqrt(dx * dx + dy * dy);
+            Y.alpha_y = (float)(1.0 / (2.0 * dt * dy));
+            Y.beta = B.beta;
+            Y.gam_x = (float)(1.0 / (4.0 * dx * dx));
+            Y.kap = (float)((dt - hd) / (dt + hd));
+            k_boundary_y<<<dim3((nx + 1 + 127) / 128, 2), 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, Y, nx, ny);
+            count_launch(c, 1);
+        }
     }
     PM2D_CUDA_CHECK(cudaGetLastError());
     return PM2D_OK;

@@ -46,7 +46,7 @@ def oracle_from_config(cfg, particles=None):
     lasers = [dict(a0=l["a0"], omega=l["omega"], y0=l["y0"], w0=l["w0"], t_rise=l["t_rise"], comp=l["comp"],
                    alpha=l.get("alpha", 0.0)) for l in cfg["lasers"]]
     return oracle.Oracle(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], species, lasers, g["ncomp"],
-                         subcycle=g.get("subcycle", 1)), particles
+                         subcycle=g.get("subcycle", 1), bc_y=g.get("bc_y", 0)), particles
 
 
 # ---- quasi-1D SRS slab (paper section 6.1: a0 = 0.06, 0.15 n_c, dx = 0.05, dt = 0.035, 1 particle per cell,

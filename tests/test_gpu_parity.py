@@ -695,3 +695,80 @@ def test_velocity_histogram_parity(P, order):
     with pytest.raises(P.PM2DError):
         sim.velocity_histogram(0, box, 0, -1.0, 1.0, 2000)
     sim.close()
+
+
+# ---- S§8(f).2: absorbing y walls and corners for a (pm2d_grid.bc_y = PM2D_BC_Y_ABSORB, Q23) ----------
+def _vacuum_cfg(nx, ny, dx, dt, bc_y, lasers=(), ncomp=1):
+    sp = [dict(sign=-1, mass=1.0, T_keV=0.0, pressure_coeff=0.0, ppc_x=0, ppc_y=0, mobile=0, shape=I.CIC, DD=1.0, load=I.LOAD_NONE),
+          dict(sign=1, mass=1836.0, T_keV=0.0, pressure_coeff=0.0, ppc_x=0, ppc_y=0, mobile=0, shape=I.CIC, DD=1.0, load=I.LOAD_NONE)]
+    return dict(grid=dict(nx=nx, ny=ny, dx=dx, dy=dx, dt=dt, ncomp=ncomp, rebin_every=8, bc_y=bc_y), seed=0, steps=1, name="vacuum",
+                profile=dict(kind=I.PROFILE_UNIFORM, p=[0.0, 0, 0, 0], taper_cells=0), species=sp, lasers=list(lasers))
+
+
+@pytest.mark.gpu
+def test_absorbing_y_walls_ring_leaves_the_box_parity(P):
+    """The set-up of pin P19 on the device: a wave packet at rest in a square vacuum box (129 x 128 nodes: ragged in x
+    for the 32-row CTAs of k_wave) leaves through all four walls and the corners.  Element by element against the
+    oracle while the ring crosses the walls (all nodes, wall columns and corners included), then the energy left."""
+    nx, ny, dx, dt = 128, 128, 0.05, 0.035
+    x = np.arange(nx + 1)[:, None] * dx
+    y = np.arange(ny)[None, :] * dx
+    r2 = (x - 3.2) ** 2 + (y - 3.175) ** 2
+    blob = (np.exp(-r2 / 0.6 ** 2) * np.cos(2 * math.pi * np.sqrt(r2))).astype(np.float32)
+    cfg = _vacuum_cfg(nx, ny, dx, dt, 1)
+    sim = P.PM2D(cfg, eager_moments=1)
+    orc, _ = oracle_from_config(cfg)
+    for lvl in (0, 1):
+        sim.set_fields(P.FIELD_A, 0, lvl, blob)
+    orc.a_now[0][:] = blob
+    orc.a_old[0][:] = blob
+    e0 = orc.energies()["W_em"]
+    amp = float(np.abs(blob).max())
+    for blk in range(5):
+        sim.step(43)
+        orc.step(43)
+        a = sim.get_fields(P.FIELD_A, 0, 0)
+        d = np.abs(a - orc.a_now[0])
+        assert d.max() < 2e-5 * amp, (blk, d.max())
+        for jw in (0, ny - 1):                                   # the walls and the corners themselves
+            assert d[:, jw].max() < 2e-5 * amp, (blk, jw)
+    assert orc.energies()["W_em"] / e0 < 5e-3
+    assert sim.diagnostics()["W_em"] / e0 < 5e-3
+    sim.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ncomp", [1, 3])
+def test_absorbing_y_walls_with_plasma_and_oblique_beam_parity(P, ncomp):
+    """The c1 slab (reduced) with absorbing y walls, driven by a Gaussian beam aimed at the lower wall (alpha = +25
+    degrees) and, with three components, a second beam in a_x aimed at the upper wall: 240 steps, the beams cross the
+    walls inside the plasma; a and the electron density stay with the oracle."""
+    cfg = small_cfg("c1", 96, 64, bc_y=1, ncomp=ncomp)
+    Ly = 64 * cfg["grid"]["dy"]
+    cfg["lasers"] = [dict(a0=0.02, omega=1.0, y0=0.4 * Ly, w0=0.25 * Ly, alpha=math.radians(25.0), comp=0, t_rise=1.5)]
+    if ncomp == 3:
+        cfg["lasers"].append(dict(a0=0.015, omega=1.0, y0=0.6 * Ly, w0=0.2 * Ly, alpha=math.radians(-20.0), comp=2, t_rise=1.0))
+    sim = P.PM2D(cfg, eager_moments=1, rebin_every=8)
+    orc, _ = oracle_from_config(cfg)
+    for blk in range(4):
+        sim.step(60)
+        orc.step(60)
+        for c in range(ncomp):
+            a = sim.get_fields(P.FIELD_A, c, 0)
+            scale = max(np.abs(orc.a_now[0]).max(), 1e-30)
+            assert np.abs(a - orc.a_now[c]).max() < 5e-5 * scale + 1e-9, (blk, c)
+    assert np.abs(orc.a_now[0][:, 0]).max() > 1e-3               # the beam is on the lower wall
+    assert rel_l2(sim.get_moments(0, P.MOMENT_N), orc.moment(0, "n")) < 1e-5
+    # and the wall matters: the periodic run differs from this one by orders of magnitude more than the tolerance
+    per = P.PM2D(dict(cfg, grid=dict(cfg["grid"], bc_y=0)), eager_moments=1, rebin_every=8)
+    per.step(240)
+    assert np.abs(per.get_fields(P.FIELD_A, 0, 0) - sim.get_fields(P.FIELD_A, 0, 0)).max() > 1e-2 * scale
+    per.close()
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_bc_y_is_validated(P):
+    cfg = small_cfg("c1", 96, 64, bc_y=2)
+    with pytest.raises(P.PM2DError):
+        P.PM2D(cfg)
