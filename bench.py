@@ -219,7 +219,7 @@ def run_cuda(args):
                                          + (f"(BASELINE.json configs[{int(args.config[1]) - 1}])" if args.config != "cbet" else
                                             "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)"),
                                 shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
-                                eager_moments=bool(args.eager), subcycle=int(g.get("subcycle", 1)), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
+                                eager_moments=bool(args.eager), subcycle=int(g.get("subcycle", 1)), bc_y=("absorbing" if g.get("bc_y", 0) else "periodic"), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
                                 l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
                                 parallelism="replicas only" if world > 1 else "1 GPU"),
                     ns_per_particle_step=1e9 / value * world,

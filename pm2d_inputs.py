@@ -225,9 +225,10 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     elif name == "cbet":  # S§8(f).1, the paper's CBET run: 8000x8000 there, 8192x8192 here (ny a power of two);
         # 0.4 n_c hydrogen slab (the standard edge taper stands in for the 20 lambda0 vacuum margins), 1 e + 1 ion per
         # cell, 1 keV / 200 eV, DD = 1.85 dx, two beams a0 = 0.008 at +-15 degrees, lambda0 and 0.9995 lambda0, centres
-        # -+50 lambda0 from the axis, w0 = 30 lambda0, particle step = 5 wave steps
+        # -+50 lambda0 from the axis, w0 = 30 lambda0, particle step = 5 wave steps, absorbing y walls for a
         c = _base(8192, 8192, 0.035, 200, 5, rebin_every=6)
         c["grid"]["subcycle"] = 5
+        c["grid"]["bc_y"] = 1                                # "absorbing ... on all of four boundaries" (Q23)
         c["profile"] = dict(kind=PROFILE_UNIFORM, p=[0.4, 0, 0, 0])
         c["species"] = [_species(-1, 1.0, 1.0, 1, 1, SINE, 1.85),
                         _species(+1, 1836.0, 0.2, 1, 1, SINE, 1.85)]
