@@ -215,6 +215,20 @@ def velocity_histogram(X, Y, u, w, box, umin, umax, nbins):
     return h
 
 
+def probe_spectrum(h, dt_s, omegas):
+    """SURVEY 8f.4 (Fig. 12(c), (e): "the frequent spectrum of the back-scattering laser light" recorded on the
+    left boundary, of the transmitted light on the right one): power spectrum of a boundary history h[m, j] (record m
+    taken at time (m0 + m) dt_s; the origin m0 drops out of the power), written out as the sum that defines it:
+        A_j(w) = dt_s sum_m h[m, j] exp(-2 pi i w m dt_s),    P(w) = sum_j |A_j(w)|^2,    w in units of omega0."""
+    h = np.asarray(h, np.float64)
+    m = np.arange(h.shape[0])[:, None]
+    out = np.zeros(len(omegas))
+    for k, w in enumerate(omegas):
+        A = dt_s * (h * np.exp(-2j * np.pi * float(w) * m * dt_s)).sum(axis=0)
+        out[k] = (np.abs(A) ** 2).sum()
+    return out
+
+
 def mode_amplitudes(n, mx, my):
     """O9: Fourier-mode amplitudes of a nodal density n[(nx+1), ny], written out as the sum that
     defines them: A(mx, my) = sum_i sum_j v_i n[i, j] exp(-2 pi i (mx i/nx + my j/ny)), v_i = 1/2 on the wall columns
@@ -308,6 +322,21 @@ class Oracle:
     @property
     def a_old(self):
         return self._abuf("old")
+
+    def probe(self, comp=0):
+        """Boundary records of the current time level t = step * S * dt (Fig. 12(b), (d); "the time
+        evolution of back-scattering laser light on the left boundary"): the scattered field a - a_inc on the left
+        wall (the incident wave split off as in P:L122) and a on the right wall, each [ny]."""
+        g = self.g
+        t = self.st.step * max(g.subcycle, 1) * g.dt
+        a = self.a_now[comp]
+        inc = np.zeros(g.ny)
+        for k in range(self.st.nlaser):
+            L = self._las[k]
+            if L.comp == comp:
+                for j in range(g.ny):
+                    inc[j] += lib().orc_a_inc(C.byref(L), 0.0, j * g.dy, t, g.ny * g.dy)
+        return a[0] - inc, a[g.nx].copy()
 
     def moment(self, s, name):
         return self.sp[s][name].reshape(self.g.nx + 1, self.g.ny)

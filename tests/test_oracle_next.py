@@ -301,3 +301,45 @@ def test_P19_y_wall_transmits_an_oblique_beam():
         up[bc] = acc[100:, ny // 2:].sum() / acc.sum()
     assert up[0] > 0.2                      # periodic: the beam comes back in from above
     assert up[1] < 0.02                     # absorbing: only the reflected part
+
+
+# ---- S§8(f).4: boundary records and their frequency spectrum (Fig. 12) --------------------------------
+def test_P20_probe_spectrum_closed_form_fft_and_parseval():
+    """The defining sum against what mathematics fixes: a sampled cosine whose period divides the record has
+    A(w0) = T/2 exactly and nothing in the other bins; at the bin frequencies k/T the sum is numpy's FFT; Parseval."""
+    M, dt_s, ny = 400, 0.035, 3
+    T = M * dt_s                                            # 14: w0 = 1 -> 14 periods, w = 0.5 -> 7
+    m = np.arange(M)[:, None]
+    h = np.cos(2 * math.pi * 1.0 * m * dt_s) * np.array([1.0, 2.0, -0.5])[None, :]
+    P = oracle.probe_spectrum(h, dt_s, [1.0, 0.5, 2.0 / T, 0.0])
+    assert P[0] == pytest.approx((T / 2) ** 2 * (1 + 4 + 0.25), rel=1e-12)
+    assert np.all(P[1:] < 1e-20 * P[0])
+    rng = np.random.default_rng(5)
+    r = rng.standard_normal((M, ny))
+    ks = np.arange(M // 2 + 1)
+    Pr = oracle.probe_spectrum(r, dt_s, ks / T)
+    assert np.allclose(Pr, (np.abs(dt_s * np.fft.rfft(r, axis=0)) ** 2).sum(axis=1), rtol=1e-10)
+    Pall = oracle.probe_spectrum(r, dt_s, np.arange(M) / T)
+    assert Pall.sum() == pytest.approx(M * dt_s ** 2 * (r ** 2).sum(), rel=1e-10)
+    # a phase-shifted sine has the same power: the time origin drops out
+    h2 = np.sin(2 * math.pi * 1.0 * (m + 17.3) * dt_s) * np.ones((1, ny))
+    assert oracle.probe_spectrum(h2, dt_s, [1.0])[0] == pytest.approx(ny * (T / 2) ** 2, rel=1e-12)
+
+
+def test_P20_probe_of_a_plane_wave_crossing_a_vacuum_box():
+    """Oracle.probe(): once a plane wave fills a vacuum box, the left record (a - a_inc at the level just reached)
+    is empty — a wrong sign, a record one time level off (2 pi dt = 22 % of a0) or a missing beam would all show —
+    and the right record is the transmitted wave: amplitude a0, spectrum peaked at omega0."""
+    nx, ny, dx, dt, a0 = 200, 8, 0.05, 0.035, 0.01
+    o = _vac(nx, ny, dx, dt, 0, [dict(a0=a0, t_rise=3.0)])
+    o.step(int(20.0 / dt))
+    M = 400                                                 # 14 periods
+    left, right = np.zeros((M, ny)), np.zeros((M, ny))
+    for k in range(M):
+        o.step()
+        left[k], right[k] = o.probe(0)
+    assert np.abs(left).max() < 0.01 * a0
+    assert np.abs(right).max() == pytest.approx(a0, rel=0.01)
+    P = oracle.probe_spectrum(right, dt, [1.0, 0.5, 1.5])       # bins of the 14-period record
+    assert P[0] == pytest.approx(ny * (a0 * M * dt / 2) ** 2, rel=0.02)
+    assert P[1] < 1e-3 * P[0] and P[2] < 1e-3 * P[0]
