@@ -44,6 +44,7 @@ extern "C" {
 #define PM2D_MAX_LASERS 4
 #define PM2D_MAX_MODES 16
 #define PM2D_MAX_BINS 1024
+#define PM2D_MAX_OMEGAS 64
 #define PM2D_TILE 32 /* particles are binned by tiles of PM2D_TILE x PM2D_TILE cells */
 
 /* particle shape: 1-D cumulative weight G(s); weights are G differences over the control volumes
@@ -103,7 +104,9 @@ typedef struct {
                               y exchanged on the walls j = 0 and j = ny-1 of `a`, first-order outgoing condition along
                               the diagonal at the four corners (Q23).  Particles, densities, Poisson and the
                               force grid stay periodic in y                                           */
-    int32_t reserved;      /* must be 0                                                               */
+    int32_t probe_steps;   /* 0: off.  R in 1..65536: the library keeps, on the device, the boundary records of the last R
+                              particle steps (pm2d_get_probe, pm2d_probe_spectrum; Fig. 12): R * ncomp * 2 * ny
+                              floats of workspace, written by the boundary kernels themselves (no extra launch)  */
     double dx, dy, dt;     /* lambda0, lambda0, T0; dt = step of the wave equation,
                               dt*sqrt(1/dx^2 + 1/dy^2 + pi^2 n_max) < 1                     */
 } pm2d_grid;
@@ -224,6 +227,21 @@ int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);
  * 1 <= nbins <= PM2D_MAX_BINS.  Synchronises the stream.  Sums in float64; the order of the additions is not fixed. */
 int pm2d_velocity_histogram(pm2d_ctx *ctx, int species, int i0, int i1, int j0, int j1, int comp, double umin, double umax,
                             int nbins, double *hist);
+
+/* Boundary records ("the time evolution of back-scattering laser light on the left boundary", P:L320;
+ * Fig. 12(b), (d)).  With pm2d_grid.probe_steps = R > 0 every particle step q = 1, 2, ... (time q * S * dt)
+ * leaves one record per component and wall: wall 0 = left, the scattered field a - a_inc on the nodes (0, j) (the
+ * incident wave split off as in P:L122); wall 1 = right, a on the nodes (nx, j).  The last min(q, R) records are kept.
+ * pm2d_get_probe copies them in time order into host[n * ny] (host float32, capacity `cap` elements), stores the step
+ * index q of the first one in *first_step (host, may be NULL) and returns n (0 before the first step) or a negative
+ * code (PM2D_ESTATE if probe_steps = 0).  Synchronises the stream. */
+int64_t pm2d_get_probe(pm2d_ctx *ctx, int wall, int comp, float *host, size_t cap, int64_t *first_step);
+/* Frequency spectrum of those records (Fig. 12(c), (e)), over the columns j0 <= j < j1:
+ *     A_j(w) = dt_s sum_m h[m, j] exp(-2 pi i w m dt_s),   power[k] = sum_j |A_j(omega[k])|^2,
+ * m = 0 .. n-1 over the kept records in time order, dt_s = S * dt, omega in units of omega0 (host double[nomega],
+ * 1 <= nomega <= PM2D_MAX_OMEGAS); power: host double[nomega].  float32 records, float64 phases and sums.
+ * Returns n, the number of records used, or a negative code.  Synchronises the stream. */
+int64_t pm2d_probe_spectrum(pm2d_ctx *ctx, int wall, int comp, int j0, int j1, int nomega, const double *omega, double *power);
 
 int pm2d_mode_amplitudes(pm2d_ctx *ctx, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re, double *im);
 int64_t pm2d_particle_count(pm2d_ctx *ctx, int species);

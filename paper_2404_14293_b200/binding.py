@@ -28,7 +28,7 @@ PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncomp", C.c_int32), ("rebin_every", C.c_int32),
                 ("eager_moments", C.c_int32), ("track_ids", C.c_int32), ("particle_order", C.c_int32), ("subcycle", C.c_int32),
-                ("bc_y", C.c_int32), ("reserved", C.c_int32),
+                ("bc_y", C.c_int32), ("probe_steps", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dt", C.c_double)]
 
 
@@ -76,6 +76,8 @@ SYMBOLS = {
     "pm2d_diagnostics": (C.c_int, [_vp, C.POINTER(Diag)]),
     "pm2d_velocity_histogram": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                          C.POINTER(C.c_double)]),
+    "pm2d_get_probe": (C.c_int64, [_vp, C.c_int, C.c_int, _fp, C.c_size_t, _lp]),
+    "pm2d_probe_spectrum": (C.c_int64, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pm2d_mode_amplitudes": (C.c_int, [_vp, C.c_int, C.c_int, _ip, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pm2d_particle_count": (C.c_int64, [_vp, C.c_int]),
     "pm2d_profile_enable": (C.c_int, [_vp, C.c_int]),
@@ -128,7 +130,7 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, part
     g = cfg["grid"]
     grid = Grid(g["nx"], g["ny"], g.get("ncomp", 1), g.get("rebin_every", 8) if rebin_every is None else rebin_every,
                 int(eager_moments), int(track_ids), int(particle_order), int(g.get("subcycle", 1)),
-                int(g.get("bc_y", 0)), 0, g["dx"], g["dy"], g["dt"])
+                int(g.get("bc_y", 0)), int(g.get("probe_steps", 0)), g["dx"], g["dy"], g["dt"])
     sp = (Species * len(cfg["species"]))()
     for k, s in enumerate(cfg["species"]):
         sp[k] = Species(s["mass"], s["T_keV"], s["pressure_coeff"], s["DD"], s["sign"], s["shape"], s["mobile"], s["load"],
@@ -266,6 +268,23 @@ class PM2D:
         _check(self.lib.pm2d_velocity_histogram(self.ctx, int(species), int(i0), int(i1), int(j0), int(j1), int(comp), float(umin),
                                                 float(umax), int(nbins), h.ctypes.data_as(C.POINTER(C.c_double))))
         return h
+
+    def get_probe(self, wall, comp=0):
+        """(records[n, ny], first_step): the kept boundary records of a wall (0 left: a - a_inc, 1 right: a) in time
+        order; needs grid["probe_steps"] > 0  [pm2d_get_probe]"""
+        n = int(self.grid.probe_steps)
+        out = np.empty((max(n, 1), self.ny), np.float32)
+        first = C.c_int64(0)
+        got = _check(self.lib.pm2d_get_probe(self.ctx, int(wall), int(comp), _ptr(out, C.c_float), out.size, C.byref(first)))
+        return out[:got], int(first.value)
+
+    def probe_spectrum(self, wall, omegas, comp=0, j0=0, j1=None):
+        """power[k] = sum_j |dt_s sum_m h[m, j] exp(-2 pi i omega_k m dt_s)|^2 over the kept records  [pm2d_probe_spectrum]"""
+        om = _np(omegas, np.float64)
+        out = np.zeros(om.size)
+        _check(self.lib.pm2d_probe_spectrum(self.ctx, int(wall), int(comp), int(j0), int(self.ny if j1 is None else j1), int(om.size),
+                                            om.ctypes.data_as(C.POINTER(C.c_double)), out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
 
     def mode_amplitudes(self, species, mx, my):
         """complex A(m_x, m_y) of the species' nodal density for the mode pairs (mx[k], my[k])  [pm2d_mode_amplitudes]"""

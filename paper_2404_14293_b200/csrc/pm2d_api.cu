@@ -79,7 +79,7 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (g->subcycle > 1 && (g->subcycle * g->dt / g->dx > 4.0 || g->subcycle * g->dt / g->dy > 4.0))
         return fail(PM2D_EINVAL, "subcycle*dt/dx must be <= 4");
     if (g->bc_y != PM2D_BC_Y_PERIODIC && g->bc_y != PM2D_BC_Y_ABSORB) return fail(PM2D_EINVAL, "unknown bc_y");
-    if (g->reserved != 0) return fail(PM2D_EINVAL, "pm2d_grid.reserved must be 0");
+    if (g->probe_steps < 0 || g->probe_steps > 65536) return fail(PM2D_EINVAL, "probe_steps must be 0..65536");
     for (int s = 0; s < nsp; s++) {
         const pm2d_species &q = sp[s];
         if (!(q.mass > 0)) return fail(PM2D_EINVAL, "species mass must be positive");
@@ -125,6 +125,7 @@ size_t layout(pm2d_ctx *c, char *base)
     c->twiddle = cv.take<float2>(g.ny / 2);
     c->red = cv.take<double>(64);
     c->hist = cv.take<double>(PM2D_MAX_BINS);
+    c->probe = g.probe_steps > 0 ? cv.take<float>((size_t)g.probe_steps * g.ncomp * 2 * g.ny) : nullptr;
     c->flags = cv.take<int32_t>(4);
     c->shape_y = cv.take<double>(g.ny);
     c->taper_x = cv.take<double>(g.nx);

@@ -170,7 +170,125 @@ __global__ void __launch_bounds__(PTHREADS) k_diag_vhist(const HistParams H)
         if (sh[b] != 0.0) atomicAdd(&H.hist[b], sh[b]);
 }
 
+// Frequency spectrum of the boundary records (pm2d_probe_spectrum): CTA = 128 columns x one omega.  The phase factors
+// of 128 records at a time are computed once per CTA in double (one record per thread) and shared; every thread then
+// walks those records of its own column (coalesced rows of the ring), accumulating A_j(w) in double.
+struct SpecParams {
+    const float *probe;      // ring base of (comp, wall): record q-1 at probe + slot * stride
+    size_t stride;           // ncomp * 2 * ny
+    int cap, first_slot, nrec;
+    int j0, j1;
+    double dts;
+    double omega[PM2D_MAX_OMEGAS];
+    double *red;             // [nomega]
+};
+__global__ void __launch_bounds__(128) k_probe_spectrum(const SpecParams S)
+{
+    __shared__ double2 tw[128];
+    __shared__ double part[4];
+    const int j = S.j0 + blockIdx.x * 128 + threadIdx.x;
+    const double w2 = 2.0 * S.omega[blockIdx.y] * S.dts;
+    double re = 0.0, im = 0.0;
+    for (int m0 = 0; m0 < S.nrec; m0 += 128) {
+        double sn, cs;
+        sincospi(w2 * (double)(m0 + threadIdx.x), &sn, &cs);
+        __syncthreads();
+        tw[threadIdx.x] = make_double2(cs, -sn);
+        __syncthreads();
+        const int mend = min(128, S.nrec - m0);
+        if (j < S.j1) {
+            int slot = (S.first_slot + m0) % S.cap;
+            for (int m = 0; m < mend; m++) {
+                const double h = (double)S.probe[(size_t)slot * S.stride + j];
+                re += h * tw[m].x;
+                im += h * tw[m].y;
+                if (++slot == S.cap) slot = 0;
+            }
+        }
+    }
+    double p = (j < S.j1) ? (re * re + im * im) * S.dts * S.dts : 0.0;
+    for (int o = 16; o > 0; o >>= 1) p += __shfl_down_sync(0xffffffffu, p, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = p;
+    __syncthreads();
+    if (threadIdx.x == 0) atomicAdd(&S.red[blockIdx.y], part[0] + part[1] + part[2] + part[3]);
+}
+
 }  // namespace
+
+// the kept boundary records: n of them, the first one of particle step `first` (1-based), in ring slot `slot`
+static int64_t probe_window(const pm2d_ctx *c, int64_t *first, int *slot)
+{
+    const int64_t R = c->g.probe_steps, n = c->step < R ? c->step : R;
+    *first = c->step - n + 1;
+    *slot = (int)((*first - 1) % R);
+    return n;
+}
+
+extern "C" int64_t pm2d_get_probe(pm2d_ctx *c, int wall, int comp, float *host, size_t cap, int64_t *first_step)
+{
+    if (!c || wall < 0 || wall > 1 || comp < 0 || comp >= c->g.ncomp || !host) {
+        pm2d_set_error("pm2d_get_probe: bad argument");
+        return PM2D_EINVAL;
+    }
+    if (!c->probe) {
+        pm2d_set_error("pm2d_get_probe: pm2d_grid.probe_steps is 0");
+        return PM2D_ESTATE;
+    }
+    int64_t first;
+    int slot;
+    const int64_t n = probe_window(c, &first, &slot);
+    const size_t ny = (size_t)c->g.ny, stride = (size_t)c->g.ncomp * 2 * ny;
+    if ((size_t)n * ny > cap) {
+        pm2d_set_error("pm2d_get_probe: host buffer too small");
+        return PM2D_EINVAL;
+    }
+    if (first_step) *first_step = first;
+    const float *base = c->probe + ((size_t)comp * 2 + wall) * ny;
+    // two pieces of the ring: slots slot .. R-1, then 0 .. slot-1
+    const int64_t n1 = n < c->g.probe_steps - slot ? n : c->g.probe_steps - slot;
+    if (n1 > 0)
+        PM2D_CUDA_CHECK(cudaMemcpy2DAsync(host, ny * sizeof(float), base + (size_t)slot * stride, stride * sizeof(float), ny * sizeof(float),
+                                          (size_t)n1, cudaMemcpyDeviceToHost, c->stream));
+    if (n > n1)
+        PM2D_CUDA_CHECK(cudaMemcpy2DAsync(host + (size_t)n1 * ny, ny * sizeof(float), base, stride * sizeof(float), ny * sizeof(float),
+                                          (size_t)(n - n1), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return n;
+}
+
+extern "C" int64_t pm2d_probe_spectrum(pm2d_ctx *c, int wall, int comp, int j0, int j1, int nomega, const double *omega,
+                                       double *power)
+{
+    if (!c || wall < 0 || wall > 1 || comp < 0 || comp >= c->g.ncomp || j0 < 0 || j1 > c->g.ny || j0 >= j1 || nomega < 1 ||
+        nomega > PM2D_MAX_OMEGAS || !omega || !power) {
+        pm2d_set_error("pm2d_probe_spectrum: bad argument");
+        return PM2D_EINVAL;
+    }
+    if (!c->probe) {
+        pm2d_set_error("pm2d_probe_spectrum: pm2d_grid.probe_steps is 0");
+        return PM2D_ESTATE;
+    }
+    int64_t first;
+    int slot;
+    const int64_t n = probe_window(c, &first, &slot);
+    for (int k = 0; k < nomega; k++) power[k] = 0.0;
+    if (n == 0) return 0;
+    SpecParams S;
+    S.probe = c->probe + ((size_t)comp * 2 + wall) * c->g.ny;
+    S.stride = (size_t)c->g.ncomp * 2 * c->g.ny;
+    S.cap = c->g.probe_steps; S.first_slot = slot; S.nrec = (int)n;
+    S.j0 = j0; S.j1 = j1;
+    S.dts = c->dtp;
+    for (int k = 0; k < PM2D_MAX_OMEGAS; k++) S.omega[k] = k < nomega ? omega[k] : 0.0;
+    S.red = c->red;
+    PM2D_CUDA_CHECK(cudaMemsetAsync(c->red, 0, 64 * sizeof(double), c->stream));
+    k_probe_spectrum<<<dim3((j1 - j0 + 127) / 128, nomega), 128, 0, c->stream>>>(S);
+    count_launch(c);
+    PM2D_CUDA_CHECK(cudaGetLastError());
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(power, c->red, (size_t)nomega * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return n;
+}
 
 extern "C" int pm2d_velocity_histogram(pm2d_ctx *c, int species, int i0, int i1, int j0, int j1, int comp, double umin, double umax,
                                        int nbins, double *hist)

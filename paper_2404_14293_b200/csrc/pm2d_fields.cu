@@ -133,7 +133,7 @@ __device__ double oblique_inc(const ObLaser &L, double x, double y, double t, do
 // scattered field s = a - a_inc and a_inc added back.  OBLIQUE: some beam has alpha != 0.
 template <bool OBLIQUE>
 __global__ void k_boundary(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap, BcParams B,
-                           ObParams O, int comp, int nx, int ny)
+                           ObParams O, int comp, int nx, int ny, float *__restrict__ probe)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= ny) return;
@@ -169,13 +169,16 @@ __global__ void k_boundary(const float *__restrict__ a, const float *__restrict_
         float D1 = (a[ny + jp] - inc[2][4]) - 2.f * s1 + (a[ny + jm] - inc[0][4]);
         float s0p = (B.alpha * (s1p - s1m + s0m) - B.beta * (s1p + s1m + s0m - 2.f * s0 - 2.f * s1) + B.gam * (D0 + D1)) * ab;
         ap[j] = s0p + inc[1][2];
+        if (probe) probe[j] = s0p;                 // boundary record, left wall: the scattered field (pm2d_get_probe)
     }
     {   // right wall: rows nx, nx-1, no incident wave
         const size_t r0 = (size_t)nx * ny, r1 = (size_t)(nx - 1) * ny;
         float E0 = a[r0 + jp] - 2.f * a[r0 + j] + a[r0 + jm];
         float E1 = a[r1 + jp] - 2.f * a[r1 + j] + a[r1 + jm];
-        ap[r0 + j] = (B.alpha * (ap[r1 + j] - am[r1 + j] + am[r0 + j]) -
-                      B.beta * (ap[r1 + j] + am[r1 + j] + am[r0 + j] - 2.f * a[r0 + j] - 2.f * a[r1 + j]) + B.gam * (E0 + E1)) * ab;
+        const float v = (B.alpha * (ap[r1 + j] - am[r1 + j] + am[r0 + j]) -
+                         B.beta * (ap[r1 + j] + am[r1 + j] + am[r0 + j] - 2.f * a[r0 + j] - 2.f * a[r1 + j]) + B.gam * (E0 + E1)) * ab;
+        ap[r0 + j] = v;
+        if (probe) probe[ny + j] = v;              // right wall: a itself
     }
 }
 
@@ -188,7 +191,7 @@ struct BcYParams {
     float alpha_y, beta, gam_x, kap;   // 1/(2 dt dy), 1/(2 dt^2), 1/(4 dx^2), (dt - hd)/(dt + hd), hd = sqrt(dx^2 + dy^2)
 };
 __global__ void k_boundary_y(const float *__restrict__ a, const float *__restrict__ am, float *__restrict__ ap, BcYParams B, int nx,
-                             int ny)
+                             int ny, float *__restrict__ probe)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;   // 0..nx
     const int side = blockIdx.y;
@@ -197,7 +200,12 @@ __global__ void k_boundary_y(const float *__restrict__ a, const float *__restric
     if (i == 0 || i == nx) {
         // corner c, diagonal neighbour d: a_c^{n+1} = a_d^n + kappa (a_d^{n+1} - a_c^n)
         const size_t kc = (size_t)i * ny + j0, kd = (size_t)(i == 0 ? 1 : nx - 1) * ny + j1;
-        ap[kc] = a[kd] + B.kap * (ap[kd] - a[kc]);
+        const float v = a[kd] + B.kap * (ap[kd] - a[kc]);
+        if (probe) {   // the corner's boundary record follows its new value (left: the incident part stays split off)
+            if (i == 0) probe[j0] += v - ap[kc];
+            else probe[ny + j0] = v;
+        }
+        ap[kc] = v;
         return;
     }
     const size_t k0 = (size_t)i * ny + j0, k1 = (size_t)i * ny + j1;
@@ -345,8 +353,11 @@ int launch_field_step(pm2d_ctx *c, int sub)
         const size_t off = (size_t)comp * c->nn;
         k_wave<<<grid, FCOLS, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, ne, nx, ny, (float)(1.0 / (dx * dx)),
                                               (float)(1.0 / (dy * dy)), (float)(dt * dt));
-        if (oblique) k_boundary<true><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
-        else k_boundary<false><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny);
+        // boundary record of particle step q = step + 1, taken from its last wave step: slot (q - 1) % probe_steps
+        float *probe = (c->probe && sub == c->nsub - 1)
+                           ? c->probe + ((size_t)(c->step % c->g.probe_steps) * c->g.ncomp + comp) * 2 * ny : nullptr;
+        if (oblique) k_boundary<true><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny, probe);
+        else k_boundary<false><<<(ny + 127) / 128, 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, B, O, comp, nx, ny, probe);
         count_launch(c, 2);
         if (c->g.bc_y == PM2D_BC_Y_ABSORB) {
             BcYParams Y;
@@ -355,7 +366,7 @@ int launch_field_step(pm2d_ctx *c, int sub)
             Y.beta = B.beta;
             Y.gam_x = (float)(1.0 / (4.0 * dx * dx));
             Y.kap = (float)((dt - hd) / (dt + hd));
-            k_boundary_y<<<dim3((nx + 1 + 127) / 128, 2), 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, Y, nx, ny);
+            k_boundary_y<<<dim3((nx + 1 + 127) / 128, 2), 128, 0, c->stream>>>(c->a[1] + off, c->a[2] + off, c->a[0] + off, Y, nx, ny, probe);
             count_launch(c, 1);
         }
     }

@@ -98,6 +98,7 @@ struct pm2d_ctx {
     float2 *twiddle;     // [ny/2]
     double *red;         // [64] reduction scratch
     double *hist;        // [PM2D_MAX_BINS] velocity histogram scratch
+    float *probe;        // [probe_steps][ncomp][2][ny] ring of boundary records (slot = (q-1) % probe_steps), or nullptr
     int32_t *flags;      // [4] device error flags
     double *shape_y, *taper_x;   // [ny], [nx] relative density tables of the number-weighted loader
     unsigned long long *stray_total; // [1] statistics

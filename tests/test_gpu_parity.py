@@ -772,3 +772,97 @@ def test_bc_y_is_validated(P):
     cfg = small_cfg("c1", 96, 64, bc_y=2)
     with pytest.raises(P.PM2DError):
         P.PM2D(cfg)
+
+
+# ---- S§8(f).4: boundary records and their frequency spectrum (pm2d_get_probe, pm2d_probe_spectrum; Fig. 12) ------
+def _probe_run(P, cfg, nsteps, R):
+    cfg["grid"]["probe_steps"] = R
+    sim = P.PM2D(cfg, eager_moments=1)
+    orc, _ = oracle_from_config(cfg)
+    ncomp = cfg["grid"]["ncomp"]
+    hist = [[[], []] for _ in range(ncomp)]
+    assert sim.get_probe(0)[0].shape[0] == 0                   # nothing recorded before the first step
+    for _ in range(nsteps):
+        sim.step(1)
+        orc.step(1)
+        for c in range(ncomp):
+            l, r = orc.probe(c)
+            hist[c][0].append(l)
+            hist[c][1].append(r)
+    return sim, orc, hist
+
+
+def _check_probe(P, sim, orc, hist, cfg, nsteps, R, omegas, jr):
+    g = cfg["grid"]
+    dts = g["dt"] * max(g.get("subcycle", 1), 1)
+    scale = max(np.abs(orc.a_now).max(), 1e-30)
+    n = min(nsteps, R)
+    for c in range(g["ncomp"]):
+        for wall in (0, 1):
+            ref = np.array(hist[c][wall][-n:])
+            rec, first = sim.get_probe(wall, c)
+            assert rec.shape == (n, g["ny"]) and first == nsteps - n + 1
+            assert np.abs(rec - ref).max() < 5e-5 * scale, (c, wall, np.abs(rec - ref).max())
+            got = sim.probe_spectrum(wall, omegas, c, jr[0], jr[1])
+            # the kernel's sums against the defining sum over the very same float32 records: rounding order only
+            own = oracle.probe_spectrum(rec[:, jr[0]:jr[1]].astype(np.float64), dts, omegas)
+            assert np.allclose(got, own, rtol=1e-9, atol=1e-12 * max(own.max(), 1e-300)), (c, wall)
+            # and against the oracle's own records, where there is power
+            exp = oracle.probe_spectrum(ref[:, jr[0]:jr[1]], dts, omegas)
+            big = exp > 1e-3 * exp.max()
+            if exp.max() > 0:
+                assert np.allclose(got[big], exp[big], rtol=2e-3), (c, wall, got, exp)
+
+
+@pytest.mark.gpu
+def test_probe_records_and_spectrum_parity_c1(P):
+    """c1 slab (reduced), 300 steps with a ring of 140 records (wraps twice, ragged: 300 = 2 x 140 + 20; more than one
+    128-record block of the spectrum kernel): the kept
+    records of both walls equal the oracle's a - a_inc / a at the same steps; the spectrum equals the defining sum."""
+    cfg = small_cfg("c1", 96, 64)
+    cfg["lasers"][0]["t_rise"] = 1.0
+    nsteps, R = 300, 140
+    sim, orc, hist = _probe_run(P, cfg, nsteps, R)
+    assert np.abs(np.array(hist[0][1][-R:])).max() > 1e-3 * cfg["lasers"][0]["a0"]          # light has reached the right wall
+    _check_probe(P, sim, orc, hist, cfg, nsteps, R, [1.0, 0.67, 0.5, 0.0, 1.33, 2.0], (0, 64))
+    _check_probe(P, sim, orc, hist, cfg, nsteps, R, [1.0, 0.9], (5, 47))                    # a ragged column window
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_probe_records_subcycled_oblique_absorbing_three_components(P):
+    """Reduced CBET set-up (two oblique beams, 5 wave steps per particle step, absorbing y walls: the corner records go
+    through k_boundary_y) with a second beam pair moved to a_x: one record per particle step, taken from its last
+    wave step; 20 records kept of 24."""
+    cfg = small_cfg("cbet", 80, 64, ncomp=3)
+    for k, las in enumerate(cfg["lasers"]):
+        las["t_rise"] = 0.3
+        las["comp"] = 2 * k
+    nsteps, R = 24, 20
+    sim, orc, hist = _probe_run(P, cfg, nsteps, R)
+    _check_probe(P, sim, orc, hist, cfg, nsteps, R, [1.0, 1.0 / 0.9995, 0.3], (0, 64))
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_probe_arguments(P):
+    cfg = small_cfg("c1", 96, 64)
+    sim = P.PM2D(cfg)
+    sim.step(1)
+    with pytest.raises(P.PM2DError):
+        sim.probe_spectrum(0, [1.0])                          # probe_steps = 0
+    sim.close()
+    cfg["grid"]["probe_steps"] = 4
+    sim = P.PM2D(cfg)
+    sim.step(2)
+    with pytest.raises(P.PM2DError):
+        sim.probe_spectrum(2, [1.0])
+    with pytest.raises(P.PM2DError):
+        sim.probe_spectrum(0, np.linspace(0, 2, 65))
+    with pytest.raises(P.PM2DError):
+        sim.probe_spectrum(0, [1.0], 0, 10, 10)
+    assert sim.get_probe(1)[0].shape == (2, 64)
+    sim.close()
+    bad = small_cfg("c1", 96, 64, probe_steps=70000)
+    with pytest.raises(P.PM2DError):
+        P.PM2D(bad)
