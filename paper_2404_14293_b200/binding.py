@@ -7,6 +7,7 @@ method runs inside the library's kernels.  There is no CPU path: importing works
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 
 import numpy as np
@@ -123,6 +124,17 @@ def _np(a, dtype):
 
 def _ptr(a, ctype):
     return None if a is None else a.ctypes.data_as(C.POINTER(ctype))
+
+
+def polarised_beam(a0, theta, beta, **laser):
+    """Laser-table entries of one beam of arbitrary polarisation (Fig. 1(a)): the vector potential makes the
+    angle theta with the z axis, its part in the x-y plane the angle beta with the x axis.  Components of `a` are
+    numbered 0 = z (S polarisation, the one BASELINE.json's configs use), 1 = x, 2 = y:
+        a_sz = a0 cos(theta),  a_px = a0 sin(theta) cos(beta),  a_py = a0 sin(theta) sin(beta).
+    Every component obeys the same wave equation (Eq. 1), so the beam is three entries that differ in `a0` and
+    `comp`; entries of zero amplitude are left out.  The grid needs ncomp = 3 unless theta = 0."""
+    amps = (a0 * math.cos(theta), a0 * math.sin(theta) * math.cos(beta), a0 * math.sin(theta) * math.sin(beta))
+    return [dict(laser, a0=float(a), comp=c) for c, a in enumerate(amps) if abs(a) > 1e-300 * abs(a0)]
 
 
 def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, particle_order=0):

@@ -55,3 +55,18 @@ def test_product_does_not_import_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2404_14293_b200", txt, flags=re.M), f
             assert not re.search(r"#include\s+\"[^\"]*(csrc|pm2d\.h|pm2d_internal)", txt), f
+
+
+def test_polarised_beam_decomposition():
+    """a_sz = a cos(theta), a_px = a sin(theta) cos(beta), a_py = a sin(theta) sin(beta); host logic only."""
+    import math
+    import pytest
+    b = P.polarised_beam(0.02, math.radians(90.0), math.radians(0.0), omega=1.0, y0=0.0, w0=0.0, alpha=0.0, t_rise=1.0)
+    assert [(l["comp"], round(l["a0"], 15)) for l in b if abs(l["a0"]) > 1e-15] == [(1, 0.02)]      # pure P, along x
+    b = P.polarised_beam(0.02, 0.0, 1.0, omega=1.0, y0=0.0, w0=0.0, alpha=0.0, t_rise=1.0)
+    assert [(l["comp"], l["a0"]) for l in b] == [(0, 0.02)]                                         # pure S
+    b = P.polarised_beam(0.02, math.radians(30.0), math.radians(90.0), omega=2.0, y0=1.0, w0=3.0, alpha=0.1, t_rise=1.0)
+    amp = {l["comp"]: l["a0"] for l in b}
+    assert amp[0] == 0.02 * math.cos(math.radians(30.0)) and abs(amp[2] - 0.01) < 1e-15 and abs(amp.get(1, 0.0)) < 1e-15
+    assert sum(l["a0"] ** 2 for l in b) == pytest.approx(0.02 ** 2, rel=1e-14)
+    assert all(l["omega"] == 2.0 and l["y0"] == 1.0 and l["w0"] == 3.0 and l["alpha"] == 0.1 for l in b)

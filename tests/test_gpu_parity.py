@@ -866,3 +866,31 @@ def test_probe_arguments(P):
     bad = small_cfg("c1", 96, 64, probe_steps=70000)
     with pytest.raises(P.PM2DError):
         P.PM2D(bad)
+
+
+@pytest.mark.gpu
+def test_polarised_beam_three_components_parity(P):
+    """A3c: a Gaussian beam of arbitrary polarisation (theta = 35 degrees from z, beta = 60 degrees from x) at
+    10 degrees of incidence through the c3 slab (reduced, mobile ions): the three components, built by
+    polarised_beam, stay with the oracle driven by the amplitudes written out here, and keep their ratio."""
+    th, be, a0 = math.radians(35.0), math.radians(60.0), 0.02
+    cfg = small_cfg("c3", 72, 64, ncomp=3)
+    Ly = 64 * cfg["grid"]["dy"]
+    beam = dict(omega=1.0, y0=0.55 * Ly, w0=0.3 * Ly, alpha=math.radians(10.0), t_rise=1.5)
+    cfg["lasers"] = P.polarised_beam(a0, th, be, **beam)
+    sim = P.PM2D(cfg, eager_moments=1)
+    ref = copy.deepcopy(cfg)
+    ref["lasers"] = [dict(beam, a0=a0 * math.cos(th), comp=0), dict(beam, a0=a0 * math.sin(th) * math.cos(be), comp=1),
+                     dict(beam, a0=a0 * math.sin(th) * math.sin(be), comp=2)]
+    orc, _ = oracle_from_config(ref)
+    sim.step(120)
+    orc.step(120)
+    scale = np.abs(orc.a_now).max()
+    assert scale > 0.5 * a0 * math.cos(th)
+    got = [sim.get_fields(P.FIELD_A, c, 0) for c in range(3)]
+    for c in range(3):
+        assert np.abs(got[c] - orc.a_now[c]).max() < 5e-5 * scale, c
+    # same equation, same density: the components differ by their amplitudes only (up to float32 rounding)
+    assert np.abs(got[1] * math.cos(th) - got[0] * math.sin(th) * math.cos(be)).max() < 1e-5 * scale
+    assert np.abs(got[2] * math.cos(be) - got[1] * math.sin(be)).max() < 1e-5 * scale
+    sim.close()
