@@ -131,6 +131,11 @@ typedef struct {
                               d = distance of the cell centre from the wall in cells; 0 = none           */
     double p[4];           /* UNIFORM: n0. LINEAR: n(0), n(Lx). EXP_CAPPED: n0, Lx/L, cap.
                               FILAMENT_Y: mean n0, amplitude A, sigma in cells: n(j) ~ 1 + A exp(-(y-Ly/2)^2/2 sigma^2) */
+    int32_t taper_cells_y; /* the same taper at both y walls (0 = none): with taper_cells it makes the paper's slab "at the
+                              center of the simulation box" with margins on all sides, the
+                              margins at PM2D_TAPER_FLOOR of the profile instead of vacuum (Q20).  Weights only: not
+                              with PM2D_NUMBER_WEIGHTED                                               */
+    int32_t pad_;
 } pm2d_profile;
 
 typedef struct {

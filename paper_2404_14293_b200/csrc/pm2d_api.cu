@@ -297,6 +297,10 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
         if ((rc = validate_laser_angle(lasers[l], grid->ny * grid->dy))) return rc;
     }
     if (profile->kind < PM2D_PROFILE_UNIFORM || profile->kind > PM2D_PROFILE_FILAMENT_Y) return fail(PM2D_EINVAL, "unknown profile");
+    if (profile->taper_cells_y < 0 || profile->taper_cells_y > grid->ny / 2) return fail(PM2D_EINVAL, "taper_cells_y must be in [0, ny/2]");
+    if (profile->taper_cells_y > 0)
+        for (int s = 0; s < nsp; s++)
+            if (species[s].load == PM2D_NUMBER_WEIGHTED) return fail(PM2D_EINVAL, "taper_cells_y is not available with PM2D_NUMBER_WEIGHTED");
     double nmax;
     if (profile->kind == PM2D_PROFILE_UNIFORM) nmax = profile->p[0];
     else if (profile->kind == PM2D_PROFILE_LINEAR) nmax = std::max(profile->p[0], profile->p[1]);

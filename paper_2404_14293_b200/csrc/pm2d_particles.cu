@@ -911,7 +911,7 @@ struct LoadParams {
     int ppc_x, ppc_y, load, species;
     uint32_t seed_lo, seed_hi;
     double vth;
-    int prof_kind, taper_cells;
+    int prof_kind, taper_cells, taper_cells_y;
     double p0, p1, p2;
     const int32_t *cell_off;     // NUMBER_WEIGHTED: the tile's cell runs give (cell, k) of a slot
     int layered;                 // storage order inside a tile: (rank in cell, cell) instead of (cell, rank)
@@ -932,6 +932,17 @@ __device__ double profile_density(const LoadParams &L, int i)
         }
     }
     return n;
+}
+
+// the same taper at the y walls (pm2d_profile.taper_cells_y)
+__device__ double taper_y(const LoadParams &L, int j)
+{
+    const double PI = 3.14159265358979323846;
+    if (L.taper_cells_y <= 0) return 1.0;
+    const double d = fmin((double)j + 0.5, (double)L.ny - 0.5 - (double)j);
+    if (d >= (double)L.taper_cells_y) return 1.0;
+    const double s = sin(0.5 * PI * d / (double)L.taper_cells_y);
+    return PM2D_TAPER_FLOOR + (1.0 - PM2D_TAPER_FLOOR) * (s * s);
 }
 
 // one CTA per chunk; a tile with wx*wy cells stores its cells row-major, ppc particles each:
@@ -993,7 +1004,7 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
         out.ux = ux;
         out.uy = uy;
         L.pv[p] = out;
-        L.w[p] = L.load == PM2D_NUMBER_WEIGHTED ? (float)(L.p0 / (double)ppc) : (float)(profile_density(L, gx0 + li) / (double)ppc);
+        L.w[p] = L.load == PM2D_NUMBER_WEIGHTED ? (float)(L.p0 / (double)ppc) : (float)(profile_density(L, gx0 + li) * taper_y(L, gy0 + lj) / (double)ppc);
         if (L.id) L.id[p] = pid;
     }
 }
@@ -1736,7 +1747,7 @@ int launch_load_particles(pm2d_ctx *c, int s)
     L.ppc_x = S.cfg.ppc_x; L.ppc_y = S.cfg.ppc_y; L.load = S.cfg.load; L.species = s;
     L.seed_lo = (uint32_t)(c->seed & 0xFFFFFFFFu); L.seed_hi = (uint32_t)(c->seed >> 32);
     L.vth = sqrt(S.cfg.T_keV / 511.0 / S.cfg.mass);
-    L.prof_kind = c->profile.kind; L.taper_cells = c->profile.taper_cells;
+    L.prof_kind = c->profile.kind; L.taper_cells = c->profile.taper_cells; L.taper_cells_y = c->profile.taper_cells_y;
     L.p0 = c->profile.p[0]; L.p1 = c->profile.p[1]; L.p2 = c->profile.p[2];
     L.cell_off = S.cell_off;
     L.layered = S.layered ? 1 : 0;

@@ -88,6 +88,17 @@ def taper_factor(profile: dict, nx: int, i_cell):
     return np.where(d < tc, TAPER_FLOOR + (1.0 - TAPER_FLOOR) * (sn * sn), 1.0)
 
 
+def taper_factor_y(profile: dict, ny: int, j_cell):
+    """The same taper at the y walls over profile["taper_cells_y"] cells (0 / absent: none)."""
+    j = np.asarray(j_cell, dtype=np.float64)
+    tc = int(profile.get("taper_cells_y", 0))
+    if tc <= 0:
+        return np.ones_like(j)
+    d = np.minimum(j + 0.5, ny - 0.5 - j)
+    sn = np.sin(0.5 * math.pi * d / tc)
+    return np.where(d < tc, TAPER_FLOOR + (1.0 - TAPER_FLOOR) * (sn * sn), 1.0)
+
+
 def filament_shape(profile: dict, ny: int):
     """Relative density of the cells of column index j (mean 1 over j): a Gaussian filament along x centred
     in y, 1 + A exp(-(y - Ly/2)^2 / 2 sigma^2), normalised; p = [n0, A, sigma in cells].  float64[ny]."""
@@ -151,7 +162,7 @@ def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None
     if sp["load"] == NUMBER_WEIGHTED:
         w = np.full(pid.size, np.float32(cfg["profile"]["p"][0] / ppc), np.float32)
     else:
-        w = (profile_density(cfg["profile"], nx, ix) / ppc).astype(np.float32)
+        w = (profile_density(cfg["profile"], nx, ix) * taper_factor_y(cfg["profile"], ny, iy) / ppc).astype(np.float32)
     return dict(id=pid, ix=ix, iy=iy, fx=fx, fy=fy, ux=ux, uy=uy, w=w)
 
 
@@ -244,6 +255,8 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     g = c["grid"]
     c["name"] = name if (nx is None and ny is None) else f"{name}@{g['nx']}x{g['ny']}"
     c["profile"]["taper_cells"] = g["nx"] // 16          # Q9
+    if name == "cbet":                                    # the paper's slab has margins on all four sides
+        c["profile"]["taper_cells_y"] = g["ny"] // 16
     if name == "c5":                                      # sigma = ny/64 cells, amplitude A such that peak = 20 x mean
         sig = g["ny"] / 64.0
         c["profile"]["p"][2] = sig

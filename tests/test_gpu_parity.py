@@ -894,3 +894,37 @@ def test_polarised_beam_three_components_parity(P):
     assert np.abs(got[1] * math.cos(th) - got[0] * math.sin(th) * math.cos(be)).max() < 1e-5 * scale
     assert np.abs(got[2] * math.cos(be) - got[1] * math.sin(be)).max() < 1e-5 * scale
     sim.close()
+
+
+@pytest.mark.gpu
+def test_y_taper_loader_and_run_parity(P):
+    """pm2d_profile.taper_cells_y: the slab with margins on all four sides.  The device loader equals
+    the numpy generator (weights to 1 ulp, the margin cells at the 1 % floor), and with absorbing y walls (the paper's
+    geometry) 10 steps of the c3 slab stay with the oracle."""
+    cfg = small_cfg("c3", 72, 64, bc_y=1)
+    cfg["profile"]["taper_cells_y"] = 9
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1)
+    for s in (0, 1):
+        ref = I.generate_particles(cfg, s)
+        got = sim.get_particles(s, with_id=True)
+        o = np.argsort(got["id"])
+        assert np.array_equal(got["id"][o], ref["id"])
+        ulp = np.abs(got["w"][o].view(np.int32).astype(np.int64) - ref["w"].view(np.int32).astype(np.int64))
+        assert ulp.max() <= 1
+        w = ref["w"].astype(np.float64)
+        mid = (ref["ix"] == 36)
+        edge, centre = w[mid & (ref["iy"] == 0)].mean(), w[mid & (ref["iy"] == 32)].mean()
+        assert edge / centre == pytest.approx(0.01 + 0.99 * math.sin(0.5 * math.pi * 0.5 / 9) ** 2, rel=1e-6)
+        assert w[mid & (ref["iy"] == 63)].mean() == pytest.approx(edge, rel=1e-6)
+    orc, _ = oracle_from_config(cfg)
+    sim.step(10)
+    orc.step(10)
+    for s in (0, 1):
+        assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < 1e-5
+    a = sim.get_fields(P.FIELD_A, 0, 0)
+    assert np.abs(a - orc.a_now[0]).max() < 2e-5 * np.abs(orc.a_now[0]).max() + 1e-9
+    sim.close()
+    bad = small_cfg("c5", 48, 64)
+    bad["profile"]["taper_cells_y"] = 4
+    with pytest.raises(P.PM2DError):
+        P.PM2D(bad)
