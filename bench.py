@@ -108,6 +108,16 @@ def sample_config(name, nx, ny):
     return I.config(name, nx=nx, ny=ny)
 
 
+def workload_name(name, full_cfg, nmob=None):
+    """config.workload of both arms: the full-size workload, whatever sample of it a CPU arm times."""
+    g = full_cfg["grid"]
+    if nmob is None:
+        nmob = sum(I.n_particles(full_cfg, s) for s, sp in enumerate(full_cfg["species"]) if sp["mobile"])
+    src = (f"(BASELINE.json configs[{int(name[1]) - 1}])" if name != "cbet" else
+           "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)")
+    return f"{name}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU {src}"
+
+
 def run_reference(args):
     """--impl reference: the oracle on host cores, same metric/config keys; each step is a bounded
     sample (a 512x256 copy of the workload: same dx, dt, particles per cell, profile, species, laser)."""
@@ -120,7 +130,7 @@ def run_reference(args):
     line = dict(impl="reference", metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=args.gpus,
                 steps=args.steps, warmup=args.warmup, ms_per_step=sec_per_step * 1e3, higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} SRS-scale slab (BASELINE.json configs[2])",
+                config=dict(workload=workload_name(args.config, I.config(args.config)),
                             sample=f"{cfg['name']} reduced copy, {nmob} mobile particles"),
                 cpu_baseline=dict(value=value, unit="particle-steps/s", cores=1, kind="oracle",
                                   sample=f"{cfg['name']}: {nmob} mobile particles x {args.steps} steps"),
@@ -215,9 +225,7 @@ def run_cuda(args):
         line = dict(metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=world, steps=args.steps,
                     warmup=args.warmup, ms_per_step=ms_max / args.steps, higher_is_better=True, scaling="weak",
                     vs_baseline=None, dtype="f32", data="synthetic",
-                    config=dict(workload=f"{args.config}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU "
-                                         + (f"(BASELINE.json configs[{int(args.config[1]) - 1}])" if args.config != "cbet" else
-                                            "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)"),
+                    config=dict(workload=workload_name(args.config, cfg, nmob),
                                 shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
                                 eager_moments=bool(args.eager), subcycle=int(g.get("subcycle", 1)), bc_y=("absorbing" if g.get("bc_y", 0) else "periodic"), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
                                 l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
