@@ -319,6 +319,8 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
 // particles a strip thread cannot serve from its register patch are listed per CTA and processed by all
 // threads after the strips (no divergence inside the strip loops); a full list spills to the global one
 constexpr int STRAY_CAP = 2048;
+constexpr int STRIP_SPLIT = 64;             // CTAs that may share one tile in k_stage
+constexpr int SPLIT_PARTICLES = 16384;      // ... one per so many particles of the tile
 constexpr int PF_ROWS = 2;            // L2 prefetch distance of the strips, in cell rows
 constexpr bool SHIFT_PATCH = true;   // one copy of the particle loop (instruction cache) at the price of register moves per cell
 constexpr uint32_t STRAY_DEP = 0x80000000u;            // flag: deposit only
@@ -386,6 +388,7 @@ struct StripCtx {
     int64_t t0;                  // first slot of the tile
     int32_t n_tile;              // particles in the tile
     const int32_t *coff;         // shared: coff[c] = first slot (tile-relative) of cell c = row * TILE + column
+    const int32_t *cend;         // shared: one past the last slot of cell c that this CTA serves (tile split)
     uint32_t ay_fix;
     int j, wc0, tile, gx0;
     const float2 *Fs;
@@ -529,7 +532,7 @@ template <int SHAPE, int STAGE, int QMASK, int ROT, bool SHIFT>
 __device__ __forceinline__ void strip_cell(const PartParams &P, Patch &pt, StripCtx &c, const int i)
 {
     const int cell = i * TILE + c.j;
-    const int32_t beg = c.coff[cell], end = c.coff[cell + 1];
+    const int32_t beg = c.coff[cell], end = c.cend[cell];
     const int32_t next_beg = c.coff[min(cell + TILE, TCELLS)];          // where this thread reads next
     const uint32_t ax_fix = (uint32_t)(i + POS_BIAS) << POS_FRAC_BITS;
     // the lanes of a warp walk their cells in lockstep: a cell much fuller than the tile's mean would stall
@@ -594,11 +597,18 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     __shared__ int32_t dep[NQ * WIN * WPITCH];
     __shared__ float2 Fs[(STAGE < 2) ? WIN * WPITCH : 1];
     __shared__ int32_t coff[TCELLS + 1];
+    __shared__ int32_t cend[TCELLS];
     __shared__ uint32_t slist[STRAY_CAP];
     __shared__ int scount;
-    const int tile = blockIdx.x;
+    // a tile is served by up to STRIP_SPLIT CTAs (blockIdx = tile * STRIP_SPLIT + part), one per SPLIT_PARTICLES
+    // particles: part k of n takes the k-th n-th of every cell's run.  A filament tile of BJ config 5 holds 1.2 M
+    // particles; as one CTA's work it would set the tail of the launch and overrun the CTA's stray list.
+    const int tile = blockIdx.x / STRIP_SPLIT, part = blockIdx.x % STRIP_SPLIT;
     const int64_t t0 = P.tile_off[tile];
-    if (P.tile_off[tile + 1] == t0) return;
+    const int64_t tile_n = P.tile_off[tile + 1] - t0;
+    if (tile_n == 0) return;
+    const int nsplit = (int)min((int64_t)STRIP_SPLIT, (tile_n + SPLIT_PARTICLES - 1) / SPLIT_PARTICLES);
+    if (part >= nsplit) return;
     const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
 
     {
@@ -617,6 +627,29 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
             if (e <= TCELLS) coff[e] = v[k];
         }
     }
+    if (nsplit > 1) {   // this CTA's share of every cell's run: [beg + len * part / nsplit, beg + len * (part + 1) / nsplit)
+        __syncthreads();
+        constexpr int IT = (TCELLS + NT - 1) / NT;
+        int32_t b[IT], e2[IT];
+#pragma unroll
+        for (int k = 0; k < IT; k++) {
+            const int e = threadIdx.x + k * NT;
+            if (e < TCELLS) {
+                const int64_t lo = coff[e], len = coff[e + 1] - lo;
+                b[k] = (int32_t)(lo + len * part / nsplit);
+                e2[k] = (int32_t)(lo + len * (part + 1) / nsplit);
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < IT; k++) {
+            const int e = threadIdx.x + k * NT;
+            if (e < TCELLS) { coff[e] = b[k]; cend[e] = e2[k]; }
+        }
+    } else {
+        __syncthreads();
+        for (int e = threadIdx.x; e < TCELLS; e += NT) cend[e] = coff[e + 1];
+    }
     for (int e = threadIdx.x; e < NQ * WIN * WPITCH; e += NT) dep[e] = 0;
     if (threadIdx.x == 0) scount = 0;
     __syncthreads();
@@ -626,6 +659,7 @@ __global__ void __launch_bounds__(TCELLS / S, S >= 8 ? 4 : 2) k_stage(const Part
     ctx.t0 = t0;
     ctx.n_tile = coff[TCELLS];
     ctx.coff = coff;
+    ctx.cend = cend;
     ctx.ay_fix = (uint32_t)(j + POS_BIAS) << POS_FRAC_BITS;
     ctx.j = j; ctx.wc0 = j - 1 + HALO; ctx.tile = tile; ctx.gx0 = gx0;
     ctx.Fs = Fs; ctx.dep = dep; ctx.slist = slist; ctx.scount = &scount;
@@ -1640,7 +1674,7 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
             k_stage_direct<SHAPE, ST, Q, true><<<grid, 256, direct_smem_bytes<ST, Q, true>(), st>>>(P); \
         } else if (sparse)                                                         \
             k_stage_direct<SHAPE, ST, Q, false><<<grid, 256, direct_smem_bytes<ST, Q, false>(), st>>>(P); \
-        else k_stage<SHAPE, ST, Q, STRIP><<<grid, TCELLS / STRIP, 0, st>>>(P);     \
+        else k_stage<SHAPE, ST, Q, STRIP><<<grid * STRIP_SPLIT, TCELLS / STRIP, 0, st>>>(P); \
         k_stage_overflow<SHAPE, ST, Q><<<148 * 8, 128, 0, st>>>(P);                    \
     } while (0)
     if (stage == 0) { if (qmask == 3) PM2D_LAUNCH(0, 3); else PM2D_LAUNCH(0, 1); }

@@ -228,7 +228,7 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
                         _species(+1, 3672.0, 1.0, 1, 1, SINE, 1.9)]
         c["lasers"] = [_laser(0.03, w0=0.3, y0=0.5)]     # w0, y0 in units of Ly, resolved below
     elif name == "c5":    # stress: 4096x4096, ~60 e/cell (1.0e9), 5 keV, Gaussian filament in y (peak 20x mean, sigma 64 cells)
-        c = _base(4096, 4096, 0.035, 50, 4, rebin_every=8)     # cell-major + strip kernel: the register patches want fresh cells
+        c = _base(4096, 4096, 0.035, 50, 4, rebin_every=4)     # cell-major + strip kernel: the register patches want fresh cells
         c["profile"] = dict(kind=PROFILE_FILAMENT_Y, p=[0.01, 87.7, 64.0, 0])
         c["species"] = [_species(-1, 1.0, 5.0, 10, 6, SINE, 1.9, load=NUMBER_WEIGHTED),
                         _species(+1, 1836.0, 0.0, 0, 0, SINE, 1.9, mobile=0, load=LOAD_NONE)]
