@@ -318,7 +318,7 @@ __device__ __forceinline__ bool process_direct(const PartParams &P, int64_t p, b
 
 // particles a strip thread cannot serve from its register patch are listed per CTA and processed by all
 // threads after the strips (no divergence inside the strip loops); a full list spills to the global one
-constexpr int STRAY_CAP = 2048;
+constexpr int STRAY_CAP = 1024;
 constexpr int STRIP_SPLIT = 64;             // CTAs that may share one tile in k_stage
 constexpr int SPLIT_PARTICLES = 16384;      // ... one per so many particles of the tile
 constexpr int PF_ROWS = 2;            // L2 prefetch distance of the strips, in cell rows
