@@ -928,3 +928,26 @@ def test_y_taper_loader_and_run_parity(P):
     bad["profile"]["taper_cells_y"] = 4
     with pytest.raises(P.PM2DError):
         P.PM2D(bad)
+
+
+@pytest.mark.gpu
+def test_strip_kernel_split_tiles_parity(P):
+    """k_stage serves a tile of more than 16384 particles with several CTAs (each takes its share of every cell's
+    run; SPLIT_PARTICLES in pm2d_particles.cu).  The reduced config 5 has such tiles (asserted): 6 steps across a
+    rebin, deposits and every particle against the oracle."""
+    cfg = small_cfg("c5", 48, 64)
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, particle_order=P.ORDER_CELL_MAJOR)
+    got = sim.get_particles(0, with_id=True)
+    per_tile = np.bincount((got["ix"] // P.TILE) * 2 + got["iy"] // P.TILE)
+    assert per_tile.max() > 2 * 16384                      # at least three CTAs on the fullest tile
+    orc, _ = oracle_from_config(cfg)
+    sim.step(6)
+    orc.step(6)
+    for name, m in (("n", P.MOMENT_N), ("Px", P.MOMENT_PX), ("Py", P.MOMENT_PY)):
+        ref = orc.moment(0, name)
+        assert np.sqrt(((sim.get_moments(0, m) - ref) ** 2).sum() / (orc.moment(0, "n") ** 2).sum()) < 1e-5, name
+    got = sim.get_particles(0, with_id=True)
+    o = np.argsort(got["id"])
+    assert np.abs(got["ux"][o] - orc.sp[0]["ux"]).max() < 2e-6
+    assert np.abs(got["ix"][o] + got["fx"][o].astype(np.float64) - orc.sp[0]["X"]).max() < 1e-4
+    sim.close()
