@@ -15,7 +15,10 @@
  *   particle positions X, Y are in CELL units (x = X*dx), velocities in c, weights in n_c.
  *   lengths in lambda0, times in T0, u in c, E in 2 pi c omega0 m_e / e.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P13 of DESIGN.md section 4.
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P14 of DESIGN.md section 3; the S8(f) widenings in
+ * tests/test_oracle_next.py: P15 oblique incidence, P16 sub-cycling, P17 mode amplitudes, P18 velocity
+ * histogram, P19 absorbing y walls and corners (Q23), P20 boundary records and their spectrum.
+ * Eq. 21 (SBS growth rate) is not pinned.
  * Parity unpinned (conventions only, identical by construction on both sides): Q3 (E to nodes),
  * Q5 (Dirichlet phi at the x walls), Q9 (wall folding), Q13, Q14, Q17.
  */
