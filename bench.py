@@ -257,7 +257,8 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=32,
+                    help="timed steps; the default spans two rebin periods of c3, so the rebin's share is its long-run share")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "cbet"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
