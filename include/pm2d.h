@@ -74,8 +74,12 @@ enum {
  * pseudo-random permutation with an explicit tile index each (+4 B per particle); no tile is staged: every particle
  * gathers from the global force grid and deposits with integer atomics on the global grids (L2).  No rebin (the
  * positions stay relative to the tile a particle was loaded into: a run may drift at most 64 cells from it, else
- * PM2D_ESTATE), pm2d_rebin and pm2d_set_particles return PM2D_ESTATE.  It exists to measure what the sort buys. */
-enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2, PM2D_ORDER_RANDOM = 3 };
+ * PM2D_ESTATE), pm2d_rebin and pm2d_set_particles return PM2D_ESTATE.  It exists to measure what the sort buys.
+ * LANES (what AUTO picks up to 16 particles per cell; never for PM2D_NUMBER_WEIGHTED): inside a sub-tile (a whole
+ * tile, or for species that drift a cell or more per rebin period its two halves of 16 cell rows) the particles are
+ * ranked by y and cut into 32 slabs of equal population; slot = 32 * (rank in x inside the slab) + slab, so lane i of a
+ * warp always works on slab i and its shared-memory accesses fall on its own bank (pm2d_lanes.cu); see pm2d_rebin. */
+enum { PM2D_ORDER_AUTO = 0, PM2D_ORDER_CELL_MAJOR = 1, PM2D_ORDER_LAYERED = 2, PM2D_ORDER_RANDOM = 3, PM2D_ORDER_LANES = 4 };
 enum { PM2D_BC_Y_PERIODIC = 0, PM2D_BC_Y_ABSORB = 1 };
 enum { PM2D_MOMENT_N = 0, PM2D_MOMENT_PX = 1, PM2D_MOMENT_PY = 2 }; /* n_s, (n u_x)_s, (n u_y)_s, Eq. 14 */
 
@@ -214,7 +218,12 @@ int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
  * receives for every NEW slot the OLD slot it came from.  CELL_MAJOR species: the result equals a stable counting
  * sort by key.  LAYERED species: with r = the rank of a particle among those of equal key in the old order, the
  * result is sorted by tile, then layer min(r, 16); inside a layer below 16 by (rank of the cell among the cells of
- * the same tile and the same iy that hold more than r particles, in ix order; iy), inside the tail by (cell, r). */
+ * the same tile and the same iy that hold more than r particles, in ix order; iy), inside the tail by (cell, r).
+ * LANES species: after the stable sort by tile, inside every tile: h = sub-tile (ix % 32 >= 16 when pm2d_lane_subs is 2,
+ * else 0); rho = rank in the stable sort by key_A = (h, iy % 32, floor(32 fy)); slab = the rho-th of the N_h particles
+ * of the sub-tile cut into 32 slabs whose sizes differ by at most one (the first N_h mod 32 slabs hold one more);
+ * w = rank inside the slab in the stable sort by key_B = (h, slab, x bin), x bin = (2 (ix % 16) + floor(2 fx)) resp.
+ * ix % 32; slot = first slot of the sub-tile + 32 w + slab. */
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);
@@ -262,6 +271,9 @@ int64_t pm2d_launch_count(pm2d_ctx *ctx);
  * register patch (the particle had drifted more than half a cell from its cell of the last rebin) but
  * from the tile's shared windows or the global grids.  Synchronises the stream; resets the counter. */
 int64_t pm2d_stray_count(pm2d_ctx *ctx);
+/* Lane order of a species: sub-tiles per tile (2: two halves of 16 cell rows; 1: whole tiles), 0 if the species is
+ * stored in another order, negative code on a bad argument. */
+int pm2d_lane_subs(pm2d_ctx *ctx, int species);
 
 void pm2d_free(pm2d_ctx *ctx);
 const char *pm2d_last_error(void);

@@ -22,7 +22,7 @@ PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 
 FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
 BC_Y_PERIODIC, BC_Y_ABSORB = 0, 1
-ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, ORDER_RANDOM, LAYERS = 0, 1, 2, 3, 16
+ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, ORDER_RANDOM, ORDER_LANES, LAYERS = 0, 1, 2, 3, 4, 16
 PHASES = ("field", "poisson", "force", "stage_a", "stage_b", "rebin")
 
 
@@ -85,6 +85,7 @@ SYMBOLS = {
     "pm2d_profile_get": (C.c_int, [_vp, C.POINTER(C.c_double), _lp, _lp]),
     "pm2d_launch_count": (C.c_int64, [_vp]),
     "pm2d_stray_count": (C.c_int64, [_vp]),
+    "pm2d_lane_subs": (C.c_int, [_vp, C.c_int]),
     "pm2d_free": (None, [_vp]),
     "pm2d_last_error": (C.c_char_p, []),
     "pm2d_version": (C.c_char_p, []),
@@ -322,3 +323,6 @@ class PM2D:
 
     def stray_count(self):
         return int(_check(self.lib.pm2d_stray_count(self.ctx)))
+
+    def lane_subs(self, s):
+        return int(_check(self.lib.pm2d_lane_subs(self.ctx, int(s))))

@@ -8,9 +8,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpm2d.so")
-SOURCES = ["pm2d_api.cu", "pm2d_particles.cu", "pm2d_fields.cu", "pm2d_poisson.cu", "pm2d_diag.cu"]
+SOURCES = ["pm2d_api.cu", "pm2d_particles.cu", "pm2d_lanes.cu", "pm2d_fields.cu", "pm2d_poisson.cu", "pm2d_diag.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-diag-suppress", "128", "-Wno-deprecated-gpu-targets", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-diag-suppress", "128", "-Wno-deprecated-gpu-targets"]
 
 
 def _stale() -> bool:
@@ -25,7 +25,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    flags = list(NVCC_FLAGS)
     objs = []
     procs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)

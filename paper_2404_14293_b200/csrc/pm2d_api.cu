@@ -71,7 +71,7 @@ int validate(const pm2d_grid *g, const pm2d_species *sp, int nsp)
     if (!is_pow2(g->ny) || g->ny < 8 || g->ny > 8192) return fail(PM2D_EINVAL, "ny must be a power of two in [8, 8192]");
     if (g->ncomp < 1 || g->ncomp > 3) return fail(PM2D_EINVAL, "ncomp must be 1..3");
     if (g->rebin_every < 0 || g->rebin_every > 32) return fail(PM2D_EINVAL, "rebin_every must be 0..32");
-    if (g->particle_order < PM2D_ORDER_AUTO || g->particle_order > PM2D_ORDER_RANDOM) return fail(PM2D_EINVAL, "unknown particle_order");
+    if (g->particle_order < PM2D_ORDER_AUTO || g->particle_order > PM2D_ORDER_LANES) return fail(PM2D_EINVAL, "unknown particle_order");
     if (!(g->dx > 0) || !(g->dy > 0) || !(g->dt > 0)) return fail(PM2D_EINVAL, "dx, dy, dt must be positive");
     if (g->dt / g->dx > 0.999 || g->dt / g->dy > 0.999)
         return fail(PM2D_EINVAL, "dt/dx must be < 1: a particle may not cross more than one cell per step");
@@ -144,15 +144,31 @@ size_t layout(pm2d_ctx *c, char *base)
         S.pxfix = S.pyfix = nullptr; S.F = nullptr;
         S.np = S.cap = species_np(g, S.cfg);
         S.layered = false;
+        S.lanes = false;
+        S.lane_subs = 1;
+        S.sub0 = nullptr;
+        S.lane_exp = nullptr;
         S.random = false;
         S.ptile = nullptr;
         if (!S.cfg.mobile) continue;
         S.random = g.particle_order == PM2D_ORDER_RANDOM;
         // layered order + thread-per-particle kernel up to 16 particles per cell on average; the number-weighted
         // loader fills cell runs, so it stays cell-major
-        if (S.cfg.load != PM2D_NUMBER_WEIGHTED)
-            S.layered = g.particle_order == PM2D_ORDER_LAYERED ||
-                        (g.particle_order == PM2D_ORDER_AUTO && S.cap <= (int64_t)PM2D_LAYERS * g.nx * g.ny);
+        // lane order + k_stage_lanes up to 16 particles per cell on average; the number-weighted loader follows a
+        // profile in y (the lanes assume a population that is uniform in y) and fills cell runs: cell-major
+        if (S.cfg.load != PM2D_NUMBER_WEIGHTED) {
+            S.layered = g.particle_order == PM2D_ORDER_LAYERED;
+            S.lanes = g.particle_order == PM2D_ORDER_LANES ||
+                      (g.particle_order == PM2D_ORDER_AUTO && S.cap <= (int64_t)PM2D_LAYERS * g.nx * g.ny);
+        }
+        if (S.lanes) {
+            // thermal drift over a rebin period, in cells: below a tenth of a cell two window copies on whole tiles do
+            const double drift = std::sqrt(S.cfg.T_keV / 511.0 / S.cfg.mass) * (g.subcycle > 1 ? g.subcycle : 1) * g.dt / std::min(g.dx, g.dy) *
+                                 (double)(g.rebin_every > 0 ? g.rebin_every : 32);
+            S.lane_subs = drift < 0.1 ? 1 : 2;
+            S.sub0 = cv.take<int32_t>(ntiles);
+            S.lane_exp = cv.take<int32_t>(ntiles);
+        }
         S.pxfix = cv.take<int32_t>(nn);
         S.pyfix = cv.take<int32_t>(nn);
         S.nhat = cv.take<int32_t>(nn);
@@ -211,6 +227,7 @@ int check_flags(pm2d_ctx *c)
     if (h[0]) return fail(PM2D_ESTATE, "a particle moved further than one tile between rebins (rebin_every too large)");
     if (h[1]) return fail(PM2D_ESTATE, "chunk table overflow");
     if (h[2]) return fail(PM2D_ESTATE, "too many particles outside their tile window (rebin_every too large)");
+    if (h[3]) return fail(PM2D_ESTATE, "lane order: a tile holds more than 65535 particles (use PM2D_ORDER_CELL_MAJOR)");
     return PM2D_OK;
 }
 
@@ -408,9 +425,11 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     for (int s = 0; s < nsp; s++) {
         SpeciesDev &S = c->sp[s];
         if (!S.cfg.mobile) continue;
+        if (S.lanes) INIT_CHECK(lanes_make_tensor_map(c, s));
         if (S.cfg.load != PM2D_LOAD_NONE) {
             INIT_CHECK(launch_load_particles(c, s));
             if (S.random) INIT_CHECK(launch_shuffle_random(c, s));
+            if (S.lanes) INIT_CHECK(launch_lanesort(c, s, true, nullptr, nullptr, nullptr));
         } else {
             S.np = 0;   // until pm2d_set_particles
             INIT_CHECK(launch_build_chunks(c, s));   // all-zero tile_off -> zero chunks
@@ -539,6 +558,11 @@ extern "C" int64_t pm2d_stray_count(pm2d_ctx *c)
     PM2D_CUDA_CHECK(cudaMemsetAsync(c->stray_total, 0, sizeof(h), c->stream));
     PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     return (int64_t)h;
+}
+extern "C" int pm2d_lane_subs(pm2d_ctx *c, int s)
+{
+    if (!c || s < 0 || s >= c->nsp) return fail(PM2D_EINVAL, "bad species");
+    return c->sp[s].lanes ? c->sp[s].lane_subs : 0;
 }
 extern "C" int64_t pm2d_particle_count(pm2d_ctx *c, int s) { return (c && s >= 0 && s < c->nsp) ? c->sp[s].np : -1; }
 
@@ -768,6 +792,7 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
     S.np = count;
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
+    if (S.lanes && (rc = launch_lanesort(c, s, true, nullptr, nullptr, nullptr))) return rc;
     if ((rc = redeposit(c, s))) return rc;
     if (refix_background && (rc = refix_backgrounds(c))) return rc;
     return check_flags(c);   // synchronises: the host vectors may now go

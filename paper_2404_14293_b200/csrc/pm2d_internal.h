@@ -40,6 +40,11 @@ struct SpeciesDev {
     int32_t *ptile;      // [cap] tile of every particle (random order only)
     bool layered;        // storage order inside a tile: (rank in cell, cell) + thread-per-particle stage kernel;
                          // else (cell, rank) + strip kernel
+    bool lanes;          // PM2D_ORDER_LANES: slot = 32 * (rank in x inside a y-slab) + y-slab; k_stage_lanes (pm2d_lanes.cu)
+    int lane_subs;       // sub-tiles per tile in the lane order: 2 (16 cell rows each; hot species, 4 window copies) or 1
+    int32_t *sub0;       // [ntiles] lane order: particles of sub-tile 0 of every tile (the tile's first sub0[t] slots)
+    alignas(64) unsigned long long tmapF[16];   // CUtensorMap of F (lane order: the force windows are bulk-async box loads)
+    int32_t *lane_exp;   // [ntiles] lane order: window units of the tile, sn | sp << 8 (pm2d_lanes.cu)
     // particles (device), stored tile by tile and, inside a tile, cell by cell (as of the last rebin)
     PV *pv;              // position + velocity
     float *w;            // density weight
@@ -143,6 +148,11 @@ int launch_rebin(pm2d_ctx *c, int s, int32_t *keys_dev, int64_t *perm_dev, int64
 int launch_set_cell_offsets_uniform(pm2d_ctx *c, int s);
 int launch_build_chunks(pm2d_ctx *c, int s);
 int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float *fx, float *fy, float *ux, float *uy);
+// pm2d_lanes.cu
+int launch_lanesort(pm2d_ctx *c, int s, bool from_primary, int32_t *keys_dev, int64_t *perm_dev, const int64_t *perm1_dev);
+int launch_stage_lanes(pm2d_ctx *c, int s, int stage, int qmask);
+double lane_ucap(const SpeciesDev &S);
+int lanes_make_tensor_map(pm2d_ctx *c, int s);
 // pm2d_fields.cu
 int launch_field_step(pm2d_ctx *c, int sub);
 int launch_force(pm2d_ctx *c, int s, const float *a_level);

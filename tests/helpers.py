@@ -51,9 +51,11 @@ def oracle_from_config(cfg, particles=None):
 
 # ---- quasi-1D SRS slab (paper section 6.1: a0 = 0.06, 0.15 n_c, dx = 0.05, dt = 0.035, 1 particle per cell,
 # DD = 1.6 dx), cold and with the pressure term off so that the vacuum edges stay put
-def srs_slab(nx=1600, ny=8, dx=0.05, n0=0.15, seed=1):
+def srs_slab(nx=1600, ny=8, dx=0.05, n0=0.15, seed=1, ripple=0.0, k_ripple=0.0):
     """Particles (canonical form) of a slab with 8 lambda0 vacuum margins and 5 lambda0 sin^2 ramps, one per
-    cell at the cell centre plus 1e-3 cell of seeded position noise in x."""
+    cell at the cell centre plus 1e-3 cell of seeded position noise in x.  ripple > 0: plus a coherent displacement
+    ripple * sin(2 pi k_ripple x) cells (k_ripple in 1/lambda0), a plasma-wave seed far above the rounding noise of
+    a float32 run."""
     def prof(x_cells):
         x, Lx, r = x_cells * dx, nx * dx, 5.0
         up, dn = np.clip((x - 8.0) / r, 0, 1), np.clip((Lx - 8.0 - x) / r, 0, 1)
@@ -63,7 +65,8 @@ def srs_slab(nx=1600, ny=8, dx=0.05, n0=0.15, seed=1):
     keep = w > 0
     ix, iy, w = ix[keep].astype(np.int32), iy[keep].astype(np.int32), w[keep].astype(np.float32)
     rng = np.random.default_rng(seed)
-    fx = (np.floor((0.5 + 1e-3 * rng.standard_normal(ix.size)) * 2 ** 24) / 2 ** 24).astype(np.float32)
+    disp = 1e-3 * rng.standard_normal(ix.size) + ripple * np.sin(2.0 * np.pi * k_ripple * (ix + 0.5) * dx)
+    fx = (np.floor((0.5 + disp) * 2 ** 24) / 2 ** 24).astype(np.float32)
     z = np.zeros(ix.size, np.float32)
     return dict(ix=ix, iy=iy, fx=fx, fy=np.full(ix.size, 0.5, np.float32), ux=z, uy=z.copy(), w=w)
 
