@@ -146,26 +146,30 @@ size_t layout(pm2d_ctx *c, char *base)
         S.layered = false;
         S.lanes = false;
         S.lane_subs = 1;
+        S.lane_copies = 2;
         S.sub0 = nullptr;
         S.lane_exp = nullptr;
         S.random = false;
         S.ptile = nullptr;
         if (!S.cfg.mobile) continue;
         S.random = g.particle_order == PM2D_ORDER_RANDOM;
-        // layered order + thread-per-particle kernel up to 16 particles per cell on average; the number-weighted
-        // loader fills cell runs, so it stays cell-major
-        // lane order + k_stage_lanes up to 16 particles per cell on average; the number-weighted loader follows a
-        // profile in y (the lanes assume a population that is uniform in y) and fills cell runs: cell-major
+        // AUTO, up to 16 particles per cell on average: the lane order + k_stage_lanes, except for species that drift a cell
+        // or more per rebin period AND hold fewer than 3 particles per cell -- there the half-tile windows of the
+        // four-copy variant serve too few particles each and the layered order + k_stage_direct wins (cbet electrons,
+        // 1 per cell: stage kernels 5.5 against 6.5 ms, rebin 1.2 against 2.1 ms per step, r02j).  The number-weighted
+        // loader follows a profile in y (the lanes assume a population that is uniform in y) and fills cell runs: cell-major.
+        // thermal drift over a rebin period, in cells: below a tenth of a cell two window copies on whole tiles do
+        const double drift = std::sqrt(S.cfg.T_keV / 511.0 / S.cfg.mass) * (g.subcycle > 1 ? g.subcycle : 1) * g.dt / std::min(g.dx, g.dy) *
+                             (double)(g.rebin_every > 0 ? g.rebin_every : 32);
         if (S.cfg.load != PM2D_NUMBER_WEIGHTED) {
-            S.layered = g.particle_order == PM2D_ORDER_LAYERED;
-            S.lanes = g.particle_order == PM2D_ORDER_LANES ||
-                      (g.particle_order == PM2D_ORDER_AUTO && S.cap <= (int64_t)PM2D_LAYERS * g.nx * g.ny);
+            const bool sparse = g.particle_order == PM2D_ORDER_AUTO && S.cap <= (int64_t)PM2D_LAYERS * g.nx * g.ny;
+            const bool thin_hot = drift >= 0.1 && S.cap < (int64_t)3 * g.nx * g.ny;
+            S.lanes = g.particle_order == PM2D_ORDER_LANES || (sparse && !thin_hot);
+            S.layered = g.particle_order == PM2D_ORDER_LAYERED || (sparse && thin_hot);
         }
         if (S.lanes) {
-            // thermal drift over a rebin period, in cells: below a tenth of a cell two window copies on whole tiles do
-            const double drift = std::sqrt(S.cfg.T_keV / 511.0 / S.cfg.mass) * (g.subcycle > 1 ? g.subcycle : 1) * g.dt / std::min(g.dx, g.dy) *
-                                 (double)(g.rebin_every > 0 ? g.rebin_every : 32);
-            S.lane_subs = drift < 0.1 ? 1 : 2;
+            S.lane_copies = drift < 0.1 ? 2 : 4;
+            S.lane_subs = S.lane_copies == 4 ? 2 : 1;
             S.sub0 = cv.take<int32_t>(ntiles);
             S.lane_exp = cv.take<int32_t>(ntiles);
         }

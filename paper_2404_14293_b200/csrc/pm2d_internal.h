@@ -41,6 +41,7 @@ struct SpeciesDev {
     bool layered;        // storage order inside a tile: (rank in cell, cell) + thread-per-particle stage kernel;
                          // else (cell, rank) + strip kernel
     bool lanes;          // PM2D_ORDER_LANES: slot = 32 * (rank in x inside a y-slab) + y-slab; k_stage_lanes (pm2d_lanes.cu)
+    int lane_copies;     // window copies of k_stage_lanes: 4 (species that drift a cell or more per rebin period) or 2
     int lane_subs;       // sub-tiles per tile in the lane order: 2 (16 cell rows each; hot species, 4 window copies) or 1
     int32_t *sub0;       // [ntiles] lane order: particles of sub-tile 0 of every tile (the tile's first sub0[t] slots)
     alignas(64) unsigned long long tmapF[16];   // CUtensorMap of F (lane order: the force windows are bulk-async box loads)
