@@ -91,11 +91,9 @@ class ClockSampler(threading.Thread):
 
 def time_oracle(cfg, steps, warmup):
     """The CPU oracle as it stands (single thread, double precision) on a reduced copy of the workload."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
     import oracle
-    from helpers import oracle_from_config
     oracle.build()
-    orc, parts = oracle_from_config(cfg)
+    orc, parts = oracle.from_config(cfg)
     nmob = sum(len(p["ix"]) for s, p in enumerate(parts) if p is not None and cfg["species"][s]["mobile"])
     orc.step(warmup)
     t0 = time.perf_counter()
@@ -111,8 +109,9 @@ def sample_config(name, nx, ny):
 def workload_name(name, full_cfg, nmob=None):
     """config.workload of both arms: the full-size workload, whatever sample of it a CPU arm times."""
     g = full_cfg["grid"]
-    if nmob is None:
-        nmob = sum(I.n_particles(full_cfg, s) for s, sp in enumerate(full_cfg["species"]) if sp["mobile"])
+    if nmob is None:                      # the CPU arm: counted by the oracle's loader
+        import oracle.loader as L
+        nmob = sum(L.n_particles(full_cfg, s) for s, sp in enumerate(full_cfg["species"]) if sp["mobile"])
     src = (f"(BASELINE.json configs[{int(name[1]) - 1}])" if name != "cbet" else
            "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)")
     return f"{name}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU {src}"
@@ -132,7 +131,7 @@ def run_reference(args):
                 vs_baseline=None, dtype="f64", data="synthetic",
                 config=dict(workload=workload_name(args.config, I.config(args.config)),
                             sample=f"{cfg['name']} reduced copy, {nmob} mobile particles"),
-                cpu_baseline=dict(value=value, unit="particle-steps/s", cores=1, kind="oracle",
+                cpu_baseline=dict(value=value, unit="particle-steps/s", cores=1, nproc=os.cpu_count(), kind="oracle",
                                   sample=f"{cfg['name']}: {nmob} mobile particles x {args.steps} steps"),
                 e2e=dict(value=value, unit="particle-steps/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line))
@@ -213,13 +212,23 @@ def run_cuda(args):
         steps_p = max(prof["steps"], 1)
         stage_ms = (prof["ms"]["stage_a"] + prof["ms"]["stage_b"]) / steps_p
         per_particle = BYTES_STAGE_A + BYTES_STAGE_B + (8 if args.order == "random" else 0)   # random order: + the tile index, read at both stages
+        # SURVEY 8(d)'s strict minimum: state read at both stages, written once = 56 B; 48 B where the weights are one
+        # constant (c1: uniform profile without y taper is still tapered in x, so only the number-weighted c5 qualifies)
+        uniform_w = all(sp["load"] == I.NUMBER_WEIGHTED for sp in cfg["species"] if sp["mobile"])
+        min_bytes = 48 if uniform_w else 56
         alg_bytes = per_particle * nmob
         achieved = alg_bytes / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
-        traffic = None
+        achieved_min = min_bytes * nmob / (stage_ms * 1e-3) / 1e9 if stage_ms > 0 else 0.0
+        # measured DRAM bytes of the stage launches of one step (ncu --set full), valid for the build that was profiled only
+        traffic, traffic_src = None, None
         tp = os.path.join(ROOT, "profiles", "stage_traffic_bytes.txt")
-        if os.path.exists(tp) and args.config == "c3" and world == 1:      # measured for c3 only
+        if os.path.exists(tp) and args.config == "c3" and world == 1 and args.order == "auto":
             try:
-                traffic = float(open(tp).read().split()[0])
+                tok = open(tp).read().split()
+                if tok[1] == sim.version().split("build ")[-1].rstrip(")"):
+                    traffic, traffic_src = float(tok[0]), tok[2]
+                else:
+                    traffic_src = f"stale: {tok[2]} was captured on build {tok[1]}"
             except Exception:
                 traffic = None
         line = dict(metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=world, steps=args.steps,
@@ -229,7 +238,8 @@ def run_cuda(args):
                                 shapes=[["cic", "tsc", "sine"][sp["shape"]] for sp in cfg["species"] if sp["mobile"]],
                                 eager_moments=bool(args.eager), subcycle=int(g.get("subcycle", 1)), bc_y=("absorbing" if g.get("bc_y", 0) else "periodic"), rebin_every=sim.grid.rebin_every, particle_order=args.order, preroll_steps=preroll,
                                 l2="inputs larger than L2 (particle state %.1f GB, grids %.1f GB)" % (nmob * 28 / 1e9, nodes * 60 / 1e9),
-                                parallelism="replicas only" if world > 1 else "1 GPU"),
+                                parallelism="replicas only" if world > 1 else "1 GPU",
+                                **({"particles_note": "BASELINE.json asks for 1.0e9; the x edge taper (Q9) of the number-weighted loading leaves 9.44e8"} if args.config == "c5" else {})),
                     ns_per_particle_step=1e9 / value * world,
                     cell_updates_per_s=nodes * g["ncomp"] * max(int(g.get("subcycle", 1)), 1) * world * args.steps / (ms_max * 1e-3),
                     field_kernel_node_updates_per_s=(nodes * g["ncomp"] * max(int(g.get("subcycle", 1)), 1) / (prof["ms"]["field"] / steps_p * 1e-3)) if prof["ms"]["field"] > 0 else None,
@@ -238,15 +248,18 @@ def run_cuda(args):
                     clocks=clocks, gpu_launches=int(launches),
                     e2e=dict(value=e2e_value, unit="particle-steps/s",
                              h2d_bytes_per_step=int(len(lasers) * 48), d2h_bytes_per_step=int(g["ny"] * 4 + 16)),
-                    roofline=dict(bound="hbm", kernel="k_stage (fused gather-push-deposit; per step: stage A + stage B launches of every mobile species)",
+                    rebin_share=(prof["ms"]["rebin"] / steps_p) / (ms_max / args.steps),
+                    roofline=dict(bound="hbm", kernel="k_stage_lanes / k_stage (fused gather-push-deposit; per step: stage A + stage B launches of every mobile species)",
                                   achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, peak_source=peak_src,
+                                  frac_basis=f"{per_particle} B per particle-step (the layout: stage A 28 + stage B 44)",
                                   algorithmic_bytes_per_particle_step=per_particle,
-                                  ms_per_step=stage_ms, traffic=traffic))
+                                  frac_min_bytes=achieved_min / peak, min_bytes_per_particle_step=min_bytes,
+                                  ms_per_step=stage_ms, traffic=traffic, traffic_source=traffic_src))
         if world == 1 and not args.no_cpu_baseline:
             # about 10-30 s of CPU work: c5 holds ~56 particles per cell, so its sample is a smaller box
             scfg = sample_config(args.config, 256, 256) if args.config == "c5" else sample_config(args.config, 1024, 512)
             v, sec, n = time_oracle(scfg, 8, 1)
-            line["cpu_baseline"] = dict(value=v, unit="particle-steps/s", cores=1, kind="oracle",
+            line["cpu_baseline"] = dict(value=v, unit="particle-steps/s", cores=1, nproc=os.cpu_count(), kind="oracle",
                                         sample=f"{scfg['name']} reduced copy of the workload: {n} mobile particles x 8 steps ({sec * 8:.1f} s)")
         print(json.dumps(line))
     sim.close()
@@ -257,8 +270,8 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=32,
-                    help="timed steps; the default spans two rebin periods of c3, so the rebin's share is its long-run share")
+    ap.add_argument("--steps", type=int, default=96,
+                    help="timed steps; the default spans six rebin periods of c3 (0.7 s: several clock samples, the rebin at its long-run share)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "cbet"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
@@ -267,12 +280,47 @@ def main():
     ap.add_argument("--order", default="auto", choices=["auto", "cellmajor", "layered", "random"],
                     help="particle storage order; random = BASELINE config 5 run A (no tile staging, global atomics, no rebin)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--selftest-cpu", action="store_true", help=argparse.SUPPRESS)   # the rank plumbing alone, gloo, no GPU (tests)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    if args.impl == "reference":
-        run_reference(args)
+    worker = run_reference if args.impl == "reference" else (run_selftest_cpu if args.selftest_cpu else run_cuda)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        spawn_ranks(args, worker)      # not under torchrun: start the N local ranks here
     else:
-        run_cuda(args)
+        worker(args)
+
+
+def _rank_entry(rank, args, worker, port):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(args.gpus), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    worker(args)
+
+
+def spawn_ranks(args, worker):
+    """`python bench.py --gpus N` without torchrun: one process per GPU on this node, the same environment torchrun
+    would set (replicas only: the ranks meet in the barrier and the MAX over their device times)."""
+    import socket
+
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    mp.spawn(_rank_entry, args=(args, worker, port), nprocs=args.gpus, join=True)
+
+
+def run_selftest_cpu(args):
+    """The multi-rank plumbing of run_cuda with the device work replaced by a fixed per-rank time (gloo, CPU): what the
+    world_size-2 test drives through the spawn entry."""
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+    value, ms_max = job_throughput(1000, args.steps, 10.0 + rank, world, None)
+    if rank == 0:
+        print(json.dumps(dict(metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=world, steps=args.steps,
+                              warmup=args.warmup, ms_per_step=ms_max / args.steps, scaling="weak", selftest=True)))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 if __name__ == "__main__":

@@ -62,7 +62,10 @@ enum {
     PM2D_FIELD_A = 0,      /* vector potential component `comp`, time level `level` (0 = n, 1 = n-1) */
     PM2D_FIELD_PHI = 1,    /* electrostatic potential on nodes (Eq. 3), recomputed from the current densities */
     PM2D_FIELD_ENODE = 2,  /* E averaged to nodes (Q3), comp 0 = x, 1 = y, from the current densities */
-    PM2D_FIELD_FORCE = 3   /* nodal force of species `level` (Eq. 16) for the current E, a^n, n^n; comp 0 = x, 1 = y */
+    PM2D_FIELD_FORCE = 3,  /* nodal force of species `level` (Eq. 16) for the current E, a^n, n^n; comp 0 = x, 1 = y.
+                              Produced by the launches of a step: the Poisson solve with the force epilogue of its inverse
+                              transform (what the stage kernels gather from) */
+    PM2D_FIELD_FORCE_REF = 4 /* the same force by the stand-alone kernel on the nodal E grid (cross-check of the epilogue) */
 };
 /* Storage order of a species inside a tile (as of the last rebin).  CELL_MAJOR: (cell, rank in cell), walked by
  * strip threads with register accumulation (dense species).  LAYERED: layer r < 16 holds particle number r of every
@@ -186,6 +189,16 @@ int pm2d_step(pm2d_ctx *ctx, int nsteps);
 /* Same, without the final synchronisation (the caller synchronises its stream). */
 int pm2d_step_async(pm2d_ctx *ctx, int nsteps);
 
+/* Polarisation decomposition of one beam (Fig. 1(a)): "assuming the direction of vector potential a has an angle
+ * of theta with respect to the z-axis, then the components of a in the S-polarization direction (z direction) is
+ * a_sz = a cos(theta) ... a_px = a sin(theta) cos(beta) and a_py = a sin(theta) sin(beta)".  Components of `a` are
+ * numbered 0 = z (S polarisation, the one BASELINE.json's configs use), 1 = x, 2 = y; every component obeys the same
+ * wave equation (Eq. 1), so the beam becomes up to three laser-table entries that differ in `a0` and `comp` only.
+ * proto: host, the beam (its a0 is the amplitude a, its comp is ignored); theta, beta in radians; out: host array of 3
+ * entries.  Returns the number of entries written (components whose amplitude is not exactly zero, in the order z, x,
+ * y), or PM2D_EINVAL on a null pointer.  The grid needs ncomp = 3 unless only the z entry comes back. */
+int pm2d_polarised_beam(const pm2d_laser *proto, double theta, double beta, pm2d_laser out[3]);
+
 /* Replace the laser table (e.g. a time-varying drive); nlaser <= PM2D_MAX_LASERS. */
 int pm2d_set_lasers(pm2d_ctx *ctx, const pm2d_laser *lasers, int nlaser);
 
@@ -203,6 +216,13 @@ int pm2d_set_fields(pm2d_ctx *ctx, int field, int comp, int level, const float *
  * Any output pointer may be NULL.  `id` needs track_ids.  Returns the number written. */
 int64_t pm2d_get_particles(pm2d_ctx *ctx, int species, int64_t first, int64_t count, int32_t *ix, int32_t *iy,
                            float *fx, float *fy, float *ux, float *uy, float *w, int64_t *id);
+/* Predictor velocities u^ (Eq. 17) that the last pm2d_step left for the slots first..first+count-1 of a
+ * species, in the storage order pm2d_get_particles had BEFORE that step (a step without rebin keeps the order).  For
+ * tests of the gather + predictor at full size.  uhx, uhy: host float[count].  PM2D_ESTATE when the arrays have been
+ * reused since (a rebin at the end of the step, pm2d_get_particles, pm2d_set_particles) or no step was taken.
+ * Returns the number written. */
+int64_t pm2d_get_predictor(pm2d_ctx *ctx, int species, int64_t first, int64_t count, float *uhx, float *uhy);
+
 /* Replace all particles of a mobile species (count <= capacity; any order; ids = 0..count-1 in
  * the order given), bin them, re-deposit every moment.  If `refix_background` != 0 the immobile
  * species of opposite sign are re-set to neutralise the new deposit (Q13). */

@@ -74,6 +74,8 @@ def lib():
         L.orc_deposit.argtypes = [C.POINTER(_Grid), C.c_int, C.c_double, C.c_int64] + [_dp] * 8
         L.orc_gather.restype = None
         L.orc_gather.argtypes = [C.POINTER(_Grid), C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
+        L.orc_polarised.restype = None
+        L.orc_polarised.argtypes = [C.c_double, C.c_double, C.c_double, _dp]
         L.orc_a_inc.restype = C.c_double
         L.orc_a_inc.argtypes = [C.POINTER(_Laser), C.c_double, C.c_double, C.c_double, C.c_double]
         L.orc_field_step.restype = None
@@ -191,6 +193,13 @@ def corrector(dt, h, x, u, uh, Fh):
     return un.value, xn.value
 
 
+def polarised(a, theta, beta):
+    """(a_sz, a_px, a_py) of P:L81 / Fig. 1(a): components 0 = z, 1 = x, 2 = y of the vector potential."""
+    out = (C.c_double * 3)()
+    lib().orc_polarised(float(a), float(theta), float(beta), out)
+    return [out[0], out[1], out[2]]
+
+
 def a_inc(laser: dict, x, y, t, Ly=1.0):
     L = _Laser(laser["a0"], laser.get("omega", 1.0), laser.get("y0", 0.0), laser.get("w0", 0.0),
                laser.get("t_rise", 0.0), laser.get("alpha", 0.0), laser.get("comp", 0), 0)
@@ -199,16 +208,13 @@ def a_inc(laser: dict, x, y, t, Ly=1.0):
 
 def velocity_histogram(X, Y, u, w, box, umin, umax, nbins):
     """SURVEY 8f.4 (Fig. 9): weighted distribution of one velocity component over the particles whose cell
-    (floor X, floor Y) lies in box = (i0, i1, j0, j1).  The bin is an integer decided by floating point, so it is
-    taken in the kernel's precision (float32: u, umin and the scale nbins/(umax-umin) rounded first, then subtract,
-    multiply, floor); the sums are float64."""
+    (floor X, floor Y) lies in box = (i0, i1, j0, j1): hist[b] = sum of w_p over the particles with
+    b = floor((u_p - umin) nbins / (umax - umin)), 0 <= b < nbins -- the definition, in float64."""
     X, Y, w = np.asarray(X, np.float64), np.asarray(Y, np.float64), np.asarray(w, np.float64)
     i0, i1, j0, j1 = box
     ix, iy = np.floor(X).astype(np.int64), np.floor(Y).astype(np.int64)
     inside = (ix >= i0) & (ix < i1) & (iy >= j0) & (iy < j1)
-    u32 = np.asarray(u).astype(np.float32)
-    scale = np.float32(float(nbins) / (float(umax) - float(umin)))
-    t = np.floor((u32 - np.float32(umin)) * scale)
+    t = np.floor((np.asarray(u, np.float64) - float(umin)) * (float(nbins) / (float(umax) - float(umin))))
     ok = inside & (t >= 0) & (t < nbins)
     h = np.zeros(nbins)
     np.add.at(h, t[ok].astype(np.int64), w[ok])
@@ -368,3 +374,49 @@ class Oracle:
              "W_kin": out[3::2].copy(), "W_th": out[4::2].copy()}
         d["W_total"] = float(out.sum())
         return d
+
+
+# ---- an Oracle from a pm2d_inputs config (tests, smoke, the CPU legs of bench.py) ----------------------------------
+def species_from_arrays(sp_cfg, parts=None, n_fixed=None):
+    d = dict(mass=sp_cfg["mass"], sign=sp_cfg["sign"], T_keV=sp_cfg["T_keV"], C=sp_cfg["pressure_coeff"],
+             shape=sp_cfg["shape"], DD=sp_cfg["DD"], mobile=sp_cfg["mobile"])
+    if parts is not None:
+        d["X"] = parts["ix"].astype(np.float64) + parts["fx"].astype(np.float64)
+        d["Y"] = parts["iy"].astype(np.float64) + parts["fy"].astype(np.float64)
+        d["ux"] = parts["ux"].astype(np.float64)
+        d["uy"] = parts["uy"].astype(np.float64)
+        d["w"] = parts["w"].astype(np.float64)
+    if n_fixed is not None:
+        d["n_fixed"] = n_fixed
+    return d
+
+
+def from_config(cfg, particles=None):
+    """particles: optional list (per species) of dicts as returned by oracle.loader.generate_particles."""
+    from . import loader
+    g = cfg["grid"]
+    grid = make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], g["ncomp"])
+    if particles is None:
+        particles = [loader.generate_particles(cfg, s) if sp["load"] != 0 else None
+                     for s, sp in enumerate(cfg["species"])]
+    species = []
+    # Q13: an immobile species without particles neutralises the summed deposit of the mobile
+    # species of opposite sign at t = 0
+    for s, sp in enumerate(cfg["species"]):
+        if particles[s] is not None:
+            species.append(species_from_arrays(sp, particles[s]))
+        else:
+            species.append(None)
+    for s, sp in enumerate(cfg["species"]):
+        if species[s] is None:
+            nfix = np.zeros((g["nx"] + 1, g["ny"]))
+            for t, sq in enumerate(cfg["species"]):
+                if particles[t] is not None and sq["sign"] == -sp["sign"]:
+                    d = species[t]
+                    n, _, _ = deposit(grid, sq["shape"], sq["DD"], d["X"], d["Y"], d["ux"], d["uy"], d["w"])
+                    nfix += n
+            species[s] = species_from_arrays(sp, None, nfix)
+    lasers = [dict(a0=l["a0"], omega=l["omega"], y0=l["y0"], w0=l["w0"], t_rise=l["t_rise"], comp=l["comp"],
+                   alpha=l.get("alpha", 0.0)) for l in cfg["lasers"]]
+    return Oracle(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], species, lasers, g["ncomp"],
+                         subcycle=g.get("subcycle", 1), bc_y=g.get("bc_y", 0)), particles

@@ -183,6 +183,18 @@ void orc_gather(const orc_grid *g, int shape, double DD, double Xp, double Yp, c
     *fy = sy;
 }
 
+/* A3c (Fig. 1(a)).  "Assuming the direction of vector potential a has an angle of theta with respect to the
+ * z-axis, then the components of a in the S-polarization direction (z direction) is a_sz = a cos(theta), and in the
+ * P-polarization plane (x-y plane) is a_p = a sin(theta). if a_p has a angle of beta with respect to the x direction
+ * ... a_px = a sin(theta) cos(beta) and a_py = a sin(theta) sin(beta)".  out[0] = a_sz, out[1] = a_px, out[2] = a_py;
+ * the components of `a` are numbered 0 = z, 1 = x, 2 = y throughout.  Pin: the three axes of Fig. 1(a) and |a|. */
+void orc_polarised(double a, double theta, double beta, double out[3])
+{
+    out[0] = a * cos(theta);
+    out[1] = a * sin(theta) * cos(beta);
+    out[2] = a * sin(theta) * sin(beta);
+}
+
 /* Incident wave, Eq. 4: a = a0 env(y) cos(omega t - k x), k = omega in vacuum, time in
  * T0 and x in lambda0 so the phase is 2 pi omega (t - x).  Turn-on (Q14): ramp(tau) =
  * sin^2(pi tau / (2 t_rise)) of the retarded time tau = t - x; t_rise = 0 is the paper's literal

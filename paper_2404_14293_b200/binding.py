@@ -19,7 +19,7 @@ MAX_SPECIES, MAX_LASERS, TILE = 4, 4, 32
 CIC, TSC, SINE = 0, 1, 2
 LOAD_NONE, LATTICE_COLD, RANDOM_MAXWELL, NUMBER_WEIGHTED = 0, 1, 2, 3
 PROFILE_UNIFORM, PROFILE_LINEAR, PROFILE_EXP_CAPPED, PROFILE_FILAMENT_Y = 0, 1, 2, 3
-FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE = 0, 1, 2, 3
+FIELD_A, FIELD_PHI, FIELD_ENODE, FIELD_FORCE, FIELD_FORCE_REF = 0, 1, 2, 3, 4
 MOMENT_N, MOMENT_PX, MOMENT_PY = 0, 1, 2
 BC_Y_PERIODIC, BC_Y_ABSORB = 0, 1
 ORDER_AUTO, ORDER_CELL_MAJOR, ORDER_LAYERED, ORDER_RANDOM, ORDER_LANES, LAYERS = 0, 1, 2, 3, 4, 16
@@ -67,10 +67,12 @@ SYMBOLS = {
     "pm2d_step": (C.c_int, [_vp, C.c_int]),
     "pm2d_step_async": (C.c_int, [_vp, C.c_int]),
     "pm2d_set_lasers": (C.c_int, [_vp, C.POINTER(Laser), C.c_int]),
+    "pm2d_polarised_beam": (C.c_int, [C.POINTER(Laser), C.c_double, C.c_double, C.POINTER(Laser)]),
     "pm2d_get_fields": (C.c_int64, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _fp, C.c_size_t]),
     "pm2d_get_moments": (C.c_int64, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _fp, C.c_size_t]),
     "pm2d_set_fields": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, _fp]),
     "pm2d_get_particles": (C.c_int64, [_vp, C.c_int, C.c_int64, C.c_int64, _ip, _ip, _fp, _fp, _fp, _fp, _fp, _lp]),
+    "pm2d_get_predictor": (C.c_int64, [_vp, C.c_int, C.c_int64, C.c_int64, _fp, _fp]),
     "pm2d_set_particles": (C.c_int, [_vp, C.c_int, C.c_int64, _ip, _ip, _fp, _fp, _fp, _fp, _fp, C.c_int]),
     "pm2d_set_background": (C.c_int, [_vp, C.c_int, _fp]),
     "pm2d_rebin": (C.c_int, [_vp, C.c_int, _ip, _lp]),
@@ -128,14 +130,13 @@ def _ptr(a, ctype):
 
 
 def polarised_beam(a0, theta, beta, **laser):
-    """Laser-table entries of one beam of arbitrary polarisation (Fig. 1(a)): the vector potential makes the
-    angle theta with the z axis, its part in the x-y plane the angle beta with the x axis.  Components of `a` are
-    numbered 0 = z (S polarisation, the one BASELINE.json's configs use), 1 = x, 2 = y:
-        a_sz = a0 cos(theta),  a_px = a0 sin(theta) cos(beta),  a_py = a0 sin(theta) sin(beta).
-    Every component obeys the same wave equation (Eq. 1), so the beam is three entries that differ in `a0` and
-    `comp`; entries of zero amplitude are left out.  The grid needs ncomp = 3 unless theta = 0."""
-    amps = (a0 * math.cos(theta), a0 * math.sin(theta) * math.cos(beta), a0 * math.sin(theta) * math.sin(beta))
-    return [dict(laser, a0=float(a), comp=c) for c, a in enumerate(amps) if abs(a) > 1e-300 * abs(a0)]
+    """Laser-table entries of one beam of arbitrary polarisation (Fig. 1(a)): pm2d_polarised_beam does the
+    decomposition; this wrapper only marshals the beam in and the up to three entries out."""
+    proto = Laser(float(a0), float(laser.get("omega", 1.0)), float(laser.get("y0", 0.0)), float(laser.get("w0", 0.0)),
+                  float(laser.get("t_rise", 0.0)), float(laser.get("alpha", 0.0)), 0, 0)
+    out = (Laser * 3)()
+    n = _check(load_library().pm2d_polarised_beam(C.byref(proto), float(theta), float(beta), out))
+    return [dict(laser, a0=out[k].a0, comp=out[k].comp) for k in range(n)]
 
 
 def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, particle_order=0):
@@ -251,6 +252,13 @@ class PM2D:
             out["id"] = ids
         return out
 
+    def get_predictor(self, species, first=0, count=None):
+        n = self.particle_count(species) - first if count is None else count
+        uhx, uhy = np.empty(n, np.float32), np.empty(n, np.float32)
+        got = _check(self.lib.pm2d_get_predictor(self.ctx, species, first, n, _ptr(uhx, C.c_float), _ptr(uhy, C.c_float)))
+        assert got == n
+        return uhx, uhy
+
     def set_particles(self, species, parts, refix_background=True):
         ix, iy = _np(parts["ix"], np.int32), _np(parts["iy"], np.int32)
         f = {k: _np(parts[k], np.float32) for k in ("fx", "fy", "ux", "uy", "w")}
@@ -323,6 +331,9 @@ class PM2D:
 
     def stray_count(self):
         return int(_check(self.lib.pm2d_stray_count(self.ctx)))
+
+    def version(self):
+        return self.lib.pm2d_version().decode()
 
     def lane_subs(self, s):
         return int(_check(self.lib.pm2d_lane_subs(self.ctx, int(s))))

@@ -1,6 +1,7 @@
 """Build libpm2d.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -21,6 +22,14 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def build_id() -> str:
+    """Hash of the sources the library is built from: pm2d_version() carries it, profiles/ tag their numbers with it."""
+    h = hashlib.sha1()
+    for f in sorted(os.listdir(CSRC)) + [os.path.join("..", "..", "include", "pm2d.h")]:
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    return h.hexdigest()[:10]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
@@ -31,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for src in SOURCES:
         obj = os.path.join(HERE, "build", src.replace(".cu", ".o"))
-        cmd = [nvcc, *flags, "-c", os.path.join(CSRC, src), "-o", obj] + (["-Xptxas", "-v"] if verbose else [])
+        cmd = [nvcc, *flags, f'-DPM2D_BUILD_ID="{build_id()}"', "-c", os.path.join(CSRC, src), "-o", obj] + (["-Xptxas", "-v"] if verbose else [])
         procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(obj)
     for cmd, p in procs:

@@ -12,7 +12,10 @@
 static thread_local std::string g_err;
 void pm2d_set_error(const std::string &s) { g_err = s; }
 extern "C" const char *pm2d_last_error(void) { return g_err.c_str(); }
-extern "C" const char *pm2d_version(void) { return "pm2d-b200 0.1 (sm_100a)"; }
+#ifndef PM2D_BUILD_ID
+#define PM2D_BUILD_ID "unknown"
+#endif
+extern "C" const char *pm2d_version(void) { return "pm2d-b200 0.2 (sm_100a, build " PM2D_BUILD_ID ")"; }
 
 static int fail(int code, const std::string &msg)
 {
@@ -356,6 +359,7 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     c->zstream = nullptr;
     for (int k = 0; k < 2; k++) c->ev_free[k] = c->ev_zero[k] = nullptr;
     c->step = 0;
+    c->uh_valid = false;
     c->cap_extra = 0;
     c->prof_on = false;
     c->cur_phase = -1;
@@ -465,6 +469,22 @@ static void destroy_ctx(pm2d_ctx *c)
 
 extern "C" void pm2d_free(pm2d_ctx *c) { destroy_ctx(c); }
 
+// P:L81, Fig. 1(a): a_sz = a cos(theta), a_px = a sin(theta) cos(beta), a_py = a sin(theta) sin(beta); components 0 = z, 1 = x, 2 = y
+extern "C" int pm2d_polarised_beam(const pm2d_laser *proto, double theta, double beta, pm2d_laser out[3])
+{
+    if (!proto || !out) return fail(PM2D_EINVAL, "null argument");
+    const double amp[3] = {proto->a0 * std::cos(theta), proto->a0 * std::sin(theta) * std::cos(beta), proto->a0 * std::sin(theta) * std::sin(beta)};
+    int n = 0;
+    for (int comp = 0; comp < 3; comp++) {
+        if (std::fabs(amp[comp]) <= 1e-300 * std::fabs(proto->a0)) continue;
+        out[n] = *proto;
+        out[n].a0 = amp[comp];
+        out[n].comp = comp;
+        n++;
+    }
+    return n;
+}
+
 extern "C" int pm2d_set_lasers(pm2d_ctx *c, const pm2d_laser *lasers, int nlaser)
 {
     if (!c || nlaser < 0 || nlaser > PM2D_MAX_LASERS || (nlaser > 0 && !lasers)) return fail(PM2D_EINVAL, "bad laser table");
@@ -525,8 +545,10 @@ static int enqueue_step(pm2d_ctx *c)
     c->a[1] = c->a[0];
     c->a[0] = t;
     c->step++;
+    c->uh_valid = true;
     if (c->prof_on) c->prof_steps++;
     if (c->g.rebin_every > 0 && c->step % c->g.rebin_every == 0) {
+        c->uh_valid = false;             // the rebin uses u^ as scratch
         phase_begin(c, PM2D_PH_REBIN);
         for (int s = 0; s < c->nsp; s++)
             if (c->sp[s].cfg.mobile && !c->sp[s].random && (rc = launch_rebin(c, s, nullptr, nullptr, nullptr))) return rc;
@@ -636,8 +658,15 @@ extern "C" int64_t pm2d_get_fields(pm2d_ctx *c, int field, int comp, int level, 
         return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
     case PM2D_FIELD_FORCE:
         if (comp < 0 || comp > 1 || level < 0 || level >= c->nsp || !c->sp[level].cfg.mobile) return fail(PM2D_EINVAL, "bad comp/species");
-        // Eq. 16 for the current state: E of the current densities, a^n, n^n (diagnostic grid;
-        // the step itself builds the force per tile inside the fused particle kernel)
+        // Eq. 16 for the current state (E of the current densities, a^n, n^n) by the PRODUCTION route: the Poisson solve
+        // whose inverse transform evaluates the force of every mobile species in its epilogue, exactly the launches of a step
+        if ((rc = launch_poisson(c, false, c->a[1], false))) return rc;
+        k_extract_comp<<<blocks, 256, 0, c->stream>>>(c->sp[level].F, comp, c->phi, (size_t)c->nn);
+        count_launch(c);
+        return copy_window(c, c->phi, i0, i1, j0, j1, host, cap);
+    case PM2D_FIELD_FORCE_REF:
+        if (comp < 0 || comp > 1 || level < 0 || level >= c->nsp || !c->sp[level].cfg.mobile) return fail(PM2D_EINVAL, "bad comp/species");
+        // the same force by the stand-alone kernel k_force on the nodal E grid: a cross-check of the fused epilogue
         if ((rc = launch_poisson(c, false))) return rc;
         if ((rc = launch_force(c, level, c->a[1]))) return rc;
         k_extract_comp<<<blocks, 256, 0, c->stream>>>(c->sp[level].F, comp, c->phi, (size_t)c->nn);
@@ -697,6 +726,7 @@ extern "C" int64_t pm2d_get_particles(pm2d_ctx *c, int s, int64_t first, int64_t
     if (id && !S.id) return fail(PM2D_EINVAL, "ids need track_ids");
     // canonical cell + offset and velocity of every particle as separate arrays in the (idle) rebin and
     // predictor buffers: pv2 holds 4 arrays of cap words, uh holds 2
+    c->uh_valid = false;                 // u^ is scratch of the unpacking below
     const size_t capw = (size_t)std::max<int64_t>(S.cap, 1);
     int32_t *dix = (int32_t *)S.pv2, *diy = dix + capw;
     float *dfx = (float *)(diy + capw), *dfy = dfx + capw;
@@ -716,6 +746,21 @@ extern "C" int64_t pm2d_get_particles(pm2d_ctx *c, int s, int64_t first, int64_t
     PM2D_CUDA_CHECK(d2h(w, S.w, 4));
     PM2D_CUDA_CHECK(d2h(id, S.id, 8));
     PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    return count;
+}
+
+extern "C" int64_t pm2d_get_predictor(pm2d_ctx *c, int s, int64_t first, int64_t count, float *uhx, float *uhy)
+{
+    if (!c || s < 0 || s >= c->nsp || !c->sp[s].cfg.mobile || !uhx || !uhy) return fail(PM2D_EINVAL, "bad argument");
+    SpeciesDev &S = c->sp[s];
+    if (!c->uh_valid) return fail(PM2D_ESTATE, "the predictor velocities of the last step are gone (rebin, pm2d_get_particles or no step yet)");
+    if (first < 0 || count < 0 || first > S.np) return fail(PM2D_EINVAL, "bad range");
+    count = std::min(count, S.np - first);
+    if (count == 0) return 0;
+    std::vector<float2> h((size_t)count);
+    PM2D_CUDA_CHECK(cudaMemcpyAsync(h.data(), S.uh + first, (size_t)count * sizeof(float2), cudaMemcpyDeviceToHost, c->stream));
+    PM2D_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+    for (int64_t p = 0; p < count; p++) { uhx[p] = h[(size_t)p].x; uhy[p] = h[(size_t)p].y; }
     return count;
 }
 
@@ -794,6 +839,7 @@ extern "C" int pm2d_set_particles(pm2d_ctx *c, int s, int64_t count, const int32
     PM2D_CUDA_CHECK(h2d(S.tile_off, off.data(), (size_t)(ntiles + 1) * 8));
     PM2D_CUDA_CHECK(h2d(S.cell_off, coff.data(), coff.size() * 4));
     S.np = count;
+    c->uh_valid = false;
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
     if (S.lanes && (rc = launch_lanesort(c, s, true, nullptr, nullptr, nullptr))) return rc;
@@ -813,6 +859,7 @@ extern "C" int pm2d_rebin(pm2d_ctx *c, int s, int32_t *keys_out, int64_t *perm_o
     if (keys_out) PM2D_CUDA_CHECK(cudaMalloc(&dk, n * sizeof(int32_t)));
     if (perm_out) PM2D_CUDA_CHECK(cudaMalloc(&dp, n * sizeof(int64_t)));
     if (keys_out || perm_out) PM2D_CUDA_CHECK(cudaMalloc(&dt, n * sizeof(int64_t)));
+    c->uh_valid = false;
     int rc = launch_rebin(c, s, dk, dp, dt);
     if (!rc && keys_out) rc = cudaMemcpyAsync(keys_out, dk, (size_t)S.np * 4, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;
     if (!rc && perm_out) rc = cudaMemcpyAsync(perm_out, dp, (size_t)S.np * 8, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess ? 0 : PM2D_ECUDA;

@@ -84,6 +84,7 @@ struct pm2d_ctx {
     cudaStream_t zstream;            // side stream: zeroes the idle deposit set while a stage kernel runs
     cudaEvent_t ev_free[2], ev_zero[2];   // [0] main set (n^n, stage B target), [1] hat set (stage A target)
     int64_t step;        // particle steps taken
+    bool uh_valid;       // the u^ arrays still hold the predictor velocities of the last step (pm2d_get_predictor)
     int nsub;            // wave-equation steps per particle step (Q21)
     double dtp;          // particle time step = nsub * g.dt
     int64_t nn;          // nodes

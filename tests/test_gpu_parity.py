@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
+import oracle.loader as L
 import pm2d_inputs as I
 from helpers import oracle_from_config
 
@@ -49,9 +50,9 @@ def test_device_loader_equals_numpy_generator(P, name, nx, ny):
     for s, sp in enumerate(cfg["species"]):
         if sp["load"] == I.LOAD_NONE:
             continue
-        ref = I.generate_particles(cfg, s)
+        ref = L.generate_particles(cfg, s)
         got = sim.get_particles(s, with_id=True)
-        assert got["id"].size == ref["id"].size == I.n_particles(cfg, s)
+        assert got["id"].size == ref["id"].size == L.n_particles(cfg, s)
         order = np.argsort(got["id"])
         assert np.array_equal(got["id"][order], ref["id"])            # ref is in id order
         for k in ("ix", "iy", "fx", "fy"):
@@ -84,7 +85,7 @@ def test_initial_deposit_parity(P, name, nx, ny):
     vol = np.ones((nx + 1, 1)); vol[0] = vol[-1] = 0.5
     for s in range(len(cfg["species"])):
         assert d["charge"][s] == pytest.approx((orc.moment(s, "n") * vol).sum(), rel=1e-6)
-        assert d["count"][s] == I.n_particles(cfg, s)
+        assert d["count"][s] == L.n_particles(cfg, s)
     sim.close()
 
 
@@ -206,7 +207,7 @@ def test_random_order_storage(P):
     rebin and host-supplied particles are refused."""
     cfg = small_cfg("c5", 64, 64)
     sim = P.PM2D(cfg, track_ids=1, particle_order=P.ORDER_RANDOM)
-    ref = I.generate_particles(cfg, 0)
+    ref = L.generate_particles(cfg, 0)
     got = sim.get_particles(0, with_id=True)
     order = np.argsort(got["id"])
     assert np.array_equal(got["id"][order], ref["id"])
@@ -481,7 +482,7 @@ def test_full_size_c2_deposit_parity_and_conservation(P):
     q0 = sim.diagnostics()["charge"][0]
     sim.step(3)
     parts = sim.get_particles(0)
-    assert parts["ix"].size == n0 == I.n_particles(cfg, 0)
+    assert parts["ix"].size == n0 == L.n_particles(cfg, 0)
     grid = oracle.make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"])
     sp = cfg["species"][0]
     n, px, py = oracle.deposit(grid, sp["shape"], sp["DD"], parts["ix"] + parts["fx"].astype(np.float64),
@@ -506,7 +507,7 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     sim.step(17)
     d1 = sim.diagnostics()
     for s in (0, 1):
-        assert d1["count"][s] == d0["count"][s] == I.n_particles(cfg, s)
+        assert d1["count"][s] == d0["count"][s] == L.n_particles(cfg, s)
         assert d1["charge"][s] == pytest.approx(d0["charge"][s], rel=1e-6)
     assert np.isfinite(d1["W_total"]) and d1["W_kin"][0] > 0
     a = sim.get_fields(P.FIELD_A, 0, 0, window=(0, 64, 0, 64))
@@ -514,9 +515,118 @@ def test_full_size_c3_conservation_across_a_rebin(P):
     sim.close()
 
 
-@pytest.mark.parametrize("name", ["c4", "c5", "cbet"])
+def _oracle_force_from_device_state(P, sim, cfg):
+    """Eq. 16 of the oracle (orc_poisson + orc_efield + orc_force) fed the device's own densities and a^n: the species
+    enter as fixed density grids, so no particle is stepped on the CPU.  -> {species: (Fx, Fy)}"""
+    g = cfg["grid"]
+    sp = []
+    for s, q in enumerate(cfg["species"]):
+        n = sim.get_moments(s, P.MOMENT_N).astype(np.float64)
+        sp.append(dict(sign=q["sign"], mass=q["mass"], T_keV=q["T_keV"], C=q["pressure_coeff"], shape=q["shape"], DD=q["DD"],
+                       mobile=0, n_fixed=n))
+    orc = oracle.Oracle(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], sp, [], g["ncomp"])
+    for c in range(g["ncomp"]):
+        orc.a_now[c][:] = sim.get_fields(P.FIELD_A, c, 0)
+    return {s: orc.force_now(s) for s, q in enumerate(cfg["species"]) if q["mobile"]}
+
+
+def _force_errors(P, sim, s, ref):
+    rx, ry = ref
+    fx, fy = sim.get_fields(P.FIELD_FORCE, 0, s), sim.get_fields(P.FIELD_FORCE, 1, s)
+    err, mag = np.hypot(fx - rx, fy - ry), np.hypot(rx, ry)
+    return np.sqrt((err ** 2).sum() / (mag ** 2).sum()), err[[0, -1]].max() / mag.max(), err.max() / mag.max()
+
+
+@pytest.mark.parametrize("nx,ny", [(72, 1024), (72, 2048), (72, 4096), (40, 8192)])
+def test_production_force_grid_parity(P, nx, ny):
+    """The nodal force the stage kernels gather from -- written by the epilogue of the inverse transform k_ifft<2>, in its
+    ny-specialised vector variants (1024, 2048, 4096, 8192) -- element by element against Eq. 16 of the oracle after one
+    step of the reduced c3 config (both on their own particles), and against the stand-alone k_force."""
+    cfg = small_cfg("c3", nx, ny)
+    sim = P.PM2D(cfg, eager_moments=1)
+    orc, _ = oracle_from_config(cfg)
+    sim.step(1)
+    orc.step(1)
+    for s in (0, 1):
+        l2, wall, mx = _force_errors(P, sim, s, orc.force_now(s))
+        assert l2 < 2e-4 and wall < 1e-3 and mx < 2e-3, (s, l2, wall, mx)
+        for comp in (0, 1):
+            a, b = sim.get_fields(P.FIELD_FORCE, comp, s), sim.get_fields(P.FIELD_FORCE_REF, comp, s)
+            assert np.abs(a - b).max() < 2e-5 * np.abs(b).max(), (s, comp)
+    sim.close()
+
+
+def _enough_host_memory(gb):
+    try:
+        import psutil
+        return psutil.virtual_memory().available > gb * 2 ** 30
+    except Exception:
+        return True
+
+
+def test_full_size_c3_force_and_predictor_parity(P):
+    """BASELINE.json config 3 at full size (8192 x 4096), in the launch configuration bench.py times.
+    (1) The production force grid of both species (k_ifft<2, ..., 4096> epilogue after the 256-partition tridiagonal
+    solve) against Eq. 16 of the oracle fed the device's own densities and a^n: all 33.6 M nodes.
+    (2) The gather and the predictor (Eq. 15, Eq. 17) of the next step: the u^ the stage-A kernels leave for the
+    particles of a wall tile, a y-wrap tile and interior tiles (bulk-async windows), electrons and ions, against
+    u + dt * orc_gather(oracle force grid) of the same particles."""
+    if not _enough_host_memory(24):
+        pytest.skip("needs about 20 GB of host memory for the oracle's grids")
+    cfg = I.config("c3")
+    g = cfg["grid"]
+    nx, ny, T = g["nx"], g["ny"], P.TILE
+    sim = P.PM2D(cfg, eager_moments=1)
+    sim.step(2)
+    ref = _oracle_force_from_device_state(P, sim, cfg)
+    for s in (0, 1):
+        l2, wall, mx = _force_errors(P, sim, s, ref[s])
+        assert l2 < 2e-4 and wall < 1e-3, (s, l2, wall, mx)
+    grid = oracle.make_grid(nx, ny, g["dx"], g["dy"], g["dt"])
+    ranges = {}
+    for s, sp in enumerate(cfg["species"]):
+        ppc = sp["ppc_x"] * sp["ppc_y"]
+        x0 = (nx // T // 2) * T
+        ranges[s] = [(0, 2 * T * T * ppc), (x0 * ny * ppc, 3 * T * T * ppc)]       # tiles (0, 0..1) and (x0/T, 0..2), loader order
+    before = {s: [sim.get_particles(s, first=f, count=c) for f, c in ranges[s]] for s in ranges}
+    sim.step(1)                                               # step 3: no rebin, the storage order stands
+    for s, sp in enumerate(cfg["species"]):
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        Fx, Fy = ref[s]
+        for (f, c), pp in zip(ranges[s], before[s]):
+            uhx, uhy = sim.get_predictor(s, first=f, count=c)
+            sel = np.arange(0, c, 7)                          # every 7th particle: 1170 to 1755 gathers per range
+            worst = 0.0
+            for p in sel:
+                fx, fy = oracle.gather(grid, sp["shape"], sp["DD"], float(pp["ix"][p]) + float(pp["fx"][p]),
+                                       float(pp["iy"][p]) + float(pp["fy"][p]), Fx, Fy)
+                ex = abs(float(uhx[p]) - (float(pp["ux"][p]) + g["dt"] * fx)) / max(abs(float(pp["ux"][p])), vth)
+                ey = abs(float(uhy[p]) - (float(pp["uy"][p]) + g["dt"] * fy)) / max(abs(float(pp["uy"][p])), vth)
+                worst = max(worst, ex, ey)
+            assert worst < 1e-5, (s, f, worst)
+    sim.close()
+
+
+def test_full_size_c4_force_parity(P):
+    """BASELINE.json config 4 at full size (16384 x 8192: the ny = 8192 transforms, 512 x-partitions and the fallback
+    k_tri_reduced of the tridiagonal solve): the production force grids against Eq. 16 of the oracle fed the device's
+    own densities and a^n, all 134 M nodes."""
+    if not _enough_host_memory(80):
+        pytest.skip("needs about 70 GB of host memory for the oracle's grids")
+    cfg = I.config("c4")
+    sim = P.PM2D(cfg, eager_moments=1)
+    sim.step(2)
+    ref = _oracle_force_from_device_state(P, sim, cfg)
+    for s in (0, 1):
+        l2, wall, mx = _force_errors(P, sim, s, ref[s])
+        assert l2 < 2e-4 and wall < 1e-3, (s, l2, wall, mx)
+    sim.close()
+
+
+@pytest.mark.parametrize("name", ["c3", "c4", "c5", "cbet"])
 def test_full_size_c4_c5_sampled_deposit_parity(P, name):
-    """(cbet: the second workload of bench.py, 8192 x 8192, particle step = 5 wave steps, same checks.)
+    """(cbet: the second workload of bench.py, 8192 x 8192, particle step = 5 wave steps, same checks; c3: the headline
+    workload.)
     BASELINE.json configs 4 (16384 x 8192, 403 M particles, Gaussian beam, ny = 8192 FFT path) and 5 (4096 x 4096,
     9.4e8 number-weighted electrons in a filament, cell-major order + strip kernel) at full size, in the launch
     configuration bench.py times.  After 3 steps: counts and charge conserved, and on a sample of the grid -- 17 node
@@ -534,14 +644,14 @@ def test_full_size_c4_c5_sampled_deposit_parity(P, name):
     d1 = sim.diagnostics()
     mobile = [s for s, sp in enumerate(cfg["species"]) if sp["mobile"]]
     for s in mobile:
-        assert d1["count"][s] == d0["count"][s] == I.n_particles(cfg, s)
+        assert d1["count"][s] == d0["count"][s] == L.n_particles(cfg, s)
         assert d1["charge"][s] == pytest.approx(d0["charge"][s], rel=1e-6)
     x0 = (nx // T // 2) * T                                        # first cell row of the two tile rows taken
     sub = oracle.make_grid(4 * T, ny, g["dx"], g["dy"], g["dt"])   # cells x0 - T .. x0 + 3 T: no wall near the sample
     for s in mobile:
         sp = cfg["species"][s]
         if sp["load"] == I.NUMBER_WEIGHTED:
-            cc = I.cell_counts(cfg, s)
+            cc = L.cell_counts(cfg, s)
             first, count = int(cc[:x0].sum()), int(cc[x0:x0 + 2 * T].sum())
         else:
             ppc = sp["ppc_x"] * sp["ppc_y"]
@@ -574,7 +684,7 @@ def test_full_length_c2_run_stays_bounded(P):
     vth = math.sqrt(cfg["species"][0]["T_keV"] / 511.0)
     well = math.sqrt(2.0 * 2.0 * vth ** 2 * math.log(1.0 / I.TAPER_FLOOR))        # u^2/2 = C v_th^2 ln(n_bulk / n_edge)
     assert u.max() < well + 6.0 * vth, (float(u.max()), well, vth)
-    assert d1["count"][0] == d0["count"][0] == I.n_particles(cfg, 0)
+    assert d1["count"][0] == d0["count"][0] == L.n_particles(cfg, 0)
     assert d1["charge"][0] == pytest.approx(d0["charge"][0], rel=1e-6)
     assert all(np.isfinite(d1[k]) for k in ("W_es", "W_em", "W_int", "W_total"))
     assert d1["W_kin"][0] == pytest.approx(d0["W_kin"][0], rel=0.03)
@@ -744,10 +854,22 @@ def test_mode_amplitudes_parity(P):
 @pytest.mark.gpu
 @pytest.mark.parametrize("order", [0, 3], ids=["auto", "random"])
 def test_velocity_histogram_parity(P, order):
-    """8f.4: pm2d_velocity_histogram against the oracle's definition.  (1) On the device's own particles (canonical
-    form read back) every bin decision is the same float32 expression: sums agree to rounding.  (2) Against the
-    oracle's particles after 5 steps of the reduced c3 config: velocities differ by ~1e-7 relative, so only
-    particles within that distance of an edge may change bins."""
+    """8f.4: pm2d_velocity_histogram.  (1) The kernel's own statement of its bin (include/pm2d.h: u, umin and the
+    scale rounded to float32, then subtract, multiply, floor) replayed here on the device's own particles: the sums
+    agree to rounding.  (2) Against the oracle's float64 definition on the oracle's particles after 5 steps of the
+    reduced c3 config: velocities differ by ~1e-7 relative and the float32 bin edges by as much, so only particles
+    within that distance of an edge may change bins (at most 2e-3 of the weight)."""
+    def replay_f32(X, Y, u, w, box, umin, umax, nbins):
+        i0, i1, j0, j1 = box
+        ix, iy = np.floor(X).astype(np.int64), np.floor(Y).astype(np.int64)
+        inside = (ix >= i0) & (ix < i1) & (iy >= j0) & (iy < j1)
+        scale = np.float32(float(nbins) / (float(umax) - float(umin)))
+        b = np.floor((np.asarray(u).astype(np.float32) - np.float32(umin)) * scale)
+        ok = inside & (b >= 0) & (b < nbins)
+        h = np.zeros(nbins)
+        np.add.at(h, b[ok].astype(np.int64), np.asarray(w, np.float64)[ok])
+        return h
+
     cfg = small_cfg("c3", 72, 64)
     sim = P.PM2D(cfg, eager_moments=1, track_ids=1, rebin_every=2, particle_order=order)
     orc, _ = oracle_from_config(cfg)
@@ -758,8 +880,8 @@ def test_velocity_histogram_parity(P, order):
         for comp, key in ((0, "ux"), (1, "uy")):
             h = sim.velocity_histogram(s, box, comp, lo, hi, nb)
             got = sim.get_particles(s)
-            own = oracle.velocity_histogram(got["ix"] + got["fx"].astype(np.float64), got["iy"] + got["fy"].astype(np.float64),
-                                            got[key], got["w"], box, lo, hi, nb)
+            own = replay_f32(got["ix"] + got["fx"].astype(np.float64), got["iy"] + got["fy"].astype(np.float64),
+                             got[key], got["w"], box, lo, hi, nb)
             assert np.abs(h - own).max() <= 1e-12 * max(own.max(), 1e-30), (s, comp)
             assert own.sum() > 0
             d = orc.sp[s]
@@ -947,7 +1069,8 @@ def test_probe_arguments(P):
 def test_polarised_beam_three_components_parity(P):
     """A3c: a Gaussian beam of arbitrary polarisation (theta = 35 degrees from z, beta = 60 degrees from x) at
     10 degrees of incidence through the c3 slab (reduced, mobile ions): the three components, built by
-    polarised_beam, stay with the oracle driven by the amplitudes written out here, and keep their ratio."""
+    pm2d_polarised_beam, stay with the oracle driven by the amplitudes of its own orc_polarised (pinned on the three
+    axes of Fig. 1(a) in tests/test_oracle_loader.py), and keep their ratio."""
     th, be, a0 = math.radians(35.0), math.radians(60.0), 0.02
     cfg = small_cfg("c3", 72, 64, ncomp=3)
     Ly = 64 * cfg["grid"]["dy"]
@@ -955,8 +1078,7 @@ def test_polarised_beam_three_components_parity(P):
     cfg["lasers"] = P.polarised_beam(a0, th, be, **beam)
     sim = P.PM2D(cfg, eager_moments=1)
     ref = copy.deepcopy(cfg)
-    ref["lasers"] = [dict(beam, a0=a0 * math.cos(th), comp=0), dict(beam, a0=a0 * math.sin(th) * math.cos(be), comp=1),
-                     dict(beam, a0=a0 * math.sin(th) * math.sin(be), comp=2)]
+    ref["lasers"] = [dict(beam, a0=amp, comp=comp) for comp, amp in enumerate(oracle.polarised(a0, th, be))]
     orc, _ = oracle_from_config(ref)
     sim.step(120)
     orc.step(120)
@@ -980,7 +1102,7 @@ def test_y_taper_loader_and_run_parity(P):
     cfg["profile"]["taper_cells_y"] = 9
     sim = P.PM2D(cfg, eager_moments=1, track_ids=1)
     for s in (0, 1):
-        ref = I.generate_particles(cfg, s)
+        ref = L.generate_particles(cfg, s)
         got = sim.get_particles(s, with_id=True)
         o = np.argsort(got["id"])
         assert np.array_equal(got["id"][o], ref["id"])

@@ -229,7 +229,7 @@ def test_P17_mode_amplitudes_closed_form_and_fft():
 def test_P18_velocity_histogram_of_a_maxwellian_and_a_box():
     """The histogram of 4e5 seeded normal velocities follows the Gaussian bin integrals within counting noise; the
     box selects by cell; the total weight inside [umin, umax) is conserved; numpy's histogram agrees where no value
-    sits on a float32 bin edge."""
+    sits on a bin edge."""
     rng = np.random.default_rng(3)
     N, vth = 400000, 0.05
     X, Y = rng.random(N) * 40, rng.random(N) * 16

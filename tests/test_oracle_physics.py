@@ -24,7 +24,7 @@ def _lattice(nx, ny, px, py):
     return X, Y
 
 
-def _run_mode(nx, ny, dx, dt, n0, px, shape, DD, sign, T_keV, C, m, nsteps, eps=0.02):
+def _run_mode(nx, ny, dx, dt, n0, px, shape, DD, sign, T_keV, C, m, nsteps, eps=0.02, mass=1.0):
     """Lattice-loaded species with displacement eps*sin(K x); returns t, cos-mode amplitude of n."""
     g = oracle.make_grid(nx, ny, dx, dx, dt)
     X0, Y0 = _lattice(nx, ny, px, 1)
@@ -32,7 +32,7 @@ def _run_mode(nx, ny, dx, dt, n0, px, shape, DD, sign, T_keV, C, m, nsteps, eps=
     n_bg, _, _ = oracle.deposit(g, shape, DD, X0, Y0, 0 * X0, 0 * X0, w)
     K = 2 * math.pi * m / nx                 # per cell
     X = X0 + eps * np.sin(K * X0)
-    sp = [dict(sign=sign, mass=1.0, T_keV=T_keV, C=C, shape=shape, DD=DD, mobile=1,
+    sp = [dict(sign=sign, mass=mass, T_keV=T_keV, C=C, shape=shape, DD=DD, mobile=1,
                X=X, Y=Y0, ux=0 * X, uy=0 * X, w=w)]
     if sign != 0:
         sp.append(dict(sign=-sign, mass=1836.0, T_keV=0.0, mobile=0, shape=shape, DD=DD, n_fixed=n_bg))
@@ -229,3 +229,61 @@ def test_P14_srs_backscatter_growth_rate():
     k = math.sqrt(1.0 - n0) + math.sqrt((1.0 - wek) ** 2 - n0)
     gamma = 2.0 * math.pi * (k * a0 / 4.0) * math.sqrt(n0 / (wek * (1.0 - wek)))
     assert rate == pytest.approx(gamma, rel=0.30), (rate, gamma)
+
+
+# ---- mobile species of mass != 1 (the ion branch of Eq. 16: F_i = -4 pi^2 (m_e/m_i) E - 2 v_ith^2 grad(n_i)/n_i,
+# v_ith = sqrt(T_i / 511 / m_i)).  BASELINE.json's configs 3, 4 and the CBET set-up push ions.
+def test_P21_ion_plasma_oscillation_scales_with_the_mass():
+    """A cold lattice of positive particles of mass m = 16 against a fixed negative background oscillates at the ion
+    plasma frequency W = 2 pi sqrt(n0 / m): period sqrt(m / n0) T0, four times that of the electrons.  Fails when the
+    1/mass of the E force in orc_force is dropped (period 3.16 instead of 12.65 T0) or applied twice."""
+    n0, dt, m = 0.1, 0.035, 16.0
+    t, amp, _ = _run_mode(64, 4, 0.05, dt, n0, 8, oracle.SINE, 1.9, +1, 0.0, 0.0, 1, 1500, mass=m)
+    period = _period_from_zero_crossings(t, amp)
+    assert period == pytest.approx(math.sqrt(m / n0), rel=0.02)
+    assert np.abs(amp).max() < 1.5 * abs(amp[0])
+
+
+def test_P21_sound_wave_of_a_heavy_neutral_species():
+    """P12c with mass 16: the pressure force alone, w = sqrt(C) K v_th with v_th = sqrt(T / 511 / m).  Fails
+    when the thermal velocity ignores the mass (oracle/__init__.py: vth2 = T / 511 / mass): period 4 times too short."""
+    T, C, m, nx, dx, dt, mass = 40.0, 2.0, 2, 64, 0.05, 0.035, 16.0
+    vth = math.sqrt(T / 511.0 / mass)
+    Kphys = 2 * math.pi * m / (nx * dx)
+    period_expected = 2 * math.pi / (math.sqrt(C) * Kphys * vth)
+    nsteps = int(4.2 * period_expected / dt)
+    t, amp, _ = _run_mode(nx, 4, dx, dt, 0.1, 8, oracle.SINE, 1.9, 0, T, C, m, nsteps, eps=0.02, mass=mass)
+    period = _period_from_zero_crossings(t, amp)
+    assert period == pytest.approx(period_expected, rel=0.02)
+
+
+def test_P22_ponderomotive_force_coefficient():
+    """The second term of Eq. 16, -1/2 grad(a_x^2 + a_y^2 + a_z^2) (Eq. 2), alone: no density, so
+    no E and no pressure term (Q10).  a_z = c x, a_x = d x gives a^2 = (c^2 + d^2) x^2, whose central difference is exact:
+    F_x = -(c^2 + d^2) x_i at the interior nodes, the one-sided value -(1/2)(c^2 + d^2) dx (2 i -+ 1) dx at the walls,
+    F_y = 0; the ions feel none of it ("the ponderomotive force ... on ions is neglected").  A coefficient 1
+    instead of 1/2, a single component instead of the sum, or the term applied to the ions fail."""
+    nx, ny, dx = 24, 8, 0.05
+    sp = [dict(sign=-1, mass=1.0, T_keV=3.0, C=2.0, shape=oracle.SINE, DD=1.9, mobile=1, X=np.zeros(0), Y=np.zeros(0),
+               ux=np.zeros(0), uy=np.zeros(0), w=np.zeros(0)),
+          dict(sign=+1, mass=3672.0, T_keV=1.0, C=2.0, shape=oracle.SINE, DD=1.9, mobile=1, X=np.zeros(0), Y=np.zeros(0),
+               ux=np.zeros(0), uy=np.zeros(0), w=np.zeros(0))]
+    o = oracle.Oracle(nx, ny, dx, dx, 0.035, sp, [], 3)
+    c, d = 0.7, -0.4
+    x = np.arange(nx + 1)[:, None] * dx * np.ones((1, ny))
+    o.a_now[0][:] = c * x
+    o.a_now[1][:] = d * x
+    fx, fy = o.force_now(0)
+    k2 = c * c + d * d
+    assert np.abs(fx[1:nx] + k2 * x[1:nx]).max() < 1e-13
+    assert np.abs(fx[0] + 0.5 * k2 * dx).max() < 1e-13 and np.abs(fx[nx] + 0.5 * k2 * (2 * nx - 1) * dx).max() < 1e-13
+    assert np.abs(fy).max() == 0.0
+    # along y: a_z = sin(2 pi j / ny): -1/2 d(a^2)/dy by central differences of the periodic grid
+    j = np.arange(ny)[None, :] * np.ones((nx + 1, 1))
+    o.a_now[0][:] = np.sin(2 * math.pi * j / ny)
+    o.a_now[1][:] = 0.0
+    fx, fy = o.force_now(0)
+    a2 = np.sin(2 * math.pi * j / ny) ** 2
+    assert np.abs(fy + 0.5 * (np.roll(a2, -1, 1) - np.roll(a2, 1, 1)) / (2 * dx)).max() < 1e-13 and np.abs(fx).max() < 1e-13
+    fx, fy = o.force_now(1)
+    assert np.abs(fx).max() == 0.0 and np.abs(fy).max() == 0.0
