@@ -1,0 +1,193 @@
+"""SURVEY 8(f).3 without a second GPU: the x-slab decomposition of the deposit, of the Poisson solve and of the particle
+lists (oracle/slabs.py) against the single-domain oracle.  world_size 2 over gloo, and the same
+arithmetic for three and five slabs in one process.  CPU only."""
+import os
+import socket
+import sys
+
+import numpy as np
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+class _SerialComm:
+    """all_gather for ranks that run one after the other in one process: two passes (publish, then compute)."""
+
+    def __init__(self, world):
+        self.world, self.box, self.replay = world, [], None
+
+    def all_gather(self, obj):
+        if self.replay is None:
+            self.box.append(obj)
+            raise _Publish
+        return self.replay
+
+
+class _Publish(Exception):
+    pass
+
+
+def _run_serial(world, fn):
+    """fn(rank, comm) with exactly one all_gather inside: first pass collects, second pass computes."""
+    comm = _SerialComm(world)
+    for r in range(world):
+        try:
+            fn(r, comm)
+        except _Publish:
+            pass
+    comm.replay = comm.box
+    return [fn(r, comm) for r in range(world)]
+
+
+class _DistComm:
+    def all_gather(self, obj):
+        out = [None] * dist.get_world_size()
+        dist.all_gather_object(out, obj)
+        return out
+
+
+def _case(nx=72, ny=16):
+    import oracle.loader as L
+    import pm2d_inputs as I
+    cfg = I.config("c3", nx=nx, ny=ny)
+    parts = [L.generate_particles(cfg, s) for s in (0, 1)]
+    return cfg, parts
+
+
+def _slab_density_and_phi(cfg, parts, world, rank, comm_n, comm_p):
+    from oracle import slabs
+    g = cfg["grid"]
+    nx, ny, dx, dy, dt = g["nx"], g["ny"], g["dx"], g["dy"], g["dt"]
+    x_lo, x_hi = slabs.slab_cells(nx, world, rank)
+    rho = 0.0
+    dens = []
+    for s, sp in enumerate(cfg["species"]):
+        p = parts[s]
+        X = p["ix"] + p["fx"].astype(np.float64)
+        Y = p["iy"] + p["fy"].astype(np.float64)
+        mine = (X >= x_lo) & (X < x_hi)
+        n, px, py, g_lo = slabs.slab_deposit(nx, ny, dx, dy, dt, sp["shape"], sp["DD"], X[mine], Y[mine], p["ux"][mine], p["uy"][mine],
+                                             p["w"][mine].astype(np.float64), x_lo, x_hi)
+        own = slabs.add_ghosts(nx, ny, world, rank, n, g_lo, comm_n[s])
+        dens.append(own)
+        rho = rho + sp["sign"] * own
+    phi = slabs.slab_poisson(nx, ny, dx, dy, world, rank, rho, comm_p)
+    return dens, phi
+
+
+def _reference(cfg, parts):
+    import oracle
+    g = cfg["grid"]
+    grid = oracle.make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"])
+    dens, rho = [], 0.0
+    for s, sp in enumerate(cfg["species"]):
+        p = parts[s]
+        n, _, _ = oracle.deposit(grid, sp["shape"], sp["DD"], p["ix"] + p["fx"].astype(np.float64), p["iy"] + p["fy"].astype(np.float64),
+                                 p["ux"], p["uy"], p["w"].astype(np.float64))
+        dens.append(n)
+        rho = rho + sp["sign"] * n
+    return dens, oracle.poisson(grid, rho).reshape(g["nx"] + 1, g["ny"])
+
+
+def _serial_check(world, nx):
+    """Every all_gather of the slab routines in its own two-pass communicator."""
+    cfg, parts = _case(nx=nx)
+    from oracle import slabs
+    g = cfg["grid"]
+    nxx, ny = g["nx"], g["ny"]
+    ref_dens, ref_phi = _reference(cfg, parts)
+    # pass 1: deposits + ghost sums, per species
+    owned = []
+    for s, sp in enumerate(cfg["species"]):
+        p = parts[s]
+        X = p["ix"] + p["fx"].astype(np.float64)
+        Y = p["iy"] + p["fy"].astype(np.float64)
+
+        def dep(rank, comm, X=X, Y=Y, p=p, sp=sp):
+            x_lo, x_hi = slabs.slab_cells(nxx, world, rank)
+            mine = (X >= x_lo) & (X < x_hi)
+            n, _, _, g_lo = slabs.slab_deposit(nxx, ny, g["dx"], g["dy"], g["dt"], sp["shape"], sp["DD"], X[mine], Y[mine], p["ux"][mine],
+                                               p["uy"][mine], p["w"][mine].astype(np.float64), x_lo, x_hi)
+            return slabs.add_ghosts(nxx, ny, world, rank, n, g_lo, comm)
+        owned.append(_run_serial(world, dep))
+        assert np.abs(np.concatenate(owned[s]) - ref_dens[s]).max() < 1e-13 * np.abs(ref_dens[s]).max()
+    rho = [sum(sp["sign"] * owned[s][r] for s, sp in enumerate(cfg["species"])) for r in range(world)]
+    phis = _run_serial(world, lambda rank, comm: slabs.slab_poisson(nxx, ny, g["dx"], g["dy"], world, rank, rho[rank], comm))
+    phi = np.concatenate(phis)
+    assert phi.shape == ref_phi.shape
+    assert np.abs(phi - ref_phi).max() < 1e-11 * np.abs(ref_phi).max()
+
+
+def test_three_and_five_slabs_equal_the_single_domain():
+    """Ghost-column deposit sums and the interface system for 3 slabs (72 cells) and 5 slabs of unequal width (73 cells:
+    15, 15, 15, 14, 14): densities to rounding, phi to 1e-11 of its maximum."""
+    sys.path.insert(0, ROOT)
+    _serial_check(3, 72)
+    _serial_check(5, 73)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from oracle import slabs
+    cfg, parts = _case()
+    comm = _DistComm()
+    dens, phi = _slab_density_and_phi(cfg, parts, world, rank, [comm, comm], comm)
+    # the particle lists after a displacement that sends some particles across the cut (both ways)
+    g = cfg["grid"]
+    x_lo, x_hi = slabs.slab_cells(g["nx"], world, rank)
+    p = parts[0]
+    X = p["ix"] + p["fx"].astype(np.float64)
+    mine = (X >= x_lo) & (X < x_hi)
+    rng = np.random.default_rng(7 + rank)
+    mov = dict(X=np.clip(X[mine] + rng.normal(0.0, 1.5, mine.sum()), 0.0, g["nx"] - 1e-9), id=p["id"][mine].copy(),
+               ux=p["ux"][mine].copy())
+    got = slabs.migrate(mov, x_lo, x_hi, rank, world, comm)
+    out.put((rank, dens, phi, mov, got))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_slabs_over_gloo_equal_the_single_domain():
+    sys.path.insert(0, ROOT)
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=300) for _ in range(world)), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    cfg, parts = _case()
+    ref_dens, ref_phi = _reference(cfg, parts)
+    for s in (0, 1):
+        n = np.concatenate([r[1][s] for r in res])
+        assert np.abs(n - ref_dens[s]).max() < 1e-13 * np.abs(ref_dens[s]).max()
+    phi = np.concatenate([r[2] for r in res])
+    assert np.abs(phi - ref_phi).max() < 1e-11 * np.abs(ref_phi).max()
+    # migration: every rank ends with exactly the particles of its slab; nothing lost, nothing doubled; the fields of a
+    # particle travel together
+    from oracle import slabs
+    g = cfg["grid"]
+    before = {int(i): (x, u) for r in res for i, x, u in zip(r[3]["id"], r[3]["X"], r[3]["ux"])}
+    after = {}
+    crossed = 0
+    for rank, _, _, mov, got in res:
+        x_lo, x_hi = slabs.slab_cells(g["nx"], world, rank)
+        assert ((got["X"] >= x_lo) & (got["X"] < x_hi)).all()
+        crossed += int(((mov["X"] < x_lo) | (mov["X"] >= x_hi)).sum())
+        for i, x, u in zip(got["id"], got["X"], got["ux"]):
+            assert int(i) not in after
+            after[int(i)] = (x, u)
+    assert crossed > 50 and after == before
