@@ -230,14 +230,18 @@ def _rank_in_group(group_sorted):
     return np.arange(n) - np.repeat(start, np.diff(np.r_[start, n]))
 
 
-def _lane_order_perm(pp, T, nty, subs):
+def _lane_order_perm(pp, T, nty, subs, predx=0.0, predy=0.0):
     """The lane order as include/pm2d.h states it for pm2d_rebin, written out with numpy's stable sorts."""
     n = pp["ix"].size
     ix, iy = pp["ix"].astype(np.int64), pp["iy"].astype(np.int64)
-    fx24 = np.round(pp["fx"].astype(np.float64) * 2 ** 24).astype(np.int64)
-    fy24 = np.round(pp["fy"].astype(np.float64) * 2 ** 24).astype(np.int64)
     tile = (ix // T) * nty + iy // T
-    cx, cy = ix % T, iy % T
+
+    def sort_pos(i, f, u, pred):
+        v = (i % T) * 2 ** 24 + np.round(f.astype(np.float64) * 2 ** 24).astype(np.int64)
+        v = v + np.rint((u.astype(np.float32) * np.float32(pred)).astype(np.float64)).astype(np.int64)
+        return np.clip(v, 0, T * 2 ** 24 - 1)
+    xs, ys = sort_pos(ix, pp["fx"], pp["ux"], predx), sort_pos(iy, pp["fy"], pp["uy"], predy)
+    cx, cy, fx24, fy24 = xs >> 24, ys >> 24, xs & (2 ** 24 - 1), ys & (2 ** 24 - 1)
     h = (cx >> 4) if subs == 2 else np.zeros_like(cx)
     key_a = (h << 10) | (cy << 5) | (fy24 >> 19)
     xb = (((cx & 15) << 1) | (fx24 >> 23)) if subs == 2 else cx
@@ -275,7 +279,12 @@ def test_rebin_is_a_stable_counting_sort(P, order):
     for sp in cfg["species"]:
         sp["T_keV"] *= 40.0                                   # fast particles: many tile and cell crossings
     cfg["species"][0]["ppc_x"], cfg["species"][0]["ppc_y"] = 5, 4        # 20 per cell: the layered tail (ranks >= 16) is used
-    sim = P.PM2D(cfg, track_ids=1, rebin_every=0, particle_order=order)
+    # the lane order sorts by the position half a rebin period ahead: give it a period (no automatic rebin falls into
+    # the 9 steps below); the other orders are tested without
+    every = 16 if order == 4 else 0
+    sim = P.PM2D(cfg, track_ids=1, rebin_every=every, particle_order=order)
+    g = cfg["grid"]
+    pred = [every * g["dt"] / (2.0 * g[d]) * 2.0 ** 24 for d in ("dx", "dy")]
     T = P.TILE
     nty = (128 + T - 1) // T
     ntx = (136 + T - 1) // T
@@ -313,7 +322,7 @@ def test_rebin_is_a_stable_counting_sort(P, order):
         key_ref = key_of(before)
         keys, perm = sim.rebin(0)
         assert np.array_equal(keys, key_ref.astype(np.int32))
-        perm_ref = _lane_order_perm(before, T, nty, sim.lane_subs(0)) if order == 4 else expected_perm(key_ref)
+        perm_ref = _lane_order_perm(before, T, nty, sim.lane_subs(0), pred[0], pred[1]) if order == 4 else expected_perm(key_ref)
         assert np.array_equal(perm, perm_ref)
         after = sim.get_particles(0, with_id=True)
         for k in before:
