@@ -239,15 +239,18 @@ int pm2d_set_background(pm2d_ctx *ctx, int species, const float *host);
  * sort by key.  LAYERED species: with r = the rank of a particle among those of equal key in the old order, the
  * result is sorted by tile, then layer min(r, 16); inside a layer below 16 by (rank of the cell among the cells of
  * the same tile and the same iy that hold more than r particles, in ix order; iy), inside the tail by (cell, r).
- * LANES species: after the stable sort by tile, inside every tile, with the SORT position of a particle = its
- * tile-relative position plus the free flight of half a rebin period, in units of 2^-24 cell,
- *     xs = clamp((ix % 32) 2^24 + fx 2^24 + rint(float(ux) * float(rebin_every * S dt / (2 dx) * 2^24)), 0, 32 * 2^24 - 1)
- * (float32 product, round to nearest; ys likewise) and ix', fx', iy', fy' the cell and offset of (xs, ys):
+ * LANES species are sorted by their SORT position: the position plus the free flight of half a rebin period, in
+ * units of 2^-24 cell,
+ *     xs = ix 2^24 + fx 2^24 + rint(float(ux) * float(rebin_every * S dt / (2 dx) * 2^24))      (float32 product, round to nearest)
+ * clamped to [0, nx 2^24 - 1] (a sort position beyond a wall stays in the wall tile), ys likewise but wrapped into [0, ny 2^24).
+ * The tile is that of (xs, ys); keys_out = tile * PM2D_TILE^2 + cell of (xs, ys) in the tile.  After the stable sort by tile,
+ * inside every tile, with ix', fx', iy', fy' the tile-relative cell and offset of (xs, ys):
  * h = sub-tile (ix' >= 16 when pm2d_lane_subs is 2,
  * else 0); rho = rank in the stable sort by key_A = (h, iy', floor(32 fy')); slab = the rho-th of the N_h particles
  * of the sub-tile cut into 32 slabs whose sizes differ by at most one (the first N_h mod 32 slabs hold one more);
  * w = rank inside the slab in the stable sort by key_B = (h, slab, x bin), x bin = (2 (ix' % 16) + floor(2 fx')) resp.
- * ix'; slot = first slot of the sub-tile + 32 w + slab. */
+ * ix'; slot = first slot of the sub-tile + 32 w + slab.  (A particle may therefore be listed in a tile next to the one
+ * it sits in; pm2d_get_particles always returns its true cell.) */
 int pm2d_rebin(pm2d_ctx *ctx, int species, int32_t *keys_out, int64_t *perm_out);
 
 int pm2d_diagnostics(pm2d_ctx *ctx, pm2d_diag *out);

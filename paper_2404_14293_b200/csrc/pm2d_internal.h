@@ -154,6 +154,7 @@ int launch_unpack_particles(pm2d_ctx *c, int s, int32_t *ix, int32_t *iy, float 
 int launch_lanesort(pm2d_ctx *c, int s, bool from_primary, int32_t *keys_dev, int64_t *perm_dev, const int64_t *perm1_dev);
 int launch_stage_lanes(pm2d_ctx *c, int s, int stage, int qmask);
 double lane_ucap(const SpeciesDev &S);
+float lane_pred(const pm2d_ctx *c, int axis);
 int lanes_make_tensor_map(pm2d_ctx *c, int s);
 // pm2d_fields.cu
 int launch_field_step(pm2d_ctx *c, int sub);

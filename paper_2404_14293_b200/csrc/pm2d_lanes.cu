@@ -660,6 +660,7 @@ struct LaneSortParams {
     int32_t *lane_exp;          // [ntiles] out: sp of the tile (momentum unit of the windows of k_stage_lanes)
     float pscale_ucap;          // global fixed-point scale of the momentum times the velocity cap
     float predx, predy;         // see lane_sort_pos
+    int nx, ny, nty;
     uint32_t *scratch;          // [np] keys between the sweeps
     const int64_t *perm1;       // optional (tests): slot before the tile pass of every slot after it
     int32_t *keys_out;
@@ -674,10 +675,10 @@ constexpr int LS_WARPS = 8, LS_BINS = 2048;
 // rebin_every * dt_p / (2 dx) * 2^24 (tile-relative, 2^-24 cells), clamped to the tile.  A particle then strays from its
 // lane by the drift of half a period in either direction instead of a whole period in one: 3 keV electrons at a period
 // of 16 steps leave the four-copy range in 0.005 % of the visits instead of 0.4 %.
-__device__ __forceinline__ uint32_t lane_sort_pos(uint32_t f, float u, float pred)
+__device__ __forceinline__ uint32_t lane_sort_pos(uint32_t f, float u, float pred, int cells)
 {
     const int64_t v = (int64_t)f - ((int64_t)POS_BIAS << POS_FRAC_BITS) + (int64_t)__float2int_rn(__fmul_rn(u, pred));
-    return (uint32_t)min(max(v, (int64_t)0), ((int64_t)TILE << POS_FRAC_BITS) - 1);
+    return (uint32_t)min(max(v, (int64_t)0), ((int64_t)cells << POS_FRAC_BITS) - 1);
 }
 
 __device__ __forceinline__ int lane_slab(int rho, int n)
@@ -782,6 +783,7 @@ __global__ void __launch_bounds__(LS_WARPS * 32) k_lanesort(const LaneSortParams
     uint16_t *myhist = hist + wid * LS_BINS;
     uint32_t *scr = C.scratch + t0;
     const bool two = C.subs == 2;
+    const int tw = min(TILE, C.nx - (tile / C.nty) * TILE), th = min(TILE, C.ny - (tile % C.nty) * TILE);     // cells of this tile
     // sweep 1: key_A | x bin << 16 of every particle, counts of key_A
     for (int64_t base = beg; base < end; base += 32) {
         const int64_t i = base + lane;
@@ -789,7 +791,7 @@ __global__ void __launch_bounds__(LS_WARPS * 32) k_lanesort(const LaneSortParams
         int k = LS_BINS + lane, xb = 0;
         if (live) {
             const PV me = C.src[t0 + i];
-            const uint32_t xk = lane_sort_pos(me.x, me.ux, C.predx), yk = lane_sort_pos(me.y, me.uy, C.predy);
+            const uint32_t xk = lane_sort_pos(me.x, me.ux, C.predx, tw), yk = lane_sort_pos(me.y, me.uy, C.predy, th);
             const int cx = (int)(xk >> POS_FRAC_BITS), cy = (int)(yk >> POS_FRAC_BITS);
             const int h = two ? cx >> 4 : 0;
             k = (h << 10) | (cy << 5) | (int)((yk >> (POS_FRAC_BITS - 5)) & 31u);
@@ -844,8 +846,9 @@ __global__ void __launch_bounds__(LS_WARPS * 32) k_lanesort(const LaneSortParams
             if (C.idsrc) C.iddst[q] = C.idsrc[t0 + i];
             if (C.perm1) {
                 const int64_t old = C.perm1[t0 + i];
-                if (C.keys_out) C.keys_out[old] = tile * TCELLS + max(0, min(TILE - 1, (int)(me.x >> POS_FRAC_BITS) - POS_BIAS)) * TILE +
-                                                  max(0, min(TILE - 1, (int)(me.y >> POS_FRAC_BITS) - POS_BIAS));
+                if (C.keys_out)
+                    C.keys_out[old] = tile * TCELLS + (int)(lane_sort_pos(me.x, me.ux, C.predx, tw) >> POS_FRAC_BITS) * TILE +
+                                      (int)(lane_sort_pos(me.y, me.uy, C.predy, th) >> POS_FRAC_BITS);
                 if (C.perm_out) C.perm_out[q] = old;
             }
         });
@@ -866,6 +869,12 @@ __global__ void k_iota64(int64_t *p, int64_t n)
 }
 
 }  // namespace
+
+// free flight of half a rebin period, in 2^-24 cells per unit velocity (axis 0 = x, 1 = y)
+float lane_pred(const pm2d_ctx *c, int axis)
+{
+    return (float)((double)c->g.rebin_every * c->dtp / (2.0 * (axis ? c->g.dy : c->g.dx)) * 16777216.0);
+}
 
 // velocity cap of the FFMA float -> int path of the momentum deposit: four thermal velocities; faster particles take the
 // exact path (a listed stray).  The smaller the cap, the finer the momentum unit of the windows.
@@ -895,8 +904,9 @@ int launch_lanesort(pm2d_ctx *c, int s, bool from_primary, int32_t *keys_dev, in
     C.sub0 = S.sub0;
     C.lane_exp = S.lane_exp;
     C.pscale_ucap = c->pscale * (float)lane_ucap(S);
-    C.predx = (float)((double)c->g.rebin_every * c->dtp / (2.0 * c->g.dx) * 16777216.0);
-    C.predy = (float)((double)c->g.rebin_every * c->dtp / (2.0 * c->g.dy) * 16777216.0);
+    C.nx = c->g.nx; C.ny = c->g.ny; C.nty = c->nty;
+    C.predx = lane_pred(c, 0);
+    C.predy = lane_pred(c, 1);
     C.scratch = reinterpret_cast<uint32_t *>(S.uh);          // u^ is scratch outside a step
     C.perm1 = perm1_dev; C.keys_out = keys_dev; C.perm_out = perm_dev;
     C.flags = c->flags;
