@@ -38,7 +38,8 @@ extern "C" {
 #define PM2D_EINVAL (-1)  /* bad argument: ny not a power of two, dt above the stability bound, ... */
 #define PM2D_ENOMEM (-2)  /* workspace or host buffer too small */
 #define PM2D_ECUDA (-3)   /* a CUDA call or kernel failed */
-#define PM2D_ESTATE (-4)  /* call not valid in the current state (e.g. particle left the rebin range) */
+#define PM2D_ESTATE (-4)  /* call not valid in the current state (e.g. particle left the rebin range; a deposit left the
+                             fixed-point range of the grids: density above 4 n_max of the profile, lane order only) */
 
 #define PM2D_MAX_SPECIES 4
 #define PM2D_MAX_LASERS 4

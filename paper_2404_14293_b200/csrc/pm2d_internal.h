@@ -115,7 +115,7 @@ struct pm2d_ctx {
     int cap_extra;       // tuning: see PartParams::cap_extra
     // profile
     bool prof_on;
-    std::vector<cudaEvent_t> ev;   // 2 per phase per step, reused ring
+    std::vector<cudaEvent_t> ev;   // 2 per phase per step while profiling is on; pm2d_profile_get folds them into prof_ms and frees them
     std::vector<int> ev_phase;
     double prof_ms[PM2D_PH_COUNT];
     int64_t prof_launch[PM2D_PH_COUNT];

@@ -583,6 +583,9 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
         const int gj = (gy0 + z + MLO - 1) & (P.ny - 1);
         const int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
         const size_t k = (size_t)gi * P.ny + gj;
+        // one window alone beyond half the int32 range of the global grids (n > n_cap / 2 = 4 n_max of the profile, |n u| >
+        // n_cap / 32): the integer sums are about to wrap -- report it instead of handing negative densities to the solvers
+        if (abs(v) > (1 << 30) / fac || abs(vx) > ((1 << 30) >> sp) / fac || abs(vy) > ((1 << 30) >> sp) / fac) P.flags[3] = 2;
         if (v) atomicAdd(&P.nfix[k], fac * v);
         if (vx) atomicAdd(&P.pxfix[k], fac * mp * vx);
         if (vy) atomicAdd(&P.pyfix[k], fac * mp * vy);
@@ -696,25 +699,38 @@ __device__ __forceinline__ int lane_slab_start(int i, int n)
 
 // stable rank of every particle of this warp's part [beg, end) in its bin: hist[bin] holds the first rank of the bin
 // for this warp (16-bit, updated as the batches go by); fn(i, rank, key) is called once per particle
-template <class KeyFn, class OutFn>
-__device__ __forceinline__ void lane_rank_sweep(int64_t beg, int64_t end, int lane, uint16_t *myhist, KeyFn key, OutFn out)
+// load(i) fetches what the particle needs (its key among it) -- the loads of LS_AHEAD batches are issued before the first
+// of them is ranked, so the serial chain match -> histogram update of a warp does not wait for memory batch by batch
+constexpr int LS_AHEAD = 4;
+template <class T, class LoadFn, class KeyFn, class OutFn>
+__device__ __forceinline__ void lane_rank_sweep(int64_t beg, int64_t end, int lane, uint16_t *myhist, LoadFn load, KeyFn key, OutFn out)
 {
-    for (int64_t base = beg; base < end; base += 32) {
-        const int64_t i = base + lane;
-        const bool live = i < end;
-        int k = LS_BINS + lane;                      // dead lanes: unique keys
-        if (live) k = key(i);
-        const unsigned peers = __match_any_sync(0xffffffffu, k);
-        const int rank = __popc(peers & ((1u << lane) - 1u));
-        const int leader = __ffs(peers) - 1;
-        int b = 0;
-        if (live && lane == leader) {
-            b = myhist[k];
-            myhist[k] = (uint16_t)(b + __popc(peers));
+    for (int64_t base0 = beg; base0 < end; base0 += 32 * LS_AHEAD) {
+        T v[LS_AHEAD];
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            const int64_t i = base0 + 32 * u + lane;
+            if (i < end) v[u] = load(i);
         }
-        b = __shfl_sync(0xffffffffu, b, leader);
-        __syncwarp();
-        if (live) out(i, b + rank, k);
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            if (base0 + 32 * u >= end) break;        // warp-uniform
+            const int64_t i = base0 + 32 * u + lane;
+            const bool live = i < end;
+            int k = LS_BINS + lane;                  // dead lanes: unique keys
+            if (live) k = key(v[u]);
+            const unsigned peers = __match_any_sync(0xffffffffu, k);
+            const int rank = __popc(peers & ((1u << lane) - 1u));
+            const int leader = __ffs(peers) - 1;
+            int b = 0;
+            if (live && lane == leader) {
+                b = myhist[k];
+                myhist[k] = (uint16_t)(b + __popc(peers));
+            }
+            b = __shfl_sync(0xffffffffu, b, leader);
+            __syncwarp();
+            if (live) out(i, b + rank, k, v[u]);
+        }
     }
 }
 
@@ -785,32 +801,42 @@ __global__ void __launch_bounds__(LS_WARPS * 32) k_lanesort(const LaneSortParams
     const bool two = C.subs == 2;
     const int tw = min(TILE, C.nx - (tile / C.nty) * TILE), th = min(TILE, C.ny - (tile % C.nty) * TILE);     // cells of this tile
     // sweep 1: key_A | x bin << 16 of every particle, counts of key_A
-    for (int64_t base = beg; base < end; base += 32) {
-        const int64_t i = base + lane;
-        const bool live = i < end;
-        int k = LS_BINS + lane, xb = 0;
-        if (live) {
-            const PV me = C.src[t0 + i];
-            const uint32_t xk = lane_sort_pos(me.x, me.ux, C.predx, tw), yk = lane_sort_pos(me.y, me.uy, C.predy, th);
-            const int cx = (int)(xk >> POS_FRAC_BITS), cy = (int)(yk >> POS_FRAC_BITS);
-            const int h = two ? cx >> 4 : 0;
-            k = (h << 10) | (cy << 5) | (int)((yk >> (POS_FRAC_BITS - 5)) & 31u);
-            xb = two ? ((cx & 15) << 1) | (int)((xk >> (POS_FRAC_BITS - 1)) & 1u) : cx;
-            scr[i] = (uint32_t)k | ((uint32_t)xb << 16);
+    for (int64_t base0 = beg; base0 < end; base0 += 32 * LS_AHEAD) {
+        PV mv[LS_AHEAD];
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            const int64_t i = base0 + 32 * u + lane;
+            if (i < end) mv[u] = C.src[t0 + i];
         }
-        const unsigned peers = __match_any_sync(0xffffffffu, k);
-        if (live && lane == __ffs(peers) - 1) myhist[k] = (uint16_t)(myhist[k] + __popc(peers));
-        __syncwarp();
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            if (base0 + 32 * u >= end) break;
+            const int64_t i = base0 + 32 * u + lane;
+            const bool live = i < end;
+            int k = LS_BINS + lane;
+            if (live) {
+                const PV me = mv[u];
+                const uint32_t xk = lane_sort_pos(me.x, me.ux, C.predx, tw), yk = lane_sort_pos(me.y, me.uy, C.predy, th);
+                const int cx = (int)(xk >> POS_FRAC_BITS), cy = (int)(yk >> POS_FRAC_BITS);
+                const int h = two ? cx >> 4 : 0;
+                k = (h << 10) | (cy << 5) | (int)((yk >> (POS_FRAC_BITS - 5)) & 31u);
+                const int xb = two ? ((cx & 15) << 1) | (int)((xk >> (POS_FRAC_BITS - 1)) & 1u) : cx;
+                scr[i] = (uint32_t)k | ((uint32_t)xb << 16);
+            }
+            const unsigned peers = __match_any_sync(0xffffffffu, k);
+            if (live && lane == __ffs(peers) - 1) myhist[k] = (uint16_t)(myhist[k] + __popc(peers));
+            __syncwarp();
+        }
     }
     __syncthreads();
     lane_scan(hist, wsum);
     const int n0 = two ? (int)hist[LS_BINS / 2] : (int)n, n1 = (int)n - n0;     // first rank of bin (h = 1, 0, 0) = particles of sub-tile 0
     if (threadIdx.x == 0) C.sub0[tile] = n0;
     // sweep 2: rank in (h, y) -> slab -> key_B
-    lane_rank_sweep(
-        beg, end, lane, myhist, [&](int64_t i) { return (int)(scr[i] & 0xffffu); },
-        [&](int64_t i, int rho, int k) {
-            const int h = k >> 10, xb = (int)(scr[i] >> 16);
+    lane_rank_sweep<uint32_t>(
+        beg, end, lane, myhist, [&](int64_t i) { return scr[i]; }, [](uint32_t v) { return (int)(v & 0xffffu); },
+        [&](int64_t i, int rho, int k, uint32_t v) {
+            const int h = k >> 10, xb = (int)(v >> 16);
             const int slab = h ? lane_slab(rho - n0, n1) : lane_slab(rho, n0);
             scr[i] = (uint32_t)((h << 10) | (slab << 5) | xb);
         });
@@ -818,28 +844,40 @@ __global__ void __launch_bounds__(LS_WARPS * 32) k_lanesort(const LaneSortParams
     for (int e = threadIdx.x; e < LS_WARPS * LS_BINS / 2; e += LS_WARPS * 32) hist32[e] = 0u;
     __syncthreads();
     // sweep 3: counts of key_B
-    for (int64_t base = beg; base < end; base += 32) {
-        const int64_t i = base + lane;
-        const bool live = i < end;
-        int k = LS_BINS + lane;
-        if (live) k = (int)scr[i];
-        const unsigned peers = __match_any_sync(0xffffffffu, k);
-        if (live && lane == __ffs(peers) - 1) myhist[k] = (uint16_t)(myhist[k] + __popc(peers));
-        __syncwarp();
+    for (int64_t base0 = beg; base0 < end; base0 += 32 * LS_AHEAD) {
+        int kk[LS_AHEAD];
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            const int64_t i = base0 + 32 * u + lane;
+            kk[u] = i < end ? (int)scr[i] : LS_BINS + lane;
+        }
+#pragma unroll
+        for (int u = 0; u < LS_AHEAD; u++) {
+            if (base0 + 32 * u >= end) break;
+            const bool live = base0 + 32 * u + lane < end;
+            const unsigned peers = __match_any_sync(0xffffffffu, kk[u]);
+            if (live && lane == __ffs(peers) - 1) myhist[kk[u]] = (uint16_t)(myhist[kk[u]] + __popc(peers));
+            __syncwarp();
+        }
     }
     __syncthreads();
     lane_scan(hist, wsum);
     // sweep 4: rank in (h, slab, x) -> slot; move the records
     float wmax = 0.f;
-    lane_rank_sweep(
-        beg, end, lane, myhist, [&](int64_t i) { return (int)scr[i]; },
-        [&](int64_t i, int rb, int k) {
+    struct Rec {
+        PV me;
+        float w;
+        int key;
+    };
+    lane_rank_sweep<Rec>(
+        beg, end, lane, myhist, [&](int64_t i) { return Rec{C.src[t0 + i], C.wsrc[t0 + i], (int)scr[i]}; }, [](const Rec &r) { return r.key; },
+        [&](int64_t i, int rb, int k, const Rec &r) {
             const int h = k >> 10, slab = (k >> 5) & 31;
             const int nn = h ? n1 : n0, hb = h ? n0 : 0;
             const int w = rb - hb - lane_slab_start(slab, nn);      // rank inside the slab
             const int64_t q = t0 + hb + 32 * w + slab;
-            const PV me = C.src[t0 + i];
-            const float wi = C.wsrc[t0 + i];
+            const PV me = r.me;
+            const float wi = r.w;
             wmax = fmaxf(wmax, wi);
             C.dst[q] = me;
             C.wdst[q] = wi;

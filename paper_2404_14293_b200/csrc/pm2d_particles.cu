@@ -1404,7 +1404,11 @@ static void launch_stage_shape(const PartParams &P, int stage, int qmask, int gr
 #define PM2D_LAUNCH(ST, Q)                                                         \
     do {                                                                           \
         if (sparse && anch) {                                                      \
-            cudaFuncSetAttribute(k_stage_direct<SHAPE, ST, Q, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)direct_smem_bytes<ST, Q, true>()); \
+            static bool once_ = false;                                             \
+            if (!once_) {                                                          \
+                cudaFuncSetAttribute(k_stage_direct<SHAPE, ST, Q, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)direct_smem_bytes<ST, Q, true>()); \
+                once_ = true;                                                      \
+            }                                                                      \
             k_stage_direct<SHAPE, ST, Q, true><<<grid, 256, direct_smem_bytes<ST, Q, true>(), st>>>(P); \
         } else if (sparse)                                                         \
             k_stage_direct<SHAPE, ST, Q, false><<<grid, 256, direct_smem_bytes<ST, Q, false>(), st>>>(P); \
