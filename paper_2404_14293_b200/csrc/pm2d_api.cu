@@ -234,7 +234,7 @@ int check_flags(pm2d_ctx *c)
     if (h[0]) return fail(PM2D_ESTATE, "a particle moved further than one tile between rebins (rebin_every too large)");
     if (h[1]) return fail(PM2D_ESTATE, "chunk table overflow");
     if (h[2]) return fail(PM2D_ESTATE, "too many particles outside their tile window (rebin_every too large)");
-    if (h[3] == 2) return fail(PM2D_ESTATE, "a deposit exceeds the fixed-point range of the grids (density above 4 n_max of the profile, or |n u| above n_max / 4)");
+    if (h[3] == 2) return fail(PM2D_ESTATE, "a deposit exceeds the fixed-point range of the grids (density above 4 n_max of the profile, or |n u| above n_max / 2)");
     if (h[3]) return fail(PM2D_ESTATE, "lane order: a tile holds more than 65535 particles (use PM2D_ORDER_CELL_MAJOR)");
     return PM2D_OK;
 }

@@ -583,9 +583,12 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
         const int gj = (gy0 + z + MLO - 1) & (P.ny - 1);
         const int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
         const size_t k = (size_t)gi * P.ny + gj;
-        // one window alone beyond half the int32 range of the global grids (n > n_cap / 2 = 4 n_max of the profile, |n u| >
-        // n_cap / 32): the integer sums are about to wrap -- report it instead of handing negative densities to the solvers
-        if (abs(v) > (1 << 30) / fac || abs(vx) > ((1 << 30) >> sp) / fac || abs(vy) > ((1 << 30) >> sp) / fac) P.flags[3] = 2;
+        // the integer sums wrap: report it instead of handing wrapped moments to the solvers.  Density (all terms of one
+        // sign): one window alone beyond half the int32 range, n > n_cap / 2 = 4 n_max of the profile.  Momentum (terms of
+        // either sign, a hot species reaches a large fraction of the range by noise alone): this window's sum itself is
+        // outside int32, |n u| > n_cap / 16 = n_max / 2
+        const int64_t wide_x = (int64_t)(fac * mp) * vx, wide_y = (int64_t)(fac * mp) * vy;
+        if (abs(v) > (1 << 30) / fac || wide_x != (int32_t)wide_x || wide_y != (int32_t)wide_y) P.flags[3] = 2;
         if (v) atomicAdd(&P.nfix[k], fac * v);
         if (vx) atomicAdd(&P.pxfix[k], fac * mp * vx);
         if (vy) atomicAdd(&P.pyfix[k], fac * mp * vy);

@@ -367,7 +367,7 @@ def test_set_particles_roundtrip_and_host_supplied_inputs(P):
                  fx=(rng.integers(0, 2 ** 24, n) / 2.0 ** 24).astype(np.float32),
                  fy=(rng.integers(0, 2 ** 24, n) / 2.0 ** 24).astype(np.float32),
                  ux=rng.normal(0, 0.08, n).astype(np.float32), uy=rng.normal(0, 0.08, n).astype(np.float32),
-                 w=rng.uniform(0.01, 0.03, n).astype(np.float32))
+                 w=rng.uniform(0.0025, 0.0075, n).astype(np.float32))
     parts["ix"][:4] = [0, nx - 1, 5, 7]
     parts["fx"][:4] = [0.0, 1.0 - 2.0 ** -24, 0.0, 0.5]
     parts["ux"][:2] = [-0.3, 0.3]                             # into the walls
@@ -395,6 +395,12 @@ def test_set_particles_roundtrip_and_host_supplied_inputs(P):
     ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, 0, math.sqrt(3.0 / 511.0))
     assert max(ex, ey, eu) < 1e-5 and dabs < 1e-4
     assert sim.particle_count(0) == n and sim.diagnostics()["count"][0] == n
+    # four times the weight: the unneutralised electrons reach the walls at |u| ~ 0.5 within these steps and the stored
+    # (doubled, Q9) wall value of n u leaves the fixed-point range n_max / 2 -- reported, not wrapped (lane order)
+    heavy = dict(parts, w=parts["w"] * np.float32(4.0))
+    sim.set_particles(0, heavy, refix_background=False)
+    with pytest.raises(P.PM2DError, match="fixed-point range"):
+        sim.step(8)
     sim.close()
 
 
