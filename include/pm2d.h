@@ -286,6 +286,23 @@ int64_t pm2d_get_probe(pm2d_ctx *ctx, int wall, int comp, float *host, size_t ca
 int64_t pm2d_probe_spectrum(pm2d_ctx *ctx, int wall, int comp, int j0, int j1, int nomega, const double *omega, double *power);
 
 int pm2d_mode_amplitudes(pm2d_ctx *ctx, int species, int nmodes, const int32_t *mx, const int32_t *my, double *re, double *im);
+/* The same sum for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * no ctx, no workspace, no cudaMalloc / cudaFree / allocating library routine, no synchronisation.
+ *   n_dev    DEVICE float[(nx + 1) * ny], a nodal density in the layout of pm2d_get_moments (read only)
+ *   mx, my   HOST int32[nmodes], copied into the launch parameters before the call returns
+ *   out_dev  DEVICE double[2 * nmodes]: Re A, Im A of mode k in out_dev[2 k], out_dev[2 k + 1], written on `stream`
+ *   stream   cudaStream_t (NULL = the default stream); two kernels are enqueued on it
+ * ny is any size >= 1 here (no FFT).  Scratch: per-row partial sums in ONE file-scope device array of the library,
+ * PM2D_STATIC_MAX_ROWS * PM2D_MAX_MODES * 16 bytes = 4.0 MiB, held by every GPU that loads libpm2d.so until the process
+ * exits.  nx + 1 > PM2D_STATIC_MAX_ROWS is refused with PM2D_EINVAL (use pm2d_mode_amplitudes).  The first call on a
+ * device resolves the array's device address (cudaGetSymbolAddress, once per device, that device current): make that
+ * call outside a graph capture.  Every call shares the array and leaves its partial sums in it; a call overwrites all
+ * the entries it reads, so nothing has to be cleared, but two calls that OVERLAP on the GPU (different streams, or
+ * graphs replayed concurrently) race on it: order them.  float32 input, float64 sums in a fixed order (the result is
+ * reproducible bit for bit, unlike pm2d_mode_amplitudes' atomics). */
+#define PM2D_STATIC_MAX_ROWS 16385
+int pm2d_mode_amplitudes_static(const float *n_dev, int nx, int ny, int nmodes, const int32_t *mx, const int32_t *my,
+                                double *out_dev, void *stream);
 int64_t pm2d_particle_count(pm2d_ctx *ctx, int species);
 
 /* CUDA-event profile of the step phases on the ctx's stream.  enable(1) starts recording one event

@@ -82,6 +82,7 @@ SYMBOLS = {
     "pm2d_get_probe": (C.c_int64, [_vp, C.c_int, C.c_int, _fp, C.c_size_t, _lp]),
     "pm2d_probe_spectrum": (C.c_int64, [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pm2d_mode_amplitudes": (C.c_int, [_vp, C.c_int, C.c_int, _ip, _ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "pm2d_mode_amplitudes_static": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, _ip, _ip, _vp, _vp]),
     "pm2d_particle_count": (C.c_int64, [_vp, C.c_int]),
     "pm2d_profile_enable": (C.c_int, [_vp, C.c_int]),
     "pm2d_profile_get": (C.c_int, [_vp, C.POINTER(C.c_double), _lp, _lp]),
@@ -137,6 +138,25 @@ def polarised_beam(a0, theta, beta, **laser):
     out = (Laser * 3)()
     n = _check(load_library().pm2d_polarised_beam(C.byref(proto), float(theta), float(beta), out))
     return [dict(laser, a0=out[k].a0, comp=out[k].comp) for k in range(n)]
+
+
+STATIC_MAX_ROWS, MAX_MODES = 16385, 16
+
+
+def mode_amplitudes_static(n_dev, nx, ny, mx, my, out_dev, stream=0):
+    """pm2d_mode_amplitudes_static: n_dev a CUDA float32 tensor of (nx + 1) * ny nodes, out_dev a CUDA float64 tensor of
+    2 * len(mx) values (Re, Im interleaved), stream a raw cudaStream_t (0 = default stream).  Allocates nothing and does
+    not synchronise; two calls that overlap on the GPU race on the library's static scratch array."""
+    import torch
+    if not (n_dev.is_cuda and n_dev.dtype == torch.float32 and n_dev.is_contiguous() and n_dev.numel() == (nx + 1) * ny):
+        raise ValueError("n_dev: contiguous CUDA float32 tensor of (nx + 1) * ny elements")
+    mx, my = np.ascontiguousarray(mx, np.int32), np.ascontiguousarray(my, np.int32)
+    if mx.size != my.size:
+        raise ValueError("mx and my differ in length")
+    if not (out_dev.is_cuda and out_dev.dtype == torch.float64 and out_dev.is_contiguous() and out_dev.numel() >= 2 * mx.size):
+        raise ValueError("out_dev: contiguous CUDA float64 tensor of at least 2 * len(mx) elements")
+    _check(load_library().pm2d_mode_amplitudes_static(n_dev.data_ptr(), int(nx), int(ny), int(mx.size), mx.ctypes.data_as(_ip),
+                                                      my.ctypes.data_as(_ip), out_dev.data_ptr(), int(stream)))
 
 
 def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, particle_order=0):

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpm2d.so")
-SOURCES = ["pm2d_api.cu", "pm2d_particles.cu", "pm2d_lanes.cu", "pm2d_fields.cu", "pm2d_poisson.cu", "pm2d_diag.cu"]
+SOURCES = ["pm2d_api.cu", "pm2d_particles.cu", "pm2d_lanes.cu", "pm2d_fields.cu", "pm2d_poisson.cu", "pm2d_diag.cu", "pm2d_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-diag-suppress", "128", "-Wno-deprecated-gpu-targets"]
 
