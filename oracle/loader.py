@@ -16,6 +16,10 @@ within each cell, Maxwellian momenta ... all drawn from seed" (Q7).  R
                      profile: count(i, j) = floor(ppc * shape(i, j) + U), shape = taper(i) * filament(j) with
                      mean 1 over j, U = philox(counter=(cell_lo, cell_hi, species, 1))[0] * 2^-32 (a
                      dithered rounding, so the expected count is exact); offsets and momenta as RANDOM_MAXWELL
+     profile["slab"] = [x_lo, x_hi, y_lo, y_hi] (cells; absent or all zero: the whole box): only cells with
+                     x_lo <= i < x_hi and y_lo <= j < y_hi hold particles -- "a plasma slab is set at the center of the
+                     simulation box, and the vacuum space is usually set around the plasma slab"; ids, offsets,
+                     momenta and weights of the loaded cells are what they are without the slab
 The CUDA library runs the same recipe on the device (k_load); the two share no code.  Pins (tests/test_oracle_loader.py):
 Philox-4x32-10 against the Random123 known-answer vectors (tests/golden/philox4x32_10_kat.txt), particles per cell exact,
 w * N * M = profile at the cell centre, moments of the Maxwellian, expected counts of the number-weighted loading.
@@ -111,6 +115,17 @@ def profile_max(profile: dict) -> float:
     return float(min(p[0] * math.exp(max(p[1], 0.0)), p[2]))
 
 
+def slab_extent(cfg: dict):
+    """(x_lo, x_hi, y_lo, y_hi) of the cells that hold particles; the whole box without profile["slab"]."""
+    g = cfg["grid"]
+    sl = cfg["profile"].get("slab")
+    if not sl or not any(sl):
+        return 0, g["nx"], 0, g["ny"]
+    x_lo, x_hi, y_lo, y_hi = (int(v) for v in sl)
+    assert 0 <= x_lo < x_hi <= g["nx"] and 0 <= y_lo < y_hi <= g["ny"], sl
+    return x_lo, x_hi, y_lo, y_hi
+
+
 def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None):
     """Particles of species ``s`` for cells with i_lo <= i < i_hi (all j), in id order
     (k-major, then cell).  Returns dict(id, ix, iy, fx, fy, ux, uy, w) -- int64/int32/float32."""
@@ -118,9 +133,11 @@ def generate_particles(cfg: dict, s: int, i_lo: int = 0, i_hi: int | None = None
     nx, ny = g["nx"], g["ny"]
     i_hi = nx if i_hi is None else i_hi
     ppc = sp["ppc_x"] * sp["ppc_y"]
-    ii, jj = np.meshgrid(np.arange(i_lo, i_hi, dtype=np.int64), np.arange(ny, dtype=np.int64), indexing="ij")
+    x_lo, x_hi, y_lo, y_hi = slab_extent(cfg)
+    ii, jj = np.meshgrid(np.arange(max(i_lo, x_lo), min(i_hi, x_hi), dtype=np.int64), np.arange(y_lo, y_hi, dtype=np.int64), indexing="ij")
     cell = (ii * ny + jj).ravel()
     if sp["load"] == NUMBER_WEIGHTED:
+        assert (x_lo, x_hi, y_lo, y_hi) == (0, nx, 0, ny), "the number-weighted loading has no slab extent"
         cnt = cell_counts(cfg, s)[i_lo:i_hi].ravel()
         kmax = int(cnt.max()) if cnt.size else 0
         k = np.concatenate([np.full(int((cnt > kk).sum()), kk, dtype=np.int64) for kk in range(kmax)]) if kmax else np.zeros(0, np.int64)
@@ -179,4 +196,5 @@ def n_particles(cfg: dict, s: int) -> int:
         return 0
     if sp["load"] == NUMBER_WEIGHTED:
         return int(cell_counts(cfg, s).sum())
-    return cfg["grid"]["nx"] * cfg["grid"]["ny"] * sp["ppc_x"] * sp["ppc_y"]
+    x_lo, x_hi, y_lo, y_hi = slab_extent(cfg)
+    return (x_hi - x_lo) * (y_hi - y_lo) * sp["ppc_x"] * sp["ppc_y"]

@@ -133,6 +133,7 @@ size_t layout(pm2d_ctx *c, char *base)
     c->shape_y = cv.take<double>(g.ny);
     c->taper_x = cv.take<double>(g.nx);
     c->stray_total = cv.take<unsigned long long>(1);
+    c->zeros = cv.take<int32_t>(PM2D_ZEROS_BYTES / 4);
     {   // overflow list of the stage kernels: a quarter of the largest species, at least 2^20 entries
         int64_t most = 0;
         for (int s = 0; s < c->nsp; s++) most = std::max<int64_t>(most, species_np(g, c->sp[s].cfg));

@@ -17,6 +17,7 @@ constexpr int CHUNK = 8192;              // max particles per CTA work item (loa
 constexpr int PTHREADS = 256;            // threads per CTA of the chunk kernels
 constexpr int TCELLS = TILE * TILE;      // cells per tile
 constexpr int CPITCH = TCELLS + 1;       // ints per tile in cell_off (last = particles in the tile)
+constexpr int PM2D_ZEROS_BYTES = 64 * 1024;   // a block of zeros in the workspace (>= the deposit windows of k_stage_lanes)
 constexpr int PM2D_LAYERS = 16;          // layered order: ranks >= PM2D_LAYERS form a cell-major tail
 constexpr int TRI_M = 32;                // rows per x-partition of the tridiagonal solve
 // fixed-point tile-relative position: (cell_rel + POS_BIAS) << 24 | frac24
@@ -109,6 +110,7 @@ struct pm2d_ctx {
     int32_t *flags;      // [4] device error flags
     double *shape_y, *taper_x;   // [ny], [nx] relative density tables of the number-weighted loader
     unsigned long long *stray_total; // [1] statistics
+    int32_t *zeros;                  // [PM2D_ZEROS_BYTES / 4] never written: source of the bulk zero fill of the lanes windows
     int64_t *ovf_p;      // [ovf_cap] particles deferred by k_stage (footprint outside the tile window)
     int32_t *ovf_tile, *ovf_count;
     int ovf_cap;

@@ -39,6 +39,12 @@ constexpr int LFP = 48;                     // force-window pitch in float2: a m
 #ifndef LANES_NT_COLD
 #define LANES_NT_COLD 256
 #endif
+#ifndef LANES_MINB_HOT
+#define LANES_MINB_HOT 3
+#endif
+#ifndef LANES_MINB_COLD
+#define LANES_MINB_COLD 3
+#endif
 // Flush of interior windows by cp.reduce.async.bulk (one bulk integer reduction per window row and quantity) instead of
 // one RED per node.  Measured on c3 (r02h): stage kernels 5.16 ms per step against 4.94 with plain REDs -- a CTA has to
 // wait for its bulk reductions to have read shared memory before it may exit, while REDs are fire and forget; off.
@@ -46,6 +52,20 @@ constexpr bool LANES_BULK_FLUSH = false;
 // Where the listed strays are served: by the CTA itself on its shared windows (one particle per thread after the main
 // loop: the whole CTA waits a full particle latency for a handful of strays), or by k_lanes_overflow on the global grids.
 constexpr bool LANES_STRAYS_IN_CTA = true;     // the global route measured 5.19 against 4.85 ms of stage kernels on c3 (r02n)
+// A box load must start on a 16-byte boundary of the global row, i.e. on an even column of float2: with the odd-shift
+// copies as box loads of their own the kernel dies with "an illegal instruction was encountered" (tried, r02p).  The even
+// copies are box loads, the odd ones shifted duplicates made in shared memory.
+// A CTA asks L2 for the particle records and the force window of the CTA that will run LANES_PF_DIST blocks later (about
+// one generation of resident CTAs: 3 per SM), three bulk prefetches and one box prefetch by one thread: r02b had 26 % of the
+// warp samples waiting on the particle loads (long scoreboard) with the records of one round loaded one round ahead.
+#ifndef LANES_PF_DIST
+#define LANES_PF_DIST 444
+#endif
+// The deposit windows are zeroed by one bulk-async copy from a block of zeros in the workspace (L2-resident) instead of
+// STS.128 by the threads: the copy engine's writes do not pass the LSU data pipe, which bounds this kernel.
+#ifndef LANES_TMA_ZERO
+#define LANES_TMA_ZERO 1
+#endif
 constexpr int LSTRAY = 256;                 // stray list of a CTA (a full list spills to the global overflow list)
 constexpr uint32_t LSTRAY_DEP = 0x80000000u;
 constexpr float MAGIC = 12582912.0f;        // 1.5 * 2^23
@@ -74,6 +94,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "r"(parity)
         : "memory");
 }
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 __device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *tm, int c0, int c1, uint64_t *bar)
 {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(smem_u32(dst)),
@@ -91,6 +117,15 @@ __device__ __forceinline__ void bulk_commit_wait_read()
 {
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+// L2 prefetches of the bulk-async family: `bytes` contiguous bytes (16-byte granules) resp. one box of a tensor map
+__device__ __forceinline__ void l2_prefetch_bulk(const void *p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void l2_prefetch_box(const CUtensorMap *tm, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tm), "r"(c0), "r"(c1) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -312,8 +347,8 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
 {
     constexpr int WR = SUBROWS + 2 * HALO + 1, SUBS = TILE / SUBROWS, MLO = NCOPY == 4 ? -1 : 0;
     constexpr int DP = LaneQ<QMASK>::DP, NDEP = NCOPY * WR * DP;
-    // force-window copy ci holds node column c at index c - (ci + MLO - 1) + TS; TS makes copy 0 start on the even column
-    // gy0 - 2: a box load wants 16-byte aligned rows, so the even copies come by TMA and the odd ones are shifted duplicates
+    // force-window copy ci holds node column c at index c - (gy0 + ci + MLO - 1) + TS; TS makes copy 0 start on the even
+    // column gy0 - 2 (box loads start on 16-byte boundaries)
     constexpr int TS = NCOPY == 2 ? 1 : 0, LTS = LT + TS;
     extern __shared__ __align__(128) int32_t lanes_smem[];
     int32_t *dep = lanes_smem;                                             // [NCOPY][WR][DP]
@@ -321,32 +356,86 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
     __shared__ uint32_t slist[LSTRAY];
     __shared__ int scount;
     __shared__ __align__(8) uint64_t fbar;
-    const int tile = blockIdx.x / SUBS, sub = blockIdx.x % SUBS;
+    const int tile = blockIdx.x / SUBS, sub = blockIdx.x % SUBS, lane_ = threadIdx.x & 31;
+    const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
+    const int row0 = sub * SUBROWS - HALO;                                  // tile-relative node row of window row 0
+    // A sub-tile whose window lies inside the grid takes the even copies as box loads of WR rows x LFP columns (bulk-async,
+    // one mbarrier) and derives the odd ones in shared memory; windows that fold at an x wall or wrap in y are copied by
+    // the threads from the global grid.  The deposit windows are zeroed by a bulk copy on the same barrier.  Both depend on
+    // the block index alone and are issued before anything is read from global memory (r02c: 7 % of the warp samples sat
+    // in the wait for them when they followed the loads of the sub-tile's particle range).
+    const bool bulk = STAGE < 2 && gy0 - 2 >= 0 && gy0 + 36 <= P.ny && gx0 + row0 >= 0 && gx0 + row0 + WR - 1 < P.nx;
+    static_assert(NDEP * 4 <= PM2D_ZEROS_BYTES && (NDEP * 4) % 16 == 0, "bulk zero fill");
+    constexpr bool USE_BAR = LANES_TMA_ZERO || STAGE < 2;
+    if (USE_BAR && threadIdx.x == 0 && (LANES_TMA_ZERO || bulk)) {
+        mbar_init(&fbar, 1);
+        mbar_expect_tx(&fbar, (uint32_t)((LANES_TMA_ZERO ? NDEP * 4 : 0) + (bulk ? (NCOPY / 2) * WR * LFP * sizeof(float2) : 0)));
+        if (bulk) {
+#pragma unroll
+            for (int ci = 0; ci < NCOPY; ci += 2) tma_load_2d(Fs + ci * WR * LFP, &tmF, gy0 + ci - 2, gx0 + row0, &fbar);
+        }
+        if (LANES_TMA_ZERO) bulk_load(dep, P.zeros, NDEP * 4, &fbar);
+    }
     const int64_t t0 = P.tile_off[tile], t1 = P.tile_off[tile + 1];
     int64_t s0 = t0, s1 = t1;
     if (SUBS == 2) {
         const int64_t mid = t0 + P.sub0[tile];
         if (sub == 0) s1 = mid; else s0 = mid;
     }
-    if (s1 == s0) return;
-    const int gx0 = (tile / P.nty) * TILE, gy0 = (tile % P.nty) * TILE;
-    const int row0 = sub * SUBROWS - HALO;                                  // tile-relative node row of window row 0
+    if (LANES_PF_DIST > 0 && threadIdx.x == NT - 32) {
+        auto prefetch_block = [&](int b) {
+            if (b >= (int)gridDim.x) return;
+            const int tl = b / SUBS, sb = b % SUBS;
+            int64_t a0 = P.tile_off[tl], a1 = P.tile_off[tl + 1];
+            if (SUBS == 2) {
+                const int64_t mid = a0 + P.sub0[tl];
+                if (sb == 0) a1 = mid; else a0 = mid;
+            }
+            if (a1 <= a0) return;
+            l2_prefetch_bulk(P.pv + a0, (uint32_t)(a1 - a0) * 16u);
+            const int64_t wl = a0 & ~(int64_t)3;                               // 16-byte granules; a short tail is left out
+            l2_prefetch_bulk(P.w + wl, ((uint32_t)(a1 - wl) * 4u) & ~15u);
+            if (STAGE == 1) {
+                const int64_t ul = a0 & ~(int64_t)1;
+                l2_prefetch_bulk(P.uh + ul, ((uint32_t)(a1 - ul) * 8u) & ~15u);
+            }
+            if (STAGE < 2) {
+                const int bx0 = (tl / P.nty) * TILE + sb * SUBROWS - HALO, by0 = (tl % P.nty) * TILE;
+                if (by0 - 2 >= 0 && by0 + 36 <= P.ny && bx0 >= 0 && bx0 + WR - 1 < P.nx) {
+#pragma unroll
+                    for (int ci = 0; ci < NCOPY; ci += 2) l2_prefetch_box(&tmF, by0 + ci - 2, bx0);
+                }
+            }
+        };
+        prefetch_block((int)blockIdx.x + LANES_PF_DIST);
+        if ((int)blockIdx.x < LANES_PF_DIST) prefetch_block((int)blockIdx.x);
+    }
+    if (s1 == s0) {          // nothing to do, but the bulk copies write this CTA's shared memory: wait them out
+        if (USE_BAR && threadIdx.x == 0 && (LANES_TMA_ZERO || bulk)) mbar_wait(&fbar, 0);
+        return;
+    }
+    // the records of the first two rounds are asked for before the windows are set up
+    PV *const pvs = P.pv + s0;
+    const float *const ws = P.w + s0;
+    float2 *const uhs = P.uh + s0;
+    const int np_sub = (int)(s1 - s0);
+    auto load = [&](int i, PV &me, float &w, float2 &uh) {
+        if (i < np_sub) {
+            me = pvs[i];
+            w = ws[i];
+            if (STAGE == 1) uh = uhs[i];
+        }
+    };
+    PV me0 = PV{0u, 0u, 0.f, 0.f}, me1 = me0;
+    float w0 = 0.f, w1 = 0.f;
+    float2 uh0 = make_float2(0.f, 0.f), uh1 = uh0;
+    load((int)threadIdx.x, me0, w0, uh0);
+    load((int)threadIdx.x + NT, me1, w1, uh1);
     // momentum windows count in units of 2^sp global units (from the tile's largest weight, k_lanesort)
     const int sp = P.lane_exp[tile];
     const float pst = P.pscale * pow2i(-sp);
 
-    // A sub-tile whose window lies inside the grid takes the even copies as box loads of WR rows x LFP columns (bulk-async,
-    // one mbarrier) and derives the odd ones in shared memory; windows that fold at an x wall or wrap in y are copied by
-    // the threads from the global grid.
-    const bool bulk = STAGE < 2 && gy0 - 2 >= 0 && gy0 + 36 <= P.ny && gx0 + row0 >= 0 && gx0 + row0 + WR - 1 < P.nx;
-    if (STAGE < 2 && bulk) {
-        if (threadIdx.x == 0) {
-            mbar_init(&fbar, 1);
-            mbar_expect_tx(&fbar, (uint32_t)((NCOPY / 2) * WR * LFP * sizeof(float2)));
-#pragma unroll
-            for (int ci = 0; ci < NCOPY; ci += 2) tma_load_2d(Fs + ci * WR * LFP, &tmF, gy0 + ci - 2, gx0 + row0, &fbar);
-        }
-    } else if (STAGE < 2) {
+    if (STAGE < 2 && !bulk) {
         constexpr int NE = NCOPY * WR * LTS, IT = (NE + NT - 1) / NT;
         float2 v[IT];
 #pragma unroll
@@ -364,58 +453,49 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
             if (e < NE) Fs[(ci * WR + r) * LFP + t] = v[k];
         }
     }
-    {
+    if (!LANES_TMA_ZERO) {
         int4 *d4 = reinterpret_cast<int4 *>(dep);
         for (int e = threadIdx.x; e < NDEP / 4; e += NT) d4[e] = make_int4(0, 0, 0, 0);
     }
     if (threadIdx.x == 0) scount = 0;
     __syncthreads();
+    if (LANES_TMA_ZERO && !(STAGE < 2 && bulk)) mbar_wait(&fbar, 0);
     if (STAGE < 2 && bulk) {
         mbar_wait(&fbar, 0);
-        constexpr int NE = (NCOPY / 2) * WR * LTS;
-        for (int e = threadIdx.x; e < NE; e += NT) {        // odd copy ci = even copy ci - 1 moved by one column
-            const int h = e / (WR * LTS), rem = e - h * (WR * LTS), r = rem / LTS, t = rem - r * LTS;
-            Fs[((2 * h + 1) * WR + r) * LFP + t] = Fs[(2 * h * WR + r) * LFP + t + 1];
+        // odd copy ci = even copy ci - 1 moved by one column: a warp takes a window row at a time (lane = column), the
+        // LTS - 32 columns beyond ride on the first lanes
+        for (int rr = threadIdx.x >> 5; rr < (NCOPY / 2) * WR; rr += NT / 32) {
+            const int h = rr / WR, r = rr - h * WR;                       // warp-uniform
+            const float2 *src = Fs + (2 * h * WR + r) * LFP + 1;
+            float2 *dst = Fs + ((2 * h + 1) * WR + r) * LFP;
+            const float2 v0 = src[lane_], v1 = lane_ < LTS - 32 ? src[32 + lane_] : make_float2(0.f, 0.f);
+            dst[lane_] = v0;
+            if (lane_ < LTS - 32) dst[32 + lane_] = v1;
         }
         __syncthreads();
     }
 
     const int lane = threadIdx.x & 31;
     constexpr float GS = LaneW<SHAPE>::inv2;
-    const float dtg = (STAGE == 1 ? 0.5f : 1.f) * GS * P.dt;
-    const float qns = P.nscale * GS, qps = pst * GS;
+    // launch constants that only scale by powers of two come ready from the host (lane_dt = GS dt, lane_qns = GS nscale):
+    // the kernel runs at 56 registers and re-derived them every round of the loop
+    const float dtg = STAGE == 1 ? P.lane_dt_half : P.lane_dt;
+    const float qns = P.lane_qns, qps = pst * GS;
     const bool wall_tile = gx0 == 0 || gx0 + TILE >= P.nx;             // only these tiles can see a particle cross a wall
     const int rofs = POS_BIAS + 1 + row0, cofs = POS_BIAS + lane + MLO;
-    PV *const pvs = P.pv + s0;
-    const float *const ws = P.w + s0;
-    float2 *const uhs = P.uh + s0;
-    const int np_sub = (int)(s1 - s0);
-    // the record of the next round is loaded before this round's arithmetic starts (24 resident warps do not hide DRAM)
-    PV nme = PV{0u, 0u, 0.f, 0.f};
-    float nw = 0.f;
-    float2 nuh = make_float2(0.f, 0.f);
-    if ((int)threadIdx.x < np_sub) {
-        nme = pvs[threadIdx.x];
-        nw = ws[threadIdx.x];
-        if (STAGE == 1) nuh = uhs[threadIdx.x];
-    }
-    for (int i = threadIdx.x; i < np_sub; i += NT) {
-        PV me = nme;
-        const float w = nw;
-        const float2 uh = nuh;
-        if (i + NT < np_sub) {
-            nme = pvs[i + NT];
-            nw = ws[i + NT];
-            if (STAGE == 1) nuh = uhs[i + NT];
-        }
+    // advance() with the factor 2^24 folded into h on the host (a power of two: the same bits)
+    const float hx24 = P.hx24, hy24 = P.hy24;
+    auto adv24 = [](uint32_t f, float h24, float usum) { return f + (uint32_t)__float2int_rn(__fmul_rn(h24, usum)); };
+    // one particle: gather, push, deposit (or hand it to the stray list)
+    auto particle = [&](PV me, const float w, const float2 uh, const int i) {
         float ux = me.ux, uy = me.uy;
         uint32_t xd = me.x, yd = me.y;
         float Wx[3], Wy[3];
         if (STAGE < 2) {
             uint32_t xg = me.x, yg = me.y;
             if (STAGE == 1) {
-                xg = advance(me.x, P.hx, __fadd_rn(uh.x, ux));
-                yg = advance(me.y, P.hy, __fadd_rn(uh.y, uy));
+                xg = adv24(me.x, hx24, __fadd_rn(uh.x, ux));
+                yg = adv24(me.y, hy24, __fadd_rn(uh.y, uy));
             }
             int cxb, cyb, dix, diy;
             lane_decode(xg, cxb, dix);
@@ -425,7 +505,7 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
                 const int slot = atomicAdd(&scount, 1);
                 if (slot < LSTRAY) slist[slot] = (uint32_t)i;
                 else push_overflow(P, s0 + i, tile, false);
-                continue;
+                return;
             }
             lane_weights_xy<SHAPE>(dix, diy, P, Wx, Wy);
             const float2 *fw = Fs + (ci * WR + rb) * LFP + lane + TS;
@@ -445,15 +525,15 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
             if (STAGE == 0) {
                 const float uhx = __fmaf_rn(dtg, fx, ux), uhy = __fmaf_rn(dtg, fy, uy);             // Eq. 17
                 uhs[i] = make_float2(uhx, uhy);
-                xd = advance(me.x, P.hx, __fadd_rn(uhx, ux));
-                yd = advance(me.y, P.hy, __fadd_rn(uhy, uy));
+                xd = adv24(me.x, hx24, __fadd_rn(uhx, ux));
+                yd = adv24(me.y, hy24, __fadd_rn(uhy, uy));
                 ux = uhx;
                 uy = uhy;
             } else {
                 float unx = __fmaf_rn(dtg, fx, 0.5f * __fadd_rn(uh.x, ux));                         // Eq. 19
                 const float uny = __fmaf_rn(dtg, fy, 0.5f * __fadd_rn(uh.y, uy));
-                xd = advance(me.x, P.hx, __fadd_rn(unx, ux));
-                yd = advance(me.y, P.hy, __fadd_rn(uny, uy));
+                xd = adv24(me.x, hx24, __fadd_rn(unx, ux));
+                yd = adv24(me.y, hy24, __fadd_rn(uny, uy));
                 if (wall_tile) reflect_x(xd, unx, gx0, P.nx);
                 me.x = xd; me.y = yd; me.ux = unx; me.uy = uny;
                 pvs[i] = me;
@@ -470,7 +550,7 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
             const int slot = atomicAdd(&scount, 1);
             if (slot < LSTRAY) slist[slot] = (uint32_t)i | LSTRAY_DEP;
             else push_overflow(P, s0 + i, tile, true);
-            continue;
+            return;
         }
         lane_weights_xy<SHAPE>(dix, diy, P, Wx, Wy);
         const float qn = w * qns, qp = w * qps, qx = qp * ux, qy = qp * uy;
@@ -490,6 +570,15 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
                 }
             }
         }
+    };
+    // Two particles per round of the loop; a register set is refilled with the record of the round after next as soon as
+    // its particle is done (36 resident warps do not hide the loads), the two sets swap roles instead of being copied.
+    for (int i = threadIdx.x; i < np_sub; i += 2 * NT) {
+        particle(me0, w0, uh0, i);
+        if (i + NT >= np_sub) break;
+        load(i + 2 * NT, me0, w0, uh0);
+        particle(me1, w1, uh1, i + NT);
+        load(i + 3 * NT, me1, w1, uh1);
     }
     __syncthreads();
     {   // strays
@@ -562,9 +651,9 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
         return;
     }
     // one global integer reduction per touched node; wall columns hold half a control volume and count twice (Q9); rows
-    // beyond a wall fold back
-    for (int e = threadIdx.x; e < WR * NCOL; e += NT) {
-        const int r = e / NCOL, z = e - r * NCOL;
+    // beyond a wall fold back.  A warp takes a window row at a time (lane = z < 32: no index arithmetic per node, the row's
+    // fold, wall factor and base address are warp-uniform); the NCOL - 32 columns beyond are spread over the CTA afterwards.
+    auto flush_node = [&](int r, int z) {
         int v = 0, vx = 0, vy = 0;
 #pragma unroll
         for (int ci = 0; ci < NCOPY; ci++) {
@@ -578,21 +667,24 @@ __global__ void __launch_bounds__(NT, MINB) k_stage_lanes(const PartParams P, co
                 }
             }
         }
-        if ((v | vx | vy) == 0) continue;
+        if ((v | vx | vy) == 0) return;
         const int gi = fold_x(gx0 + row0 + r, P.nx);
         const int gj = (gy0 + z + MLO - 1) & (P.ny - 1);
-        const int fac = (gi == 0 || gi == P.nx) ? 2 : 1;
+        const int wall = (gi == 0 || gi == P.nx) ? 1 : 0;
         const size_t k = (size_t)gi * P.ny + gj;
         // the integer sums wrap: report it instead of handing wrapped moments to the solvers.  Density (all terms of one
         // sign): one window alone beyond half the int32 range, n > n_cap / 2 = 4 n_max of the profile.  Momentum (terms of
         // either sign, a hot species reaches a large fraction of the range by noise alone): this window's sum itself is
         // outside int32, |n u| > n_cap / 16 = n_max / 2
-        const int64_t wide_x = (int64_t)(fac * mp) * vx, wide_y = (int64_t)(fac * mp) * vy;
-        if (abs(v) > (1 << 30) / fac || wide_x != (int32_t)wide_x || wide_y != (int32_t)wide_y) P.flags[3] = 2;
-        if (v) atomicAdd(&P.nfix[k], fac * v);
-        if (vx) atomicAdd(&P.pxfix[k], fac * mp * vx);
-        if (vy) atomicAdd(&P.pyfix[k], fac * mp * vy);
-    }
+        if (abs(v) > ((1 << 30) >> wall) || max(abs(vx), abs(vy)) > (0x7fffffff >> (sp + wall))) P.flags[3] = 2;
+        const int mpw = 1 << (sp + wall);
+        if (v) atomicAdd(&P.nfix[k], v * (1 + wall));
+        if (vx) atomicAdd(&P.pxfix[k], vx * mpw);
+        if (vy) atomicAdd(&P.pyfix[k], vy * mpw);
+    };
+    for (int r = threadIdx.x >> 5; r < WR; r += NT / 32) flush_node(r, lane);
+    constexpr int NTAIL = NCOL - 32;
+    for (int e = threadIdx.x; e < WR * NTAIL; e += NT) flush_node(e / NTAIL, 32 + e % NTAIL);
 }
 
 // the deferred particles of k_stage_lanes: same arithmetic, gather from the global force grid, deposit on the global grids
@@ -975,8 +1067,8 @@ static int launch_lanes_variant(const PartParams &P, const CUtensorMap &tm, int 
         }                                                                                                                    \
         kern<<<ntiles * (TILE / SUBROWS), NT, bytes, st>>>(P, tm);                                                           \
     } while (0)
-    if (hot) PM2D_LANES_LAUNCH(4, 16, LANES_NT_HOT, 3);
-    else PM2D_LANES_LAUNCH(2, 32, LANES_NT_COLD, 3);     // half tiles for the cold species: 4.83 instead of 4.74 ms on c3 (r02j)
+    if (hot) PM2D_LANES_LAUNCH(4, 16, LANES_NT_HOT, LANES_MINB_HOT);
+    else PM2D_LANES_LAUNCH(2, 32, LANES_NT_COLD, LANES_MINB_COLD);     // half tiles for the cold species: 4.83 instead of 4.74 ms on c3 (r02j)
 #undef PM2D_LANES_LAUNCH
     k_lanes_overflow<SHAPE, STAGE, QMASK><<<148 * 8, 128, 0, st>>>(P);
     return PM2D_OK;

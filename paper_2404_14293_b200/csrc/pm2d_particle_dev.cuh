@@ -16,6 +16,7 @@ struct PartParams {
     int32_t *nfix, *pxfix, *pyfix;
     int32_t *flags;
     unsigned long long *stray_total;   // statistics: particles served outside the register patch
+    const int32_t *zeros;              // PM2D_ZEROS_BYTES of zeros (bulk zero fill of the lanes windows)
     int64_t *ovf_p;           // overflow list: particles whose gather footprint left the tile window
     int32_t *ovf_tile, *ovf_count;
     int ovf_cap;
@@ -34,6 +35,12 @@ struct PartParams {
     const int32_t *sub0;     // [ntiles] particles of sub-tile 0
     const int32_t *lane_exp; // [ntiles] sn | sp << 8
     float ucap;              // |u| beyond this takes the exact (F2I) path
+    // constants of k_stage_lanes that differ from the above by powers of two only (exact on the host): GS = 1/4 for the
+    // sine cloud (the 1/2 of each axis' G = (1 - cos)/2), 1 otherwise
+    float hx24, hy24;        // hx 2^24, hy 2^24: displacement in units of 2^-24 cell per unit (u' + u)
+    float lane_dt;           // GS dt
+    float lane_dt_half;      // GS dt / 2
+    float lane_qns;          // GS nscale
 };
 
 // host side: fill the parameters of species s (pm2d_particles.cu)

@@ -1376,6 +1376,7 @@ PartParams make_part_params(pm2d_ctx *c, int s)
     P.F = S.F;
     P.nfix = S.nfix; P.pxfix = S.pxfix; P.pyfix = S.pyfix; P.flags = c->flags;
     P.stray_total = c->stray_total;
+    P.zeros = c->zeros;
     P.ovf_p = c->ovf_p; P.ovf_tile = c->ovf_tile; P.ovf_count = c->ovf_count; P.ovf_cap = c->ovf_cap;
     P.nx = c->g.nx; P.ny = c->g.ny; P.nty = c->nty;
     P.dt = (float)c->dtp;                                   // particle step: S wave steps (Q21)
@@ -1393,6 +1394,12 @@ PartParams make_part_params(pm2d_ctx *c, int s)
     P.sub0 = S.sub0;
     P.lane_exp = S.lane_exp;
     P.ucap = (float)lane_ucap(S);
+    const float gs = S.cfg.shape == PM2D_SINE ? 0.25f : 1.f;
+    P.hx24 = P.hx * 16777216.0f;
+    P.hy24 = P.hy * 16777216.0f;
+    P.lane_dt = gs * P.dt;
+    P.lane_dt_half = 0.5f * gs * P.dt;
+    P.lane_qns = gs * P.nscale;
     return P;
 }
 
