@@ -112,8 +112,9 @@ def workload_name(name, full_cfg, nmob=None):
     if nmob is None:                      # the CPU arm: counted by the oracle's loader
         import oracle.loader as L
         nmob = sum(L.n_particles(full_cfg, s) for s, sp in enumerate(full_cfg["species"]) if sp["mobile"])
-    src = (f"(BASELINE.json configs[{int(name[1]) - 1}])" if name != "cbet" else
-           "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps)")
+    src = (f"(BASELINE.json configs[{int(name[1]) - 1}])" if not name.startswith("cbet") else
+           "(SURVEY 8f.1: the paper's CBET set-up P:L380, two beams at +-15 deg, particle step = 5 wave steps"
+           + (", true vacuum margins P:L81)" if name == "cbet_vac" else ")"))
     return f"{name}: {g['nx']}x{g['ny']} cells, {nmob} mobile particles per GPU {src}"
 
 
@@ -273,7 +274,7 @@ def main():
     ap.add_argument("--steps", type=int, default=96,
                     help="timed steps; the default spans six rebin periods of c3 (0.7 s: several clock samples, the rebin at its long-run share)")
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "cbet"])
+    ap.add_argument("--config", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "cbet", "cbet_vac"])
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--eager", type=int, default=1, help="1: deposit n, Px, Py at both stages (paper's flow); 0: n only")
     ap.add_argument("--rebin-every", type=int, default=None)

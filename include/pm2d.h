@@ -144,6 +144,13 @@ typedef struct {
                               margins at PM2D_TAPER_FLOOR of the profile instead of vacuum (Q20).  Weights only: not
                               with PM2D_NUMBER_WEIGHTED                                               */
     int32_t pad_;
+    int32_t slab[4];       /* x_lo, x_hi, y_lo, y_hi in cells; all zero = the whole box.  Only cells with x_lo <= i < x_hi and
+                              y_lo <= j < y_hi hold particles: "a plasma slab is set at the center of the simulation box, and
+                              the vacuum space is usually set around the plasma slab ... allowing the plasma expanding"
+                              (P:L81).  The loaded cells get the ids, offsets, momenta and weights they have without the slab
+                              (the profile still spans the box; use taper_cells = 0 for a hard edge).  The margins are true
+                              vacuum: no particles, Q10 keeps the pressure term out where n = 0.  Not with
+                              PM2D_NUMBER_WEIGHTED.  EINVAL unless 0 <= lo < hi <= nx resp. ny                       */
 } pm2d_profile;
 
 typedef struct {

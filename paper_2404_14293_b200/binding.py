@@ -40,7 +40,8 @@ class Species(C.Structure):
 
 
 class Profile(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("taper_cells", C.c_int32), ("p", C.c_double * 4), ("taper_cells_y", C.c_int32), ("pad_", C.c_int32)]
+    _fields_ = [("kind", C.c_int32), ("taper_cells", C.c_int32), ("p", C.c_double * 4), ("taper_cells_y", C.c_int32), ("pad_", C.c_int32),
+                ("slab", C.c_int32 * 4)]
 
 
 class Laser(C.Structure):
@@ -170,7 +171,8 @@ def make_structs(cfg: dict, eager_moments=1, track_ids=0, rebin_every=None, part
         sp[k] = Species(s["mass"], s["T_keV"], s["pressure_coeff"], s["DD"], s["sign"], s["shape"], s["mobile"], s["load"],
                         s.get("ppc_x", 0), s.get("ppc_y", 0), int(s.get("capacity", 0)))
     p = cfg["profile"]
-    prof = Profile(p["kind"], p.get("taper_cells", 0), (C.c_double * 4)(*[float(v) for v in p["p"]]), int(p.get("taper_cells_y", 0)), 0)
+    prof = Profile(p["kind"], p.get("taper_cells", 0), (C.c_double * 4)(*[float(v) for v in p["p"]]), int(p.get("taper_cells_y", 0)), 0,
+                   (C.c_int32 * 4)(*[int(v) for v in (p.get("slab") or (0, 0, 0, 0))]))
     las = (Laser * max(len(cfg["lasers"]), 1))()
     for k, l in enumerate(cfg["lasers"]):
         las[k] = Laser(l["a0"], l["omega"], l["y0"], l["w0"], l["t_rise"], l.get("alpha", 0.0), l["comp"], 0)

@@ -327,6 +327,13 @@ extern "C" int pm2d_init(const pm2d_grid *grid, const pm2d_species *species, int
     if (profile->taper_cells_y > 0)
         for (int s = 0; s < nsp; s++)
             if (species[s].load == PM2D_NUMBER_WEIGHTED) return fail(PM2D_EINVAL, "taper_cells_y is not available with PM2D_NUMBER_WEIGHTED");
+    if (profile->slab[0] | profile->slab[1] | profile->slab[2] | profile->slab[3]) {
+        const int32_t *b = profile->slab;
+        if (b[0] < 0 || b[0] >= b[1] || b[1] > grid->nx || b[2] < 0 || b[2] >= b[3] || b[3] > grid->ny)
+            return fail(PM2D_EINVAL, "profile slab must satisfy 0 <= x_lo < x_hi <= nx and 0 <= y_lo < y_hi <= ny");
+        for (int s = 0; s < nsp; s++)
+            if (species[s].load == PM2D_NUMBER_WEIGHTED) return fail(PM2D_EINVAL, "a slab extent is not available with PM2D_NUMBER_WEIGHTED");
+    }
     double nmax;
     if (profile->kind == PM2D_PROFILE_UNIFORM) nmax = profile->p[0];
     else if (profile->kind == PM2D_PROFILE_LINEAR) nmax = std::max(profile->p[0], profile->p[1]);

@@ -658,7 +658,23 @@ struct LoadParams {
     double p0, p1, p2;
     const int32_t *cell_off;     // NUMBER_WEIGHTED: the tile's cell runs give (cell, k) of a slot
     int layered;                 // storage order inside a tile: (rank in cell, cell) instead of (cell, rank)
+    int sx0, sx1, sy0, sy1;      // pm2d_profile.slab resolved: cells with sx0 <= i < sx1, sy0 <= j < sy1 are loaded
 };
+
+// the loaded cells of a tile: rows [ri0, ri1) x columns [rj0, rj1), tile-relative (empty: ri1 <= ri0 or rj1 <= rj0)
+struct TileRect {
+    int ri0, ri1, rj0, rj1;
+    __host__ __device__ int rows() const { return ri1 > ri0 ? ri1 - ri0 : 0; }
+    __host__ __device__ int cols() const { return rj1 > rj0 ? rj1 - rj0 : 0; }
+};
+__host__ __device__ inline TileRect tile_rect(int gx0, int gy0, int nx, int ny, int sx0, int sx1, int sy0, int sy1)
+{
+    const int wx = min(TILE, nx - gx0), wy = min(TILE, ny - gy0);
+    TileRect r;
+    r.ri0 = min(max(sx0 - gx0, 0), wx); r.ri1 = min(max(sx1 - gx0, 0), wx);
+    r.rj0 = min(max(sy0 - gy0, 0), wy); r.rj1 = min(max(sy1 - gy0, 0), wy);
+    return r;
+}
 
 __device__ double profile_density(const LoadParams &L, int i)
 {
@@ -701,7 +717,8 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
     int64_t end = beg + CHUNK;
     if (L.tile_off[tile + 1] < end) end = L.tile_off[tile + 1];
     const int gx0 = (tile / L.nty) * TILE, gy0 = (tile % L.nty) * TILE;
-    const int wy = min(TILE, L.ny - gy0);
+    const TileRect tr = tile_rect(gx0, gy0, L.nx, L.ny, L.sx0, L.sx1, L.sy0, L.sy1);
+    const int wy = max(tr.cols(), 1);                  // loaded columns per row of this tile
     const int ppc = L.ppc_x * L.ppc_y;
     for (int64_t p = beg + threadIdx.x; p < end; p += PTHREADS) {
         int s = (int)(p - t0);
@@ -715,14 +732,16 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
             }
             li = lo >> 5; lj = lo & 31; k = s - co[lo];
         } else if (L.layered) {                    // layer-major: the k-th particles of all cells are contiguous
-            const int cells = min(TILE, L.nx - gx0) * wy;
+            const int cells = tr.rows() * wy;
             k = s / cells;
             int lc = s - k * cells;
             li = lc / wy; lj = lc - li * wy;
+            li += tr.ri0; lj += tr.rj0;
         } else {
             int lc = s / ppc;
             k = s - lc * ppc;
             li = lc / wy; lj = lc - li * wy;
+            li += tr.ri0; lj += tr.rj0;
         }
         int64_t cell = (int64_t)(gx0 + li) * L.ny + (gy0 + lj);
         int64_t pid = (int64_t)k * ((int64_t)L.nx * L.ny) + cell;
@@ -752,17 +771,19 @@ __global__ void __launch_bounds__(PTHREADS) k_load(const LoadParams L)
     }
 }
 
-// cell offsets of the loader's order: ppc particles in every cell that exists
-__global__ void k_uniform_cell_off(int32_t *cell_off, int ntiles, int nty, int nx, int ny, int ppc)
+// cell offsets of the loader's order: ppc particles in every cell of the slab (the whole box without one)
+__global__ void k_uniform_cell_off(int32_t *cell_off, int ntiles, int nty, int nx, int ny, int ppc, int sx0, int sx1, int sy0, int sy1)
 {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= (int64_t)ntiles * CPITCH) return;
     const int t = (int)(e / CPITCH), c = (int)(e - (int64_t)t * CPITCH);
     const int gx0 = (t / nty) * TILE, gy0 = (t % nty) * TILE;
-    const int wx = min(TILE, nx - gx0), wy = min(TILE, ny - gy0);
+    const TileRect tr = tile_rect(gx0, gy0, nx, ny, sx0, sx1, sy0, sy1);
     const int li = c >> 5, lj = c & 31;                 // c == TCELLS: li = 32
-    const int before = li < wx ? li * wy + min(lj, wy) : wx * wy;
-    cell_off[e] = ppc * before;
+    // loaded cells before (li, lj) in row-major order
+    const int full = min(max(li - tr.ri0, 0), tr.rows());
+    const int part = (li >= tr.ri0 && li < tr.ri1) ? min(max(lj - tr.rj0, 0), tr.cols()) : 0;
+    cell_off[e] = ppc * (full * tr.cols() + part);
 }
 
 // NUMBER_WEIGHTED: particles per cell = floor(ppc * taper(i) * filament(j) + U), U a Philox uniform of the cell
@@ -885,12 +906,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_build_chunks(const int64_t *ti
     }
 }
 
-__global__ void k_uniform_tile_counts(int32_t *cnt, int ntx, int nty, int nx, int ny, int ppc)
+__global__ void k_uniform_tile_counts(int32_t *cnt, int ntx, int nty, int nx, int ny, int ppc, int sx0, int sx1, int sy0, int sy1)
 {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntx * nty) return;
     int gx0 = (t / nty) * TILE, gy0 = (t % nty) * TILE;
-    cnt[t] = ppc * min(TILE, nx - gx0) * min(TILE, ny - gy0);
+    const TileRect tr = tile_rect(gx0, gy0, nx, ny, sx0, sx1, sy0, sy1);
+    cnt[t] = ppc * tr.rows() * tr.cols();
 }
 
 // ---- rebin, pass 1: stable move between neighbouring tiles ------------------------------------------
@@ -1517,6 +1539,9 @@ int launch_load_particles(pm2d_ctx *c, int s)
 {
     SpeciesDev &S = c->sp[s];
     const int ppc = S.cfg.ppc_x * S.cfg.ppc_y;
+    const int32_t *sl = c->profile.slab;
+    const bool whole = !(sl[0] | sl[1] | sl[2] | sl[3]);
+    const int sx0 = whole ? 0 : sl[0], sx1 = whole ? c->g.nx : sl[1], sy0 = whole ? 0 : sl[2], sy1 = whole ? c->g.ny : sl[3];
     if (S.cfg.load == PM2D_NUMBER_WEIGHTED) {
         k_weighted_cell_off<<<c->ntiles, 256, 0, c->stream>>>(S.cell_off, S.tile_cnt, c->shape_y, c->taper_x, c->nty, c->g.nx, c->g.ny,
                                                               (double)ppc, s, (uint32_t)(c->seed & 0xFFFFFFFFu), (uint32_t)(c->seed >> 32));
@@ -1531,11 +1556,13 @@ int launch_load_particles(pm2d_ctx *c, int s)
         }
         S.np = total;
     } else {
-        k_uniform_tile_counts<<<(c->ntiles + 255) / 256, 256, 0, c->stream>>>(S.tile_cnt, c->ntx, c->nty, c->g.nx, c->g.ny, ppc);
+        k_uniform_tile_counts<<<(c->ntiles + 255) / 256, 256, 0, c->stream>>>(S.tile_cnt, c->ntx, c->nty, c->g.nx, c->g.ny, ppc, sx0, sx1, sy0, sy1);
         k_scan_tiles<<<1, SCAN_THREADS, 0, c->stream>>>(S.tile_cnt, c->ntiles, S.tile_off);
         const int64_t ncell = (int64_t)c->ntiles * CPITCH;
-        k_uniform_cell_off<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>(S.cell_off, c->ntiles, c->nty, c->g.nx, c->g.ny, ppc);
+        k_uniform_cell_off<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>(S.cell_off, c->ntiles, c->nty, c->g.nx, c->g.ny, ppc, sx0, sx1,
+                                                                                   sy0, sy1);
         count_launch(c, 3);
+        S.np = (int64_t)(sx1 - sx0) * (sy1 - sy0) * ppc;          // the slab's cells; capacity stays that of the whole box
     }
     int rc = launch_build_chunks(c, s);
     if (rc) return rc;
@@ -1550,6 +1577,7 @@ int launch_load_particles(pm2d_ctx *c, int s)
     L.p0 = c->profile.p[0]; L.p1 = c->profile.p[1]; L.p2 = c->profile.p[2];
     L.cell_off = S.cell_off;
     L.layered = S.layered ? 1 : 0;
+    L.sx0 = sx0; L.sx1 = sx1; L.sy0 = sy0; L.sy1 = sy1;
     k_load<<<S.max_chunks, PTHREADS, 0, c->stream>>>(L);
     count_launch(c);
     PM2D_CUDA_CHECK(cudaGetLastError());

@@ -71,7 +71,7 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
         c["species"] = [_species(-1, 1.0, 5.0, 10, 6, SINE, 1.9, load=NUMBER_WEIGHTED),
                         _species(+1, 1836.0, 0.0, 0, 0, SINE, 1.9, mobile=0, load=LOAD_NONE)]
         c["lasers"] = [_laser(0.01)]
-    elif name == "cbet":  # S§8(f).1, the paper's CBET run: 8000x8000 there, 8192x8192 here (ny a power of two);
+    elif name in ("cbet", "cbet_vac"):  # S§8(f).1, the paper's CBET run: 8000x8000 there, 8192x8192 here (ny a power of two);
         # 0.4 n_c hydrogen slab (the standard edge taper stands in for the 20 lambda0 vacuum margins), 1 e + 1 ion per
         # cell, 1 keV / 200 eV, DD = 1.85 dx, two beams a0 = 0.008 at +-15 degrees, lambda0 and 0.9995 lambda0, centres
         # -+50 lambda0 from the axis, w0 = 30 lambda0, particle step = 5 wave steps, absorbing y walls for a
@@ -95,6 +95,12 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     c["profile"]["taper_cells"] = g["nx"] // 16          # Q9
     if name == "cbet":                                    # the paper's slab has margins on all four sides
         c["profile"]["taper_cells_y"] = g["ny"] // 16
+    if name == "cbet_vac":                                # S§8(f).2: the same slab with TRUE vacuum margins (a
+        # 360 x 360 lambda slab in the centre of a 400 x 400 lambda box = margins of a twentieth of the box on every
+        # side), hard-edged: no particles outside, no taper by weight (Q20)
+        c["profile"]["taper_cells"] = 0
+        mx, my = max(g["nx"] // 20, 1), max(g["ny"] // 20, 1)
+        c["profile"]["slab"] = [mx, g["nx"] - mx, my, g["ny"] - my]
     if name == "c5":                                      # sigma = ny/64 cells, amplitude A such that peak = 20 x mean
         sig = g["ny"] / 64.0
         c["profile"]["p"][2] = sig
@@ -102,7 +108,7 @@ def config(name: str, nx: int | None = None, ny: int | None = None) -> dict:
     for sp in c["species"]:
         if sp["load"] == NUMBER_WEIGHTED:                 # slots: an upper bound of the dithered counts
             sp["capacity"] = g["nx"] * g["ny"] * sp["ppc_x"] * sp["ppc_y"] + 4096
-    if name in ("c4", "cbet"):
+    if name in ("c4", "cbet", "cbet_vac"):
         Ly = g["ny"] * g["dy"]
         for las in c["lasers"]:
             las["w0"] *= Ly

@@ -1169,3 +1169,74 @@ def test_strip_kernel_split_tiles_parity(P):
     assert np.abs(got["ux"][o] - orc.sp[0]["ux"]).max() < 2e-6
     assert np.abs(got["ix"][o] + got["fx"][o].astype(np.float64) - orc.sp[0]["X"]).max() < 1e-4
     sim.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("order", [0, 1, 2, 4], ids=["auto", "cellmajor", "layered", "lanes"])
+def test_vacuum_margin_slab_parity_and_expansion(P, order):
+    """S§8f.2, P:L81 / P:L380: the paper's slab "at the center of the simulation box" with TRUE vacuum around it
+    (pm2d_profile.slab; pm2d_inputs "cbet_vac": margins of a twentieth of the box on every side, hard-edged, no particles
+    outside) on a reduced copy of the CBET set-up, with all four stage kernels.
+
+    - The device loader fills exactly the slab's cells with the oracle loader's particles, bit for bit; the margins hold
+      exact zeros.
+    - Fields and deposits agree with the oracle at BASELINE.json's 1e-5 for the first two particle steps (10 wave steps).
+      From the third step on the ELECTRON quantities agree to 1e-4 (n), 5e-4 (n u) and the electron phase space after 10
+      steps to 2e-3 / 2e-2 instead: the pressure term of Eq. 16, -C v_th^2 grad(n) / n, is evaluated at nodes that only
+      the tail of a cloud reaches (n = 1e-4 .. 1e-6 of the slab's), where the 5e-7 absolute error of a float32 weight is a
+      per-cent error of n, and the edge electrons it accelerates carry that into n u (all four kernels give the same
+      numbers: measured 2.9e-5, 1.2e-4, 3e-4 / 2.5e-3).  The ions, which feel the edge only through
+      E, stay at 1e-5 in n and position.
+    - Over 200 particle steps (1000 wave steps) both sides keep their particle counts and the device its total charge, the
+      electrons have spread through the margin to the wall on both sides ("allowing the plasma expanding"), and the
+      width of the electron cloud agrees to 2 % (a property: float32 and float64 runs of this set-up drift apart, 6.5)."""
+    cfg = small_cfg("cbet_vac", 80, 64)
+    for las in cfg["lasers"]:
+        las["t_rise"] = 0.3
+    x_lo, x_hi, y_lo, y_hi = cfg["profile"]["slab"]
+    sim = P.PM2D(cfg, eager_moments=1, track_ids=1, particle_order=order)
+    orc, parts = oracle_from_config(cfg)
+    for s in (0, 1):
+        assert sim.particle_count(s) == L.n_particles(cfg, s) == (x_hi - x_lo) * (y_hi - y_lo)
+        got = sim.get_particles(s, with_id=True)
+        o = np.argsort(got["id"])
+        ref = parts[s]
+        assert np.array_equal(got["id"][o], ref["id"]) and np.array_equal(got["ix"][o], ref["ix"]) and np.array_equal(got["iy"][o], ref["iy"])
+        assert np.array_equal(got["fx"][o], ref["fx"]) and np.array_equal(got["fy"][o], ref["fy"])
+        n = sim.get_moments(s, P.MOMENT_N)
+        assert rel_l2(n, orc.moment(s, "n")) < 1e-5
+        assert np.all(n[:x_lo - 1] == 0) and np.all(n[x_hi + 2:] == 0) and np.all(n[:, :y_lo - 1] == 0)     # vacuum
+    d0 = sim.diagnostics()
+    for step in range(10):
+        sim.step(1)
+        orc.step(1)
+        a = sim.get_fields(P.FIELD_A, 0, 0)
+        scale = max(np.abs(orc.a_now[0]).max(), 1e-30)
+        assert np.abs(a - orc.a_now[0]).max() < 2e-5 * scale + 1e-9, step
+        for s in (0, 1):
+            tol_n, tol_p = (1e-5, 1e-5) if step < 2 else ((1e-4, 5e-4) if s == 0 else (1e-5, 2e-5))
+            assert rel_l2(sim.get_moments(s, P.MOMENT_N), orc.moment(s, "n")) < tol_n, (step, s)
+            assert rel_l2(sim.get_moments(s, P.MOMENT_PX), orc.moment(s, "Px")) < tol_p, (step, s)
+            assert rel_l2(sim.get_moments(s, P.MOMENT_PY), orc.moment(s, "Py")) < tol_p, (step, s)
+    for s, sp in enumerate(cfg["species"]):
+        vth = math.sqrt(sp["T_keV"] / 511.0 / sp["mass"])
+        ex, ey, eu, dabs = _compare_particles(sim, orc, cfg, s, vth)
+        if s == 0:
+            assert max(ex, ey) < 2e-3 and eu < 2e-2 and dabs < 2e-2, (s, ex, ey, eu, dabs)
+        else:
+            assert max(ex, ey) < 1e-5 and eu < 1e-3 and dabs < 1e-4, (s, ex, ey, eu, dabs)
+    sim.step(190)
+    orc.step(190)
+    d1 = sim.diagnostics()
+    assert d1["step"] == 200
+    for s in (0, 1):
+        assert d1["count"][s] == d0["count"][s] == orc.sp[s]["np"]
+        assert d1["charge"][s] == pytest.approx(d0["charge"][s], rel=1e-5)
+    got = sim.get_particles(0)
+    X = got["ix"] + got["fx"].astype(np.float64)
+    oX = orc.sp[0]["X"]
+    assert X.min() < x_lo - 1 and oX.min() < x_lo - 1            # expanded through the margin (measured 0.2 .. 1.3 and 0.45)
+    assert np.std(X) == pytest.approx(np.std(oX), rel=0.02)      # measured 20.83 against 20.84
+    u = np.hypot(got["ux"], got["uy"])
+    assert np.isfinite(u).all() and u.max() < 0.7               # measured 0.17 (oracle 0.16): hot edge, no runaway
+    sim.close()

@@ -145,3 +145,29 @@ def test_polarisation_decomposition_on_the_axes_of_fig_1a():
         assert c[0] == pytest.approx(a * math.cos(th), rel=1e-14)         # a_sz = a cos(theta) as printed
         assert math.hypot(c[1], c[2]) == pytest.approx(a * abs(math.sin(th)), rel=1e-14)      # a_p = a sin(theta)
         assert math.atan2(c[2], c[1]) == pytest.approx(math.atan2(math.sin(be) * math.sin(th), math.cos(be) * math.sin(th)), abs=1e-14)
+
+
+def test_slab_extent_loads_only_the_slab_cells():
+    """profile["slab"] ("a plasma slab is set at the center of the simulation box, and the vacuum space is usually
+    set around the plasma slab"): exactly the cells x_lo <= i < x_hi, y_lo <= j < y_hi hold particles, and each of them
+    holds what it holds without the slab (same ids, offsets, momenta, weights) -- an off-by-one edge, a profile
+    re-stretched over the slab or re-drawn random numbers fail."""
+    cfg = I.config("cbet_vac", nx=80, ny=64)
+    x_lo, x_hi, y_lo, y_hi = cfg["profile"]["slab"]
+    assert (x_lo, x_hi, y_lo, y_hi) == (4, 76, 3, 61) and cfg["profile"]["taper_cells"] == 0
+    assert L.slab_extent(cfg) == (4, 76, 3, 61)
+    full = I.config("cbet_vac", nx=80, ny=64)
+    del full["profile"]["slab"]
+    assert L.slab_extent(full) == (0, 80, 0, 64)
+    for s in (0, 1):
+        p, q = L.generate_particles(cfg, s), L.generate_particles(full, s)
+        assert len(p["id"]) == L.n_particles(cfg, s) == 72 * 58
+        inside = (q["ix"] >= x_lo) & (q["ix"] < x_hi) & (q["iy"] >= y_lo) & (q["iy"] < y_hi)
+        assert inside.sum() == len(p["id"])
+        for key in ("id", "ix", "iy", "fx", "fy", "ux", "uy", "w"):
+            assert np.array_equal(p[key], q[key][inside]), key
+        assert p["ix"].min() == x_lo and p["ix"].max() == x_hi - 1 and p["iy"].min() == y_lo and p["iy"].max() == y_hi - 1
+        assert np.all(p["w"] == np.float32(0.4))          # hard edge: no taper by weight
+    # the x-range argument of generate_particles intersects the slab
+    part = L.generate_particles(cfg, 0, 0, 10)
+    assert set(np.unique(part["ix"])) == set(range(4, 10))

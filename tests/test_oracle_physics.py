@@ -6,6 +6,8 @@ import numpy as np
 import pytest
 
 import oracle
+import pm2d_inputs as I
+import oracle.loader as L
 
 
 def _period_from_zero_crossings(t, y):
@@ -287,3 +289,53 @@ def test_P22_ponderomotive_force_coefficient():
     assert np.abs(fy + 0.5 * (np.roll(a2, -1, 1) - np.roll(a2, 1, 1)) / (2 * dx)).max() < 1e-13 and np.abs(fx).max() < 1e-13
     fx, fy = o.force_now(1)
     assert np.abs(fx).max() == 0.0 and np.abs(fy).max() == 0.0
+
+
+def test_Q20_hard_edged_slab_expands_but_a_weight_taper_to_zero_runs_away():
+    """DESIGN.md Q20, S§8f.2 ("allowing the plasma expanding"; P:L60 the pressure term -C v_th^2 grad(n)/n).  Three
+    copies of a quasi-1D 2 keV electron slab on fixed ions, no laser, 300 steps:
+      (a) a HARD-EDGED slab of equal-weight particles with vacuum on both sides (profile["slab"]): the edge electrons are
+          pushed out by the pressure term and pulled back by the charge separation -- the slab expands into the vacuum and
+          the velocities stay bounded (the contribution of a near-empty node to a particle's force is at most
+          C v_th^2 (n_in / w_p) / 2dx, and n_in / w_p is the number of particles per cell when the weights are equal);
+      (b) the same box filled everywhere, with the profile tapered BY WEIGHT down to TAPER_FLOOR = 1 % (the configs' recipe):
+          bounded, nothing expands;
+      (c) the taper continued to zero weight: a particle 10^3 times lighter than its neighbours sees grad(n)/n of the
+          heavy ones at a node whose density is its own deposit, and runs away.
+    A pressure term that ignored Q10 (n = 0 -> 0), or a loader that tapered the slab's edge by weight, fails (a)."""
+    nx, ny, steps = 96, 8, 300
+
+    def run(kind):
+        cfg = I.config("c2", nx=nx, ny=ny)
+        cfg["lasers"] = []
+        parts = None
+        if kind == "hard":
+            cfg["profile"]["taper_cells"] = 0
+            cfg["profile"]["slab"] = [nx // 4, nx - nx // 4, 0, ny]
+        else:
+            tc = cfg["profile"]["taper_cells"] = nx // 4
+            if kind == "zero":
+                parts = [L.generate_particles(cfg, 0), None]
+                i = parts[0]["ix"].astype(np.float64)
+                d = np.minimum(i + 0.5, nx - 0.5 - i)
+                s2 = np.where(d < tc, np.sin(0.5 * math.pi * d / tc) ** 2, 1.0)
+                parts[0]["w"] = (parts[0]["w"].astype(np.float64) * s2 / (I.TAPER_FLOOR + (1.0 - I.TAPER_FLOOR) * s2)).astype(np.float32)
+        orc, _ = oracle.from_config(cfg, parts)
+        n0 = orc.sp[0]["np"]
+        vth = math.sqrt(cfg["species"][0]["T_keV"] / 511.0)
+        umax, x_lo, x_hi = 0.0, float(nx), 0.0
+        for _ in range(steps // 20):
+            orc.step(20)
+            umax = max(umax, float(np.hypot(orc.sp[0]["ux"], orc.sp[0]["uy"]).max()) / vth)
+            x_lo, x_hi = min(x_lo, float(orc.sp[0]["X"].min())), max(x_hi, float(orc.sp[0]["X"].max()))
+        assert orc.sp[0]["np"] == n0 and np.all(np.isfinite(orc.sp[0]["X"]))
+        return umax, x_lo, x_hi, orc
+
+    u_hard, lo, hi, orc = run("hard")
+    assert u_hard < 12.0                                   # measured 8.8 v_th: hot edge electrons, no runaway
+    assert lo < nx // 4 - 8 and hi > nx - nx // 4 + 8      # the slab has expanded into both margins
+    assert abs(orc.sp[0]["w"].sum() - 48 * ny * 0.15 * 1.0) / (48 * ny * 0.15) < 0.35      # nothing lost (linear profile: mean ~0.15)
+    u_floor, _, _, _ = run("floor")
+    assert u_floor < 7.0                                   # measured 5.2 v_th
+    u_zero, _, _, _ = run("zero")
+    assert u_zero > 2.5 * u_floor                          # measured 25 v_th at step 300 and growing
