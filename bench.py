@@ -225,11 +225,13 @@ def run_cuda(args):
         tp = os.path.join(ROOT, "profiles", "stage_traffic_bytes.txt")
         if os.path.exists(tp) and args.config == "c3" and world == 1 and args.order == "auto":
             try:
+                # bytes, hash of the stage kernel's sources at the time of the capture, the profile that holds the capture
+                from paper_2404_14293_b200.build import stage_id
                 tok = open(tp).read().split()
-                if tok[1] == sim.version().split("build ")[-1].rstrip(")"):
-                    traffic, traffic_src = float(tok[0]), tok[2]
+                if tok[1] == stage_id():
+                    traffic, traffic_src = float(tok[0]), f"{tok[2]} (ncu --set full, stage-kernel sources {tok[1]})"
                 else:
-                    traffic_src = f"stale: {tok[2]} was captured on build {tok[1]}"
+                    traffic_src = f"stale: {tok[2]} was captured on stage-kernel sources {tok[1]}, these are {stage_id()}"
             except Exception:
                 traffic = None
         line = dict(metric="particle-steps/s", value=value, unit="particle-steps/s", n_gpus=world, steps=args.steps,

@@ -30,6 +30,18 @@ def build_id() -> str:
     return h.hexdigest()[:10]
 
 
+STAGE_SOURCES = ["pm2d_lanes.cu", "pm2d_particle_dev.cuh", "pm2d_internal.h"]
+
+
+def stage_id() -> str:
+    """Hash of the sources the fused stage kernel of the lane order (k_stage_lanes) is compiled from: profiles/ tag the
+    ncu figures of that kernel with it, bench.py drops them when it differs."""
+    h = hashlib.sha1()
+    for f in STAGE_SOURCES:
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    return h.hexdigest()[:10]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
