@@ -339,3 +339,51 @@ def test_Q20_hard_edged_slab_expands_but_a_weight_taper_to_zero_runs_away():
     assert u_floor < 7.0                                   # measured 5.2 v_th
     u_zero, _, _, _ = run("zero")
     assert u_zero > 2.5 * u_floor                          # measured 25 v_th at step 300 and growing
+
+
+def test_P23_ion_acoustic_wave_of_two_mobile_species():
+    """Both species mobile (BASELINE.json configs 3, 4, the CBET set-up; the wave SBS and CBET scatter from, P:L324-326,
+    P:L378): a quasi-neutral displacement of electrons and ions of mass M oscillates at the low root of the two-fluid
+    dispersion of Eqs. 2-3 linearised,
+        1 = W_pe^2 / (W^2 - C K^2 v_te^2) + W_pi^2 / (W^2 - C K^2 v_ti^2),   W_ps^2 = 4 pi^2 n0 / m_s,
+    i.e. W ~ K sqrt(C (T_e + T_i) / M) up to the (K lambda_D)^2 correction: the ions' inertia against the electrons'
+    pressure, handed over by E.  Fails with the sign of one species in rho = sum_s q_s n_s flipped (no low root), with the
+    ion mass missing from either the E force or v_ti (period off by sqrt(M) / by the T_i share), with C applied to one
+    species only."""
+    nx, ny, dx, dt, n0, px, M, Te, Ti, C, m = 64, 4, 0.05, 0.035, 0.1, 8, 25.0, 10.0, 1.0, 2.0, 1
+    g = oracle.make_grid(nx, ny, dx, dx, dt)
+    X0, Y0 = _lattice(nx, ny, px, 1)
+    w = np.full(X0.size, n0 / px)
+    n_bg, _, _ = oracle.deposit(g, oracle.SINE, 1.9, X0, Y0, 0 * X0, 0 * X0, w)
+    K = 2 * math.pi * m / nx
+    X = X0 + 0.02 * np.sin(K * X0)
+    sp = [dict(sign=-1, mass=1.0, T_keV=Te, C=C, shape=oracle.SINE, DD=1.9, mobile=1, X=X.copy(), Y=Y0.copy(), ux=0 * X, uy=0 * X, w=w.copy()),
+          dict(sign=+1, mass=M, T_keV=Ti, C=C, shape=oracle.SINE, DD=1.9, mobile=1, X=X.copy(), Y=Y0.copy(), ux=0 * X, uy=0 * X, w=w.copy())]
+    o = oracle.Oracle(nx, ny, dx, dx, dt, sp)
+    basis = np.cos(K * np.arange(nx + 1)[:, None])
+    Kp = K / dx
+    a, b = C * Kp ** 2 * Te / 511.0, C * Kp ** 2 * Ti / 511.0 / M
+    wpe2, wpi2 = 4 * math.pi ** 2 * n0, 4 * math.pi ** 2 * n0 / M
+    s, p = a + b + wpe2 + wpi2, a * b + wpe2 * b + wpi2 * a
+    W = math.sqrt(0.5 * (s - math.sqrt(s * s - 4 * p)))
+    assert W == pytest.approx(Kp * math.sqrt(C * (Te + Ti) / 511.0 / M), rel=0.05)      # the textbook limit; C (K lambda_De)^2 = 4 % lowers W^2
+    nsteps = int(1.6 * 2 * math.pi / W / dt)
+    t, amp_i, amp_e = [], [], []
+    for n in range(nsteps):
+        amp_i.append(((o.moment(1, "n") - n_bg) * basis).sum())
+        amp_e.append(((o.moment(0, "n") - n_bg) * basis).sum())
+        t.append(n * dt)
+        o.step()
+    t, amp_i, amp_e = np.array(t), np.array(amp_i), np.array(amp_e)
+    sg = np.sign(amp_i)
+    idx = np.where(sg[:-1] * sg[1:] < 0)[0]
+    tc = t[idx] - amp_i[idx] * (t[idx + 1] - t[idx]) / (amp_i[idx + 1] - amp_i[idx])
+    assert len(tc) == 3                                                                 # 1.6 periods of a cosine
+    period = tc[2] - tc[0]
+    assert period == pytest.approx(2 * math.pi / W, rel=0.02), (period, 2 * math.pi / W)
+    assert tc[0] == pytest.approx(0.25 * period, rel=0.1)                               # starts at its maximum: a standing wave
+    assert np.abs(amp_i).max() < 1.3 * abs(amp_i[0])                                    # an oscillation, not an instability
+    # quasi-neutral: averaged over the fast Langmuir ripple the electrons follow the ions
+    k = int(round(1.0 / math.sqrt(n0) / dt))
+    sm = np.convolve(amp_e, np.ones(k) / k, mode="valid")
+    assert np.abs(sm - amp_i[k // 2:k // 2 + sm.size]).max() < 0.1 * abs(amp_i[0])
