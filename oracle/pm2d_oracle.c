@@ -17,10 +17,17 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1..P14 of DESIGN.md section 3; the S8(f) widenings in
  * tests/test_oracle_next.py: P15 oblique incidence, P16 sub-cycling, P17 mode amplitudes, P18 velocity
- * histogram, P19 absorbing y walls and corners (Q23), P20 boundary records and their spectrum.
- * Eq. 21 (SBS growth rate) is not pinned.
+ * histogram, P19 absorbing y walls and corners (Q23), P20 boundary records and their spectrum; round 2
+ * (tests/test_oracle_physics.py, test_oracle_pins.py, test_oracle_loader.py): P21 mobile species of mass != 1 (ion
+ * plasma oscillation, heavy neutral sound wave), P22 the ponderomotive coefficient of Eq. 16, P7b the transverse term
+ * of Eq. 8 (oblique reflection is second order), P23 the ion-acoustic wave of two mobile species (two-fluid
+ * dispersion), Q20 (a hard-edged slab expands with bounded velocities, a weight taper to zero runs away), the
+ * loader (oracle/loader.py: Philox known-answer vectors, counts, weights, moments, the slab extent of P:L81) and
+ * orc_polarised (Fig. 1(a)).
+ * Eq. 21 (SBS growth rate) is not pinned: parity unpinned for that formula (DESIGN.md section 9 says why a
+ * slab between walls cannot show it); P23 pins the sound wave it scatters from.
  * Parity unpinned (conventions only, identical by construction on both sides): Q3 (E to nodes),
- * Q5 (Dirichlet phi at the x walls), Q9 (wall folding), Q13, Q14, Q17.
+ * Q5 (Dirichlet phi at the x walls), Q9 (wall folding), Q10, Q13, Q14, Q17, Q24.
  */
 #include <math.h>
 #include <stdint.h>
