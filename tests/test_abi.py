@@ -43,6 +43,32 @@ def test_argument_validation_needs_no_gpu():
     assert lib.pm2d_query_workspace(C.byref(grid), sp, len(cfg["species"])) == 0
 
 
+def test_slab_extent_is_validated_before_any_device_work():
+    """pm2d_profile.slab: 0 <= lo < hi <= nx resp. ny or all zero, never with the number-weighted loading; the check
+    sits in front of every CUDA call, so it answers on a machine without a GPU."""
+    import ctypes as C
+    import pm2d_inputs as I
+    from paper_2404_14293_b200.binding import make_structs
+
+    lib = P.load_library()
+    out = C.c_void_p()
+
+    def init(cfg):
+        grid, sp, prof, las = make_structs(cfg)
+        return lib.pm2d_init(C.byref(grid), sp, len(cfg["species"]), C.byref(prof), las, len(cfg["lasers"]), 0, None, 0, None, C.byref(out))
+
+    for bad in ([0, 65, 0, 32], [10, 10, 0, 32], [-1, 20, 0, 32], [4, 60, 8, 33], [4, 60, 20, 8]):
+        cfg = I.config("c1", nx=64, ny=32)
+        cfg["profile"]["slab"] = bad
+        assert init(cfg) == -1 and b"profile slab" in lib.pm2d_last_error(), bad          # PM2D_EINVAL
+    cfg = I.config("c5", nx=64, ny=32)
+    cfg["profile"]["slab"] = [4, 60, 4, 28]
+    assert init(cfg) == -1 and b"NUMBER_WEIGHTED" in lib.pm2d_last_error()
+    cfg = I.config("c1", nx=64, ny=32)
+    cfg["profile"]["slab"] = [4, 60, 4, 28]              # a valid slab gets past the check (and then fails for want of a workspace / GPU)
+    assert init(cfg) != 0 and b"profile slab" not in lib.pm2d_last_error()
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2404_14293_b200")
     for dirpath, _, files in os.walk(pkg):
