@@ -1183,10 +1183,13 @@ def test_vacuum_margin_slab_parity_and_expansion(P, order):
     - Fields and deposits agree with the oracle at BASELINE.json's 1e-5 for the first two particle steps (10 wave steps).
       From the third step on the ELECTRON quantities agree to 1e-4 (n), 5e-4 (n u) and the electron phase space after 10
       steps to 2e-3 / 2e-2 instead: the pressure term of Eq. 16, -C v_th^2 grad(n) / n, is evaluated at nodes that only
-      the tail of a cloud reaches (n = 1e-4 .. 1e-6 of the slab's), where the 5e-7 absolute error of a float32 weight is a
-      per-cent error of n, and the edge electrons it accelerates carry that into n u (all four kernels give the same
-      numbers: measured 2.9e-5, 1.2e-4, 3e-4 / 2.5e-3).  The ions, which feel the edge only through
-      E, stay at 1e-5 in n and position.
+      the tail of a cloud reaches (n = 1e-4 .. 1e-6 of the slab's), where the ABSOLUTE resolution of the deposit -- the
+      int32 unit n_cap / 2^31 = 1.9e-9 n_c each contribution is rounded to, and the float32 weights -- is a relative error
+      of 1e-4 .. 1e-2, and the edge electrons it accelerates carry that into n u (all four kernels give the same numbers:
+      measured 2.9e-5, 1.2e-4, 3e-4 / 2.5e-3).  tests/test_oracle_physics.py::
+      test_vacuum_edge_amplifies_the_absolute_resolution_of_the_deposit shows the same size with the oracle alone (+-2
+      units on the density move edge electrons by 8.5e-4 v_th per step here, by 1.8e-6 in the floor-tapered slab).  The ions,
+      which feel the edge only through E, stay at 1e-5 in n and position.
     - Over 200 particle steps (1000 wave steps) both sides keep their particle counts and the device its total charge, the
       electrons have spread through the margin to the wall on both sides ("allowing the plasma expanding"), and the
       width of the electron cloud agrees to 2 % (a property: float32 and float64 runs of this set-up drift apart, 6.5)."""
