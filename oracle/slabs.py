@@ -15,6 +15,8 @@ the world_size-2 gloo test can check it against the single-domain oracle:
                           the rank's interior nodes with its two interface values as unknowns g: phi = y + g_l V + g_r W
   * interface_solve       the (world - 1) x (world - 1) tridiagonal system for the interface values, per k_y
   * migrate               the paper's leaver / arrival bookkeeping
+  * SlabField             Eqs. 6-8 on the rank's node columns plus one halo column of `a` per internal cut, exchanged
+                          once per step: bit for bit the single-domain field
 
 `comm` is any object with all_gather(obj) -> list (torch.distributed in the test, a loop in the serial check).
 """
@@ -197,3 +199,51 @@ def migrate(parts, x_lo, x_hi, rank, world, comm):
         keep[holes[nfill:]] = False
         out = {k: v[keep] for k, v in out.items()}
     return out
+
+
+# ---- the stencil halo of the wave equation --------------------------------------------------------------------------------
+class SlabField:
+    """Eqs. 6-8 on one x-slab: the rank's owned node columns plus ONE halo column of `a` per internal cut
+    ("a stencil halo for a"; Eq. 6 reaches one node in x).  The local grid is an ordinary oracle grid whose
+    end columns are either a true wall of the box (rank 0: the left wall with the injected beams, last rank: the right
+    wall; Eq. 8 applies there and only there) or a halo column, whose value after a step is whatever the local wall
+    condition made of it and is overwritten by the neighbour's owned column before the next step.  n_e is held fixed (the
+    deposit exchange is slab_deposit / add_ghosts).  One exchange per step and cut: ncomp x ny values each way.
+
+    step()            one wave step of the local grid
+    boundary()        -> (first owned column, last owned column) of the newest level, each [ncomp][ny]
+    set_halo(l, r)    the neighbours' columns into the halo (None at a true wall)
+    owned()           the owned columns of the newest level, [ncomp][n_own][ny]"""
+
+    def __init__(self, nx, ny, dx, dy, dt, ncomp, n_e, lasers, world, rank, bc_y=0):
+        from . import Oracle
+        x_lo, x_hi = slab_cells(nx, world, rank)
+        self.left_halo, self.right_halo = rank > 0, rank < world - 1
+        self.first = x_lo - (1 if self.left_halo else 0)                 # first local node (global index)
+        self.last = x_hi if self.right_halo else nx                      # last local node
+        self.n_own = x_hi - x_lo + (0 if self.right_halo else 1)
+        fixed = dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, n_fixed=np.ascontiguousarray(n_e[self.first:self.last + 1]))
+        self.orc = Oracle(self.last - self.first, ny, dx, dy, dt, [fixed], lasers if rank == 0 else [], ncomp, bc_y=bc_y)
+
+    def step(self):
+        self.orc.step(1)
+
+    def _cols(self):
+        a = self.orc.a_now                                               # [ncomp][local nodes][ny]
+        lo = 1 if self.left_halo else 0
+        return a, lo, lo + self.n_own
+
+    def boundary(self):
+        a, lo, hi = self._cols()
+        return a[:, lo].copy(), a[:, hi - 1].copy()
+
+    def set_halo(self, from_left, from_right):
+        a, lo, hi = self._cols()
+        if self.left_halo:
+            a[:, 0] = from_left
+        if self.right_halo:
+            a[:, hi] = from_right
+
+    def owned(self):
+        a, lo, hi = self._cols()
+        return a[:, lo:hi].copy()

@@ -1,6 +1,7 @@
 """SURVEY 8(f).3 without a second GPU: the x-slab decomposition of the deposit, of the Poisson solve and of the particle
 lists (oracle/slabs.py) against the single-domain oracle.  world_size 2 over gloo, and the same
-arithmetic for three and five slabs in one process.  CPU only."""
+arithmetic for three and five slabs in one process; the wave equation by slabs with a one-column halo of `a` (SlabField),
+bit for bit.  CPU only."""
 import os
 import socket
 import sys
@@ -10,6 +11,9 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import oracle  # noqa: E402
 
 
 class _SerialComm:
@@ -128,6 +132,52 @@ def test_three_and_five_slabs_equal_the_single_domain():
     _serial_check(5, 73)
 
 
+FIELD_STEPS = 120
+
+
+def _field_case(nx=72, ny=16, ncomp=1):
+    """A fixed electron density (the reduced c3 deposit) and an oblique Gaussian beam that crosses the cuts."""
+    cfg, parts = _case(nx=nx, ny=ny)
+    g = cfg["grid"]
+    p = parts[0]
+    grid = oracle.make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"])
+    n_e, _, _ = oracle.deposit(grid, cfg["species"][0]["shape"], cfg["species"][0]["DD"], p["ix"] + p["fx"].astype(np.float64),
+                               p["iy"] + p["fy"].astype(np.float64), p["ux"].astype(np.float64), p["uy"].astype(np.float64), p["w"].astype(np.float64))
+    Ly = g["ny"] * g["dy"]
+    lasers = [dict(a0=0.02, omega=1.0, y0=0.5 * Ly, w0=0.3 * Ly, t_rise=0.5, alpha=0.15, comp=0)]
+    return g, n_e, lasers
+
+
+def _field_reference(g, n_e, lasers, nsteps):
+    fixed = dict(sign=-1, mass=1.0, T_keV=0.0, mobile=0, n_fixed=n_e)
+    orc = oracle.Oracle(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], [fixed], lasers, 1)
+    orc.step(nsteps)
+    return orc.a_now.copy()
+
+
+def test_wave_equation_by_slabs_with_a_one_column_halo_is_the_single_domain_bit_for_bit():
+    """SURVEY 8e (1) / P:L256: Eqs. 6-8 advanced slab by slab, one halo column of `a` exchanged per cut and step, give on
+    every owned node exactly the bits of the single-domain run (the update of a node reads its four neighbours and n_e,
+    nothing else) -- for 3 equal and 5 unequal slabs, through the turn-on of an oblique beam that crosses every cut.  A
+    halo taken from the wrong time level, a wall condition applied at a cut, or an off-by-one in the owned range fails."""
+    sys.path.insert(0, ROOT)
+    from oracle import slabs
+    for world, nx in ((3, 72), (5, 73)):
+        g, n_e, lasers = _field_case(nx=nx)
+        nsteps = 140
+        ref = _field_reference(g, n_e, lasers, nsteps)
+        assert np.abs(ref).max() > 0.005 and np.abs(ref[0, g["nx"] - 4:]).max() > 1e-4          # the beam has reached the right wall
+        ranks = [slabs.SlabField(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], 1, n_e, lasers, world, r) for r in range(world)]
+        for _ in range(nsteps):
+            for f in ranks:
+                f.step()
+            edges = [f.boundary() for f in ranks]
+            for r, f in enumerate(ranks):
+                f.set_halo(edges[r - 1][1] if r > 0 else None, edges[r + 1][0] if r < world - 1 else None)
+        got = np.concatenate([f.owned() for f in ranks], axis=1)
+        assert got.shape == ref.shape and np.array_equal(got, ref)
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
@@ -152,7 +202,14 @@ def _worker(rank, world, port, out):
     mov = dict(X=np.clip(X[mine] + rng.normal(0.0, 1.5, mine.sum()), 0.0, g["nx"] - 1e-9), id=p["id"][mine].copy(),
                ux=p["ux"][mine].copy())
     got = slabs.migrate(mov, x_lo, x_hi, rank, world, comm)
-    out.put((rank, dens, phi, mov, got))
+    # the wave equation with its halo column sent over the process group, one exchange per step
+    gg, n_e, lasers = _field_case()
+    f = slabs.SlabField(gg["nx"], gg["ny"], gg["dx"], gg["dy"], gg["dt"], 1, n_e, lasers, world, rank)
+    for _ in range(FIELD_STEPS):
+        f.step()
+        edges = comm.all_gather(f.boundary())
+        f.set_halo(edges[rank - 1][1] if rank > 0 else None, edges[rank + 1][0] if rank < world - 1 else None)
+    out.put((rank, dens, phi, mov, got, f.owned()))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -183,7 +240,9 @@ def test_two_slabs_over_gloo_equal_the_single_domain():
     before = {int(i): (x, u) for r in res for i, x, u in zip(r[3]["id"], r[3]["X"], r[3]["ux"])}
     after = {}
     crossed = 0
-    for rank, _, _, mov, got in res:
+    gg, n_e, lasers = _field_case()
+    assert np.array_equal(np.concatenate([r[5] for r in res], axis=1), _field_reference(gg, n_e, lasers, FIELD_STEPS))
+    for rank, _, _, mov, got, _ in res:
         x_lo, x_hi = slabs.slab_cells(g["nx"], world, rank)
         assert ((got["X"] >= x_lo) & (got["X"] < x_hi)).all()
         crossed += int(((mov["X"] < x_lo) | (mov["X"] >= x_hi)).sum())
