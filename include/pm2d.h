@@ -331,6 +331,11 @@ void pm2d_free(pm2d_ctx *ctx);
 const char *pm2d_last_error(void);
 const char *pm2d_version(void);
 
+/* sizeof of the structs above as this library was compiled: which = 0 pm2d_grid, 1 pm2d_species, 2 pm2d_profile,
+ * 3 pm2d_laser, 4 pm2d_diag; -1 for any other value.  Host only, no ctx, no GPU: a binding checks its own layout
+ * against it before it hands a struct over (tests/test_abi.py does, on a machine without a GPU). */
+int pm2d_struct_size(int which);
+
 #ifdef __cplusplus
 }
 #endif

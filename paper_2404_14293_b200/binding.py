@@ -93,6 +93,7 @@ SYMBOLS = {
     "pm2d_free": (None, [_vp]),
     "pm2d_last_error": (C.c_char_p, []),
     "pm2d_version": (C.c_char_p, []),
+    "pm2d_struct_size": (C.c_int, [C.c_int]),
 }
 
 _lib = None
@@ -109,6 +110,11 @@ def load_library():
             f = getattr(L, name)            # AttributeError if the library does not export it
             f.restype = res
             f.argtypes = args
+        # the ctypes mirrors must have the layout the library was compiled with (a struct grown on one side only would be
+        # read past its end on the other)
+        for which, st in enumerate((Grid, Species, Profile, Laser, Diag)):
+            if L.pm2d_struct_size(which) != C.sizeof(st):
+                raise RuntimeError(f"{st.__name__}: the binding has {C.sizeof(st)} bytes, {LIB_PATH} has {L.pm2d_struct_size(which)}: rebuild the library")
         _lib = L
     return _lib
 

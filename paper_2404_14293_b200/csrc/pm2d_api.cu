@@ -17,6 +17,18 @@ extern "C" const char *pm2d_last_error(void) { return g_err.c_str(); }
 #endif
 extern "C" const char *pm2d_version(void) { return "pm2d-b200 0.2 (sm_100a, build " PM2D_BUILD_ID ")"; }
 
+extern "C" int pm2d_struct_size(int which)
+{
+    switch (which) {
+    case 0: return (int)sizeof(pm2d_grid);
+    case 1: return (int)sizeof(pm2d_species);
+    case 2: return (int)sizeof(pm2d_profile);
+    case 3: return (int)sizeof(pm2d_laser);
+    case 4: return (int)sizeof(pm2d_diag);
+    default: return -1;
+    }
+}
+
 static int fail(int code, const std::string &msg)
 {
     g_err = msg;

@@ -69,6 +69,22 @@ def test_slab_extent_is_validated_before_any_device_work():
     assert init(cfg) != 0 and b"profile slab" not in lib.pm2d_last_error()
 
 
+def test_struct_layouts_of_the_binding_match_the_library():
+    """pm2d_struct_size: the ctypes mirrors of pm2d_grid / species / profile / laser / diag have the sizes the library was
+    compiled with (load_library refuses a mismatch); the fields the header lists last sit at the end of the mirrors."""
+    import ctypes as C
+    from paper_2404_14293_b200 import binding as B
+    lib = P.load_library()
+    for which, st in enumerate((B.Grid, B.Species, B.Profile, B.Laser, B.Diag)):
+        assert lib.pm2d_struct_size(which) == C.sizeof(st) > 0, st.__name__
+    assert lib.pm2d_struct_size(5) == -1 and lib.pm2d_struct_size(-1) == -1
+    assert B.Profile.slab.offset + 16 == C.sizeof(B.Profile) and B.Profile.p.offset == 8
+    hdr = open(os.path.join(ROOT, "include", "pm2d.h")).read()
+    body = "    " + hdr[hdr.index("int32_t kind;          /* PM2D_PROFILE_*"):hdr.index("} pm2d_profile;")]
+    order = [m for m in re.findall(r"^\s+(?:int32_t|double)\s+(\w+)", body, flags=re.M)]
+    assert order == [n for n, _ in B.Profile._fields_], order
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2404_14293_b200")
     for dirpath, _, files in os.walk(pkg):
