@@ -17,6 +17,9 @@ the world_size-2 gloo test can check it against the single-domain oracle:
   * migrate               the paper's leaver / arrival bookkeeping
   * SlabField             Eqs. 6-8 on the rank's node columns plus one halo column of `a` per internal cut, exchanged
                           once per step: bit for bit the single-domain field
+  * SlabRank              the whole program flow of P:L229-238 for one rank: the pieces above plus Eq. 16 / 18 on the
+                          rank's window of nodes (HALO columns of n_s, phi, a from each neighbour), gather, predictor,
+                          corrector and walls for the rank's own particles; equals the single-domain oracle step
 
 `comm` is any object with all_gather(obj) -> list (torch.distributed in the test, a loop in the serial check).
 """
@@ -247,3 +250,133 @@ class SlabField:
     def owned(self):
         a, lo, hi = self._cols()
         return a[:, lo:hi].copy()
+
+
+# ---- the whole time step, slab by slab ------------------------------------------------------------------------------------
+HALO = 4       # node columns of n_s, phi and a that a rank reads beyond its owned nodes when it builds the force grid its own
+#                particles gather from: a footprint reaches 2 nodes beyond the slab at the predicted position, Eq. 16 one more
+#                (central differences, E on cell centres), and the last column of a window that ends on a cut is not used
+
+
+class SlabRank:
+    """One rank of the program flow of P:L229-238 on x-slabs: everything a rank computes is on its own nodes and
+    its own particles; what it reads from its neighbours is named at each exchange.  `comm.all_gather` stands in for
+    the neighbour exchanges (a device version sends HALO / GHOST columns to two neighbours instead of gathering
+    everything; the values used are the same).  All species mobile, no sub-cycling, periodic y.
+
+    per step:   halo of n_s^n  ->  a^{n+1} (SlabField, 1-column halo of a)  ->  halo of a^{n+1}
+                rho -> slab Poisson (interface system) -> halo of phi  ->  E, F_s^n on the rank's window (Eq. 16)
+                gather + predictor (Eqs. 15, 17) for the rank's particles  ->  deposit (x^, u^) + ghost sums
+                slab Poisson again -> F_s^ (Eq. 18)  ->  gather at x^ + corrector (Eq. 19) + walls
+                migrate  ->  deposit (x^{n+1}, u^{n+1}) + ghost sums = item (1) of the next step"""
+
+    def __init__(self, cfg, parts, world, rank):
+        from . import Oracle
+        g = cfg["grid"]
+        assert all(sp["mobile"] for sp in cfg["species"]) and g.get("subcycle", 1) <= 1 and not g.get("bc_y", 0)
+        self.cfg, self.world, self.rank = cfg, world, rank
+        self.nx, self.ny, self.dx, self.dy, self.dt, self.ncomp = g["nx"], g["ny"], g["dx"], g["dy"], g["dt"], g["ncomp"]
+        self.x_lo, self.x_hi = slab_cells(self.nx, world, rank)
+        self.n_own = self.x_hi - self.x_lo + (1 if rank == world - 1 else 0)
+        self.w_lo, self.w_hi = max(0, self.x_lo - HALO), min(self.nx, self.x_hi + HALO)         # the rank's window of nodes
+        self.wgrid = _make_grid(self.w_hi - self.w_lo, self.ny, self.dx, self.dy, self.dt, self.ncomp)
+        self.sp = []
+        for s, q in enumerate(cfg["species"]):
+            p = parts[s]
+            X = p["ix"] + p["fx"].astype(np.float64)
+            m = (X >= self.x_lo) & (X < self.x_hi)
+            self.sp.append(dict(X=X[m], Y=(p["iy"] + p["fy"].astype(np.float64))[m], ux=p["ux"][m].astype(np.float64),
+                                uy=p["uy"][m].astype(np.float64), w=p["w"][m].astype(np.float64), id=p["id"][m].copy()))
+        lasers = [dict(a0=l["a0"], omega=l["omega"], y0=l["y0"], w0=l["w0"], t_rise=l["t_rise"], comp=l["comp"], alpha=l.get("alpha", 0.0))
+                  for l in cfg["lasers"]]
+        self.field = SlabField(self.nx, self.ny, self.dx, self.dy, self.dt, self.ncomp, np.zeros((self.nx + 1, self.ny)), lasers, world, rank)
+        nw = self.w_hi - self.w_lo + 1
+        fixed = [dict(sign=q["sign"], mass=q["mass"], T_keV=q["T_keV"], C=q["pressure_coeff"], shape=q["shape"], DD=q["DD"], mobile=0,
+                      n_fixed=np.zeros((nw, self.ny))) for q in cfg["species"]]
+        self.loc = Oracle(self.w_hi - self.w_lo, self.ny, self.dx, self.dy, self.dt, fixed, [], self.ncomp)      # Eq. 16 on the window
+        self.a_win = np.zeros((self.ncomp, nw, self.ny))                                                 # a^n
+        self.n_own_s = None
+
+    # -- exchanges ----------------------------------------------------------------------------------------------------
+    def _window(self, comm, own):
+        """Owned node columns [.., n_own, ny] of every rank -> this rank's window (its own columns + HALO columns of each
+        neighbour's)."""
+        full = np.concatenate(comm.all_gather(own), axis=-2)
+        return np.ascontiguousarray(full[..., self.w_lo:self.w_hi + 1, :])
+
+    def _deposit(self, comm, s, X, Y, ux, uy):
+        """Eq. 14 of the rank's particles on its window, ghost columns summed at their owners -> owned n, Px, Py."""
+        q = self.cfg["species"][s]
+        loc = _deposit(self.wgrid, q["shape"], q["DD"], X - self.w_lo, Y, ux, uy, self.sp[s]["w"])
+        return [add_ghosts(self.nx, self.ny, self.world, self.rank, a, self.w_lo, comm) for a in loc]
+
+    def initial_deposit(self, comm):
+        self.n_own_s = [self._deposit(comm, s, d["X"], d["Y"], d["ux"], d["uy"])[0] for s, d in enumerate(self.sp)]
+
+    # -- Eq. 16 / 18 on the window --------------------------------------------------------------------------------------
+    def _forces(self, comm, n_own_s, a_win):
+        import ctypes as C
+        from . import efield, lib, _p
+        signs = [q["sign"] for q in self.cfg["species"]]
+        rho_own = sum(sg * n for sg, n in zip(signs, n_own_s))
+        phi_win = self._window(comm, slab_poisson(self.nx, self.ny, self.dx, self.dy, self.world, self.rank, rho_own, comm))
+        Ex, Ey = efield(self.loc.g, phi_win)
+        Ex, Ey = np.ascontiguousarray(Ex), np.ascontiguousarray(Ey)
+        F = []
+        for s in range(len(self.sp)):
+            self.loc.sp[s]["n"][:] = self._window(comm, n_own_s[s]).ravel()
+            Fx, Fy = np.zeros(self.loc.nn), np.zeros(self.loc.nn)
+            lib().orc_force(C.byref(self.loc.g), C.byref(self.loc._sp[s]), _p(np.ascontiguousarray(a_win)), _p(Ex), _p(Ey), _p(Fx), _p(Fy))
+            F.append((Fx, Fy))
+        return F
+
+    # -- one step -------------------------------------------------------------------------------------------------------
+    def step(self, comm):
+        from . import gather, predictor, corrector
+        nx, ny, dt = self.nx, self.ny, self.dt
+        hx, hy = dt / (2.0 * self.dx), dt / (2.0 * self.dy)
+        cfgs = self.cfg["species"]
+        # (2) the wave equation with n_e^n on the field's local nodes (1-column halo of a^n is in place), then the halos
+        n_e = sum(self._window(comm, n) for n, q in zip(self.n_own_s, cfgs) if q["sign"] < 0)
+        f = self.field
+        f.orc.sp[0]["n"][:] = n_e[f.first - self.w_lo:f.last - self.w_lo + 1].ravel()
+        f.step()
+        edges = comm.all_gather(f.boundary())
+        f.set_halo(edges[self.rank - 1][1] if self.rank > 0 else None, edges[self.rank + 1][0] if self.rank < self.world - 1 else None)
+        a_new_win = self._window(comm, f.owned())
+        # (2)(3) E^n, F^n with a^n;  (3)(4) gather at x^n, predictor
+        F = self._forces(comm, self.n_own_s, self.a_win)
+        hat = []
+        for s, d in enumerate(self.sp):
+            q = cfgs[s]
+            npart = d["X"].size
+            uhx, uhy, Xh, Yh = (np.zeros(npart) for _ in range(4))
+            for p in range(npart):
+                fx, fy = gather(self.wgrid, q["shape"], q["DD"], d["X"][p] - self.w_lo, d["Y"][p], F[s][0], F[s][1])
+                uhx[p], Xh[p] = predictor(dt, hx, d["X"][p], d["ux"][p], fx)
+                uhy[p], Yh[p] = predictor(dt, hy, d["Y"][p], d["uy"][p], fy)
+            d["uhx"], d["uhy"] = uhx, uhy
+            hat.append(self._deposit(comm, s, Xh, Yh, uhx, uhy)[0])                                   # (5)
+        # (6)(7) E^, F^ with a^{n+1} and n^;  (8) gather at x^, corrector, walls
+        F = self._forces(comm, hat, a_new_win)
+        for s, d in enumerate(self.sp):
+            q = cfgs[s]
+            for p in range(d["X"].size):
+                xh = d["X"][p] + hx * (d["uhx"][p] + d["ux"][p])
+                yh = d["Y"][p] + hy * (d["uhy"][p] + d["uy"][p])
+                fx, fy = gather(self.wgrid, q["shape"], q["DD"], xh - self.w_lo, yh, F[s][0], F[s][1])
+                unx, xn = corrector(dt, hx, d["X"][p], d["ux"][p], d["uhx"][p], fx)
+                uny, yn = corrector(dt, hy, d["Y"][p], d["uy"][p], d["uhy"][p], fy)
+                if xn < 0.0:
+                    xn, unx = -xn, -unx
+                if xn > nx:
+                    xn, unx = 2.0 * nx - xn, -unx
+                yn -= np.floor(yn / ny) * ny
+                if yn >= ny:
+                    yn -= ny
+                d["X"][p], d["Y"][p], d["ux"][p], d["uy"][p] = xn, yn, unx, uny
+            # the list reconstruction of P:L274-276, then item (1) of the next step
+            moved = migrate({k: d[k] for k in ("X", "Y", "ux", "uy", "w", "id")}, self.x_lo, self.x_hi, self.rank, self.world, comm)
+            self.sp[s] = moved
+        self.n_own_s = [self._deposit(comm, s, d["X"], d["Y"], d["ux"], d["uy"])[0] for s, d in enumerate(self.sp)]
+        self.a_win = a_new_win

@@ -178,6 +178,97 @@ def test_wave_equation_by_slabs_with_a_one_column_halo_is_the_single_domain_bit_
         assert got.shape == ref.shape and np.array_equal(got, ref)
 
 
+class _ThreadComm:
+    """all_gather between ranks that run as threads of one process (any number of exchanges, in lockstep)."""
+
+    def __init__(self, world):
+        import threading
+        self.world, self.slots, self.bar = world, [None] * world, threading.Barrier(world)
+
+    def bind(self, rank):
+        comm = self
+
+        class _Bound:
+            def all_gather(self, obj):
+                comm.slots[rank] = obj
+                comm.bar.wait()
+                out = list(comm.slots)
+                comm.bar.wait()
+                return out
+        return _Bound()
+
+
+def _whole_step_by_slabs(cfg, parts, world, nsteps, comm_of_rank, ranks):
+    from oracle import slabs
+    out = {}
+    for rank in ranks:
+        r = slabs.SlabRank(cfg, parts, world, rank)
+        comm = comm_of_rank(rank)
+        r.initial_deposit(comm)
+        for _ in range(nsteps):
+            r.step(comm)
+        out[rank] = (r.sp, r.field.owned(), r.n_own_s)
+    return out
+
+
+def _compare_with_single_domain(cfg, parts, res, world, nsteps, a_min=5e-3):
+    orc, _ = oracle.from_config(cfg, parts)
+    orc.step(nsteps)
+    a = np.concatenate([res[r][1] for r in range(world)], axis=1)
+    assert np.abs(a - orc.a_now).max() < 1e-12 * np.abs(orc.a_now).max() and np.abs(orc.a_now).max() > a_min, (
+        np.abs(a - orc.a_now).max(), np.abs(orc.a_now).max())
+    from oracle import slabs
+    moved = 0
+    for s in range(len(cfg["species"])):
+        n = np.concatenate([res[r][2][s] for r in range(world)])
+        assert np.abs(n - orc.moment(s, "n")).max() < 1e-11 * np.abs(orc.moment(s, "n")).max()
+        ids = np.concatenate([res[r][0][s]["id"] for r in range(world)])
+        order = np.argsort(ids)
+        assert np.array_equal(ids[order], np.sort(parts[s]["id"]))               # every particle exactly once
+        ref_order = np.argsort(parts[s]["id"])
+        for key in ("X", "Y", "ux", "uy"):
+            got = np.concatenate([res[r][0][s][key] for r in range(world)])[order]
+            want = orc.sp[s][key][ref_order]
+            assert np.abs(got - want).max() < 1e-10, (s, key, np.abs(got - want).max())
+        for r in range(world):
+            x_lo, x_hi = slabs.slab_cells(cfg["grid"]["nx"], world, r)
+            X = res[r][0][s]["X"]
+            assert ((X >= x_lo) & (X < x_hi)).all()
+            X0 = parts[s]["ix"][np.isin(parts[s]["id"], res[r][0][s]["id"])]
+            moved += int(((X0 < x_lo) | (X0 >= x_hi)).sum())
+    return moved
+
+
+def test_the_whole_time_step_by_slabs_equals_the_single_domain():
+    """three ranks (threads of this process) carry the program flow of P:L229-238 on x-slabs
+    for ten steps of the reduced c3 set-up (electrons and mobile ions, sine clouds, the laser turning on) -- deposit with
+    ghost sums, wave equation with its halo, slab Poisson with the interface system, Eq. 16 on the rank's window, gather,
+    predictor, corrector, walls, migration -- and end with the single-domain oracle's particles (1e-10 cell, by id), field
+    and densities; particles have crossed the cuts."""
+    import threading
+    cfg, parts = _case(nx=72, ny=16)
+    cfg["lasers"][0]["t_rise"] = 0.2               # the beam is at full amplitude within the run: the ponderomotive term of Eq. 16 acts
+    world, nsteps = 3, 10
+    comm = _ThreadComm(world)
+    res, err = {}, []
+
+    def run(rank):
+        try:
+            res.update(_whole_step_by_slabs(cfg, parts, world, nsteps, comm.bind, [rank]))
+        except BaseException as e:          # a dead rank would leave the others at the barrier
+            err.append(e)
+            comm.bar.abort()
+
+    th = [threading.Thread(target=run, args=(r,)) for r in range(world)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join(timeout=600)
+    assert not err, err
+    moved = _compare_with_single_domain(cfg, parts, res, world, nsteps)
+    assert moved > 20
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
@@ -209,7 +300,9 @@ def _worker(rank, world, port, out):
         f.step()
         edges = comm.all_gather(f.boundary())
         f.set_halo(edges[rank - 1][1] if rank > 0 else None, edges[rank + 1][0] if rank < world - 1 else None)
-    out.put((rank, dens, phi, mov, got, f.owned()))
+    # and the whole time step (SlabRank), four steps
+    whole = _whole_step_by_slabs(cfg, parts, world, 4, lambda r: comm, [rank])[rank]
+    out.put((rank, dens, phi, mov, got, f.owned(), whole))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -242,7 +335,8 @@ def test_two_slabs_over_gloo_equal_the_single_domain():
     crossed = 0
     gg, n_e, lasers = _field_case()
     assert np.array_equal(np.concatenate([r[5] for r in res], axis=1), _field_reference(gg, n_e, lasers, FIELD_STEPS))
-    for rank, _, _, mov, got, _ in res:
+    _compare_with_single_domain(cfg, parts, {r[0]: r[6] for r in res}, world, 4, a_min=0.0)
+    for rank, _, _, mov, got, _, _ in res:
         x_lo, x_hi = slabs.slab_cells(g["nx"], world, rank)
         assert ((got["X"] >= x_lo) & (got["X"] < x_hi)).all()
         crossed += int(((mov["X"] < x_lo) | (mov["X"] >= x_hi)).sum())
