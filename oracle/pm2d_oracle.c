@@ -27,7 +27,8 @@
  * Eq. 21 (SBS growth rate) is not pinned: parity unpinned for that formula (DESIGN.md section 9 says why a
  * slab between walls cannot show it); P23 pins the sound wave it scatters from.
  * Parity unpinned (conventions only, identical by construction on both sides): Q3 (E to nodes),
- * Q5 (Dirichlet phi at the x walls), Q9 (wall folding), Q10, Q13, Q14, Q17, Q24.
+ * Q5 (Dirichlet phi at the x walls), Q13, Q14, Q24, the value 0 of Q10 and the taper recipe of Q9 (the wall weights of Q9
+ * and the cell-centre sampling of Q17 are pinned: uniform lattice on wall nodes, loader weights).
  */
 #include <math.h>
 #include <stdint.h>
