@@ -26,9 +26,10 @@
  * orc_polarised (Fig. 1(a)).
  * Eq. 21 (SBS growth rate) is not pinned: parity unpinned for that formula (DESIGN.md section 9 says why a
  * slab between walls cannot show it); P23 pins the sound wave it scatters from.
- * Parity unpinned (conventions only, identical by construction on both sides): Q3 (E to nodes),
+ * Parity unpinned (conventions only, identical by construction on both sides):
  * Q5 (Dirichlet phi at the x walls), Q13, Q14, Q24, the value 0 of Q10 and the taper recipe of Q9 (the wall weights of Q9
- * and the cell-centre sampling of Q17 are pinned: uniform lattice on wall nodes, loader weights).
+ * and the cell-centre sampling of Q17 are pinned: uniform lattice on wall nodes, loader weights; Q3, E to the nodes, by
+ * the closed-form transfer factors of a Fourier mode).
  */
 #include <math.h>
 #include <stdint.h>

@@ -447,3 +447,38 @@ def test_P7_oblique_reflection_is_second_order(deg, m):
     else:      # 0.005: the discretisation (16 cells per wavelength) takes its share; still 30 times below first order
         assert 0.3 * second < refl < 1.5 * second, (refl, second, first)
     assert refl < 0.6 * first
+
+
+def test_Q3_nodal_field_is_the_mean_of_the_adjacent_cell_centres():
+    """P:L140-148 puts E on cell centres ("first calculated in the x direction by a central difference scheme and then
+    averaged in the y direction"), the forces of Eq. 16 live on nodes; reading Q3 takes the mean of the (up to)
+    four adjacent cell-centre values, two at the x walls.  For phi = A sin(Kx x + th) cos(Ky y) both steps are exact
+    multipliers of the mode, so the nodal force of a cold species without light, F = -q (4 pi^2 / m) E, has the closed form
+        E_x(i, j) = -A cos(Kx x_i + th) cos(Ky y_j) sin(Kx dx)/dx cos^2(Ky dy/2)
+        E_y(i, j) = +A sin(Kx x_i + th) sin(Ky y_j) sin(Ky dy)/dy cos^2(Kx dx/2)
+    at interior nodes, and at the wall i = 0 the two-cell mean
+        E_x(0, j) = -A cos(Kx dx/2 + th) cos(Ky y_j) 2 sin(Kx dx/2)/dx cos^2(Ky dy/2).
+    A nearest-cell value instead of the mean (no cos^2 factor, half a cell of phase), E = +grad(phi), a four-cell rule at
+    the wall, or the mass / charge factor of the force fail."""
+    import ctypes as C
+    nx, ny, dx, dy, A, th, mass = 24, 16, 0.05, 0.08, 0.7, 0.3, 2.0
+    Kx, Ky = 2 * math.pi * 2.0 / (nx * dx), 2 * math.pi * 3 / (ny * dy)
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny), indexing="ij")
+    phi = A * np.sin(Kx * i * dx + th) * np.cos(Ky * j * dy)
+    sp = [dict(sign=-1, mass=mass, T_keV=0.0, mobile=0, shape=oracle.CIC, DD=1.0, n_fixed=np.zeros((nx + 1, ny)))]
+    o = oracle.Oracle(nx, ny, dx, dy, 0.035, sp)
+    Ex, Ey = oracle.efield(o.g, phi)
+    Ex, Ey = np.ascontiguousarray(Ex), np.ascontiguousarray(Ey)
+    Fx, Fy = np.zeros((nx + 1) * ny), np.zeros((nx + 1) * ny)
+    oracle.lib().orc_force(C.byref(o.g), C.byref(o._sp[0]), o.st.a_now, oracle._p(Ex), oracle._p(Ey), oracle._p(Fx), oracle._p(Fy))
+    Fx, Fy = Fx.reshape(nx + 1, ny), Fy.reshape(nx + 1, ny)
+    q = 4 * math.pi ** 2 / mass                                       # F = -sign (4 pi^2 / m) E with sign = -1
+    ex = -A * np.cos(Kx * i * dx + th) * np.cos(Ky * j * dy) * math.sin(Kx * dx) / dx * math.cos(Ky * dy / 2) ** 2
+    ey = A * np.sin(Kx * i * dx + th) * np.sin(Ky * j * dy) * math.sin(Ky * dy) / dy * math.cos(Kx * dx / 2) ** 2
+    scale = q * A * max(Kx, Ky)
+    assert np.abs(Fx[1:-1] - q * ex[1:-1]).max() < 1e-12 * scale
+    assert np.abs(Fy[1:-1] - q * ey[1:-1]).max() < 1e-12 * scale
+    wall = -A * math.cos(Kx * dx / 2 + th) * np.cos(Ky * np.arange(ny) * dy) * 2 * math.sin(Kx * dx / 2) / dx * math.cos(Ky * dy / 2) ** 2
+    assert np.abs(Fx[0] - q * wall).max() < 1e-12 * scale
+    # the readings it excludes, in numbers: without the y-mean the factor cos^2(Ky dy/2) = 0.69 would be 1
+    assert math.cos(Ky * dy / 2) ** 2 < 0.75
