@@ -53,3 +53,53 @@ def backscatter_growth_rate(t, scattered, dt=0.035, lo=2e-4, hi=2e-2):
     i0, i1 = int(np.argmax(env > lo)), int(np.argmax(env > hi))
     assert i1 - i0 >= 10, "no clean exponential phase"
     return float(np.polyfit(te[i0:i1], np.log(env[i0:i1]), 1)[0])
+
+
+# ---- the lane storage order (include/pm2d.h, pm2d_rebin) as a numpy specification: the GPU test
+# checks the device's permutation against it bit for bit, tests/test_lane_order_spec.py checks on the CPU what the order is for
+def rank_in_group(group_sorted):
+    """rank of every element inside its run of equal values (the array is sorted by group)"""
+    n = group_sorted.size
+    start = np.r_[0, np.flatnonzero(np.diff(group_sorted)) + 1]
+    return np.arange(n) - np.repeat(start, np.diff(np.r_[start, n]))
+
+
+def lane_order_perm(pp, T, nx, ny, subs, predx=0.0, predy=0.0):
+    """The lane order as include/pm2d.h states it for pm2d_rebin, written out with numpy's stable sorts.
+    -> (perm, key) with key = destination tile * T^2 + cell of the sort position."""
+    n = pp["ix"].size
+    nty = (ny + T - 1) // T
+
+    def sort_pos(i, f, u, pred):            # global, 2^-24 cells: position + free flight of half a rebin period
+        v = i.astype(np.int64) * 2 ** 24 + np.round(f.astype(np.float64) * 2 ** 24).astype(np.int64)
+        return v + np.rint((u.astype(np.float32) * np.float32(pred)).astype(np.float64)).astype(np.int64)
+    xg = np.clip(sort_pos(pp["ix"], pp["fx"], pp["ux"], predx), 0, nx * 2 ** 24 - 1)     # beyond a wall: stays in the wall tile
+    yg = sort_pos(pp["iy"], pp["fy"], pp["uy"], predy) % (ny * 2 ** 24)                  # y is periodic
+    tile = ((xg >> 24) // T) * nty + (yg >> 24) // T
+    xs, ys = xg - ((xg >> 24) // T) * T * 2 ** 24, yg - ((yg >> 24) // T) * T * 2 ** 24
+    cx, cy, fx24, fy24 = xs >> 24, ys >> 24, xs & (2 ** 24 - 1), ys & (2 ** 24 - 1)
+    h = (cx >> 4) if subs == 2 else np.zeros_like(cx)
+    key_a = (h << 10) | (cy << 5) | (fy24 >> 19)
+    xb = (((cx & 15) << 1) | (fx24 >> 23)) if subs == 2 else cx
+    o1 = np.argsort(tile, kind="stable")                                   # the tile pass
+    t1, ka, xb1, h1 = tile[o1], key_a[o1], xb[o1], h[o1]
+    tstart = np.searchsorted(t1, np.arange(t1.max() + 2))                  # first slot of every tile
+    n0 = np.bincount(t1[h1 == 0], minlength=t1.max() + 1)                  # particles of sub-tile 0
+    oa = np.lexsort((ka, t1))
+    rho = np.empty(n, np.int64)
+    rho[oa] = rank_in_group(t1[oa])
+    hb = np.where(h1 == 1, n0[t1], 0)
+    nh = np.where(h1 == 1, (tstart[t1 + 1] - tstart[t1]) - n0[t1], n0[t1])
+    rho_h = rho - hb
+    base, rem = nh // 32, nh % 32
+    cut = rem * (base + 1)
+    slab = np.where(rho_h < cut, rho_h // (base + 1), rem + (rho_h - cut) // np.maximum(base, 1))
+    key_b = (h1 << 10) | (slab << 5) | xb1
+    ob = np.lexsort((key_b, t1))
+    rb = np.empty(n, np.int64)
+    rb[ob] = rank_in_group(t1[ob])
+    w = rb - hb - (slab * base + np.minimum(slab, rem))
+    q = tstart[t1] + hb + 32 * w + slab
+    perm = np.empty(n, np.int64)
+    perm[q] = o1
+    return perm, tile * (T * T) + cx * T + cy
