@@ -99,3 +99,39 @@ def test_sorting_by_the_position_half_a_period_ahead_keeps_the_particles_in_thei
     assert ahead < 3e-4 and now > 3e-3, (ahead, now)                 # measured 1.0e-4 and 5.2e-3
     vth = math.sqrt(3.0 / 511.0)
     assert 0.05 < vth * cfg["grid"]["dt"] / cfg["grid"]["dx"] < 0.06
+
+
+def test_shifted_window_copies_remove_the_bank_conflicts_a_single_window_has():
+    """a warp of the lane order holds one particle of every slab.  With ONE copy of the shared windows the bank
+    of a deposit is its node column: lanes whose particles round to the same column modulo 32 collide (slab i straddles
+    the node columns i and i + 1, so neighbours collide all the time) and a shared atomic costs as many wavefronts as the
+    fullest bank -- the model gives 2.1-2.3 per atomic, what ncu measured on round 1's single-window kernel (2.0-2.4,
+    profiles/r01i).  With the copies shifted by one column each, lane i takes copy m = cy - i and index i + b: its bank is
+    i + b whatever cy is, one wavefront, for every visit that is in lane (all but 1e-4)."""
+    cfg, p = _particles()
+    g = cfg["grid"]
+    perm, tile, sub, lane, w = _lanes(cfg, p, 16)
+    nty = g["ny"] // T
+    y0 = p["iy"] + p["fy"].astype(np.float64)
+    vy = p["uy"].astype(np.float64) * g["dt"] / g["dy"]
+    gy0 = (tile % nty) * T
+    warp = (tile * 2 + sub) * 1024 + w                       # 32 consecutive slots of a sub-tile = one rank w of every slab
+    o = np.lexsort((lane, warp))
+    full = np.flatnonzero(np.bincount(np.unique(warp[o], return_inverse=True)[1]) == 32)
+    _, inv = np.unique(warp[o], return_inverse=True)
+    rows = o[np.isin(inv, full)].reshape(-1, 32)             # particle indices, one row per full warp, lanes in order
+    assert rows.shape[0] > 400 and (lane[rows] == np.arange(32)).all()
+    single, copies = [], []
+    for k in (1, 8, 16):
+        cy = np.floor(y0 + k * vy + 0.5) - gy0
+        cy = ((cy - 16 + g["ny"] / 2) % g["ny"] - g["ny"] / 2 + 16).astype(np.int64)
+        c = cy[rows]
+        in_lane = ((c - lane[rows] >= -1) & (c - lane[rows] <= 2)).all(axis=1)
+        c = c[in_lane]
+        one = np.array([np.bincount(r % 32, minlength=32).max() for r in c])            # bank = node column
+        m = c - np.arange(32)
+        shifted = np.array([np.bincount((r - mm) % 32, minlength=32).max() for r, mm in zip(c, m)])   # index c - m = lane
+        single.append(one.mean())
+        copies.append(shifted.mean())
+    assert all(v == 1.0 for v in copies)
+    assert all(1.9 < v < 2.6 for v in single), single
