@@ -136,29 +136,3 @@ def test_shifted_window_copies_remove_the_bank_conflicts_a_single_window_has():
     assert all(v == 1.0 for v in copies)
     assert all(1.9 < v < 2.6 for v in single), single
 
-
-def test_the_magic_number_conversion_is_round_to_nearest_even_below_2_to_the_22():
-    """DESIGN.md 6.1c / pm2d_lanes.cu: float -> int without the XU pipe.  fma(w, q, 1.5 * 2^23) in float32 has the integer
-    rint(w q) in its mantissa -- bits(result) - bits(1.5 * 2^23) -- for every |w q| <= 2^22, ties to even, both signs; one
-    step beyond 2^22 the sum leaves the binade of 1.5 * 2^23 and the trick breaks, which is why the kernel sends particles
-    faster than `ucap` (4 thermal velocities) down the exact F2I path and chooses the per-tile momentum unit 2^sp so that
-    a single contribution stays below 2^22.  The float32 FMA is emulated exactly in float64 (a 48-bit product plus a
-    constant 50 bits above its last bit is exact there, then rounded once)."""
-    MAGIC, BITS = np.float32(12582912.0), np.int32(0x4B400000)
-    assert MAGIC.view(np.int32) == BITS
-
-    def magic_int(w, q):
-        s = np.float64(w) * np.float64(q) + np.float64(MAGIC)                  # exact
-        return s.astype(np.float32).view(np.int32) - BITS
-
-    rng = np.random.default_rng(11)
-    w = rng.uniform(0.0, 2.0, 200000).astype(np.float32)                        # weights (scale 2 of the sine cloud)
-    q = (rng.uniform(-1.0, 1.0, 200000) * 2.0 ** 21).astype(np.float32)         # |w q| < 2^22
-    exact = np.float64(w) * np.float64(q)
-    assert np.array_equal(magic_int(w, q), np.rint(exact).astype(np.int64).astype(np.int32))
-    # ties go to even, on both sides of zero
-    half = np.array([0.5, 1.5, 2.5, -0.5, -1.5, -2.5, 4194303.5, -4194303.5], np.float32)
-    assert list(magic_int(np.float32(1.0), half)) == [0, 2, 2, 0, -2, -2, 4194304, -4194304]
-    # the edge of the range: 2^22 itself still converts, 2^22 + 1 on the negative side does not
-    assert magic_int(np.float32(1.0), np.float32(4194304.0)) == 4194304 and magic_int(np.float32(1.0), np.float32(-4194304.0)) == -4194304
-    assert magic_int(np.float32(1.0), np.float32(-4194305.0)) != -4194305
