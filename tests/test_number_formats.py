@@ -72,3 +72,32 @@ def test_int32_fixed_point_deposits_resolve_the_density_to_1e_7_of_the_grid_and_
     assert math.sqrt((err ** 2).sum() / (ref ** 2).sum()) < 1e-7                 # measured 9e-9
     assert np.abs(err).max() < 8 * unit                                          # measured 5.4 units: ~36 contributions per node, each off by at most half a unit
     assert np.abs(err).max() / ref.max() < 1e-7 and 3 * unit / (1e-5 * ref.max()) > 1e-4
+
+
+def test_per_tile_momentum_units_of_the_lane_kernel_cost_a_quarter_of_the_tolerance():
+    """k_stage_lanes converts a momentum contribution with the magic-number FMA, which holds 2^22; the shared
+    windows therefore count momentum in units of 2^sp global units (global unit = n_cap / 2^35: |n u| <= n_cap / 16), sp =
+    ilogb(w_max pscale u_cap) + 1 - 22 from the tile's largest weight and u_cap = 4 v_th.  For the electrons of c3 that is
+    sp = 7: each contribution is rounded to 7.5e-9 n_c c.  Modelled against the float64 momentum deposit of the same
+    particles: 3.5e-6 relative L2 -- inside BASELINE.json's 1e-5, and the largest single share of it (the density, in
+    global units, is at 9e-9)."""
+    cfg = I.config("c3", nx=48, ny=32)
+    g, q = cfg["grid"], cfg["species"][0]
+    p = L.generate_particles(cfg, 0)
+    pscale = 2.0 ** 35 / 2.0                                               # n_cap = 2 n_c
+    ucap = max(4.0 * math.sqrt(q["T_keV"] / 511.0 / q["mass"]), 0.004)
+    sp = max(0, math.frexp(float(p["w"].max()) * pscale * ucap)[1] - 1 + 1 - 22)
+    assert sp == 7
+    unit = 2.0 ** sp / pscale
+    X = p["ix"] + p["fx"].astype(np.float64)
+    Y = p["iy"] + p["fy"].astype(np.float64)
+    use = (X > 2.0) & (X < g["nx"] - 2.0) & (np.hypot(p["ux"], p["uy"]) <= ucap)      # the others take the exact path
+    out = np.zeros((g["nx"] + 1, g["ny"]), np.int64)
+    for x, y, w, u in zip(X[use], Y[use], p["w"][use].astype(np.float64), p["ux"][use].astype(np.float64)):
+        fx, Wx = oracle.weights_1d(q["shape"], q["DD"], x)
+        fy, Wy = oracle.weights_1d(q["shape"], q["DD"], y)
+        out[fx:fx + len(Wx), (fy + np.arange(len(Wy))) % g["ny"]] += np.rint(w * u * np.outer(Wx, Wy) / unit).astype(np.int64)
+    grid = oracle.make_grid(g["nx"], g["ny"], g["dx"], g["dy"], g["dt"])
+    _, ref, _ = oracle.deposit(grid, q["shape"], q["DD"], X[use], Y[use], p["ux"][use].astype(np.float64), 0 * X[use], p["w"][use].astype(np.float64))
+    rel = math.sqrt(((out * unit - ref) ** 2).sum() / (ref ** 2).sum())
+    assert 5e-7 < rel < 5e-6, rel
