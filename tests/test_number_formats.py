@@ -74,7 +74,7 @@ def test_int32_fixed_point_deposits_resolve_the_density_to_1e_7_of_the_grid_and_
     assert np.abs(err).max() / ref.max() < 1e-7 and 3 * unit / (1e-5 * ref.max()) > 1e-4
 
 
-def test_per_tile_momentum_units_of_the_lane_kernel_cost_a_quarter_of_the_tolerance():
+def test_per_tile_momentum_units_of_the_lane_kernel_cost_a_third_of_the_tolerance():
     """k_stage_lanes converts a momentum contribution with the magic-number FMA, which holds 2^22; the shared
     windows therefore count momentum in units of 2^sp global units (global unit = n_cap / 2^35: |n u| <= n_cap / 16), sp =
     ilogb(w_max pscale u_cap) + 1 - 22 from the tile's largest weight and u_cap = 4 v_th.  For the electrons of c3 that is
